@@ -1,0 +1,507 @@
+/* cosmo_oracle.c -- ORACLE. TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * A plain, slow, obviously-correct CPU implementation of what the hot path of
+ * arXiv:2212.01937 ("Analytic auto-differentiable LCDM cosmography") computes,
+ * written from the paper's DEFINITIONS, in x87 80-bit `long double`.
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may load it.  It shares no code with the CUDA path
+ * (paper_2212_01937_b200/csrc) and neither includes the other.
+ *
+ * What is here, with the passage each part follows (PAPER.md = /root/reference/PAPER.md):
+ *
+ *  (1) oracle_integrals      : the three fundamental integrals, eqs. (2.3)-(2.5)
+ *                               with E^2 of eq. (2.2) and
+ *                              Omega_k = 1 - sum of the others, z1 = 0,
+ *                              by adaptive 21-point Gauss-Kronrod quadrature -- the
+ *                              method the paper itself validates against (PAPER.md:233,
+ *                              :243 fn.18).  These integrals are the plain definition
+ *                              of what eqs. (3.7)-(3.9) re-express exactly.
+ *                              Parameter derivatives: Leibniz's integrand rule applied
+ *                              to the same integrals (the route PAPER.md:285 fn.23
+ *                              names), by the same quadrature.
+ *  (2) oracle_observables    : D_C, D_M (sin/sinh curvature transform), D_L=(1+z)D_M,
+ *                              mu = 5 log10(D_L / 10 pc) (PAPER.md:277 fn.22),
+ *                              lookback time, absorption distance, and
+ *                              their total derivatives wrt (z, Om, OL, Or, H0).
+ *                              DESIGN.md readings R-units, R-sinn.
+ *  (3) oracle_age            : int_z^inf of eq. (2.4) -- used only to pin
+ *                              (1) through lookback + age(z) = age(0).
+ *  (4) oracle_rf/rc/rd/rj    : independent scalar Carlson symmetric integrals, eqs.
+ *                              (2.6)-(2.9), complex arguments, by the
+ *                              duplication algorithm the paper cites (ref. [10],
+ *                              PAPER.md:113, :420; the algorithm itself is not printed in
+ *                              the paper: this follows its statement in DLMF 19.36(i),
+ *                              ref. [12]).  Not used by (1)-(3); used by tests to check
+ *                              that the paper's closed forms equal the quadrature.
+ *  (5) oracle_snia_loglike   : the Gaussian mu-likelihood of PAPER.md:283 summed over
+ *                              objects, with parameter gradients, by direct summation.
+ *
+ * Pins (tests/test_oracle_*.py): closed forms (Einstein-de Sitter, de Sitter, Milne,
+ * radiation-only, flat LCDM t_L/age/d_abs, Mattig), flat-LCDM 2F1 expression,
+ * 40-digit mpmath quadrature goldens, central finite differences of every gradient,
+ * lookback<->age consistency, Carlson special values / identities / SciPy elliprX.
+ *
+ * Build: python oracle/build.py  (gcc -O2 -fopenmp, no -ffast-math).
+ */
+#include <complex.h>
+#include <float.h>
+#include <math.h>
+#include <stddef.h>
+#include <stdint.h>
+#include <string.h>
+
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#include "gk21_nodes.h"
+
+#if LDBL_MANT_DIG < 64
+#error "oracle needs an extended-precision long double (x87 80-bit or wider)"
+#endif
+
+typedef long double ld;
+typedef long double complex ldc;
+
+/* ---- units (reading R-units; the paper is silent) ---- */
+#define C_KM_S 299792.458L                   /* speed of light, km/s (exact, SI)         */
+#define HUBBLE_GYR 977.7922216807891L        /* (1 km/s/Mpc)^-1 in Gyr (Julian years)    */
+
+int oracle_ldbl_mant_dig(void) { return LDBL_MANT_DIG; }
+int oracle_max_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+void oracle_set_threads(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+/* ======================================================================================
+ * (1) quadrature of the defining integrals
+ * ====================================================================================== */
+
+/* integrand components, all as functions of u = ln(1+z'), x = e^u, dz' = x du:
+ *   0 I0 = int dz'/E                 (2.3) without c/H0
+ *   1 T  = int dz'/((1+z')E)         (2.4) without 1/H0
+ *   2 A  = int (1+z')^2 dz'/E        (2.5) without c/H0
+ *   3..5   dI0/d(Om,OL,Or)   6..8 dT/d(Om,OL,Or)   9..11 dA/d(Om,OL,Or)
+ * with dE^2/dOm = x^3-x^2, dE^2/dOL = 1-x^2, dE^2/dOr = x^4-x^2 (Omega_k eliminated,
+ * PAPER.md:73) and d(E^-1)/dtheta = -1/2 (dE^2/dtheta) E^-3 (Leibniz rule). */
+#define NV 12
+
+typedef struct { ld Om, OL, Or, Ok; int nv; } cosmo_t;
+
+static inline ld E2_of_x(const cosmo_t *c, ld x) {
+    /* eq. (2.2), written exactly as printed */
+    return c->Or * x * x * x * x + c->Om * x * x * x + c->Ok * x * x + c->OL;
+}
+
+/* returns kappa >= 1, the rounding amplification of E^2 at x (sum of |terms| / |sum|), used only
+ * by the acceptance test's rounding floor (near a loitering phase E^2 is a small difference of O(1) terms) */
+static ld integrand_u(const cosmo_t *c, ld u, ld f[NV]) {
+    ld x = expl(u);
+    ld E2 = E2_of_x(c, x);
+    ld kappa = (c->Or * x * x * x * x + c->Om * x * x * x + fabsl(c->Ok) * x * x + fabsl(c->OL)) / fabsl(E2);
+    ld E = sqrtl(E2);
+    f[0] = x / E;
+    f[1] = 1.0L / E;
+    f[2] = x * x * x / E;
+    if (c->nv > 3) {
+        ld E3 = E2 * E;
+        ld x2 = x * x;
+        ld zz = expm1l(u); /* x - 1 without cancellation at small z */
+        ld dOm = x2 * zz, dOL = -zz * (x + 1.0L), dOr = x2 * zz * (x + 1.0L); /* x^3-x^2, 1-x^2, x^4-x^2 */
+        ld w0 = -0.5L * x / E3, w1 = -0.5L / E3, w2 = -0.5L * x2 * x / E3;
+        f[3] = w0 * dOm; f[4] = w0 * dOL; f[5] = w0 * dOr;
+        f[6] = w1 * dOm; f[7] = w1 * dOL; f[8] = w1 * dOr;
+        f[9] = w2 * dOm; f[10] = w2 * dOL; f[11] = w2 * dOr;
+    }
+    return kappa;
+}
+
+/* one 21-point Gauss-Kronrod panel on [a,b]; K = Kronrod estimate, G = embedded Gauss */
+static void gk21_panel(const cosmo_t *c, ld a, ld b, ld K[NV], ld G[NV], ld Kabs[NV]) {
+    ld h = 0.5L * (b - a), m = 0.5L * (a + b), f[NV];
+    int nv = c->nv;
+    for (int v = 0; v < nv; ++v) K[v] = G[v] = Kabs[v] = 0.0L;
+    for (int i = 0; i < 21; ++i) {
+        ld kappa = integrand_u(c, m + h * GK21_X[i], f);
+        for (int v = 0; v < nv; ++v) {
+            K[v] += GK21_WK[i] * f[v];
+            G[v] += GK21_WG[i] * f[v];
+            Kabs[v] += GK21_WK[i] * fabsl(f[v]) * kappa;
+        }
+    }
+    for (int v = 0; v < nv; ++v) { K[v] *= h; G[v] *= h; Kabs[v] *= h; }
+}
+
+/* adaptive bisection: a panel is accepted when, for every component, |K-G| is below
+ * tol * |scale| * (panel width / total width), or below the rounding floor of the panel sum
+ * (GK_ROUND * LDBL_EPSILON * int |f| kappa, kappa = rounding amplification of E^2); the accepted value is K.  For these analytic integrands the
+ * Kronrod value is far more accurate than |K-G| indicates. */
+#define GK_TOL 1e-16L
+#define GK_ROUND 64.0L
+#define GK_MAXDEPTH 60
+#define GK_MAXPANELS 20000 /* safety net; oracle_integrals returns -2 when hit */
+
+static void gk21_adapt(const cosmo_t *c, ld a, ld b, ld frac, const ld scale[NV], int depth,
+                       ld acc[NV], int *npanels) {
+    ld K[NV], G[NV], Kabs[NV];
+    gk21_panel(c, a, b, K, G, Kabs);
+    int ok = 1;
+    for (int v = 0; v < c->nv; ++v) {
+        ld err = fabsl(K[v] - G[v]);
+        if (err > GK_TOL * scale[v] * frac && err > GK_ROUND * LDBL_EPSILON * Kabs[v]) ok = 0;
+        if (err != err) ok = 1; /* NaN integrand (E^2 < 0 between the validity samples): give up, NaN propagates */
+    }
+    if (ok || depth >= GK_MAXDEPTH || *npanels >= GK_MAXPANELS) {
+        for (int v = 0; v < c->nv; ++v) acc[v] += K[v];
+        ++*npanels;
+        return;
+    }
+    ld m = 0.5L * (a + b);
+    gk21_adapt(c, a, m, 0.5L * frac, scale, depth + 1, acc, npanels);
+    gk21_adapt(c, m, b, 0.5L * frac, scale, depth + 1, acc, npanels);
+}
+
+/* out[0..2] = I0,T,A ; if with_grad out[3..11] = their d/d(Om,OL,Or).  Returns panels used,
+ * or -1 if E^2 <= 0 somewhere on the sampled path (unphysical, no Big Bang). */
+int oracle_integrals(ld z, ld Om, ld OL, ld Or, int with_grad, ld out[NV]) {
+    cosmo_t c = { Om, OL, Or, 1.0L - Om - OL - Or, with_grad ? NV : 3 };
+    for (int v = 0; v < NV; ++v) out[v] = 0.0L;
+    if (!(z > -1.0L)) return -1;
+    if (z == 0.0L) return 0;
+    ld U = log1pl(z);
+    /* validity: E^2 must stay positive on the path */
+    for (int i = 0; i <= 64; ++i) {
+        ld x = expl(U * i / 64.0L);
+        if (!(E2_of_x(&c, x) > 0.0L)) return -1;
+    }
+    /* first pass on fixed panels gives the scale used by the acceptance test */
+    ld scale[NV], K[NV], G[NV], Kabs[NV];
+    gk21_panel(&c, 0.0L, U, K, G, Kabs);
+    for (int v = 0; v < c.nv; ++v) scale[v] = fabsl(K[v]);
+    int npanels = 0;
+    /* integrate on panels of width <= 1 in u (a decade of 1+z is ~2.3 panels) */
+    int nseg = (int)ceill(fabsl(U));
+    if (nseg < 1) nseg = 1;
+    for (int s = 0; s < nseg; ++s) {
+        ld a = U * s / nseg, b = U * (s + 1) / nseg;
+        gk21_adapt(&c, a, b, 1.0L / nseg, scale, 0, out, &npanels);
+    }
+    if (npanels >= GK_MAXPANELS) return -2;
+    return npanels;
+}
+
+/* ======================================================================================
+ * (3) age: int_z^inf dz'/((1+z')E) = int_0^{a} a' da'/sqrt(P(a')),  P = Or + Om a + Ok a^2 + OL a^4,
+ *     with a' = s^2 so that the Or = 0 endpoint behaviour sqrt(a') becomes polynomial.
+ * ====================================================================================== */
+static ld age_integrand_s(const cosmo_t *c, ld s) {
+    ld a = s * s;
+    ld P = c->Or + c->Om * a + c->Ok * a * a + c->OL * a * a * a * a;
+    /* a da = s^2 * 2 s ds ; if Or == 0 factor s out of sqrt(P) analytically */
+    if (c->Or == 0.0L) {
+        ld P1 = c->Om + c->Ok * a + c->OL * a * a * a; /* P / a */
+        return 2.0L * s * s / sqrtl(P1);
+    }
+    return 2.0L * s * s * s / sqrtl(P);
+}
+static ld age_panel(const cosmo_t *c, ld a, ld b, ld *G) {
+    ld h = 0.5L * (b - a), m = 0.5L * (a + b), K = 0.0L;
+    *G = 0.0L;
+    for (int i = 0; i < 21; ++i) {
+        ld f = age_integrand_s(c, m + h * GK21_X[i]);
+        K += GK21_WK[i] * f;
+        *G += GK21_WG[i] * f;
+    }
+    *G *= h;
+    return K * h;
+}
+static ld age_adapt(const cosmo_t *c, ld a, ld b, ld tolabs, int depth) {
+    ld G, K = age_panel(c, a, b, &G);
+    if (fabsl(K - G) <= tolabs || depth >= GK_MAXDEPTH) return K;
+    ld m = 0.5L * (a + b);
+    return age_adapt(c, a, m, 0.5L * tolabs, depth + 1) + age_adapt(c, m, b, 0.5L * tolabs, depth + 1);
+}
+/* H0 * age at redshift z (dimensionless) */
+ld oracle_age_dimless(ld z, ld Om, ld OL, ld Or) {
+    cosmo_t c = { Om, OL, Or, 1.0L - Om - OL - Or, 3 };
+    ld smax = sqrtl(1.0L / (1.0L + z));
+    ld G, K0 = age_panel(&c, 0.0L, smax, &G);
+    return age_adapt(&c, 0.0L, smax, GK_TOL * fabsl(K0), 0);
+}
+
+/* ======================================================================================
+ * (2) observables and their total derivatives
+ * ====================================================================================== */
+enum { OBS_DC = 0, OBS_DM, OBS_DL, OBS_MU, OBS_TL, OBS_DABS, N_OBS };
+enum { WRT_Z = 0, WRT_OM, WRT_OL, WRT_OR, WRT_H0, N_WRT };
+
+/* sinn(k, chi) = sinh(sqrt(k) chi)/sqrt(k) (k>0), sin(sqrt(-k) chi)/sqrt(-k) (k<0), chi (k=0);
+ * also d/dchi and d/dk at fixed chi.  Series in w = k chi^2 for small |w| (the closed forms cancel). */
+static void sinn_transform(ld k, ld chi, ld *F, ld *dF_dI, ld *dF_dk) {
+    ld w = k * chi * chi;
+    if (fabsl(w) < 1e-2L) {
+        /* F = chi sum w^n/(2n+1)!, dF/dI = sum w^n/(2n)!, dF/dk = chi^3 sum n w^(n-1)/(2n+1)! */
+        ld S = 0, C = 0, D = 0, term_s = 1.0L, term_c = 1.0L; /* w^n/(2n+1)!, w^n/(2n)! */
+        ld wpow_prev_over = 0.0L;                              /* w^(n-1)/(2n+1)!       */
+        for (int n = 0; n < 12; ++n) {
+            S += term_s; C += term_c;
+            if (n >= 1) D += n * wpow_prev_over;
+            /* advance to n+1 */
+            wpow_prev_over = term_s / ((2.0L * n + 2) * (2.0L * n + 3)); /* w^n/(2n+3)! */
+            term_s = term_s * w / ((2.0L * n + 2) * (2.0L * n + 3));
+            term_c = term_c * w / ((2.0L * n + 1) * (2.0L * n + 2));
+        }
+        *F = chi * S; *dF_dI = C; *dF_dk = chi * chi * chi * D;
+        return;
+    }
+    if (k > 0) {
+        ld s = sqrtl(k);
+        ld sh = sinhl(s * chi), ch = coshl(s * chi);
+        *F = sh / s; *dF_dI = ch; *dF_dk = (chi * ch - sh / s) / (2.0L * k);
+    } else {
+        ld s = sqrtl(-k);
+        ld sn = sinl(s * chi), cs = cosl(s * chi);
+        *F = sn / s; *dF_dI = cs; *dF_dk = (chi * cs - sn / s) / (2.0L * k);
+    }
+}
+
+/* val[N_OBS], grad[N_OBS][N_WRT] (grad may be NULL).  Units: H0 in km/s/Mpc, distances in Mpc,
+ * t_L in Gyr, mu in mag.  Returns 0, or -1 invalid path (values NaN), or 1 if D_L <= 0 (mu = NaN). */
+int oracle_observables(ld z, ld Om, ld OL, ld Or, ld H0, ld val[N_OBS], ld *grad /* [N_OBS*N_WRT] or NULL */) {
+    ld q[NV];
+    int rc = oracle_integrals(z, Om, OL, Or, grad != NULL, q);
+    if (rc < 0) {
+        for (int i = 0; i < N_OBS; ++i) val[i] = NAN;
+        if (grad) for (int i = 0; i < N_OBS * N_WRT; ++i) grad[i] = NAN;
+        return -1;
+    }
+    ld Ok = 1.0L - Om - OL - Or;
+    ld x = 1.0L + z;
+    ld E = sqrtl(Or * x * x * x * x + Om * x * x * x + Ok * x * x + OL);
+    ld dH = C_KM_S / H0, tH = HUBBLE_GYR / H0;
+    ld I0 = q[0], T = q[1], A = q[2];
+    ld F, Fi, Fk;
+    sinn_transform(Ok, I0, &F, &Fi, &Fk);
+    val[OBS_DC] = dH * I0;
+    val[OBS_DM] = dH * F;
+    val[OBS_DL] = x * dH * F;
+    int status = 0;
+    if (val[OBS_DL] > 0) val[OBS_MU] = 5.0L * log10l(val[OBS_DL]) + 25.0L; /* D_L in Mpc; 10 pc = 1e-5 Mpc */
+    else { val[OBS_MU] = NAN; status = 1; }
+    val[OBS_TL] = tH * T;
+    val[OBS_DABS] = dH * A;
+    if (!grad) return status;
+    ld (*g)[N_WRT] = (ld (*)[N_WRT])grad;
+    /* d/dz = integrand at the upper limit */
+    ld dI_dz = 1.0L / E, dT_dz = 1.0L / (x * E), dA_dz = x * x / E;
+    g[OBS_DC][WRT_Z] = dH * dI_dz;
+    g[OBS_DM][WRT_Z] = dH * Fi * dI_dz;
+    g[OBS_DL][WRT_Z] = dH * F + x * g[OBS_DM][WRT_Z];
+    g[OBS_TL][WRT_Z] = tH * dT_dz;
+    g[OBS_DABS][WRT_Z] = dH * dA_dz;
+    for (int p = 0; p < 3; ++p) { /* Om, OL, Or ; dOk/dtheta = -1 for each */
+        ld dI = q[3 + p], dT = q[6 + p], dA = q[9 + p];
+        g[OBS_DC][WRT_OM + p] = dH * dI;
+        g[OBS_DM][WRT_OM + p] = dH * (Fi * dI - Fk);
+        g[OBS_DL][WRT_OM + p] = x * g[OBS_DM][WRT_OM + p];
+        g[OBS_TL][WRT_OM + p] = tH * dT;
+        g[OBS_DABS][WRT_OM + p] = dH * dA;
+    }
+    g[OBS_DC][WRT_H0] = -val[OBS_DC] / H0;
+    g[OBS_DM][WRT_H0] = -val[OBS_DM] / H0;
+    g[OBS_DL][WRT_H0] = -val[OBS_DL] / H0;
+    g[OBS_TL][WRT_H0] = -val[OBS_TL] / H0;
+    g[OBS_DABS][WRT_H0] = -val[OBS_DABS] / H0;
+    for (int w = 0; w < N_WRT; ++w)
+        g[OBS_MU][w] = (status == 0) ? 5.0L / logl(10.0L) * g[OBS_DL][w] / val[OBS_DL] : NAN;
+    return status;
+}
+
+/* Batch over n elements (OpenMP over elements).  Parameter arrays have length n_cosmo in {1, n}
+ * (n_cosmo == 1 broadcasts).  val: [n][N_OBS]; grad: [n][N_OBS][N_WRT] or NULL; status: [n] or NULL.
+ * Inputs are doubles (the very values the GPU path is given); outputs long double. */
+void oracle_observables_batch(int64_t n, const double *z, const double *Om, const double *OL, const double *Or,
+                              const double *H0, int64_t n_cosmo, ld *val, ld *grad, int32_t *status) {
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < n; ++i) {
+        int64_t j = (n_cosmo == 1) ? 0 : i;
+        int rc = oracle_observables((ld)z[i], (ld)Om[j], (ld)OL[j], (ld)Or[j], (ld)H0[j], val + i * N_OBS,
+                                    grad ? grad + i * N_OBS * N_WRT : NULL);
+        if (status) status[i] = rc;
+    }
+}
+
+/* ======================================================================================
+ * (5) SN Ia Gaussian mu-likelihood: mu_obs_n | mu_n ~ N(mu_n, sigma_n^2)
+ *     logL = sum_n [ -1/2 ((mu_obs_n - mu_n)/sigma_n)^2 - ln sigma_n - 1/2 ln 2 pi ]
+ *     dlogL/dtheta = sum_n ((mu_obs_n - mu_n)/sigma_n^2) dmu_n/dtheta,  theta in (Om, OL, Or, H0)
+ *     one cosmology; out = {logL, d/dOm, d/dOL, d/dOr, d/dH0}.  Long-double accumulation in index order.
+ * ====================================================================================== */
+int oracle_snia_loglike(int64_t n, const double *z, const double *mu_obs, const double *sigma, double Om, double OL,
+                        double Or, double H0, int with_grad, ld out[5]) {
+    ld acc[5] = { 0, 0, 0, 0, 0 };
+    int bad = 0;
+    const ld half_ln_2pi = 0.5L * logl(2.0L * acosl(-1.0L));
+#pragma omp parallel
+    {
+        ld loc[5] = { 0, 0, 0, 0, 0 };
+        int locbad = 0;
+#pragma omp for schedule(static)
+        for (int64_t i = 0; i < n; ++i) {
+            ld val[N_OBS], grad[N_OBS * N_WRT];
+            int rc = oracle_observables((ld)z[i], (ld)Om, (ld)OL, (ld)Or, (ld)H0, val, with_grad ? grad : NULL);
+            if (rc != 0) { locbad = 1; continue; }
+            ld s = (ld)sigma[i];
+            ld r = ((ld)mu_obs[i] - val[OBS_MU]) / s;
+            loc[0] += -0.5L * r * r - logl(s) - half_ln_2pi;
+            if (with_grad)
+                for (int p = 0; p < 4; ++p) loc[1 + p] += (r / s) * grad[OBS_MU * N_WRT + WRT_OM + p];
+        }
+#pragma omp critical
+        {
+            for (int k = 0; k < 5; ++k) acc[k] += loc[k];
+            bad |= locbad;
+        }
+    }
+    for (int k = 0; k < 5; ++k) out[k] = acc[k];
+    return bad ? -1 : 0;
+}
+
+/* ======================================================================================
+ * (4) independent scalar Carlson integrals, complex arguments, duplication (DLMF 19.36(i))
+ *     r = requested relative accuracy.  csqrtl is the principal root (Re >= 0) throughout.
+ * ====================================================================================== */
+#define CARLSON_R 1e-18L
+#define CARLSON_MAXIT 200
+
+static ld max3(ld a, ld b, ld c) { return fmaxl(a, fmaxl(b, c)); }
+
+ldc oracle_rf_c(ldc x, ldc y, ldc z) {
+    ldc A0 = (x + y + z) / 3.0L, A = A0;
+    ld Q = powl(3.0L * CARLSON_R, -1.0L / 6.0L) * max3(cabsl(A0 - x), cabsl(A0 - y), cabsl(A0 - z));
+    ld f = 1.0L; /* 4^n */
+    for (int n = 0; n < CARLSON_MAXIT && !(Q / f < cabsl(A)); ++n) {
+        ldc sx = csqrtl(x), sy = csqrtl(y), sz = csqrtl(z);
+        ldc lam = sx * sy + sx * sz + sy * sz;
+        A = (A + lam) / 4.0L; x = (x + lam) / 4.0L; y = (y + lam) / 4.0L; z = (z + lam) / 4.0L;
+        f *= 4.0L;
+    }
+    ldc X = 1.0L - x / A, Y = 1.0L - y / A, Z = -X - Y; /* = (A0-x0)/(4^n A_n) etc. */
+    ldc E2 = X * Y - Z * Z, E3 = X * Y * Z;
+    return (1.0L - E2 / 10.0L + E3 / 14.0L + E2 * E2 / 24.0L - 3.0L * E2 * E3 / 44.0L - 5.0L * E2 * E2 * E2 / 208.0L +
+            3.0L * E3 * E3 / 104.0L + E2 * E2 * E3 / 16.0L) / csqrtl(A);
+}
+
+/* R_C(x,y) = R_F(x,y,y); real y < 0 (with real x >= 0): Cauchy principal value */
+ldc oracle_rc_c(ldc x, ldc y) {
+    if (cimagl(y) == 0.0L && creall(y) < 0.0L && cimagl(x) == 0.0L && creall(x) >= 0.0L) {
+        ld xr = creall(x), yr = creall(y);
+        return sqrtl(xr / (xr - yr)) * oracle_rc_c(xr - yr, -yr);
+    }
+    ldc A0 = (x + 2.0L * y) / 3.0L, A = A0, y0 = y;
+    ld Q = powl(3.0L * CARLSON_R, -1.0L / 8.0L) * cabsl(A0 - x);
+    ld f = 1.0L;
+    for (int n = 0; n < CARLSON_MAXIT && !(Q / f < cabsl(A)); ++n) {
+        ldc lam = 2.0L * csqrtl(x) * csqrtl(y) + y;
+        A = (A + lam) / 4.0L; x = (x + lam) / 4.0L; y = (y + lam) / 4.0L;
+        f *= 4.0L;
+    }
+    ldc s = (y0 - A0) / (f * A);
+    ldc s2 = s * s;
+    return (1.0L + s2 * (3.0L / 10.0L + s * (1.0L / 7.0L + s * (3.0L / 8.0L + s * (9.0L / 22.0L + s * (159.0L / 208.0L + s * (9.0L / 8.0L))))))) /
+           csqrtl(A);
+}
+
+static ldc carlson_series_dj(ldc E2, ldc E3, ldc E4, ldc E5) {
+    return 1.0L - 3.0L * E2 / 14.0L + E3 / 6.0L + 9.0L * E2 * E2 / 88.0L - 3.0L * E4 / 22.0L - 9.0L * E2 * E3 / 52.0L +
+           3.0L * E5 / 26.0L - E2 * E2 * E2 / 16.0L + 3.0L * E3 * E3 / 40.0L + 3.0L * E2 * E4 / 20.0L +
+           45.0L * E2 * E2 * E3 / 272.0L - 9.0L * (E3 * E4 + E2 * E5) / 68.0L;
+}
+
+ldc oracle_rd_c(ldc x, ldc y, ldc z) {
+    ldc A0 = (x + y + 3.0L * z) / 5.0L, A = A0, x0 = x, y0 = y, sum = 0.0L;
+    ld Q = powl(CARLSON_R / 4.0L, -1.0L / 6.0L) * max3(cabsl(A0 - x), cabsl(A0 - y), cabsl(A0 - z));
+    ld f = 1.0L;
+    for (int n = 0; n < CARLSON_MAXIT && !(Q / f < cabsl(A)); ++n) {
+        ldc sx = csqrtl(x), sy = csqrtl(y), sz = csqrtl(z);
+        ldc lam = sx * sy + sx * sz + sy * sz;
+        sum += 1.0L / (f * sz * (z + lam));
+        A = (A + lam) / 4.0L; x = (x + lam) / 4.0L; y = (y + lam) / 4.0L; z = (z + lam) / 4.0L;
+        f *= 4.0L;
+    }
+    ldc X = (A0 - x0) / (f * A), Y = (A0 - y0) / (f * A), Z = -(X + Y) / 3.0L;
+    ldc E2 = X * Y - 6.0L * Z * Z, E3 = (3.0L * X * Y - 8.0L * Z * Z) * Z, E4 = 3.0L * (X * Y - Z * Z) * Z * Z,
+        E5 = X * Y * Z * Z * Z;
+    return carlson_series_dj(E2, E3, E4, E5) / (f * A * csqrtl(A)) + 3.0L * sum;
+}
+
+/* R_J(x,y,z,p); real p < 0 with real non-negative x,y,z: Cauchy principal value via DLMF 19.20.14 */
+ldc oracle_rj_c(ldc x, ldc y, ldc z, ldc p) {
+    if (cimagl(p) == 0.0L && creall(p) < 0.0L && cimagl(x) == 0.0L && cimagl(y) == 0.0L && cimagl(z) == 0.0L) {
+        ld a = creall(x), b = creall(y), c = creall(z), t;
+        /* order a <= b <= c */
+        if (a > b) { t = a; a = b; b = t; }
+        if (b > c) { t = b; b = c; c = t; }
+        if (a > b) { t = a; a = b; b = t; }
+        ld q = -creall(p);
+        /* DLMF 19.20.14: (q + y) R_J(x,y,z,-q) = (p - y) R_J(x,y,z,p) - 3 R_F(x,y,z) + 3 sqrt(xyz/(xz+pq)) R_C(xz+pq, pq),
+         * p = y + (z-y)(y-x)/(y+q), valid for y between x and z; here y := b (the middle one), x := a, z := c. */
+        ld pp = b + (c - b) * (b - a) / (b + q);
+        ldc rj = oracle_rj_c(a, b, c, pp);
+        ldc rf = oracle_rf_c(a, b, c);
+        ld xzpq = a * c + pp * q;
+        ldc rc = oracle_rc_c(xzpq, pp * q);
+        return ((pp - b) * rj - 3.0L * rf + 3.0L * sqrtl(a * b * c / xzpq) * rc) / (q + b);
+    }
+    ldc A0 = (x + y + z + 2.0L * p) / 5.0L, A = A0, x0 = x, y0 = y, z0 = z, sum = 0.0L;
+    ldc delta = (p - x) * (p - y) * (p - z);
+    ld Q = powl(CARLSON_R / 4.0L, -1.0L / 6.0L) *
+           fmaxl(max3(cabsl(A0 - x), cabsl(A0 - y), cabsl(A0 - z)), cabsl(A0 - p));
+    ld f = 1.0L;
+    for (int n = 0; n < CARLSON_MAXIT && !(Q / f < cabsl(A)); ++n) {
+        ldc sx = csqrtl(x), sy = csqrtl(y), sz = csqrtl(z), sp = csqrtl(p);
+        ldc lam = sx * sy + sx * sz + sy * sz;
+        ldc d = (sp + sx) * (sp + sy) * (sp + sz);
+        ldc e = delta / (f * f * f * d * d);
+        sum += oracle_rc_c(1.0L, 1.0L + e) / (f * d);
+        A = (A + lam) / 4.0L; x = (x + lam) / 4.0L; y = (y + lam) / 4.0L; z = (z + lam) / 4.0L; p = (p + lam) / 4.0L;
+        f *= 4.0L;
+    }
+    ldc X = (A0 - x0) / (f * A), Y = (A0 - y0) / (f * A), Z = (A0 - z0) / (f * A), P = (-X - Y - Z) / 2.0L;
+    ldc E2 = X * Y + X * Z + Y * Z - 3.0L * P * P, E3 = X * Y * Z + 2.0L * E2 * P + 4.0L * P * P * P,
+        E4 = (2.0L * X * Y * Z + E2 * P + 3.0L * P * P * P) * P, E5 = X * Y * Z * P * P;
+    return carlson_series_dj(E2, E3, E4, E5) / (f * A * csqrtl(A)) + 6.0L * sum;
+}
+
+/* ctypes-friendly wrappers: double in, long double (re, im) out */
+void oracle_rf(double xr, double xi, double yr, double yi, double zr, double zi, ld out[2]) {
+    ldc r = oracle_rf_c(xr + I * (ld)xi, yr + I * (ld)yi, zr + I * (ld)zi);
+    out[0] = creall(r); out[1] = cimagl(r);
+}
+void oracle_rc(double xr, double xi, double yr, double yi, ld out[2]) {
+    ldc r = oracle_rc_c(xr + I * (ld)xi, yr + I * (ld)yi);
+    out[0] = creall(r); out[1] = cimagl(r);
+}
+void oracle_rd(double xr, double xi, double yr, double yi, double zr, double zi, ld out[2]) {
+    ldc r = oracle_rd_c(xr + I * (ld)xi, yr + I * (ld)yi, zr + I * (ld)zi);
+    out[0] = creall(r); out[1] = cimagl(r);
+}
+void oracle_rj(double xr, double xi, double yr, double yi, double zr, double zi, double pr, double pi_, ld out[2]) {
+    ldc r = oracle_rj_c(xr + I * (ld)xi, yr + I * (ld)yi, zr + I * (ld)zi, pr + I * (ld)pi_);
+    out[0] = creall(r); out[1] = cimagl(r);
+}
+
+/* GK21 rule exposed for the quadrature-rule pin (exactness degree, weights) */
+void oracle_gk21_rule(ld x[21], ld wk[21], ld wg[21]) {
+    memcpy(x, GK21_X, sizeof(GK21_X)); memcpy(wk, GK21_WK, sizeof(GK21_WK)); memcpy(wg, GK21_WG, sizeof(GK21_WG));
+}
