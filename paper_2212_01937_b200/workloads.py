@@ -156,7 +156,7 @@ def _block_a(rng, m, Or):
 def _block_b(rng, m, Or):
     """Near-degenerate REAL pair: two real roots of E^2 in x in (0,1) separated by gap (recollapsing closed models)."""
     xc = rng.uniform(0.03, 0.35, m)
-    gap = 10.0 ** rng.uniform(-6.0, -1.0, m)
+    gap = np.minimum(10.0 ** rng.uniform(-6.0, -1.0, m), xc)
     x1, x2 = xc - 0.5 * gap, xc + 0.5 * gap
     rows = np.stack([_e2_linear_rows(x1), _e2_linear_rows(x2)], axis=-2)
     rhs = np.stack([-(Or * (x1 ** 4 - x1 ** 2) + x1 ** 2), -(Or * (x2 ** 4 - x2 ** 2) + x2 ** 2)], axis=-1)
