@@ -1,0 +1,114 @@
+/* cosmo_b200.h -- C ABI of the B200-native LCDM+radiation cosmography library (libcosmo_b200.so).
+ *
+ * What the calls compute (PAPER.md = arXiv:2212.01937 text; DESIGN.md lists every reading of it):
+ *   E^2(z) = Or (1+z)^4 + Om (1+z)^3 + Ok (1+z)^2 + OL,  Ok = 1 - Om - OL - Or      eq. (2.2)
+ *   chi   = (c/H0) int_0^z dz'/E                                                       eq. (2.3)
+ *   t     = (1/H0) int_0^z dz'/((1+z')E)          (lookback time)                      eq. (2.4)
+ *   d_abs = (c/H0) int_0^z (1+z')^2 dz'/E                                              eq. (2.5)
+ * evaluated in closed form by Carlson's symmetric integrals R_F, R_J, R_D, R_C, eqs. (3.7)-(3.9)
+ * and (B.1)-(B.3) when Or = 0, plus the derived observables of PAPER.md:95 and :277 fn.22:
+ *   D_C = chi;  D_M = (c/H0) sinn(sqrt|Ok| I0)/sqrt|Ok|  (sin for Ok<0, sinh for Ok>0);  D_L = (1+z) D_M;
+ *   mu = 5 log10(D_L / 10 pc);  t_L = t;  d_abs.
+ * and their analytic gradients with respect to z and (Om, OL, Or, H0), Ok eliminated.
+ *
+ * Units: H0 in km/s/Mpc; distances in Mpc (c = 299792.458 km/s); t_L in Gyr (1/H0 = 977.7922216807891/H0 Gyr); mu in mag.
+ *
+ * Conventions for every call:
+ *   - every pointer is a DEVICE pointer owned by the caller unless marked "host"; the library allocates nothing;
+ *   - the call only enqueues kernels on `stream` (a cudaStream_t passed as void*; NULL = legacy default stream),
+ *     it never synchronises; results are valid after the stream reaches the end of the enqueued work;
+ *   - return value 0 = enqueued; negative = COSMO_E_* below, nothing was launched (argument errors) or the CUDA
+ *     launch failed (COSMO_E_CUDA; cosmo_last_cuda_error() gives the cudaError_t);
+ *   - per-element domain problems never abort: the element's outputs are NaN and its status byte carries
+ *       1  a root of E^2 lies on (0, z] (no-Big-Bang region)
+ *       2  unsupported input: Om <= 0, Or < 0, OL < 0, H0 <= 0, z <= -1, non-finite, or no two real negative roots
+ *          (the method needs E^2 of degree 3 or 4)
+ *       4  D_L <= 0 (closed universe at/after the antipode): mu is NaN, the other outputs are valid
+ *       8  the duplication loop hit its iteration cap before Carlson's stopping rule was met
+ *      16  gradient ill-conditioned (near-degenerate roots; the 1/prod(r_j - r_k) of PAPER.md:320-345): values valid,
+ *          gradients may have lost more than the documented accuracy (elementwise calls only)
+ */
+#ifndef COSMO_B200_H
+#define COSMO_B200_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ELEMENTWISE: n_cosmo == n_z (one cosmology per redshift) or n_cosmo == 1; rows = 1.
+ * OUTER      : every redshift with every cosmology (PAPER.md:287 fn.24); rows = n_cosmo, element (s, n) at [s*n_z + n]. */
+typedef enum { COSMO_ELEMENTWISE = 0, COSMO_OUTER = 1 } cosmo_mode;
+
+/* `which` bitmask; the selected planes are stored in ascending bit order: out[plane][row][n]. */
+enum { COSMO_DC = 1, COSMO_DM = 2, COSMO_DL = 4, COSMO_MU = 8, COSMO_TL = 16, COSMO_DABS = 32 };
+
+enum {
+    COSMO_OK = 0,
+    COSMO_E_NULL = -1,      /* a required pointer is NULL                        */
+    COSMO_E_SIZE = -2,      /* negative size, or n_cosmo incompatible with mode  */
+    COSMO_E_WHICH = -3,     /* which == 0 or has unknown bits                    */
+    COSMO_E_MODE = -4,      /* unknown mode                                      */
+    COSMO_E_WORKSPACE = -5, /* ws_bytes < cosmo_workspace_bytes(...)             */
+    COSMO_E_CUDA = -6       /* kernel launch failed                              */
+};
+
+/* SoA cosmological parameters, each of length n_cosmo.  Always FP64, also for the _f32 entry points
+ * (reading R-fp32). */
+typedef struct { const double *Om, *OL, *Or, *H0; } cosmo_params;
+
+/* Bytes of scratch the calls below need (device memory, 256-byte aligned, contents undefined on entry and exit). */
+size_t cosmo_workspace_bytes(int64_t n_z, int64_t n_cosmo, int mode, uint32_t which, int with_grad);
+
+/* Forward.  z[n_z]; out[n_which][rows][n_z]; status: nullable, [rows][n_z] bytes. */
+int cosmo_eval(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode, uint32_t which,
+               double* out, uint8_t* status, void* workspace, size_t ws_bytes, void* stream);
+
+/* Fused forward + vector-Jacobian product (no tape).  grad_out has the layout of out.  out: nullable.
+ * grad_z[n_z]            = sum over rows and planes of grad_out * d out / d z        (overwritten)
+ * grad_params[4][n_cosmo] = sum over the redshifts that use cosmology s, order (Om, OL, Or, H0), total derivatives
+ *                           with Ok = 1 - Om - OL - Or eliminated                     (overwritten)
+ * Invalid elements (status 1, 2) contribute NaN. */
+int cosmo_vjp(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode, uint32_t which,
+              const double* grad_out, double* out, double* grad_z, double* grad_params, uint8_t* status,
+              void* workspace, size_t ws_bytes, void* stream);
+
+/* Fused distance-modulus -> Gaussian log-likelihood for S cosmology samples over N supernovae:
+ *   logL[s] = sum_n [ -1/2 ((mu_obs[n] - mu(z[n]; theta_s)) / sigma[n])^2 - ln sigma[n] - 1/2 ln 2 pi ]
+ *   grad[4][S] = d logL[s] / d (Om, OL, Or, H0)   (nullable)
+ * Elements with status != 0 contribute NaN. */
+int cosmo_snia_loglike(const double* z, const double* mu_obs, const double* sigma, int64_t N, cosmo_params p, int64_t S,
+                       double* logL, double* grad, void* workspace, size_t ws_bytes, void* stream);
+
+/* FP32 variants: z, out, grad_out, grad_z, mu_obs, sigma are float and the per-element arithmetic is FP32;
+ * parameters, the per-cosmology constants (root solve) and the reduced outputs grad_params / logL / grad stay FP64. */
+int cosmo_eval_f32(const float* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode, uint32_t which,
+                   float* out, uint8_t* status, void* workspace, size_t ws_bytes, void* stream);
+int cosmo_vjp_f32(const float* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode, uint32_t which,
+                  const float* grad_out, float* out, float* grad_z, double* grad_params, uint8_t* status,
+                  void* workspace, size_t ws_bytes, void* stream);
+int cosmo_snia_loglike_f32(const float* z, const float* mu_obs, const float* sigma, int64_t N, cosmo_params p, int64_t S,
+                           double* logL, double* grad, void* workspace, size_t ws_bytes, void* stream);
+
+/* Host-buffer convenience (every pointer is a HOST pointer; allocates device scratch, copies in, runs cosmo_vjp or
+ * cosmo_eval (grad_out == NULL), copies out, synchronises).  This is the end-to-end call bench.py times as `e2e`. */
+int cosmo_eval_host(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode, uint32_t which,
+                    const double* grad_out, double* out, double* grad_z, double* grad_params, uint8_t* status);
+
+/* ALU roofline probes: each thread runs `iters` rounds of 8 independent dependent-FMA chains (FP64 / FP32) and
+ * stores one value per thread in sink[blocks*256].  flops = blocks * 256 * iters * 8 * 2.  Used by bench.py to
+ * measure the DFMA / FFMA peak that the roofline fraction is quoted against. */
+int cosmo_probe_fma_f64(int blocks, int iters, double* sink, void* stream);
+int cosmo_probe_fma_f32(int blocks, int iters, float* sink, void* stream);
+
+/* number of kernels the library has launched in this process (all entry points) */
+int64_t cosmo_launch_count(void);
+int cosmo_last_cuda_error(void);
+const char* cosmo_strerror(int code);
+const char* cosmo_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* COSMO_B200_H */

@@ -1,0 +1,249 @@
+"""Thin Python binding of the C ABI in include/cosmo_b200.h: argument marshalling only.
+
+Every step of the hot path runs inside libcosmo_b200.so's CUDA kernels.  PyTorch supplies device memory and the
+current stream.  There is no CPU path: loading fails loudly if the library is missing, and every call requires
+CUDA tensors.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libcosmo_b200.so")
+
+ELEMENTWISE, OUTER = 0, 1
+DC, DM, DL, MU, TL, DABS = 1, 2, 4, 8, 16, 32
+WHICH_BITS = {"DC": DC, "DM": DM, "DL": DL, "MU": MU, "TL": TL, "DABS": DABS}
+WHICH_ORDER = ("DC", "DM", "DL", "MU", "TL", "DABS")
+
+# every symbol include/cosmo_b200.h declares
+SYMBOLS = ("cosmo_workspace_bytes", "cosmo_eval", "cosmo_vjp", "cosmo_snia_loglike", "cosmo_eval_f32", "cosmo_vjp_f32",
+           "cosmo_snia_loglike_f32", "cosmo_eval_host", "cosmo_probe_fma_f64", "cosmo_probe_fma_f32",
+           "cosmo_launch_count", "cosmo_last_cuda_error", "cosmo_strerror", "cosmo_version")
+
+
+class CosmoParams(C.Structure):
+    _fields_ = [("Om", C.c_void_p), ("OL", C.c_void_p), ("Or", C.c_void_p), ("H0", C.c_void_p)]
+
+
+class CosmoError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def lib():
+    """dlopen the CUDA library (no GPU needed to load it); raises if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise CosmoError(f"{LIB_PATH} is missing: build it with `python -m paper_2212_01937_b200.build` "
+                         "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, i64, u32, sz, ci = C.c_void_p, C.c_int64, C.c_uint32, C.c_size_t, C.c_int
+    L.cosmo_workspace_bytes.argtypes = [i64, i64, ci, u32, ci]
+    L.cosmo_workspace_bytes.restype = sz
+    for name in ("cosmo_eval", "cosmo_eval_f32"):
+        f = getattr(L, name)
+        f.argtypes = [vp, i64, CosmoParams, i64, ci, u32, vp, vp, vp, sz, vp]
+        f.restype = ci
+    for name in ("cosmo_vjp", "cosmo_vjp_f32"):
+        f = getattr(L, name)
+        f.argtypes = [vp, i64, CosmoParams, i64, ci, u32, vp, vp, vp, vp, vp, vp, sz, vp]
+        f.restype = ci
+    for name in ("cosmo_snia_loglike", "cosmo_snia_loglike_f32"):
+        f = getattr(L, name)
+        f.argtypes = [vp, vp, vp, i64, CosmoParams, i64, vp, vp, vp, sz, vp]
+        f.restype = ci
+    L.cosmo_eval_host.argtypes = [vp, i64, CosmoParams, i64, ci, u32, vp, vp, vp, vp, vp]
+    L.cosmo_eval_host.restype = ci
+    for name in ("cosmo_probe_fma_f64", "cosmo_probe_fma_f32"):
+        f = getattr(L, name)
+        f.argtypes = [ci, ci, vp, vp]
+        f.restype = ci
+    L.cosmo_launch_count.restype = i64
+    L.cosmo_last_cuda_error.restype = ci
+    L.cosmo_strerror.argtypes = [ci]
+    L.cosmo_strerror.restype = C.c_char_p
+    L.cosmo_version.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def which_mask(which) -> int:
+    if isinstance(which, int):
+        return which
+    m = 0
+    for w in which:
+        m |= WHICH_BITS[w]
+    return m
+
+
+def which_names(mask: int):
+    return tuple(n for n in WHICH_ORDER if mask & WHICH_BITS[n])
+
+
+def _check(rc: int):
+    if rc != 0:
+        L = lib()
+        msg = L.cosmo_strerror(rc).decode()
+        if rc == -6:
+            msg += f" [cudaError {L.cosmo_last_cuda_error()}]"
+        raise CosmoError(f"cosmo_b200 error {rc}: {msg}")
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise CosmoError("CUDA device required: the hot path runs only in CUDA kernels (no CPU fallback)")
+    return torch
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)
+
+
+def _dev(t, dtype, torch, name):
+    if not (t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise CosmoError(f"{name}: expected a contiguous CUDA tensor of dtype {dtype}")
+    return t
+
+
+def _params(Om, OL, Or, H0, torch):
+    ps = [_dev(p, torch.float64, torch, "params") for p in (Om, OL, Or, H0)]
+    n = ps[0].numel()
+    if any(p.numel() != n for p in ps):
+        raise CosmoError("Om, OL, Or, H0 must have the same length")
+    return CosmoParams(*[p.data_ptr() for p in ps]), n, ps
+
+
+def _stream(torch):
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def workspace_bytes(n_z, n_cosmo, mode, which, with_grad) -> int:
+    return int(lib().cosmo_workspace_bytes(n_z, n_cosmo, mode, which_mask(which), int(with_grad)))
+
+
+def _workspace(torch, nbytes, device, workspace):
+    if workspace is not None:
+        if workspace.numel() * workspace.element_size() < nbytes:
+            raise CosmoError("workspace tensor too small")
+        return workspace
+    return torch.empty(max(nbytes, 256), dtype=torch.uint8, device=device)
+
+
+def cosmo_eval(z, Om, OL, Or, H0, mode=ELEMENTWISE, which=("DC",), out=None, status=None, workspace=None):
+    """Forward.  Returns (out[n_which, rows, n_z], status[rows, n_z] uint8)."""
+    torch = _torch()
+    mask = which_mask(which)
+    f32 = z.dtype == torch.float32
+    dt = torch.float32 if f32 else torch.float64
+    _dev(z, dt, torch, "z")
+    P, n_cosmo, keep = _params(Om, OL, Or, H0, torch)
+    n_z = z.numel()
+    rows = n_cosmo if mode == OUTER else 1
+    nw = bin(mask).count("1")
+    if out is None:
+        out = torch.empty((nw, rows, n_z), dtype=dt, device=z.device)
+    if status is None:
+        status = torch.empty((rows, n_z), dtype=torch.uint8, device=z.device)
+    ws_b = workspace_bytes(n_z, n_cosmo, mode, mask, False)
+    ws = _workspace(torch, ws_b, z.device, workspace)
+    fn = lib().cosmo_eval_f32 if f32 else lib().cosmo_eval
+    _check(fn(_ptr(z), n_z, P, n_cosmo, mode, mask, _ptr(out), _ptr(status), _ptr(ws), ws.numel(), _stream(torch)))
+    return out, status
+
+
+def cosmo_vjp(z, Om, OL, Or, H0, grad_out, mode=ELEMENTWISE, which=("DC",), want_out=False, out=None, grad_z=None,
+              grad_params=None, status=None, workspace=None):
+    """Fused forward + VJP.  Returns (grad_z[n_z], grad_params[4, n_cosmo] float64, out or None, status)."""
+    torch = _torch()
+    mask = which_mask(which)
+    f32 = z.dtype == torch.float32
+    dt = torch.float32 if f32 else torch.float64
+    _dev(z, dt, torch, "z")
+    _dev(grad_out, dt, torch, "grad_out")
+    P, n_cosmo, keep = _params(Om, OL, Or, H0, torch)
+    n_z = z.numel()
+    rows = n_cosmo if mode == OUTER else 1
+    nw = bin(mask).count("1")
+    if grad_out.numel() != nw * rows * n_z:
+        raise CosmoError("grad_out must have shape [n_which, rows, n_z]")
+    if want_out and out is None:
+        out = torch.empty((nw, rows, n_z), dtype=dt, device=z.device)
+    if grad_z is None:
+        grad_z = torch.empty(n_z, dtype=dt, device=z.device)
+    if grad_params is None:
+        grad_params = torch.empty((4, n_cosmo), dtype=torch.float64, device=z.device)
+    if status is None:
+        status = torch.empty((rows, n_z), dtype=torch.uint8, device=z.device)
+    ws_b = workspace_bytes(n_z, n_cosmo, mode, mask, True)
+    ws = _workspace(torch, ws_b, z.device, workspace)
+    fn = lib().cosmo_vjp_f32 if f32 else lib().cosmo_vjp
+    _check(fn(_ptr(z), n_z, P, n_cosmo, mode, mask, _ptr(grad_out), _ptr(out), _ptr(grad_z), _ptr(grad_params), _ptr(status),
+              _ptr(ws), ws.numel(), _stream(torch)))
+    return grad_z, grad_params, out, status
+
+
+def cosmo_snia_loglike(z, mu_obs, sigma, Om, OL, Or, H0, want_grad=True, logL=None, grad=None, workspace=None):
+    """Fused SN-Ia Gaussian log-likelihood.  Returns (logL[S], grad[4, S] or None), float64."""
+    torch = _torch()
+    f32 = z.dtype == torch.float32
+    dt = torch.float32 if f32 else torch.float64
+    for t, nm in ((z, "z"), (mu_obs, "mu_obs"), (sigma, "sigma")):
+        _dev(t, dt, torch, nm)
+    P, S, keep = _params(Om, OL, Or, H0, torch)
+    N = z.numel()
+    if logL is None:
+        logL = torch.empty(S, dtype=torch.float64, device=z.device)
+    if want_grad and grad is None:
+        grad = torch.empty((4, S), dtype=torch.float64, device=z.device)
+    ws_b = workspace_bytes(N, S, OUTER, MU, True)
+    ws = _workspace(torch, ws_b, z.device, workspace)
+    fn = lib().cosmo_snia_loglike_f32 if f32 else lib().cosmo_snia_loglike
+    _check(fn(_ptr(z), _ptr(mu_obs), _ptr(sigma), N, P, S, _ptr(logL), _ptr(grad), _ptr(ws), ws.numel(), _stream(torch)))
+    return logL, grad
+
+
+def cosmo_eval_host(z, Om, OL, Or, H0, mode=ELEMENTWISE, which=("DC",), grad_out=None, want_out=True):
+    """Host-buffer call (numpy float64 arrays in, numpy out): H2D + kernels + D2H inside the library, synchronous."""
+    import numpy as np
+    _torch()
+    mask = which_mask(which)
+    arrs = [np.ascontiguousarray(a, dtype=np.float64) for a in (z, Om, OL, Or, H0)]
+    n_z, n_cosmo = arrs[0].shape[0], arrs[1].shape[0]
+    rows = n_cosmo if mode == OUTER else 1
+    nw = bin(mask).count("1")
+    vp = lambda a: C.c_void_p(a.ctypes.data) if a is not None else C.c_void_p(0)
+    P = CosmoParams(*[a.ctypes.data for a in arrs[1:]])
+    out = np.empty((nw, rows, n_z)) if (want_out or grad_out is None) else None
+    status = np.empty((rows, n_z), dtype=np.uint8)
+    gz = gp = None
+    if grad_out is not None:
+        grad_out = np.ascontiguousarray(grad_out, dtype=np.float64)
+        gz = np.empty(n_z)
+        gp = np.empty((4, n_cosmo))
+    _check(lib().cosmo_eval_host(vp(arrs[0]), n_z, P, n_cosmo, mode, mask, vp(grad_out), vp(out), vp(gz), vp(gp), vp(status)))
+    return out, gz, gp, status
+
+
+def probe_fma(dtype="f64", blocks=148 * 8, iters=4096):
+    """Launch the FMA-chain roofline probe on the current stream; returns flops of the launch."""
+    torch = _torch()
+    dt = torch.float64 if dtype == "f64" else torch.float32
+    sink = torch.empty(blocks * 256, dtype=dt, device="cuda")
+    fn = lib().cosmo_probe_fma_f64 if dtype == "f64" else lib().cosmo_probe_fma_f32
+    _check(fn(blocks, iters, _ptr(sink), _stream(torch)))
+    return blocks * 256 * iters * 8 * 2, sink
+
+
+def launch_count() -> int:
+    return int(lib().cosmo_launch_count())
+
+
+def version() -> str:
+    return lib().cosmo_version().decode()

@@ -1,0 +1,297 @@
+// cosmo_b200.cu -- launchers and the C ABI declared in include/cosmo_b200.h.  sm_100a only; no CPU path.
+#include <atomic>
+#include <mutex>
+#include "../../include/cosmo_b200.h"
+#include "cosmo_kernels.cuh"
+
+using namespace cb;
+
+namespace {
+
+std::atomic<int64_t> g_launches{0};
+std::atomic<int> g_last_cuda{0};
+
+inline size_t align256(size_t b) { return (b + 255) & ~size_t(255); }
+inline int64_t cdiv(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+int check_launch() {
+    ++g_launches;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { g_last_cuda = (int)e; return COSMO_E_CUDA; }
+    return COSMO_OK;
+}
+
+// S-chunk groups in gridDim.y: 1 when the redshift tiles alone fill the chip, else spread cosmologies too
+int grid_y(int64_t ntiles, int64_t S) {
+    const int64_t nchunks = cdiv(S, S_CHUNK);
+    if (ntiles >= 2 * 148 || nchunks <= 1) return 1;
+    int64_t want = cdiv(4 * 148, ntiles);
+    return (int)(want < nchunks ? want : nchunks);
+}
+
+struct WsLayout { size_t consts, part, gzpart, total; int ny; int64_t ntiles; };
+
+WsLayout ws_layout(int64_t n_z, int64_t n_cosmo, int mode, int with_grad, size_t elt) {
+    WsLayout L{};
+    const bool per_elem = (mode == COSMO_ELEMENTWISE && n_cosmo != 1);
+    if (per_elem) { L.total = 0; L.ny = 1; L.ntiles = 0; return L; }
+    L.ntiles = cdiv(n_z > 0 ? n_z : 1, TILE);
+    L.ny = grid_y(L.ntiles, n_cosmo);
+    L.consts = 0;
+    size_t off = align256((size_t)n_cosmo * sizeof(Cosmo<double>));
+    if (with_grad) {
+        L.part = off;
+        off += align256((size_t)L.ntiles * n_cosmo * 5 * sizeof(double));
+        L.gzpart = off;
+        if (L.ny > 1) off += align256((size_t)L.ny * n_z * elt);
+    }
+    L.total = off;
+    return L;
+}
+
+int check_common(const void* z, int64_t n_z, const cosmo_params& p, int64_t n_cosmo, int mode, uint32_t which) {
+    if (n_z < 0 || n_cosmo < 0) return COSMO_E_SIZE;
+    if (mode != COSMO_ELEMENTWISE && mode != COSMO_OUTER) return COSMO_E_MODE;
+    if (which == 0 || (which & ~uint32_t(W_ALL))) return COSMO_E_WHICH;
+    if (mode == COSMO_ELEMENTWISE && !(n_cosmo == 1 || n_cosmo == n_z)) return COSMO_E_SIZE;
+    if (n_z > 0 && n_cosmo == 0) return COSMO_E_SIZE;
+    if (n_z > 0 && (!z || !p.Om || !p.OL || !p.Or || !p.H0)) return COSMO_E_NULL;
+    return COSMO_OK;
+}
+
+template <typename T, int MODE>
+int launch_outer(OuterArgs& a, dim3 grid, cudaStream_t st) {
+    const bool kT = a.which & W_TL, kA = a.which & W_DABS;
+    if (MODE == MODE_SNIA) k_outer<T, false, false, MODE><<<grid, OUTER_THREADS, 0, st>>>(a);
+    else if (kT && kA) k_outer<T, true, true, MODE><<<grid, OUTER_THREADS, 0, st>>>(a);
+    else if (kT) k_outer<T, true, false, MODE><<<grid, OUTER_THREADS, 0, st>>>(a);
+    else if (kA) k_outer<T, false, true, MODE><<<grid, OUTER_THREADS, 0, st>>>(a);
+    else k_outer<T, false, false, MODE><<<grid, OUTER_THREADS, 0, st>>>(a);
+    return check_launch();
+}
+
+template <typename T, bool kG>
+int launch_elem(const T* z, const cosmo_params& p, int64_t N, unsigned which, const T* gout, T* out, T* gz, double* gparams,
+                uint8_t* status, cudaStream_t st) {
+    const bool kT = which & W_TL, kA = which & W_DABS;
+    dim3 grid((unsigned)cdiv(N, ELEM_THREADS));
+    if (kT && kA) k_elem<T, true, true, kG><<<grid, ELEM_THREADS, 0, st>>>(z, p.Om, p.OL, p.Or, p.H0, N, which, gout, out, gz, gparams, status);
+    else if (kT) k_elem<T, true, false, kG><<<grid, ELEM_THREADS, 0, st>>>(z, p.Om, p.OL, p.Or, p.H0, N, which, gout, out, gz, gparams, status);
+    else if (kA) k_elem<T, false, true, kG><<<grid, ELEM_THREADS, 0, st>>>(z, p.Om, p.OL, p.Or, p.H0, N, which, gout, out, gz, gparams, status);
+    else k_elem<T, false, false, kG><<<grid, ELEM_THREADS, 0, st>>>(z, p.Om, p.OL, p.Or, p.H0, N, which, gout, out, gz, gparams, status);
+    return check_launch();
+}
+
+// forward (gout == nullptr) or fused forward+VJP
+template <typename T>
+int run_eval(const T* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode, uint32_t which, const T* gout, T* out, T* gz,
+             double* gparams, uint8_t* status, void* ws, size_t ws_bytes, void* stream, bool with_grad) {
+    int rc = check_common(z, n_z, p, n_cosmo, mode, which);
+    if (rc) return rc;
+    if (with_grad && n_z > 0 && (!gout || !gz || !gparams)) return COSMO_E_NULL;
+    if (!with_grad && n_z > 0 && !out) return COSMO_E_NULL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (n_z == 0) {
+        if (with_grad && gparams && n_cosmo > 0 && mode == COSMO_OUTER) {
+            cudaMemsetAsync(gparams, 0, sizeof(double) * 4 * n_cosmo, st);
+        }
+        return COSMO_OK;
+    }
+    const bool per_elem = (mode == COSMO_ELEMENTWISE && n_cosmo != 1);
+    if (per_elem) {
+        return with_grad ? launch_elem<T, true>(z, p, n_z, which, gout, out, gz, gparams, status, st)
+                         : launch_elem<T, false>(z, p, n_z, which, nullptr, out, nullptr, nullptr, status, st);
+    }
+    WsLayout L = ws_layout(n_z, n_cosmo, mode, with_grad, sizeof(T));
+    if (ws_bytes < L.total || !ws) return ws ? COSMO_E_WORKSPACE : COSMO_E_NULL;
+    char* w = static_cast<char*>(ws);
+    Cosmo<double>* consts = reinterpret_cast<Cosmo<double>*>(w + L.consts);
+    const bool kT = which & W_TL, kA = which & W_DABS;
+    k_prep<<<(unsigned)cdiv(n_cosmo, 64), 64, 0, st>>>(p.Om, p.OL, p.Or, p.H0, n_cosmo, with_grad ? ((kT || kA) ? 2 : 1) : 0, consts);
+    if ((rc = check_launch())) return rc;
+    OuterArgs a{};
+    a.z = z; a.gout = gout; a.out = out; a.status = status; a.consts = consts;
+    a.N = n_z; a.S = n_cosmo; a.which = which;
+    {
+        const uintptr_t m = sizeof(T) == 8 ? 15 : 7;
+        a.vec = (n_z % 2 == 0) && ((reinterpret_cast<uintptr_t>(z) | reinterpret_cast<uintptr_t>(out) |
+                                    reinterpret_cast<uintptr_t>(gout) | reinterpret_cast<uintptr_t>(gz)) & m) == 0;
+    }
+    dim3 grid((unsigned)L.ntiles, (unsigned)L.ny);
+    if (!with_grad) return launch_outer<T, MODE_FWD>(a, grid, st);
+    a.part = reinterpret_cast<double*>(w + L.part);
+    a.gz_accumulate = L.ny > 1;
+    a.gz = a.gz_accumulate ? static_cast<void*>(w + L.gzpart) : static_cast<void*>(gz);
+    if ((rc = launch_outer<T, MODE_VJP>(a, grid, st))) return rc;
+    k_reduce_params<4><<<(unsigned)cdiv(n_cosmo * 4 * 32, 256), 256, 0, st>>>(a.part, L.ntiles, n_cosmo, nullptr, gparams);
+    if ((rc = check_launch())) return rc;
+    if (a.gz_accumulate) {
+        k_reduce_gz<T><<<(unsigned)cdiv(n_z, 256), 256, 0, st>>>(static_cast<const T*>(a.gz), L.ny, n_z, gz);
+        if ((rc = check_launch())) return rc;
+    }
+    return COSMO_OK;
+}
+
+template <typename T>
+int run_snia(const T* z, const T* mu_obs, const T* sigma, int64_t N, cosmo_params p, int64_t S, double* logL, double* grad,
+             void* ws, size_t ws_bytes, void* stream) {
+    if (N < 0 || S < 0) return COSMO_E_SIZE;
+    if (S > 0 && (!p.Om || !p.OL || !p.Or || !p.H0 || !logL)) return COSMO_E_NULL;
+    if (N > 0 && (!z || !mu_obs || !sigma)) return COSMO_E_NULL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (S == 0) return COSMO_OK;
+    if (N == 0) {
+        cudaMemsetAsync(logL, 0, sizeof(double) * S, st);
+        if (grad) cudaMemsetAsync(grad, 0, sizeof(double) * 4 * S, st);
+        return COSMO_OK;
+    }
+    WsLayout L = ws_layout(N, S, COSMO_OUTER, 1, sizeof(T));
+    if (!ws) return COSMO_E_NULL;
+    if (ws_bytes < L.total) return COSMO_E_WORKSPACE;
+    char* w = static_cast<char*>(ws);
+    Cosmo<double>* consts = reinterpret_cast<Cosmo<double>*>(w + L.consts);
+    int rc;
+    k_prep<<<(unsigned)cdiv(S, 64), 64, 0, st>>>(p.Om, p.OL, p.Or, p.H0, S, 1, consts);
+    if ((rc = check_launch())) return rc;
+    OuterArgs a{};
+    a.z = z; a.mu_obs = mu_obs; a.sigma = sigma; a.consts = consts; a.N = N; a.S = S; a.which = W_MU;
+    a.part = reinterpret_cast<double*>(w + L.part);
+    const uintptr_t m = sizeof(T) == 8 ? 15 : 7;
+    a.vec = (N % 2 == 0) && ((reinterpret_cast<uintptr_t>(z) | reinterpret_cast<uintptr_t>(mu_obs) | reinterpret_cast<uintptr_t>(sigma)) & m) == 0;
+    // the likelihood has no per-redshift output, so cosmology chunks can always spread over gridDim.y
+    int ny = (int)cdiv(S, S_CHUNK);
+    int64_t cap = cdiv(8 * 148, L.ntiles);
+    if (cap < 1) cap = 1;
+    if (ny > cap) ny = (int)cap;
+    dim3 grid((unsigned)L.ntiles, (unsigned)ny);
+    if ((rc = launch_outer<T, MODE_SNIA>(a, grid, st))) return rc;
+    k_reduce_params<5><<<(unsigned)cdiv(S * 5 * 32, 256), 256, 0, st>>>(a.part, L.ntiles, S, logL, grad);
+    return check_launch();
+}
+
+// grow-only device scratch of the host-buffer convenience call
+std::mutex g_host_mu;
+void* g_host_buf = nullptr;
+size_t g_host_cap = 0;
+
+}  // namespace
+
+extern "C" {
+
+size_t cosmo_workspace_bytes(int64_t n_z, int64_t n_cosmo, int mode, uint32_t which, int with_grad) {
+    (void)which;
+    if (n_z < 0 || n_cosmo < 0) return 0;
+    WsLayout L = ws_layout(n_z, n_cosmo, mode, with_grad, sizeof(double));
+    return L.total;
+}
+
+int cosmo_eval(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode, uint32_t which, double* out,
+               uint8_t* status, void* workspace, size_t ws_bytes, void* stream) {
+    return run_eval<double>(z, n_z, p, n_cosmo, mode, which, nullptr, out, nullptr, nullptr, status, workspace, ws_bytes, stream, false);
+}
+int cosmo_vjp(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode, uint32_t which, const double* grad_out,
+              double* out, double* grad_z, double* grad_params, uint8_t* status, void* workspace, size_t ws_bytes, void* stream) {
+    return run_eval<double>(z, n_z, p, n_cosmo, mode, which, grad_out, out, grad_z, grad_params, status, workspace, ws_bytes, stream, true);
+}
+int cosmo_snia_loglike(const double* z, const double* mu_obs, const double* sigma, int64_t N, cosmo_params p, int64_t S,
+                       double* logL, double* grad, void* workspace, size_t ws_bytes, void* stream) {
+    return run_snia<double>(z, mu_obs, sigma, N, p, S, logL, grad, workspace, ws_bytes, stream);
+}
+int cosmo_eval_f32(const float* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode, uint32_t which, float* out,
+                   uint8_t* status, void* workspace, size_t ws_bytes, void* stream) {
+    return run_eval<float>(z, n_z, p, n_cosmo, mode, which, nullptr, out, nullptr, nullptr, status, workspace, ws_bytes, stream, false);
+}
+int cosmo_vjp_f32(const float* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode, uint32_t which, const float* grad_out,
+                  float* out, float* grad_z, double* grad_params, uint8_t* status, void* workspace, size_t ws_bytes, void* stream) {
+    return run_eval<float>(z, n_z, p, n_cosmo, mode, which, grad_out, out, grad_z, grad_params, status, workspace, ws_bytes, stream, true);
+}
+int cosmo_snia_loglike_f32(const float* z, const float* mu_obs, const float* sigma, int64_t N, cosmo_params p, int64_t S,
+                           double* logL, double* grad, void* workspace, size_t ws_bytes, void* stream) {
+    return run_snia<float>(z, mu_obs, sigma, N, p, S, logL, grad, workspace, ws_bytes, stream);
+}
+
+int cosmo_eval_host(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode, uint32_t which,
+                    const double* grad_out, double* out, double* grad_z, double* grad_params, uint8_t* status) {
+    int rc = check_common(z, n_z, p, n_cosmo, mode, which);
+    if (rc) return rc;
+    if (n_z == 0) return COSMO_OK;
+    const bool with_grad = grad_out != nullptr;
+    if (with_grad && (!grad_z || !grad_params)) return COSMO_E_NULL;
+    if (!with_grad && !out) return COSMO_E_NULL;
+    const int64_t rows = (mode == COSMO_OUTER) ? n_cosmo : 1;
+    const int np = __builtin_popcount(which);
+    const size_t b_z = align256(sizeof(double) * n_z), b_p = align256(sizeof(double) * n_cosmo);
+    const size_t b_out = align256(sizeof(double) * np * rows * n_z);
+    const size_t b_gp = align256(sizeof(double) * 4 * n_cosmo), b_st = align256((size_t)rows * n_z);
+    const size_t b_ws = align256(cosmo_workspace_bytes(n_z, n_cosmo, mode, which, with_grad));
+    size_t total = b_z + 4 * b_p + (out ? b_out : 0) + (with_grad ? b_out + b_z + b_gp : 0) + (status ? b_st : 0) + b_ws;
+    std::lock_guard<std::mutex> lk(g_host_mu);
+    if (total > g_host_cap) {
+        if (g_host_buf) cudaFree(g_host_buf);
+        g_host_buf = nullptr; g_host_cap = 0;
+        cudaError_t e = cudaMalloc(&g_host_buf, total);
+        if (e != cudaSuccess) { g_last_cuda = (int)e; return COSMO_E_CUDA; }
+        g_host_cap = total;
+    }
+    char* base = static_cast<char*>(g_host_buf);
+    size_t off = 0;
+    auto take = [&](size_t b) { char* q = base + off; off += b; return q; };
+    double* d_z = (double*)take(b_z);
+    double* d_p[4];
+    for (int i = 0; i < 4; ++i) d_p[i] = (double*)take(b_p);
+    double* d_out = out ? (double*)take(b_out) : nullptr;
+    double* d_gout = with_grad ? (double*)take(b_out) : nullptr;
+    double* d_gz = with_grad ? (double*)take(b_z) : nullptr;
+    double* d_gp = with_grad ? (double*)take(b_gp) : nullptr;
+    uint8_t* d_st = status ? (uint8_t*)take(b_st) : nullptr;
+    void* d_ws = take(b_ws);
+    cudaStream_t st = nullptr;
+    cudaMemcpyAsync(d_z, z, sizeof(double) * n_z, cudaMemcpyHostToDevice, st);
+    const double* hp[4] = {p.Om, p.OL, p.Or, p.H0};
+    for (int i = 0; i < 4; ++i) cudaMemcpyAsync(d_p[i], hp[i], sizeof(double) * n_cosmo, cudaMemcpyHostToDevice, st);
+    if (with_grad) cudaMemcpyAsync(d_gout, grad_out, sizeof(double) * np * rows * n_z, cudaMemcpyHostToDevice, st);
+    cosmo_params dp{d_p[0], d_p[1], d_p[2], d_p[3]};
+    rc = with_grad ? cosmo_vjp(d_z, n_z, dp, n_cosmo, mode, which, d_gout, d_out, d_gz, d_gp, d_st, d_ws, b_ws, st)
+                   : cosmo_eval(d_z, n_z, dp, n_cosmo, mode, which, d_out, d_st, d_ws, b_ws, st);
+    if (rc) return rc;
+    if (out) cudaMemcpyAsync(out, d_out, sizeof(double) * np * rows * n_z, cudaMemcpyDeviceToHost, st);
+    if (with_grad) {
+        cudaMemcpyAsync(grad_z, d_gz, sizeof(double) * n_z, cudaMemcpyDeviceToHost, st);
+        cudaMemcpyAsync(grad_params, d_gp, sizeof(double) * 4 * n_cosmo, cudaMemcpyDeviceToHost, st);
+    }
+    if (status) cudaMemcpyAsync(status, d_st, (size_t)rows * n_z, cudaMemcpyDeviceToHost, st);
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { g_last_cuda = (int)e; return COSMO_E_CUDA; }
+    return COSMO_OK;
+}
+
+int cosmo_probe_fma_f64(int blocks, int iters, double* sink, void* stream) {
+    if (blocks <= 0 || iters < 0) return COSMO_E_SIZE;
+    if (!sink) return COSMO_E_NULL;
+    k_probe_fma<double><<<blocks, 256, 0, static_cast<cudaStream_t>(stream)>>>(iters, sink);
+    return check_launch();
+}
+int cosmo_probe_fma_f32(int blocks, int iters, float* sink, void* stream) {
+    if (blocks <= 0 || iters < 0) return COSMO_E_SIZE;
+    if (!sink) return COSMO_E_NULL;
+    k_probe_fma<float><<<blocks, 256, 0, static_cast<cudaStream_t>(stream)>>>(iters, sink);
+    return check_launch();
+}
+
+int64_t cosmo_launch_count(void) { return g_launches.load(); }
+int cosmo_last_cuda_error(void) { return g_last_cuda.load(); }
+const char* cosmo_strerror(int code) {
+    switch (code) {
+        case COSMO_OK: return "ok";
+        case COSMO_E_NULL: return "a required pointer is NULL";
+        case COSMO_E_SIZE: return "bad size (negative, or n_cosmo incompatible with mode)";
+        case COSMO_E_WHICH: return "bad `which` bitmask";
+        case COSMO_E_MODE: return "unknown mode";
+        case COSMO_E_WORKSPACE: return "workspace too small (see cosmo_workspace_bytes)";
+        case COSMO_E_CUDA: return "CUDA launch or runtime error (see cosmo_last_cuda_error)";
+        default: return "unknown error code";
+    }
+}
+const char* cosmo_version(void) { return "cosmo_b200 0.1.0 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,317 @@
+// cosmo_kernels.cuh -- the CUDA kernels of the hot path (sm_100a).  Launchers and the C ABI are in cosmo_b200.cu.
+//
+// Layout in HBM: SoA everywhere; z[N]; parameters Om/OL/Or/H0[S]; outputs and upstream
+// gradients as planes [plane][row][N] with N fastest, so that a warp reads/writes 512 contiguous bytes per plane row
+// (two consecutive elements per thread, 128-bit accesses in FP64).  Per-cosmology constants (82 numbers) are
+// computed once by k_prep and staged in shared memory by the OUTER kernels, one block = one tile of redshifts
+// looping over a chunk of cosmologies, so the only per-eval HBM traffic is grad_out (8 B) and, if asked, out.
+#pragma once
+#include <cuda_runtime.h>
+#include "cosmo_prep.cuh"
+#include "cosmo_obs.cuh"
+
+namespace cb {
+
+constexpr int OUTER_THREADS = 128;
+constexpr int KZ = 2;                               // consecutive redshifts per thread
+constexpr int TILE = OUTER_THREADS * KZ;            // redshifts per block
+constexpr int S_CHUNK = 32;                         // cosmologies staged in shared memory at a time
+constexpr int NWARP = OUTER_THREADS / 32;
+constexpr int ELEM_THREADS = 128;
+
+enum { MODE_FWD = 0, MODE_VJP = 1, MODE_SNIA = 2 };
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+    return v;
+}
+
+// S1-S3, one thread per cosmology
+__global__ void k_prep(const double* __restrict__ Om, const double* __restrict__ OL, const double* __restrict__ Or,
+                       const double* __restrict__ H0, int64_t S, int want_grad, Cosmo<double>* __restrict__ out) {
+    int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (s >= S) return;
+    Cosmo<double> C;
+    cosmo_prep(Om[s], OL[s], Or[s], H0[s], want_grad, C);
+    if (want_grad < 2) {
+        for (int t = 0; t < 3; ++t) {
+            for (int j = 0; j < 7; ++j) C.GA[t][j] = 0.0;
+            if (want_grad < 1) { for (int j = 0; j < 5; ++j) C.GI[t][j] = 0.0; for (int j = 0; j < 6; ++j) C.GT[t][j] = 0.0; }
+        }
+    }
+    out[s] = C;
+}
+
+template <typename T> struct Vec2;
+template <> struct Vec2<double> { using type = double2; };
+template <> struct Vec2<float> { using type = float2; };
+
+template <typename T>
+__device__ __forceinline__ void load2(const T* __restrict__ p, int64_t i, int64_t n, bool vec, T v[KZ]) {
+    if (vec && i + 1 < n) {
+        typename Vec2<T>::type t = *reinterpret_cast<const typename Vec2<T>::type*>(p + i);
+        v[0] = t.x; v[1] = t.y;
+    } else {
+        v[0] = p[i < n ? i : n - 1];
+        v[1] = p[i + 1 < n ? i + 1 : n - 1];
+    }
+}
+template <typename T>
+__device__ __forceinline__ void store2(T* __restrict__ p, int64_t i, int64_t n, bool vec, const T v[KZ]) {
+    if (vec && i + 1 < n) {
+        typename Vec2<T>::type t; t.x = v[0]; t.y = v[1];
+        *reinterpret_cast<typename Vec2<T>::type*>(p + i) = t;
+    } else {
+        if (i < n) p[i] = v[0];
+        if (i + 1 < n) p[i + 1] = v[1];
+    }
+}
+
+struct OuterArgs {
+    const void* z; const void* gout; const void* mu_obs; const void* sigma;
+    void* out; void* gz; uint8_t* status;
+    const Cosmo<double>* consts;
+    double* part;            // [ntiles][S][NP] partial parameter sums (NP = 4 vjp, 5 snia)
+    int64_t N, S;
+    unsigned which;
+    int gz_accumulate;       // gridDim.y > 1: gz holds [gridDim.y][N] partials
+    int vec;                 // N even and pointers 16-byte aligned
+};
+
+// OUTER forward / fused forward+VJP / fused likelihood.  grid = (tiles of TILE redshifts, S-chunk groups).
+template <typename T, bool kT, bool kA, int MODE>
+__global__ void __launch_bounds__(OUTER_THREADS) k_outer(OuterArgs a) {
+    constexpr bool kG = MODE != MODE_FWD;
+    constexpr int NP = MODE == MODE_SNIA ? 5 : 4;
+    __shared__ Cosmo<T> sc[S_CHUNK];
+    __shared__ double sacc[kG ? NWARP : 1][kG ? S_CHUNK : 1][NP];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t N = a.N, S = a.S;
+    const int64_t n0 = (int64_t)blockIdx.x * TILE + (int64_t)tid * KZ;
+    const bool vec = a.vec != 0;
+    const T* zp = static_cast<const T*>(a.z);
+    T zv[KZ];
+    load2<T>(zp, n0, N, vec, zv);
+    bool live[KZ];
+#pragma unroll
+    for (int k = 0; k < KZ; ++k) live[k] = n0 + k < N;
+    T mo[KZ], isig2[KZ], lnorm[KZ];
+    if (MODE == MODE_SNIA) {
+        T sg[KZ];
+        load2<T>(static_cast<const T*>(a.mu_obs), n0, N, vec, mo);
+        load2<T>(static_cast<const T*>(a.sigma), n0, N, vec, sg);
+#pragma unroll
+        for (int k = 0; k < KZ; ++k) {
+            isig2[k] = T(1) / (sg[k] * sg[k]);
+            lnorm[k] = -Num<T>::log_(sg[k]) - T(0.91893853320467274178);   // - ln sigma - ln(2 pi)/2
+        }
+    }
+    T gzacc[KZ];
+#pragma unroll
+    for (int k = 0; k < KZ; ++k) gzacc[k] = T(0);
+    int nplanes = __popc(a.which);
+    const VoteWarp vote;
+
+    for (int64_t c0 = (int64_t)blockIdx.y * S_CHUNK; c0 < S; c0 += (int64_t)gridDim.y * S_CHUNK) {
+        const int ns = (int)((S - c0 < S_CHUNK) ? (S - c0) : S_CHUNK);
+        __syncthreads();
+        for (int i = tid; i < ns * COSMO_NFIELDS; i += OUTER_THREADS) {
+            int sl = i / COSMO_NFIELDS, f = i - sl * COSMO_NFIELDS;
+            reinterpret_cast<T*>(&sc[sl])[f] = (T) reinterpret_cast<const double*>(&a.consts[c0 + sl])[f];
+        }
+        for (int sl = tid; sl < ns; sl += OUTER_THREADS) {
+            sc[sl].status = a.consts[c0 + sl].status;
+            sc[sl].cubic = a.consts[c0 + sl].cubic;
+        }
+        __syncthreads();
+        for (int sl = 0; sl < ns; ++sl) {
+            const Cosmo<T>& C = sc[sl];
+            const int64_t row = c0 + sl;
+            T pacc[NP];
+#pragma unroll
+            for (int j = 0; j < NP; ++j) pacc[j] = T(0);
+            T g[KZ][6];
+            if (MODE == MODE_VJP) {
+#pragma unroll
+                for (int k = 0; k < KZ; ++k)
+#pragma unroll
+                    for (int w = 0; w < 6; ++w) g[k][w] = T(0);
+                int pl = 0;
+                for (int w = 0; w < 6; ++w) {
+                    if (!(a.which >> w & 1)) continue;
+                    T t[KZ];
+                    load2<T>(static_cast<const T*>(a.gout) + ((int64_t)pl * S + row) * N, n0, N, vec, t);
+#pragma unroll
+                    for (int k = 0; k < KZ; ++k) g[k][w] = t[k];
+                    ++pl;
+                }
+            }
+            T ov[6][KZ];
+            uint8_t stv[KZ];
+#pragma unroll
+            for (int k = 0; k < KZ; ++k) {
+                Core<T> R;
+                R.K = T(0); R.TT = T(0); R.AA = T(0);
+                eval_core<T, kT, kA, kG, VoteWarp>(C, zv[k], vote, R);
+                Obs<T> O;
+                observables<T, kT, kA>(C, zv[k], R, MODE == MODE_SNIA ? (unsigned)W_MU : a.which, O);
+#pragma unroll
+                for (int w = 0; w < 6; ++w) ov[w][k] = O.v[w];
+                stv[k] = (uint8_t)O.status;
+                if (MODE == MODE_SNIA) {
+                    const T resid = mo[k] - O.v[3];
+                    T gg[6] = {T(0), T(0), T(0), resid * isig2[k], T(0), T(0)};
+                    T dummy = T(0), gp[4] = {T(0), T(0), T(0), T(0)};
+                    backward<T, false, false>(C, zv[k], R, O, gg, dummy, gp);
+                    const T ll = Num<T>::fma_(T(-0.5) * resid, resid * isig2[k], lnorm[k]);
+                    if (live[k]) {
+                        pacc[0] += ll;
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) pacc[1 + j] += gp[j];
+                    }
+                }
+                if (MODE == MODE_VJP) {
+                    T dz = T(0), gp[4] = {T(0), T(0), T(0), T(0)};
+                    backward<T, kT, kA>(C, zv[k], R, O, g[k], dz, gp);
+                    if (live[k]) {
+                        gzacc[k] += dz;
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) pacc[j] += gp[j];
+                    }
+                }
+            }
+            if (MODE != MODE_SNIA && a.out != nullptr) {
+                int pl = 0;
+                for (int w = 0; w < 6; ++w) {
+                    if (!(a.which >> w & 1)) continue;
+                    store2<T>(static_cast<T*>(a.out) + ((int64_t)pl * S + row) * N, n0, N, vec, ov[w]);
+                    ++pl;
+                }
+            }
+            if (MODE != MODE_SNIA && a.status != nullptr) {
+#pragma unroll
+                for (int k = 0; k < KZ; ++k)
+                    if (live[k]) a.status[row * N + n0 + k] = stv[k];
+            }
+            if (kG) {
+#pragma unroll
+                for (int j = 0; j < NP; ++j) {
+                    double v = warp_sum((double)pacc[j]);
+                    if (lane == 0) sacc[warp][sl][j] = v;
+                }
+            }
+        }
+        if (kG) {
+            __syncthreads();
+            for (int i = tid; i < ns * NP; i += OUTER_THREADS) {
+                int sl = i / NP, j = i - sl * NP;
+                double v = 0.0;
+#pragma unroll
+                for (int w = 0; w < NWARP; ++w) v += sacc[w][sl][j];
+                a.part[((int64_t)blockIdx.x * S + (c0 + sl)) * NP + j] = v;
+            }
+        }
+    }
+    (void)nplanes;
+    if (MODE == MODE_VJP) {
+        T* gzp = static_cast<T*>(a.gz) + (a.gz_accumulate ? (int64_t)blockIdx.y * N : 0);
+        store2<T>(gzp, n0, N, vec, gzacc);
+    }
+}
+
+// partial parameter sums [ntiles][S][NP] -> dst planes: dst_first[S] (snia logL) and dst_grad[4][S]; fixed order => deterministic
+template <int NP>
+__global__ void k_reduce_params(const double* __restrict__ part, int64_t ntiles, int64_t S, double* __restrict__ logL,
+                                double* __restrict__ grad) {
+    // one warp per (s, j)
+    const int64_t wid = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (wid >= S * NP) return;
+    const int64_t s = wid / NP;
+    const int j = (int)(wid - s * NP);
+    double v = 0.0;
+    for (int64_t t = lane; t < ntiles; t += 32) v += part[(t * S + s) * NP + j];
+    v = warp_sum(v);
+    if (lane == 0) {
+        if (NP == 5) {
+            if (j == 0) logL[s] = v;
+            else if (grad) grad[(int64_t)(j - 1) * S + s] = v;
+        } else {
+            grad[(int64_t)j * S + s] = v;
+        }
+    }
+}
+
+template <typename T>
+__global__ void k_reduce_gz(const T* __restrict__ part, int ny, int64_t N, T* __restrict__ gz) {
+    int64_t n = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (n >= N) return;
+    T v = T(0);
+    for (int y = 0; y < ny; ++y) v += part[(int64_t)y * N + n];
+    gz[n] = v;
+}
+
+// ELEMENTWISE with one cosmology per redshift: S1-S8 per thread, no reductions.
+template <typename T, bool kT, bool kA, bool kG>
+__global__ void __launch_bounds__(ELEM_THREADS) k_elem(const T* __restrict__ z, const double* __restrict__ Om,
+                                                       const double* __restrict__ OL, const double* __restrict__ Or,
+                                                       const double* __restrict__ H0, int64_t N, unsigned which,
+                                                       const T* __restrict__ gout, T* __restrict__ out, T* __restrict__ gz,
+                                                       double* __restrict__ gparams, uint8_t* __restrict__ status) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const bool live = i < N;
+    const int64_t ii = live ? i : N - 1;
+    Cosmo<T> C;
+    {
+        Cosmo<double> Cd;
+        cosmo_prep(Om[ii], OL[ii], Or[ii], H0[ii], kG ? ((kT || kA) ? 2 : 1) : 0, Cd);
+        convert_cosmo<T>(Cd, C);
+    }
+    const T zv = z[ii];
+    Core<T> R;
+    R.K = T(0); R.TT = T(0); R.AA = T(0);
+    eval_core<T, kT, kA, kG, VoteWarp>(C, zv, VoteWarp(), R);
+    Obs<T> O;
+    observables<T, kT, kA>(C, zv, R, which, O);
+    if (!live) return;
+    if (out != nullptr) {
+        int pl = 0;
+        for (int w = 0; w < 6; ++w) {
+            if (!(which >> w & 1)) continue;
+            out[(int64_t)pl * N + i] = O.v[w];
+            ++pl;
+        }
+    }
+    if (status != nullptr) status[i] = (uint8_t)O.status;
+    if (kG) {
+        T g[6];
+        int pl = 0;
+        for (int w = 0; w < 6; ++w) {
+            g[w] = T(0);
+            if (!(which >> w & 1)) continue;
+            g[w] = gout[(int64_t)pl * N + i];
+            ++pl;
+        }
+        T dz = T(0), gp[4] = {T(0), T(0), T(0), T(0)};
+        backward<T, kT, kA>(C, zv, R, O, g, dz, gp);
+        gz[i] = dz;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) gparams[(int64_t)j * N + i] = (double)gp[j];
+    }
+}
+
+// ALU roofline probes: 8 independent FMA chains per thread
+template <typename T>
+__global__ void __launch_bounds__(256) k_probe_fma(int iters, T* __restrict__ sink) {
+    T a0 = T(threadIdx.x) * T(1e-3), a1 = a0 + T(1), a2 = a0 + T(2), a3 = a0 + T(3), a4 = a0 + T(4), a5 = a0 + T(5), a6 = a0 + T(6),
+      a7 = a0 + T(7);
+    const T m = T(0.999999), c = T(1e-7);
+    for (int i = 0; i < iters; ++i) {
+        a0 = Num<T>::fma_(a0, m, c); a1 = Num<T>::fma_(a1, m, c); a2 = Num<T>::fma_(a2, m, c); a3 = Num<T>::fma_(a3, m, c);
+        a4 = Num<T>::fma_(a4, m, c); a5 = Num<T>::fma_(a5, m, c); a6 = Num<T>::fma_(a6, m, c); a7 = Num<T>::fma_(a7, m, c);
+    }
+    sink[blockIdx.x * (int64_t)blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+}
+
+}  // namespace cb

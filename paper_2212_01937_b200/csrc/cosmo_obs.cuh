@@ -1,0 +1,85 @@
+// cosmo_obs.cuh -- hot-path steps S7 (observables) and S8 (fused backward, no tape) for one element.
+//
+// S7: D_C = d_H I0, D_M = d_H sinn, D_L = (1+z) D_M, mu = 5 log10(D_L / 10 pc), t_L = T / H0, d_abs = d_H A
+//     (PAPER.md:88-95, :277 fn.22; readings R-units, R-sinn).
+// S8: d/dz = integrand at z; d/dH0 analytic; d/d(Om, OL, Or) with Ok eliminated from the SAME
+//     forward intermediates (I0, K, T, A and boundary terms), DESIGN.md "Gradients" (replaces the tape of
+//     eqs. (2.10)-(2.12) + appendix A, by their closed combination).
+#pragma once
+#include "cosmo_eval.cuh"
+
+namespace cb {
+
+template <typename T>
+struct Obs {
+    T v[6];            // DC, DM, DL, MU, TL, DABS
+    T F, Fi, Fk;       // curvature transform and its partials
+    unsigned status;
+};
+
+template <typename T, bool kT, bool kA>
+CB_HD void observables(const Cosmo<T>& C, T z, const Core<T>& R, unsigned which, Obs<T>& O) {
+    using N = Num<T>;
+    const T x = T(1) + z;
+    unsigned st = R.status;
+    sinn<T>(C.Ok, R.I0, O.F, O.Fi, O.Fk);
+    O.v[0] = C.dH * R.I0;
+    O.v[1] = C.dH * O.F;
+    O.v[2] = x * O.v[1];
+    O.v[3] = T(0);
+    if (which & W_MU) {
+        if (O.v[2] > T(0)) O.v[3] = N::fma_(T(FIVE_OVER_LN10), N::log_(O.v[2]), T(25));
+        else { O.v[3] = T(NAN); st |= ST_DL_NONPOS; }
+    }
+    O.v[4] = kT ? C.tH * R.TT : T(0);
+    O.v[5] = kA ? C.dH * R.AA : T(0);
+    if (st & (ST_ROOT_ON_PATH | ST_UNSUPPORTED)) {
+#pragma unroll
+        for (int i = 0; i < 6; ++i) O.v[i] = T(NAN);
+    }
+    O.status = st;
+}
+
+// VJP of one element: g[6] upstream (entries outside `which` must be 0).  Adds to gz and gp[0..3] = (Om, OL, Or, H0).
+template <typename T, bool kT, bool kA>
+CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, const T g[6], T& gz, T gp[4]) {
+    using N = Num<T>;
+    const T x = T(1) + z;
+    const T iE = T(1) / R.E;
+    // boundary terms b_k = x^k / E - 1 (cancellation-free)
+    const T xp1 = x + T(1);
+    const T n1 = z, n2 = z * xp1, n3 = z * N::fma_(xp1, x, T(1)), n4 = n2 * N::fma_(x, x, T(1));
+    const T bt0 = -R.Em1 * iE, bt1 = (n1 - R.Em1) * iE, bt2 = (n2 - R.Em1) * iE;
+    T gM = g[1] + x * g[2];
+    if (g[3] != T(0)) gM += T(FIVE_OVER_LN10) * g[3] / O.v[1];
+    const T aI = C.dH * N::fma_(gM, O.Fi, g[0]);
+    const T aK = -gM * C.dH * O.Fk;
+    T btA = T(0);
+    if (kA) btA = ((C.cubic ? n4 : n3) - R.Em1) * iE;
+#pragma unroll
+    for (int t = 0; t < 3; ++t) {
+        T dI = C.GI[t][0] * R.I0 + C.GI[t][1] * R.K + C.GI[t][2] * bt0 + C.GI[t][3] * bt1 + C.GI[t][4] * bt2;
+        T acc = N::fma_(aI, T(-0.5) * dI, aK);
+        if (kT) {
+            T dT = C.GT[t][0] * R.I0 + C.GT[t][1] * R.K + C.GT[t][2] * bt0 + C.GT[t][3] * bt1 + C.GT[t][4] * bt2 + C.GT[t][5] * R.TT;
+            acc = N::fma_(g[4] * C.tH, T(-0.5) * dT, acc);
+        }
+        if (kA) {
+            T dA = C.GA[t][0] * R.I0 + C.GA[t][1] * R.K + C.GA[t][2] * bt0 + C.GA[t][3] * bt1 + C.GA[t][4] * bt2 + C.GA[t][5] * btA
+                   + C.GA[t][6] * R.AA;
+            acc = N::fma_(g[5] * C.dH, T(-0.5) * dA, acc);
+        }
+        gp[t] += acc;
+    }
+    T h = g[0] * O.v[0] + g[1] * O.v[1] + g[2] * O.v[2] + g[3] * T(FIVE_OVER_LN10);
+    if (kT) h += g[4] * O.v[4];
+    if (kA) h += g[5] * O.v[5];
+    gp[3] -= h / C.H0;
+    T dz = aI * iE + g[2] * O.v[1];
+    if (g[3] != T(0)) dz += T(FIVE_OVER_LN10) * g[3] / x;
+    if (kT) dz += g[4] * C.tH * iE / x;
+    if (kA) dz += g[5] * C.dH * x * x * iE;
+    gz += dz;
+}
+
+}  // namespace cb

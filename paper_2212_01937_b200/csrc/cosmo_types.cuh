@@ -1,0 +1,71 @@
+// cosmo_types.cuh -- shared definitions of the CUDA path (no arithmetic of the method lives here).
+//
+// Notation follows arXiv:2212.01937: x = 1+z, E^2(x) of eq. (2.2),
+// the three fundamental integrals I0, T, A of eqs. (2.3)-(2.5) without their
+// unit prefactors.  DESIGN.md "Real-quadratic form" explains how the root tuple r of eq. (3.2)
+// is carried as two real quadratic factors.
+#pragma once
+#include <math.h>
+#include <stdint.h>
+
+#ifdef __CUDACC__
+#define CB_HD __host__ __device__ __forceinline__
+#else
+#define CB_HD inline
+#endif
+
+namespace cb {
+
+// units: DESIGN.md reading R-units (the paper is silent)
+constexpr double C_KM_S = 299792.458;             // km/s
+constexpr double HUBBLE_GYR = 977.7922216807891;  // (1 km/s/Mpc)^-1 in Gyr
+constexpr double FIVE_OVER_LN10 = 2.171472409516259138;
+
+// `which` bits, planes in ascending bit order (include/cosmo_b200.h)
+enum : unsigned { W_DC = 1, W_DM = 2, W_DL = 4, W_MU = 8, W_TL = 16, W_DABS = 32, W_ALL = 63 };
+// status bits (include/cosmo_b200.h)
+enum : unsigned { ST_ROOT_ON_PATH = 1, ST_UNSUPPORTED = 2, ST_DL_NONPOS = 4, ST_ITER_CAP = 8 };
+
+constexpr int NIT_CAP = 14;   // duplication steps never exceed this (status bit 8 when hit)
+
+// Per-cosmology constant block ("S3" of the hot path).  E^2(x) = Q1(x) Q2(x),
+//   Q1(x) = (Or x + m)(x - rn)        (the two negative real roots  -m/Or  and  rn;  Or = 0: linear)
+//   Q2(x) = x^2 + b x + c             (the remaining pair: complex-conjugate or two reals)
+template <typename T>
+struct Cosmo {
+    T Or, m, rn, b, c;
+    T Om, Ok, OL, H0;
+    T q11, q21;        // Q1(1), Q2(1)
+    T sD, sDr;         // disc(Q1) disc(Q2) / 4  and sqrt|.|   (u13^2 - u14^2)^2 = 4 z^4 sD
+    T theta;           // 2 f1 h2 + 2 h1 f2 - g1 g2 :  u12^2 - (u13^2+u14^2)/2 = z^2 theta / 2
+    T W;               // Or^2 Q2(-m/Or) = m^2 - Or b m + Or^2 c
+    T kf;              // (Or + m)/(1 - rn)
+    T xlim;            // smallest real root of E^2 above 1 (+inf if none): x >= xlim -> status 1
+    T dH, tH;          // c/H0 [Mpc], 1/H0 [Gyr]
+    // lookback time, eq. (3.8) with i = big root, j = rn
+    T p5c, Gp, qhc, OrM;
+    // absorption distance, eq. (3.9) with (i,j,k,l) = (rn, pair, pair, big); (B.3) when Or = 0
+    T Q2n, aF, WoOr, sig, mOrn;
+    // gradient basis coefficients: dX/dtheta = -1/2 sum_j G[theta][j] basis_j
+    T GI[3][5];        // X = I0 : basis (I0, K, b0, b1, b2)
+    T GT[3][6];        // X = T  : basis (I0, K, b0, b1, b2, T)
+    T GA[3][7];        // X = A  : basis (I0, K, b0, b1, b2, b3 (b4 when Or = 0), A)
+    unsigned status;
+    unsigned cubic;    // Or == 0
+};
+
+constexpr int COSMO_NFIELDS = 82;   // floating-point members of Cosmo<T>, in declaration order
+static_assert(sizeof(Cosmo<double>) == COSMO_NFIELDS * sizeof(double) + 2 * sizeof(unsigned), "Cosmo<T> layout");
+static_assert(sizeof(Cosmo<float>) == COSMO_NFIELDS * sizeof(float) + 2 * sizeof(unsigned), "Cosmo<T> layout");
+
+// FP64 block -> arithmetic type of the per-element path
+template <typename T>
+CB_HD void convert_cosmo(const Cosmo<double>& a, Cosmo<T>& b) {
+    const double* pa = reinterpret_cast<const double*>(&a);
+    T* pb = reinterpret_cast<T*>(&b);
+    for (int i = 0; i < COSMO_NFIELDS; ++i) pb[i] = (T)pa[i];
+    b.status = a.status;
+    b.cubic = a.cubic;
+}
+
+}  // namespace cb

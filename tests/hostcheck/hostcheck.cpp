@@ -1,0 +1,48 @@
+// hostcheck.cpp -- TEST HELPER ONLY (never loaded by the product path).
+// Compiles the per-element math headers of the CUDA path (paper_2212_01937_b200/csrc/*.cuh) with plain g++ so that
+// `-m "not gpu"` tests can check that host-compiled arithmetic against the oracle before any GPU time is spent.
+// The product runs these same headers inside CUDA kernels only; there is no CPU fallback (see binding.py).
+#include <stdint.h>
+#include "../../paper_2212_01937_b200/csrc/cosmo_prep.cuh"
+#include "../../paper_2212_01937_b200/csrc/cosmo_obs.cuh"
+
+using namespace cb;
+
+template <typename T>
+static void run(int64_t n, const double* z, const double* Om, const double* OL, const double* Or, const double* H0,
+                unsigned which, const double* gup, double* out, double* gz, double* gp, uint8_t* status) {
+    for (int64_t i = 0; i < n; ++i) {
+        Cosmo<double> Cd;
+        cosmo_prep(Om[i], OL[i], Or[i], H0[i], gup ? 2 : 0, Cd);
+        Cosmo<T> C;
+        convert_cosmo<T>(Cd, C);
+        Core<T> R;
+        R.K = 0; R.TT = 0; R.AA = 0;
+        eval_core<T, true, true, true, VoteNone>(C, (T)z[i], VoteNone(), R);
+        Obs<T> O;
+        observables<T, true, true>(C, (T)z[i], R, which, O);
+        for (int w = 0; w < 6; ++w) out[w * n + i] = (double)O.v[w];
+        status[i] = (uint8_t)O.status;
+        if (gup) {
+            T g[6], a = 0, p[4] = {0, 0, 0, 0};
+            for (int w = 0; w < 6; ++w) g[w] = (which >> w & 1) ? (T)gup[w * n + i] : T(0);
+            backward<T, true, true>(C, (T)z[i], R, O, g, a, p);
+            gz[i] = (double)a;
+            for (int t = 0; t < 4; ++t) gp[t * n + i] = (double)p[t];
+        }
+    }
+}
+
+extern "C" void hostcheck_f64(int64_t n, const double* z, const double* Om, const double* OL, const double* Or, const double* H0,
+                              unsigned which, const double* gup, double* out, double* gz, double* gp, uint8_t* status) {
+    run<double>(n, z, Om, OL, Or, H0, which, gup, out, gz, gp, status);
+}
+extern "C" void hostcheck_f32(int64_t n, const double* z, const double* Om, const double* OL, const double* Or, const double* H0,
+                              unsigned which, const double* gup, double* out, double* gz, double* gp, uint8_t* status) {
+    run<float>(n, z, Om, OL, Or, H0, which, gup, out, gz, gp, status);
+}
+extern "C" void hostcheck_factor(double Om, double OL, double Or, double* out5) {
+    Cosmo<double> C;
+    cosmo_prep(Om, OL, Or, 70.0, 0, C);
+    out5[0] = C.m; out5[1] = C.rn; out5[2] = C.b; out5[3] = C.c; out5[4] = (double)C.status;
+}
