@@ -102,6 +102,14 @@ int cosmo_eval_host(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosm
 int cosmo_probe_fma_f64(int blocks, int iters, double* sink, void* stream);
 int cosmo_probe_fma_f32(int blocks, int iters, float* sink, void* stream);
 
+/* Optional timing of the DOMINANT kernel of each call (the OUTER / ELEMENTWISE evaluation kernel, not prep/reduce) with
+ * CUDA events recorded on the launching stream.  cosmo_profile(1) starts (and resets) the statistics, cosmo_profile(0)
+ * stops; cosmo_profile_mean_ms synchronises on the last recorded launch and returns the mean duration in ms over the
+ * launches since the reset (count in *n_launches, nullable).  When on, each call first waits for the previous call's
+ * kernel to finish (host side), so leave it off outside measurements.  Not thread-safe. */
+int cosmo_profile(int on);
+double cosmo_profile_mean_ms(int64_t* n_launches);
+
 /* number of kernels the library has launched in this process (all entry points) */
 int64_t cosmo_launch_count(void);
 int cosmo_last_cuda_error(void);

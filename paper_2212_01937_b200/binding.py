@@ -20,6 +20,7 @@ WHICH_ORDER = ("DC", "DM", "DL", "MU", "TL", "DABS")
 # every symbol include/cosmo_b200.h declares
 SYMBOLS = ("cosmo_workspace_bytes", "cosmo_eval", "cosmo_vjp", "cosmo_snia_loglike", "cosmo_eval_f32", "cosmo_vjp_f32",
            "cosmo_snia_loglike_f32", "cosmo_eval_host", "cosmo_probe_fma_f64", "cosmo_probe_fma_f32",
+           "cosmo_profile", "cosmo_profile_mean_ms",
            "cosmo_launch_count", "cosmo_last_cuda_error", "cosmo_strerror", "cosmo_version")
 
 
@@ -65,6 +66,10 @@ def lib():
         f.argtypes = [ci, ci, vp, vp]
         f.restype = ci
     L.cosmo_launch_count.restype = i64
+    L.cosmo_profile.argtypes = [ci]
+    L.cosmo_profile.restype = ci
+    L.cosmo_profile_mean_ms.argtypes = [C.POINTER(i64)]
+    L.cosmo_profile_mean_ms.restype = C.c_double
     L.cosmo_last_cuda_error.restype = ci
     L.cosmo_strerror.argtypes = [ci]
     L.cosmo_strerror.restype = C.c_char_p
@@ -209,7 +214,7 @@ def cosmo_snia_loglike(z, mu_obs, sigma, Om, OL, Or, H0, want_grad=True, logL=No
     return logL, grad
 
 
-def cosmo_eval_host(z, Om, OL, Or, H0, mode=ELEMENTWISE, which=("DC",), grad_out=None, want_out=True):
+def cosmo_eval_host(z, Om, OL, Or, H0, mode=ELEMENTWISE, which=("DC",), grad_out=None, want_out=True, want_status=True):
     """Host-buffer call (numpy float64 arrays in, numpy out): H2D + kernels + D2H inside the library, synchronous."""
     import numpy as np
     _torch()
@@ -221,7 +226,7 @@ def cosmo_eval_host(z, Om, OL, Or, H0, mode=ELEMENTWISE, which=("DC",), grad_out
     vp = lambda a: C.c_void_p(a.ctypes.data) if a is not None else C.c_void_p(0)
     P = CosmoParams(*[a.ctypes.data for a in arrs[1:]])
     out = np.empty((nw, rows, n_z)) if (want_out or grad_out is None) else None
-    status = np.empty((rows, n_z), dtype=np.uint8)
+    status = np.empty((rows, n_z), dtype=np.uint8) if want_status else None
     gz = gp = None
     if grad_out is not None:
         grad_out = np.ascontiguousarray(grad_out, dtype=np.float64)
@@ -239,6 +244,17 @@ def probe_fma(dtype="f64", blocks=148 * 8, iters=4096):
     fn = lib().cosmo_probe_fma_f64 if dtype == "f64" else lib().cosmo_probe_fma_f32
     _check(fn(blocks, iters, _ptr(sink), _stream(torch)))
     return blocks * 256 * iters * 8 * 2, sink
+
+
+def profile(on: bool):
+    """start/stop CUDA-event timing of the dominant kernel of each call (see include/cosmo_b200.h)"""
+    _check(lib().cosmo_profile(int(on)))
+
+
+def profile_mean_ms():
+    n = C.c_int64(0)
+    ms = lib().cosmo_profile_mean_ms(C.byref(n))
+    return float(ms), int(n.value)
 
 
 def launch_count() -> int:

@@ -11,6 +11,30 @@ namespace {
 std::atomic<int64_t> g_launches{0};
 std::atomic<int> g_last_cuda{0};
 
+// optional timing of the dominant kernel (k_outer / k_elem) with CUDA events on the launching stream
+bool g_prof_on = false;
+cudaEvent_t g_prof_ev[2] = {nullptr, nullptr};
+double g_prof_ms_sum = 0.0;
+int64_t g_prof_n = 0;
+bool g_prof_pending = false;
+
+void prof_begin(cudaStream_t st) {
+    if (!g_prof_on) return;
+    if (g_prof_pending) {   // fold the previous launch in before reusing the events
+        float ms = 0.f;
+        if (cudaEventSynchronize(g_prof_ev[1]) == cudaSuccess && cudaEventElapsedTime(&ms, g_prof_ev[0], g_prof_ev[1]) == cudaSuccess) {
+            g_prof_ms_sum += ms; ++g_prof_n;
+        }
+        g_prof_pending = false;
+    }
+    cudaEventRecord(g_prof_ev[0], st);
+}
+void prof_end(cudaStream_t st) {
+    if (!g_prof_on) return;
+    cudaEventRecord(g_prof_ev[1], st);
+    g_prof_pending = true;
+}
+
 inline size_t align256(size_t b) { return (b + 255) & ~size_t(255); }
 inline int64_t cdiv(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
@@ -62,11 +86,13 @@ int check_common(const void* z, int64_t n_z, const cosmo_params& p, int64_t n_co
 template <typename T, int MODE>
 int launch_outer(OuterArgs& a, dim3 grid, cudaStream_t st) {
     const bool kT = a.which & W_TL, kA = a.which & W_DABS;
+    prof_begin(st);
     if (MODE == MODE_SNIA) k_outer<T, false, false, MODE><<<grid, OUTER_THREADS, 0, st>>>(a);
     else if (kT && kA) k_outer<T, true, true, MODE><<<grid, OUTER_THREADS, 0, st>>>(a);
     else if (kT) k_outer<T, true, false, MODE><<<grid, OUTER_THREADS, 0, st>>>(a);
     else if (kA) k_outer<T, false, true, MODE><<<grid, OUTER_THREADS, 0, st>>>(a);
     else k_outer<T, false, false, MODE><<<grid, OUTER_THREADS, 0, st>>>(a);
+    prof_end(st);
     return check_launch();
 }
 
@@ -75,10 +101,12 @@ int launch_elem(const T* z, const cosmo_params& p, int64_t N, unsigned which, co
                 uint8_t* status, cudaStream_t st) {
     const bool kT = which & W_TL, kA = which & W_DABS;
     dim3 grid((unsigned)cdiv(N, ELEM_THREADS));
+    prof_begin(st);
     if (kT && kA) k_elem<T, true, true, kG><<<grid, ELEM_THREADS, 0, st>>>(z, p.Om, p.OL, p.Or, p.H0, N, which, gout, out, gz, gparams, status);
     else if (kT) k_elem<T, true, false, kG><<<grid, ELEM_THREADS, 0, st>>>(z, p.Om, p.OL, p.Or, p.H0, N, which, gout, out, gz, gparams, status);
     else if (kA) k_elem<T, false, true, kG><<<grid, ELEM_THREADS, 0, st>>>(z, p.Om, p.OL, p.Or, p.H0, N, which, gout, out, gz, gparams, status);
     else k_elem<T, false, false, kG><<<grid, ELEM_THREADS, 0, st>>>(z, p.Om, p.OL, p.Or, p.H0, N, which, gout, out, gz, gparams, status);
+    prof_end(st);
     return check_launch();
 }
 
@@ -276,6 +304,29 @@ int cosmo_probe_fma_f32(int blocks, int iters, float* sink, void* stream) {
     if (!sink) return COSMO_E_NULL;
     k_probe_fma<float><<<blocks, 256, 0, static_cast<cudaStream_t>(stream)>>>(iters, sink);
     return check_launch();
+}
+
+int cosmo_profile(int on) {
+    if (on && !g_prof_ev[0]) {
+        if (cudaEventCreate(&g_prof_ev[0]) != cudaSuccess || cudaEventCreate(&g_prof_ev[1]) != cudaSuccess) {
+            g_last_cuda = (int)cudaGetLastError();
+            return COSMO_E_CUDA;
+        }
+    }
+    g_prof_on = on != 0;
+    g_prof_ms_sum = 0.0; g_prof_n = 0; g_prof_pending = false;
+    return COSMO_OK;
+}
+double cosmo_profile_mean_ms(int64_t* n_launches) {
+    if (g_prof_pending) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(g_prof_ev[1]) == cudaSuccess && cudaEventElapsedTime(&ms, g_prof_ev[0], g_prof_ev[1]) == cudaSuccess) {
+            g_prof_ms_sum += ms; ++g_prof_n;
+        }
+        g_prof_pending = false;
+    }
+    if (n_launches) *n_launches = g_prof_n;
+    return g_prof_n ? g_prof_ms_sum / (double)g_prof_n : 0.0;
 }
 
 int64_t cosmo_launch_count(void) { return g_launches.load(); }

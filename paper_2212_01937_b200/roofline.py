@@ -1,0 +1,20 @@
+"""Roofline bookkeeping for bench.py (no arithmetic of the method lives here).
+
+The hot path is bound by the plain FP64 ALUs (nothing is a dense contraction; HBM traffic is <= 16 B per eval).
+`achieved` = algorithmic FP64 flops per launch / kernel time, where the per-eval figure is the count of FP64
+instructions the kernel executes per (z, cosmology) pair, measured ONCE with Nsight Compute SASS counters
+(smsp__sass_thread_inst_executed_op_{dfma,dmul,dadd}_pred_on.sum, 2 flops per DFMA; profiles/ holds the capture and
+DESIGN.md "Roofline" the derivation).  `peak` = the DFMA rate bench.py measures live with the library's FMA-chain
+probe (cosmo_probe_fma_f64); the nominal figure beside it is 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz.
+"""
+
+# FP64 flops per eval of the config-3 fused forward+VJP kernel k_outer<double,0,0,VJP> (ncu, profiles/r01_*.md)
+FLOPS_PER_EVAL = {
+    "config3_vjp_mu_f64": 774.8,   # r01 capture: 2*273.8 DFMA + 169.1 DMUL + 58.1 DADD per eval (profiles/r01_k_outer_vjp.md)
+}
+
+# nominal B200 FP64 vector peak (context only; the denominator is the measured probe)
+NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+
+# algorithmic HBM bytes per eval, config 3 (grad_out read; z, params and constants stay on chip)
+BYTES_PER_EVAL_C3 = 8.0 + (8.0 + 8.0) / 64.0
