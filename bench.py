@@ -123,7 +123,7 @@ class ClockSampler(threading.Thread):
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_2212_01937_b200 import binding as cb, workloads as W, roofline as RL
+    from paper_2212_01937_b200 import binding as cb, workloads as W, roofline as RL, sharding
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -158,7 +158,7 @@ def run_ours(args):
     def step():
         cb.cosmo_vjp(z, Om, OL, Or, H0, gout, cb.OUTER, which, grad_z=gz, grad_params=gp, status=st, workspace=ws)
         if world > 1:
-            dist.all_reduce(gp)     # the path's only exchange: [4][S] parameter-gradient sums over the z shards
+            sharding.allreduce_sums(gp)     # the path's only exchange: [4][S] parameter-gradient sums over the z shards
 
     for _ in range(max(3, args.warmup)):
         step()
