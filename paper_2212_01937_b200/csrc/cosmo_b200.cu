@@ -87,11 +87,12 @@ template <typename T, int MODE>
 int launch_outer(OuterArgs& a, dim3 grid, cudaStream_t st) {
     const bool kT = a.which & W_TL, kA = a.which & W_DABS;
     prof_begin(st);
-    if (MODE == MODE_SNIA) k_outer<T, false, false, MODE><<<grid, OUTER_THREADS, 0, st>>>(a);
-    else if (kT && kA) k_outer<T, true, true, MODE><<<grid, OUTER_THREADS, 0, st>>>(a);
-    else if (kT) k_outer<T, true, false, MODE><<<grid, OUTER_THREADS, 0, st>>>(a);
-    else if (kA) k_outer<T, false, true, MODE><<<grid, OUTER_THREADS, 0, st>>>(a);
-    else k_outer<T, false, false, MODE><<<grid, OUTER_THREADS, 0, st>>>(a);
+    if (MODE == MODE_SNIA) k_outer<T, false, false, MODE, W_MU><<<grid, OUTER_THREADS, 0, st>>>(a);
+    else if (kT && kA) k_outer<T, true, true, MODE, 0><<<grid, OUTER_THREADS, 0, st>>>(a);
+    else if (kT) k_outer<T, true, false, MODE, 0><<<grid, OUTER_THREADS, 0, st>>>(a);
+    else if (kA) k_outer<T, false, true, MODE, 0><<<grid, OUTER_THREADS, 0, st>>>(a);
+    else if (a.which == W_MU) k_outer<T, false, false, MODE, W_MU><<<grid, OUTER_THREADS, 0, st>>>(a);
+    else k_outer<T, false, false, MODE, 0><<<grid, OUTER_THREADS, 0, st>>>(a);
     prof_end(st);
     return check_launch();
 }

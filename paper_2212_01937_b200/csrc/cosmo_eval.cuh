@@ -24,6 +24,30 @@ template <> struct Num<double> {
     static CB_HD double fma_(double a, double b, double c) { return fma(a, b, c); }
     static CB_HD double abs_(double a) { return fabs(a); }
     static CB_HD double max_(double a, double b) { return fmax(a, b); }
+    // Branch-free reciprocal square root / reciprocal: MUFU seed (2^-20, measured) + one cubic step (error ~ 2^-58).
+    // No special-case handling: arguments on the hot path are positive, finite and far from the subnormal range.
+    static CB_HD double rsqrt_(double a) {
+#ifdef __CUDA_ARCH__
+        double y;
+        asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+        const double t = a * y;
+        const double e = fma(-t, y, 1.0);
+        const double p = fma(0.375, e, 0.5);
+        return fma(y * e, p, y);
+#else
+        return 1.0 / sqrt(a);
+#endif
+    }
+    static CB_HD double rcp_(double b) {
+#ifdef __CUDA_ARCH__
+        double r;
+        asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(b));
+        const double e = fma(-b, r, 1.0);
+        return fma(r, fma(e, e, e), r);
+#else
+        return 1.0 / b;
+#endif
+    }
     static constexpr double QF = 400.0;    // (3 r)^(-1/6), r = 1e-16 (R_F stopping rule, ref. [10])
     static constexpr double QJ = 600.0;    // (r/4)^(-1/6)            (R_D, R_J)
     static constexpr double RC_SMALL = 0.03;
@@ -37,6 +61,14 @@ template <> struct Num<float> {
     static CB_HD float fma_(float a, float b, float c) { return fmaf(a, b, c); }
     static CB_HD float abs_(float a) { return fabsf(a); }
     static CB_HD float max_(float a, float b) { return fmaxf(a, b); }
+    static CB_HD float rsqrt_(float a) {
+#ifdef __CUDA_ARCH__
+        return rsqrtf(a);
+#else
+        return 1.0f / sqrtf(a);
+#endif
+    }
+    static CB_HD float rcp_(float b) { return 1.0f / b; }
     static constexpr float QF = 12.0f;     // r = 1e-7
     static constexpr float QJ = 19.0f;
     static constexpr float RC_SMALL = 0.25f;
@@ -80,182 +112,226 @@ template <typename T>
 struct Core {
     T I0, TT, AA;      // eqs. (2.3)-(2.5) without unit prefactors
     T K;               // int (Or x + m)/(x - rn) dx/E  (second kind; basis function of the gradients)
-    T E;               // E(z)
+    T E, iE;           // E(z), 1/E(z)
     T Em1;             // E(z) - 1, cancellation-free
     unsigned status;
 };
 
-// S4-S6.  kT: lookback integral, kA: absorption integral, kK: the second-kind integral K (needs R_D).
-template <typename T, bool kT, bool kA, bool kK, typename Vote>
-CB_HD void eval_core(const Cosmo<T>& C, T z, const Vote& vote, Core<T>& R) {
+// S4-S6 for K elements of the SAME cosmology in lock-step (K independent dependency chains per thread: the FP64
+// pipe has ~9 cycles of latency and few warps fit, so instruction-level parallelism is what keeps it busy).
+// kT: lookback integral, kA: absorption integral, kK: the second-kind integral K (needs R_D).
+template <typename T, bool kT, bool kA, bool kK, int K, typename Vote>
+CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Core<T> (&R)[K]) {
     using N = Num<T>;
     constexpr bool kD = kK || kA;          // R_D tail needed
-    const T x = T(1) + z;
-    const T z2 = z * z;
-    unsigned st = C.status;
-    if (!(x > T(0))) st |= ST_UNSUPPORTED;
-    if (x >= C.xlim) st |= ST_ROOT_ON_PATH;
-    // ---- S4 radicands
-    const T lin = N::fma_(C.Or, x, C.m);                 // Or x + m
-    const T xmr = x - C.rn;
-    const T q1x = lin * xmr;
-    const T q2x = N::fma_(x + C.b, x, C.c);
-    const T ra = N::sqrt_(q1x * C.q21), rb = N::sqrt_(C.q11 * q2x);
-    const T U12 = ra + rb;
-    T xa = U12 * U12;
-    T mp = N::fma_(T(-0.5) * z2, C.theta, xa);
-    T s = z2 * z2 * C.sD;
-    const T xa0 = xa, m0 = mp, s0 = s;
-    const T hs = z2 * C.sDr;                             // |h|
-    // E(z) and E(z) - 1 (for d/dz and the boundary terms of the gradients)
-    const T E2 = q1x * q2x;
-    const T Ev = N::sqrt_(E2);
-    {
-        T t = N::fma_(C.Or, N::fma_(N::fma_(x + T(1), x, T(1)), x, T(1)), N::fma_(C.Om, N::fma_(x + T(1), x, T(1)), C.Ok * (x + T(1))));
-        R.Em1 = z * t / (Ev + T(1));
-    }
-    R.E = Ev;
-    // ---- R_J parameters
-    T p5 = T(0), p0 = T(0), dl5 = T(0), dl0 = T(0), p5_0 = T(0), p0_0 = T(0);
-    if (kT) {
-        p5 = N::fma_(z2, C.p5c, xa);
-        p5_0 = p5;
-        T pm = p5 - mp;
-        dl5 = (p5 - xa) * N::fma_(pm, pm, -s);
-    }
+    T x[K], z2[K], lin[K], xmr[K], q2x[K], U12[K], xa[K], mp[K], s[K], xa0[K], m0[K], s0[K], hs[K], iE[K];
+    unsigned st[K];
+    T p5[K], p0[K], dl5[K], dl0[K], p5_0[K], p0_0[K], QFv[K], QDv[K], Q5v[K], Q0v[K];
     const bool quartA = kA && !C.cubic;
-    if (kA) {
-        p0 = quartA ? N::fma_(-C.Or * z2, C.Q2n, xa) : xa;
-        p0_0 = p0;
-        T pm = p0 - mp;
-        dl0 = (p0 - xa) * N::fma_(pm, pm, -s);
-    }
-    // ---- stopping rule (ref. [10]): 4^-n Q < |A_n| for every series that is summed
-    const T dxm = N::abs_(xa - mp);
-    const T QFv = N::QF * (T(2.0 / 3) * dxm + hs);
-    const T QDv = kD ? N::QJ * (T(3.0 / 5) * dxm + hs) : T(0);
-    T Q5v = T(0), Q0v = T(0);
-    if (kT) {
-        T A0 = (xa + T(2) * mp + T(2) * p5) * T(0.2);
-        Q5v = N::QJ * N::max_(N::max_(N::abs_(A0 - xa), N::abs_(A0 - mp) + hs), N::abs_(A0 - p5));
-    }
-    if (kA) {
-        T A0 = (xa + T(2) * mp + T(2) * p0) * T(0.2);
-        Q0v = N::QJ * N::max_(N::max_(N::abs_(A0 - xa), N::abs_(A0 - mp) + hs), N::abs_(A0 - p0));
-    }
-    // ---- S5 fused duplication
-    T f = T(1), tailD = T(0), sum5 = T(0), sum0 = T(0);
-    int nit = 0;
-    for (;;) {
-        bool more = f * QFv >= N::abs_(xa + T(2) * mp) * T(1.0 / 3);
-        if (kD) more = more || (f * QDv >= N::abs_(T(3) * xa + T(2) * mp) * T(0.2));
-        if (kT) more = more || (f * Q5v >= N::abs_(xa + T(2) * mp + T(2) * p5) * T(0.2));
-        if (kA) more = more || (f * Q0v >= N::abs_(xa + T(2) * mp + T(2) * p0) * T(0.2));
-        more = more && (st == 0);
-        if (nit >= NIT_CAP) { if (more) st |= ST_ITER_CAP; more = false; }
-        if (!vote.any(more)) break;
-        const T sx = N::sqrt_(xa);
-        const T spd = N::sqrt_(N::fma_(mp, mp, -s));
-        const T sa = N::sqrt_(T(2) * (mp + spd));
-        const T lam = N::fma_(sx, sa, spd);
-        if (kD) tailD += f / (sx * (xa + lam));
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        x[k] = T(1) + z[k];
+        z2[k] = z[k] * z[k];
+        st[k] = C.status;
+        if (!(x[k] > T(0))) st[k] |= ST_UNSUPPORTED;
+        if (x[k] >= C.xlim) st[k] |= ST_ROOT_ON_PATH;
+        // ---- S4 radicands
+        lin[k] = N::fma_(C.Or, x[k], C.m);               // Or x + m
+        xmr[k] = x[k] - C.rn;
+        const T q1x = lin[k] * xmr[k];
+        q2x[k] = N::fma_(x[k] + C.b, x[k], C.c);
+        const T a1 = q1x * C.q21, a2 = C.q11 * q2x[k];
+        const T ra = a1 * N::rsqrt_(a1), rb = a2 * N::rsqrt_(a2);
+        U12[k] = ra + rb;
+        xa[k] = U12[k] * U12[k];
+        mp[k] = N::fma_(T(-0.5) * z2[k], C.theta, xa[k]);
+        s[k] = z2[k] * z2[k] * C.sD;
+        xa0[k] = xa[k]; m0[k] = mp[k]; s0[k] = s[k];
+        hs[k] = z2[k] * C.sDr;                           // |h|
+        // E(z), 1/E(z) and E(z) - 1 (for d/dz and the boundary terms of the gradients)
+        const T E2 = q1x * q2x[k];
+        iE[k] = N::rsqrt_(E2);
+        const T Ev = E2 * iE[k];
+        const T xp1 = x[k] + T(1);
+        const T c2 = N::fma_(xp1, x[k], T(1));
+        const T t = N::fma_(C.Or, N::fma_(c2, x[k], T(1)), N::fma_(C.Om, c2, C.Ok * xp1));
+        R[k].Em1 = z[k] * t * N::rcp_(Ev + T(1));
+        R[k].E = Ev;
+        R[k].iE = iE[k];
+        // ---- R_J parameters
+        p5[k] = p0[k] = dl5[k] = dl0[k] = p5_0[k] = p0_0[k] = Q5v[k] = Q0v[k] = T(0);
         if (kT) {
-            const T rp = N::sqrt_(p5);
-            const T d = (rp + sx) * (p5 + N::fma_(rp, sa, spd));
-            const T e = f * f * f * dl5 / (d * d);
-            sum5 += f / d * rc1<T>(e);
-            p5 = T(0.25) * (p5 + lam);
+            p5[k] = N::fma_(z2[k], C.p5c, xa[k]);
+            p5_0[k] = p5[k];
+            const T pm = p5[k] - mp[k];
+            dl5[k] = (p5[k] - xa[k]) * N::fma_(pm, pm, -s[k]);
         }
         if (kA) {
-            const T rp = N::sqrt_(p0);
-            const T d = (rp + sx) * (p0 + N::fma_(rp, sa, spd));
-            const T e = f * f * f * dl0 / (d * d);
-            sum0 += f / d * rc1<T>(e);
-            p0 = T(0.25) * (p0 + lam);
+            p0[k] = quartA ? N::fma_(-C.Or * z2[k], C.Q2n, xa[k]) : xa[k];
+            p0_0[k] = p0[k];
+            const T pm = p0[k] - mp[k];
+            dl0[k] = (p0[k] - xa[k]) * N::fma_(pm, pm, -s[k]);
         }
-        xa = T(0.25) * (xa + lam);
-        mp = T(0.25) * (mp + lam);
-        s *= T(1.0 / 16);
+        // ---- stopping rule (ref. [10]): 4^-n Q < |A_n| for every series that is summed
+        const T dxm = N::abs_(xa[k] - mp[k]);
+        QFv[k] = N::QF * (T(2.0 / 3) * dxm + hs[k]);
+        QDv[k] = kD ? N::QJ * (T(3.0 / 5) * dxm + hs[k]) : T(0);
+        if (kT) {
+            const T A0 = (xa[k] + T(2) * mp[k] + T(2) * p5[k]) * T(0.2);
+            Q5v[k] = N::QJ * N::max_(N::max_(N::abs_(A0 - xa[k]), N::abs_(A0 - mp[k]) + hs[k]), N::abs_(A0 - p5[k]));
+        }
+        if (kA) {
+            const T A0 = (xa[k] + T(2) * mp[k] + T(2) * p0[k]) * T(0.2);
+            Q0v[k] = N::QJ * N::max_(N::max_(N::abs_(A0 - xa[k]), N::abs_(A0 - mp[k]) + hs[k]), N::abs_(A0 - p0[k]));
+        }
+    }
+    // ---- S5 fused duplication
+    T f = T(1), tailD[K], sum5[K], sum0[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) tailD[k] = sum5[k] = sum0[k] = T(0);
+    int nit = 0;
+    for (;;) {
+        bool more = false;
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            bool mk = f * QFv[k] >= N::abs_(xa[k] + T(2) * mp[k]) * T(1.0 / 3);
+            if (kD) mk = mk || (f * QDv[k] >= N::abs_(T(3) * xa[k] + T(2) * mp[k]) * T(0.2));
+            if (kT) mk = mk || (f * Q5v[k] >= N::abs_(xa[k] + T(2) * mp[k] + T(2) * p5[k]) * T(0.2));
+            if (kA) mk = mk || (f * Q0v[k] >= N::abs_(xa[k] + T(2) * mp[k] + T(2) * p0[k]) * T(0.2));
+            mk = mk && (st[k] == 0);
+            if (nit >= NIT_CAP && mk) { st[k] |= ST_ITER_CAP; mk = false; }
+            more = more || mk;
+        }
+        if (!vote.any(more)) break;
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            const T rx = N::rsqrt_(xa[k]);
+            const T sx = xa[k] * rx;
+            const T P = N::fma_(mp[k], mp[k], -s[k]);
+            const T spd = P * N::rsqrt_(P);
+            const T Q = T(2) * (mp[k] + spd);
+            const T sa = Q * N::rsqrt_(Q);
+            const T lam = N::fma_(sx, sa, spd);
+            if (kD) tailD[k] = N::fma_(f * rx, N::rcp_(xa[k] + lam), tailD[k]);
+            if (kT) {
+                const T rp = p5[k] * N::rsqrt_(p5[k]);
+                const T d = (rp + sx) * (p5[k] + N::fma_(rp, sa, spd));
+                const T id = N::rcp_(d);
+                const T e = f * f * f * dl5[k] * id * id;
+                sum5[k] = N::fma_(f * id, rc1<T>(e), sum5[k]);
+                p5[k] = T(0.25) * (p5[k] + lam);
+            }
+            if (kA) {
+                const T rp = p0[k] * N::rsqrt_(p0[k]);
+                const T d = (rp + sx) * (p0[k] + N::fma_(rp, sa, spd));
+                const T id = N::rcp_(d);
+                const T e = f * f * f * dl0[k] * id * id;
+                sum0[k] = N::fma_(f * id, rc1<T>(e), sum0[k]);
+                p0[k] = T(0.25) * (p0[k] + lam);
+            }
+            const T ql = T(0.25) * lam;
+            xa[k] = N::fma_(T(0.25), xa[k], ql);
+            mp[k] = N::fma_(T(0.25), mp[k], ql);
+            s[k] *= T(1.0 / 16);
+        }
         f *= T(0.25);
         ++nit;
     }
-    // ---- series: R_F
-    T RF;
-    {
-        const T An = (xa + T(2) * mp) * T(1.0 / 3);
-        const T g = f / An;
-        const T dl = (xa0 - m0) * T(1.0 / 3) * g;
-        const T vs = s0 * g * g;
-        const T e2 = T(-3) * dl * dl - vs;
-        const T e3 = T(-2) * dl * (dl * dl - vs);
-        const T S = T(1) - T(0.1) * e2 + T(1.0 / 14) * e3 + T(1.0 / 24) * e2 * e2 - T(3.0 / 44) * e2 * e3
-                    - T(5.0 / 208) * e2 * e2 * e2 + T(3.0 / 104) * e3 * e3 + T(1.0 / 16) * e2 * e2 * e3;
-        RF = S / N::sqrt_(An);
-    }
-    R.I0 = T(2) * z * RF;                                 // eq. (3.7) / (B.1)
-    // ---- series: R_D(u13^2, u14^2, u12^2)
-    T RD = T(0);
-    if (kD) {
-        const T AD = (T(3) * xa + T(2) * mp) * T(0.2);
-        const T g = f / AD;
-        const T dd = (xa0 - m0) * T(0.2) * g;
-        const T XY = T(9) * dd * dd - s0 * g * g;
-        const T Z = T(-2) * dd, Z2 = Z * Z;
-        const T e2 = XY - T(6) * Z2;
-        const T e3 = (T(3) * XY - T(8) * Z2) * Z;
-        const T e4 = T(3) * (XY - Z2) * Z2;
-        const T e5 = XY * Z2 * Z;
-        RD = f * series_J<T>(e2, e3, e4, e5) / (AD * N::sqrt_(AD)) + T(3) * tailD;
-    }
-    const T rU = T(1) / U12;
-    if (kK) {
-        // K = 2 z [ z^2/3 W R_D + sqrt((Or x + m) kf / (x - rn)) / u12 ]   (Carlson's [p_n = -3] integral)
-        R.K = T(2) * z * N::fma_(z2 * T(1.0 / 3) * C.W, RD, N::sqrt_(lin * C.kf / xmr) * rU);
-    }
-    auto rj_series = [&](T p_n, T p_init, T sum) -> T {
-        const T An = (xa + T(2) * mp + T(2) * p_n) * T(0.2);
-        const T A0 = (xa0 + T(2) * m0 + T(2) * p_init) * T(0.2);
-        const T g = f / An;
-        const T X = (A0 - xa0) * g;
-        const T am = A0 - m0;
-        const T YpZ = T(2) * am * g;
-        const T YZ = N::fma_(am, am, -s0) * g * g;
-        const T P = T(-0.5) * (X + YpZ);
-        const T XYZ = X * YZ;
-        const T P2 = P * P;
-        const T e2 = N::fma_(X, YpZ, YZ) - T(3) * P2;
-        const T e3 = XYZ + T(2) * e2 * P + T(4) * P2 * P;
-        const T e4 = (T(2) * XYZ + e2 * P + T(3) * P2 * P) * P;
-        const T e5 = XYZ * P2;
-        return f * series_J<T>(e2, e3, e4, e5) / (An * N::sqrt_(An)) + T(6) * sum;
-    };
-    if (kT) {
-        // eq. (3.8) with i = big root, j = rn, scaled so that Or -> 0 reproduces (B.2)
-        const T RJ5 = rj_series(p5, p5_0, sum5);
-        const T qh = x * p5_0 * C.qhc / lin;
-        const T sh = N::fma_(z2, C.OL, qh);
-        R.TT = T(2) * z * (z2 * T(1.0 / 3) * C.Gp * RJ5 + rc<T>(sh, qh) - C.OrM * RF);
-    }
-    if (kA) {
-        const T bnd = N::sqrt_(xmr * (T(1) - C.rn)) * rU;
-        if (quartA) {
-            // eq. (3.9) with (i,j,k,l) = (rn, pair, pair, big)
-            const T RJ0 = rj_series(p0, p0_0, sum0);
-            const T q0 = p0_0 / ((T(1) - C.rn) * xmr);
-            const T s0q = N::fma_(C.Or, z2, q0);
-            const T t1 = N::sqrt_(xmr * q2x / lin) - N::sqrt_((T(1) - C.rn) * C.q21 / (C.Or + C.m));
-            const T t2 = z * C.aF * RF;
-            const T t3 = z * C.WoOr * N::fma_(z2 * T(1.0 / 3) * C.Q2n, RD, bnd / N::sqrt_(lin * (C.Or + C.m)));
-            const T t4 = z * C.sig * N::fma_(z2 * T(1.0 / 3) * C.Q2n * C.mOrn, RJ0, rc<T>(s0q, q0));
-            R.AA = (t1 + t2) + (t3 + t4);
-        } else {
-            // eq. (B.3) with i = rn
-            R.AA = T(2.0 / 3) * z * (R.Em1 / (C.m * z) + C.aF * RF
-                                     + T(2) * C.sig * N::fma_(z2 * T(1.0 / 3) * C.Q2n * C.m, RD, bnd));
-            if (z == T(0)) R.AA = T(0);
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        // ---- series: R_F
+        T RF;
+        {
+            const T An = (xa[k] + T(2) * mp[k]) * T(1.0 / 3);
+            const T rA = N::rsqrt_(An);
+            const T g = f * rA * rA;
+            const T dl = (xa0[k] - m0[k]) * T(1.0 / 3) * g;
+            const T vs = s0[k] * g * g;
+            const T e2 = T(-3) * dl * dl - vs;
+            const T e3 = T(-2) * dl * (dl * dl - vs);
+            const T S = T(1) - T(0.1) * e2 + T(1.0 / 14) * e3 + T(1.0 / 24) * e2 * e2 - T(3.0 / 44) * e2 * e3
+                        - T(5.0 / 208) * e2 * e2 * e2 + T(3.0 / 104) * e3 * e3 + T(1.0 / 16) * e2 * e2 * e3;
+            RF = S * rA;
         }
+        R[k].I0 = T(2) * z[k] * RF;                       // eq. (3.7) / (B.1)
+        // ---- series: R_D(u13^2, u14^2, u12^2)
+        T RD = T(0);
+        if (kD) {
+            const T AD = (T(3) * xa[k] + T(2) * mp[k]) * T(0.2);
+            const T rA = N::rsqrt_(AD);
+            const T g = f * rA * rA;
+            const T dd = (xa0[k] - m0[k]) * T(0.2) * g;
+            const T XY = T(9) * dd * dd - s0[k] * g * g;
+            const T Z = T(-2) * dd, Z2 = Z * Z;
+            const T e2 = XY - T(6) * Z2;
+            const T e3 = (T(3) * XY - T(8) * Z2) * Z;
+            const T e4 = T(3) * (XY - Z2) * Z2;
+            const T e5 = XY * Z2 * Z;
+            RD = N::fma_(g * rA, series_J<T>(e2, e3, e4, e5), T(3) * tailD[k]);
+        }
+        const T rU = N::rcp_(U12[k]);
+        const T ixmr = N::rcp_(xmr[k]);
+        R[k].K = T(0); R[k].TT = T(0); R[k].AA = T(0);
+        if (kK) {
+            // K = 2 z [ z^2/3 W R_D + sqrt((Or x + m) kf / (x - rn)) / u12 ]   (Carlson's [p_n = -3] integral)
+            const T w = lin[k] * C.kf * ixmr;
+            R[k].K = T(2) * z[k] * N::fma_(z2[k] * T(1.0 / 3) * C.W, RD, w * N::rsqrt_(w) * rU);
+        }
+        auto rj_series = [&](T p_n, T p_init, T sum) -> T {
+            const T An = (xa[k] + T(2) * mp[k] + T(2) * p_n) * T(0.2);
+            const T A0 = (xa0[k] + T(2) * m0[k] + T(2) * p_init) * T(0.2);
+            const T rA = N::rsqrt_(An);
+            const T g = f * rA * rA;
+            const T X = (A0 - xa0[k]) * g;
+            const T am = A0 - m0[k];
+            const T YpZ = T(2) * am * g;
+            const T YZ = N::fma_(am, am, -s0[k]) * g * g;
+            const T P = T(-0.5) * (X + YpZ);
+            const T XYZ = X * YZ;
+            const T P2 = P * P;
+            const T e2 = N::fma_(X, YpZ, YZ) - T(3) * P2;
+            const T e3 = XYZ + T(2) * e2 * P + T(4) * P2 * P;
+            const T e4 = (T(2) * XYZ + e2 * P + T(3) * P2 * P) * P;
+            const T e5 = XYZ * P2;
+            return N::fma_(g * rA, series_J<T>(e2, e3, e4, e5), T(6) * sum);
+        };
+        if (kT) {
+            // eq. (3.8) with i = big root, j = rn, scaled so that Or -> 0 reproduces (B.2)
+            const T RJ5 = rj_series(p5[k], p5_0[k], sum5[k]);
+            const T qh = x[k] * p5_0[k] * C.qhc / lin[k];
+            const T sh = N::fma_(z2[k], C.OL, qh);
+            R[k].TT = T(2) * z[k] * (z2[k] * T(1.0 / 3) * C.Gp * RJ5 + rc<T>(sh, qh) - C.OrM * RF);
+        }
+        if (kA) {
+            const T bnd = N::sqrt_(xmr[k] * (T(1) - C.rn)) * rU;
+            if (quartA) {
+                // eq. (3.9) with (i,j,k,l) = (rn, pair, pair, big)
+                const T RJ0 = rj_series(p0[k], p0_0[k], sum0[k]);
+                const T q0 = p0_0[k] / ((T(1) - C.rn) * xmr[k]);
+                const T s0q = N::fma_(C.Or, z2[k], q0);
+                const T t1 = N::sqrt_(xmr[k] * q2x[k] / lin[k]) - N::sqrt_((T(1) - C.rn) * C.q21 / (C.Or + C.m));
+                const T t2 = z[k] * C.aF * RF;
+                const T t3 = z[k] * C.WoOr * N::fma_(z2[k] * T(1.0 / 3) * C.Q2n, RD, bnd / N::sqrt_(lin[k] * (C.Or + C.m)));
+                const T t4 = z[k] * C.sig * N::fma_(z2[k] * T(1.0 / 3) * C.Q2n * C.mOrn, RJ0, rc<T>(s0q, q0));
+                R[k].AA = (t1 + t2) + (t3 + t4);
+            } else {
+                // eq. (B.3) with i = rn
+                R[k].AA = T(2.0 / 3) * z[k] * (R[k].Em1 / (C.m * z[k]) + C.aF * RF
+                                               + T(2) * C.sig * N::fma_(z2[k] * T(1.0 / 3) * C.Q2n * C.m, RD, bnd));
+                if (z[k] == T(0)) R[k].AA = T(0);
+            }
+        }
+        R[k].status = st[k];
     }
-    R.status = st;
+}
+
+// single-element form (ELEMENTWISE kernel, host checks)
+template <typename T, bool kT, bool kA, bool kK, typename Vote>
+CB_HD void eval_core(const Cosmo<T>& C, T z, const Vote& vote, Core<T>& R) {
+    const T zz[1] = {z};
+    Core<T> RR[1];
+    eval_core_k<T, kT, kA, kK, 1, Vote>(C, zz, vote, RR);
+    R = RR[0];
 }
 
 // unified curvature transform in w = Ok I0^2 (reading R-sinn):

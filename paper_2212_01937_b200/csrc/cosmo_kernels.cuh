@@ -80,8 +80,12 @@ struct OuterArgs {
 };
 
 // OUTER forward / fused forward+VJP / fused likelihood.  grid = (tiles of TILE redshifts, S-chunk groups).
-template <typename T, bool kT, bool kA, int MODE>
-__global__ void __launch_bounds__(OUTER_THREADS) k_outer(OuterArgs a) {
+#ifndef CB_MINBLOCKS
+#define CB_MINBLOCKS 3
+#endif
+template <typename T, bool kT, bool kA, int MODE, unsigned WCT>
+__global__ void __launch_bounds__(OUTER_THREADS, CB_MINBLOCKS) k_outer(OuterArgs a) {
+    const unsigned which = WCT ? WCT : a.which;      // WCT != 0: output set known at compile time (drops dead planes)
     constexpr bool kG = MODE != MODE_FWD;
     constexpr int NP = MODE == MODE_SNIA ? 5 : 4;
     __shared__ Cosmo<T> sc[S_CHUNK];
@@ -110,7 +114,6 @@ __global__ void __launch_bounds__(OUTER_THREADS) k_outer(OuterArgs a) {
     T gzacc[KZ];
 #pragma unroll
     for (int k = 0; k < KZ; ++k) gzacc[k] = T(0);
-    int nplanes = __popc(a.which);
     const VoteWarp vote;
 
     for (int64_t c0 = (int64_t)blockIdx.y * S_CHUNK; c0 < S; c0 += (int64_t)gridDim.y * S_CHUNK) {
@@ -139,7 +142,7 @@ __global__ void __launch_bounds__(OUTER_THREADS) k_outer(OuterArgs a) {
                     for (int w = 0; w < 6; ++w) g[k][w] = T(0);
                 int pl = 0;
                 for (int w = 0; w < 6; ++w) {
-                    if (!(a.which >> w & 1)) continue;
+                    if (!(which >> w & 1)) continue;
                     T t[KZ];
                     load2<T>(static_cast<const T*>(a.gout) + ((int64_t)pl * S + row) * N, n0, N, vec, t);
 #pragma unroll
@@ -149,13 +152,12 @@ __global__ void __launch_bounds__(OUTER_THREADS) k_outer(OuterArgs a) {
             }
             T ov[6][KZ];
             uint8_t stv[KZ];
+            Core<T> R[KZ];
+            eval_core_k<T, kT, kA, kG, KZ, VoteWarp>(C, zv, vote, R);
 #pragma unroll
             for (int k = 0; k < KZ; ++k) {
-                Core<T> R;
-                R.K = T(0); R.TT = T(0); R.AA = T(0);
-                eval_core<T, kT, kA, kG, VoteWarp>(C, zv[k], vote, R);
                 Obs<T> O;
-                observables<T, kT, kA>(C, zv[k], R, MODE == MODE_SNIA ? (unsigned)W_MU : a.which, O);
+                observables<T, kT, kA>(C, zv[k], R[k], MODE == MODE_SNIA ? (unsigned)W_MU : which, O);
 #pragma unroll
                 for (int w = 0; w < 6; ++w) ov[w][k] = O.v[w];
                 stv[k] = (uint8_t)O.status;
@@ -163,7 +165,7 @@ __global__ void __launch_bounds__(OUTER_THREADS) k_outer(OuterArgs a) {
                     const T resid = mo[k] - O.v[3];
                     T gg[6] = {T(0), T(0), T(0), resid * isig2[k], T(0), T(0)};
                     T dummy = T(0), gp[4] = {T(0), T(0), T(0), T(0)};
-                    backward<T, false, false>(C, zv[k], R, O, gg, dummy, gp);
+                    backward<T, false, false>(C, zv[k], R[k], O, gg, dummy, gp);
                     const T ll = Num<T>::fma_(T(-0.5) * resid, resid * isig2[k], lnorm[k]);
                     if (live[k]) {
                         pacc[0] += ll;
@@ -173,7 +175,7 @@ __global__ void __launch_bounds__(OUTER_THREADS) k_outer(OuterArgs a) {
                 }
                 if (MODE == MODE_VJP) {
                     T dz = T(0), gp[4] = {T(0), T(0), T(0), T(0)};
-                    backward<T, kT, kA>(C, zv[k], R, O, g[k], dz, gp);
+                    backward<T, kT, kA>(C, zv[k], R[k], O, g[k], dz, gp);
                     if (live[k]) {
                         gzacc[k] += dz;
 #pragma unroll
@@ -184,7 +186,7 @@ __global__ void __launch_bounds__(OUTER_THREADS) k_outer(OuterArgs a) {
             if (MODE != MODE_SNIA && a.out != nullptr) {
                 int pl = 0;
                 for (int w = 0; w < 6; ++w) {
-                    if (!(a.which >> w & 1)) continue;
+                    if (!(which >> w & 1)) continue;
                     store2<T>(static_cast<T*>(a.out) + ((int64_t)pl * S + row) * N, n0, N, vec, ov[w]);
                     ++pl;
                 }
@@ -213,7 +215,6 @@ __global__ void __launch_bounds__(OUTER_THREADS) k_outer(OuterArgs a) {
             }
         }
     }
-    (void)nplanes;
     if (MODE == MODE_VJP) {
         T* gzp = static_cast<T*>(a.gz) + (a.gz_accumulate ? (int64_t)blockIdx.y * N : 0);
         store2<T>(gzp, n0, N, vec, gzacc);

@@ -45,13 +45,14 @@ template <typename T, bool kT, bool kA>
 CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, const T g[6], T& gz, T gp[4]) {
     using N = Num<T>;
     const T x = T(1) + z;
-    const T iE = T(1) / R.E;
+    const T iE = R.iE;
+    const T ix = N::rcp_(x);
     // boundary terms b_k = x^k / E - 1 (cancellation-free)
     const T xp1 = x + T(1);
     const T n1 = z, n2 = z * xp1, n3 = z * N::fma_(xp1, x, T(1)), n4 = n2 * N::fma_(x, x, T(1));
     const T bt0 = -R.Em1 * iE, bt1 = (n1 - R.Em1) * iE, bt2 = (n2 - R.Em1) * iE;
     T gM = g[1] + x * g[2];
-    if (g[3] != T(0)) gM += T(FIVE_OVER_LN10) * g[3] / O.v[1];
+    if (g[3] != T(0)) gM += T(FIVE_OVER_LN10) * g[3] * N::rcp_(O.v[1]);
     const T aI = C.dH * N::fma_(gM, O.Fi, g[0]);
     const T aK = -gM * C.dH * O.Fk;
     T btA = T(0);
@@ -74,10 +75,10 @@ CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, c
     T h = g[0] * O.v[0] + g[1] * O.v[1] + g[2] * O.v[2] + g[3] * T(FIVE_OVER_LN10);
     if (kT) h += g[4] * O.v[4];
     if (kA) h += g[5] * O.v[5];
-    gp[3] -= h / C.H0;
+    gp[3] -= h * C.dH * T(1.0 / C_KM_S);        // / H0
     T dz = aI * iE + g[2] * O.v[1];
-    if (g[3] != T(0)) dz += T(FIVE_OVER_LN10) * g[3] / x;
-    if (kT) dz += g[4] * C.tH * iE / x;
+    if (g[3] != T(0)) dz += T(FIVE_OVER_LN10) * g[3] * ix;
+    if (kT) dz += g[4] * C.tH * iE * ix;
     if (kA) dz += g[5] * C.dH * x * x * iE;
     gz += dz;
 }
