@@ -17,7 +17,28 @@ namespace cb {
 template <typename T> struct Num;
 template <> struct Num<double> {
     static CB_HD double sqrt_(double a) { return sqrt(a); }
-    static CB_HD double log_(double a) { return log(a); }
+    // ln(a) for positive normal a (hot path: D_L in Mpc).  Device: exponent split, t = (m-1)/(m+1) with m in
+    // [1/sqrt2, sqrt2), 2 atanh(t) by a degree-10 odd series (|t| <= 0.172, next term 2e-17); no special cases.
+    static CB_HD double log_(double a) {
+#ifdef __CUDA_ARCH__
+        int hi = __double2hiint(a), lo = __double2loint(a);
+        int e = (hi >> 20) - 1023;
+        hi = (hi & 0x000fffff) | 0x3ff00000;
+        if (hi >= 0x3ff6a09e) { hi -= 0x00100000; ++e; }          // m >= sqrt(2): halve
+        const double m = __hiloint2double(hi, lo);
+        const double t = (m - 1.0) * rcp_(m + 1.0);
+        const double t2 = t * t;
+        double p = CB_KT.rc[9];
+#pragma unroll
+        for (int j = 8; j >= 0; --j) p = fma(p, t2, CB_KT.rc[j]);
+        p = p * t2;                                                // atanh(t)/t - 1
+        const double ed = (double)e;
+        // e ln2 + 2t + 2t p, ln2 split so that e*ln2_hi is exact
+        return fma(ed, 6.93147180369123816490e-01, fma(2.0 * t, p, fma(ed, 1.90821492927058770002e-10, 2.0 * t)));
+#else
+        return log(a);
+#endif
+    }
     static CB_HD double exp_(double a) { return exp(a); }
     static CB_HD double atan_(double a) { return atan(a); }
     static CB_HD void sincos_(double a, double* s, double* c) { *s = sin(a); *c = cos(a); }
@@ -85,10 +106,9 @@ template <typename T>
 CB_HD T rc1(T e) {
     using N = Num<T>;
     if (N::abs_(e) < N::RC_SMALL) {
-        T s = T(1.0 / 21);
-        s = N::fma_(s, -e, T(1.0 / 19)); s = N::fma_(s, -e, T(1.0 / 17)); s = N::fma_(s, -e, T(1.0 / 15));
-        s = N::fma_(s, -e, T(1.0 / 13)); s = N::fma_(s, -e, T(1.0 / 11)); s = N::fma_(s, -e, T(1.0 / 9));
-        s = N::fma_(s, -e, T(1.0 / 7)); s = N::fma_(s, -e, T(1.0 / 5)); s = N::fma_(s, -e, T(1.0 / 3));
+        T s = T(CB_KT.rc[9]);
+#pragma unroll
+        for (int j = 8; j >= 0; --j) s = N::fma_(s, -e, T(CB_KT.rc[j]));
         return N::fma_(s, -e, T(1));
     }
     if (e > T(0)) { T r = N::sqrt_(e); return N::atan_(r) / r; }
@@ -102,9 +122,15 @@ CB_HD T rc(T x, T y) { return rc1<T>(y / x - T(1)) / Num<T>::sqrt_(x); }
 // Carlson's degree-7 series in the elementary symmetric functions (R_D / R_J form, ref. [10] as in DLMF 19.36.2)
 template <typename T>
 CB_HD T series_J(T E2, T E3, T E4, T E5) {
-    return T(1) - T(3.0 / 14) * E2 + T(1.0 / 6) * E3 + T(9.0 / 88) * E2 * E2 - T(3.0 / 22) * E4 - T(9.0 / 52) * E2 * E3
-           + T(3.0 / 26) * E5 - T(1.0 / 16) * E2 * E2 * E2 + T(3.0 / 40) * E3 * E3 + T(3.0 / 20) * E2 * E4
-           + T(45.0 / 272) * E2 * E2 * E3 - T(9.0 / 68) * (E3 * E4 + E2 * E5);
+    //  1 - 3E2/14 + E3/6 + 9E2^2/88 - 3E4/22 - 9E2E3/52 + 3E5/26 - E2^3/16 + 3E3^2/40 + 3E2E4/20 + 45E2^2E3/272
+    //    - 9(E3E4 + E2E5)/68, nested for FMAs
+    using N = Num<T>;
+    const double* c = CB_KT.rj;
+    const T a2 = N::fma_(E2, N::fma_(E2, T(c[2]), T(c[1])), T(c[0]));
+    const T a3 = N::fma_(E4, T(c[7]), N::fma_(E3, T(c[6]), N::fma_(E2, N::fma_(E2, T(c[5]), T(c[4])), T(c[3]))));
+    const T a4 = N::fma_(E2, T(c[9]), T(c[8]));
+    const T a5 = N::fma_(E2, T(c[7]), T(c[10]));
+    return N::fma_(E5, a5, N::fma_(E4, a4, N::fma_(E3, a3, N::fma_(E2, a2, T(1)))));
 }
 
 // what one element needs from the fused Carlson pass
@@ -124,65 +150,56 @@ template <typename T, bool kT, bool kA, bool kK, int K, typename Vote>
 CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Core<T> (&R)[K]) {
     using N = Num<T>;
     constexpr bool kD = kK || kA;          // R_D tail needed
-    T x[K], z2[K], lin[K], xmr[K], q2x[K], U12[K], xa[K], mp[K], s[K], xa0[K], m0[K], s0[K], hs[K], iE[K];
+    // Only U12 and the loop state stay live across the duplication loop; everything cheap is recomputed after it
+    // (registers decide how many warps fit).
+    T U12[K], ra[K], iE[K], xa[K], mp[K], s[K], Qc[K];
     unsigned st[K];
-    T p5[K], p0[K], dl5[K], dl0[K], p5_0[K], p0_0[K], QFv[K], QDv[K], Q5v[K], Q0v[K];
+    T p5[K], p0[K], dl5[K], dl0[K], p5_0[K], p0_0[K], Q5v[K], Q0v[K];
     const bool quartA = kA && !C.cubic;
 #pragma unroll
     for (int k = 0; k < K; ++k) {
-        x[k] = T(1) + z[k];
-        z2[k] = z[k] * z[k];
+        const T x = T(1) + z[k];
+        const T z2 = z[k] * z[k];
         st[k] = C.status;
-        if (!(x[k] > T(0))) st[k] |= ST_UNSUPPORTED;
-        if (x[k] >= C.xlim) st[k] |= ST_ROOT_ON_PATH;
+        if (!(x > T(0))) st[k] |= ST_UNSUPPORTED;
+        if (x >= C.xlim) st[k] |= ST_ROOT_ON_PATH;
         // ---- S4 radicands
-        lin[k] = N::fma_(C.Or, x[k], C.m);               // Or x + m
-        xmr[k] = x[k] - C.rn;
-        const T q1x = lin[k] * xmr[k];
-        q2x[k] = N::fma_(x[k] + C.b, x[k], C.c);
-        const T a1 = q1x * C.q21, a2 = C.q11 * q2x[k];
-        const T ra = a1 * N::rsqrt_(a1), rb = a2 * N::rsqrt_(a2);
-        U12[k] = ra + rb;
+        const T q1x = N::fma_(C.Or, x, C.m) * (x - C.rn);
+        const T q2x = N::fma_(x + C.b, x, C.c);
+        const T a1 = q1x * C.q21, a2 = C.q11 * q2x;
+        const T r1 = N::rsqrt_(a1), r2 = N::rsqrt_(a2);
+        ra[k] = a1 * r1;
+        iE[k] = r1 * r2;                                  // a1 a2 = E^2(x) E^2(1) and E(1) = 1 (sum of Omegas)
+        U12[k] = N::fma_(a2, r2, ra[k]);
         xa[k] = U12[k] * U12[k];
-        mp[k] = N::fma_(T(-0.5) * z2[k], C.theta, xa[k]);
-        s[k] = z2[k] * z2[k] * C.sD;
-        xa0[k] = xa[k]; m0[k] = mp[k]; s0[k] = s[k];
-        hs[k] = z2[k] * C.sDr;                           // |h|
-        // E(z), 1/E(z) and E(z) - 1 (for d/dz and the boundary terms of the gradients)
-        const T E2 = q1x * q2x[k];
-        iE[k] = N::rsqrt_(E2);
-        const T Ev = E2 * iE[k];
-        const T xp1 = x[k] + T(1);
-        const T c2 = N::fma_(xp1, x[k], T(1));
-        const T t = N::fma_(C.Or, N::fma_(c2, x[k], T(1)), N::fma_(C.Om, c2, C.Ok * xp1));
-        R[k].Em1 = z[k] * t * N::rcp_(Ev + T(1));
-        R[k].E = Ev;
-        R[k].iE = iE[k];
+        const T hd = T(0.5) * z2 * C.theta;               // u12^2 - (u13^2 + u14^2)/2
+        mp[k] = xa[k] - hd;
+        s[k] = z2 * z2 * C.sD;
+        const T hs = z2 * C.sDr;                          // |h|
         // ---- R_J parameters
         p5[k] = p0[k] = dl5[k] = dl0[k] = p5_0[k] = p0_0[k] = Q5v[k] = Q0v[k] = T(0);
         if (kT) {
-            p5[k] = N::fma_(z2[k], C.p5c, xa[k]);
+            p5[k] = N::fma_(z2, C.p5c, xa[k]);
             p5_0[k] = p5[k];
             const T pm = p5[k] - mp[k];
             dl5[k] = (p5[k] - xa[k]) * N::fma_(pm, pm, -s[k]);
         }
         if (kA) {
-            p0[k] = quartA ? N::fma_(-C.Or * z2[k], C.Q2n, xa[k]) : xa[k];
+            p0[k] = quartA ? N::fma_(-C.Or * z2, C.Q2n, xa[k]) : xa[k];
             p0_0[k] = p0[k];
             const T pm = p0[k] - mp[k];
             dl0[k] = (p0[k] - xa[k]) * N::fma_(pm, pm, -s[k]);
         }
-        // ---- stopping rule (ref. [10]): 4^-n Q < |A_n| for every series that is summed
-        const T dxm = N::abs_(xa[k] - mp[k]);
-        QFv[k] = N::QF * (T(2.0 / 3) * dxm + hs[k]);
-        QDv[k] = kD ? N::QJ * (T(3.0 / 5) * dxm + hs[k]) : T(0);
+        // ---- stopping rule (ref. [10]): 4^-n Q < |A_n| for every series that is summed.  R_F and R_D share one Q:
+        // the larger deviation bound (2/3 |xa - mp| + |h|) with the stricter constant of the two.
+        Qc[k] = (kD ? N::QJ : N::QF) * N::fma_(T(CB_KT.two_thirds), N::abs_(hd), hs);
         if (kT) {
             const T A0 = (xa[k] + T(2) * mp[k] + T(2) * p5[k]) * T(0.2);
-            Q5v[k] = N::QJ * N::max_(N::max_(N::abs_(A0 - xa[k]), N::abs_(A0 - mp[k]) + hs[k]), N::abs_(A0 - p5[k]));
+            Q5v[k] = N::QJ * N::max_(N::max_(N::abs_(A0 - xa[k]), N::abs_(A0 - mp[k]) + hs), N::abs_(A0 - p5[k]));
         }
         if (kA) {
             const T A0 = (xa[k] + T(2) * mp[k] + T(2) * p0[k]) * T(0.2);
-            Q0v[k] = N::QJ * N::max_(N::max_(N::abs_(A0 - xa[k]), N::abs_(A0 - mp[k]) + hs[k]), N::abs_(A0 - p0[k]));
+            Q0v[k] = N::QJ * N::max_(N::max_(N::abs_(A0 - xa[k]), N::abs_(A0 - mp[k]) + hs), N::abs_(A0 - p0[k]));
         }
     }
     // ---- S5 fused duplication
@@ -194,8 +211,9 @@ CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Cor
         bool more = false;
 #pragma unroll
         for (int k = 0; k < K; ++k) {
-            bool mk = f * QFv[k] >= N::abs_(xa[k] + T(2) * mp[k]) * T(1.0 / 3);
-            if (kD) mk = mk || (f * QDv[k] >= N::abs_(T(3) * xa[k] + T(2) * mp[k]) * T(0.2));
+            const T fq = f * Qc[k];
+            bool mk = T(3) * fq >= N::abs_(N::fma_(T(2), mp[k], xa[k]));
+            if (kD) mk = mk || (T(5) * fq >= N::abs_(N::fma_(T(3), xa[k], T(2) * mp[k])));
             if (kT) mk = mk || (f * Q5v[k] >= N::abs_(xa[k] + T(2) * mp[k] + T(2) * p5[k]) * T(0.2));
             if (kA) mk = mk || (f * Q0v[k] >= N::abs_(xa[k] + T(2) * mp[k] + T(2) * p0[k]) * T(0.2));
             mk = mk && (st[k] == 0);
@@ -232,25 +250,44 @@ CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Cor
             const T ql = T(0.25) * lam;
             xa[k] = N::fma_(T(0.25), xa[k], ql);
             mp[k] = N::fma_(T(0.25), mp[k], ql);
-            s[k] *= T(1.0 / 16);
+            s[k] *= T(CB_KT.sixteenth_inv);
         }
         f *= T(0.25);
         ++nit;
     }
 #pragma unroll
     for (int k = 0; k < K; ++k) {
+        const T x = T(1) + z[k];
+        const T z2 = z[k] * z[k];
+        const T lin = N::fma_(C.Or, x, C.m);               // Or x + m
+        const T xmr = x - C.rn;
+        const T q2x = N::fma_(x + C.b, x, C.c);
+        const T hd = T(0.5) * z2 * C.theta;                // xa0 - m0
+        const T xa0 = U12[k] * U12[k], m0 = xa0 - hd, s0 = z2 * z2 * C.sD;
+        {   // E(z), 1/E(z) and E(z) - 1 (for d/dz and the boundary terms of the gradients)
+            const T Ev = (U12[k] - ra[k]) * ra[k];          // sqrt(a2) sqrt(a1)
+            const T xp1 = x + T(1);
+            const T c2 = N::fma_(xp1, x, T(1));
+            const T t = N::fma_(C.Or, N::fma_(c2, x, T(1)), N::fma_(C.Om, c2, C.Ok * xp1));
+            R[k].Em1 = z[k] * t * N::rcp_(Ev + T(1));
+            R[k].E = Ev;
+            R[k].iE = iE[k];
+        }
         // ---- series: R_F
         T RF;
         {
-            const T An = (xa[k] + T(2) * mp[k]) * T(1.0 / 3);
+            const T An = (xa[k] + T(2) * mp[k]) * T(CB_KT.third);
             const T rA = N::rsqrt_(An);
             const T g = f * rA * rA;
-            const T dl = (xa0[k] - m0[k]) * T(1.0 / 3) * g;
-            const T vs = s0[k] * g * g;
+            const T dl = hd * T(CB_KT.third) * g;
+            const T vs = s0 * g * g;
             const T e2 = T(-3) * dl * dl - vs;
             const T e3 = T(-2) * dl * (dl * dl - vs);
-            const T S = T(1) - T(0.1) * e2 + T(1.0 / 14) * e3 + T(1.0 / 24) * e2 * e2 - T(3.0 / 44) * e2 * e3
-                        - T(5.0 / 208) * e2 * e2 * e2 + T(3.0 / 104) * e3 * e3 + T(1.0 / 16) * e2 * e2 * e3;
+            // 1 - e2/10 + e3/14 + e2^2/24 - 3 e2 e3/44 - 5 e2^3/208 + 3 e3^2/104 + e2^2 e3/16, nested for FMAs
+            const double* c = CB_KT.rf;
+            const T ta = N::fma_(e2, N::fma_(e2, T(c[2]), T(c[1])), T(c[0]));
+            const T tb = N::fma_(e3, T(c[6]), N::fma_(e2, N::fma_(e2, T(c[5]), T(c[4])), T(c[3])));
+            const T S = N::fma_(e3, tb, N::fma_(e2, ta, T(1)));
             RF = S * rA;
         }
         R[k].I0 = T(2) * z[k] * RF;                       // eq. (3.7) / (B.1)
@@ -260,8 +297,8 @@ CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Cor
             const T AD = (T(3) * xa[k] + T(2) * mp[k]) * T(0.2);
             const T rA = N::rsqrt_(AD);
             const T g = f * rA * rA;
-            const T dd = (xa0[k] - m0[k]) * T(0.2) * g;
-            const T XY = T(9) * dd * dd - s0[k] * g * g;
+            const T dd = hd * T(0.2) * g;
+            const T XY = T(9) * dd * dd - s0 * g * g;
             const T Z = T(-2) * dd, Z2 = Z * Z;
             const T e2 = XY - T(6) * Z2;
             const T e3 = (T(3) * XY - T(8) * Z2) * Z;
@@ -269,23 +306,23 @@ CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Cor
             const T e5 = XY * Z2 * Z;
             RD = N::fma_(g * rA, series_J<T>(e2, e3, e4, e5), T(3) * tailD[k]);
         }
-        const T rU = N::rcp_(U12[k]);
-        const T ixmr = N::rcp_(xmr[k]);
+        const T rUx = N::rcp_(U12[k] * xmr);               // 1/(u12 (x - rn))
+        const T rU = xmr * rUx;
         R[k].K = T(0); R[k].TT = T(0); R[k].AA = T(0);
         if (kK) {
             // K = 2 z [ z^2/3 W R_D + sqrt((Or x + m) kf / (x - rn)) / u12 ]   (Carlson's [p_n = -3] integral)
-            const T w = lin[k] * C.kf * ixmr;
-            R[k].K = T(2) * z[k] * N::fma_(z2[k] * T(1.0 / 3) * C.W, RD, w * N::rsqrt_(w) * rU);
+            // sqrt((Or x + m) kf / (x - rn)) = sqrt(kf / Q2(1)) sqrt(Q1(x) Q2(1)) / (x - rn)
+            R[k].K = T(2) * z[k] * N::fma_(z2 * T(CB_KT.third) * C.W, RD, C.ck * ra[k] * rUx);
         }
         auto rj_series = [&](T p_n, T p_init, T sum) -> T {
             const T An = (xa[k] + T(2) * mp[k] + T(2) * p_n) * T(0.2);
-            const T A0 = (xa0[k] + T(2) * m0[k] + T(2) * p_init) * T(0.2);
+            const T A0 = (xa0 + T(2) * m0 + T(2) * p_init) * T(0.2);
             const T rA = N::rsqrt_(An);
             const T g = f * rA * rA;
-            const T X = (A0 - xa0[k]) * g;
-            const T am = A0 - m0[k];
+            const T X = (A0 - xa0) * g;
+            const T am = A0 - m0;
             const T YpZ = T(2) * am * g;
-            const T YZ = N::fma_(am, am, -s0[k]) * g * g;
+            const T YZ = N::fma_(am, am, -s0) * g * g;
             const T P = T(-0.5) * (X + YpZ);
             const T XYZ = X * YZ;
             const T P2 = P * P;
@@ -298,26 +335,26 @@ CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Cor
         if (kT) {
             // eq. (3.8) with i = big root, j = rn, scaled so that Or -> 0 reproduces (B.2)
             const T RJ5 = rj_series(p5[k], p5_0[k], sum5[k]);
-            const T qh = x[k] * p5_0[k] * C.qhc / lin[k];
-            const T sh = N::fma_(z2[k], C.OL, qh);
-            R[k].TT = T(2) * z[k] * (z2[k] * T(1.0 / 3) * C.Gp * RJ5 + rc<T>(sh, qh) - C.OrM * RF);
+            const T qh = x * p5_0[k] * C.qhc / lin;
+            const T sh = N::fma_(z2, C.OL, qh);
+            R[k].TT = T(2) * z[k] * (z2 * T(CB_KT.third) * C.Gp * RJ5 + rc<T>(sh, qh) - C.OrM * RF);
         }
         if (kA) {
-            const T bnd = N::sqrt_(xmr[k] * (T(1) - C.rn)) * rU;
+            const T bnd = N::sqrt_(xmr * (T(1) - C.rn)) * rU;
             if (quartA) {
                 // eq. (3.9) with (i,j,k,l) = (rn, pair, pair, big)
                 const T RJ0 = rj_series(p0[k], p0_0[k], sum0[k]);
-                const T q0 = p0_0[k] / ((T(1) - C.rn) * xmr[k]);
-                const T s0q = N::fma_(C.Or, z2[k], q0);
-                const T t1 = N::sqrt_(xmr[k] * q2x[k] / lin[k]) - N::sqrt_((T(1) - C.rn) * C.q21 / (C.Or + C.m));
+                const T q0 = p0_0[k] / ((T(1) - C.rn) * xmr);
+                const T s0q = N::fma_(C.Or, z2, q0);
+                const T t1 = N::sqrt_(xmr * q2x / lin) - N::sqrt_((T(1) - C.rn) * C.q21 / (C.Or + C.m));
                 const T t2 = z[k] * C.aF * RF;
-                const T t3 = z[k] * C.WoOr * N::fma_(z2[k] * T(1.0 / 3) * C.Q2n, RD, bnd / N::sqrt_(lin[k] * (C.Or + C.m)));
-                const T t4 = z[k] * C.sig * N::fma_(z2[k] * T(1.0 / 3) * C.Q2n * C.mOrn, RJ0, rc<T>(s0q, q0));
+                const T t3 = z[k] * C.WoOr * N::fma_(z2 * T(CB_KT.third) * C.Q2n, RD, bnd / N::sqrt_(lin * (C.Or + C.m)));
+                const T t4 = z[k] * C.sig * N::fma_(z2 * T(CB_KT.third) * C.Q2n * C.mOrn, RJ0, rc<T>(s0q, q0));
                 R[k].AA = (t1 + t2) + (t3 + t4);
             } else {
                 // eq. (B.3) with i = rn
-                R[k].AA = T(2.0 / 3) * z[k] * (R[k].Em1 / (C.m * z[k]) + C.aF * RF
-                                               + T(2) * C.sig * N::fma_(z2[k] * T(1.0 / 3) * C.Q2n * C.m, RD, bnd));
+                R[k].AA = T(CB_KT.two_thirds) * z[k] * (R[k].Em1 / (C.m * z[k]) + C.aF * RF
+                                               + T(2) * C.sig * N::fma_(z2 * T(CB_KT.third) * C.Q2n * C.m, RD, bnd));
                 if (z[k] == T(0)) R[k].AA = T(0);
             }
         }
@@ -334,24 +371,30 @@ CB_HD void eval_core(const Cosmo<T>& C, T z, const Vote& vote, Core<T>& R) {
     R = RR[0];
 }
 
+// Horner evaluation of f = sum_{j<=D} w^j/(2j+1)!, g = sum w^j/(2j)!, f' = sum j w^(j-1)/(2j+1)!
+template <typename T, int D>
+CB_HD void sinn_poly(T w, T& sf, T& sg, T& sd) {
+    using N = Num<T>;
+    sf = T(CB_KT.fo[D]); sg = T(CB_KT.go[D]); sd = T(CB_KT.dfo[D]);
+#pragma unroll
+    for (int j = D - 1; j >= 0; --j) {
+        sf = N::fma_(sf, w, T(CB_KT.fo[j]));
+        sg = N::fma_(sg, w, T(CB_KT.go[j]));
+        if (j >= 1) sd = N::fma_(sd, w, T(CB_KT.dfo[j]));
+    }
+}
+
 // unified curvature transform in w = Ok I0^2 (reading R-sinn):
 //   F = I0 f(w), dF/dI0 = g(w), dF/dOk = I0^3 f'(w);  f = sum w^j/(2j+1)!, g = sum w^j/(2j)!
+// degree 7 for |w| <= 1/2 (next term 0.5^8/17! ~ 1e-17), degree 10 for |w| <= 1, libm beyond.
 template <typename T>
 CB_HD void sinn(T k, T I0, T& F, T& Fi, T& Fk) {
     using N = Num<T>;
     const T w = k * I0 * I0;
     if (N::abs_(w) <= T(1)) {
-        T sf = T(1.0 / 51090942171709440000.0), sg = T(1.0 / 2432902008176640000.0), sd = T(10.0 / 51090942171709440000.0);
-        const double FO[10] = {1.0 / 121645100408832000.0, 1.0 / 355687428096000.0, 1.0 / 1307674368000.0, 1.0 / 6227020800.0,
-                               1.0 / 39916800.0, 1.0 / 362880.0, 1.0 / 5040.0, 1.0 / 120.0, 1.0 / 6.0, 1.0};
-        const double GO[10] = {1.0 / 6402373705728000.0, 1.0 / 20922789888000.0, 1.0 / 87178291200.0, 1.0 / 479001600.0,
-                               1.0 / 3628800.0, 1.0 / 40320.0, 1.0 / 720.0, 1.0 / 24.0, 0.5, 1.0};
-#pragma unroll
-        for (int j = 0; j < 10; ++j) {
-            sf = N::fma_(sf, w, T(FO[j]));
-            sg = N::fma_(sg, w, T(GO[j]));
-            if (j < 9) sd = N::fma_(sd, w, T((9 - j) * FO[j]));
-        }
+        T sf, sg, sd;
+        if (N::abs_(w) <= T(0.5)) sinn_poly<T, 7>(w, sf, sg, sd);
+        else sinn_poly<T, 10>(w, sf, sg, sd);
         F = I0 * sf; Fi = sg; Fk = I0 * I0 * I0 * sd;
         return;
     }

@@ -13,7 +13,10 @@
 namespace cb {
 
 constexpr int OUTER_THREADS = 128;
-constexpr int KZ = 2;                               // consecutive redshifts per thread
+#ifndef CB_KZ
+#define CB_KZ 2
+#endif
+constexpr int KZ = CB_KZ;                           // consecutive redshifts per thread (even)
 constexpr int TILE = OUTER_THREADS * KZ;            // redshifts per block
 constexpr int S_CHUNK = 32;                         // cosmologies staged in shared memory at a time
 constexpr int NWARP = OUTER_THREADS / 32;
@@ -48,23 +51,29 @@ template <> struct Vec2<double> { using type = double2; };
 template <> struct Vec2<float> { using type = float2; };
 
 template <typename T>
-__device__ __forceinline__ void load2(const T* __restrict__ p, int64_t i, int64_t n, bool vec, T v[KZ]) {
-    if (vec && i + 1 < n) {
-        typename Vec2<T>::type t = *reinterpret_cast<const typename Vec2<T>::type*>(p + i);
-        v[0] = t.x; v[1] = t.y;
-    } else {
-        v[0] = p[i < n ? i : n - 1];
-        v[1] = p[i + 1 < n ? i + 1 : n - 1];
+__device__ __forceinline__ void load2(const T* __restrict__ p, int64_t i, int64_t n, bool vec, T (&v)[KZ]) {
+#pragma unroll
+    for (int k = 0; k < KZ; k += 2) {
+        if (vec && i + k + 1 < n) {
+            typename Vec2<T>::type t = *reinterpret_cast<const typename Vec2<T>::type*>(p + i + k);
+            v[k] = t.x; v[k + 1] = t.y;
+        } else {
+            v[k] = p[i + k < n ? i + k : n - 1];
+            v[k + 1] = p[i + k + 1 < n ? i + k + 1 : n - 1];
+        }
     }
 }
 template <typename T>
-__device__ __forceinline__ void store2(T* __restrict__ p, int64_t i, int64_t n, bool vec, const T v[KZ]) {
-    if (vec && i + 1 < n) {
-        typename Vec2<T>::type t; t.x = v[0]; t.y = v[1];
-        *reinterpret_cast<typename Vec2<T>::type*>(p + i) = t;
-    } else {
-        if (i < n) p[i] = v[0];
-        if (i + 1 < n) p[i + 1] = v[1];
+__device__ __forceinline__ void store2(T* __restrict__ p, int64_t i, int64_t n, bool vec, const T (&v)[KZ]) {
+#pragma unroll
+    for (int k = 0; k < KZ; k += 2) {
+        if (vec && i + k + 1 < n) {
+            typename Vec2<T>::type t; t.x = v[k]; t.y = v[k + 1];
+            *reinterpret_cast<typename Vec2<T>::type*>(p + i + k) = t;
+        } else {
+            if (i + k < n) p[i + k] = v[k];
+            if (i + k + 1 < n) p[i + k + 1] = v[k + 1];
+        }
     }
 }
 
@@ -81,10 +90,10 @@ struct OuterArgs {
 
 // OUTER forward / fused forward+VJP / fused likelihood.  grid = (tiles of TILE redshifts, S-chunk groups).
 #ifndef CB_MINBLOCKS
-#define CB_MINBLOCKS 3
+#define CB_MINBLOCKS 5     // chi-family kernels: 96 registers, 20 warps/SM (measured best, profiles/)
 #endif
 template <typename T, bool kT, bool kA, int MODE, unsigned WCT>
-__global__ void __launch_bounds__(OUTER_THREADS, CB_MINBLOCKS) k_outer(OuterArgs a) {
+__global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) k_outer(OuterArgs a) {
     const unsigned which = WCT ? WCT : a.which;      // WCT != 0: output set known at compile time (drops dead planes)
     constexpr bool kG = MODE != MODE_FWD;
     constexpr int NP = MODE == MODE_SNIA ? 5 : 4;
@@ -108,7 +117,7 @@ __global__ void __launch_bounds__(OUTER_THREADS, CB_MINBLOCKS) k_outer(OuterArgs
 #pragma unroll
         for (int k = 0; k < KZ; ++k) {
             isig2[k] = T(1) / (sg[k] * sg[k]);
-            lnorm[k] = -Num<T>::log_(sg[k]) - T(0.91893853320467274178);   // - ln sigma - ln(2 pi)/2
+            lnorm[k] = -Num<T>::log_(sg[k]) - T(CB_KT.half_ln_2pi);   // - ln sigma - ln(2 pi)/2
         }
     }
     T gzacc[KZ];

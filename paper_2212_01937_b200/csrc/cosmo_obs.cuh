@@ -28,7 +28,7 @@ CB_HD void observables(const Cosmo<T>& C, T z, const Core<T>& R, unsigned which,
     O.v[2] = x * O.v[1];
     O.v[3] = T(0);
     if (which & W_MU) {
-        if (O.v[2] > T(0)) O.v[3] = N::fma_(T(FIVE_OVER_LN10), N::log_(O.v[2]), T(25));
+        if (O.v[2] > T(0)) O.v[3] = N::fma_(T(CB_KT.five_over_ln10), N::log_(O.v[2]), T(25));
         else { O.v[3] = T(NAN); st |= ST_DL_NONPOS; }
     }
     O.v[4] = kT ? C.tH * R.TT : T(0);
@@ -46,13 +46,14 @@ CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, c
     using N = Num<T>;
     const T x = T(1) + z;
     const T iE = R.iE;
-    const T ix = N::rcp_(x);
+    const T rxd = N::rcp_(x * O.v[1]);                   // 1/(x D_M): one reciprocal serves 1/x and 1/D_M
+    const T ix = O.v[1] * rxd;
     // boundary terms b_k = x^k / E - 1 (cancellation-free)
     const T xp1 = x + T(1);
     const T n1 = z, n2 = z * xp1, n3 = z * N::fma_(xp1, x, T(1)), n4 = n2 * N::fma_(x, x, T(1));
     const T bt0 = -R.Em1 * iE, bt1 = (n1 - R.Em1) * iE, bt2 = (n2 - R.Em1) * iE;
     T gM = g[1] + x * g[2];
-    if (g[3] != T(0)) gM += T(FIVE_OVER_LN10) * g[3] * N::rcp_(O.v[1]);
+    if (g[3] != T(0)) gM += T(CB_KT.five_over_ln10) * g[3] * (x * rxd);
     const T aI = C.dH * N::fma_(gM, O.Fi, g[0]);
     const T aK = -gM * C.dH * O.Fk;
     T btA = T(0);
@@ -72,12 +73,12 @@ CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, c
         }
         gp[t] += acc;
     }
-    T h = g[0] * O.v[0] + g[1] * O.v[1] + g[2] * O.v[2] + g[3] * T(FIVE_OVER_LN10);
+    T h = g[0] * O.v[0] + g[1] * O.v[1] + g[2] * O.v[2] + g[3] * T(CB_KT.five_over_ln10);
     if (kT) h += g[4] * O.v[4];
     if (kA) h += g[5] * O.v[5];
     gp[3] -= h * C.dH * T(1.0 / C_KM_S);        // / H0
     T dz = aI * iE + g[2] * O.v[1];
-    if (g[3] != T(0)) dz += T(FIVE_OVER_LN10) * g[3] * ix;
+    if (g[3] != T(0)) dz += T(CB_KT.five_over_ln10) * g[3] * ix;
     if (kT) dz += g[4] * C.tH * iE * ix;
     if (kA) dz += g[5] * C.dH * x * x * iE;
     gz += dz;

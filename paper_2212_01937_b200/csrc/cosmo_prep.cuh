@@ -148,6 +148,7 @@ CB_HD void cosmo_prep(double Om, double OL, double Or, double H0, int want_grad,
     C.theta = 2.0 * f1 * c + 2.0 * h1 - g1 * b;
     C.W = fma(Or, fma(Or, c, -b * m), m * m);
     C.kf = (Or + m) / (1.0 - rn);
+    C.ck = sqrt(C.kf / C.q21);
     // validity: a real root of E^2 in (1, 1+z] -- only the pair can sit there
     C.xlim = INFINITY;
     if (D2 >= 0.0 && -0.5 * b > 1.0) {

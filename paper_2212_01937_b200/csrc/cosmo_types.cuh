@@ -21,6 +21,39 @@ constexpr double C_KM_S = 299792.458;             // km/s
 constexpr double HUBBLE_GYR = 977.7922216807891;  // (1 km/s/Mpc)^-1 in Gyr
 constexpr double FIVE_OVER_LN10 = 2.171472409516259138;
 
+// Numeric constants of the per-element path.  On the device they live in the constant bank so that FP64 instructions
+// take them as c[bank][offset] operands (a 64-bit literal otherwise costs two moves every time registers run short).
+struct KTab {
+    double third, two_thirds, sixteenth_inv;                      // 1/3, 2/3, 1/16
+    double five_over_ln10, half_ln_2pi;
+    double rf[7];      // R_F series: -1/10, 1/24, -5/208, 1/14, -3/44, 1/16, 3/104
+    double rj[11];     // R_D/R_J series: -3/14, 9/88, -1/16, 1/6, -9/52, 45/272, 3/40, -9/68, -3/22, 3/20, 3/26
+    double fo[11];     // 1/(2j+1)!
+    double go[11];     // 1/(2j)!
+    double dfo[11];    // j/(2j+1)!
+    double rc[10];     // 1/3, 1/5, ..., 1/21
+};
+#define CB_KTAB_INIT {                                                                                                          \
+    1.0 / 3, 2.0 / 3, 1.0 / 16, 2.171472409516259138, 0.91893853320467274178,                                                  \
+    {-0.1, 1.0 / 24, -5.0 / 208, 1.0 / 14, -3.0 / 44, 1.0 / 16, 3.0 / 104},                                                    \
+    {-3.0 / 14, 9.0 / 88, -1.0 / 16, 1.0 / 6, -9.0 / 52, 45.0 / 272, 3.0 / 40, -9.0 / 68, -3.0 / 22, 3.0 / 20, 3.0 / 26},      \
+    {1.0, 1.0 / 6.0, 1.0 / 120.0, 1.0 / 5040.0, 1.0 / 362880.0, 1.0 / 39916800.0, 1.0 / 6227020800.0, 1.0 / 1307674368000.0,   \
+     1.0 / 355687428096000.0, 1.0 / 121645100408832000.0, 1.0 / 51090942171709440000.0},                                       \
+    {1.0, 0.5, 1.0 / 24.0, 1.0 / 720.0, 1.0 / 40320.0, 1.0 / 3628800.0, 1.0 / 479001600.0, 1.0 / 87178291200.0,                \
+     1.0 / 20922789888000.0, 1.0 / 6402373705728000.0, 1.0 / 2432902008176640000.0},                                           \
+    {0.0, 1.0 / 6.0, 2.0 / 120.0, 3.0 / 5040.0, 4.0 / 362880.0, 5.0 / 39916800.0, 6.0 / 6227020800.0, 7.0 / 1307674368000.0,   \
+     8.0 / 355687428096000.0, 9.0 / 121645100408832000.0, 10.0 / 51090942171709440000.0},                                      \
+    {1.0 / 3, 1.0 / 5, 1.0 / 7, 1.0 / 9, 1.0 / 11, 1.0 / 13, 1.0 / 15, 1.0 / 17, 1.0 / 19, 1.0 / 21}}
+#ifdef __CUDACC__
+static __constant__ KTab KT_dev = CB_KTAB_INIT;
+#endif
+static const KTab KT_host = CB_KTAB_INIT;
+#ifdef __CUDA_ARCH__
+#define CB_KT KT_dev
+#else
+#define CB_KT KT_host
+#endif
+
 // `which` bits, planes in ascending bit order (include/cosmo_b200.h)
 enum : unsigned { W_DC = 1, W_DM = 2, W_DL = 4, W_MU = 8, W_TL = 16, W_DABS = 32, W_ALL = 63 };
 // status bits (include/cosmo_b200.h)
@@ -40,6 +73,7 @@ struct Cosmo {
     T theta;           // 2 f1 h2 + 2 h1 f2 - g1 g2 :  u12^2 - (u13^2+u14^2)/2 = z^2 theta / 2
     T W;               // Or^2 Q2(-m/Or) = m^2 - Or b m + Or^2 c
     T kf;              // (Or + m)/(1 - rn)
+    T ck;              // sqrt(kf / Q2(1))
     T xlim;            // smallest real root of E^2 above 1 (+inf if none): x >= xlim -> status 1
     T dH, tH;          // c/H0 [Mpc], 1/H0 [Gyr]
     // lookback time, eq. (3.8) with i = big root, j = rn
@@ -54,7 +88,7 @@ struct Cosmo {
     unsigned cubic;    // Or == 0
 };
 
-constexpr int COSMO_NFIELDS = 82;   // floating-point members of Cosmo<T>, in declaration order
+constexpr int COSMO_NFIELDS = 83;   // floating-point members of Cosmo<T>, in declaration order
 static_assert(sizeof(Cosmo<double>) == COSMO_NFIELDS * sizeof(double) + 2 * sizeof(unsigned), "Cosmo<T> layout");
 static_assert(sizeof(Cosmo<float>) == COSMO_NFIELDS * sizeof(float) + 2 * sizeof(unsigned), "Cosmo<T> layout");
 
