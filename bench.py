@@ -150,13 +150,14 @@ def run_ours(args):
     which = w.which
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     z, Om, OL, Or, H0, gout = t(w.z), t(w.Om), t(w.OL), t(w.Or), t(w.H0), t(w.grad_out)
+    out = torch.empty((len(which), S, N), dtype=torch.float64, device=dev)     # forward values are written too
     gz = torch.empty(N, dtype=torch.float64, device=dev)
     gp = torch.empty((4, S), dtype=torch.float64, device=dev)
     st = torch.empty((S, N), dtype=torch.uint8, device=dev)
     ws = torch.empty(max(256, cb.workspace_bytes(N, S, cb.OUTER, which, True)), dtype=torch.uint8, device=dev)
 
     def step():
-        cb.cosmo_vjp(z, Om, OL, Or, H0, gout, cb.OUTER, which, grad_z=gz, grad_params=gp, status=st, workspace=ws)
+        cb.cosmo_vjp(z, Om, OL, Or, H0, gout, cb.OUTER, which, out=out, grad_z=gz, grad_params=gp, status=st, workspace=ws)
         if world > 1:
             sharding.allreduce_sums(gp)     # the path's only exchange: [4][S] parameter-gradient sums over the z shards
 

@@ -45,12 +45,13 @@ int check_launch() {
     return COSMO_OK;
 }
 
-// S-chunk groups in gridDim.y: 1 when the redshift tiles alone fill the chip, else spread cosmologies too
+// S-chunk groups in gridDim.y.  The chip holds 148 SMs x 5 resident blocks; with fewer than ~16 blocks per slot the last
+// partial wave costs up to 10 % (measured, profiles/), so cosmology chunks are spread over gridDim.y until there are
+// enough blocks; grad_z is then accumulated through [ny][N] partials and a tiny reduction kernel.
 int grid_y(int64_t ntiles, int64_t S) {
     const int64_t nchunks = cdiv(S, S_CHUNK);
-    if (ntiles >= 2 * 148 || nchunks <= 1) return 1;
-    int64_t want = cdiv(4 * 148, ntiles);
-    return (int)(want < nchunks ? want : nchunks);
+    const int64_t want = cdiv((int64_t)16 * 148 * 5, ntiles);
+    return (int)(want < nchunks ? (want < 1 ? 1 : want) : nchunks);
 }
 
 struct WsLayout { size_t consts, part, gzpart, total; int ny; int64_t ntiles; };
@@ -189,7 +190,7 @@ int run_snia(const T* z, const T* mu_obs, const T* sigma, int64_t N, cosmo_param
     a.vec = (N % 2 == 0) && ((reinterpret_cast<uintptr_t>(z) | reinterpret_cast<uintptr_t>(mu_obs) | reinterpret_cast<uintptr_t>(sigma)) & m) == 0;
     // the likelihood has no per-redshift output, so cosmology chunks can always spread over gridDim.y
     int ny = (int)cdiv(S, S_CHUNK);
-    int64_t cap = cdiv(8 * 148, L.ntiles);
+    int64_t cap = cdiv((int64_t)16 * 148 * 5, L.ntiles);
     if (cap < 1) cap = 1;
     if (ny > cap) ny = (int)cap;
     dim3 grid((unsigned)L.ntiles, (unsigned)ny);

@@ -18,7 +18,10 @@ constexpr int OUTER_THREADS = 128;
 #endif
 constexpr int KZ = CB_KZ;                           // consecutive redshifts per thread (even)
 constexpr int TILE = OUTER_THREADS * KZ;            // redshifts per block
-constexpr int S_CHUNK = 32;                         // cosmologies staged in shared memory at a time
+#ifndef CB_SCHUNK
+#define CB_SCHUNK 16
+#endif
+constexpr int S_CHUNK = CB_SCHUNK;                         // cosmologies staged in shared memory at a time
 constexpr int NWARP = OUTER_THREADS / 32;
 constexpr int ELEM_THREADS = 128;
 

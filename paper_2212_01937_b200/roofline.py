@@ -16,5 +16,5 @@ FLOPS_PER_EVAL = {
 # nominal B200 FP64 vector peak (context only; the denominator is the measured probe)
 NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 
-# algorithmic HBM bytes per eval, config 3 (grad_out read; z, params and constants stay on chip)
-BYTES_PER_EVAL_C3 = 8.0 + (8.0 + 8.0) / 64.0
+# algorithmic HBM bytes per eval, config 3 as bench.py runs it (z, params and constants stay on chip)
+BYTES_PER_EVAL_C3 = 8.0 + 8.0 + 1.0 + (8.0 + 8.0) / 64.0   # grad_out read, out + status written, z/grad_z amortised over S
