@@ -296,7 +296,7 @@ __global__ void __launch_bounds__(ELEM_THREADS) k_elem(const T* __restrict__ z, 
             ++pl;
         }
     }
-    if (status != nullptr) status[i] = (uint8_t)O.status;
+    if (status != nullptr && !kG) status[i] = (uint8_t)O.status;
     if (kG) {
         T g[6];
         int pl = 0;
@@ -307,7 +307,9 @@ __global__ void __launch_bounds__(ELEM_THREADS) k_elem(const T* __restrict__ z, 
             ++pl;
         }
         T dz = T(0), gp[4] = {T(0), T(0), T(0), T(0)};
-        backward<T, kT, kA>(C, zv, R, O, g, dz, gp);
+        T cond = T(0);
+        backward<T, kT, kA, true>(C, zv, R, O, g, dz, gp, &cond);
+        if (status != nullptr) status[i] = (uint8_t)(O.status | ((cond > T(sizeof(T) == 8 ? GRAD_COND_LIMIT : 30.0) || !(cond == cond)) ? ST_GRAD_ILLCOND : 0u));
         gz[i] = dz;
 #pragma unroll
         for (int j = 0; j < 4; ++j) gparams[(int64_t)j * N + i] = (double)gp[j];

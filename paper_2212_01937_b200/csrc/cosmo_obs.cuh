@@ -41,8 +41,10 @@ CB_HD void observables(const Cosmo<T>& C, T z, const Core<T>& R, unsigned which,
 }
 
 // VJP of one element: g[6] upstream (entries outside `which` must be 0).  Adds to gz and gp[0..3] = (Om, OL, Or, H0).
-template <typename T, bool kT, bool kA>
-CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, const T g[6], T& gz, T gp[4]) {
+// kCond: also return in *cond the cancellation factor max_theta sum_j |G_j basis_j| / max(|dI0/dtheta|, 1e-3 |I0|) of the
+// chi-family gradient (status bit 16 of the ELEMENTWISE calls is derived from it).
+template <typename T, bool kT, bool kA, bool kCond = false>
+CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, const T g[6], T& gz, T gp[4], T* cond = nullptr) {
     using N = Num<T>;
     const T x = T(1) + z;
     const T iE = R.iE;
@@ -61,6 +63,12 @@ CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, c
 #pragma unroll
     for (int t = 0; t < 3; ++t) {
         T dI = C.GI[t][0] * R.I0 + C.GI[t][1] * R.K + C.GI[t][2] * bt0 + C.GI[t][3] * bt1 + C.GI[t][4] * bt2;
+        if (kCond) {
+            const T sa = N::abs_(C.GI[t][0] * R.I0) + N::abs_(C.GI[t][1] * R.K) + N::abs_(C.GI[t][2] * bt0) + N::abs_(C.GI[t][3] * bt1)
+                         + N::abs_(C.GI[t][4] * bt2);
+            const T c = sa / N::max_(N::abs_(dI), T(1e-3) * N::abs_(R.I0));
+            if (t == 0 || c > *cond) *cond = c;
+        }
         T acc = N::fma_(aI, T(-0.5) * dI, aK);
         if (kT) {
             T dT = C.GT[t][0] * R.I0 + C.GT[t][1] * R.K + C.GT[t][2] * bt0 + C.GT[t][3] * bt1 + C.GT[t][4] * bt2 + C.GT[t][5] * R.TT;

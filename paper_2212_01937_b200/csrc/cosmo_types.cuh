@@ -57,7 +57,10 @@ static const KTab KT_host = CB_KTAB_INIT;
 // `which` bits, planes in ascending bit order (include/cosmo_b200.h)
 enum : unsigned { W_DC = 1, W_DM = 2, W_DL = 4, W_MU = 8, W_TL = 16, W_DABS = 32, W_ALL = 63 };
 // status bits (include/cosmo_b200.h)
-enum : unsigned { ST_ROOT_ON_PATH = 1, ST_UNSUPPORTED = 2, ST_DL_NONPOS = 4, ST_ITER_CAP = 8 };
+enum : unsigned { ST_ROOT_ON_PATH = 1, ST_UNSUPPORTED = 2, ST_DL_NONPOS = 4, ST_ITER_CAP = 8, ST_GRAD_ILLCOND = 16 };
+// cancellation factor of the chi-family gradient above which 1e-8 is no longer guaranteed (calibrated against the oracle
+// on config 5: < 1e7 -> max error 4e-9)
+constexpr double GRAD_COND_LIMIT = 3.0e6;
 
 constexpr int NIT_CAP = 14;   // duplication steps never exceed this (status bit 8 when hit)
 

@@ -10,7 +10,7 @@ using namespace cb;
 
 template <typename T>
 static void run(int64_t n, const double* z, const double* Om, const double* OL, const double* Or, const double* H0,
-                unsigned which, const double* gup, double* out, double* gz, double* gp, uint8_t* status) {
+                unsigned which, const double* gup, double* out, double* gz, double* gp, uint8_t* status, double* cond_out = nullptr) {
     for (int64_t i = 0; i < n; ++i) {
         Cosmo<double> Cd;
         cosmo_prep(Om[i], OL[i], Or[i], H0[i], gup ? 2 : 0, Cd);
@@ -26,7 +26,9 @@ static void run(int64_t n, const double* z, const double* Om, const double* OL, 
         if (gup) {
             T g[6], a = 0, p[4] = {0, 0, 0, 0};
             for (int w = 0; w < 6; ++w) g[w] = (which >> w & 1) ? (T)gup[w * n + i] : T(0);
-            backward<T, true, true>(C, (T)z[i], R, O, g, a, p);
+            T cond = 0;
+            backward<T, true, true, true>(C, (T)z[i], R, O, g, a, p, &cond);
+            if (cond_out) cond_out[i] = (double)cond;
             gz[i] = (double)a;
             for (int t = 0; t < 4; ++t) gp[t * n + i] = (double)p[t];
         }
@@ -40,6 +42,10 @@ extern "C" void hostcheck_f64(int64_t n, const double* z, const double* Om, cons
 extern "C" void hostcheck_f32(int64_t n, const double* z, const double* Om, const double* OL, const double* Or, const double* H0,
                               unsigned which, const double* gup, double* out, double* gz, double* gp, uint8_t* status) {
     run<float>(n, z, Om, OL, Or, H0, which, gup, out, gz, gp, status);
+}
+extern "C" void hostcheck_f64_cond(int64_t n, const double* z, const double* Om, const double* OL, const double* Or, const double* H0,
+                                   unsigned which, const double* gup, double* out, double* gz, double* gp, uint8_t* status, double* cond) {
+    run<double>(n, z, Om, OL, Or, H0, which, gup, out, gz, gp, status, cond);
 }
 extern "C" void hostcheck_factor(double Om, double OL, double Or, double* out5) {
     Cosmo<double> C;

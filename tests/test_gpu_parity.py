@@ -265,12 +265,12 @@ def test_config5_forward_and_vjp(cb):
             assert np.mean(ae <= 2e-11 * np.maximum(scale[m], np.abs(ref[m]))) > 0.995, name
         else:
             assert np.mean(e[m] <= 3e-11) > 0.9, name
-    # gradients of the chi-family and t_L on the random block (near-degenerate blocks: documented limit)
+    # status bit 16 (gradient ill-conditioned: near-degenerate roots): rare on the random block, and
+    # every element WITHOUT it meets the gradient tolerance for the chi-family
+    assert np.mean((st[idx][rnd] & 16) != 0) < 0.02
     g = w.grad_out[:, 0, idx]
-    for k, name in enumerate(w.which):
-        pass
     mine = np.vstack([gz[idx][None], gp[:, idx]])
-    fin = np.isfinite(val).all(axis=1) & rnd
+    fin = np.isfinite(val).all(axis=1)
     ref = np.zeros((5, len(idx)))
     ref_abs = np.zeros((5, len(idx)))
     for k, name in enumerate(w.which):
@@ -279,8 +279,19 @@ def test_config5_forward_and_vjp(cb):
             ref[p] += np.where(np.isfinite(t), t, 0.0)
             ref_abs[p] += np.abs(np.where(np.isfinite(t), t, 0.0))
     for p in (0, 4):    # d/dz and d/dH0 are closed-form: tight everywhere finite
-        e = np.abs(mine[p] - ref[p])[fin] / ref_abs[p][fin]
+        e = np.abs(mine[p] - ref[p])[fin & rnd] / ref_abs[p][fin & rnd]
         assert e.max() <= 1e-9, (p, e.max())
+    # chi-family parameter gradients alone (one-hot upstream on D_C), all blocks, unflagged elements
+    g1 = np.zeros_like(w.grad_out)
+    g1[0] = 1.0
+    _, gp1, _, st1 = cb.cosmo_vjp(dev(w.z), dev(w.Om), dev(w.OL), dev(w.Or), dev(w.H0), dev(g1), cb.ELEMENTWISE, w.which)
+    gp1, st1 = gp1.cpu().numpy()[:, idx], st1.cpu().numpy()[0][idx]
+    okm = fin & ((st1 & 16) == 0)
+    assert okm.mean() > 0.6
+    for p in range(3):
+        r = grad[:, OBS["DC"], 1 + p]
+        e = np.abs(gp1[p] - r) / np.maximum(np.abs(r), 1e-3 * np.abs(val[:, OBS["DC"]]))
+        assert e[okm].max() <= TOL_GRAD, (p, e[okm].max())
 
 
 def test_empty_and_ragged(cb):
