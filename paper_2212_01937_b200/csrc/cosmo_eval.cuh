@@ -346,11 +346,45 @@ CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Cor
                 const T RJ0 = rj_series(p0[k], p0_0[k], sum0[k]);
                 const T q0 = p0_0[k] / ((T(1) - C.rn) * xmr);
                 const T s0q = N::fma_(C.Or, z2, q0);
-                const T t1 = N::sqrt_(xmr * q2x / lin) - N::sqrt_((T(1) - C.rn) * C.q21 / (C.Or + C.m));
+                // third-kind bracket of (3.9): 2 z B0 = int (x - rn) dx / E
+                const T B0 = N::fma_(z2 * T(CB_KT.third) * C.Q2n * C.mOrn, RJ0, rc<T>(s0q, q0));
+                // boundary term [sqrt((x-rn) Q2 / (Or x + m))] between 1 and x, with the factor z taken out analytically
+                const T Fx = N::sqrt_(xmr * q2x / lin);
+                const T c2 = C.b - C.rn, c1 = N::fma_(-C.rn, C.b, C.c);
+                const T dC = N::fma_(x, x + T(1), T(1)) + N::fma_(c2, x + T(1), c1);          // (C(x) - C(1)) / z
+                const T t1 = z[k] * (N::fma_(C.Or + C.m, dC, -C.C1 * C.Or)) / (lin * (C.Or + C.m) * (Fx + C.F1));
                 const T t2 = z[k] * C.aF * RF;
                 const T t3 = z[k] * C.WoOr * N::fma_(z2 * T(CB_KT.third) * C.Q2n, RD, bnd / N::sqrt_(lin * (C.Or + C.m)));
-                const T t4 = z[k] * C.sig * N::fma_(z2 * T(CB_KT.third) * C.Q2n * C.mOrn, RJ0, rc<T>(s0q, q0));
-                R[k].AA = (t1 + t2) + (t3 + t4);
+                const T t4 = z[k] * C.sig * B0;
+                const T A39 = (t1 + t2) + (t3 + t4);
+                // The R_D and R_J groups of (3.9) cancel by ~Om/(Or x).  Where radiation is a perturbation
+                // the same Carlson values are assembled without that cancellation: with
+                // u_j = int x^j dx/E, d(x^k E) gives  (k+3/2) Om u_{k+2} = [x^k E] - (k+2) Or u_{k+3} - (k+1) Ok u_{k+1}
+                // - k OL u_{k-1};  u_0 = I0 and u_1 = 2 z B0 + rn I0 are known, the Or terms are iterated (Gauss-Seidel).
+                constexpr int KS = 8;
+                T u[KS + 4], bk[KS + 1];
+                u[0] = R[k].I0;
+                u[1] = N::fma_(T(2) * z[k], B0, C.rn * R[k].I0);
+                {
+                    T xk = T(1);
+#pragma unroll
+                    for (int j = 0; j <= KS; ++j) { bk[j] = N::fma_(xk - T(1), R[k].E, R[k].Em1); xk *= x; }
+#pragma unroll
+                    for (int j = 2; j < KS + 4; ++j) u[j] = T(0);
+                }
+                T prev = T(0);
+#pragma unroll
+                for (int sw = 0; sw < KS; ++sw) {
+                    if (sw == KS - 1) prev = u[2];
+#pragma unroll
+                    for (int j = 0; j <= KS - sw; ++j) {
+                        T acc = bk[j] - T(j + 2) * C.Or * u[j + 3] - T(j + 1) * C.Ok * u[j + 1];
+                        if (j >= 1) acc -= T(j) * C.OL * u[j - 1];
+                        u[j + 2] = acc * C.iOm * T(1.0 / (j + 1.5));
+                    }
+                }
+                const bool conv = N::abs_(u[2] - prev) <= T(sizeof(T) == 8 ? 1e-14 : 1e-6) * N::abs_(u[2]);
+                R[k].AA = conv ? u[2] : A39;
             } else {
                 // eq. (B.3) with i = rn
                 R[k].AA = T(CB_KT.two_thirds) * z[k] * (R[k].Em1 / (C.m * z[k]) + C.aF * RF

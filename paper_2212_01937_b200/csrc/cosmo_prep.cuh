@@ -164,6 +164,9 @@ CB_HD void cosmo_prep(double Om, double OL, double Or, double H0, int want_grad,
     // absorption distance constants
     C.Q2n = fma(rn + b, rn, c);
     C.mOrn = D1r;
+    C.C1 = (1.0 - rn) * C.q21;
+    C.F1 = sqrt(C.C1 / (Or + m));
+    C.iOm = 1.0 / Om;
     if (C.cubic) {
         C.aF = 3.0 * rn * rn - C.Q2n;
         C.sig = -Ok / Om;                 // sum of the three roots

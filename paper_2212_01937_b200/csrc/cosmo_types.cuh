@@ -82,7 +82,7 @@ struct Cosmo {
     // lookback time, eq. (3.8) with i = big root, j = rn
     T p5c, Gp, qhc, OrM;
     // absorption distance, eq. (3.9) with (i,j,k,l) = (rn, pair, pair, big); (B.3) when Or = 0
-    T Q2n, aF, WoOr, sig, mOrn;
+    T Q2n, aF, WoOr, sig, mOrn, C1, F1, iOm;   // C1 = (1-rn) Q2(1), F1 = sqrt(C1/(Or+m)), iOm = 1/Om
     // gradient basis coefficients: dX/dtheta = -1/2 sum_j G[theta][j] basis_j
     T GI[3][5];        // X = I0 : basis (I0, K, b0, b1, b2)
     T GT[3][6];        // X = T  : basis (I0, K, b0, b1, b2, T)
@@ -91,7 +91,7 @@ struct Cosmo {
     unsigned cubic;    // Or == 0
 };
 
-constexpr int COSMO_NFIELDS = 83;   // floating-point members of Cosmo<T>, in declaration order
+constexpr int COSMO_NFIELDS = 86;   // floating-point members of Cosmo<T>, in declaration order
 static_assert(sizeof(Cosmo<double>) == COSMO_NFIELDS * sizeof(double) + 2 * sizeof(unsigned), "Cosmo<T> layout");
 static_assert(sizeof(Cosmo<float>) == COSMO_NFIELDS * sizeof(float) + 2 * sizeof(unsigned), "Cosmo<T> layout");
 

@@ -97,7 +97,7 @@ def test_host_math_matches_oracle(hc, cfg):
     val, grad = val.astype(np.float64), grad.astype(np.float64)
     for i, name in enumerate(oracle.OBS):
         e = np.abs(out[i] - val[:, i]) / np.abs(val[:, i])
-        tol = 1e-11 if name != "DABS" else 4e-11
+        tol = 1e-11
         assert e.max() <= tol, (name, e.max())
         if name != "DABS":
             assert e.max() <= 5e-15, (name, e.max())
@@ -116,13 +116,13 @@ def test_dabs_gradient_documented_limit(hc):
     _, gz, gp, _ = run(hc, w.z, w.Om, w.OL, w.Or, w.H0, 63, g1)
     val, grad, _ = oracle.observables_batch(w.z, w.Om, w.OL, w.Or, w.H0, with_grad=True)
     val, grad = val.astype(np.float64), grad.astype(np.float64)
-    for p, tol in ((1, 5e-8), (2, 1e-9)):
+    for p, tol in ((1, 1e-8), (2, 1e-9)):
         ref = grad[:, 5, p]
         e = np.abs(gp[p - 1] - ref) / np.maximum(np.abs(ref), 1e-3 * np.abs(val[:, 5]))
         assert e.max() <= tol, (p, e.max())
     ref = grad[:, 5, 3]
     e = np.abs(gp[2] - ref) / np.maximum(np.abs(ref), 1e-3 * np.abs(val[:, 5]))
-    assert np.isfinite(e).all() and e.max() <= 1e-2
+    assert np.isfinite(e).all() and e.max() <= 1e-5
 
 
 def test_host_math_stress_blocks(hc):
