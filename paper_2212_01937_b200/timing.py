@@ -1,0 +1,115 @@
+"""Times the C-ABI calls on the five BASELINE.json configs (seeded synthetic inputs, device-resident, CUDA events).
+
+    python -m paper_2212_01937_b200.timing [--steps 10] [--small]
+
+One JSON line per config: evals/s of the whole call and the mean duration of its dominant kernel (library hook).
+bench.py stays the headline (config 3); this is the per-config table quoted in DESIGN.md / profiles/.
+"""
+import argparse
+import json
+
+import numpy as np
+
+
+def main():
+    import torch
+    from . import binding as cb, workloads as W
+
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--small", action="store_true", help="1/10 of the sizes (smoke)")
+    ap.add_argument("--only", default="")
+    args = ap.parse_args()
+    f = 10 if args.small else 1
+    dev = lambda a, dt=None: (torch.from_numpy(np.ascontiguousarray(a)).cuda() if dt is None
+                              else torch.from_numpy(np.ascontiguousarray(a)).cuda().to(dt))
+    rng = np.random.default_rng(0)
+
+    def timed(fn, evals, name, extra=None):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        cb.profile(True)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        k_ms, k_n = cb.profile_mean_ms()
+        cb.profile(False)
+        e0.record()
+        for _ in range(args.steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / args.steps
+        line = {"config": name, "evals_per_call": int(evals), "ms_per_call": ms, "evals_per_s": evals / (ms * 1e-3),
+                "dominant_kernel_ms": k_ms}
+        line.update(extra or {})
+        print(json.dumps(line), flush=True)
+
+    def want(name):
+        return not args.only or name in args.only.split(",")
+
+    if want("config1"):
+        w = W.config1()
+        a = [dev(x) for x in (w.z, w.Om, w.OL, w.Or, w.H0)]
+        timed(lambda: cb.cosmo_eval(*a, cb.ELEMENTWISE, w.which), w.n_z, "config1 fwd D_C,mu N=1e4 one cosmology f64")
+    if want("config2"):
+        w = W.config2(n=1_000_000 // f)
+        a = [dev(x) for x in (w.z, w.Om, w.OL, w.Or, w.H0)]
+        out = torch.empty((4, 1, w.n_z), dtype=torch.float64, device="cuda")
+        st = torch.empty((1, w.n_z), dtype=torch.uint8, device="cuda")
+        timed(lambda: cb.cosmo_eval(*a, cb.ELEMENTWISE, w.which, out=out, status=st), w.n_z,
+              "config2 fwd D_C,D_M,t_L,d_abs per-element cosmology f64")
+        timed(lambda: cb.cosmo_eval(*a, cb.ELEMENTWISE, ("DC", "DM"), out=out[:2], status=st), w.n_z,
+              "config2 fwd D_C,D_M only per-element cosmology f64")
+    if want("config3"):
+        w = W.config3(n=1_000_000 // f)
+        a = [dev(x) for x in (w.z, w.Om, w.OL, w.Or, w.H0)]
+        g = dev(w.grad_out)
+        S, N = w.n_cosmo, w.n_z
+        out = torch.empty((1, S, N), dtype=torch.float64, device="cuda")
+        gz = torch.empty(N, dtype=torch.float64, device="cuda")
+        gp = torch.empty((4, S), dtype=torch.float64, device="cuda")
+        st = torch.empty((S, N), dtype=torch.uint8, device="cuda")
+        ws = torch.empty(cb.workspace_bytes(N, S, cb.OUTER, w.which, True), dtype=torch.uint8, device="cuda")
+        timed(lambda: cb.cosmo_vjp(*a, g, cb.OUTER, w.which, out=out, grad_z=gz, grad_params=gp, status=st, workspace=ws), S * N,
+              "config3 fwd+VJP mu OUTER f64")
+        timed(lambda: cb.cosmo_eval(*a, cb.OUTER, w.which, out=out, status=st, workspace=ws), S * N, "config3 fwd only mu OUTER f64")
+        a32 = [dev(w.z, torch.float32)] + a[1:]
+        g32, out32, gz32 = g.to(torch.float32), out.to(torch.float32), gz.to(torch.float32)
+        timed(lambda: cb.cosmo_vjp(*a32, g32, cb.OUTER, w.which, out=out32, grad_z=gz32, grad_params=gp, status=st, workspace=ws), S * N,
+              "config3 fwd+VJP mu OUTER f32")
+    if want("config4"):
+        n = 1_000_000 // f
+        z = rng.uniform(0.01, 1.5, n)
+        one = lambda v: dev(np.array([v]))
+        mu, _ = cb.cosmo_eval(dev(z), one(0.3), one(0.7), one(0.0), one(70.0), cb.ELEMENTWISE, ("MU",))   # timing only: any mu source does
+        w = W.config4(lambda zz, *p: mu[0, 0].cpu().numpy(), n=n, S=256, seed=4)
+        a = [dev(x) for x in (z, w.extra["mu_obs"], w.extra["sigma"], w.Om, w.OL, w.Or, w.H0)]
+        logL = torch.empty(256, dtype=torch.float64, device="cuda")
+        grad = torch.empty((4, 256), dtype=torch.float64, device="cuda")
+        ws = torch.empty(cb.workspace_bytes(n, 256, cb.OUTER, ("MU",), True), dtype=torch.uint8, device="cuda")
+        timed(lambda: cb.cosmo_snia_loglike(*a, logL=logL, grad=grad, workspace=ws), 256 * n, "config4 fused SN-Ia logL + grad S=256 f64")
+    if want("config5"):
+        w = W.config5(n=10_000_000 // f, n_struct=100_000 // f)
+        a = [dev(x) for x in (w.z, w.Om, w.OL, w.Or, w.H0)]
+        N = w.n_z
+        g = torch.randn((6, 1, N), dtype=torch.float64, device="cuda")
+        out = torch.empty((6, 1, N), dtype=torch.float64, device="cuda")
+        gz = torch.empty(N, dtype=torch.float64, device="cuda")
+        gp = torch.empty((4, N), dtype=torch.float64, device="cuda")
+        st = torch.empty((1, N), dtype=torch.uint8, device="cuda")
+        timed(lambda: cb.cosmo_vjp(*a, g, cb.ELEMENTWISE, w.which, out=out, grad_z=gz, grad_params=gp, status=st), N,
+              "config5 fwd+VJP all six outputs per-element cosmology f64")
+        timed(lambda: cb.cosmo_eval(*a, cb.ELEMENTWISE, w.which, out=out, status=st), N, "config5 fwd all six outputs f64")
+        a32 = [dev(w.z, torch.float32)] + a[1:]
+        g32, out32, gz32 = g.to(torch.float32), out.to(torch.float32), gz.to(torch.float32)
+        timed(lambda: cb.cosmo_vjp(*a32, g32, cb.ELEMENTWISE, w.which, out=out32, grad_z=gz32, grad_params=gp, status=st), N,
+              "config5 fwd+VJP all six outputs f32")
+
+
+if __name__ == "__main__":
+    main()
