@@ -93,7 +93,7 @@ struct OuterArgs {
 
 // OUTER forward / fused forward+VJP / fused likelihood.  grid = (tiles of TILE redshifts, S-chunk groups).
 #ifndef CB_MINBLOCKS
-#define CB_MINBLOCKS 5     // chi-family kernels: 96 registers, 20 warps/SM (measured best, profiles/)
+#define CB_MINBLOCKS 4     // chi-family kernels: 128 registers, 16 warps/SM (measured best, profiles/)
 #endif
 template <typename T, bool kT, bool kA, int MODE, unsigned WCT>
 __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) k_outer(OuterArgs a) {
