@@ -33,6 +33,21 @@ __device__ __forceinline__ double warp_sum(double v) {
     return v;
 }
 
+// Sum of four values over the warp with 6 shuffles instead of 20: the exchange halves the number of values a lane
+// carries at each of the first two steps.  On return the lanes 0, 8, 16, 24 hold the totals of v[0], v[1], v[2], v[3].
+__device__ __forceinline__ double warp_sum4(const double (&v)[4], int lane) {
+    const bool hi = lane & 16;
+    double a = hi ? v[2] : v[0], b = hi ? v[3] : v[1];
+    a += __shfl_xor_sync(0xffffffffu, hi ? v[0] : v[2], 16);
+    b += __shfl_xor_sync(0xffffffffu, hi ? v[1] : v[3], 16);
+    const bool h3 = lane & 8;
+    double k = h3 ? b : a;
+    k += __shfl_xor_sync(0xffffffffu, h3 ? a : b, 8);
+#pragma unroll
+    for (int off = 4; off > 0; off >>= 1) k += __shfl_xor_sync(0xffffffffu, k, off);
+    return k;
+}
+
 // S1-S3, one thread per cosmology
 __global__ void k_prep(const double* __restrict__ Om, const double* __restrict__ OL, const double* __restrict__ Or,
                        const double* __restrict__ H0, int64_t S, int want_grad, Cosmo<double>* __restrict__ out) {
@@ -209,10 +224,12 @@ __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) 
                     if (live[k]) a.status[row * N + n0 + k] = stv[k];
             }
             if (kG) {
-#pragma unroll
-                for (int j = 0; j < NP; ++j) {
-                    double v = warp_sum((double)pacc[j]);
-                    if (lane == 0) sacc[warp][sl][j] = v;
+                const double v4[4] = {(double)pacc[NP - 4], (double)pacc[NP - 3], (double)pacc[NP - 2], (double)pacc[NP - 1]};
+                const double tot = warp_sum4(v4, lane);
+                if ((lane & 7) == 0) sacc[warp][sl][NP - 4 + (lane >> 3)] = tot;
+                if (NP == 5) {
+                    const double l = warp_sum((double)pacc[0]);
+                    if (lane == 0) sacc[warp][sl][0] = l;
                 }
             }
         }
