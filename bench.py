@@ -84,7 +84,7 @@ def run_reference(args):
 
 # ------------------------------------------------------------------------------------------ clocks
 class ClockSampler(threading.Thread):
-    def __init__(self, index=0, period=0.02):
+    def __init__(self, index=0, period=0.005):
         super().__init__(daemon=True)
         self.period, self.samples, self.reasons, self.stop_flag = period, [], set(), False
         self.max_mhz = None
@@ -247,7 +247,12 @@ def run_ours(args):
     achieved = fpe * evals / (k_ms * 1e-3) / 1e12 if k_ms > 0 else None
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": (achieved / peak_tflops) if (achieved and peak_tflops) else None,
-                "traffic": None, "kernel": "k_outer<double,false,false,VJP>", "kernel_ms": k_ms, "kernel_launches_timed": k_n,
+                "traffic": RL.DRAM_TRAFFIC_BYTES_PER_LAUNCH["config3_vjp_mu_f64"] if (N, S) == (1_000_000, 64) else None,
+                "traffic_unit": "bytes/launch (ncu dram read+write, profiles/r01_final_k_outer_vjp.md)",
+                "algorithmic_bytes": RL.BYTES_PER_EVAL_C3 * evals,
+                "fp64_pipe_frac": (RL.FP64_PIPE_INST_PER_EVAL["config3_vjp_mu_f64"] * evals / (k_ms * 1e-3)) / (peak_tflops * 0.5e12)
+                if (k_ms > 0 and peak_tflops) else None,
+                "kernel": "k_outer<double,false,false,VJP,MU>", "kernel_ms": k_ms, "kernel_launches_timed": k_n,
                 "flops_per_eval": fpe, "peak_source": "measured live: cosmo_probe_fma_f64 (8 DFMA chains/thread)",
                 "nominal_fp64_tflops": RL.NOMINAL_FP64_TFLOPS,
                 "hbm_gbs_achieved": RL.BYTES_PER_EVAL_C3 * evals / (k_ms * 1e-3) / 1e9 if k_ms > 0 else None}

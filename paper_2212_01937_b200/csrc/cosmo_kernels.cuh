@@ -99,7 +99,7 @@ struct OuterArgs {
     const void* z; const void* gout; const void* mu_obs; const void* sigma;
     void* out; void* gz; uint8_t* status;
     const Cosmo<double>* consts;
-    double* part;            // [ntiles][S][NP] partial parameter sums (NP = 4 vjp, 5 snia)
+    double* part;            // [S][NP][ntiles] partial parameter sums (NP = 4 vjp, 5 snia)
     int64_t N, S;
     unsigned which;
     int gz_accumulate;       // gridDim.y > 1: gz holds [gridDim.y][N] partials
@@ -240,7 +240,7 @@ __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) 
                 double v = 0.0;
 #pragma unroll
                 for (int w = 0; w < NWARP; ++w) v += sacc[w][sl][j];
-                a.part[((int64_t)blockIdx.x * S + (c0 + sl)) * NP + j] = v;
+                a.part[((c0 + sl) * NP + j) * (int64_t)gridDim.x + blockIdx.x] = v;    // [S][NP][ntiles]: the reduction reads contiguously
             }
         }
     }
@@ -250,7 +250,7 @@ __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) 
     }
 }
 
-// partial parameter sums [ntiles][S][NP] -> dst planes: dst_first[S] (snia logL) and dst_grad[4][S]; fixed order => deterministic
+// partial parameter sums [S][NP][ntiles] -> dst planes: dst_first[S] (snia logL) and dst_grad[4][S]; fixed order => deterministic
 template <int NP>
 __global__ void k_reduce_params(const double* __restrict__ part, int64_t ntiles, int64_t S, double* __restrict__ logL,
                                 double* __restrict__ grad) {
@@ -261,7 +261,8 @@ __global__ void k_reduce_params(const double* __restrict__ part, int64_t ntiles,
     const int64_t s = wid / NP;
     const int j = (int)(wid - s * NP);
     double v = 0.0;
-    for (int64_t t = lane; t < ntiles; t += 32) v += part[(t * S + s) * NP + j];
+    const double* __restrict__ row = part + (s * NP + j) * ntiles;
+    for (int64_t t = lane; t < ntiles; t += 32) v += row[t];
     v = warp_sum(v);
     if (lane == 0) {
         if (NP == 5) {

@@ -8,9 +8,20 @@ DESIGN.md "Roofline" the derivation).  `peak` = the DFMA rate bench.py measures 
 probe (cosmo_probe_fma_f64); the nominal figure beside it is 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz.
 """
 
-# FP64 flops per eval of the config-3 fused forward+VJP kernel k_outer<double,0,0,VJP> (ncu, profiles/r01_*.md)
+# FP64 work per eval of the config-3 fused forward+VJP kernel k_outer<double,false,false,VJP,MU> as committed, from the
+# ncu capture profiles/r01_final_k_outer_vjp.md (6.4e7 evals/launch):
+#   DFMA 138.8, DMUL 115.0, DADD 32.6 thread-instructions per eval -> 2*138.8 + 115.0 + 32.6 = 425.2 flops
+#   FP64-pipe instructions per eval (the above + 9.3 DSETP) = 295.7
+# (first working version, profiles/r01_k_outer_vjp.md: 774.8 flops, 513.7 pipe instructions per eval)
 FLOPS_PER_EVAL = {
-    "config3_vjp_mu_f64": 774.8,   # r01 capture: 2*273.8 DFMA + 169.1 DMUL + 58.1 DADD per eval (profiles/r01_k_outer_vjp.md)
+    "config3_vjp_mu_f64": 425.2,
+}
+FP64_PIPE_INST_PER_EVAL = {
+    "config3_vjp_mu_f64": 295.7,
+}
+# dram__bytes_read.sum + dram__bytes_write.sum of that kernel, per launch (same capture)
+DRAM_TRAFFIC_BYTES_PER_LAUNCH = {
+    "config3_vjp_mu_f64": 544.09e6 + 570.56e6,
 }
 
 # nominal B200 FP64 vector peak (context only; the denominator is the measured probe)
