@@ -2,7 +2,7 @@
 //
 // Layout in HBM: SoA everywhere; z[N]; parameters Om/OL/Or/H0[S]; outputs and upstream
 // gradients as planes [plane][row][N] with N fastest, so that a warp reads/writes 512 contiguous bytes per plane row
-// (two consecutive elements per thread, 128-bit accesses in FP64).  Per-cosmology constants (82 numbers) are
+// (two consecutive elements per thread, 128-bit accesses in FP64).  Per-cosmology constants (86 numbers) are
 // computed once by k_prep and staged in shared memory by the OUTER kernels, one block = one tile of redshifts
 // looping over a chunk of cosmologies, so the only per-eval HBM traffic is grad_out (8 B) and, if asked, out.
 #pragma once
