@@ -21,12 +21,14 @@
  *     launch failed (COSMO_E_CUDA; cosmo_last_cuda_error() gives the cudaError_t);
  *   - per-element domain problems never abort: the element's outputs are NaN and its status byte carries
  *       1  a root of E^2 lies on (0, z] (no-Big-Bang region)
- *       2  unsupported input: Om <= 0, Or < 0, OL < 0, H0 <= 0, z <= -1, non-finite, or no two real negative roots
- *          (the method needs E^2 of degree 3 or 4)
+ *       2  unsupported input: Om <= 0, Or < 0, OL < 0, H0 <= 0, z <= -1, non-finite, or a root structure that could not be
+ *          factorised (the method needs E^2 of degree 3 or 4)
  *       4  D_L <= 0 (closed universe at/after the antipode): mu is NaN, the other outputs are valid
  *       8  the duplication loop hit its iteration cap before Carlson's stopping rule was met
- *      16  gradient ill-conditioned (near-degenerate roots; the 1/prod(r_j - r_k) of PAPER.md:320-345): values valid,
- *          gradients may have lost more than the documented accuracy (elementwise calls only)
+ *      16  gradient ill-conditioned (near-degenerate roots; the 1/prod(r_j - r_k) of PAPER.md:320-345) or not available
+ *          (E^2 without a real negative root: values by the complex slow path, gradients NaN): values valid, gradients
+ *          may have lost more than the documented accuracy (set by the VJP calls; the conditioning estimate is per element
+ *          in ELEMENTWISE calls only)
  */
 #ifndef COSMO_B200_H
 #define COSMO_B200_H

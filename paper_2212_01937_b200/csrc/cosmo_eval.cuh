@@ -165,7 +165,7 @@ CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Cor
     T U12[K], ra[K], iE[K], xa[K], mp[K], s[K], Qc[K];
     unsigned st[K];
     T p5[K], p0[K], dl5[K], dl0[K], p5_0[K], p0_0[K], Q5v[K], Q0v[K];
-    const bool quartA = kA && !C.cubic;
+    const bool quartA = kA && !(C.cubic & 1u);
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         const T x = T(1) + z[k];

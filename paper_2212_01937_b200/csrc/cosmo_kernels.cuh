@@ -106,6 +106,50 @@ struct OuterArgs {
     int vec;                 // N even and pointers 16-byte aligned
 };
 
+// One cosmology row of the OUTER kernels whose E^2 has no real negative root (Cosmo::cubic bit 1): complex slow path,
+// forward values only.  Never inlined and called at the top of the per-cosmology iteration, where almost nothing is live,
+// so that this rare case costs the hot loop no registers.  Parameter gradients of the row and its contribution to grad_z
+// are NaN ("not available", status bit 16); the likelihood value itself is valid.
+template <typename T, bool kT, bool kA, int MODE>
+__device__ __noinline__ void outer_c4_row(const OuterArgs& a, const Cosmo<T>& C, int64_t row, int64_t n0, const T* zv, const T* mo,
+                                          const T* isig2, const T* lnorm, unsigned which, double* sacc_row, int lane, T* gzacc) {
+    constexpr int NP = MODE == MODE_SNIA ? 5 : 4;
+    const int64_t N = a.N, S = a.S;
+    T ll = T(0);
+    for (int k = 0; k < KZ; ++k) {
+        const bool live = n0 + k < N;
+        Core<T> R;
+        R.I0 = R.TT = R.AA = R.K = R.E = R.iE = R.Em1 = T(0);
+        R.status = C.status;
+        apply_c4<T, kT, kA, MODE != MODE_FWD>(C, zv[k], R);
+        Obs<T> O;
+        observables<T, kT, kA>(C, zv[k], R, which, O);
+        if (MODE == MODE_SNIA) {
+            const T resid = mo[k] - O.v[3];
+            if (live) ll += Num<T>::fma_(T(-0.5) * resid, resid * isig2[k], lnorm[k]);
+        } else if (live) {
+            if (a.out != nullptr) {
+                int pl = 0;
+                for (int w = 0; w < 6; ++w) {
+                    if (!(which >> w & 1)) continue;
+                    static_cast<T*>(a.out)[((int64_t)pl * S + row) * N + n0 + k] = O.v[w];
+                    ++pl;
+                }
+            }
+            if (a.status != nullptr) a.status[row * N + n0 + k] = (uint8_t)O.status;
+        }
+        if (MODE == MODE_VJP) gzacc[k] = T(NAN);
+    }
+    if (MODE != MODE_FWD) {
+        if (MODE == MODE_SNIA) {
+            const double l = warp_sum((double)ll);
+            if (lane == 0) sacc_row[0] = l;
+        }
+        if (lane == 0)
+            for (int j = NP - 4; j < NP; ++j) sacc_row[j] = NAN;
+    }
+}
+
 // OUTER forward / fused forward+VJP / fused likelihood.  grid = (tiles of TILE redshifts, S-chunk groups).
 #ifndef CB_MINBLOCKS
 #define CB_MINBLOCKS 4     // chi-family kernels: 128 registers, 16 warps/SM (measured best, profiles/)
@@ -158,6 +202,11 @@ __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) 
         for (int sl = 0; sl < ns; ++sl) {
             const Cosmo<T>& C = sc[sl];
             const int64_t row = c0 + sl;
+            if (C.cubic & 2u) {
+                outer_c4_row<T, kT, kA, MODE>(a, C, row, n0, zv, mo, isig2, lnorm, MODE == MODE_SNIA ? (unsigned)W_MU : which,
+                                              kG ? &sacc[warp][sl][0] : nullptr, lane, gzacc);
+                continue;
+            }
             T pacc[NP];
 #pragma unroll
             for (int j = 0; j < NP; ++j) pacc[j] = T(0);
@@ -303,6 +352,7 @@ __global__ void __launch_bounds__(ELEM_THREADS) k_elem(const T* __restrict__ z, 
     Core<T> R;
     R.K = T(0); R.TT = T(0); R.AA = T(0);
     eval_core<T, kT, kA, kG, VoteWarp>(C, zv, VoteWarp(), R);
+    apply_c4<T, kT, kA, kG>(C, zv, R);
     Obs<T> O;
     observables<T, kT, kA>(C, zv, R, which, O);
     if (!live) return;

@@ -7,6 +7,7 @@
 //     eqs. (2.10)-(2.12) + appendix A, by their closed combination).
 #pragma once
 #include "cosmo_eval.cuh"
+#include "cosmo_c4.cuh"
 
 namespace cb {
 
@@ -16,6 +17,18 @@ struct Obs {
     T F, Fi, Fk;       // curvature transform and its partials
     unsigned status;
 };
+
+// Rows whose E^2 has no real negative root (Cosmo::cubic bit 1): replace the fused real path's result by the complex
+// slow path (cosmo_c4.cuh).  Forward values only: K, 1/E are poisoned so that every gradient of such a row is NaN.
+template <typename T, bool kT, bool kA, bool kGrad>
+CB_HD void apply_c4(const Cosmo<T>& C, T z, Core<T>& R) {
+    if (!(C.cubic & 2u)) return;
+    double I0, TT, AA;
+    eval_c4((double)C.Or, (double)C.m, (double)C.rn, (double)C.b, (double)C.c, (double)z, kT, kA, I0, TT, AA);
+    R.I0 = (T)I0; R.TT = (T)TT; R.AA = (T)AA;
+    R.K = T(NAN); R.iE = T(NAN);
+    R.status = C.status | ((T(1) + z > T(0)) ? 0u : (unsigned)ST_UNSUPPORTED) | (kGrad ? (unsigned)ST_GRAD_ILLCOND : 0u);
+}
 
 template <typename T, bool kT, bool kA>
 CB_HD void observables(const Cosmo<T>& C, T z, const Core<T>& R, unsigned which, Obs<T>& O) {
@@ -59,7 +72,7 @@ CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, c
     const T aI = C.dH * N::fma_(gM, O.Fi, g[0]);
     const T aK = -gM * C.dH * O.Fk;
     T btA = T(0);
-    if (kA) btA = ((C.cubic ? n4 : n3) - R.Em1) * iE;
+    if (kA) btA = (((C.cubic & 1u) ? n4 : n3) - R.Em1) * iE;
 #pragma unroll
     for (int t = 0; t < 3; ++t) {
         T dI = C.GI[t][0] * R.I0 + C.GI[t][1] * R.K + C.GI[t][2] * bt0 + C.GI[t][3] * bt1 + C.GI[t][4] * bt2;

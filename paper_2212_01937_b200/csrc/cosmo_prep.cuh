@@ -136,6 +136,29 @@ CB_HD void cosmo_prep(double Om, double OL, double Or, double H0, int want_grad,
         double res = fabs(e3 - Om) + fabs(e2 - Ok) + fabs(e1) + fabs(e0 - OL);
         if (!(res <= 1e-9 * scale) || !(m > 0.0) || !(rn <= 1e-12)) st |= ST_UNSUPPORTED;   // also catches NaN
     }
+    // --- no real negative root (two complex pairs): factor P = (Or x^2 + g1 x + h1)(x^2 + b x + c) by Bairstow from the
+    // small pair x^2 ~ -OL/Ok; such rows are evaluated by the complex slow path of cosmo_c4.cuh (C.m, C.rn carry g1, h1)
+    if ((st & ST_UNSUPPORTED) && Or > 0.0 && Om > 0.0 && OL >= 0.0 && H0 > 0.0 && Ok > 0.0 && isfinite(Ok)) {
+        double bb = 0.0, cc = OL / Ok;
+        for (int it = 0; it < 12; ++it) {
+            double q2 = Or, q1 = Om - bb * q2, q0 = Ok - bb * q1 - cc * q2;
+            double r1 = -bb * q0 - cc * q1, r0 = OL - cc * q0;
+            double s1 = q1 - bb * q2, s0 = q0 - cc * q2;
+            double u1 = s0 - bb * s1, u0 = -cc * s1;
+            double det = u1 * s0 - u0 * s1;
+            if (det == 0.0 || !isfinite(det)) break;
+            bb += (r1 * s0 - r0 * s1) / det;
+            cc += (u1 * r0 - u0 * r1) / det;
+        }
+        const double g1 = Om - bb * Or, h1 = Ok - bb * g1 - cc * Or;
+        const double e1 = g1 * cc + h1 * bb, e0 = h1 * cc;
+        const double scale = fabs(Om) + fabs(Ok) + fabs(OL) + fabs(Or);
+        if (fabs(e1) + fabs(e0 - OL) <= 1e-9 * scale && 4.0 * Or * h1 - g1 * g1 > 0.0 && 4.0 * cc - bb * bb > 0.0) {
+            st &= ~ST_UNSUPPORTED;
+            C.cubic |= 2u;
+            m = g1; rn = h1; b = bb; c = cc;
+        }
+    }
     C.m = m; C.rn = rn; C.b = b; C.c = c;
     // --- per-cosmology constants (S3)
     const double f1 = Or, g1 = m - Or * rn, h1 = -m * rn;
@@ -167,7 +190,7 @@ CB_HD void cosmo_prep(double Om, double OL, double Or, double H0, int want_grad,
     C.C1 = (1.0 - rn) * C.q21;
     C.F1 = sqrt(C.C1 / (Or + m));
     C.iOm = 1.0 / Om;
-    if (C.cubic) {
+    if (C.cubic & 1u) {
         C.aF = 3.0 * rn * rn - C.Q2n;
         C.sig = -Ok / Om;                 // sum of the three roots
         C.WoOr = 0.0;
@@ -209,7 +232,7 @@ CB_HD void cosmo_prep(double Om, double OL, double Or, double H0, int want_grad,
         double M[7][7 + 3];
         for (int r = 0; r < 7; ++r) for (int k = 0; k < 10; ++k) M[r][k] = 0.0;
         for (int p = 0; p < 5; ++p) { M[p][0] = e[p]; M[p][1] = NK[p]; M[p + 2][6] = e[p]; }
-        add_Nk(M, 2, 0, e); add_Nk(M, 3, 1, e); add_Nk(M, 4, 2, e); add_Nk(M, 5, C.cubic ? 4 : 3, e);
+        add_Nk(M, 2, 0, e); add_Nk(M, 3, 1, e); add_Nk(M, 4, 2, e); add_Nk(M, 5, (C.cubic & 1u) ? 4 : 3, e);
         M[5][7] = 1.0; M[4][7] = -1.0;
         M[2][8] = 1.0; M[4][8] = -1.0;
         M[6][9] = 1.0; M[4][9] = -1.0;

@@ -10,8 +10,10 @@
 
 #ifdef __CUDACC__
 #define CB_HD __host__ __device__ __forceinline__
+#define CB_HD_NOINLINE __host__ __device__ __noinline__
 #else
 #define CB_HD inline
+#define CB_HD_NOINLINE inline
 #endif
 
 namespace cb {
@@ -88,7 +90,7 @@ struct Cosmo {
     T GT[3][6];        // X = T  : basis (I0, K, b0, b1, b2, T)
     T GA[3][7];        // X = A  : basis (I0, K, b0, b1, b2, b3 (b4 when Or = 0), A)
     unsigned status;
-    unsigned cubic;    // Or == 0
+    unsigned cubic;    // bit 0: Or == 0 (cubic case, appendix B.1);  bit 1: two complex pairs (cosmo_c4.cuh; m, rn hold g1, h1)
 };
 
 constexpr int COSMO_NFIELDS = 86;   // floating-point members of Cosmo<T>, in declaration order

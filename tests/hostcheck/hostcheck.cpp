@@ -19,6 +19,7 @@ static void run(int64_t n, const double* z, const double* Om, const double* OL, 
         Core<T> R;
         R.K = 0; R.TT = 0; R.AA = 0;
         eval_core<T, true, true, true, VoteNone>(C, (T)z[i], VoteNone(), R);
+        if (gup) apply_c4<T, true, true, true>(C, (T)z[i], R); else apply_c4<T, true, true, false>(C, (T)z[i], R);
         Obs<T> O;
         observables<T, true, true>(C, (T)z[i], R, which, O);
         for (int w = 0; w < 6; ++w) out[w * n + i] = (double)O.v[w];
