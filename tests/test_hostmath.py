@@ -137,6 +137,26 @@ def test_host_math_stress_blocks(hc):
         assert e.max() <= tol and np.mean(e <= 1e-11) > 0.995, (i, e.max())
 
 
+def test_two_complex_pairs_slow_path(hc):
+    """E^2 without a real negative root (Om^2 < 4 Or Ok): eqs. (3.8)/(3.9) with a complex r_i (cosmo_c4.cuh) against the oracle"""
+    rng = np.random.default_rng(7)
+    n = 60
+    Om = rng.uniform(0.050, 0.056, n); Or = rng.uniform(9.3e-4, 1e-3, n); OL = rng.uniform(0.0, 0.12, n)
+    z = rng.uniform(0.001, 5.0, n); H0 = rng.uniform(60, 80, n)
+    for i in range(n):   # every row really has no real negative root
+        r = np.roots([Or[i], Om[i], 1 - Om[i] - OL[i] - Or[i], 0.0, OL[i]])
+        assert not np.any((np.abs(r.imag) < 1e-9 * np.abs(r)) & (r.real < 0))
+    out, _, _, st = run(hc, z, Om, OL, Or, H0)
+    assert (st == 0).all()
+    val, _, sto = oracle.observables_batch(z, Om, OL, Or, H0, with_grad=False)
+    val = val.astype(np.float64)
+    for i, tol in ((0, 1e-14), (1, 1e-14), (3, 1e-14), (4, 1e-14), (5, 1e-11)):
+        assert (np.abs(out[i] - val[:, i]) / np.abs(val[:, i])).max() <= tol, i
+    g1 = np.zeros((6, n)); g1[0] = 1
+    _, gz, gp, st = run(hc, z, Om, OL, Or, H0, 63, g1)
+    assert np.isnan(gp[:3]).all() and ((st & 16) != 0).all()
+
+
 def test_host_math_fp32(hc):
     w = W.config3(n=3000, S=1)
     z = w.z.astype(np.float32).astype(np.float64)
