@@ -12,7 +12,10 @@
 
 namespace cb {
 
-constexpr int OUTER_THREADS = 128;
+#ifndef CB_THREADS
+#define CB_THREADS 128
+#endif
+constexpr int OUTER_THREADS = CB_THREADS;
 #ifndef CB_KZ
 #define CB_KZ 2
 #endif

@@ -13,45 +13,6 @@
 
 namespace cb {
 
-// Solve the n x n system M a = rhs_k (k < nrhs) in place by Gaussian elimination with partial pivoting.
-// M is row-major [n][n+nrhs] augmented.  Singular systems leave inf/nan (degenerate roots).
-template <int N, int NR>
-CB_HD void solve_aug(double (&M)[N][N + NR]) {
-    for (int col = 0; col < N; ++col) {
-        int piv = col;
-        double best = fabs(M[col][col]);
-        for (int r = col + 1; r < N; ++r) {
-            double v = fabs(M[r][col]);
-            if (v > best) { best = v; piv = r; }
-        }
-        if (piv != col) {
-            for (int k = col; k < N + NR; ++k) { double t = M[col][k]; M[col][k] = M[piv][k]; M[piv][k] = t; }
-        }
-        double inv = 1.0 / M[col][col];
-        for (int r = col + 1; r < N; ++r) {
-            double f = M[r][col] * inv;
-            for (int k = col + 1; k < N + NR; ++k) M[r][k] = fma(-f, M[col][k], M[r][k]);
-        }
-    }
-    for (int col = N - 1; col >= 0; --col) {
-        double inv = 1.0 / M[col][col];
-        for (int k = N; k < N + NR; ++k) {
-            double s = M[col][k];
-            for (int j = col + 1; j < N; ++j) s = fma(-M[col][j], M[j][k], s);
-            M[col][k] = s * inv;
-        }
-    }
-}
-
-// N_k(x) = k x^(k-1) E^2 - x^k (E^2)'/2 : d(x^k / E)/dx = N_k / E^3.  Adds coef * N_k to column `dst` (rows = powers).
-template <int ROWS, int COLS>
-CB_HD void add_Nk(double (&M)[ROWS][COLS], int dst, int k, const double e[5]) {
-    for (int p = 0; p < 5; ++p) {
-        if (k > 0 && p + k - 1 < ROWS) M[p + k - 1][dst] += k * e[p];
-        if (p > 0 && p - 1 + k < ROWS) M[p - 1 + k][dst] -= 0.5 * p * e[p];
-    }
-}
-
 // S1-S3.  want_grad: 0 none, 1 chi-family (GI), 2 all (GI, GT, GA).
 CB_HD void cosmo_prep(double Om, double OL, double Or, double H0, int want_grad, Cosmo<double>& C) {
     const double Ok = 1.0 - Om - OL - Or;
@@ -202,42 +163,75 @@ CB_HD void cosmo_prep(double Om, double OL, double Or, double H0, int want_grad,
     C.status = st;
     if (!want_grad) return;
 
-    // --- gradient basis coefficients: polynomial identities in x, solved per cosmology
-    const double e[5] = {OL, 0.0, Ok, Om, Or};
-    const double NK[5] = {m * m * c, m * m * b + 2.0 * Or * m * c, m * m + 2.0 * Or * m * b + Or * Or * c,
-                          2.0 * Or * m + Or * Or * b, Or * Or};
-    {   // I0 and T share the 5x5 matrix: columns E^2, N_K, N_0, N_1, N_2 ; rhs: 3 for I0 then 3 for T
-        double M[5][5 + 6];
-        for (int r = 0; r < 5; ++r) for (int k = 0; k < 11; ++k) M[r][k] = 0.0;
-        for (int p = 0; p < 5; ++p) { M[p][0] = e[p]; M[p][1] = NK[p]; }
-        add_Nk(M, 2, 0, e); add_Nk(M, 3, 1, e); add_Nk(M, 4, 2, e);
-        // D_theta = dE^2/dtheta with Ok eliminated: x^3 - x^2, 1 - x^2, x^4 - x^2
-        M[3][5] = 1.0; M[2][5] = -1.0;
-        M[0][6] = 1.0; M[2][6] = -1.0;
-        M[4][7] = 1.0; M[2][7] = -1.0;
-        // T: D_theta / x - aT E^2 / x with aT = D_theta(0)/OL (the 1/x pole goes to the forward T)
-        const double aT[3] = {0.0, 1.0 / OL, 0.0};
-        M[2][8] = 1.0; M[1][8] = -1.0;                       // x^2 - x
-        M[1][9] = -1.0;                                      // (1 - x^2)/x = 1/x - x
-        M[3][10] = 1.0; M[1][10] = -1.0;                     // x^3 - x
-        for (int p = 1; p < 5; ++p) M[p - 1][9] -= aT[1] * e[p];
-        solve_aug<5, 6>(M);
-        for (int t = 0; t < 3; ++t) {
-            for (int j = 0; j < 5; ++j) { C.GI[t][j] = M[j][5 + t]; C.GT[t][j] = M[j][8 + t]; }
-            C.GT[t][5] = aT[t];
-        }
-    }
+    // --- gradient basis coefficients: polynomial identities in x, solved per cosmology.
+    // Unknowns (a, bK, c0, c1, c2) multiply the columns E^2, N_K, N_0, N_1, N_2 (N_k = k x^(k-1) E^2 - x^k (E^2)'/2);
+    // rows are the powers x^0..x^4.  With e = (OL, 0, Ok, Om, Or):
+    //   x^0: e0 a + NK0 bK            + e0 c1             = D0
+    //   x^1:        NK1 bK - e2 c0             + 2 e0 c2  = D1
+    //   x^2: e2 a + NK2 bK - 1.5 e3 c0                    = D2     <- pivot on Om (> 0): c0
+    //   x^3: e3 a + NK3 bK - 2 e4 c0 - 0.5 e3 c1 + e2 c2  = D3
+    //   x^4: e4 a + NK4 bK           - e4 c1   + 0.5 e3 c2 = D4    <- pivot on Om: c2
+    // Eliminating c0 and c2 leaves a 3x3 system in (a, bK, c1), solved by its adjugate: no pivot search, no indexed
+    // storage, so the whole solve stays in registers (the ELEMENTWISE kernels do it once per element).
+    const double e0 = OL, e2 = Ok, e3 = Om, e4 = Or;
+    const double NK0 = m * m * c, NK1 = m * m * b + 2.0 * Or * m * c, NK2 = m * m + 2.0 * Or * m * b + Or * Or * c,
+                 NK3 = 2.0 * Or * m + Or * Or * b, NK4 = Or * Or;
+    const double k0 = 2.0 / (3.0 * e3), k2 = 2.0 / e3;
+    const double al0 = e2 * k0, be0 = NK2 * k0;                              // c0 = al0 a + be0 bK - k0 D2
+    const double al2 = -e4 * k2, be2 = -NK4 * k2, de2 = e4 * k2;             // c2 = al2 a + be2 bK + de2 c1 + k2 D4
+    // 3x3 rows: (x^0), (x^1), (x^3)
+    const double m00 = e0, m01 = NK0, m02 = e0;
+    const double m10 = -e2 * al0 + 2.0 * e0 * al2, m11 = NK1 - e2 * be0 + 2.0 * e0 * be2, m12 = 2.0 * e0 * de2;
+    const double m20 = e3 - 2.0 * e4 * al0 + e2 * al2, m21 = NK3 - 2.0 * e4 * be0 + e2 * be2, m22 = -0.5 * e3 + e2 * de2;
+    const double c00 = m11 * m22 - m12 * m21, c01 = m12 * m20 - m10 * m22, c02 = m10 * m21 - m11 * m20;
+    const double idet = 1.0 / (m00 * c00 + m01 * c01 + m02 * c02);
+    const double i00 = c00 * idet, i01 = (m02 * m21 - m01 * m22) * idet, i02 = (m01 * m12 - m02 * m11) * idet;
+    const double i10 = c01 * idet, i11 = (m00 * m22 - m02 * m20) * idet, i12 = (m02 * m10 - m00 * m12) * idet;
+    const double i20 = c02 * idet, i21 = (m01 * m20 - m00 * m21) * idet, i22 = (m00 * m11 - m01 * m10) * idet;
+    auto solve5 = [&](double D0, double D1, double D2, double D3, double D4, double* out5) {
+        const double g0 = -k0 * D2, g2 = k2 * D4;
+        const double r0 = D0, r1 = D1 + e2 * g0 - 2.0 * e0 * g2, r2 = D3 + 2.0 * e4 * g0 - e2 * g2;
+        const double av = i00 * r0 + i01 * r1 + i02 * r2;
+        const double bv = i10 * r0 + i11 * r1 + i12 * r2;
+        const double c1v = i20 * r0 + i21 * r1 + i22 * r2;
+        out5[0] = av; out5[1] = bv;
+        out5[2] = al0 * av + be0 * bv + g0;
+        out5[3] = c1v;
+        out5[4] = al2 * av + be2 * bv + de2 * c1v + g2;
+    };
+    // I0: D_theta = dE^2/dtheta with Ok eliminated: x^3 - x^2, 1 - x^2, x^4 - x^2
+    solve5(0.0, 0.0, -1.0, 1.0, 0.0, C.GI[0]);
+    solve5(1.0, 0.0, -1.0, 0.0, 0.0, C.GI[1]);
+    solve5(0.0, 0.0, -1.0, 0.0, 1.0, C.GI[2]);
+    // T: D_theta / x - aT E^2 / x with aT = D_theta(0)/OL (the 1/x pole goes to the forward T): x^2 - x, 1/x - x, x^3 - x
+    const double aT = 1.0 / OL;
+    solve5(0.0, -1.0, 1.0, 0.0, 0.0, C.GT[0]);
+    solve5(0.0, -1.0 - aT * e2, -aT * e3, -aT * e4, 0.0, C.GT[1]);
+    solve5(0.0, -1.0, 0.0, 1.0, 0.0, C.GT[2]);
+    C.GT[0][5] = 0.0; C.GT[1][5] = aT; C.GT[2][5] = 0.0;
     if (want_grad < 2) return;
-    {   // A: x^2 D_theta over columns E^2, N_K, N_0, N_1, N_2, N_3 (N_4 when Or = 0), x^2 E^2
-        double M[7][7 + 3];
-        for (int r = 0; r < 7; ++r) for (int k = 0; k < 10; ++k) M[r][k] = 0.0;
-        for (int p = 0; p < 5; ++p) { M[p][0] = e[p]; M[p][1] = NK[p]; M[p + 2][6] = e[p]; }
-        add_Nk(M, 2, 0, e); add_Nk(M, 3, 1, e); add_Nk(M, 4, 2, e); add_Nk(M, 5, (C.cubic & 1u) ? 4 : 3, e);
-        M[5][7] = 1.0; M[4][7] = -1.0;
-        M[2][8] = 1.0; M[4][8] = -1.0;
-        M[6][9] = 1.0; M[4][9] = -1.0;
-        solve_aug<7, 3>(M);
-        for (int t = 0; t < 3; ++t) for (int j = 0; j < 7; ++j) C.GA[t][j] = M[j][7 + t];
+    // A: x^2 D_theta (x^5 - x^4, x^2 - x^4, x^6 - x^4) over the five columns above plus N_3 (N_4 when Or = 0) and x^2 E^2.
+    // The rows x^5, x^6 involve only those two extra unknowns (c3, aA); their columns then move to the right-hand side
+    // of the same 5x5 system.
+    for (int t = 0; t < 3; ++t) {
+        const double D5 = (t == 0) ? 1.0 : 0.0, D6 = (t == 2) ? 1.0 : 0.0;
+        double c3, aA, n3[5];
+        if (C.cubic & 1u) {         // N_4 = (0,0,0,4 e0,0 | 3 e2, 2.5 e3);  x^2 E^2 = (0,0,e0,0,e2 | e3, 0)
+            c3 = D6 / (2.5 * e3);
+            aA = (D5 - 3.0 * e2 * c3) / e3;
+            n3[0] = 0.0; n3[1] = 0.0; n3[2] = 0.0; n3[3] = 4.0 * e0; n3[4] = 0.0;
+        } else {                    // N_3 = (0,0,3 e0,0,2 e2 | 1.5 e3, e4);  x^2 E^2 = (0,0,e0,0,e2 | e3, e4)
+            const double id = 1.0 / (0.5 * e3 * e4);
+            c3 = (D5 * e4 - e3 * D6) * id;
+            aA = (1.5 * e3 * D6 - e4 * D5) * id;
+            n3[0] = 0.0; n3[1] = 0.0; n3[2] = 3.0 * e0; n3[3] = 0.0; n3[4] = 2.0 * e2;
+        }
+        const double D2 = ((t == 1) ? 1.0 : 0.0) - c3 * n3[2] - aA * e0;
+        const double D3 = -c3 * n3[3];
+        const double D4 = -1.0 - c3 * n3[4] - aA * e2;
+        solve5(0.0, 0.0, D2, D3, D4, C.GA[t]);
+        C.GA[t][5] = c3;
+        C.GA[t][6] = aA;
     }
 }
 
