@@ -382,3 +382,68 @@ def test_two_complex_pairs_outer_and_likelihood(cb):
     ref = oracle.snia_loglike(z, mu_obs, sigma, Om[1], OL[1], Or[1], H0[1], with_grad=False)
     assert abs(float(logL[1]) - float(ref[0])) <= 1e-10 * abs(float(ref[0]))
     assert np.isnan(grad.cpu().numpy()[:, 1]).all() and np.isfinite(grad.cpu().numpy()[:, 0]).all()
+
+
+# ---------------------------------------------------------------- full sizes of configs 4 and 5 (sampled oracle + properties)
+def test_config4_full_size_sampled(cb):
+    """BASELINE.json config 4 at full size (10^6 SNe x 256 samples); oracle on full N for 2 samples, properties for all"""
+    import torch
+    n, S = 1_000_000, 256
+    rng = np.random.default_rng(4)
+    z = rng.uniform(0.01, 1.5, n)
+    idx = np.sort(rng.choice(n, 4000, replace=False))
+    # mu_obs from the ORACLE on a subsample would not cover all N: use the oracle for ALL N here (about 3 s on 16 threads)
+    w = W.config4(_mu_oracle, n=n, S=S)
+    mu_obs, sigma = w.extra["mu_obs"], w.extra["sigma"]
+    logL, grad = cb.cosmo_snia_loglike(dev(w.z), dev(mu_obs), dev(sigma), dev(w.Om), dev(w.OL), dev(w.Or), dev(w.H0))
+    assert bool(torch.isfinite(logL).all()) and bool(torch.isfinite(grad).all())
+    logL, grad = logL.cpu().numpy(), grad.cpu().numpy()
+    # the data were drawn at (0.3, 0.7, 0, 70): the best of the 256 samples must be close to it
+    best = int(np.argmax(logL))
+    assert abs(w.Om[best] - 0.3) < 0.06 and abs(w.H0[best] - 70.0) < 3.0
+    for s in (0, 131):
+        ref = oracle.snia_loglike(w.z, mu_obs, sigma, w.Om[s], w.OL[s], w.Or[s], w.H0[s]).astype(np.float64)
+        assert abs(logL[s] - ref[0]) <= 1e-10 * abs(ref[0]), s
+        val, g, _ = oracle_batch(w.z[idx], w.Om[s:s + 1], w.OL[s:s + 1], w.Or[s:s + 1], w.H0[s:s + 1], True)
+        resid = (mu_obs[idx] - val[:, OBS["MU"]]) / sigma[idx] ** 2
+        for p in range(4):
+            scale = np.abs(resid * g[:, OBS["MU"], 1 + p]).mean() * n      # ~ sum of |terms|
+            assert abs(grad[p, s] - ref[1 + p]) <= TOL_GRAD * scale, (s, p)
+
+
+def test_config5_full_size_sampled(cb):
+    """BASELINE.json config 5 at full size (10^7 + 3 x 10^5 rows, all six outputs, forward + VJP); oracle on a sample"""
+    import torch
+    w = W.config5()
+    n = w.n_z
+    g = torch.randn((6, 1, n), dtype=torch.float64, device="cuda", generator=torch.Generator("cuda").manual_seed(5))
+    gz, gp, out, st = cb.cosmo_vjp(dev(w.z), dev(w.Om), dev(w.OL), dev(w.Or), dev(w.H0), g, cb.ELEMENTWISE, w.which, want_out=True)
+    st = st[0]
+    assert int(((st & 3) != 0).sum()) == 0            # every row is a valid cosmology
+    rng = np.random.default_rng(55)
+    idx = np.sort(np.concatenate([rng.choice(10_000_000, 6000, replace=False), 10_000_000 + rng.choice(300_000, 3000, replace=False)]))
+    ti = torch.from_numpy(idx).cuda()
+    o = out[:, 0, :][:, ti].cpu().numpy()
+    s_ = st[ti].cpu().numpy()
+    val, grad, sto = oracle_batch(w.z[idx], w.Om[idx], w.OL[idx], w.Or[idx], w.H0[idx], True)
+    assert (sto >= 0).all() and (((s_ & 4) != 0) == (sto == 1)).all()
+    rnd = idx < 10_000_000
+    for k, name in enumerate(w.which):
+        ref = val[:, OBS[name]]
+        m = np.isfinite(ref) & rnd
+        if name in ("DC", "TL", "DABS"):
+            e = relerr(o[k], ref)[m]
+            assert np.mean(e <= TOL_VAL) > 0.998 and e.max() <= 1e-9, (name, e.max())
+        else:
+            scale = np.abs(val[:, OBS["DC"]]) * ((1 + w.z[idx]) if name == "DL" else 1.0) if name != "MU" else np.ones_like(ref)
+            ae = np.abs(o[k] - ref)[m]
+            assert np.mean(ae <= 2e-11 * np.maximum(scale[m], np.abs(ref[m]))) > 0.995, name
+    # closed-form gradients (d/dz, d/dH0) on the sampled random rows
+    gs = g[:, 0, :][:, ti].cpu().numpy()
+    fin = np.isfinite(val).all(axis=1) & rnd
+    for p, mine in ((0, gz[ti].cpu().numpy()), (4, gp[3][ti].cpu().numpy())):
+        ref = np.zeros(len(idx)); ref_abs = np.zeros(len(idx))
+        for k, name in enumerate(w.which):
+            t = gs[k] * grad[:, OBS[name], p]
+            ref += np.where(np.isfinite(t), t, 0.0); ref_abs += np.abs(np.where(np.isfinite(t), t, 0.0))
+        assert (np.abs(mine - ref)[fin] <= 1e-9 * ref_abs[fin]).all(), p
