@@ -447,3 +447,27 @@ def test_config5_full_size_sampled(cb):
             t = gs[k] * grad[:, OBS[name], p]
             ref += np.where(np.isfinite(t), t, 0.0); ref_abs += np.abs(np.where(np.isfinite(t), t, 0.0))
         assert (np.abs(mine - ref)[fin] <= 1e-9 * ref_abs[fin]).all(), p
+
+
+# ---------------------------------------------------------------- OUTER and ELEMENTWISE are the same arithmetic
+@pytest.mark.parametrize("N,S", [(333, 37), (100, 300), (1, 1), (4097, 2)])
+def test_outer_equals_elementwise(cb, N, S):
+    rng = np.random.default_rng(N + S)
+    z = rng.uniform(0.01, 3.0, N)
+    Om = rng.uniform(0.1, 0.5, S); OL = rng.uniform(0.3, 0.9, S); Or = rng.choice([0.0, 9e-5, 1e-3], S); H0 = rng.uniform(60, 80, S)
+    which = ("DC", "MU", "TL", "DABS")
+    g = rng.standard_normal((4, S, N))
+    gz, gp, out, st = cb.cosmo_vjp(dev(z), dev(Om), dev(OL), dev(Or), dev(H0), dev(g), cb.OUTER, which, want_out=True)
+    zz = np.tile(z, S)
+    rep = lambda a: np.repeat(a, N)
+    ge = g.reshape(4, 1, S * N)
+    gz_e, gp_e, out_e, st_e = cb.cosmo_vjp(dev(zz), dev(rep(Om)), dev(rep(OL)), dev(rep(Or)), dev(rep(H0)), dev(ge), cb.ELEMENTWISE,
+                                           which, want_out=True)
+    out, out_e = out.cpu().numpy(), out_e.cpu().numpy().reshape(4, S, N)
+    assert np.allclose(out, out_e, rtol=1e-13, atol=0)
+    gz_ref = gz_e.cpu().numpy().reshape(S, N).sum(axis=0)
+    gz_abs = np.abs(gz_e.cpu().numpy().reshape(S, N)).sum(axis=0)
+    assert (np.abs(gz.cpu().numpy() - gz_ref) <= 1e-12 * gz_abs).all()
+    gpe = gp_e.cpu().numpy().reshape(4, S, N)
+    assert (np.abs(gp.cpu().numpy() - gpe.sum(axis=2)) <= 1e-12 * np.abs(gpe).sum(axis=2)).all()
+    assert np.array_equal(st.cpu().numpy() & 15, st_e.cpu().numpy().reshape(S, N) & 15)
