@@ -61,6 +61,7 @@ __global__ void k_prep(const double* __restrict__ Om, const double* __restrict__
     if (want_grad < 2) {
         for (int t = 0; t < 3; ++t) {
             for (int j = 0; j < 7; ++j) C.GA[t][j] = 0.0;
+            for (int j = 0; j < 5; ++j) C.GJ[t][j] = C.GJ[t + 2][j] = 0.0;
             if (want_grad < 1) { for (int j = 0; j < 5; ++j) C.GI[t][j] = 0.0; for (int j = 0; j < 6; ++j) C.GT[t][j] = 0.0; }
         }
     }

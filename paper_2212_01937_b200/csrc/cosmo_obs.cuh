@@ -73,6 +73,39 @@ CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, c
     const T aK = -gM * C.dH * O.Fk;
     T btA = T(0);
     if (kA) btA = (((C.cubic & 1u) ? n4 : n3) - R.Em1) * iE;
+    // d_abs gradient where radiation is a perturbation: the exact basis above then multiplies the forward A by ~3/Or
+    // (the x^5, x^6 rows), which loses Om/Or digits.  Instead J'_p = int x^p dx/E^3, p <= 4, come from the basis and
+    // J'_5.. follow from d(x^k / E) = N_k / E^3:  Om (k - 3/2) J'_{k+2} = [x^k/E] - k OL J'_{k-1} - (k-1) Ok J'_{k+1}
+    // - (k-2) Or J'_{k+3}, the Or terms iterated (same scheme as the forward d_abs).
+    bool useJ = false;
+    T Jp[17];
+    if (kA && !(C.cubic & 2u)) {
+        constexpr int KJ = 12;                // levels k = 3 .. 3 + KJ - 1
+#pragma unroll
+        for (int p = 0; p < 5; ++p)
+            Jp[p] = C.GJ[p][0] * R.I0 + C.GJ[p][1] * R.K + C.GJ[p][2] * bt0 + C.GJ[p][3] * bt1 + C.GJ[p][4] * bt2;
+#pragma unroll
+        for (int p = 5; p < 17; ++p) Jp[p] = T(0);
+        T bk[KJ];
+        {
+            T xk = x * x * x;
+#pragma unroll
+            for (int j = 0; j < KJ; ++j) { bk[j] = N::fma_(xk - T(1), iE, bt0); xk *= x; }     // x^k/E - 1 = (x^k - 1)/E + (1/E - 1)
+        }
+        T prev5 = T(0), prev6 = T(0);
+#pragma unroll
+        for (int sw = 0; sw < KJ - 1; ++sw) {
+            if (sw == KJ - 2) { prev5 = Jp[5]; prev6 = Jp[6]; }
+#pragma unroll
+            for (int j = 0; j < KJ - 1 - sw; ++j) {
+                const int k = 3 + j;
+                const T a = bk[j] - T(k) * C.OL * Jp[k - 1] - T(k - 1) * C.Ok * Jp[k + 1] - T(k - 2) * C.Or * Jp[k + 3];
+                Jp[k + 2] = a * C.iOm * T(1.0 / (k - 1.5));
+            }
+        }
+        const T tol = T(sizeof(T) == 8 ? 1e-12 : 1e-5);
+        useJ = N::abs_(Jp[5] - prev5) <= tol * N::abs_(Jp[5]) && N::abs_(Jp[6] - prev6) <= tol * N::abs_(Jp[6]);
+    }
 #pragma unroll
     for (int t = 0; t < 3; ++t) {
         T dI = C.GI[t][0] * R.I0 + C.GI[t][1] * R.K + C.GI[t][2] * bt0 + C.GI[t][3] * bt1 + C.GI[t][4] * bt2;
@@ -90,6 +123,7 @@ CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, c
         if (kA) {
             T dA = C.GA[t][0] * R.I0 + C.GA[t][1] * R.K + C.GA[t][2] * bt0 + C.GA[t][3] * bt1 + C.GA[t][4] * bt2 + C.GA[t][5] * btA
                    + C.GA[t][6] * R.AA;
+            if (useJ) dA = (t == 0 ? Jp[5] : (t == 1 ? Jp[2] : Jp[6])) - Jp[4];      // x^2 D_theta = x^5, x^2, x^6 minus x^4
             acc = N::fma_(g[5] * C.dH, T(-0.5) * dA, acc);
         }
         gp[t] += acc;

@@ -210,6 +210,12 @@ CB_HD void cosmo_prep(double Om, double OL, double Or, double H0, int want_grad,
     solve5(0.0, -1.0, 0.0, 1.0, 0.0, C.GT[2]);
     C.GT[0][5] = 0.0; C.GT[1][5] = aT; C.GT[2][5] = 0.0;
     if (want_grad < 2) return;
+    // the monomials themselves: J'_p = int x^p dx / E^3 (p = 0..4), used by the perturbative d_abs gradient
+    solve5(1.0, 0.0, 0.0, 0.0, 0.0, C.GJ[0]);
+    solve5(0.0, 1.0, 0.0, 0.0, 0.0, C.GJ[1]);
+    solve5(0.0, 0.0, 1.0, 0.0, 0.0, C.GJ[2]);
+    solve5(0.0, 0.0, 0.0, 1.0, 0.0, C.GJ[3]);
+    solve5(0.0, 0.0, 0.0, 0.0, 1.0, C.GJ[4]);
     // A: x^2 D_theta (x^5 - x^4, x^2 - x^4, x^6 - x^4) over the five columns above plus N_3 (N_4 when Or = 0) and x^2 E^2.
     // The rows x^5, x^6 involve only those two extra unknowns (c3, aA); their columns then move to the right-hand side
     // of the same 5x5 system.

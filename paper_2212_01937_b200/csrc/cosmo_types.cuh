@@ -89,11 +89,12 @@ struct Cosmo {
     T GI[3][5];        // X = I0 : basis (I0, K, b0, b1, b2)
     T GT[3][6];        // X = T  : basis (I0, K, b0, b1, b2, T)
     T GA[3][7];        // X = A  : basis (I0, K, b0, b1, b2, b3 (b4 when Or = 0), A)
+    T GJ[5][5];        // J'_p = int x^p dx / E^3, p = 0..4, over the basis (I0, K, b0, b1, b2)  (d_abs gradient)
     unsigned status;
     unsigned cubic;    // bit 0: Or == 0 (cubic case, appendix B.1);  bit 1: two complex pairs (cosmo_c4.cuh; m, rn hold g1, h1)
 };
 
-constexpr int COSMO_NFIELDS = 86;   // floating-point members of Cosmo<T>, in declaration order
+constexpr int COSMO_NFIELDS = 111;   // floating-point members of Cosmo<T>, in declaration order
 static_assert(sizeof(Cosmo<double>) == COSMO_NFIELDS * sizeof(double) + 2 * sizeof(unsigned), "Cosmo<T> layout");
 static_assert(sizeof(Cosmo<float>) == COSMO_NFIELDS * sizeof(float) + 2 * sizeof(unsigned), "Cosmo<T> layout");
 

@@ -90,7 +90,6 @@ def test_host_math_matches_oracle(hc, cfg):
     n = w.n_z
     rng = np.random.default_rng(1)
     gup = rng.standard_normal((6, n))
-    gup[5] = 0.0          # d(d_abs)/dOr has a documented accuracy limit: checked separately below
     out, gz, gp, st = run(hc, w.z, w.Om, w.OL, w.Or, w.H0, 63, gup)
     assert (st == 0).all()
     val, grad, sto = oracle.observables_batch(w.z, w.Om, w.OL, w.Or, w.H0, with_grad=True)
@@ -105,24 +104,21 @@ def test_host_math_matches_oracle(hc, cfg):
     for p in range(5):
         ref = sum(gup[i] * grad[:, i, p] for i in range(6))
         scale = sum(np.abs(gup[i] * grad[:, i, p]) for i in range(6))
-        assert (np.abs(mine[p] - ref) <= 1e-9 * scale).all(), p
+        assert (np.abs(mine[p] - ref) <= 1e-8 * scale).all(), p
 
 
-def test_dabs_gradient_documented_limit(hc):
-    """d(d_abs)/d(Om, OL) meet 1e-8; d(d_abs)/dOr does not for small Or: assert the bound we state."""
-    w = W.config2(n=800)
+def test_dabs_gradient(hc):
+    """d(d_abs)/d(Om, OL, Or) on config 2 (the perturbative J' recursion of cosmo_obs.cuh where radiation is small)"""
+    w = W.config2(n=1500)
     n = w.n_z
     g1 = np.zeros((6, n)); g1[5] = 1
     _, gz, gp, _ = run(hc, w.z, w.Om, w.OL, w.Or, w.H0, 63, g1)
     val, grad, _ = oracle.observables_batch(w.z, w.Om, w.OL, w.Or, w.H0, with_grad=True)
     val, grad = val.astype(np.float64), grad.astype(np.float64)
-    for p, tol in ((1, 1e-8), (2, 1e-9)):
+    for p, tol in ((1, 1e-8), (2, 1e-9), (3, 1e-8)):
         ref = grad[:, 5, p]
         e = np.abs(gp[p - 1] - ref) / np.maximum(np.abs(ref), 1e-3 * np.abs(val[:, 5]))
         assert e.max() <= tol, (p, e.max())
-    ref = grad[:, 5, 3]
-    e = np.abs(gp[2] - ref) / np.maximum(np.abs(ref), 1e-3 * np.abs(val[:, 5]))
-    assert np.isfinite(e).all() and e.max() <= 1e-5
 
 
 def test_host_math_stress_blocks(hc):
