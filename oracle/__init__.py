@@ -33,6 +33,8 @@ def lib():
         _lib.oracle_observables_batch.argtypes = [C.c_int64, _DP, _DP, _DP, _DP, _DP, C.c_int64, _LDP, _LDP,
                                                   C.POINTER(C.c_int32)]
         _lib.oracle_observables_batch.restype = None
+        _lib.oracle_derived_batch.argtypes = [C.c_int64, _DP, _DP, _DP, _DP, _DP, C.c_int64, _LDP, _LDP, C.POINTER(C.c_int32)]
+        _lib.oracle_derived_batch.restype = None
         _lib.oracle_snia_loglike.argtypes = [C.c_int64, _DP, _DP, _DP] + [C.c_double] * 4 + [C.c_int, _LDP]
         _lib.oracle_snia_loglike.restype = C.c_int
         for name, nin in (("oracle_rf", 6), ("oracle_rc", 4), ("oracle_rd", 6), ("oracle_rj", 8)):
@@ -94,6 +96,28 @@ def observables_batch(z, Om, OL, Or, H0, with_grad=True, threads=None):
         L.oracle_set_threads(int(threads))
     L.oracle_observables_batch(n, _dp(z), *[_dp(p) for p in ps], n_cosmo, _ldp(val),
                                _ldp(grad) if with_grad else None, status.ctypes.data_as(C.POINTER(C.c_int32)))
+    return val, grad, status
+
+
+DERIVED = ("DA", "VC", "AGE")                       # order of oracle_derived's observable axis
+
+
+def derived_batch(z, Om, OL, Or, H0, with_grad=True, threads=None):
+    """Further derived observables: D_A [Mpc], V_C [Mpc^3, whole sky], age at z [Gyr].
+    Returns val[n,3], grad[n,3,5] or None, status[n]; np.longdouble."""
+    z = np.ascontiguousarray(z, dtype=np.float64)
+    n = z.shape[0]
+    ps = [np.ascontiguousarray(np.atleast_1d(p), dtype=np.float64) for p in (Om, OL, Or, H0)]
+    n_cosmo = ps[0].shape[0]
+    assert all(p.shape[0] == n_cosmo for p in ps) and n_cosmo in (1, n)
+    val = np.zeros((n, 3), dtype=np.longdouble)
+    grad = np.zeros((n, 3, N_WRT), dtype=np.longdouble) if with_grad else None
+    status = np.zeros(n, dtype=np.int32)
+    L = lib()
+    if threads:
+        L.oracle_set_threads(int(threads))
+    L.oracle_derived_batch(n, _dp(z), *[_dp(p) for p in ps], n_cosmo, _ldp(val), _ldp(grad) if with_grad else None,
+                           status.ctypes.data_as(C.POINTER(C.c_int32)))
     return val, grad, status
 
 

@@ -342,6 +342,143 @@ void oracle_observables_batch(int64_t n, const double *z, const double *Om, cons
 }
 
 /* ======================================================================================
+ * (2b) further derived observables of PAPER.md:95: angular-diameter distance
+ *      D_A = D_M/(1+z), comoving volume out to z over the whole sky V_C = 4 pi int_0^chi D_M^2 dchi'
+ *      (ref. [59] eq. (13.60)), and the age at z, int_z^inf of eq. (2.4), with their total derivatives
+ *      wrt (z, Om, OL, Or, H0).  val[3] = {DA [Mpc], VC [Mpc^3], AGE [Gyr]}, grad[3][5].
+ *      The age gradient integrals are Leibniz integrals of the same integrand, in a = 1/(1+z'), a = s^2:
+ *        d(H0 age)/dtheta = -1/2 int_0^{a_z} q_theta(a) P(a)^{-3/2} da,  q = a^2-a^3 (Om), a^5-a^3 (OL), a-a^3 (Or).
+ * ====================================================================================== */
+static void age_grad_integrand_s(const cosmo_t *c, ld s, ld f[4]) {
+    ld a = s * s;
+    if (c->Or == 0.0L) {
+        /* P = a P1, P^{3/2} = a^{3/2} P1^{3/2}; da = 2 s ds = 2 a^{1/2} ds */
+        ld P1 = c->Om + c->Ok * a + c->OL * a * a * a, r = P1 * sqrtl(P1);
+        f[0] = 2.0L * a / sqrtl(P1);                      /* a da / sqrt(P) = 2 s^2 ds / sqrt(P1) */
+        f[1] = 2.0L * (a - a * a) / r;                    /* (a^2 - a^3) a^{-3/2} 2 a^{1/2} */
+        f[2] = 2.0L * (a * a * a * a - a * a) / r;
+        f[3] = 2.0L * (1.0L - a * a) / r;
+        return;
+    }
+    ld P = c->Or + c->Om * a + c->Ok * a * a + c->OL * a * a * a * a, r = P * sqrtl(P);
+    f[0] = 2.0L * s * a / sqrtl(P);
+    f[1] = 2.0L * s * (a * a - a * a * a) / r;
+    f[2] = 2.0L * s * (a * a * a * a * a - a * a * a) / r;
+    f[3] = 2.0L * s * (a - a * a * a) / r;
+}
+static void age_grad_panel(const cosmo_t *c, ld a, ld b, ld K[4], ld G[4]) {
+    ld h = 0.5L * (b - a), m = 0.5L * (a + b), f[4];
+    for (int v = 0; v < 4; ++v) K[v] = G[v] = 0.0L;
+    for (int i = 0; i < 21; ++i) {
+        age_grad_integrand_s(c, m + h * GK21_X[i], f);
+        for (int v = 0; v < 4; ++v) { K[v] += GK21_WK[i] * f[v]; G[v] += GK21_WG[i] * f[v]; }
+    }
+    for (int v = 0; v < 4; ++v) { K[v] *= h; G[v] *= h; }
+}
+static void age_grad_adapt(const cosmo_t *c, ld a, ld b, const ld tolabs[4], int depth, ld acc[4], int *npanels) {
+    ld K[4], G[4];
+    age_grad_panel(c, a, b, K, G);
+    int ok = 1;
+    for (int v = 0; v < 4; ++v) {
+        ld err = fabsl(K[v] - G[v]);
+        if (err > tolabs[v]) ok = 0;
+        if (err != err) ok = 1;   /* NaN/inf integrand (e.g. a divergent gradient integral when Om = 0): give up, it propagates */
+    }
+    if (ok || depth >= GK_MAXDEPTH || *npanels >= GK_MAXPANELS) { for (int v = 0; v < 4; ++v) acc[v] += K[v]; ++*npanels; return; }
+    ld m = 0.5L * (a + b), t2[4];
+    for (int v = 0; v < 4; ++v) t2[v] = 0.5L * tolabs[v];
+    age_grad_adapt(c, a, m, t2, depth + 1, acc, npanels);
+    age_grad_adapt(c, m, b, t2, depth + 1, acc, npanels);
+}
+
+/* V_C / (4 pi d_H^3) = v(k, chi) = int_0^chi F(k, chi')^2 dchi' and its partial wrt k; F = sinn transform (dv/dchi = F^2) */
+static void volume_transform(ld k, ld chi, ld *v, ld *dv_dk) {
+    ld w = k * chi * chi;
+    if (fabsl(w) < 1e-2L) {
+        /* v = chi^3 sum_{j>=1} 4^j w^(j-1) / (2 (2j+1)!),  dv/dk = chi^5 sum_{j>=2} (j-1) 4^j w^(j-2) / (2 (2j+1)!) */
+        ld S = 0, D = 0, coef = 1.0L; /* 4^j/(2j+1)! */
+        ld wp1 = 1.0L, wp2 = 1.0L;
+        for (int j = 1; j < 14; ++j) {
+            coef = coef * 4.0L / ((2.0L * j) * (2.0L * j + 1.0L));
+            S += 0.5L * coef * wp1;
+            if (j >= 2) { D += 0.5L * (j - 1) * coef * wp2; wp2 *= w; }
+            wp1 *= w;
+        }
+        *v = chi * chi * chi * S; *dv_dk = chi * chi * chi * chi * chi * D;
+        return;
+    }
+    if (k > 0) {
+        /* v = (sinh(2 s chi)/(2 s) - chi)/(2k), s = sqrt(k);  d/dk of the numerator = chi cosh/(2k) - sinh/(4 k s) */
+        ld s = sqrtl(k), sh2 = sinhl(2.0L * s * chi), ch2 = coshl(2.0L * s * chi);
+        *v = (sh2 / (2.0L * s) - chi) / (2.0L * k);
+        ld dnum = chi * ch2 / (2.0L * k) - sh2 / (4.0L * k * s);
+        *dv_dk = dnum / (2.0L * k) - (*v) / k;
+    } else {
+        /* with kk = -k: v = (chi - sin(2 s chi)/(2 s))/(2 kk), s = sqrt(kk) */
+        ld kk = -k, s = sqrtl(kk), sn2 = sinl(2.0L * s * chi), cs2 = cosl(2.0L * s * chi);
+        *v = (chi - sn2 / (2.0L * s)) / (2.0L * kk);
+        ld dnum = -(chi * cs2 / (2.0L * kk) - sn2 / (4.0L * kk * s));
+        ld dv_dkk = dnum / (2.0L * kk) - (*v) / kk;
+        *dv_dk = -dv_dkk;
+    }
+}
+
+int oracle_derived(ld z, ld Om, ld OL, ld Or, ld H0, ld val[3], ld *grad /* [3*N_WRT] or NULL */) {
+    ld base[N_OBS], bgrad[N_OBS * N_WRT];
+    int rc = oracle_observables(z, Om, OL, Or, H0, base, bgrad);
+    if (rc < 0) {
+        for (int i = 0; i < 3; ++i) val[i] = NAN;
+        if (grad) for (int i = 0; i < 3 * N_WRT; ++i) grad[i] = NAN;
+        return -1;
+    }
+    ld (*bg)[N_WRT] = (ld (*)[N_WRT])bgrad;
+    ld x = 1.0L + z, Ok = 1.0L - Om - OL - Or, dH = C_KM_S / H0, tH = HUBBLE_GYR / H0;
+    ld I0 = base[OBS_DC] / dH;
+    /* D_A */
+    val[0] = base[OBS_DM] / x;
+    /* V_C */
+    ld v, dv_dk, F, Fi, Fk;
+    volume_transform(Ok, I0, &v, &dv_dk);
+    sinn_transform(Ok, I0, &F, &Fi, &Fk);
+    const ld FOURPI = 12.566370614359172953850573533118L;
+    val[1] = FOURPI * dH * dH * dH * v;
+    /* age */
+    cosmo_t c = { Om, OL, Or, Ok, 3 };
+    ld smax = sqrtl(1.0L / x), K0[4], G0[4], tol[4], acc[4] = {0, 0, 0, 0};
+    age_grad_panel(&c, 0.0L, smax, K0, G0);
+    for (int i = 0; i < 4; ++i) tol[i] = GK_TOL * fabsl(K0[i]) + 1e-30L;
+    int npanels = 0;
+    age_grad_adapt(&c, 0.0L, smax, tol, 0, acc, &npanels);
+    val[2] = tH * acc[0];
+    if (!grad) return rc;
+    ld (*g)[N_WRT] = (ld (*)[N_WRT])grad;
+    for (int w = 0; w < N_WRT; ++w) g[0][w] = bg[OBS_DM][w] / x;
+    g[0][WRT_Z] -= base[OBS_DM] / (x * x);
+    /* dv = F^2 dI0 + dv_dk dk ; dI0/dtheta = grad(DC)/dH (params), dI0/dz = 1/E */
+    ld E = sqrtl(Or * x * x * x * x + Om * x * x * x + Ok * x * x + OL);
+    g[1][WRT_Z] = FOURPI * dH * dH * dH * F * F / E;
+    for (int p = 0; p < 3; ++p) {
+        ld dI = bg[OBS_DC][WRT_OM + p] / dH;
+        g[1][WRT_OM + p] = FOURPI * dH * dH * dH * (F * F * dI - dv_dk);
+    }
+    g[1][WRT_H0] = -3.0L * val[1] / H0;
+    g[2][WRT_Z] = -tH / (x * E);
+    for (int p = 0; p < 3; ++p) g[2][WRT_OM + p] = tH * (-0.5L) * acc[1 + p];
+    g[2][WRT_H0] = -val[2] / H0;
+    return rc;
+}
+
+void oracle_derived_batch(int64_t n, const double *z, const double *Om, const double *OL, const double *Or,
+                          const double *H0, int64_t n_cosmo, ld *val, ld *grad, int32_t *status) {
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < n; ++i) {
+        int64_t j = (n_cosmo == 1) ? 0 : i;
+        int rc = oracle_derived((ld)z[i], (ld)Om[j], (ld)OL[j], (ld)Or[j], (ld)H0[j], val + i * 3, grad ? grad + i * 3 * N_WRT : NULL);
+        if (status) status[i] = rc;
+    }
+}
+
+/* ======================================================================================
  * (5) SN Ia Gaussian mu-likelihood: mu_obs_n | mu_n ~ N(mu_n, sigma_n^2)
  *     logL = sum_n [ -1/2 ((mu_obs_n - mu_n)/sigma_n)^2 - ln sigma_n - 1/2 ln 2 pi ]
  *     dlogL/dtheta = sum_n ((mu_obs_n - mu_n)/sigma_n^2) dmu_n/dtheta,  theta in (Om, OL, Or, H0)
