@@ -8,7 +8,9 @@
  * evaluated in closed form by Carlson's symmetric integrals R_F, R_J, R_D, R_C, eqs. (3.7)-(3.9)
  * and (B.1)-(B.3) when Or = 0, plus the derived observables of PAPER.md:95 and :277 fn.22:
  *   D_C = chi;  D_M = (c/H0) sinn(sqrt|Ok| I0)/sqrt|Ok|  (sin for Ok<0, sinh for Ok>0);  D_L = (1+z) D_M;
- *   mu = 5 log10(D_L / 10 pc);  t_L = t;  d_abs.
+ *   mu = 5 log10(D_L / 10 pc);  t_L = t;  d_abs;
+ *   and D_A = D_M/(1+z) [Mpc], the comoving volume of the whole sky out to z,
+ *   V_C = 4 pi int_0^chi D_M^2 dchi' [Mpc^3], and the age at z, int_z^inf of eq. (2.4) [Gyr].
  * and their analytic gradients with respect to z and (Om, OL, Or, H0), Ok eliminated.
  *
  * Units: H0 in km/s/Mpc; distances in Mpc (c = 299792.458 km/s); t_L in Gyr (1/H0 = 977.7922216807891/H0 Gyr); mu in mag.
@@ -44,7 +46,8 @@ extern "C" {
 typedef enum { COSMO_ELEMENTWISE = 0, COSMO_OUTER = 1 } cosmo_mode;
 
 /* `which` bitmask; the selected planes are stored in ascending bit order: out[plane][row][n]. */
-enum { COSMO_DC = 1, COSMO_DM = 2, COSMO_DL = 4, COSMO_MU = 8, COSMO_TL = 16, COSMO_DABS = 32 };
+enum { COSMO_DC = 1, COSMO_DM = 2, COSMO_DL = 4, COSMO_MU = 8, COSMO_TL = 16, COSMO_DABS = 32,
+       COSMO_DA = 64, COSMO_VC = 128, COSMO_AGE = 256 };
 
 enum {
     COSMO_OK = 0,

@@ -13,9 +13,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libcosmo_b200.so")
 
 ELEMENTWISE, OUTER = 0, 1
-DC, DM, DL, MU, TL, DABS = 1, 2, 4, 8, 16, 32
-WHICH_BITS = {"DC": DC, "DM": DM, "DL": DL, "MU": MU, "TL": TL, "DABS": DABS}
-WHICH_ORDER = ("DC", "DM", "DL", "MU", "TL", "DABS")
+DC, DM, DL, MU, TL, DABS, DA, VC, AGE = 1, 2, 4, 8, 16, 32, 64, 128, 256
+WHICH_BITS = {"DC": DC, "DM": DM, "DL": DL, "MU": MU, "TL": TL, "DABS": DABS, "DA": DA, "VC": VC, "AGE": AGE}
+WHICH_ORDER = ("DC", "DM", "DL", "MU", "TL", "DABS", "DA", "VC", "AGE")
 
 # every symbol include/cosmo_b200.h declares
 SYMBOLS = ("cosmo_workspace_bytes", "cosmo_eval", "cosmo_vjp", "cosmo_snia_loglike", "cosmo_eval_f32", "cosmo_vjp_f32",

@@ -86,7 +86,7 @@ int check_common(const void* z, int64_t n_z, const cosmo_params& p, int64_t n_co
 
 template <typename T, int MODE>
 int launch_outer(OuterArgs& a, dim3 grid, cudaStream_t st) {
-    const bool kT = a.which & W_TL, kA = a.which & W_DABS;
+    const bool kT = a.which & (W_TL | W_AGE), kA = a.which & W_DABS;
     prof_begin(st);
     if (MODE == MODE_SNIA) k_outer<T, false, false, MODE, W_MU><<<grid, OUTER_THREADS, 0, st>>>(a);
     else if (kT && kA) k_outer<T, true, true, MODE, 0><<<grid, OUTER_THREADS, 0, st>>>(a);
@@ -101,7 +101,7 @@ int launch_outer(OuterArgs& a, dim3 grid, cudaStream_t st) {
 template <typename T, bool kG>
 int launch_elem(const T* z, const cosmo_params& p, int64_t N, unsigned which, const T* gout, T* out, T* gz, double* gparams,
                 uint8_t* status, cudaStream_t st) {
-    const bool kT = which & W_TL, kA = which & W_DABS;
+    const bool kT = which & (W_TL | W_AGE), kA = which & W_DABS;
     dim3 grid((unsigned)cdiv(N, ELEM_THREADS));
     prof_begin(st);
     if (kT && kA) k_elem<T, true, true, kG><<<grid, ELEM_THREADS, 0, st>>>(z, p.Om, p.OL, p.Or, p.H0, N, which, gout, out, gz, gparams, status);
@@ -136,8 +136,8 @@ int run_eval(const T* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode,
     if (ws_bytes < L.total || !ws) return ws ? COSMO_E_WORKSPACE : COSMO_E_NULL;
     char* w = static_cast<char*>(ws);
     Cosmo<double>* consts = reinterpret_cast<Cosmo<double>*>(w + L.consts);
-    const bool kT = which & W_TL, kA = which & W_DABS;
-    k_prep<<<(unsigned)cdiv(n_cosmo, 64), 64, 0, st>>>(p.Om, p.OL, p.Or, p.H0, n_cosmo, with_grad ? ((kT || kA) ? 2 : 1) : 0, consts);
+    const bool kT = which & (W_TL | W_AGE), kA = which & W_DABS;
+    k_prep<<<(unsigned)cdiv(n_cosmo, 64), 64, 0, st>>>(p.Om, p.OL, p.Or, p.H0, n_cosmo, (with_grad ? ((kT || kA) ? 2 : 1) : 0) | ((which & W_AGE) ? 4 : 0), consts);
     if ((rc = check_launch())) return rc;
     OuterArgs a{};
     a.z = z; a.gout = gout; a.out = out; a.status = status; a.consts = consts;

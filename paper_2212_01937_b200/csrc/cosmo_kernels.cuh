@@ -57,12 +57,14 @@ __global__ void k_prep(const double* __restrict__ Om, const double* __restrict__
     int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (s >= S) return;
     Cosmo<double> C;
-    cosmo_prep(Om[s], OL[s], Or[s], H0[s], want_grad, C);
-    if (want_grad < 2) {
+    cosmo_prep(Om[s], OL[s], Or[s], H0[s], want_grad & 3, C);
+    if (want_grad & 4) prep_age(C, (want_grad & 3) != 0);
+    else { C.Tinf = 0.0; C.dTinf[0] = C.dTinf[1] = C.dTinf[2] = 0.0; }
+    if ((want_grad & 3) < 2) {
         for (int t = 0; t < 3; ++t) {
             for (int j = 0; j < 7; ++j) C.GA[t][j] = 0.0;
             for (int j = 0; j < 5; ++j) C.GJ[t][j] = C.GJ[t + 2][j] = 0.0;
-            if (want_grad < 1) { for (int j = 0; j < 5; ++j) C.GI[t][j] = 0.0; for (int j = 0; j < 6; ++j) C.GT[t][j] = 0.0; }
+            if ((want_grad & 3) < 1) { for (int j = 0; j < 5; ++j) C.GI[t][j] = 0.0; for (int j = 0; j < 6; ++j) C.GT[t][j] = 0.0; }
         }
     }
     out[s] = C;
@@ -134,7 +136,7 @@ __device__ __noinline__ void outer_c4_row(const OuterArgs& a, const Cosmo<T>& C,
         } else if (live) {
             if (a.out != nullptr) {
                 int pl = 0;
-                for (int w = 0; w < 6; ++w) {
+                for (int w = 0; w < N_PLANES; ++w) {
                     if (!(which >> w & 1)) continue;
                     static_cast<T*>(a.out)[((int64_t)pl * S + row) * N + n0 + k] = O.v[w];
                     ++pl;
@@ -214,14 +216,14 @@ __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) 
             T pacc[NP];
 #pragma unroll
             for (int j = 0; j < NP; ++j) pacc[j] = T(0);
-            T g[KZ][6];
+            T g[KZ][N_PLANES];
             if (MODE == MODE_VJP) {
 #pragma unroll
                 for (int k = 0; k < KZ; ++k)
 #pragma unroll
-                    for (int w = 0; w < 6; ++w) g[k][w] = T(0);
+                    for (int w = 0; w < N_PLANES; ++w) g[k][w] = T(0);
                 int pl = 0;
-                for (int w = 0; w < 6; ++w) {
+                for (int w = 0; w < N_PLANES; ++w) {
                     if (!(which >> w & 1)) continue;
                     T t[KZ];
                     load2<T>(static_cast<const T*>(a.gout) + ((int64_t)pl * S + row) * N, n0, N, vec, t);
@@ -230,7 +232,7 @@ __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) 
                     ++pl;
                 }
             }
-            T ov[6][KZ];
+            T ov[N_PLANES][KZ];
             uint8_t stv[KZ];
             Core<T> R[KZ];
             eval_core_k<T, kT, kA, kG, KZ, VoteWarp>(C, zv, vote, R);
@@ -239,11 +241,11 @@ __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) 
                 Obs<T> O;
                 observables<T, kT, kA>(C, zv[k], R[k], MODE == MODE_SNIA ? (unsigned)W_MU : which, O);
 #pragma unroll
-                for (int w = 0; w < 6; ++w) ov[w][k] = O.v[w];
+                for (int w = 0; w < N_PLANES; ++w) ov[w][k] = O.v[w];
                 stv[k] = (uint8_t)O.status;
                 if (MODE == MODE_SNIA) {
                     const T resid = mo[k] - O.v[3];
-                    T gg[6] = {T(0), T(0), T(0), resid * isig2[k], T(0), T(0)};
+                    T gg[N_PLANES] = {T(0), T(0), T(0), resid * isig2[k], T(0), T(0), T(0), T(0), T(0)};
                     T dummy = T(0), gp[4] = {T(0), T(0), T(0), T(0)};
                     backward<T, false, false>(C, zv[k], R[k], O, gg, dummy, gp);
                     const T ll = Num<T>::fma_(T(-0.5) * resid, resid * isig2[k], lnorm[k]);
@@ -265,7 +267,7 @@ __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) 
             }
             if (MODE != MODE_SNIA && a.out != nullptr) {
                 int pl = 0;
-                for (int w = 0; w < 6; ++w) {
+                for (int w = 0; w < N_PLANES; ++w) {
                     if (!(which >> w & 1)) continue;
                     store2<T>(static_cast<T*>(a.out) + ((int64_t)pl * S + row) * N, n0, N, vec, ov[w]);
                     ++pl;
@@ -350,6 +352,8 @@ __global__ void __launch_bounds__(ELEM_THREADS) k_elem(const T* __restrict__ z, 
     {
         Cosmo<double> Cd;
         cosmo_prep(Om[ii], OL[ii], Or[ii], H0[ii], kG ? ((kT || kA) ? 2 : 1) : 0, Cd);
+        if (kT && (which & W_AGE)) prep_age(Cd, kG);
+        else { Cd.Tinf = 0.0; Cd.dTinf[0] = Cd.dTinf[1] = Cd.dTinf[2] = 0.0; }
         convert_cosmo<T>(Cd, C);
     }
     const T zv = z[ii];
@@ -362,7 +366,7 @@ __global__ void __launch_bounds__(ELEM_THREADS) k_elem(const T* __restrict__ z, 
     if (!live) return;
     if (out != nullptr) {
         int pl = 0;
-        for (int w = 0; w < 6; ++w) {
+        for (int w = 0; w < N_PLANES; ++w) {
             if (!(which >> w & 1)) continue;
             out[(int64_t)pl * N + i] = O.v[w];
             ++pl;
@@ -370,9 +374,9 @@ __global__ void __launch_bounds__(ELEM_THREADS) k_elem(const T* __restrict__ z, 
     }
     if (status != nullptr && !kG) status[i] = (uint8_t)O.status;
     if (kG) {
-        T g[6];
+        T g[N_PLANES];
         int pl = 0;
-        for (int w = 0; w < 6; ++w) {
+        for (int w = 0; w < N_PLANES; ++w) {
             g[w] = T(0);
             if (!(which >> w & 1)) continue;
             g[w] = gout[(int64_t)pl * N + i];

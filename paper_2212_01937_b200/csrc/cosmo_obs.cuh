@@ -13,8 +13,9 @@ namespace cb {
 
 template <typename T>
 struct Obs {
-    T v[6];            // DC, DM, DL, MU, TL, DABS
+    T v[N_PLANES];     // DC, DM, DL, MU, TL, DABS, DA, VC, AGE
     T F, Fi, Fk;       // curvature transform and its partials
+    T Vk;              // d(V_C / (4 pi dH^3)) / dOk at fixed I0 (W_VC only)
     unsigned status;
 };
 
@@ -28,6 +29,43 @@ CB_HD void apply_c4(const Cosmo<T>& C, T z, Core<T>& R) {
     R.I0 = (T)I0; R.TT = (T)TT; R.AA = (T)AA;
     R.K = T(NAN); R.iE = T(NAN);
     R.status = C.status | ((T(1) + z > T(0)) ? 0u : (unsigned)ST_UNSUPPORTED) | (kGrad ? (unsigned)ST_GRAD_ILLCOND : 0u);
+}
+
+// Comoving volume over the whole sky, V_C = 4 pi dH^3 v, v(k, I0) = int_0^{I0} F(k, I)^2 dI (ref. [59] eq. (13.60)):
+//   v = I0^3 h(w), dv/dk = I0^5 h'(w), w = Ok I0^2, h = sum_{j>=1} 4^j w^(j-1) / (2 (2j+1)!)  (|w| <= 1), closed forms beyond;
+//   dv/dI0 = F^2.
+template <typename T>
+CB_HD void volume(T k, T I0, T& v, T& vk) {
+    using N = Num<T>;
+    const T w = k * I0 * I0;
+    const T I3 = I0 * I0 * I0;
+    if (N::abs_(w) <= T(1)) {
+        // coefficients 4^j / (2 (2j+1)!), j = 1..12
+        const double H[12] = {1.0 / 3.0, 1.0 / 15.0, 2.0 / 315.0, 1.0 / 2835.0, 2.0 / 155925.0, 2.0 / 6081075.0, 4.0 / 638512875.0,
+                              1.0 / 10854718875.0, 2.0 / 1856156927625.0, 2.0 / 194896477400625.0, 4.0 / 49308808782358125.0,
+                              2.0 / 3698160658676859375.0};
+        T sh = T(H[11]), sd = T(11.0 * H[11]);
+#pragma unroll
+        for (int j = 10; j >= 0; --j) {
+            sh = N::fma_(sh, w, T(H[j]));
+            if (j >= 1) sd = N::fma_(sd, w, T(j * H[j]));
+        }
+        v = I3 * sh;
+        vk = I3 * I0 * I0 * sd;
+        return;
+    }
+    if (k > T(0)) {
+        const T sq = N::sqrt_(k), y2 = T(2) * sq * I0, ey = N::exp_(y2), iey = T(1) / ey;
+        const T sh2 = T(0.5) * (ey - iey), ch2 = T(0.5) * (ey + iey);
+        v = (sh2 / (T(2) * sq) - I0) / (T(2) * k);
+        vk = (I0 * ch2 / (T(2) * k) - sh2 / (T(4) * k * sq)) / (T(2) * k) - v / k;
+    } else {
+        const T kk = -k, sq = N::sqrt_(kk);
+        T sn2, cs2;
+        N::sincos_(T(2) * sq * I0, &sn2, &cs2);
+        v = (I0 - sn2 / (T(2) * sq)) / (T(2) * kk);
+        vk = -((-(I0 * cs2 / (T(2) * kk) - sn2 / (T(4) * kk * sq))) / (T(2) * kk) - v / kk);
+    }
 }
 
 template <typename T, bool kT, bool kA>
@@ -46,18 +84,53 @@ CB_HD void observables(const Cosmo<T>& C, T z, const Core<T>& R, unsigned which,
     }
     O.v[4] = kT ? C.tH * R.TT : T(0);
     O.v[5] = kA ? C.dH * R.AA : T(0);
+    O.v[6] = O.v[7] = O.v[8] = T(0);
+    O.Vk = T(0);
+    if (which & W_DA) O.v[6] = O.v[1] / x;
+    if (which & W_VC) {
+        T v;
+        volume<T>(C.Ok, R.I0, v, O.Vk);
+        O.v[7] = T(12.566370614359172954) * C.dH * C.dH * C.dH * v;
+    }
+    if (kT && (which & W_AGE)) O.v[8] = C.tH * (C.Tinf - R.TT);
     if (st & (ST_ROOT_ON_PATH | ST_UNSUPPORTED)) {
 #pragma unroll
-        for (int i = 0; i < 6; ++i) O.v[i] = T(NAN);
+        for (int i = 0; i < N_PLANES; ++i) O.v[i] = T(NAN);
     }
     O.status = st;
 }
 
-// VJP of one element: g[6] upstream (entries outside `which` must be 0).  Adds to gz and gp[0..3] = (Om, OL, Or, H0).
+// Age (int_z^inf of eq. (2.4)): age(z) = tH (Tinf - T(z)).  Tinf = int_1^inf dx/(x E) is one more evaluation of
+// eq. (3.8) per cosmology at x = 1e10 (the formula is scale-free) plus the analytic remainder of the integrand's leading
+// term beyond it (< 2e-15); its parameter derivatives use the same T-basis at that point.  FP64; called after cosmo_prep.
+CB_HD void prep_age(Cosmo<double>& C, bool with_grad) {
+    C.Tinf = NAN; C.dTinf[0] = C.dTinf[1] = C.dTinf[2] = NAN;
+    if ((C.cubic & 2u) || C.status) return;
+    const double X = 1.0e10, z = X - 1.0;
+    Core<double> R;
+    eval_core<double, true, false, true, VoteNone>(C, z, VoteNone(), R);
+    if (R.status) return;
+    const double tail = (C.Or * X > C.Om) ? 0.5 / (sqrt(C.Or) * X * X) : (2.0 / 3.0) / (sqrt(C.Om) * X * sqrt(X));
+    C.Tinf = R.TT + tail;
+    if (!with_grad) return;
+    const double iE = R.iE;
+    const double bt0 = -R.Em1 * iE, bt1 = (z - R.Em1) * iE, bt2 = (z * (X + 1.0) - R.Em1) * iE;
+    for (int t = 0; t < 3; ++t)
+        C.dTinf[t] = -0.5 * (C.GT[t][0] * R.I0 + C.GT[t][1] * R.K + C.GT[t][2] * bt0 + C.GT[t][3] * bt1 + C.GT[t][4] * bt2
+                             + C.GT[t][5] * R.TT);
+    // remainder beyond X of the Or-derivative, -1/2 int_X^inf (x^3 - x)/E^3 dx with E^2 ~ x^3 (Or x + Om): it decays only like
+    // X^(-1/2) while matter dominates at X (2e-5/Om^1.5 at Or = 0); the Om and OL remainders are O(X^-3/2) and dropped.
+    double rem;
+    if (C.Or * X > 1.0e3 * C.Om) rem = 0.5 / (C.Or * sqrt(C.Or) * X * X);
+    else rem = 2.0 * (2.0 * C.Or * X + C.Om) / (C.Om * C.Om * sqrt(X) * sqrt(C.Or * X + C.Om)) - 4.0 * sqrt(C.Or) / (C.Om * C.Om);
+    C.dTinf[2] -= 0.5 * rem;
+}
+
+// VJP of one element: g[N_PLANES] upstream (entries outside `which` must be 0).  Adds to gz and gp[0..3] = (Om, OL, Or, H0).
 // kCond: also return in *cond the cancellation factor max_theta sum_j |G_j basis_j| / max(|dI0/dtheta|, 1e-3 |I0|) of the
 // chi-family gradient (status bit 16 of the ELEMENTWISE calls is derived from it).
 template <typename T, bool kT, bool kA, bool kCond = false>
-CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, const T g[6], T& gz, T gp[4], T* cond = nullptr) {
+CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, const T g[N_PLANES], T& gz, T gp[4], T* cond = nullptr) {
     using N = Num<T>;
     const T x = T(1) + z;
     const T iE = R.iE;
@@ -69,8 +142,14 @@ CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, c
     const T bt0 = -R.Em1 * iE, bt1 = (n1 - R.Em1) * iE, bt2 = (n2 - R.Em1) * iE;
     T gM = g[1] + x * g[2];
     if (g[3] != T(0)) gM += T(CB_KT.five_over_ln10) * g[3] * (x * rxd);
-    const T aI = C.dH * N::fma_(gM, O.Fi, g[0]);
-    const T aK = -gM * C.dH * O.Fk;
+    if (g[6] != T(0)) gM += g[6] * ix;                                  // D_A = D_M / (1+z)
+    T aI = C.dH * N::fma_(gM, O.Fi, g[0]);
+    T aK = -gM * C.dH * O.Fk;
+    if (g[7] != T(0)) {                                                 // V_C = 4 pi dH^3 v(Ok, I0): dv = F^2 dI0 + v_k dOk
+        const T c4pi = T(12.566370614359172954) * C.dH * C.dH * C.dH * g[7];
+        aI = N::fma_(c4pi, O.F * O.F, aI);
+        aK = N::fma_(-c4pi, O.Vk, aK);
+    }
     T btA = T(0);
     if (kA) btA = (((C.cubic & 1u) ? n4 : n3) - R.Em1) * iE;
     // d_abs gradient where radiation is a perturbation: the exact basis above then multiplies the forward A by ~3/Or
@@ -118,7 +197,8 @@ CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, c
         T acc = N::fma_(aI, T(-0.5) * dI, aK);
         if (kT) {
             T dT = C.GT[t][0] * R.I0 + C.GT[t][1] * R.K + C.GT[t][2] * bt0 + C.GT[t][3] * bt1 + C.GT[t][4] * bt2 + C.GT[t][5] * R.TT;
-            acc = N::fma_(g[4] * C.tH, T(-0.5) * dT, acc);
+            acc = N::fma_((g[4] - g[8]) * C.tH, T(-0.5) * dT, acc);       // t_L = tH T, age = tH (Tinf - T)
+            acc = N::fma_(g[8] * C.tH, C.dTinf[t], acc);
         }
         if (kA) {
             T dA = C.GA[t][0] * R.I0 + C.GA[t][1] * R.K + C.GA[t][2] * bt0 + C.GA[t][3] * bt1 + C.GA[t][4] * bt2 + C.GA[t][5] * btA
@@ -129,12 +209,14 @@ CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, c
         gp[t] += acc;
     }
     T h = g[0] * O.v[0] + g[1] * O.v[1] + g[2] * O.v[2] + g[3] * T(CB_KT.five_over_ln10);
-    if (kT) h += g[4] * O.v[4];
+    if (kT) h += g[4] * O.v[4] + g[8] * O.v[8];
     if (kA) h += g[5] * O.v[5];
+    h += g[6] * O.v[6] + T(3) * g[7] * O.v[7];
     gp[3] -= h * C.dH * T(1.0 / C_KM_S);        // / H0
     T dz = aI * iE + g[2] * O.v[1];
     if (g[3] != T(0)) dz += T(CB_KT.five_over_ln10) * g[3] * ix;
-    if (kT) dz += g[4] * C.tH * iE * ix;
+    if (kT) dz += (g[4] - g[8]) * C.tH * iE * ix;
+    if (g[6] != T(0)) dz -= g[6] * O.v[6] * ix;
     if (kA) dz += g[5] * C.dH * x * x * iE;
     gz += dz;
 }

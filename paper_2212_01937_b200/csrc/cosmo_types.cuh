@@ -57,7 +57,8 @@ static const KTab KT_host = CB_KTAB_INIT;
 #endif
 
 // `which` bits, planes in ascending bit order (include/cosmo_b200.h)
-enum : unsigned { W_DC = 1, W_DM = 2, W_DL = 4, W_MU = 8, W_TL = 16, W_DABS = 32, W_ALL = 63 };
+enum : unsigned { W_DC = 1, W_DM = 2, W_DL = 4, W_MU = 8, W_TL = 16, W_DABS = 32, W_DA = 64, W_VC = 128, W_AGE = 256, W_ALL = 511 };
+constexpr int N_PLANES = 9;                        // number of `which` bits
 // status bits (include/cosmo_b200.h)
 enum : unsigned { ST_ROOT_ON_PATH = 1, ST_UNSUPPORTED = 2, ST_DL_NONPOS = 4, ST_ITER_CAP = 8, ST_GRAD_ILLCOND = 16 };
 // cancellation factor of the chi-family gradient above which 1e-8 is no longer guaranteed (calibrated against the oracle
@@ -89,12 +90,13 @@ struct Cosmo {
     T GI[3][5];        // X = I0 : basis (I0, K, b0, b1, b2)
     T GT[3][6];        // X = T  : basis (I0, K, b0, b1, b2, T)
     T GA[3][7];        // X = A  : basis (I0, K, b0, b1, b2, b3 (b4 when Or = 0), A)
+    T Tinf, dTinf[3];  // int_1^inf dx/(x E) and its derivatives wrt (Om, OL, Or): age(z) = tH (Tinf - T(z))  (W_AGE only)
     T GJ[5][5];        // J'_p = int x^p dx / E^3, p = 0..4, over the basis (I0, K, b0, b1, b2)  (d_abs gradient)
     unsigned status;
     unsigned cubic;    // bit 0: Or == 0 (cubic case, appendix B.1);  bit 1: two complex pairs (cosmo_c4.cuh; m, rn hold g1, h1)
 };
 
-constexpr int COSMO_NFIELDS = 111;   // floating-point members of Cosmo<T>, in declaration order
+constexpr int COSMO_NFIELDS = 115;   // floating-point members of Cosmo<T>, in declaration order
 static_assert(sizeof(Cosmo<double>) == COSMO_NFIELDS * sizeof(double) + 2 * sizeof(unsigned), "Cosmo<T> layout");
 static_assert(sizeof(Cosmo<float>) == COSMO_NFIELDS * sizeof(float) + 2 * sizeof(unsigned), "Cosmo<T> layout");
 

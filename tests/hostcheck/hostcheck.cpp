@@ -14,6 +14,8 @@ static void run(int64_t n, const double* z, const double* Om, const double* OL, 
     for (int64_t i = 0; i < n; ++i) {
         Cosmo<double> Cd;
         cosmo_prep(Om[i], OL[i], Or[i], H0[i], gup ? 2 : 0, Cd);
+        if (which & W_AGE) prep_age(Cd, gup != nullptr);
+        else { Cd.Tinf = 0; Cd.dTinf[0] = Cd.dTinf[1] = Cd.dTinf[2] = 0; }
         Cosmo<T> C;
         convert_cosmo<T>(Cd, C);
         Core<T> R;
@@ -22,11 +24,11 @@ static void run(int64_t n, const double* z, const double* Om, const double* OL, 
         if (gup) apply_c4<T, true, true, true>(C, (T)z[i], R); else apply_c4<T, true, true, false>(C, (T)z[i], R);
         Obs<T> O;
         observables<T, true, true>(C, (T)z[i], R, which, O);
-        for (int w = 0; w < 6; ++w) out[w * n + i] = (double)O.v[w];
+        for (int w = 0; w < N_PLANES; ++w) out[w * n + i] = (double)O.v[w];
         status[i] = (uint8_t)O.status;
         if (gup) {
-            T g[6], a = 0, p[4] = {0, 0, 0, 0};
-            for (int w = 0; w < 6; ++w) g[w] = (which >> w & 1) ? (T)gup[w * n + i] : T(0);
+            T g[N_PLANES], a = 0, p[4] = {0, 0, 0, 0};
+            for (int w = 0; w < N_PLANES; ++w) g[w] = (which >> w & 1) ? (T)gup[w * n + i] : T(0);
             T cond = 0;
             backward<T, true, true, true>(C, (T)z[i], R, O, g, a, p, &cond);
             if (cond_out) cond_out[i] = (double)cond;

@@ -471,3 +471,50 @@ def test_outer_equals_elementwise(cb, N, S):
     gpe = gp_e.cpu().numpy().reshape(4, S, N)
     assert (np.abs(gp.cpu().numpy() - gpe.sum(axis=2)) <= 1e-12 * np.abs(gpe).sum(axis=2)).all()
     assert np.array_equal(st.cpu().numpy() & 15, st_e.cpu().numpy().reshape(S, N) & 15)
+
+
+# ---------------------------------------------------------------- D_A, comoving volume, age
+@pytest.mark.parametrize("mode", ["outer", "elementwise"])
+def test_derived_observables(cb, mode):
+    rng = np.random.default_rng(21)
+    which = ("DC", "TL", "DA", "VC", "AGE")
+    if mode == "outer":
+        N, S = 1501, 5
+        z = np.sort(rng.uniform(0.01, 6.0, N))
+        Om = rng.uniform(0.15, 0.5, S); OL = rng.uniform(0.3, 1.0, S); Or = np.array([0.0, 9e-5, 1e-3, 1e-5, 0.0]); H0 = rng.uniform(60, 80, S)
+        g = rng.standard_normal((5, S, N))
+        gz, gp, out, st = cb.cosmo_vjp(dev(z), dev(Om), dev(OL), dev(Or), dev(H0), dev(g), cb.OUTER, which, want_out=True)
+        out, gz, gp = out.cpu().numpy(), gz.cpu().numpy(), gp.cpu().numpy()
+        gz_ref = np.zeros(N); gz_abs = np.zeros(N)
+        for s in range(S):
+            val, grad, _ = oracle_batch(z, Om[s:s + 1], OL[s:s + 1], Or[s:s + 1], H0[s:s + 1], True)
+            dv, dg, _ = oracle.derived_batch(z, Om[s:s + 1], OL[s:s + 1], Or[s:s + 1], H0[s:s + 1])
+            dv, dg = dv.astype(np.float64), dg.astype(np.float64)
+            refs = [(val[:, 0], grad[:, 0]), (val[:, 4], grad[:, 4]), (dv[:, 0], dg[:, 0]), (dv[:, 1], dg[:, 1]), (dv[:, 2], dg[:, 2])]
+            sums = np.zeros(4); sabs = np.zeros(4)
+            for k, (v, gr) in enumerate(refs):
+                assert relerr(out[k, s], v).max() <= TOL_VAL, (which[k], s)
+                gz_ref += g[k, s] * gr[:, 0]; gz_abs += np.abs(g[k, s] * gr[:, 0])
+                for p in range(4):
+                    sums[p] += (g[k, s] * gr[:, 1 + p]).sum(); sabs[p] += np.abs(g[k, s] * gr[:, 1 + p]).sum()
+            assert (np.abs(gp[:, s] - sums) <= TOL_GRAD * sabs).all(), s
+        assert (np.abs(gz - gz_ref) <= TOL_GRAD * gz_abs).all()
+    else:
+        n = 20_000
+        w = W.config2(n=n)
+        g = rng.standard_normal((5, 1, n))
+        gz, gp, out, st = cb.cosmo_vjp(dev(w.z), dev(w.Om), dev(w.OL), dev(w.Or), dev(w.H0), dev(g), cb.ELEMENTWISE, which, want_out=True)
+        out, gz, gp, st = out.cpu().numpy()[:, 0], gz.cpu().numpy(), gp.cpu().numpy(), st.cpu().numpy()[0]
+        ok = (st & 16) == 0
+        assert ok.mean() > 0.99
+        val, grad, _ = oracle_batch(w.z, w.Om, w.OL, w.Or, w.H0, True)
+        dv, dg, _ = oracle.derived_batch(w.z, w.Om, w.OL, w.Or, w.H0)
+        dv, dg = dv.astype(np.float64), dg.astype(np.float64)
+        refs = [(val[:, 0], grad[:, 0]), (val[:, 4], grad[:, 4]), (dv[:, 0], dg[:, 0]), (dv[:, 1], dg[:, 1]), (dv[:, 2], dg[:, 2])]
+        mine = np.vstack([gz[None], gp])
+        for p in range(5):
+            ref = sum(g[k, 0] * gr[:, p] for k, (v, gr) in enumerate(refs))
+            sab = sum(np.abs(g[k, 0] * gr[:, p]) for k, (v, gr) in enumerate(refs))
+            assert (np.abs(mine[p] - ref)[ok] <= TOL_GRAD * sab[ok]).all(), p
+        for k, (v, gr) in enumerate(refs):
+            assert relerr(out[k], v)[ok].max() <= TOL_VAL, which[k]

@@ -38,7 +38,7 @@ def hc():
 def run(hc, z, Om, OL, Or, H0, which=63, gup=None, f32=False):
     n = len(z)
     arrs = [np.ascontiguousarray(np.broadcast_to(np.asarray(a, dtype=np.float64), (n,))) for a in (z, Om, OL, Or, H0)]
-    out = np.zeros((6, n)); gz = np.zeros(n); gp = np.zeros((4, n)); st = np.zeros(n, dtype=np.uint8)
+    out = np.zeros((9, n)); gz = np.zeros(n); gp = np.zeros((4, n)); st = np.zeros(n, dtype=np.uint8)
     dp = lambda a: a.ctypes.data_as(DP) if a is not None else None
     f = hc.hostcheck_f32 if f32 else hc.hostcheck_f64
     f(C.c_int64(n), *[dp(a) for a in arrs], C.c_uint(which), dp(gup), dp(out), dp(gz), dp(gp), st.ctypes.data_as(C.POINTER(C.c_uint8)))
@@ -151,6 +151,24 @@ def test_two_complex_pairs_slow_path(hc):
     g1 = np.zeros((6, n)); g1[0] = 1
     _, gz, gp, st = run(hc, z, Om, OL, Or, H0, 63, g1)
     assert np.isnan(gp[:3]).all() and ((st & 16) != 0).all()
+
+
+def test_derived_observables_host(hc):
+    """D_A, comoving volume and age (planes 64, 128, 256) with their gradients against oracle.derived_batch"""
+    for w in (W.config1(n=300), W.config2(n=800)):
+        n = w.n_z
+        bc = lambda a: np.ascontiguousarray(np.broadcast_to(a, (n,)) if a.shape[0] == 1 else a)
+        z, Om, OL, Or, H0 = w.z, bc(w.Om), bc(w.OL), bc(w.Or), bc(w.H0)
+        val, grad, _ = oracle.derived_batch(z, Om, OL, Or, H0)
+        val, grad = val.astype(np.float64), grad.astype(np.float64)
+        for i in range(3):
+            g1 = np.zeros((9, n)); g1[6 + i] = 1
+            out, gz, gp, st = run(hc, z, Om, OL, Or, H0, 511, g1)
+            assert (np.abs(out[6 + i] - val[:, i]) / np.abs(val[:, i])).max() <= 1e-12, oracle.DERIVED[i]
+            mine = np.vstack([gz[None], gp])
+            for k in range(5):
+                e = np.abs(mine[k] - grad[:, i, k]) / np.maximum(np.abs(grad[:, i, k]), 1e-3 * np.abs(val[:, i]))
+                assert e.max() <= 1e-8, (oracle.DERIVED[i], oracle.WRT[k], e.max())
 
 
 def test_host_math_fp32(hc):
