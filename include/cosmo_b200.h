@@ -101,6 +101,14 @@ int cosmo_snia_loglike_f32(const float* z, const float* mu_obs, const float* sig
 int cosmo_eval_host(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode, uint32_t which,
                     const double* grad_out, double* out, double* grad_z, double* grad_params, uint8_t* status);
 
+/* The device Carlson functions of the hot path on their own (eqs. (2.6), (2.7), (2.9); duplication
+ * algorithm of ref. [10]), in the real-symmetric form the path uses: for each i
+ *   rf[i] = R_F(x, m+h, m-h),  rd[i] = R_D(m+h, m-h, x),  rj[i] = R_J(x, m+h, m-h, p),   h^2 = s[i]
+ * with x > 0, p > 0 and either s >= 0 with m - h > 0 (three positive reals) or s < 0 (a complex-conjugate pair m +- i|h|).
+ * All arrays have length n (device pointers). */
+int cosmo_carlson_pair(const double* x, const double* m, const double* s, const double* p, int64_t n, double* rf, double* rd,
+                       double* rj, void* stream);
+
 /* ALU roofline probes: each thread runs `iters` rounds of 8 independent dependent-FMA chains (FP64 / FP32) and
  * stores one value per thread in sink[blocks*256].  flops = blocks * 256 * iters * 8 * 2.  Used by bench.py to
  * measure the DFMA / FFMA peak that the roofline fraction is quoted against. */

@@ -19,7 +19,7 @@ WHICH_ORDER = ("DC", "DM", "DL", "MU", "TL", "DABS", "DA", "VC", "AGE")
 
 # every symbol include/cosmo_b200.h declares
 SYMBOLS = ("cosmo_workspace_bytes", "cosmo_eval", "cosmo_vjp", "cosmo_snia_loglike", "cosmo_eval_f32", "cosmo_vjp_f32",
-           "cosmo_snia_loglike_f32", "cosmo_eval_host", "cosmo_probe_fma_f64", "cosmo_probe_fma_f32",
+           "cosmo_snia_loglike_f32", "cosmo_eval_host", "cosmo_carlson_pair", "cosmo_probe_fma_f64", "cosmo_probe_fma_f32",
            "cosmo_profile", "cosmo_profile_mean_ms",
            "cosmo_launch_count", "cosmo_last_cuda_error", "cosmo_strerror", "cosmo_version")
 
@@ -65,6 +65,8 @@ def lib():
         f = getattr(L, name)
         f.argtypes = [ci, ci, vp, vp]
         f.restype = ci
+    L.cosmo_carlson_pair.argtypes = [vp, vp, vp, vp, i64, vp, vp, vp, vp]
+    L.cosmo_carlson_pair.restype = ci
     L.cosmo_launch_count.restype = i64
     L.cosmo_profile.argtypes = [ci]
     L.cosmo_profile.restype = ci
@@ -234,6 +236,17 @@ def cosmo_eval_host(z, Om, OL, Or, H0, mode=ELEMENTWISE, which=("DC",), grad_out
         gp = np.empty((4, n_cosmo))
     _check(lib().cosmo_eval_host(vp(arrs[0]), n_z, P, n_cosmo, mode, mask, vp(grad_out), vp(out), vp(gz), vp(gp), vp(status)))
     return out, gz, gp, status
+
+
+def carlson_pair(x, m, s, p):
+    """R_F(x, m+h, m-h), R_D(m+h, m-h, x), R_J(x, m+h, m-h, p) with h^2 = s, by the hot path's device functions"""
+    torch = _torch()
+    for t in (x, m, s, p):
+        _dev(t, torch.float64, torch, "carlson_pair argument")
+    n = x.numel()
+    rf, rd, rj = (torch.empty(n, dtype=torch.float64, device=x.device) for _ in range(3))
+    _check(lib().cosmo_carlson_pair(_ptr(x), _ptr(m), _ptr(s), _ptr(p), n, _ptr(rf), _ptr(rd), _ptr(rj), _stream(torch)))
+    return rf, rd, rj
 
 
 def probe_fma(dtype="f64", blocks=148 * 8, iters=4096):

@@ -295,6 +295,15 @@ int cosmo_eval_host(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosm
     return COSMO_OK;
 }
 
+int cosmo_carlson_pair(const double* x, const double* m, const double* s, const double* p, int64_t n, double* rf, double* rd,
+                       double* rj, void* stream) {
+    if (n < 0) return COSMO_E_SIZE;
+    if (n == 0) return COSMO_OK;
+    if (!x || !m || !s || !p || !rf || !rd || !rj) return COSMO_E_NULL;
+    k_carlson_pair<<<(unsigned)cdiv(n, 128), 128, 0, static_cast<cudaStream_t>(stream)>>>(x, m, s, p, n, rf, rd, rj);
+    return check_launch();
+}
+
 int cosmo_probe_fma_f64(int blocks, int iters, double* sink, void* stream) {
     if (blocks <= 0 || iters < 0) return COSMO_E_SIZE;
     if (!sink) return COSMO_E_NULL;

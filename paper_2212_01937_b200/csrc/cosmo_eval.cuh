@@ -153,67 +153,18 @@ struct Core {
     unsigned status;
 };
 
-// S4-S6 for K elements of the SAME cosmology in lock-step (K independent dependency chains per thread: the FP64
-// pipe has ~9 cycles of latency and few warps fit, so instruction-level parallelism is what keeps it busy).
-// kT: lookback integral, kA: absorption integral, kK: the second-kind integral K (needs R_D).
-template <typename T, bool kT, bool kA, bool kK, int K, typename Vote>
-CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Core<T> (&R)[K]) {
+// ---- Carlson's duplication algorithm (ref. [10]; eqs. (2.6)-(2.9)) in the
+// real-symmetric form: K argument triples (xa, mp + h, mp - h), h^2 = s (s < 0: a complex-conjugate pair), advanced in
+// lock-step by lambda = sqrt(x)sqrt(y) + sqrt(x)sqrt(z) + sqrt(y)sqrt(z) until every lane of the warp meets the stopping
+// rule (no divergence).  One pass serves R_F, the R_D(., ., xa) tail (kD) and the tails of R_J(., ., ., p5) (kT) and
+// R_J(., ., ., p0) (kA); dl = (p - xa)((p - mp)^2 - s) is Carlson's delta of each R_J.  On return the arguments hold the
+// reduced values, f = 4^-n.
+template <typename T, bool kD, bool kT, bool kA, int K, typename Vote>
+CB_HD void carlson_dup(T (&xa)[K], T (&mp)[K], T (&s)[K], T (&p5)[K], T (&p0)[K], const T (&dl5)[K], const T (&dl0)[K],
+                       const T (&Qc)[K], const T (&Q5v)[K], const T (&Q0v)[K], unsigned (&st)[K], const Vote& vote, T& f,
+                       T (&tailD)[K], T (&sum5)[K], T (&sum0)[K]) {
     using N = Num<T>;
-    constexpr bool kD = kK || kA;          // R_D tail needed
-    // Only U12 and the loop state stay live across the duplication loop; everything cheap is recomputed after it
-    // (registers decide how many warps fit, DESIGN.md section 5).
-    T U12[K], ra[K], iE[K], xa[K], mp[K], s[K], Qc[K];
-    unsigned st[K];
-    T p5[K], p0[K], dl5[K], dl0[K], p5_0[K], p0_0[K], Q5v[K], Q0v[K];
-    const bool quartA = kA && !(C.cubic & 1u);
-#pragma unroll
-    for (int k = 0; k < K; ++k) {
-        const T x = T(1) + z[k];
-        const T z2 = z[k] * z[k];
-        st[k] = C.status;
-        if (!(x > T(0))) st[k] |= ST_UNSUPPORTED;
-        if (x >= C.xlim) st[k] |= ST_ROOT_ON_PATH;
-        // ---- S4 radicands
-        const T q1x = N::fma_(C.Or, x, C.m) * (x - C.rn);
-        const T q2x = N::fma_(x + C.b, x, C.c);
-        const T a1 = q1x * C.q21, a2 = C.q11 * q2x;
-        const T r1 = N::rsqrt_(a1), r2 = N::rsqrt_(a2);
-        ra[k] = a1 * r1;
-        iE[k] = r1 * r2;                                  // a1 a2 = E^2(x) E^2(1) and E(1) = 1 (sum of Omegas)
-        U12[k] = N::fma_(a2, r2, ra[k]);
-        xa[k] = U12[k] * U12[k];
-        const T hd = T(0.5) * z2 * C.theta;               // u12^2 - (u13^2 + u14^2)/2
-        mp[k] = xa[k] - hd;
-        s[k] = z2 * z2 * C.sD;
-        const T hs = z2 * C.sDr;                          // |h|
-        // ---- R_J parameters
-        p5[k] = p0[k] = dl5[k] = dl0[k] = p5_0[k] = p0_0[k] = Q5v[k] = Q0v[k] = T(0);
-        if (kT) {
-            p5[k] = N::fma_(z2, C.p5c, xa[k]);
-            p5_0[k] = p5[k];
-            const T pm = p5[k] - mp[k];
-            dl5[k] = (p5[k] - xa[k]) * N::fma_(pm, pm, -s[k]);
-        }
-        if (kA) {
-            p0[k] = quartA ? N::fma_(-C.Or * z2, C.Q2n, xa[k]) : xa[k];
-            p0_0[k] = p0[k];
-            const T pm = p0[k] - mp[k];
-            dl0[k] = (p0[k] - xa[k]) * N::fma_(pm, pm, -s[k]);
-        }
-        // ---- stopping rule (ref. [10]): 4^-n Q < |A_n| for every series that is summed.  R_F and R_D share one Q:
-        // the larger deviation bound (2/3 |xa - mp| + |h|) with the stricter constant of the two.
-        Qc[k] = (kD ? N::QJ : N::QF) * N::fma_(T(CB_KT.two_thirds), N::abs_(hd), hs);
-        if (kT) {
-            const T A0 = (xa[k] + T(2) * mp[k] + T(2) * p5[k]) * T(0.2);
-            Q5v[k] = N::QJ * N::max_(N::max_(N::abs_(A0 - xa[k]), N::abs_(A0 - mp[k]) + hs), N::abs_(A0 - p5[k]));
-        }
-        if (kA) {
-            const T A0 = (xa[k] + T(2) * mp[k] + T(2) * p0[k]) * T(0.2);
-            Q0v[k] = N::QJ * N::max_(N::max_(N::abs_(A0 - xa[k]), N::abs_(A0 - mp[k]) + hs), N::abs_(A0 - p0[k]));
-        }
-    }
-    // ---- S5 fused duplication
-    T f = T(1), tailD[K], sum5[K], sum0[K];
+    f = T(1);
 #pragma unroll
     for (int k = 0; k < K; ++k) tailD[k] = sum5[k] = sum0[k] = T(0);
     int nit = 0;
@@ -265,6 +216,135 @@ CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Cor
         f *= T(0.25);
         ++nit;
     }
+}
+
+// R_F(xa0, m0 + h0, m0 - h0) from the reduced arguments: degree-7 series in E2, E3 (DLMF 19.36.1); hd = xa0 - m0, s0 = h0^2
+template <typename T>
+CB_HD T carlson_rf_series(T xa_n, T mp_n, T f, T hd, T s0) {
+    using N = Num<T>;
+    const T An = (xa_n + T(2) * mp_n) * T(CB_KT.third);
+    const T rA = N::rsqrt_(An);
+    const T g = f * rA * rA;
+    const T dl = hd * T(CB_KT.third) * g;
+    const T vs = s0 * g * g;
+    const T e2 = T(-3) * dl * dl - vs;
+    const T e3 = T(-2) * dl * (dl * dl - vs);
+    // 1 - e2/10 + e3/14 + e2^2/24 - 3 e2 e3/44 - 5 e2^3/208 + 3 e3^2/104 + e2^2 e3/16, nested for FMAs
+    const double* c = CB_KT.rf;
+    const T ta = N::fma_(e2, N::fma_(e2, T(c[2]), T(c[1])), T(c[0]));
+    const T tb = N::fma_(e3, T(c[6]), N::fma_(e2, N::fma_(e2, T(c[5]), T(c[4])), T(c[3])));
+    const T S = N::fma_(e3, tb, N::fma_(e2, ta, T(1)));
+    return S * rA;
+}
+
+// R_D(m0 + h0, m0 - h0, xa0): series (DLMF 19.36.2) + 3 x the tail summed by carlson_dup
+template <typename T>
+CB_HD T carlson_rd_series(T xa_n, T mp_n, T f, T hd, T s0, T tailD) {
+    using N = Num<T>;
+    const T AD = (T(3) * xa_n + T(2) * mp_n) * T(0.2);
+    const T rA = N::rsqrt_(AD);
+    const T g = f * rA * rA;
+    const T dd = hd * T(0.2) * g;
+    const T XY = T(9) * dd * dd - s0 * g * g;
+    const T Z = T(-2) * dd, Z2 = Z * Z;
+    const T e2 = XY - T(6) * Z2;
+    const T e3 = (T(3) * XY - T(8) * Z2) * Z;
+    const T e4 = T(3) * (XY - Z2) * Z2;
+    const T e5 = XY * Z2 * Z;
+    return N::fma_(g * rA, series_J<T>(e2, e3, e4, e5), T(3) * tailD);
+}
+
+// R_J(xa0, m0 + h0, m0 - h0, p_init): series + 6 x the tail summed by carlson_dup
+template <typename T>
+CB_HD T carlson_rj_series(T xa_n, T mp_n, T p_n, T f, T xa0, T m0, T s0, T p_init, T sum) {
+    using N = Num<T>;
+    const T An = (xa_n + T(2) * mp_n + T(2) * p_n) * T(0.2);
+    const T A0 = (xa0 + T(2) * m0 + T(2) * p_init) * T(0.2);
+    const T rA = N::rsqrt_(An);
+    const T g = f * rA * rA;
+    const T X = (A0 - xa0) * g;
+    const T am = A0 - m0;
+    const T YpZ = T(2) * am * g;
+    const T YZ = N::fma_(am, am, -s0) * g * g;
+    const T P = T(-0.5) * (X + YpZ);
+    const T XYZ = X * YZ;
+    const T P2 = P * P;
+    const T e2 = N::fma_(X, YpZ, YZ) - T(3) * P2;
+    const T e3 = XYZ + T(2) * e2 * P + T(4) * P2 * P;
+    const T e4 = (T(2) * XYZ + e2 * P + T(3) * P2 * P) * P;
+    const T e5 = XYZ * P2;
+    return N::fma_(g * rA, series_J<T>(e2, e3, e4, e5), T(6) * sum);
+}
+
+// stopping-rule bounds (ref. [10]; constants: see Num<T>::QF): Qc for R_F / R_D, Qj for an R_J with parameter p
+template <typename T>
+CB_HD T carlson_Qc(T hd, T hs, bool with_rd) {
+    using N = Num<T>;
+    return (with_rd ? N::QJ : N::QF) * N::fma_(T(CB_KT.two_thirds), N::abs_(hd), hs);
+}
+template <typename T>
+CB_HD T carlson_Qj(T xa, T mp, T hs, T p) {
+    using N = Num<T>;
+    const T A0 = (xa + T(2) * mp + T(2) * p) * T(0.2);
+    return N::QJ * N::max_(N::max_(N::abs_(A0 - xa), N::abs_(A0 - mp) + hs), N::abs_(A0 - p));
+}
+
+// S4-S6 for K elements of the SAME cosmology in lock-step (K independent dependency chains per thread: the FP64
+// pipe has ~9 cycles of latency and few warps fit, so instruction-level parallelism is what keeps it busy).
+// kT: lookback integral, kA: absorption integral, kK: the second-kind integral K (needs R_D).
+template <typename T, bool kT, bool kA, bool kK, int K, typename Vote>
+CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Core<T> (&R)[K]) {
+    using N = Num<T>;
+    constexpr bool kD = kK || kA;          // R_D tail needed
+    // Only U12 and the loop state stay live across the duplication loop; everything cheap is recomputed after it
+    // (registers decide how many warps fit, DESIGN.md section 5).
+    T U12[K], ra[K], iE[K], xa[K], mp[K], s[K], Qc[K];
+    unsigned st[K];
+    T p5[K], p0[K], dl5[K], dl0[K], p5_0[K], p0_0[K], Q5v[K], Q0v[K];
+    const bool quartA = kA && !(C.cubic & 1u);
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        const T x = T(1) + z[k];
+        const T z2 = z[k] * z[k];
+        st[k] = C.status;
+        if (!(x > T(0))) st[k] |= ST_UNSUPPORTED;
+        if (x >= C.xlim) st[k] |= ST_ROOT_ON_PATH;
+        // ---- S4 radicands
+        const T q1x = N::fma_(C.Or, x, C.m) * (x - C.rn);
+        const T q2x = N::fma_(x + C.b, x, C.c);
+        const T a1 = q1x * C.q21, a2 = C.q11 * q2x;
+        const T r1 = N::rsqrt_(a1), r2 = N::rsqrt_(a2);
+        ra[k] = a1 * r1;
+        iE[k] = r1 * r2;                                  // a1 a2 = E^2(x) E^2(1) and E(1) = 1 (sum of Omegas)
+        U12[k] = N::fma_(a2, r2, ra[k]);
+        xa[k] = U12[k] * U12[k];
+        const T hd = T(0.5) * z2 * C.theta;               // u12^2 - (u13^2 + u14^2)/2
+        mp[k] = xa[k] - hd;
+        s[k] = z2 * z2 * C.sD;
+        const T hs = z2 * C.sDr;                          // |h|
+        // ---- R_J parameters
+        p5[k] = p0[k] = dl5[k] = dl0[k] = p5_0[k] = p0_0[k] = Q5v[k] = Q0v[k] = T(0);
+        if (kT) {
+            p5[k] = N::fma_(z2, C.p5c, xa[k]);
+            p5_0[k] = p5[k];
+            const T pm = p5[k] - mp[k];
+            dl5[k] = (p5[k] - xa[k]) * N::fma_(pm, pm, -s[k]);
+        }
+        if (kA) {
+            p0[k] = quartA ? N::fma_(-C.Or * z2, C.Q2n, xa[k]) : xa[k];
+            p0_0[k] = p0[k];
+            const T pm = p0[k] - mp[k];
+            dl0[k] = (p0[k] - xa[k]) * N::fma_(pm, pm, -s[k]);
+        }
+        // ---- stopping rule (ref. [10]): 4^-n Q < |A_n| for every series that is summed.  R_F and R_D share one Q:
+        // the larger deviation bound (2/3 |xa - mp| + |h|) with the stricter constant of the two.
+        Qc[k] = carlson_Qc<T>(hd, hs, kD);
+        if (kT) Q5v[k] = carlson_Qj<T>(xa[k], mp[k], hs, p5[k]);
+        if (kA) Q0v[k] = carlson_Qj<T>(xa[k], mp[k], hs, p0[k]);
+    }
+    // ---- S5 fused duplication
+    T f, tailD[K], sum5[K], sum0[K];
+    carlson_dup<T, kD, kT, kA, K, Vote>(xa, mp, s, p5, p0, dl5, dl0, Qc, Q5v, Q0v, st, vote, f, tailD, sum5, sum0);
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         const T x = T(1) + z[k];
@@ -283,39 +363,10 @@ CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Cor
             R[k].E = Ev;
             R[k].iE = iE[k];
         }
-        // ---- series: R_F
-        T RF;
-        {
-            const T An = (xa[k] + T(2) * mp[k]) * T(CB_KT.third);
-            const T rA = N::rsqrt_(An);
-            const T g = f * rA * rA;
-            const T dl = hd * T(CB_KT.third) * g;
-            const T vs = s0 * g * g;
-            const T e2 = T(-3) * dl * dl - vs;
-            const T e3 = T(-2) * dl * (dl * dl - vs);
-            // 1 - e2/10 + e3/14 + e2^2/24 - 3 e2 e3/44 - 5 e2^3/208 + 3 e3^2/104 + e2^2 e3/16, nested for FMAs
-            const double* c = CB_KT.rf;
-            const T ta = N::fma_(e2, N::fma_(e2, T(c[2]), T(c[1])), T(c[0]));
-            const T tb = N::fma_(e3, T(c[6]), N::fma_(e2, N::fma_(e2, T(c[5]), T(c[4])), T(c[3])));
-            const T S = N::fma_(e3, tb, N::fma_(e2, ta, T(1)));
-            RF = S * rA;
-        }
+        // ---- series
+        const T RF = carlson_rf_series<T>(xa[k], mp[k], f, hd, s0);
         R[k].I0 = T(2) * z[k] * RF;                       // eq. (3.7) / (B.1)
-        // ---- series: R_D(u13^2, u14^2, u12^2)
-        T RD = T(0);
-        if (kD) {
-            const T AD = (T(3) * xa[k] + T(2) * mp[k]) * T(0.2);
-            const T rA = N::rsqrt_(AD);
-            const T g = f * rA * rA;
-            const T dd = hd * T(0.2) * g;
-            const T XY = T(9) * dd * dd - s0 * g * g;
-            const T Z = T(-2) * dd, Z2 = Z * Z;
-            const T e2 = XY - T(6) * Z2;
-            const T e3 = (T(3) * XY - T(8) * Z2) * Z;
-            const T e4 = T(3) * (XY - Z2) * Z2;
-            const T e5 = XY * Z2 * Z;
-            RD = N::fma_(g * rA, series_J<T>(e2, e3, e4, e5), T(3) * tailD[k]);
-        }
+        const T RD = kD ? carlson_rd_series<T>(xa[k], mp[k], f, hd, s0, tailD[k]) : T(0);     // R_D(u13^2, u14^2, u12^2)
         const T rUx = N::rcp_(U12[k] * xmr);               // 1/(u12 (x - rn))
         const T rU = xmr * rUx;
         R[k].K = T(0); R[k].TT = T(0); R[k].AA = T(0);
@@ -324,27 +375,9 @@ CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Cor
             // sqrt((Or x + m) kf / (x - rn)) = sqrt(kf / Q2(1)) sqrt(Q1(x) Q2(1)) / (x - rn)
             R[k].K = T(2) * z[k] * N::fma_(z2 * T(CB_KT.third) * C.W, RD, C.ck * ra[k] * rUx);
         }
-        auto rj_series = [&](T p_n, T p_init, T sum) -> T {
-            const T An = (xa[k] + T(2) * mp[k] + T(2) * p_n) * T(0.2);
-            const T A0 = (xa0 + T(2) * m0 + T(2) * p_init) * T(0.2);
-            const T rA = N::rsqrt_(An);
-            const T g = f * rA * rA;
-            const T X = (A0 - xa0) * g;
-            const T am = A0 - m0;
-            const T YpZ = T(2) * am * g;
-            const T YZ = N::fma_(am, am, -s0) * g * g;
-            const T P = T(-0.5) * (X + YpZ);
-            const T XYZ = X * YZ;
-            const T P2 = P * P;
-            const T e2 = N::fma_(X, YpZ, YZ) - T(3) * P2;
-            const T e3 = XYZ + T(2) * e2 * P + T(4) * P2 * P;
-            const T e4 = (T(2) * XYZ + e2 * P + T(3) * P2 * P) * P;
-            const T e5 = XYZ * P2;
-            return N::fma_(g * rA, series_J<T>(e2, e3, e4, e5), T(6) * sum);
-        };
         if (kT) {
             // eq. (3.8) with i = big root, j = rn, scaled so that Or -> 0 reproduces (B.2)
-            const T RJ5 = rj_series(p5[k], p5_0[k], sum5[k]);
+            const T RJ5 = carlson_rj_series<T>(xa[k], mp[k], p5[k], f, xa0, m0, s0, p5_0[k], sum5[k]);
             const T qh = x * p5_0[k] * C.qhc / lin;
             const T sh = N::fma_(z2, C.OL, qh);
             R[k].TT = T(2) * z[k] * (z2 * T(CB_KT.third) * C.Gp * RJ5 + rc<T>(sh, qh) - C.OrM * RF);
@@ -353,7 +386,7 @@ CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Cor
             const T bnd = N::sqrt_(xmr * (T(1) - C.rn)) * rU;
             if (quartA) {
                 // eq. (3.9) with (i,j,k,l) = (rn, pair, pair, big)
-                const T RJ0 = rj_series(p0[k], p0_0[k], sum0[k]);
+                const T RJ0 = carlson_rj_series<T>(xa[k], mp[k], p0[k], f, xa0, m0, s0, p0_0[k], sum0[k]);
                 const T q0 = p0_0[k] / ((T(1) - C.rn) * xmr);
                 const T s0q = N::fma_(C.Or, z2, q0);
                 // third-kind bracket of (3.9): 2 z B0 = int (x - rn) dx / E

@@ -392,6 +392,28 @@ __global__ void __launch_bounds__(ELEM_THREADS) k_elem(const T* __restrict__ z, 
     }
 }
 
+// The device Carlson functions on their own (same code as the hot path): R_F(x, m+h, m-h), R_D(m+h, m-h, x) and
+// R_J(x, m+h, m-h, p) with h^2 = s (s < 0: complex-conjugate pair), positive x and p.
+__global__ void k_carlson_pair(const double* __restrict__ x, const double* __restrict__ m, const double* __restrict__ s,
+                               const double* __restrict__ p, int64_t n, double* __restrict__ rf, double* __restrict__ rd,
+                               double* __restrict__ rj) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const int64_t ii = i < n ? i : n - 1;
+    double xa[1] = {x[ii]}, mp[1] = {m[ii]}, ss[1] = {s[ii]}, p5[1] = {p[ii]}, p0[1] = {0.0};
+    const double xa0 = xa[0], m0 = mp[0], s0 = ss[0], pp0 = p5[0];
+    const double hd = xa0 - m0, hs = sqrt(fabs(s0));
+    const double pm = pp0 - m0;
+    const double dl5[1] = {(pp0 - xa0) * fma(pm, pm, -s0)}, dl0[1] = {0.0};
+    const double Qc[1] = {carlson_Qc<double>(hd, hs, true)}, Q5v[1] = {carlson_Qj<double>(xa0, m0, hs, pp0)}, Q0v[1] = {0.0};
+    unsigned st[1] = {0u};
+    double f, tailD[1], sum5[1], sum0[1];
+    carlson_dup<double, true, true, false, 1, VoteWarp>(xa, mp, ss, p5, p0, dl5, dl0, Qc, Q5v, Q0v, st, VoteWarp(), f, tailD, sum5, sum0);
+    if (i >= n) return;
+    rf[i] = carlson_rf_series<double>(xa[0], mp[0], f, hd, s0);
+    rd[i] = carlson_rd_series<double>(xa[0], mp[0], f, hd, s0, tailD[0]);
+    rj[i] = carlson_rj_series<double>(xa[0], mp[0], p5[0], f, xa0, m0, s0, pp0, sum5[0]);
+}
+
 // ALU roofline probes: 8 independent FMA chains per thread
 template <typename T>
 __global__ void __launch_bounds__(256) k_probe_fma(int iters, T* __restrict__ sink) {

@@ -518,3 +518,39 @@ def test_derived_observables(cb, mode):
             assert (np.abs(mine[p] - ref)[ok] <= TOL_GRAD * sab[ok]).all(), p
         for k, (v, gr) in enumerate(refs):
             assert relerr(out[k], v)[ok].max() <= TOL_VAL, which[k]
+
+
+# ---------------------------------------------------------------- the device Carlson functions on their own
+def test_carlson_device_functions(cb, goldens):
+    """R_F, R_D, R_J of the hot path (real-symmetric form) against the oracle's independent complex scalar implementation
+    on positive triples and complex-conjugate pairs, and against the survey's mpmath values"""
+    rng = np.random.default_rng(9)
+    n = 4000
+    x = 10.0 ** rng.uniform(-2, 3, n)
+    m = x * 10.0 ** rng.uniform(-1.5, 1.5, n)
+    real = rng.random(n) < 0.4
+    h2 = np.where(real, (m * rng.uniform(0.0, 0.98, n)) ** 2, -(m * 10.0 ** rng.uniform(-2, 1, n)) ** 2)
+    neg = ~real & (rng.random(n) < 0.3)                                  # some pairs with negative real part, away from the cut
+    h2 = np.where(neg, -(m * rng.uniform(1.0, 10.0, n)) ** 2, h2)
+    m = np.where(neg, -0.3 * m, m)
+    p = x * 10.0 ** rng.uniform(-1, 1, n)
+    rf, rd, rj = (t.cpu().numpy() for t in cb.carlson_pair(dev(x), dev(m), dev(h2), dev(p)))
+    for i in range(0, n, 4):
+        h = np.sqrt(complex(h2[i]))
+        y, z = m[i] + h, m[i] - h
+        assert abs(rf[i] - complex(oracle.rf(x[i], y, z)).real) <= 1e-14 * abs(rf[i]), i
+        assert abs(rd[i] - complex(oracle.rd(y, z, x[i])).real) <= 2e-14 * abs(rd[i]), i
+        assert abs(rj[i] - complex(oracle.rj(x[i], y, z, p[i])).real) <= 2e-14 * abs(rj[i]), i
+    # mpmath values (tests/golden/survey_goldens.json: 'carlson')
+    cases = [  # x, m, s, p  ->  (which, value)
+        (2.0, 3.5, 0.25, 5.0, "rf", 0.5840828416771517), (2.0, 0.0, -1.0, 1.0, "rf", 1.044144565406436),
+        (2.0, 3.5, 0.25, 5.0, "rj", 0.1429757966715675), (1.0, -1.0, -1.0, 2.0, "rj", 0.9414835884122024),
+        (4.0, 2.5, 0.25, 1.0, "rd", 0.1651052729426105), (2.0, 0.0, -1.0, 1.0, "rd", 0.6593385415421977)]
+    a = np.array([c[:4] for c in cases])
+    out = dict(zip(("rf", "rd", "rj"), (t.cpu().numpy() for t in cb.carlson_pair(dev(a[:, 0]), dev(a[:, 1]), dev(a[:, 2]), dev(a[:, 3])))))
+    for i, c in enumerate(cases):
+        assert abs(out[c[4]][i] - c[5]) <= 1e-14 * c[5], c
+    # degenerate arguments: R_F(x,x,x) = x^-1/2, R_D(x,x,x) = R_J(x,x,x,x) = x^-3/2 (PAPER.md:127-131)
+    xv = np.array([0.37, 1.0, 42.0])
+    r = [t.cpu().numpy() for t in cb.carlson_pair(dev(xv), dev(xv), dev(np.zeros(3)), dev(xv))]
+    assert np.allclose(r[0], xv ** -0.5, rtol=1e-15) and np.allclose(r[1], xv ** -1.5, rtol=1e-15) and np.allclose(r[2], xv ** -1.5, rtol=1e-15)
