@@ -37,6 +37,8 @@ def lib():
         _lib.oracle_derived_batch.restype = None
         _lib.oracle_snia_loglike.argtypes = [C.c_int64, _DP, _DP, _DP] + [C.c_double] * 4 + [C.c_int, _LDP]
         _lib.oracle_snia_loglike.restype = C.c_int
+        _lib.oracle_snia_logjoint.argtypes = [C.c_int64, _DP, _DP, _DP, _DP] + [C.c_double] * 7 + [C.c_int, _LDP, _LDP]
+        _lib.oracle_snia_logjoint.restype = C.c_int
         for name, nin in (("oracle_rf", 6), ("oracle_rc", 4), ("oracle_rd", 6), ("oracle_rj", 8)):
             f = getattr(_lib, name)
             f.argtypes = [C.c_double] * nin + [_LDP]
@@ -130,6 +132,20 @@ def snia_loglike(z, mu_obs, sigma, Om, OL, Or, H0, with_grad=True):
     if rc != 0:
         out[:] = np.nan
     return out
+
+
+def snia_logjoint(z, z_obs, mu_obs, sigma_mu, sigma_z, beta, shape, Om, OL, Or, H0, with_grad=True):
+    """Log-joint of the section-4 toy model with latent redshifts, one cosmology:
+    (np.longdouble[5] = log p, d/d(Om, OL, Or, H0);  grad_z[n] np.longdouble or None)."""
+    z, z_obs, mu_obs, sigma_mu = (np.ascontiguousarray(a, dtype=np.float64) for a in (z, z_obs, mu_obs, sigma_mu))
+    out = np.zeros(5, dtype=np.longdouble)
+    gz = np.zeros(z.shape[0], dtype=np.longdouble) if with_grad else None
+    rc = lib().oracle_snia_logjoint(z.shape[0], _dp(z), _dp(z_obs), _dp(mu_obs), _dp(sigma_mu), float(sigma_z), float(beta),
+                                    float(shape), float(Om), float(OL), float(Or), float(H0), int(with_grad), _ldp(out),
+                                    _ldp(gz) if with_grad else None)
+    if rc != 0:
+        out[:] = np.nan
+    return out, gz
 
 
 def _carlson(name, *args):

@@ -642,3 +642,49 @@ void oracle_rj(double xr, double xi, double yr, double yi, double zr, double zi,
 void oracle_gk21_rule(ld x[21], ld wk[21], ld wg[21]) {
     memcpy(x, GK21_X, sizeof(GK21_X)); memcpy(wk, GK21_WK, sizeof(GK21_WK)); memcpy(wg, GK21_WG, sizeof(GK21_WG));
 }
+
+/* ======================================================================================
+ * (6) the log-joint of the paper's section-4 toy model with LATENT redshifts:
+ *       mu_obs_n | z_n, theta ~ N(mu(z_n; theta), sigma_mu_n^2)
+ *       z_obs_n  | z_n        ~ N(z_n, (1+z_n)^2 sigma_z^2)                      (photometric-redshift toy model)
+ *       z_n                  ~ Gamma(shape, rate beta):  p(z) = beta^shape z^(shape-1) e^(-beta z) / Gamma(shape)
+ *     (the paper fixes beta = 3, sigma_mu = 0.14, sigma_z = 0.04 and does not print the shape: DESIGN.md reading R-prior.)
+ *     out = {log p, d/dOm, d/dOL, d/dOr, d/dH0};  gz[n] = d log p / d z_n  (nullable).  One cosmology, direct summation.
+ * ====================================================================================== */
+int oracle_snia_logjoint(int64_t n, const double *z, const double *z_obs, const double *mu_obs, const double *sigma_mu,
+                         double sigma_z, double beta, double shape, double Om, double OL, double Or, double H0,
+                         int with_grad, ld out[5], ld *gz) {
+    ld acc[5] = { 0, 0, 0, 0, 0 };
+    int bad = 0;
+    const ld half_ln_2pi = 0.5L * logl(2.0L * acosl(-1.0L));
+    const ld prior_norm = (ld)shape * logl((ld)beta) - lgammal((ld)shape);
+#pragma omp parallel
+    {
+        ld loc[5] = { 0, 0, 0, 0, 0 };
+        int locbad = 0;
+#pragma omp for schedule(static)
+        for (int64_t i = 0; i < n; ++i) {
+            ld val[N_OBS], grad[N_OBS * N_WRT];
+            int rc = oracle_observables((ld)z[i], (ld)Om, (ld)OL, (ld)Or, (ld)H0, val, with_grad ? grad : NULL);
+            if (rc != 0) { locbad = 1; if (gz) gz[i] = NAN; continue; }
+            ld zi = (ld)z[i], x = 1.0L + zi;
+            ld s = (ld)sigma_mu[i], r = ((ld)mu_obs[i] - val[OBS_MU]) / s;
+            ld sz = x * (ld)sigma_z, rz = ((ld)z_obs[i] - zi) / sz;
+            loc[0] += (-0.5L * r * r - logl(s) - half_ln_2pi) + (-0.5L * rz * rz - logl(sz) - half_ln_2pi)
+                      + (prior_norm + ((ld)shape - 1.0L) * logl(zi) - (ld)beta * zi);
+            if (with_grad) {
+                for (int p = 0; p < 4; ++p) loc[1 + p] += (r / s) * grad[OBS_MU * N_WRT + WRT_OM + p];
+                if (gz) gz[i] = (r / s) * grad[OBS_MU * N_WRT + WRT_Z]
+                                + (rz / sz + rz * rz / x - 1.0L / x)                 /* d/dz of the photo-z term */
+                                + (((ld)shape - 1.0L) / zi - (ld)beta);              /* d/dz of the prior         */
+            }
+        }
+#pragma omp critical
+        {
+            for (int k = 0; k < 5; ++k) acc[k] += loc[k];
+            bad |= locbad;
+        }
+    }
+    for (int k = 0; k < 5; ++k) out[k] = acc[k];
+    return bad ? -1 : 0;
+}
