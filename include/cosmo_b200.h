@@ -86,6 +86,18 @@ int cosmo_vjp(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int
 int cosmo_snia_loglike(const double* z, const double* mu_obs, const double* sigma, int64_t N, cosmo_params p, int64_t S,
                        double* logL, double* grad, void* workspace, size_t ws_bytes, void* stream);
 
+/* Log-joint of the paper's section-4 toy model with LATENT redshifts (one step of its variational fit evaluates this
+ * and its gradient for S posterior samples): for sample s with redshifts z[s][0..N) and cosmology theta_s
+ *   log p[s] = sum_n [ ln N(mu_obs[n] | mu(z[s][n]; theta_s), sigma_mu[n]^2) + ln N(z_obs[n] | z[s][n], (1+z[s][n])^2 sigma_z^2)
+ *                      + ln Gamma(z[s][n]; shape, rate beta) ]
+ *   grad[4][S]    = d log p[s] / d (Om, OL, Or, H0)      (nullable)
+ *   grad_z[S][N]  = d log p[s] / d z[s][n]               (nullable)
+ * (the paper fixes beta = 3, sigma_mu = 0.14, sigma_z = 0.04; it does not print the gamma shape: DESIGN.md reading R-prior.)
+ * Workspace: cosmo_workspace_bytes(N, S, COSMO_OUTER, COSMO_MU, 1).  Samples whose E^2 has no real negative root give NaN. */
+int cosmo_snia_logjoint(const double* z, const double* z_obs, const double* mu_obs, const double* sigma_mu, double sigma_z,
+                        double beta, double shape, int64_t N, cosmo_params p, int64_t S, double* logp, double* grad, double* grad_z,
+                        void* workspace, size_t ws_bytes, void* stream);
+
 /* FP32 variants: z, out, grad_out, grad_z, mu_obs, sigma are float and the per-element arithmetic is FP32;
  * parameters, the per-cosmology constants (root solve) and the reduced outputs grad_params / logL / grad stay FP64. */
 int cosmo_eval_f32(const float* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode, uint32_t which,

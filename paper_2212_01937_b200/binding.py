@@ -19,7 +19,7 @@ WHICH_ORDER = ("DC", "DM", "DL", "MU", "TL", "DABS", "DA", "VC", "AGE")
 
 # every symbol include/cosmo_b200.h declares
 SYMBOLS = ("cosmo_workspace_bytes", "cosmo_eval", "cosmo_vjp", "cosmo_snia_loglike", "cosmo_eval_f32", "cosmo_vjp_f32",
-           "cosmo_snia_loglike_f32", "cosmo_eval_host", "cosmo_carlson_pair", "cosmo_probe_fma_f64", "cosmo_probe_fma_f32",
+           "cosmo_snia_loglike_f32", "cosmo_snia_logjoint", "cosmo_eval_host", "cosmo_carlson_pair", "cosmo_probe_fma_f64", "cosmo_probe_fma_f32",
            "cosmo_profile", "cosmo_profile_mean_ms",
            "cosmo_launch_count", "cosmo_last_cuda_error", "cosmo_strerror", "cosmo_version")
 
@@ -65,6 +65,8 @@ def lib():
         f = getattr(L, name)
         f.argtypes = [ci, ci, vp, vp]
         f.restype = ci
+    L.cosmo_snia_logjoint.argtypes = [vp, vp, vp, vp, C.c_double, C.c_double, C.c_double, i64, CosmoParams, i64, vp, vp, vp, vp, sz, vp]
+    L.cosmo_snia_logjoint.restype = ci
     L.cosmo_carlson_pair.argtypes = [vp, vp, vp, vp, i64, vp, vp, vp, vp]
     L.cosmo_carlson_pair.restype = ci
     L.cosmo_launch_count.restype = i64
@@ -214,6 +216,24 @@ def cosmo_snia_loglike(z, mu_obs, sigma, Om, OL, Or, H0, want_grad=True, logL=No
     fn = lib().cosmo_snia_loglike_f32 if f32 else lib().cosmo_snia_loglike
     _check(fn(_ptr(z), _ptr(mu_obs), _ptr(sigma), N, P, S, _ptr(logL), _ptr(grad), _ptr(ws), ws.numel(), _stream(torch)))
     return logL, grad
+
+
+def cosmo_snia_logjoint(z, z_obs, mu_obs, sigma_mu, sigma_z, beta, shape, Om, OL, Or, H0, want_grad=True, workspace=None):
+    """Log-joint with latent redshifts z[S, N].  Returns (logp[S], grad[4, S] or None, grad_z[S, N] or None)."""
+    torch = _torch()
+    for t, nm in ((z, "z"), (z_obs, "z_obs"), (mu_obs, "mu_obs"), (sigma_mu, "sigma_mu")):
+        _dev(t, torch.float64, torch, nm)
+    P, S, keep = _params(Om, OL, Or, H0, torch)
+    N = z_obs.numel()
+    if z.numel() != S * N:
+        raise CosmoError("z must have shape [S, N]")
+    logp = torch.empty(S, dtype=torch.float64, device=z.device)
+    grad = torch.empty((4, S), dtype=torch.float64, device=z.device) if want_grad else None
+    gz = torch.empty((S, N), dtype=torch.float64, device=z.device) if want_grad else None
+    ws = _workspace(torch, workspace_bytes(N, S, OUTER, MU, True), z.device, workspace)
+    _check(lib().cosmo_snia_logjoint(_ptr(z), _ptr(z_obs), _ptr(mu_obs), _ptr(sigma_mu), float(sigma_z), float(beta), float(shape), N, P, S,
+                                     _ptr(logp), _ptr(grad), _ptr(gz), _ptr(ws), ws.numel(), _stream(torch)))
+    return logp, grad, gz
 
 
 def cosmo_eval_host(z, Om, OL, Or, H0, mode=ELEMENTWISE, which=("DC",), grad_out=None, want_out=True, want_status=True):

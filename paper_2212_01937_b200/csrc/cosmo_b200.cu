@@ -88,7 +88,7 @@ template <typename T, int MODE>
 int launch_outer(OuterArgs& a, dim3 grid, cudaStream_t st) {
     const bool kT = a.which & (W_TL | W_AGE), kA = a.which & W_DABS;
     prof_begin(st);
-    if (MODE == MODE_SNIA) k_outer<T, false, false, MODE, W_MU><<<grid, OUTER_THREADS, 0, st>>>(a);
+    if (MODE == MODE_SNIA || MODE == MODE_JOINT) k_outer<T, false, false, MODE, W_MU><<<grid, OUTER_THREADS, 0, st>>>(a);
     else if (kT && kA) k_outer<T, true, true, MODE, 0><<<grid, OUTER_THREADS, 0, st>>>(a);
     else if (kT) k_outer<T, true, false, MODE, 0><<<grid, OUTER_THREADS, 0, st>>>(a);
     else if (kA) k_outer<T, false, true, MODE, 0><<<grid, OUTER_THREADS, 0, st>>>(a);
@@ -199,6 +199,46 @@ int run_snia(const T* z, const T* mu_obs, const T* sigma, int64_t N, cosmo_param
     return check_launch();
 }
 
+// log-joint with latent redshifts z[S][N] (MODE_JOINT)
+template <typename T>
+int run_joint(const T* z, const T* z_obs, const T* mu_obs, const T* sigma_mu, double sigma_z, double beta, double shape, int64_t N,
+              cosmo_params p, int64_t S, double* logp, double* grad, T* grad_z, void* ws, size_t ws_bytes, void* stream) {
+    if (N < 0 || S < 0 || !(sigma_z > 0.0) || !(beta > 0.0) || !(shape > 0.0)) return COSMO_E_SIZE;
+    if (S > 0 && (!p.Om || !p.OL || !p.Or || !p.H0 || !logp)) return COSMO_E_NULL;
+    if (N > 0 && S > 0 && (!z || !z_obs || !mu_obs || !sigma_mu)) return COSMO_E_NULL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (S == 0) return COSMO_OK;
+    if (N == 0) {
+        cudaMemsetAsync(logp, 0, sizeof(double) * S, st);
+        if (grad) cudaMemsetAsync(grad, 0, sizeof(double) * 4 * S, st);
+        return COSMO_OK;
+    }
+    WsLayout L = ws_layout(N, S, COSMO_OUTER, 1, sizeof(T));
+    if (!ws) return COSMO_E_NULL;
+    if (ws_bytes < L.total) return COSMO_E_WORKSPACE;
+    char* w = static_cast<char*>(ws);
+    Cosmo<double>* consts = reinterpret_cast<Cosmo<double>*>(w + L.consts);
+    int rc;
+    k_prep<<<(unsigned)cdiv(S, 64), 64, 0, st>>>(p.Om, p.OL, p.Or, p.H0, S, 1, consts);
+    if ((rc = check_launch())) return rc;
+    OuterArgs a{};
+    a.z = z; a.z_obs = z_obs; a.mu_obs = mu_obs; a.sigma = sigma_mu; a.gz = grad_z; a.consts = consts; a.N = N; a.S = S; a.which = W_MU;
+    a.sigma_z = sigma_z; a.beta = beta; a.shape_m1 = shape - 1.0;
+    a.prior_norm = shape * log(beta) - lgamma(shape) - log(sigma_z) - 0.91893853320467274178;
+    a.part = reinterpret_cast<double*>(w + L.part);
+    const uintptr_t m = sizeof(T) == 8 ? 15 : 7;
+    a.vec = (N % 2 == 0) && ((reinterpret_cast<uintptr_t>(z) | reinterpret_cast<uintptr_t>(z_obs) | reinterpret_cast<uintptr_t>(mu_obs) |
+                              reinterpret_cast<uintptr_t>(sigma_mu) | reinterpret_cast<uintptr_t>(grad_z)) & m) == 0;
+    int ny = (int)cdiv(S, S_CHUNK);
+    int64_t cap = cdiv((int64_t)16 * 148 * 5, L.ntiles);
+    if (cap < 1) cap = 1;
+    if (ny > cap) ny = (int)cap;
+    dim3 grid((unsigned)L.ntiles, (unsigned)ny);
+    if ((rc = launch_outer<T, MODE_JOINT>(a, grid, st))) return rc;
+    k_reduce_params<5><<<(unsigned)cdiv(S * 5 * 32, 256), 256, 0, st>>>(a.part, L.ntiles, S, logp, grad);
+    return check_launch();
+}
+
 // grow-only device scratch of the host-buffer convenience call
 std::mutex g_host_mu;
 void* g_host_buf = nullptr;
@@ -226,6 +266,11 @@ int cosmo_vjp(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int
 int cosmo_snia_loglike(const double* z, const double* mu_obs, const double* sigma, int64_t N, cosmo_params p, int64_t S,
                        double* logL, double* grad, void* workspace, size_t ws_bytes, void* stream) {
     return run_snia<double>(z, mu_obs, sigma, N, p, S, logL, grad, workspace, ws_bytes, stream);
+}
+int cosmo_snia_logjoint(const double* z, const double* z_obs, const double* mu_obs, const double* sigma_mu, double sigma_z,
+                        double beta, double shape, int64_t N, cosmo_params p, int64_t S, double* logp, double* grad, double* grad_z,
+                        void* workspace, size_t ws_bytes, void* stream) {
+    return run_joint<double>(z, z_obs, mu_obs, sigma_mu, sigma_z, beta, shape, N, p, S, logp, grad, grad_z, workspace, ws_bytes, stream);
 }
 int cosmo_eval_f32(const float* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode, uint32_t which, float* out,
                    uint8_t* status, void* workspace, size_t ws_bytes, void* stream) {

@@ -28,7 +28,7 @@ constexpr int S_CHUNK = CB_SCHUNK;                         // cosmologies staged
 constexpr int NWARP = OUTER_THREADS / 32;
 constexpr int ELEM_THREADS = 128;
 
-enum { MODE_FWD = 0, MODE_VJP = 1, MODE_SNIA = 2 };
+enum { MODE_FWD = 0, MODE_VJP = 1, MODE_SNIA = 2, MODE_JOINT = 3 };   // JOINT: SNIA + latent redshifts z[S][N]
 
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
@@ -102,7 +102,9 @@ __device__ __forceinline__ void store2(T* __restrict__ p, int64_t i, int64_t n, 
 }
 
 struct OuterArgs {
-    const void* z; const void* gout; const void* mu_obs; const void* sigma;
+    const void* z; const void* gout; const void* mu_obs; const void* sigma; const void* z_obs;
+    double sigma_z, beta, shape_m1, prior_norm;   // MODE_JOINT: photo-z scatter, gamma prior rate, shape - 1, and the constant
+                                                  // shape ln(beta) - lnGamma(shape) - ln(sigma_z) - ln(2 pi)/2
     void* out; void* gz; uint8_t* status;
     const Cosmo<double>* consts;
     double* part;            // [S][NP][ntiles] partial parameter sums (NP = 4 vjp, 5 snia)
@@ -119,7 +121,7 @@ struct OuterArgs {
 template <typename T, bool kT, bool kA, int MODE>
 __device__ __noinline__ void outer_c4_row(const OuterArgs& a, const Cosmo<T>& C, int64_t row, int64_t n0, const T* zv, const T* mo,
                                           const T* isig2, const T* lnorm, unsigned which, double* sacc_row, int lane, T* gzacc) {
-    constexpr int NP = MODE == MODE_SNIA ? 5 : 4;
+    constexpr int NP = (MODE == MODE_SNIA || MODE == MODE_JOINT) ? 5 : 4;
     const int64_t N = a.N, S = a.S;
     T ll = T(0);
     for (int k = 0; k < KZ; ++k) {
@@ -164,7 +166,8 @@ template <typename T, bool kT, bool kA, int MODE, unsigned WCT>
 __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) k_outer(OuterArgs a) {
     const unsigned which = WCT ? WCT : a.which;      // WCT != 0: output set known at compile time (drops dead planes)
     constexpr bool kG = MODE != MODE_FWD;
-    constexpr int NP = MODE == MODE_SNIA ? 5 : 4;
+    constexpr bool kLike = MODE == MODE_SNIA || MODE == MODE_JOINT;
+    constexpr int NP = kLike ? 5 : 4;
     __shared__ Cosmo<T> sc[S_CHUNK];
     __shared__ double sacc[kG ? NWARP : 1][kG ? S_CHUNK : 1][NP];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -177,8 +180,9 @@ __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) 
     bool live[KZ];
 #pragma unroll
     for (int k = 0; k < KZ; ++k) live[k] = n0 + k < N;
-    T mo[KZ], isig2[KZ], lnorm[KZ];
-    if (MODE == MODE_SNIA) {
+    T mo[KZ], isig2[KZ], lnorm[KZ], zo[KZ];
+    if (MODE == MODE_JOINT) load2<T>(static_cast<const T*>(a.z_obs), n0, N, vec, zo);
+    if (kLike) {
         T sg[KZ];
         load2<T>(static_cast<const T*>(a.mu_obs), n0, N, vec, mo);
         load2<T>(static_cast<const T*>(a.sigma), n0, N, vec, sg);
@@ -208,8 +212,18 @@ __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) 
         for (int sl = 0; sl < ns; ++sl) {
             const Cosmo<T>& C = sc[sl];
             const int64_t row = c0 + sl;
-            if (C.cubic & 2u) {
-                outer_c4_row<T, kT, kA, MODE>(a, C, row, n0, zv, mo, isig2, lnorm, MODE == MODE_SNIA ? (unsigned)W_MU : which,
+            if (MODE == MODE_JOINT) load2<T>(zp + row * N, n0, N, vec, zv);      // latent redshifts: one row per sample
+            if (MODE == MODE_JOINT && (C.cubic & 2u)) {                          // no gradients on the complex slow path: NaN row
+                if (lane == 0)
+                    for (int j = 0; j < NP; ++j) sacc[warp][sl][j] = NAN;
+                if (a.gz != nullptr) {
+                    const T nn[KZ] = {T(NAN), T(NAN)};
+                    store2<T>(static_cast<T*>(a.gz) + row * N, n0, N, vec, nn);
+                }
+                continue;
+            }
+            if (MODE != MODE_JOINT && (C.cubic & 2u)) {
+                outer_c4_row<T, kT, kA, MODE == MODE_JOINT ? MODE_SNIA : MODE>(a, C, row, n0, zv, mo, isig2, lnorm, kLike ? (unsigned)W_MU : which,
                                               kG ? &sacc[warp][sl][0] : nullptr, lane, gzacc);
                 continue;
             }
@@ -239,16 +253,26 @@ __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) 
 #pragma unroll
             for (int k = 0; k < KZ; ++k) {
                 Obs<T> O;
-                observables<T, kT, kA>(C, zv[k], R[k], MODE == MODE_SNIA ? (unsigned)W_MU : which, O);
+                observables<T, kT, kA>(C, zv[k], R[k], kLike ? (unsigned)W_MU : which, O);
 #pragma unroll
                 for (int w = 0; w < N_PLANES; ++w) ov[w][k] = O.v[w];
                 stv[k] = (uint8_t)O.status;
-                if (MODE == MODE_SNIA) {
+                if (kLike) {
                     const T resid = mo[k] - O.v[3];
                     T gg[N_PLANES] = {T(0), T(0), T(0), resid * isig2[k], T(0), T(0), T(0), T(0), T(0)};
-                    T dummy = T(0), gp[4] = {T(0), T(0), T(0), T(0)};
-                    backward<T, false, false>(C, zv[k], R[k], O, gg, dummy, gp);
-                    const T ll = Num<T>::fma_(T(-0.5) * resid, resid * isig2[k], lnorm[k]);
+                    T dz = T(0), gp[4] = {T(0), T(0), T(0), T(0)};
+                    backward<T, false, false>(C, zv[k], R[k], O, gg, dz, gp);
+                    T ll = Num<T>::fma_(T(-0.5) * resid, resid * isig2[k], lnorm[k]);
+                    if (MODE == MODE_JOINT) {
+                        // photometric-redshift term N(z_obs | z, (1+z)^2 sigma_z^2) and gamma prior on the latent redshift
+                        const T x = T(1) + zv[k], ix = Num<T>::rcp_(x);
+                        const T isz = ix * T(1.0 / a.sigma_z);
+                        const T rz = (zo[k] - zv[k]) * isz;
+                        ll += Num<T>::fma_(T(-0.5) * rz, rz, -Num<T>::log_(x));
+                        ll += T(a.prior_norm) + T(a.shape_m1) * Num<T>::log_(zv[k]) - T(a.beta) * zv[k];
+                        dz += rz * isz + (rz * rz - T(1)) * ix + T(a.shape_m1) * Num<T>::rcp_(zv[k]) - T(a.beta);
+                        gzacc[k] = dz;
+                    }
                     if (live[k]) {
                         pacc[0] += ll;
 #pragma unroll
@@ -265,7 +289,8 @@ __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) 
                     }
                 }
             }
-            if (MODE != MODE_SNIA && a.out != nullptr) {
+            if (MODE == MODE_JOINT && a.gz != nullptr) store2<T>(static_cast<T*>(a.gz) + row * N, n0, N, vec, gzacc);
+            if (!kLike && a.out != nullptr) {
                 int pl = 0;
                 for (int w = 0; w < N_PLANES; ++w) {
                     if (!(which >> w & 1)) continue;
@@ -273,7 +298,7 @@ __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) 
                     ++pl;
                 }
             }
-            if (MODE != MODE_SNIA && a.status != nullptr) {
+            if (!kLike && a.status != nullptr) {
 #pragma unroll
                 for (int k = 0; k < KZ; ++k)
                     if (live[k]) a.status[row * N + n0 + k] = stv[k];

@@ -93,6 +93,19 @@ def main():
         grad = torch.empty((4, 256), dtype=torch.float64, device="cuda")
         ws = torch.empty(cb.workspace_bytes(n, 256, cb.OUTER, ("MU",), True), dtype=torch.uint8, device="cuda")
         timed(lambda: cb.cosmo_snia_loglike(*a, logL=logL, grad=grad, workspace=ws), 256 * n, "config4 fused SN-Ia logL + grad S=256 f64")
+    if want("logjoint"):
+        n, S = 1_000_000 // f, 64
+        zt = rng.gamma(3.0, 1 / 3.0, n) + 0.02
+        one = lambda v: dev(np.array([v]))
+        mu, _ = cb.cosmo_eval(dev(zt), one(0.3), one(0.7), one(0.0), one(70.0), cb.ELEMENTWISE, ("MU",))
+        mu_obs = mu[0, 0] + 0.14 * torch.randn(n, dtype=torch.float64, device="cuda")
+        z_obs = dev(zt + (1 + zt) * 0.04 * rng.standard_normal(n))
+        z = (z_obs[None, :] + 0.03 * torch.randn((S, n), dtype=torch.float64, device="cuda")).abs() + 0.01
+        sig = torch.full((n,), 0.14, dtype=torch.float64, device="cuda")
+        P = [dev(rng.normal(0.3, 0.03, S)), dev(rng.normal(0.7, 0.03, S)), dev(np.zeros(S)), dev(rng.normal(70, 1, S))]
+        ws = torch.empty(cb.workspace_bytes(n, S, cb.OUTER, ("MU",), True), dtype=torch.uint8, device="cuda")
+        timed(lambda: cb.cosmo_snia_logjoint(z, z_obs, mu_obs.contiguous(), sig, 0.04, 3.0, 3.0, *P, workspace=ws), S * n,
+              "section-4 log-joint with latent z (one VI step): N=1e6 SNe x S=64 samples, logp + grad_params + grad_z f64")
     if want("config5"):
         w = W.config5(n=10_000_000 // f, n_struct=100_000 // f)
         a = [dev(x) for x in (w.z, w.Om, w.OL, w.Or, w.H0)]

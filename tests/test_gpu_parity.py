@@ -554,3 +554,26 @@ def test_carlson_device_functions(cb, goldens):
     xv = np.array([0.37, 1.0, 42.0])
     r = [t.cpu().numpy() for t in cb.carlson_pair(dev(xv), dev(xv), dev(np.zeros(3)), dev(xv))]
     assert np.allclose(r[0], xv ** -0.5, rtol=1e-15) and np.allclose(r[1], xv ** -1.5, rtol=1e-15) and np.allclose(r[2], xv ** -1.5, rtol=1e-15)
+
+
+# ---------------------------------------------------------------- section-4 log-joint with latent redshifts
+@pytest.mark.parametrize("N,S", [(7, 2), (20_001, 19)])
+def test_snia_logjoint(cb, N, S):
+    rng = np.random.default_rng(N)
+    zt = rng.gamma(3.0, 1 / 3.0, N) + 0.02                 # "true" redshifts from the prior
+    mu_obs = _mu_oracle(zt, 0.3, 0.7, 0.0, 70.0) + rng.normal(0, 0.14, N)
+    z_obs = zt + (1 + zt) * 0.04 * rng.standard_normal(N)
+    sig = np.full(N, 0.14)
+    Om = rng.normal(0.3, 0.03, S); OL = rng.normal(0.7, 0.03, S); Or = np.zeros(S); H0 = rng.normal(70, 1, S)
+    z = np.abs(z_obs[None, :] + 0.03 * rng.standard_normal((S, N))) + 0.01           # latent-redshift samples of a guide
+    logp, grad, gz = cb.cosmo_snia_logjoint(dev(z), dev(z_obs), dev(mu_obs), dev(sig), 0.04, 3.0, 3.0, dev(Om), dev(OL), dev(Or), dev(H0))
+    logp, grad, gz = logp.cpu().numpy(), grad.cpu().numpy(), gz.cpu().numpy()
+    for s in range(0, S, max(1, S // 4)):
+        ref, gz_ref = oracle.snia_logjoint(z[s], z_obs, mu_obs, sig, 0.04, 3.0, 3.0, Om[s], OL[s], Or[s], H0[s])
+        ref, gz_ref = ref.astype(np.float64), gz_ref.astype(np.float64)
+        assert abs(logp[s] - ref[0]) <= 1e-11 * abs(ref[0]), s
+        val, g, _ = oracle_batch(z[s], Om[s:s + 1], OL[s:s + 1], Or[s:s + 1], H0[s:s + 1], True)
+        resid = (mu_obs - val[:, OBS["MU"]]) / sig ** 2
+        for p in range(4):
+            assert abs(grad[p, s] - ref[1 + p]) <= TOL_GRAD * np.abs(resid * g[:, OBS["MU"], 1 + p]).sum(), (s, p)
+        assert (np.abs(gz[s] - gz_ref) <= TOL_GRAD * np.maximum(np.abs(gz_ref), 1.0)).all(), s
