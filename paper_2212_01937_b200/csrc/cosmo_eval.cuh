@@ -170,16 +170,17 @@ CB_HD void carlson_dup(T (&xa)[K], T (&mp)[K], T (&s)[K], T (&p5)[K], T (&p0)[K]
     int nit = 0;
     for (;;) {
         bool more = false;
+        const bool cap = nit >= NIT_CAP;
 #pragma unroll
-        for (int k = 0; k < K; ++k) {
+        for (int k = 0; k < K; ++k) {      // branch-free: plain | and & on the comparison results
             const T fq = f * Qc[k];
             bool mk = T(3) * fq >= N::abs_(N::fma_(T(2), mp[k], xa[k]));
-            if (kD) mk = mk || (T(5) * fq >= N::abs_(N::fma_(T(3), xa[k], T(2) * mp[k])));
-            if (kT) mk = mk || (f * Q5v[k] >= N::abs_(xa[k] + T(2) * mp[k] + T(2) * p5[k]) * T(0.2));
-            if (kA) mk = mk || (f * Q0v[k] >= N::abs_(xa[k] + T(2) * mp[k] + T(2) * p0[k]) * T(0.2));
-            mk = mk && (st[k] == 0);
-            if (nit >= NIT_CAP && mk) { st[k] |= ST_ITER_CAP; mk = false; }
-            more = more || mk;
+            if (kD) mk = mk | (T(5) * fq >= N::abs_(N::fma_(T(3), xa[k], T(2) * mp[k])));
+            if (kT) mk = mk | (f * Q5v[k] >= N::abs_(xa[k] + T(2) * mp[k] + T(2) * p5[k]) * T(0.2));
+            if (kA) mk = mk | (f * Q0v[k] >= N::abs_(xa[k] + T(2) * mp[k] + T(2) * p0[k]) * T(0.2));
+            mk = mk & (st[k] == 0);
+            if (cap) { st[k] |= mk ? (unsigned)ST_ITER_CAP : 0u; mk = false; }
+            more = more | mk;
         }
         if (!vote.any(more)) break;
 #pragma unroll
