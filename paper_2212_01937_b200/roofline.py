@@ -10,18 +10,18 @@ probe (cosmo_probe_fma_f64); the nominal figure beside it is 148 SMs x 64 FP64 F
 
 # FP64 work per eval of the config-3 fused forward+VJP kernel k_outer<double,false,false,VJP,MU> as committed, from the
 # ncu capture profiles/r01_final_k_outer_vjp.md (6.4e7 evals/launch):
-#   DFMA 138.8, DMUL 115.0, DADD 32.6 thread-instructions per eval -> 2*138.8 + 115.0 + 32.6 = 425.2 flops
-#   FP64-pipe instructions per eval (the above + 9.3 DSETP) = 295.7
+#   DFMA 140.9, DMUL 115.3, DADD 33.3 thread-instructions per eval -> 2*140.9 + 115.3 + 33.3 = 430.6 flops
+#   FP64-pipe instructions per eval (the above + 10.6 DSETP) = 300.1
 # (first working version, profiles/r01_k_outer_vjp.md: 774.8 flops, 513.7 pipe instructions per eval)
 FLOPS_PER_EVAL = {
-    "config3_vjp_mu_f64": 425.2,
+    "config3_vjp_mu_f64": 430.6,
 }
 FP64_PIPE_INST_PER_EVAL = {
-    "config3_vjp_mu_f64": 295.7,
+    "config3_vjp_mu_f64": 300.1,
 }
 # dram__bytes_read.sum + dram__bytes_write.sum of that kernel, per launch (same capture)
 DRAM_TRAFFIC_BYTES_PER_LAUNCH = {
-    "config3_vjp_mu_f64": 544.09e6 + 570.56e6,
+    "config3_vjp_mu_f64": 544.86e6 + 633.18e6,
 }
 
 # nominal B200 FP64 vector peak (context only; the denominator is the measured probe)
