@@ -37,6 +37,8 @@ def lib():
         _lib.oracle_derived_batch.restype = None
         _lib.oracle_snia_loglike.argtypes = [C.c_int64, _DP, _DP, _DP] + [C.c_double] * 4 + [C.c_int, _LDP]
         _lib.oracle_snia_loglike.restype = C.c_int
+        _lib.oracle_observables2_batch.argtypes = [C.c_int64, _DP, _DP, _DP, _DP, _DP, _DP, C.c_int64, _LDP, _LDP, C.POINTER(C.c_int32)]
+        _lib.oracle_observables2_batch.restype = None
         _lib.oracle_snia_logjoint.argtypes = [C.c_int64, _DP, _DP, _DP, _DP] + [C.c_double] * 7 + [C.c_int, _LDP, _LDP]
         _lib.oracle_snia_logjoint.restype = C.c_int
         for name, nin in (("oracle_rf", 6), ("oracle_rc", 4), ("oracle_rd", 6), ("oracle_rj", 8)):
@@ -132,6 +134,28 @@ def snia_loglike(z, mu_obs, sigma, Om, OL, Or, H0, with_grad=True):
     if rc != 0:
         out[:] = np.nan
     return out
+
+
+OBS2 = ("DC", "DM", "TL", "DABS", "DA")              # two-limit observables
+WRT2 = ("z1", "z2", "Om", "OL", "Or", "H0")
+
+
+def observables2_batch(z1, z2, Om, OL, Or, H0, with_grad=True, threads=None):
+    """Two-limit forms of eqs. (2.3)-(2.5): val[n,5] (OBS2), grad[n,5,6] (WRT2) or None, status[n]."""
+    z1 = np.ascontiguousarray(z1, dtype=np.float64); z2 = np.ascontiguousarray(z2, dtype=np.float64)
+    n = z1.shape[0]
+    ps = [np.ascontiguousarray(np.atleast_1d(p), dtype=np.float64) for p in (Om, OL, Or, H0)]
+    n_cosmo = ps[0].shape[0]
+    assert z2.shape[0] == n and all(p.shape[0] == n_cosmo for p in ps) and n_cosmo in (1, n)
+    val = np.zeros((n, 5), dtype=np.longdouble)
+    grad = np.zeros((n, 5, 6), dtype=np.longdouble) if with_grad else None
+    status = np.zeros(n, dtype=np.int32)
+    L = lib()
+    if threads:
+        L.oracle_set_threads(int(threads))
+    L.oracle_observables2_batch(n, _dp(z1), _dp(z2), *[_dp(p) for p in ps], n_cosmo, _ldp(val), _ldp(grad) if with_grad else None,
+                                status.ctypes.data_as(C.POINTER(C.c_int32)))
+    return val, grad, status
 
 
 def snia_logjoint(z, z_obs, mu_obs, sigma_mu, sigma_z, beta, shape, Om, OL, Or, H0, with_grad=True):

@@ -688,3 +688,77 @@ int oracle_snia_logjoint(int64_t n, const double *z, const double *z_obs, const 
     for (int k = 0; k < 5; ++k) out[k] = acc[k];
     return bad ? -1 : 0;
 }
+
+/* ======================================================================================
+ * (7) the TWO-LIMIT forms of eqs. (2.3)-(2.5) (PAPER.md:88-93 define chi(z1,z2), t(z1,z2), d_abs(z1,z2)):
+ *     same quadrature on [ln(1+z1), ln(1+z2)].  out[12] as oracle_integrals.
+ *     oracle_observables2: val[5] = {D_C12, D_M12 (sinn of the comoving distance between z1 and z2), t12, d_abs12,
+ *     D_A12 = D_M12/(1+z2)} and grad[5][6] wrt (z1, z2, Om, OL, Or, H0).
+ * ====================================================================================== */
+int oracle_integrals2(ld z1, ld z2, ld Om, ld OL, ld Or, int with_grad, ld out[NV]) {
+    cosmo_t c = { Om, OL, Or, 1.0L - Om - OL - Or, with_grad ? NV : 3 };
+    for (int v = 0; v < NV; ++v) out[v] = 0.0L;
+    if (!(z1 > -1.0L) || !(z2 > -1.0L)) return -1;
+    if (z1 == z2) return 0;
+    ld U1 = log1pl(z1), U2 = log1pl(z2);
+    for (int i = 0; i <= 64; ++i) {
+        ld x = expl(U1 + (U2 - U1) * i / 64.0L);
+        if (!(E2_of_x(&c, x) > 0.0L)) return -1;
+    }
+    ld scale[NV], K[NV], G[NV], Kabs[NV];
+    gk21_panel(&c, U1, U2, K, G, Kabs);
+    for (int v = 0; v < c.nv; ++v) scale[v] = fabsl(K[v]);
+    int npanels = 0;
+    int nseg = (int)ceill(fabsl(U2 - U1));
+    if (nseg < 1) nseg = 1;
+    for (int s = 0; s < nseg; ++s) {
+        ld a = U1 + (U2 - U1) * s / nseg, b = U1 + (U2 - U1) * (s + 1) / nseg;
+        gk21_adapt(&c, a, b, 1.0L / nseg, scale, 0, out, &npanels);
+    }
+    if (npanels >= GK_MAXPANELS) return -2;
+    return npanels;
+}
+
+int oracle_observables2(ld z1, ld z2, ld Om, ld OL, ld Or, ld H0, ld val[5], ld *grad /* [5*6] or NULL */) {
+    ld q[NV];
+    int rc = oracle_integrals2(z1, z2, Om, OL, Or, grad != NULL, q);
+    if (rc < 0) {
+        for (int i = 0; i < 5; ++i) val[i] = NAN;
+        if (grad) for (int i = 0; i < 30; ++i) grad[i] = NAN;
+        return -1;
+    }
+    ld Ok = 1.0L - Om - OL - Or, x1 = 1.0L + z1, x2 = 1.0L + z2;
+    cosmo_t c = { Om, OL, Or, Ok, 3 };
+    ld E1 = sqrtl(E2_of_x(&c, x1)), E2 = sqrtl(E2_of_x(&c, x2));
+    ld dH = C_KM_S / H0, tH = HUBBLE_GYR / H0;
+    ld F, Fi, Fk;
+    sinn_transform(Ok, q[0], &F, &Fi, &Fk);
+    val[0] = dH * q[0]; val[1] = dH * F; val[2] = tH * q[1]; val[3] = dH * q[2]; val[4] = dH * F / x2;
+    if (!grad) return 0;
+    ld (*g)[6] = (ld (*)[6])grad;
+    /* d/dz1 = -integrand(z1), d/dz2 = +integrand(z2) */
+    g[0][0] = -dH / E1;            g[0][1] = dH / E2;
+    g[1][0] = -dH * Fi / E1;       g[1][1] = dH * Fi / E2;
+    g[2][0] = -tH / (x1 * E1);     g[2][1] = tH / (x2 * E2);
+    g[3][0] = -dH * x1 * x1 / E1;  g[3][1] = dH * x2 * x2 / E2;
+    g[4][0] = g[1][0] / x2;        g[4][1] = g[1][1] / x2 - val[1] / (x2 * x2);
+    for (int p = 0; p < 3; ++p) {
+        g[0][2 + p] = dH * q[3 + p];
+        g[1][2 + p] = dH * (Fi * q[3 + p] - Fk);
+        g[2][2 + p] = tH * q[6 + p];
+        g[3][2 + p] = dH * q[9 + p];
+        g[4][2 + p] = g[1][2 + p] / x2;
+    }
+    for (int o = 0; o < 5; ++o) g[o][5] = -val[o] / H0;
+    return 0;
+}
+
+void oracle_observables2_batch(int64_t n, const double *z1, const double *z2, const double *Om, const double *OL, const double *Or,
+                               const double *H0, int64_t n_cosmo, ld *val, ld *grad, int32_t *status) {
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < n; ++i) {
+        int64_t j = (n_cosmo == 1) ? 0 : i;
+        int rc = oracle_observables2((ld)z1[i], (ld)z2[i], (ld)Om[j], (ld)OL[j], (ld)Or[j], (ld)H0[j], val + i * 5, grad ? grad + i * 30 : NULL);
+        if (status) status[i] = rc;
+    }
+}
