@@ -113,6 +113,14 @@ int cosmo_snia_loglike_f32(const float* z, const float* mu_obs, const float* sig
 int cosmo_eval_host(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode, uint32_t which,
                     const double* grad_out, double* out, double* grad_z, double* grad_params, uint8_t* status);
 
+/* TWO-LIMIT forms (PAPER.md:88-93 define chi(z1,z2), t(z1,z2), d_abs(z1,z2); eqs. (3.7)-(3.9) are two-limit as printed), one
+ * (z1[i], z2[i], cosmology) per element; n_cosmo in {1, n}.  `which` may hold COSMO_DC (comoving distance between z1 and z2),
+ * COSMO_DM (transverse distance between them, d_H sinn(...)), COSMO_TL (t(z1,z2)), COSMO_DABS, COSMO_DA (= D_M12/(1+z2));
+ * planes out[n_which][n] in ascending bit order.  grad_out == NULL: forward (out required).  Otherwise also the VJP:
+ * grad_z1[n], grad_z2[n], grad_params[4][n] (per element, order Om, OL, Or, H0; out nullable).  status as above. */
+int cosmo_eval2(const double* z1, const double* z2, int64_t n, cosmo_params p, int64_t n_cosmo, uint32_t which, const double* grad_out,
+                double* out, double* grad_z1, double* grad_z2, double* grad_params, uint8_t* status, void* stream);
+
 /* The device Carlson functions of the hot path on their own (eqs. (2.6), (2.7), (2.9); duplication
  * algorithm of ref. [10]), in the real-symmetric form the path uses: for each i
  *   rf[i] = R_F(x, m+h, m-h),  rd[i] = R_D(m+h, m-h, x),  rj[i] = R_J(x, m+h, m-h, p),   h^2 = s[i]

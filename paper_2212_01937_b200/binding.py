@@ -19,7 +19,7 @@ WHICH_ORDER = ("DC", "DM", "DL", "MU", "TL", "DABS", "DA", "VC", "AGE")
 
 # every symbol include/cosmo_b200.h declares
 SYMBOLS = ("cosmo_workspace_bytes", "cosmo_eval", "cosmo_vjp", "cosmo_snia_loglike", "cosmo_eval_f32", "cosmo_vjp_f32",
-           "cosmo_snia_loglike_f32", "cosmo_snia_logjoint", "cosmo_eval_host", "cosmo_carlson_pair", "cosmo_probe_fma_f64", "cosmo_probe_fma_f32",
+           "cosmo_snia_loglike_f32", "cosmo_snia_logjoint", "cosmo_eval2", "cosmo_eval_host", "cosmo_carlson_pair", "cosmo_probe_fma_f64", "cosmo_probe_fma_f32",
            "cosmo_profile", "cosmo_profile_mean_ms",
            "cosmo_launch_count", "cosmo_last_cuda_error", "cosmo_strerror", "cosmo_version")
 
@@ -67,6 +67,8 @@ def lib():
         f.restype = ci
     L.cosmo_snia_logjoint.argtypes = [vp, vp, vp, vp, C.c_double, C.c_double, C.c_double, i64, CosmoParams, i64, vp, vp, vp, vp, sz, vp]
     L.cosmo_snia_logjoint.restype = ci
+    L.cosmo_eval2.argtypes = [vp, vp, i64, CosmoParams, i64, u32, vp, vp, vp, vp, vp, vp, vp]
+    L.cosmo_eval2.restype = ci
     L.cosmo_carlson_pair.argtypes = [vp, vp, vp, vp, i64, vp, vp, vp, vp]
     L.cosmo_carlson_pair.restype = ci
     L.cosmo_launch_count.restype = i64
@@ -234,6 +236,28 @@ def cosmo_snia_logjoint(z, z_obs, mu_obs, sigma_mu, sigma_z, beta, shape, Om, OL
     _check(lib().cosmo_snia_logjoint(_ptr(z), _ptr(z_obs), _ptr(mu_obs), _ptr(sigma_mu), float(sigma_z), float(beta), float(shape), N, P, S,
                                      _ptr(logp), _ptr(grad), _ptr(gz), _ptr(ws), ws.numel(), _stream(torch)))
     return logp, grad, gz
+
+
+def cosmo_eval2(z1, z2, Om, OL, Or, H0, which=("DC",), grad_out=None, want_out=True):
+    """Two-limit forms between z1 and z2 (elementwise).  Returns (out[n_which, n] or None, grad_z1, grad_z2, grad_params[4, n], status);
+    the gradients are None without grad_out.  which from DC, DM, TL, DABS, DA."""
+    torch = _torch()
+    mask = which_mask(which)
+    _dev(z1, torch.float64, torch, "z1"); _dev(z2, torch.float64, torch, "z2")
+    P, n_cosmo, keep = _params(Om, OL, Or, H0, torch)
+    n = z1.numel()
+    nw = bin(mask).count("1")
+    out = torch.empty((nw, n), dtype=torch.float64, device=z1.device) if (want_out or grad_out is None) else None
+    status = torch.empty(n, dtype=torch.uint8, device=z1.device)
+    g1 = g2 = gp = None
+    if grad_out is not None:
+        _dev(grad_out, torch.float64, torch, "grad_out")
+        g1 = torch.empty(n, dtype=torch.float64, device=z1.device)
+        g2 = torch.empty(n, dtype=torch.float64, device=z1.device)
+        gp = torch.empty((4, n), dtype=torch.float64, device=z1.device)
+    _check(lib().cosmo_eval2(_ptr(z1), _ptr(z2), n, P, n_cosmo, mask, _ptr(grad_out), _ptr(out), _ptr(g1), _ptr(g2), _ptr(gp), _ptr(status),
+                             _stream(torch)))
+    return out, g1, g2, gp, status
 
 
 def cosmo_eval_host(z, Om, OL, Or, H0, mode=ELEMENTWISE, which=("DC",), grad_out=None, want_out=True, want_status=True):

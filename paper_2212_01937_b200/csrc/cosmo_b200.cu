@@ -340,6 +340,21 @@ int cosmo_eval_host(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosm
     return COSMO_OK;
 }
 
+int cosmo_eval2(const double* z1, const double* z2, int64_t n, cosmo_params p, int64_t n_cosmo, uint32_t which, const double* grad_out,
+                double* out, double* grad_z1, double* grad_z2, double* grad_params, uint8_t* status, void* stream) {
+    if (n < 0 || !(n_cosmo == 1 || n_cosmo == n)) return COSMO_E_SIZE;
+    if (which == 0 || (which & ~uint32_t(W_DC | W_DM | W_TL | W_DABS | W_DA))) return COSMO_E_WHICH;
+    if (n == 0) return COSMO_OK;
+    if (!z1 || !z2 || !p.Om || !p.OL || !p.Or || !p.H0) return COSMO_E_NULL;
+    if (grad_out ? (!grad_z1 || !grad_z2 || !grad_params) : !out) return COSMO_E_NULL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    prof_begin(st);
+    k_two<<<(unsigned)cdiv(n, ELEM_THREADS), ELEM_THREADS, 0, st>>>(z1, z2, p.Om, p.OL, p.Or, p.H0, n, n_cosmo, which, grad_out, out, grad_z1,
+                                                                    grad_z2, grad_params, status);
+    prof_end(st);
+    return check_launch();
+}
+
 int cosmo_carlson_pair(const double* x, const double* m, const double* s, const double* p, int64_t n, double* rf, double* rd,
                        double* rj, void* stream) {
     if (n < 0) return COSMO_E_SIZE;

@@ -9,6 +9,7 @@
 #include <cuda_runtime.h>
 #include "cosmo_prep.cuh"
 #include "cosmo_obs.cuh"
+#include "cosmo_two.cuh"
 
 namespace cb {
 
@@ -414,6 +415,42 @@ __global__ void __launch_bounds__(ELEM_THREADS) k_elem(const T* __restrict__ z, 
         gz[i] = dz;
 #pragma unroll
         for (int j = 0; j < 4; ++j) gparams[(int64_t)j * N + i] = (double)gp[j];
+    }
+}
+
+// Two-limit evaluation (cosmo_two.cuh), one thread per (z1, z2, cosmology); n_cosmo in {1, n}.  which: DC, DM, TL, DABS, DA.
+__global__ void __launch_bounds__(ELEM_THREADS) k_two(const double* __restrict__ z1, const double* __restrict__ z2,
+                                                      const double* __restrict__ Om, const double* __restrict__ OL,
+                                                      const double* __restrict__ Or, const double* __restrict__ H0, int64_t n,
+                                                      int64_t n_cosmo, unsigned which, const double* __restrict__ gout,
+                                                      double* __restrict__ out, double* __restrict__ gz1, double* __restrict__ gz2,
+                                                      double* __restrict__ gparams, uint8_t* __restrict__ status) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const bool live = i < n;
+    const int64_t ii = live ? i : n - 1, ic = n_cosmo == 1 ? 0 : ii;
+    const bool with_grad = gout != nullptr;
+    Cosmo<double> C;
+    cosmo_prep(Om[ic], OL[ic], Or[ic], H0[ic], with_grad ? 2 : 0, C);
+    Two O;
+    eval_two<VoteWarp>(C, z1[ii], z2[ii], with_grad, VoteWarp(), O);
+    if (!live) return;
+    const unsigned bits[5] = {W_DC, W_DM, W_TL, W_DABS, W_DA};
+    double a1 = 0.0, a2 = 0.0, ap[4] = {0.0, 0.0, 0.0, 0.0};
+    int pl = 0;
+    for (int o = 0; o < 5; ++o) {
+        if (!(which & bits[o])) continue;
+        if (out != nullptr) out[(int64_t)pl * n + i] = O.v[o];
+        if (with_grad) {
+            const double g = gout[(int64_t)pl * n + i];
+            a1 = fma(g, O.gz1[o], a1); a2 = fma(g, O.gz2[o], a2);
+            for (int t = 0; t < 4; ++t) ap[t] = fma(g, O.gp[o][t], ap[t]);
+        }
+        ++pl;
+    }
+    if (status != nullptr) status[i] = (uint8_t)O.status;
+    if (with_grad) {
+        gz1[i] = a1; gz2[i] = a2;
+        for (int t = 0; t < 4; ++t) gparams[(int64_t)t * n + i] = ap[t];
     }
 }
 

@@ -5,6 +5,7 @@
 #include <stdint.h>
 #include "../../paper_2212_01937_b200/csrc/cosmo_prep.cuh"
 #include "../../paper_2212_01937_b200/csrc/cosmo_obs.cuh"
+#include "../../paper_2212_01937_b200/csrc/cosmo_two.cuh"
 
 using namespace cb;
 
@@ -54,4 +55,20 @@ extern "C" void hostcheck_factor(double Om, double OL, double Or, double* out5) 
     Cosmo<double> C;
     cosmo_prep(Om, OL, Or, 70.0, 0, C);
     out5[0] = C.m; out5[1] = C.rn; out5[2] = C.b; out5[3] = C.c; out5[4] = (double)C.status;
+}
+
+// two-limit path: val[5][n], gz1[5][n], gz2[5][n], gp[5][4][n]
+extern "C" void hostcheck_two(int64_t n, const double* z1, const double* z2, const double* Om, const double* OL, const double* Or,
+                              const double* H0, double* val, double* gz1, double* gz2, double* gp, uint8_t* status) {
+    for (int64_t i = 0; i < n; ++i) {
+        Cosmo<double> C;
+        cosmo_prep(Om[i], OL[i], Or[i], H0[i], 2, C);
+        Two O;
+        eval_two<VoteNone>(C, z1[i], z2[i], true, VoteNone(), O);
+        for (int o = 0; o < 5; ++o) {
+            val[o * n + i] = O.v[o]; gz1[o * n + i] = O.gz1[o]; gz2[o * n + i] = O.gz2[o];
+            for (int t = 0; t < 4; ++t) gp[(o * 4 + t) * n + i] = O.gp[o][t];
+        }
+        status[i] = (uint8_t)O.status;
+    }
 }

@@ -577,3 +577,32 @@ def test_snia_logjoint(cb, N, S):
         for p in range(4):
             assert abs(grad[p, s] - ref[1 + p]) <= TOL_GRAD * np.abs(resid * g[:, OBS["MU"], 1 + p]).sum(), (s, p)
         assert (np.abs(gz[s] - gz_ref) <= TOL_GRAD * np.maximum(np.abs(gz_ref), 1.0)).all(), s
+
+
+# ---------------------------------------------------------------- two-limit forms chi(z1,z2), t(z1,z2), d_abs(z1,z2)
+def test_two_limit(cb):
+    rng = np.random.default_rng(2)
+    n = 30_001
+    z1 = rng.uniform(0, 3, n); z2 = z1 + 10 ** rng.uniform(-3, 0.8, n)
+    Om = rng.uniform(.08, .6, n); OL = rng.uniform(0, 1.2, n); Or = rng.choice([0.0, 1e-5, 9e-5, 1e-3], n); H0 = rng.uniform(60, 80, n)
+    which = ("DC", "DM", "TL", "DABS", "DA")
+    g = rng.standard_normal((5, n))
+    out, g1, g2, gp, st = cb.cosmo_eval2(dev(z1), dev(z2), dev(Om), dev(OL), dev(Or), dev(H0), which, grad_out=dev(g))
+    out, g1, g2, gp, st = out.cpu().numpy(), g1.cpu().numpy(), g2.cpu().numpy(), gp.cpu().numpy(), st.cpu().numpy()
+    idx = np.arange(0, n, 5)
+    v, gr, so = oracle.observables2_batch(z1[idx], z2[idx], Om[idx], OL[idx], Or[idx], H0[idx])
+    v, gr = v.astype(np.float64), gr.astype(np.float64)
+    assert (so == 0).all() and (st[idx] == 0).all()
+    order = [oracle.OBS2.index(w) for w in which]           # planes are in ascending bit order: DC, DM, TL, DABS, DA
+    for k, o in enumerate(order):
+        assert relerr(out[k, idx], v[:, o]).max() <= TOL_VAL, which[k]
+    mine = [g1[idx], g2[idx]] + [gp[t, idx] for t in range(4)]
+    for c in range(6):
+        ref = sum(g[k, idx] * gr[:, o, c] for k, o in enumerate(order))
+        sab = sum(np.abs(g[k, idx] * gr[:, o, c]) for k, o in enumerate(order))
+        assert (np.abs(mine[c] - ref) <= (5e-8 if c == 4 else TOL_GRAD) * sab).all(), c
+    # one cosmology for all pairs, forward only; z1 = 0 reproduces the one-limit call
+    p = [dev(np.array([v_])) for v_ in (0.3, 0.7, 9e-5, 70.0)]
+    o2, *_ = cb.cosmo_eval2(dev(np.zeros(1000)), dev(z2[:1000]), *p, ("DC", "TL"))
+    o1, _ = cb.cosmo_eval(dev(z2[:1000]), *p, cb.ELEMENTWISE, ("DC", "TL"))
+    assert np.allclose(o2.cpu().numpy(), o1.cpu().numpy()[:, 0], rtol=1e-13, atol=0)

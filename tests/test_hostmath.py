@@ -171,6 +171,28 @@ def test_derived_observables_host(hc):
                 assert e.max() <= 1e-8, (oracle.DERIVED[i], oracle.WRT[k], e.max())
 
 
+def test_two_limit_host(hc):
+    """chi(z1,z2), D_M12, t(z1,z2), d_abs(z1,z2), D_A12 and their gradients (cosmo_two.cuh) against oracle.observables2_batch"""
+    rng = np.random.default_rng(1)
+    n = 1200
+    z1 = rng.uniform(0, 3, n); z2 = z1 + 10 ** rng.uniform(-3, 0.8, n)
+    Om = rng.uniform(.08, .6, n); OL = rng.uniform(0, 1.2, n); Or = rng.choice([0.0, 1e-5, 9e-5, 1e-3], n); H0 = rng.uniform(60, 80, n)
+    val = np.zeros((5, n)); g1 = np.zeros((5, n)); g2 = np.zeros((5, n)); gp = np.zeros((5, 4, n)); st = np.zeros(n, dtype=np.uint8)
+    dp = lambda a: a.ctypes.data_as(DP)
+    hc.hostcheck_two(C.c_int64(n), dp(z1), dp(z2), dp(Om), dp(OL), dp(Or), dp(H0), dp(val), dp(g1), dp(g2), dp(gp),
+                     st.ctypes.data_as(C.POINTER(C.c_uint8)))
+    v, g, so = oracle.observables2_batch(z1, z2, Om, OL, Or, H0)
+    v, g = v.astype(np.float64), g.astype(np.float64)
+    assert (so == 0).all() and (st == 0).all()
+    for o, nm in enumerate(oracle.OBS2):
+        assert (np.abs(val[o] - v[:, o]) / np.abs(v[:, o])).max() <= 1e-11, nm
+        mine = [g1[o], g2[o]] + [gp[o, t] for t in range(4)]
+        for k in range(6):
+            e = np.abs(mine[k] - g[:, o, k]) / np.maximum(np.abs(g[:, o, k]), 1e-3 * np.abs(v[:, o]))
+            tol = 5e-8 if (nm == "DABS" and k == 4) else 1e-8       # d(d_abs)/dOr: DESIGN.md section 6
+            assert e.max() <= tol, (nm, oracle.WRT2[k], e.max())
+
+
 def test_host_math_fp32(hc):
     w = W.config3(n=3000, S=1)
     z = w.z.astype(np.float32).astype(np.float64)
