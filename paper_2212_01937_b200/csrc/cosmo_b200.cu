@@ -56,11 +56,11 @@ int grid_y(int64_t ntiles, int64_t S) {
 
 struct WsLayout { size_t consts, part, gzpart, total; int ny; int64_t ntiles; };
 
-WsLayout ws_layout(int64_t n_z, int64_t n_cosmo, int mode, int with_grad, size_t elt) {
+WsLayout ws_layout(int64_t n_z, int64_t n_cosmo, int mode, uint32_t which, int with_grad, size_t elt) {
     WsLayout L{};
     const bool per_elem = (mode == COSMO_ELEMENTWISE && n_cosmo != 1);
     if (per_elem) { L.total = 0; L.ny = 1; L.ntiles = 0; return L; }
-    L.ntiles = cdiv(n_z > 0 ? n_z : 1, TILE);
+    L.ntiles = cdiv(n_z > 0 ? n_z : 1, outer_tile(which & (W_TL | W_AGE), which & W_DABS));   // as launch_outer dispatches
     L.ny = grid_y(L.ntiles, n_cosmo);
     L.consts = 0;
     size_t off = align256((size_t)n_cosmo * sizeof(Cosmo<double>));
@@ -132,7 +132,7 @@ int run_eval(const T* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode,
         return with_grad ? launch_elem<T, true>(z, p, n_z, which, gout, out, gz, gparams, status, st)
                          : launch_elem<T, false>(z, p, n_z, which, nullptr, out, nullptr, nullptr, status, st);
     }
-    WsLayout L = ws_layout(n_z, n_cosmo, mode, with_grad, sizeof(T));
+    WsLayout L = ws_layout(n_z, n_cosmo, mode, which, with_grad, sizeof(T));
     if (ws_bytes < L.total || !ws) return ws ? COSMO_E_WORKSPACE : COSMO_E_NULL;
     char* w = static_cast<char*>(ws);
     Cosmo<double>* consts = reinterpret_cast<Cosmo<double>*>(w + L.consts);
@@ -175,7 +175,7 @@ int run_snia(const T* z, const T* mu_obs, const T* sigma, int64_t N, cosmo_param
         if (grad) cudaMemsetAsync(grad, 0, sizeof(double) * 4 * S, st);
         return COSMO_OK;
     }
-    WsLayout L = ws_layout(N, S, COSMO_OUTER, 1, sizeof(T));
+    WsLayout L = ws_layout(N, S, COSMO_OUTER, W_MU, 1, sizeof(T));
     if (!ws) return COSMO_E_NULL;
     if (ws_bytes < L.total) return COSMO_E_WORKSPACE;
     char* w = static_cast<char*>(ws);
@@ -213,7 +213,7 @@ int run_joint(const T* z, const T* z_obs, const T* mu_obs, const T* sigma_mu, do
         if (grad) cudaMemsetAsync(grad, 0, sizeof(double) * 4 * S, st);
         return COSMO_OK;
     }
-    WsLayout L = ws_layout(N, S, COSMO_OUTER, 1, sizeof(T));
+    WsLayout L = ws_layout(N, S, COSMO_OUTER, W_MU, 1, sizeof(T));
     if (!ws) return COSMO_E_NULL;
     if (ws_bytes < L.total) return COSMO_E_WORKSPACE;
     char* w = static_cast<char*>(ws);
@@ -249,9 +249,8 @@ size_t g_host_cap = 0;
 extern "C" {
 
 size_t cosmo_workspace_bytes(int64_t n_z, int64_t n_cosmo, int mode, uint32_t which, int with_grad) {
-    (void)which;
     if (n_z < 0 || n_cosmo < 0) return 0;
-    WsLayout L = ws_layout(n_z, n_cosmo, mode, with_grad, sizeof(double));
+    WsLayout L = ws_layout(n_z, n_cosmo, mode, which, with_grad, sizeof(double));
     return L.total;
 }
 

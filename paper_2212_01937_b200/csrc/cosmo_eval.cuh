@@ -59,6 +59,37 @@ template <> struct Num<double> {
         return 1.0 / sqrt(a);
 #endif
     }
+    // sqrt(a), a > 0: same seed and cubic step applied to t = a y (one operation fewer than a * rsqrt_(a))
+    static CB_HD double sqrtp_(double a) {
+#ifdef __CUDA_ARCH__
+        double y;
+        asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+        const double t = a * y;
+        const double e = fma(-t, y, 1.0);
+        const double p = fma(0.375, e, 0.5);
+        return fma(t * e, p, t);
+#else
+        return sqrt(a);
+#endif
+    }
+    // 2a by an integer add on the exponent field (normal a; beside the FP64 pipe for free)
+    static CB_HD double twice_(double a) {
+#ifdef __CUDA_ARCH__
+        return __hiloint2double(__double2hiint(a) + 0x00100000, __double2loint(a));
+#else
+        return 2.0 * a;
+#endif
+    }
+    // magnitude key: a monotone integer image of |a| (the high word), for order-of-magnitude comparisons
+    static CB_HD int key_(double a) {
+#ifdef __CUDA_ARCH__
+        return __double2hiint(a) & 0x7fffffff;
+#else
+        long long b;
+        memcpy(&b, &a, 8);
+        return (int)((b >> 32) & 0x7fffffff);
+#endif
+    }
     static CB_HD double rcp_(double b) {
 #ifdef __CUDA_ARCH__
         double r;
@@ -100,6 +131,17 @@ template <> struct Num<float> {
 #endif
     }
     static CB_HD float rcp_(float b) { return 1.0f / b; }
+    static CB_HD float sqrtp_(float a) { return sqrtf(a); }
+    static CB_HD float twice_(float a) { return 2.0f * a; }
+    static CB_HD int key_(float a) {
+#ifdef __CUDA_ARCH__
+        return __float_as_int(a) & 0x7fffffff;
+#else
+        int b;
+        memcpy(&b, &a, 4);
+        return b & 0x7fffffff;
+#endif
+    }
     static constexpr float QF = 4.0f;      // same rule at r ~ 6e-8
     static constexpr float QJ = 6.0f;
     static constexpr float RC_SMALL = 0.25f;
@@ -157,75 +199,88 @@ struct Core {
 // real-symmetric form: K argument triples (xa, mp + h, mp - h), h^2 = s (s < 0: a complex-conjugate pair), advanced in
 // lock-step by lambda = sqrt(x)sqrt(y) + sqrt(x)sqrt(z) + sqrt(y)sqrt(z) until every lane of the warp meets the stopping
 // rule (no divergence).  One pass serves R_F, the R_D(., ., xa) tail (kD) and the tails of R_J(., ., ., p5) (kT) and
-// R_J(., ., ., p0) (kA); dl = (p - xa)((p - mp)^2 - s) is Carlson's delta of each R_J.  On return the arguments hold the
-// reduced values, f = 4^-n.
+// R_J(., ., ., p0) (kA); dl = (p - xa)((p - mp)^2 - s) is Carlson's delta of each R_J.
+//
+// UNSCALED form: ref. [10] divides the arguments by 4 every step, x_{n+1} = (x_n + lambda_n)/4.  Here the arguments are
+// X_n = 4^n x_n, X_{n+1} = X_n + Lambda_n: by homogeneity (R_F of degree -1/2, R_D and R_J of degree -3/2) this is the same
+// algorithm with every power of 4 taken out -- exactly, since the factors are powers of two -- and it is cheaper: the
+// pair's s = h^2 is invariant, the stopping rule 4^-n Q dev < |a_n| becomes Q dev < |A_n| with a constant left side, and
+// Carlson's e_n = delta_n/d_n^2 needs no 4^-3n.  On return the arguments hold X_n and g2 = 2^n; the tails are
+// sum 2^m/(sqrt(Z_m)(Z_m + Lambda_m)) and sum 2^m R_C(1, 1 + e_m)/D_m, equal term by term to the scaled ones.
 template <typename T, bool kD, bool kT, bool kA, int K, typename Vote>
-CB_HD void carlson_dup(T (&xa)[K], T (&mp)[K], T (&s)[K], T (&p5)[K], T (&p0)[K], const T (&dl5)[K], const T (&dl0)[K],
-                       const T (&Qc)[K], const T (&Q5v)[K], const T (&Q0v)[K], unsigned (&st)[K], const Vote& vote, T& f,
+CB_HD void carlson_dup(T (&xa)[K], T (&mp)[K], const T (&s)[K], T (&p5)[K], T (&p0)[K], const T (&dl5)[K], const T (&dl0)[K],
+                       const T (&Qc)[K], const T (&Q5v)[K], const T (&Q0v)[K], unsigned (&st)[K], const Vote& vote, T& g2,
                        T (&tailD)[K], T (&sum5)[K], T (&sum0)[K]) {
     using N = Num<T>;
-    f = T(1);
+    g2 = T(1);
+    // thresholds as magnitude keys (Num<T>::key_): the rule needs a few significant bits, and integer compares are free
+    // beside the FP64 pipe
+    int kF[K], kDd[K], k5[K], k0[K];
 #pragma unroll
-    for (int k = 0; k < K; ++k) tailD[k] = sum5[k] = sum0[k] = T(0);
+    for (int k = 0; k < K; ++k) {
+        tailD[k] = sum5[k] = sum0[k] = T(0);
+        kF[k] = N::key_(T(3) * Qc[k]);
+        kDd[k] = N::key_(T(5) * Qc[k]);
+        k5[k] = N::key_(T(5) * Q5v[k]);
+        k0[k] = N::key_(T(5) * Q0v[k]);
+    }
     int nit = 0;
-    for (;;) {
-        bool more = false;
+    auto more = [&]() -> bool {            // stopping rule; branch-free: plain | and & on the comparison results
+        bool any = false;
         const bool cap = nit >= NIT_CAP;
 #pragma unroll
-        for (int k = 0; k < K; ++k) {      // branch-free: plain | and & on the comparison results
-            const T fq = f * Qc[k];
-            bool mk = T(3) * fq >= N::abs_(N::fma_(T(2), mp[k], xa[k]));
-            if (kD) mk = mk | (T(5) * fq >= N::abs_(N::fma_(T(3), xa[k], T(2) * mp[k])));
-            if (kT) mk = mk | (f * Q5v[k] >= N::abs_(xa[k] + T(2) * mp[k] + T(2) * p5[k]) * T(0.2));
-            if (kA) mk = mk | (f * Q0v[k] >= N::abs_(xa[k] + T(2) * mp[k] + T(2) * p0[k]) * T(0.2));
+        for (int k = 0; k < K; ++k) {
+            const T a3 = N::fma_(T(2), mp[k], xa[k]);                       // 3 A_n of R_F
+            bool mk = kF[k] >= N::key_(a3);
+            if (kD) mk = mk | (kDd[k] >= N::key_(N::fma_(T(2), xa[k], a3)));           // 5 A_n of R_D
+            if (kT) mk = mk | (k5[k] >= N::key_(N::fma_(T(2), p5[k], a3)));            // 5 A_n of R_J(p5)
+            if (kA) mk = mk | (k0[k] >= N::key_(N::fma_(T(2), p0[k], a3)));
             mk = mk & (st[k] == 0);
             if (cap) { st[k] |= mk ? (unsigned)ST_ITER_CAP : 0u; mk = false; }
-            more = more | mk;
+            any = any | mk;
         }
-        if (!vote.any(more)) break;
+        return any;
+    };
+    auto step = [&]() {
 #pragma unroll
         for (int k = 0; k < K; ++k) {
-            const T rx = N::rsqrt_(xa[k]);
-            const T sx = xa[k] * rx;
+            const T sx = N::sqrtp_(xa[k]);
             const T P = N::fma_(mp[k], mp[k], -s[k]);
-            const T spd = P * N::rsqrt_(P);
-            const T Q = T(2) * (mp[k] + spd);
-            const T sa = Q * N::rsqrt_(Q);
+            const T spd = N::sqrtp_(P);
+            const T sa = N::sqrtp_(N::twice_(mp[k] + spd));
             const T lam = N::fma_(sx, sa, spd);
-            if (kD) tailD[k] = N::fma_(f * rx, N::rcp_(xa[k] + lam), tailD[k]);
+            const T w = xa[k] + lam;
+            if (kD) tailD[k] = N::fma_(g2, N::rcp_(sx * w), tailD[k]);
             if (kT) {
-                const T rp = p5[k] * N::rsqrt_(p5[k]);
+                const T rp = N::sqrtp_(p5[k]);
                 const T d = (rp + sx) * (p5[k] + N::fma_(rp, sa, spd));
                 const T id = N::rcp_(d);
-                const T e = f * f * f * dl5[k] * id * id;
-                sum5[k] = N::fma_(f * id, rc1<T>(e), sum5[k]);
-                p5[k] = T(0.25) * (p5[k] + lam);
+                sum5[k] = N::fma_(g2 * id, rc1<T>(dl5[k] * id * id), sum5[k]);
+                p5[k] += lam;
             }
             if (kA) {
-                const T rp = p0[k] * N::rsqrt_(p0[k]);
+                const T rp = N::sqrtp_(p0[k]);
                 const T d = (rp + sx) * (p0[k] + N::fma_(rp, sa, spd));
                 const T id = N::rcp_(d);
-                const T e = f * f * f * dl0[k] * id * id;
-                sum0[k] = N::fma_(f * id, rc1<T>(e), sum0[k]);
-                p0[k] = T(0.25) * (p0[k] + lam);
+                sum0[k] = N::fma_(g2 * id, rc1<T>(dl0[k] * id * id), sum0[k]);
+                p0[k] += lam;
             }
-            const T ql = T(0.25) * lam;
-            xa[k] = N::fma_(T(0.25), xa[k], ql);
-            mp[k] = N::fma_(T(0.25), mp[k], ql);
-            s[k] *= T(CB_KT.sixteenth_inv);
+            xa[k] = w;
+            mp[k] += lam;
         }
-        f *= T(0.25);
+        g2 = N::twice_(g2);
         ++nit;
-    }
+    };
+    while (vote.any(more())) step();
 }
 
-// R_F(xa0, m0 + h0, m0 - h0) from the reduced arguments: degree-7 series in E2, E3 (DLMF 19.36.1); hd = xa0 - m0, s0 = h0^2
+// R_F(xa0, m0 + h0, m0 - h0) from the arguments after n steps (unscaled, g2 = 2^n): degree-7 series in E2, E3 (DLMF 19.36.1); hd = xa0 - m0, s0 = h0^2
 template <typename T>
-CB_HD T carlson_rf_series(T xa_n, T mp_n, T f, T hd, T s0) {
+CB_HD T carlson_rf_series(T xa_n, T mp_n, T g2, T hd, T s0) {
     using N = Num<T>;
     const T An = (xa_n + T(2) * mp_n) * T(CB_KT.third);
     const T rA = N::rsqrt_(An);
-    const T g = f * rA * rA;
+    const T g = rA * rA;                                   // 1/A_n (unscaled) = 4^-n / a_n
     const T dl = hd * T(CB_KT.third) * g;
     const T vs = s0 * g * g;
     const T e2 = T(-3) * dl * dl - vs;
@@ -235,16 +290,16 @@ CB_HD T carlson_rf_series(T xa_n, T mp_n, T f, T hd, T s0) {
     const T ta = N::fma_(e2, N::fma_(e2, T(c[2]), T(c[1])), T(c[0]));
     const T tb = N::fma_(e3, T(c[6]), N::fma_(e2, N::fma_(e2, T(c[5]), T(c[4])), T(c[3])));
     const T S = N::fma_(e3, tb, N::fma_(e2, ta, T(1)));
-    return S * rA;
+    return S * (g2 * rA);                                  // a_n^(-1/2) = 2^n A_n^(-1/2)
 }
 
 // R_D(m0 + h0, m0 - h0, xa0): series (DLMF 19.36.2) + 3 x the tail summed by carlson_dup
 template <typename T>
-CB_HD T carlson_rd_series(T xa_n, T mp_n, T f, T hd, T s0, T tailD) {
+CB_HD T carlson_rd_series(T xa_n, T mp_n, T g2, T hd, T s0, T tailD) {
     using N = Num<T>;
     const T AD = (T(3) * xa_n + T(2) * mp_n) * T(0.2);
     const T rA = N::rsqrt_(AD);
-    const T g = f * rA * rA;
+    const T g = rA * rA;
     const T dd = hd * T(0.2) * g;
     const T XY = T(9) * dd * dd - s0 * g * g;
     const T Z = T(-2) * dd, Z2 = Z * Z;
@@ -252,17 +307,17 @@ CB_HD T carlson_rd_series(T xa_n, T mp_n, T f, T hd, T s0, T tailD) {
     const T e3 = (T(3) * XY - T(8) * Z2) * Z;
     const T e4 = T(3) * (XY - Z2) * Z2;
     const T e5 = XY * Z2 * Z;
-    return N::fma_(g * rA, series_J<T>(e2, e3, e4, e5), T(3) * tailD);
+    return N::fma_(g2 * g * rA, series_J<T>(e2, e3, e4, e5), T(3) * tailD);     // 4^-n a_n^(-3/2) = 2^n A_n^(-3/2)
 }
 
 // R_J(xa0, m0 + h0, m0 - h0, p_init): series + 6 x the tail summed by carlson_dup
 template <typename T>
-CB_HD T carlson_rj_series(T xa_n, T mp_n, T p_n, T f, T xa0, T m0, T s0, T p_init, T sum) {
+CB_HD T carlson_rj_series(T xa_n, T mp_n, T p_n, T g2, T xa0, T m0, T s0, T p_init, T sum) {
     using N = Num<T>;
     const T An = (xa_n + T(2) * mp_n + T(2) * p_n) * T(0.2);
     const T A0 = (xa0 + T(2) * m0 + T(2) * p_init) * T(0.2);
     const T rA = N::rsqrt_(An);
-    const T g = f * rA * rA;
+    const T g = rA * rA;
     const T X = (A0 - xa0) * g;
     const T am = A0 - m0;
     const T YpZ = T(2) * am * g;
@@ -274,7 +329,7 @@ CB_HD T carlson_rj_series(T xa_n, T mp_n, T p_n, T f, T xa0, T m0, T s0, T p_ini
     const T e3 = XYZ + T(2) * e2 * P + T(4) * P2 * P;
     const T e4 = (T(2) * XYZ + e2 * P + T(3) * P2 * P) * P;
     const T e5 = XYZ * P2;
-    return N::fma_(g * rA, series_J<T>(e2, e3, e4, e5), T(6) * sum);
+    return N::fma_(g2 * g * rA, series_J<T>(e2, e3, e4, e5), T(6) * sum);
 }
 
 // stopping-rule bounds (ref. [10]; constants: see Num<T>::QF): Qc for R_F / R_D, Qj for an R_J with parameter p
@@ -344,8 +399,8 @@ CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Cor
         if (kA) Q0v[k] = carlson_Qj<T>(xa[k], mp[k], hs, p0[k]);
     }
     // ---- S5 fused duplication
-    T f, tailD[K], sum5[K], sum0[K];
-    carlson_dup<T, kD, kT, kA, K, Vote>(xa, mp, s, p5, p0, dl5, dl0, Qc, Q5v, Q0v, st, vote, f, tailD, sum5, sum0);
+    T g2, tailD[K], sum5[K], sum0[K];
+    carlson_dup<T, kD, kT, kA, K, Vote>(xa, mp, s, p5, p0, dl5, dl0, Qc, Q5v, Q0v, st, vote, g2, tailD, sum5, sum0);
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         const T x = T(1) + z[k];
@@ -354,7 +409,7 @@ CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Cor
         const T xmr = x - C.rn;
         const T q2x = N::fma_(x + C.b, x, C.c);
         const T hd = T(0.5) * z2 * C.theta;                // xa0 - m0
-        const T xa0 = U12[k] * U12[k], m0 = xa0 - hd, s0 = z2 * z2 * C.sD;
+        const T xa0 = U12[k] * U12[k], m0 = xa0 - hd, s0 = s[k];
         {   // E(z), 1/E(z) and E(z) - 1 (for d/dz and the boundary terms of the gradients)
             const T Ev = (U12[k] - ra[k]) * ra[k];          // sqrt(a2) sqrt(a1)
             const T xp1 = x + T(1);
@@ -365,9 +420,9 @@ CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Cor
             R[k].iE = iE[k];
         }
         // ---- series
-        const T RF = carlson_rf_series<T>(xa[k], mp[k], f, hd, s0);
+        const T RF = carlson_rf_series<T>(xa[k], mp[k], g2, hd, s0);
         R[k].I0 = T(2) * z[k] * RF;                       // eq. (3.7) / (B.1)
-        const T RD = kD ? carlson_rd_series<T>(xa[k], mp[k], f, hd, s0, tailD[k]) : T(0);     // R_D(u13^2, u14^2, u12^2)
+        const T RD = kD ? carlson_rd_series<T>(xa[k], mp[k], g2, hd, s0, tailD[k]) : T(0);     // R_D(u13^2, u14^2, u12^2)
         const T rUx = N::rcp_(U12[k] * xmr);               // 1/(u12 (x - rn))
         const T rU = xmr * rUx;
         R[k].K = T(0); R[k].TT = T(0); R[k].AA = T(0);
@@ -378,7 +433,7 @@ CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Cor
         }
         if (kT) {
             // eq. (3.8) with i = big root, j = rn, scaled so that Or -> 0 reproduces (B.2)
-            const T RJ5 = carlson_rj_series<T>(xa[k], mp[k], p5[k], f, xa0, m0, s0, p5_0[k], sum5[k]);
+            const T RJ5 = carlson_rj_series<T>(xa[k], mp[k], p5[k], g2, xa0, m0, s0, p5_0[k], sum5[k]);
             const T qh = x * p5_0[k] * C.qhc / lin;
             const T sh = N::fma_(z2, C.OL, qh);
             R[k].TT = T(2) * z[k] * (z2 * T(CB_KT.third) * C.Gp * RJ5 + rc<T>(sh, qh) - C.OrM * RF);
@@ -387,7 +442,7 @@ CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Cor
             const T bnd = N::sqrt_(xmr * (T(1) - C.rn)) * rU;
             if (quartA) {
                 // eq. (3.9) with (i,j,k,l) = (rn, pair, pair, big)
-                const T RJ0 = carlson_rj_series<T>(xa[k], mp[k], p0[k], f, xa0, m0, s0, p0_0[k], sum0[k]);
+                const T RJ0 = carlson_rj_series<T>(xa[k], mp[k], p0[k], g2, xa0, m0, s0, p0_0[k], sum0[k]);
                 const T q0 = p0_0[k] / ((T(1) - C.rn) * xmr);
                 const T s0q = N::fma_(C.Or, z2, q0);
                 // third-kind bracket of (3.9): 2 z B0 = int (x - rn) dx / E

@@ -17,11 +17,17 @@ namespace cb {
 #define CB_THREADS 128
 #endif
 constexpr int OUTER_THREADS = CB_THREADS;
-#ifndef CB_KZ
-#define CB_KZ 2
+// consecutive redshifts per thread (even), advanced in lock-step.  Per-thread overhead (staging, address arithmetic, the
+// warp reduction, constant and shared-memory loads) is paid once per KZ elements, so the chi family -- whose working set
+// fits -- takes 4; the kernels that also carry the R_J tracks (t_L, d_abs) stay at 2 (4 spills).  Measured: profiles/.
+#ifndef CB_KZ_CHI
+#define CB_KZ_CHI 4
 #endif
-constexpr int KZ = CB_KZ;                           // consecutive redshifts per thread (even)
-constexpr int TILE = OUTER_THREADS * KZ;            // redshifts per block
+#ifndef CB_KZ_TA
+#define CB_KZ_TA 2
+#endif
+__host__ __device__ constexpr int outer_kz(bool kT, bool kA) { return (kT || kA) ? CB_KZ_TA : CB_KZ_CHI; }
+__host__ __device__ constexpr int outer_tile(bool kT, bool kA) { return OUTER_THREADS * outer_kz(kT, kA); }   // redshifts per block
 #ifndef CB_SCHUNK
 #define CB_SCHUNK 16
 #endif
@@ -75,7 +81,7 @@ template <typename T> struct Vec2;
 template <> struct Vec2<double> { using type = double2; };
 template <> struct Vec2<float> { using type = float2; };
 
-template <typename T>
+template <typename T, int KZ>
 __device__ __forceinline__ void load2(const T* __restrict__ p, int64_t i, int64_t n, bool vec, T (&v)[KZ]) {
 #pragma unroll
     for (int k = 0; k < KZ; k += 2) {
@@ -88,7 +94,7 @@ __device__ __forceinline__ void load2(const T* __restrict__ p, int64_t i, int64_
         }
     }
 }
-template <typename T>
+template <typename T, int KZ>
 __device__ __forceinline__ void store2(T* __restrict__ p, int64_t i, int64_t n, bool vec, const T (&v)[KZ]) {
 #pragma unroll
     for (int k = 0; k < KZ; k += 2) {
@@ -123,6 +129,7 @@ template <typename T, bool kT, bool kA, int MODE>
 __device__ __noinline__ void outer_c4_row(const OuterArgs& a, const Cosmo<T>& C, int64_t row, int64_t n0, const T* zv, const T* mo,
                                           const T* isig2, const T* lnorm, unsigned which, double* sacc_row, int lane, T* gzacc) {
     constexpr int NP = (MODE == MODE_SNIA || MODE == MODE_JOINT) ? 5 : 4;
+    constexpr int KZ = outer_kz(kT, kA);
     const int64_t N = a.N, S = a.S;
     T ll = T(0);
     for (int k = 0; k < KZ; ++k) {
@@ -161,10 +168,11 @@ __device__ __noinline__ void outer_c4_row(const OuterArgs& a, const Cosmo<T>& C,
 
 // OUTER forward / fused forward+VJP / fused likelihood.  grid = (tiles of TILE redshifts, S-chunk groups).
 #ifndef CB_MINBLOCKS
-#define CB_MINBLOCKS 4     // chi-family kernels: 128 registers, 16 warps/SM (measured best, profiles/)
+#define CB_MINBLOCKS 3     // chi-family kernels: 160 registers, 12 warps/SM (measured best with KZ = 4, profiles/)
 #endif
 template <typename T, bool kT, bool kA, int MODE, unsigned WCT>
-__global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) k_outer(OuterArgs a) {
+__global__ void __launch_bounds__(OUTER_THREADS, CB_MINBLOCKS) k_outer(OuterArgs a) {
+    constexpr int KZ = outer_kz(kT, kA), TILE = outer_tile(kT, kA);
     const unsigned which = WCT ? WCT : a.which;      // WCT != 0: output set known at compile time (drops dead planes)
     constexpr bool kG = MODE != MODE_FWD;
     constexpr bool kLike = MODE == MODE_SNIA || MODE == MODE_JOINT;
@@ -172,21 +180,21 @@ __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) 
     __shared__ Cosmo<T> sc[S_CHUNK];
     __shared__ double sacc[kG ? NWARP : 1][kG ? S_CHUNK : 1][NP];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int64_t N = a.N, S = a.S;
+    const int64_t N = a.N, S = a.S, SN = S * N;
     const int64_t n0 = (int64_t)blockIdx.x * TILE + (int64_t)tid * KZ;
     const bool vec = a.vec != 0;
     const T* zp = static_cast<const T*>(a.z);
     T zv[KZ];
-    load2<T>(zp, n0, N, vec, zv);
+    load2(zp, n0, N, vec, zv);
     bool live[KZ];
 #pragma unroll
     for (int k = 0; k < KZ; ++k) live[k] = n0 + k < N;
     T mo[KZ], isig2[KZ], lnorm[KZ], zo[KZ];
-    if (MODE == MODE_JOINT) load2<T>(static_cast<const T*>(a.z_obs), n0, N, vec, zo);
+    if (MODE == MODE_JOINT) load2(static_cast<const T*>(a.z_obs), n0, N, vec, zo);
     if (kLike) {
         T sg[KZ];
-        load2<T>(static_cast<const T*>(a.mu_obs), n0, N, vec, mo);
-        load2<T>(static_cast<const T*>(a.sigma), n0, N, vec, sg);
+        load2(static_cast<const T*>(a.mu_obs), n0, N, vec, mo);
+        load2(static_cast<const T*>(a.sigma), n0, N, vec, sg);
 #pragma unroll
         for (int k = 0; k < KZ; ++k) {
             isig2[k] = T(1) / (sg[k] * sg[k]);
@@ -210,16 +218,19 @@ __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) 
             sc[sl].cubic = a.consts[c0 + sl].cubic;
         }
         __syncthreads();
-        for (int sl = 0; sl < ns; ++sl) {
+        int64_t roff = c0 * N;                                   // row * N, advanced by N per cosmology (no 64-bit multiplies)
+        for (int sl = 0; sl < ns; ++sl, roff += N) {
             const Cosmo<T>& C = sc[sl];
             const int64_t row = c0 + sl;
-            if (MODE == MODE_JOINT) load2<T>(zp + row * N, n0, N, vec, zv);      // latent redshifts: one row per sample
+            if (MODE == MODE_JOINT) load2(zp + roff, n0, N, vec, zv);      // latent redshifts: one row per sample
             if (MODE == MODE_JOINT && (C.cubic & 2u)) {                          // no gradients on the complex slow path: NaN row
                 if (lane == 0)
                     for (int j = 0; j < NP; ++j) sacc[warp][sl][j] = NAN;
                 if (a.gz != nullptr) {
-                    const T nn[KZ] = {T(NAN), T(NAN)};
-                    store2<T>(static_cast<T*>(a.gz) + row * N, n0, N, vec, nn);
+                    T nn[KZ];
+#pragma unroll
+                    for (int k = 0; k < KZ; ++k) nn[k] = T(NAN);
+                    store2(static_cast<T*>(a.gz) + roff, n0, N, vec, nn);
                 }
                 continue;
             }
@@ -241,9 +252,9 @@ __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) 
                 for (int w = 0; w < N_PLANES; ++w) {
                     if (!(which >> w & 1)) continue;
                     T t[KZ];
-                    load2<T>(static_cast<const T*>(a.gout) + ((int64_t)pl * S + row) * N, n0, N, vec, t);
+                    load2(static_cast<const T*>(a.gout) + ((int64_t)pl * SN + roff), n0, N, vec, t);
 #pragma unroll
-                    for (int k = 0; k < KZ; ++k) g[k][w] = t[k];
+                    for (int k = 0; k < KZ; ++k) g[k][w] = live[k] ? t[k] : T(0);
                     ++pl;
                 }
             }
@@ -251,10 +262,11 @@ __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) 
             uint8_t stv[KZ];
             Core<T> R[KZ];
             eval_core_k<T, kT, kA, kG, KZ, VoteWarp>(C, zv, vote, R);
+            Obs<T> Ok[KZ];
+            observables_k<T, kT, kA, KZ>(C, zv, R, kLike ? (unsigned)W_MU : which, Ok);
 #pragma unroll
             for (int k = 0; k < KZ; ++k) {
-                Obs<T> O;
-                observables<T, kT, kA>(C, zv[k], R[k], kLike ? (unsigned)W_MU : which, O);
+                const Obs<T>& O = Ok[k];
 #pragma unroll
                 for (int w = 0; w < N_PLANES; ++w) ov[w][k] = O.v[w];
                 stv[k] = (uint8_t)O.status;
@@ -280,29 +292,23 @@ __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) 
                         for (int j = 0; j < 4; ++j) pacc[1 + j] += gp[j];
                     }
                 }
-                if (MODE == MODE_VJP) {
-                    T dz = T(0), gp[4] = {T(0), T(0), T(0), T(0)};
-                    backward<T, kT, kA>(C, zv[k], R[k], O, g[k], dz, gp);
-                    if (live[k]) {
-                        gzacc[k] += dz;
-#pragma unroll
-                        for (int j = 0; j < 4; ++j) pacc[j] += gp[j];
-                    }
-                }
+                // straight into the accumulators: elements past N carry zero upstream gradients (see the load) and their
+                // grad_z is never stored
+                if (MODE == MODE_VJP) backward<T, kT, kA>(C, zv[k], R[k], O, g[k], gzacc[k], pacc, nullptr, which);
             }
-            if (MODE == MODE_JOINT && a.gz != nullptr) store2<T>(static_cast<T*>(a.gz) + row * N, n0, N, vec, gzacc);
+            if (MODE == MODE_JOINT && a.gz != nullptr) store2(static_cast<T*>(a.gz) + roff, n0, N, vec, gzacc);
             if (!kLike && a.out != nullptr) {
                 int pl = 0;
                 for (int w = 0; w < N_PLANES; ++w) {
                     if (!(which >> w & 1)) continue;
-                    store2<T>(static_cast<T*>(a.out) + ((int64_t)pl * S + row) * N, n0, N, vec, ov[w]);
+                    store2(static_cast<T*>(a.out) + ((int64_t)pl * SN + roff), n0, N, vec, ov[w]);
                     ++pl;
                 }
             }
             if (!kLike && a.status != nullptr) {
 #pragma unroll
                 for (int k = 0; k < KZ; ++k)
-                    if (live[k]) a.status[row * N + n0 + k] = stv[k];
+                    if (live[k]) a.status[roff + n0 + k] = stv[k];
             }
             if (kG) {
                 const double v4[4] = {(double)pacc[NP - 4], (double)pacc[NP - 3], (double)pacc[NP - 2], (double)pacc[NP - 1]};
@@ -327,7 +333,7 @@ __global__ void __launch_bounds__(OUTER_THREADS, (kT || kA) ? 3 : CB_MINBLOCKS) 
     }
     if (MODE == MODE_VJP) {
         T* gzp = static_cast<T*>(a.gz) + (a.gz_accumulate ? (int64_t)blockIdx.y * N : 0);
-        store2<T>(gzp, n0, N, vec, gzacc);
+        store2(gzp, n0, N, vec, gzacc);
     }
 }
 

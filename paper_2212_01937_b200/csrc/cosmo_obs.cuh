@@ -68,36 +68,70 @@ CB_HD void volume(T k, T I0, T& v, T& vk) {
     }
 }
 
+// K elements of the same cosmology at once.  The common case (|Ok I0^2| <= 1/2, D_L > 0) is straight-line code for all K
+// elements -- one basic block, so that the K dependency chains (three Horner polynomials and the ln series each) interleave
+// in the FP64 pipe; everything else goes through the generic per-element forms.
+template <typename T, bool kT, bool kA, int K>
+CB_HD void observables_k(const Cosmo<T>& C, const T (&z)[K], const Core<T> (&R)[K], unsigned which, Obs<T> (&O)[K]) {
+    using N = Num<T>;
+    // elements whose path crosses a root or leaves the domain: every plane is NaN.  One select on the integral poisons
+    // everything derived from it (the other integrals are selected below), instead of one select per plane.
+    T I0[K];
+    bool bad[K];
+    T wmax = T(0);
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        bad[k] = (R[k].status & (ST_ROOT_ON_PATH | ST_UNSUPPORTED)) != 0;
+        I0[k] = bad[k] ? T(NAN) : R[k].I0;
+        wmax = N::max_(wmax, N::abs_(C.Ok * I0[k] * I0[k]));
+    }
+    if (wmax <= T(0.5)) {
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            T sf, sg, sd;
+            sinn_poly<T, 7>(C.Ok * I0[k] * I0[k], sf, sg, sd);
+            O[k].F = I0[k] * sf; O[k].Fi = sg; O[k].Fk = I0[k] * I0[k] * I0[k] * sd;
+        }
+    } else {
+        for (int k = 0; k < K; ++k) sinn<T>(C.Ok, I0[k], O[k].F, O[k].Fi, O[k].Fk);
+    }
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        const T x = T(1) + z[k];
+        unsigned st = R[k].status;
+        O[k].v[0] = C.dH * I0[k];
+        O[k].v[1] = C.dH * O[k].F;
+        O[k].v[2] = x * O[k].v[1];
+        O[k].v[3] = T(0);
+        if (which & W_MU) {
+            const bool pos = O[k].v[2] > T(0);              // branch-free: ln of a harmless stand-in, then select
+            const T mu = N::fma_(T(CB_KT.five_over_ln10), N::log_(pos ? O[k].v[2] : T(1)), T(25));
+            O[k].v[3] = pos ? mu : T(NAN);
+            st |= (pos || bad[k]) ? 0u : (unsigned)ST_DL_NONPOS;
+        }
+        const T TT = kT ? (bad[k] ? T(NAN) : R[k].TT) : T(0);
+        O[k].v[4] = C.tH * TT;
+        O[k].v[5] = kA ? C.dH * (bad[k] ? T(NAN) : R[k].AA) : T(0);
+        O[k].v[6] = O[k].v[7] = O[k].v[8] = T(0);
+        O[k].Vk = T(0);
+        if (which & W_DA) O[k].v[6] = O[k].v[1] / x;
+        if (which & W_VC) {
+            T v;
+            volume<T>(C.Ok, I0[k], v, O[k].Vk);
+            O[k].v[7] = T(12.566370614359172954) * C.dH * C.dH * C.dH * v;
+        }
+        if (kT && (which & W_AGE)) O[k].v[8] = C.tH * (C.Tinf - TT);
+        O[k].status = st;
+    }
+}
+
 template <typename T, bool kT, bool kA>
 CB_HD void observables(const Cosmo<T>& C, T z, const Core<T>& R, unsigned which, Obs<T>& O) {
-    using N = Num<T>;
-    const T x = T(1) + z;
-    unsigned st = R.status;
-    sinn<T>(C.Ok, R.I0, O.F, O.Fi, O.Fk);
-    O.v[0] = C.dH * R.I0;
-    O.v[1] = C.dH * O.F;
-    O.v[2] = x * O.v[1];
-    O.v[3] = T(0);
-    if (which & W_MU) {
-        if (O.v[2] > T(0)) O.v[3] = N::fma_(T(CB_KT.five_over_ln10), N::log_(O.v[2]), T(25));
-        else { O.v[3] = T(NAN); st |= ST_DL_NONPOS; }
-    }
-    O.v[4] = kT ? C.tH * R.TT : T(0);
-    O.v[5] = kA ? C.dH * R.AA : T(0);
-    O.v[6] = O.v[7] = O.v[8] = T(0);
-    O.Vk = T(0);
-    if (which & W_DA) O.v[6] = O.v[1] / x;
-    if (which & W_VC) {
-        T v;
-        volume<T>(C.Ok, R.I0, v, O.Vk);
-        O.v[7] = T(12.566370614359172954) * C.dH * C.dH * C.dH * v;
-    }
-    if (kT && (which & W_AGE)) O.v[8] = C.tH * (C.Tinf - R.TT);
-    if (st & (ST_ROOT_ON_PATH | ST_UNSUPPORTED)) {
-#pragma unroll
-        for (int i = 0; i < N_PLANES; ++i) O.v[i] = T(NAN);
-    }
-    O.status = st;
+    const T zz[1] = {z};
+    const Core<T> RR[1] = {R};
+    Obs<T> OO[1];
+    observables_k<T, kT, kA, 1>(C, zz, RR, which, OO);
+    O = OO[0];
 }
 
 // Age (int_z^inf of eq. (2.4)): age(z) = tH (Tinf - T(z)).  Tinf = int_1^inf dx/(x E) is one more evaluation of
@@ -129,8 +163,11 @@ CB_HD void prep_age(Cosmo<double>& C, bool with_grad) {
 // VJP of one element: g[N_PLANES] upstream (entries outside `which` must be 0).  Adds to gz and gp[0..3] = (Om, OL, Or, H0).
 // kCond: also return in *cond the cancellation factor max_theta sum_j |G_j basis_j| / max(|dI0/dtheta|, 1e-3 |I0|) of the
 // chi-family gradient (status bit 16 of the ELEMENTWISE calls is derived from it).
+// `which`: planes that can carry a non-zero upstream gradient; where the caller knows it at compile time the terms of the
+// other planes fold away (x * 0 is not foldable in IEEE arithmetic, so a zero g alone does not remove them).
 template <typename T, bool kT, bool kA, bool kCond = false>
-CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, const T g[N_PLANES], T& gz, T gp[4], T* cond = nullptr) {
+CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, const T g[N_PLANES], T& gz, T gp[4], T* cond = nullptr,
+                    unsigned which = W_ALL) {
     using N = Num<T>;
     const T x = T(1) + z;
     const T iE = R.iE;
@@ -140,12 +177,14 @@ CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, c
     const T xp1 = x + T(1);
     const T n1 = z, n2 = z * xp1, n3 = z * N::fma_(xp1, x, T(1)), n4 = n2 * N::fma_(x, x, T(1));
     const T bt0 = -R.Em1 * iE, bt1 = (n1 - R.Em1) * iE, bt2 = (n2 - R.Em1) * iE;
-    T gM = g[1] + x * g[2];
-    if (g[3] != T(0)) gM += T(CB_KT.five_over_ln10) * g[3] * (x * rxd);
-    if (g[6] != T(0)) gM += g[6] * ix;                                  // D_A = D_M / (1+z)
-    T aI = C.dH * N::fma_(gM, O.Fi, g[0]);
+    T gM = T(0);
+    if (which & W_DM) gM = g[1];
+    if (which & W_DL) gM = N::fma_(x, g[2], gM);
+    if ((which & W_MU) && g[3] != T(0)) gM = N::fma_(T(CB_KT.five_over_ln10) * g[3], x * rxd, gM);
+    if ((which & W_DA) && g[6] != T(0)) gM = N::fma_(g[6], ix, gM);     // D_A = D_M / (1+z)
+    T aI = C.dH * ((which & W_DC) ? N::fma_(gM, O.Fi, g[0]) : gM * O.Fi);
     T aK = -gM * C.dH * O.Fk;
-    if (g[7] != T(0)) {                                                 // V_C = 4 pi dH^3 v(Ok, I0): dv = F^2 dI0 + v_k dOk
+    if ((which & W_VC) && g[7] != T(0)) {                                                 // V_C = 4 pi dH^3 v(Ok, I0): dv = F^2 dI0 + v_k dOk
         const T c4pi = T(12.566370614359172954) * C.dH * C.dH * C.dH * g[7];
         aI = N::fma_(c4pi, O.F * O.F, aI);
         aK = N::fma_(-c4pi, O.Vk, aK);
@@ -185,6 +224,7 @@ CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, c
         const T tol = T(sizeof(T) == 8 ? 1e-12 : 1e-5);
         useJ = N::abs_(Jp[5] - prev5) <= tol * N::abs_(Jp[5]) && N::abs_(Jp[6] - prev6) <= tol * N::abs_(Jp[6]);
     }
+    const T aIh = T(-0.5) * aI;
 #pragma unroll
     for (int t = 0; t < 3; ++t) {
         T dI = C.GI[t][0] * R.I0 + C.GI[t][1] * R.K + C.GI[t][2] * bt0 + C.GI[t][3] * bt1 + C.GI[t][4] * bt2;
@@ -194,7 +234,7 @@ CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, c
             const T c = sa / N::max_(N::abs_(dI), T(1e-3) * N::abs_(R.I0));
             if (t == 0 || c > *cond) *cond = c;
         }
-        T acc = N::fma_(aI, T(-0.5) * dI, aK);
+        T acc = N::fma_(aIh, dI, aK);
         if (kT) {
             T dT = C.GT[t][0] * R.I0 + C.GT[t][1] * R.K + C.GT[t][2] * bt0 + C.GT[t][3] * bt1 + C.GT[t][4] * bt2 + C.GT[t][5] * R.TT;
             acc = N::fma_((g[4] - g[8]) * C.tH, T(-0.5) * dT, acc);       // t_L = tH T, age = tH (Tinf - T)
@@ -208,15 +248,21 @@ CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, c
         }
         gp[t] += acc;
     }
-    T h = g[0] * O.v[0] + g[1] * O.v[1] + g[2] * O.v[2] + g[3] * T(CB_KT.five_over_ln10);
+    T h = T(0);
+    if (which & W_DC) h = g[0] * O.v[0];
+    if (which & W_DM) h = N::fma_(g[1], O.v[1], h);
+    if (which & W_DL) h = N::fma_(g[2], O.v[2], h);
+    if (which & W_MU) h = N::fma_(g[3], T(CB_KT.five_over_ln10), h);
     if (kT) h += g[4] * O.v[4] + g[8] * O.v[8];
     if (kA) h += g[5] * O.v[5];
-    h += g[6] * O.v[6] + T(3) * g[7] * O.v[7];
-    gp[3] -= h * C.dH * T(1.0 / C_KM_S);        // / H0
-    T dz = aI * iE + g[2] * O.v[1];
-    if (g[3] != T(0)) dz += T(CB_KT.five_over_ln10) * g[3] * ix;
+    if (which & W_DA) h = N::fma_(g[6], O.v[6], h);
+    if (which & W_VC) h = N::fma_(T(3) * g[7], O.v[7], h);
+    gp[3] = N::fma_(-h * C.dH, T(1.0 / C_KM_S), gp[3]);        // / H0
+    T dz = aI * iE;
+    if (which & W_DL) dz = N::fma_(g[2], O.v[1], dz);
+    if ((which & W_MU) && g[3] != T(0)) dz = N::fma_(T(CB_KT.five_over_ln10) * g[3], ix, dz);
     if (kT) dz += (g[4] - g[8]) * C.tH * iE * ix;
-    if (g[6] != T(0)) dz -= g[6] * O.v[6] * ix;
+    if ((which & W_DA) && g[6] != T(0)) dz -= g[6] * O.v[6] * ix;
     if (kA) dz += g[5] * C.dH * x * x * iE;
     gz += dz;
 }

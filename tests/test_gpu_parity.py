@@ -375,7 +375,9 @@ def test_two_complex_pairs_outer_and_likelihood(cb):
     gp, st2, o2 = gp.cpu().numpy(), st2.cpu().numpy(), o2.cpu().numpy()
     assert np.isnan(gp[:, 1]).all() and np.isfinite(gp[:, [0, 2]]).all()
     assert ((st2[1] & 16) != 0).all() and (st2[[0, 2]] == 0).all()
-    assert np.array_equal(o2[0], out[2])
+    # two different kernels (chi family, four redshifts per thread; t_L/d_abs family, two): the warp-wide stopping vote can
+    # give an element a different number of (exact) duplication steps, so agreement is to rounding, not bit for bit
+    assert relerr(o2[0], out[2]).max() <= 8 * np.finfo(float).eps
     mu_obs = out[2, 1] + 0.05
     sigma = np.full(len(z), 0.1)
     logL, grad = cb.cosmo_snia_loglike(dev(z), dev(mu_obs), dev(sigma), dev(Om), dev(OL), dev(Or), dev(H0))
