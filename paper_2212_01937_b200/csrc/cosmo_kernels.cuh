@@ -1,8 +1,8 @@
 // cosmo_kernels.cuh -- the CUDA kernels of the hot path (sm_100a).  Launchers and the C ABI are in cosmo_b200.cu.
 //
 // Layout in HBM: SoA everywhere; z[N]; parameters Om/OL/Or/H0[S]; outputs and upstream
-// gradients as planes [plane][row][N] with N fastest, so that a warp reads/writes 512 contiguous bytes per plane row
-// (two consecutive elements per thread, 128-bit accesses in FP64).  Per-cosmology constants (86 numbers) are
+// gradients as planes [plane][row][N] with N fastest, so that a warp reads/writes contiguous 512-byte runs per plane row
+// (two or four consecutive elements per thread, 128-bit accesses in FP64).  Per-cosmology constants (Cosmo<T>) are
 // computed once by k_prep and staged in shared memory by the OUTER kernels, one block = one tile of redshifts
 // looping over a chunk of cosmologies, so the only per-eval HBM traffic is grad_out (8 B) and, if asked, out.
 #pragma once
