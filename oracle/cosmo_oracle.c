@@ -762,3 +762,78 @@ void oracle_observables2_batch(int64_t n, const double *z1, const double *z2, co
         if (status) status[i] = rc;
     }
 }
+
+/* ======================================================================================
+ * (9) extra components with constant equation of state w in {-2/3, -1/3} (PAPER.md:82 fn.4):
+ *       E^2(x) = Or x^4 + Om x^3 + (Ok + Ow13) x^2 + Ow23 x + OL,   Ok = 1 - Om - OL - Or - Ow13 - Ow23,
+ *     each component evolving as x^(3(1+w)) (fn.4 with constant w); the curvature of the transverse distance is Ok
+ *     alone.  chi family only: I0 = int_1^x dx'/E (eq. (2.3)), then D_C, D_M, D_L, mu as in (2), and
+ *     their d/dz (the integrand at the upper limit, chained).  Same adaptive GK21 in u = ln x as (1), written out
+ *     again for this polynomial so that (1) stays exactly as pinned. */
+typedef struct { ld a4, a3, a2, a1, a0; } poly4_t;
+
+static inline ld w_E2(const poly4_t *p, ld x) { return (((p->a4 * x + p->a3) * x + p->a2) * x + p->a1) * x + p->a0; }
+
+static void w_panel(const poly4_t *p, ld a, ld b, ld *K, ld *G, ld *Kabs) {
+    ld h = 0.5L * (b - a), m = 0.5L * (a + b);
+    *K = *G = *Kabs = 0.0L;
+    for (int i = 0; i < 21; ++i) {
+        ld x = expl(m + h * GK21_X[i]);
+        ld E2 = w_E2(p, x);
+        ld kappa = ((((fabsl(p->a4) * x + fabsl(p->a3)) * x + fabsl(p->a2)) * x + fabsl(p->a1)) * x + fabsl(p->a0)) / fabsl(E2);
+        ld f = x / sqrtl(E2);                       /* dx/E = x du/E */
+        *K += GK21_WK[i] * f; *G += GK21_WG[i] * f; *Kabs += GK21_WK[i] * fabsl(f) * kappa;
+    }
+    *K *= h; *G *= h; *Kabs *= h;
+}
+
+static void w_adapt(const poly4_t *p, ld a, ld b, ld frac, ld scale, int depth, ld *acc, int *npanels) {
+    ld K, G, Kabs;
+    w_panel(p, a, b, &K, &G, &Kabs);
+    ld err = fabsl(K - G);
+    int ok = !(err > GK_TOL * scale * frac && err > GK_ROUND * LDBL_EPSILON * Kabs);
+    if (err != err) ok = 1;
+    if (ok || depth >= GK_MAXDEPTH || *npanels >= GK_MAXPANELS) { *acc += K; ++*npanels; return; }
+    ld m = 0.5L * (a + b);
+    w_adapt(p, a, m, 0.5L * frac, scale, depth + 1, acc, npanels);
+    w_adapt(p, m, b, 0.5L * frac, scale, depth + 1, acc, npanels);
+}
+
+/* val[4] = D_C, D_M, D_L [Mpc], mu [mag]; dz[4] = their d/dz.  Returns 0, -1 (E^2 <= 0 on the path or z <= -1:
+ * NaN) or 1 (D_L <= 0: mu NaN). */
+int oracle_w_chi(ld z, ld Om, ld OL, ld Or, ld Ow13, ld Ow23, ld H0, ld val[4], ld dz[4]) {
+    ld Ok = 1.0L - Om - OL - Or - Ow13 - Ow23;
+    poly4_t p = { Or, Om, Ok + Ow13, Ow23, OL };
+    for (int i = 0; i < 4; ++i) val[i] = dz[i] = NAN;
+    if (!(z > -1.0L)) return -1;
+    ld U = log1pl(z), I0 = 0.0L;
+    for (int i = 0; i <= 64; ++i)
+        if (!(w_E2(&p, expl(U * i / 64.0L)) > 0.0L)) return -1;
+    if (z != 0.0L) {
+        ld K, G, Kabs;
+        w_panel(&p, 0.0L, U, &K, &G, &Kabs);
+        int npanels = 0, nseg = (int)ceill(fabsl(U));
+        if (nseg < 1) nseg = 1;
+        for (int s = 0; s < nseg; ++s) w_adapt(&p, U * s / nseg, U * (s + 1) / nseg, 1.0L / nseg, fabsl(K), 0, &I0, &npanels);
+    }
+    ld x = 1.0L + z, E = sqrtl(w_E2(&p, x)), dH = C_KM_S / H0;
+    ld F, Fi, Fk;
+    sinn_transform(Ok, I0, &F, &Fi, &Fk);
+    val[0] = dH * I0; val[1] = dH * F; val[2] = x * dH * F;
+    dz[0] = dH / E; dz[1] = dH * Fi / E; dz[2] = dH * F + x * dz[1];
+    if (!(val[2] > 0)) return 1;
+    val[3] = 5.0L * log10l(val[2]) + 25.0L;
+    dz[3] = 5.0L / logl(10.0L) * dz[2] / val[2];
+    return 0;
+}
+
+/* batch; parameter arrays of length n_cosmo in {1, n}; val, dz: [n][4] */
+void oracle_w_chi_batch(int64_t n, const double *z, const double *Om, const double *OL, const double *Or, const double *Ow13,
+                        const double *Ow23, const double *H0, int64_t n_cosmo, ld *val, ld *dz, int32_t *status) {
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < n; ++i) {
+        int64_t j = (n_cosmo == 1) ? 0 : i;
+        int rc = oracle_w_chi((ld)z[i], (ld)Om[j], (ld)OL[j], (ld)Or[j], (ld)Ow13[j], (ld)Ow23[j], (ld)H0[j], val + i * 4, dz + i * 4);
+        if (status) status[i] = rc;
+    }
+}
