@@ -121,6 +121,17 @@ int cosmo_eval_host(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosm
 int cosmo_eval2(const double* z1, const double* z2, int64_t n, cosmo_params p, int64_t n_cosmo, uint32_t which, const double* grad_out,
                 double* out, double* grad_z1, double* grad_z2, double* grad_params, uint8_t* status, void* stream);
 
+/* EXTRA CONSTANT-w COMPONENTS (PAPER.md:82 fn.4: E^2 must be a polynomial of degree <= 4, which admits w in
+ * {-1, -2/3, -1/3, 0, 1/3}):  E^2(x) = Or x^4 + Om x^3 + (Ok + Ow13) x^2 + Ow23 x + OL with Ok = 1 - Om - OL - Or - Ow13 - Ow23
+ * (the curvature of the transverse distance is Ok alone).  chi family only: `which` from COSMO_DC, COSMO_DM, COSMO_DL, COSMO_MU,
+ * by eq. (3.7)/(B.1) on a general real factorisation of the quartic.  One (z[i], cosmology) per element, parameter arrays of
+ * length n_cosmo in {1, n} (device pointers).  out[n_which][n] in ascending bit order; dout_dz (nullable), same shape: the
+ * derivative of each plane with respect to z.  status (nullable) as above: 1 root of E^2 on the path / E^2 <= 0,
+ * 2 unsupported input or factorisation failure, 4 D_L <= 0, 8 iteration cap.  Forward only: no parameter gradients. */
+int cosmo_eval_w(const double* z, int64_t n, const double* Om, const double* OL, const double* Or, const double* Ow13,
+                 const double* Ow23, const double* H0, int64_t n_cosmo, uint32_t which, double* out, double* dout_dz, uint8_t* status,
+                 void* stream);
+
 /* The device Carlson functions of the hot path on their own (eqs. (2.6), (2.7), (2.9); duplication
  * algorithm of ref. [10]), in the real-symmetric form the path uses: for each i
  *   rf[i] = R_F(x, m+h, m-h),  rd[i] = R_D(m+h, m-h, x),  rj[i] = R_J(x, m+h, m-h, p),   h^2 = s[i]

@@ -19,7 +19,7 @@ WHICH_ORDER = ("DC", "DM", "DL", "MU", "TL", "DABS", "DA", "VC", "AGE")
 
 # every symbol include/cosmo_b200.h declares
 SYMBOLS = ("cosmo_workspace_bytes", "cosmo_eval", "cosmo_vjp", "cosmo_snia_loglike", "cosmo_eval_f32", "cosmo_vjp_f32",
-           "cosmo_snia_loglike_f32", "cosmo_snia_logjoint", "cosmo_eval2", "cosmo_eval_host", "cosmo_carlson_pair", "cosmo_probe_fma_f64", "cosmo_probe_fma_f32",
+           "cosmo_snia_loglike_f32", "cosmo_snia_logjoint", "cosmo_eval2", "cosmo_eval_w", "cosmo_eval_host", "cosmo_carlson_pair", "cosmo_probe_fma_f64", "cosmo_probe_fma_f32",
            "cosmo_profile", "cosmo_profile_mean_ms",
            "cosmo_launch_count", "cosmo_last_cuda_error", "cosmo_strerror", "cosmo_version")
 
@@ -69,6 +69,8 @@ def lib():
     L.cosmo_snia_logjoint.restype = ci
     L.cosmo_eval2.argtypes = [vp, vp, i64, CosmoParams, i64, u32, vp, vp, vp, vp, vp, vp, vp]
     L.cosmo_eval2.restype = ci
+    L.cosmo_eval_w.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, i64, u32, vp, vp, vp, vp]
+    L.cosmo_eval_w.restype = ci
     L.cosmo_carlson_pair.argtypes = [vp, vp, vp, vp, i64, vp, vp, vp, vp]
     L.cosmo_carlson_pair.restype = ci
     L.cosmo_launch_count.restype = i64
@@ -258,6 +260,28 @@ def cosmo_eval2(z1, z2, Om, OL, Or, H0, which=("DC",), grad_out=None, want_out=T
     _check(lib().cosmo_eval2(_ptr(z1), _ptr(z2), n, P, n_cosmo, mask, _ptr(grad_out), _ptr(out), _ptr(g1), _ptr(g2), _ptr(gp), _ptr(status),
                              _stream(torch)))
     return out, g1, g2, gp, status
+
+
+def cosmo_eval_w(z, Om, OL, Or, Ow13, Ow23, H0, which=("DC",), want_dz=True):
+    """chi family with extra constant-w components w = -1/3 (Ow13) and w = -2/3 (Ow23), PAPER.md:82 fn.4 (elementwise; parameters of
+    length 1 or n).  Returns (out[n_which, n], dout_dz[n_which, n] or None, status[n]).  which from DC, DM, DL, MU."""
+    torch = _torch()
+    mask = which_mask(which)
+    _dev(z, torch.float64, torch, "z")
+    n = z.numel()
+    ps = []
+    for t, nm in ((Om, "Om"), (OL, "OL"), (Or, "Or"), (Ow13, "Ow13"), (Ow23, "Ow23"), (H0, "H0")):
+        _dev(t, torch.float64, torch, nm)
+        ps.append(t)
+    n_cosmo = ps[0].numel()
+    if any(t.numel() != n_cosmo for t in ps):
+        raise CosmoError("parameter arrays must have equal lengths")
+    nw = bin(mask).count("1")
+    out = torch.empty((nw, n), dtype=torch.float64, device=z.device)
+    dz = torch.empty((nw, n), dtype=torch.float64, device=z.device) if want_dz else None
+    status = torch.empty(n, dtype=torch.uint8, device=z.device)
+    _check(lib().cosmo_eval_w(_ptr(z), n, *[_ptr(t) for t in ps], n_cosmo, mask, _ptr(out), _ptr(dz), _ptr(status), _stream(torch)))
+    return out, dz, status
 
 
 def cosmo_eval_host(z, Om, OL, Or, H0, mode=ELEMENTWISE, which=("DC",), grad_out=None, want_out=True, want_status=True):

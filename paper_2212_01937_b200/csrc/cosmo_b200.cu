@@ -354,6 +354,20 @@ int cosmo_eval2(const double* z1, const double* z2, int64_t n, cosmo_params p, i
     return check_launch();
 }
 
+int cosmo_eval_w(const double* z, int64_t n, const double* Om, const double* OL, const double* Or, const double* Ow13,
+                 const double* Ow23, const double* H0, int64_t n_cosmo, uint32_t which, double* out, double* dout_dz, uint8_t* status,
+                 void* stream) {
+    if (n < 0 || !(n_cosmo == 1 || n_cosmo == n)) return COSMO_E_SIZE;
+    if (which == 0 || (which & ~uint32_t(W_DC | W_DM | W_DL | W_MU))) return COSMO_E_WHICH;
+    if (n == 0) return COSMO_OK;
+    if (!z || !Om || !OL || !Or || !Ow13 || !Ow23 || !H0 || !out) return COSMO_E_NULL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    prof_begin(st);
+    k_w<<<(unsigned)cdiv(n, ELEM_THREADS), ELEM_THREADS, 0, st>>>(z, Om, OL, Or, Ow13, Ow23, H0, n, n_cosmo, which, out, dout_dz, status);
+    prof_end(st);
+    return check_launch();
+}
+
 int cosmo_carlson_pair(const double* x, const double* m, const double* s, const double* p, int64_t n, double* rf, double* rd,
                        double* rj, void* stream) {
     if (n < 0) return COSMO_E_SIZE;

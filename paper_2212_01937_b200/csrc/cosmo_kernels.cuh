@@ -10,6 +10,7 @@
 #include "cosmo_prep.cuh"
 #include "cosmo_obs.cuh"
 #include "cosmo_two.cuh"
+#include "cosmo_w.cuh"
 
 namespace cb {
 
@@ -458,6 +459,31 @@ __global__ void __launch_bounds__(ELEM_THREADS) k_two(const double* __restrict__
         gz1[i] = a1; gz2[i] = a2;
         for (int t = 0; t < 4; ++t) gparams[(int64_t)t * n + i] = ap[t];
     }
+}
+
+// chi family with extra constant-w components (cosmo_w.cuh), one thread per (z, cosmology); n_cosmo in {1, n}.
+// which: DC, DM, DL, MU.  out[n_which][n]; dout[n_which][n] = d out / dz (nullable).
+__global__ void __launch_bounds__(ELEM_THREADS) k_w(const double* __restrict__ z, const double* __restrict__ Om,
+                                                    const double* __restrict__ OL, const double* __restrict__ Or,
+                                                    const double* __restrict__ Ow13, const double* __restrict__ Ow23,
+                                                    const double* __restrict__ H0, int64_t n, int64_t n_cosmo, unsigned which,
+                                                    double* __restrict__ out, double* __restrict__ dout, uint8_t* __restrict__ status) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const bool live = i < n;
+    const int64_t ii = live ? i : n - 1, ic = n_cosmo == 1 ? 0 : ii;
+    WCosmo W;
+    w_prep(Om[ic], OL[ic], Or[ic], Ow13[ic], Ow23[ic], H0[ic], W);
+    double v[4], dz[4];
+    const unsigned st = w_eval<VoteWarp>(W, z[ii], VoteWarp(), v, dz);
+    if (!live) return;
+    int pl = 0;
+    for (int o = 0; o < 4; ++o) {
+        if (!(which >> o & 1)) continue;
+        out[(int64_t)pl * n + i] = v[o];
+        if (dout != nullptr) dout[(int64_t)pl * n + i] = dz[o];
+        ++pl;
+    }
+    if (status != nullptr) status[i] = (uint8_t)st;
 }
 
 // The device Carlson functions on their own (same code as the hot path): R_F(x, m+h, m-h), R_D(m+h, m-h, x) and

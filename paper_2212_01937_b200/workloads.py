@@ -254,3 +254,34 @@ def invalid_rows():
         (-1.5, 0.3, 0.7, 9e-5, 70.0, 2),
     ]
     return rows
+
+
+def wmix(n: int = 20_000, seed: int = 7):
+    """Inputs for the extra-w family (PAPER.md:82 fn.4): per-element cosmologies with components of w = -1/3 and
+    w = -2/3 beside matter, Lambda, radiation and curvature; log-uniform z in [1e-3, 10].  The first rows are the structural
+    cases: single-component universes and polynomials of every degree 0..4.  Returns dict of float64 arrays
+    z, Om, OL, Or, Ow13, Ow23, H0."""
+    rng = np.random.default_rng(seed)
+    z = 10.0 ** rng.uniform(-3.0, 1.0, n)
+    Om = rng.uniform(0.05, 0.5, n)
+    OL = rng.uniform(0.0, 0.9, n)
+    Or = rng.choice([0.0, 1e-5, 9e-5, 1e-3], n)
+    Ow13 = np.where(rng.random(n) < 0.9, rng.uniform(0.0, 0.3, n), rng.uniform(-0.05, 0.0, n))
+    Ow23 = np.where(rng.random(n) < 0.9, rng.uniform(0.0, 0.3, n), rng.uniform(-0.05, 0.0, n))
+    H0 = rng.uniform(60.0, 80.0, n)
+    special = [  # (Om, OL, Or, Ow13, Ow23)
+        (0.0, 0.0, 0.0, 0.0, 1.0),      # E^2 = x
+        (0.0, 0.0, 0.0, 1.0, 0.0),      # E^2 = x^2, flat
+        (0.0, 0.0, 0.0, 0.0, 0.0),      # Milne
+        (0.0, 1.0, 0.0, 0.0, 0.0),      # de Sitter: degree 0
+        (1.0, 0.0, 0.0, 0.0, 0.0),      # Einstein-de Sitter
+        (0.0, 0.0, 1.0, 0.0, 0.0),      # radiation only
+        (0.0, 0.65, 0.0, 0.0, 0.35),    # degree 1
+        (0.0, 0.65, 0.0, 0.35, 0.0),    # degree 2, flat
+        (0.35, 0.0, 0.0, 0.0, 0.65),    # degree 3 without constant term
+        (0.3, 0.7, 0.0, 0.0, 0.0), (0.3, 0.7, 9e-5, 0.0, 0.0), (0.27, 0.55, 8e-5, 0.06, 0.09),
+    ]
+    k = min(len(special), n)
+    for i in range(k):
+        Om[i], OL[i], Or[i], Ow13[i], Ow23[i] = special[i]
+    return {"z": z, "Om": Om, "OL": OL, "Or": Or, "Ow13": Ow13, "Ow23": Ow23, "H0": H0}

@@ -6,6 +6,7 @@
 #include "../../paper_2212_01937_b200/csrc/cosmo_prep.cuh"
 #include "../../paper_2212_01937_b200/csrc/cosmo_obs.cuh"
 #include "../../paper_2212_01937_b200/csrc/cosmo_two.cuh"
+#include "../../paper_2212_01937_b200/csrc/cosmo_w.cuh"
 
 using namespace cb;
 
@@ -70,5 +71,17 @@ extern "C" void hostcheck_two(int64_t n, const double* z1, const double* z2, con
             for (int t = 0; t < 4; ++t) gp[(o * 4 + t) * n + i] = O.gp[o][t];
         }
         status[i] = (uint8_t)O.status;
+    }
+}
+
+// extra constant-w components (cosmo_w.cuh): val[4][n], dz[4][n]
+extern "C" void hostcheck_w(int64_t n, const double* z, const double* Om, const double* OL, const double* Or, const double* Ow13,
+                            const double* Ow23, const double* H0, double* val, double* dz, uint8_t* status) {
+    for (int64_t i = 0; i < n; ++i) {
+        WCosmo W;
+        w_prep(Om[i], OL[i], Or[i], Ow13[i], Ow23[i], H0[i], W);
+        double v[4], d[4];
+        status[i] = (uint8_t)w_eval<VoteNone>(W, z[i], VoteNone(), v, d);
+        for (int o = 0; o < 4; ++o) { val[o * n + i] = v[o]; dz[o * n + i] = d[o]; }
     }
 }

@@ -608,3 +608,37 @@ def test_two_limit(cb):
     o2, *_ = cb.cosmo_eval2(dev(np.zeros(1000)), dev(z2[:1000]), *p, ("DC", "TL"))
     o1, _ = cb.cosmo_eval(dev(z2[:1000]), *p, cb.ELEMENTWISE, ("DC", "TL"))
     assert np.allclose(o2.cpu().numpy(), o1.cpu().numpy()[:, 0], rtol=1e-13, atol=0)
+
+
+# ---------------------------------------------------------------- extra constant-w components (PAPER.md:82 fn.4)
+def test_extra_w_components(cb):
+    """cosmo_eval_w (general quartic E^2 with w = -1/3 and w = -2/3 components; chi family + d/dz) against oracle.w_chi_batch:
+    per-element cosmologies incl. every polynomial degree, one shared cosmology, an invalid path, argument errors."""
+    w = W.wmix(n=50_000)
+    names = ("z", "Om", "OL", "Or", "Ow13", "Ow23", "H0")
+    out, dz, st = cb.cosmo_eval_w(*[dev(w[k]) for k in names], which=oracle.OBSW)
+    out, dz, st = out.cpu().numpy(), dz.cpu().numpy(), st.cpu().numpy()
+    v, d, so = oracle.w_chi_batch(*[w[k] for k in names])
+    v, d = v.astype(np.float64), d.astype(np.float64)
+    ok = so == 0
+    assert ok.mean() > 0.95 and (st[ok] == 0).all() and (st[so == -1] & 3).all()
+    for o, nm in enumerate(oracle.OBSW):
+        assert relerr(out[o][ok], v[ok, o]).max() <= TOL_VAL, nm
+        assert relerr(dz[o][ok], d[ok, o]).max() <= TOL_VAL, nm          # d/dz is closed form (the integrand), not a basis solve
+    # a subset of planes, one shared cosmology
+    z = np.linspace(0.0, 6.0, 4001)
+    p = (0.27, 0.55, 8e-5, 0.06, 0.09, 70.0)
+    out1, dz1, st1 = cb.cosmo_eval_w(dev(z), *[dev(np.array([x])) for x in p], which=("DM", "MU"), want_dz=False)
+    v1, _, _ = oracle.w_chi_batch(z, *p)
+    assert dz1 is None and out1.shape == (2, len(z)) and (st1.cpu().numpy()[1:] == 0).all()
+    assert relerr(out1[0].cpu().numpy()[1:], v1[1:, 1].astype(np.float64)).max() <= TOL_VAL
+    assert relerr(out1[1].cpu().numpy()[1:], v1[1:, 3].astype(np.float64)).max() <= TOL_VAL
+    assert out1[0, 0] == 0.0 and (st1[0] & 4)                            # z = 0: D_L = 0, mu undefined
+    # no Big Bang: E^2 < 0 before z = 5
+    o2, _, s2 = cb.cosmo_eval_w(dev(np.array([0.2, 5.0])), *[dev(np.array([x])) for x in (0.1, 2.0, 0.0, 0.0, 0.05, 70.0)])
+    _, _, so2 = oracle.w_chi_batch(np.array([0.2, 5.0]), 0.1, 2.0, 0.0, 0.0, 0.05, 70.0)
+    assert so2[0] == 0 and so2[1] == -1 and s2[0] == 0 and (s2[1] & 1) and np.isnan(float(o2[0, 1])) and np.isfinite(float(o2[0, 0]))
+    with pytest.raises(cb.CosmoError):
+        cb.cosmo_eval_w(dev(z), *[dev(np.array([x])) for x in p], which=("TL",))
+    e, _, _ = cb.cosmo_eval_w(dev(np.zeros(0)), *[dev(np.array([x])) for x in p])
+    assert e.shape == (1, 0)

@@ -193,6 +193,24 @@ def test_two_limit_host(hc):
             assert e.max() <= tol, (nm, oracle.WRT2[k], e.max())
 
 
+def test_extra_w_components_host(hc):
+    """chi family on the general quartic (cosmo_w.cuh; PAPER.md:82 fn.4) against oracle.w_chi_batch"""
+    w = W.wmix(n=6000)
+    n = len(w["z"])
+    val = np.zeros((4, n)); dz = np.zeros((4, n)); st = np.zeros(n, dtype=np.uint8)
+    dp = lambda a: np.ascontiguousarray(a).ctypes.data_as(DP)
+    hc.hostcheck_w(C.c_int64(n), dp(w["z"]), dp(w["Om"]), dp(w["OL"]), dp(w["Or"]), dp(w["Ow13"]), dp(w["Ow23"]), dp(w["H0"]), dp(val), dp(dz),
+                   st.ctypes.data_as(C.POINTER(C.c_uint8)))
+    v, d, so = oracle.w_chi_batch(w["z"], w["Om"], w["OL"], w["Or"], w["Ow13"], w["Ow23"], w["H0"])
+    v, d = v.astype(np.float64), d.astype(np.float64)
+    ok = so == 0
+    assert ok.mean() > 0.95 and (st[ok] == 0).all() and (st[so == -1] & 3).all()
+    for o, nm in enumerate(oracle.OBSW):
+        assert (np.abs(val[o][ok] - v[ok, o]) / np.abs(v[ok, o])).max() <= 1e-11, nm
+        assert (np.abs(dz[o][ok] - d[ok, o]) / np.abs(d[ok, o])).max() <= 1e-11, nm
+    assert np.isnan(val[:, so == -1]).all()
+
+
 def test_host_math_fp32(hc):
     w = W.config3(n=3000, S=1)
     z = w.z.astype(np.float32).astype(np.float64)
