@@ -106,6 +106,20 @@ def main():
         ws = torch.empty(cb.workspace_bytes(n, S, cb.OUTER, ("MU",), True), dtype=torch.uint8, device="cuda")
         timed(lambda: cb.cosmo_snia_logjoint(z, z_obs, mu_obs.contiguous(), sig, 0.04, 3.0, 3.0, *P, workspace=ws), S * n,
               "section-4 log-joint with latent z (one VI step): N=1e6 SNe x S=64 samples, logp + grad_params + grad_z f64")
+    if want("twolimit"):
+        n = 1_000_000 // f
+        z1 = dev(rng.uniform(0.0, 3.0, n)); z2 = z1 + dev(10.0 ** rng.uniform(-3.0, 0.8, n))
+        P = [dev(rng.uniform(0.08, 0.6, n)), dev(rng.uniform(0.0, 1.2, n)), dev(rng.choice([0.0, 1e-5, 9e-5, 1e-3], n)), dev(rng.uniform(60, 80, n))]
+        timed(lambda: cb.cosmo_eval2(z1, z2, *P, which=("DC", "DM", "TL", "DABS", "DA")), n,
+              "two-limit forms (z1, z2), five outputs, per-element cosmology, forward f64")
+        g = torch.randn((5, n), dtype=torch.float64, device="cuda")
+        timed(lambda: cb.cosmo_eval2(z1, z2, *P, which=("DC", "DM", "TL", "DABS", "DA"), grad_out=g), n,
+              "two-limit forms (z1, z2), five outputs, per-element cosmology, forward + VJP f64")
+    if want("wmix"):
+        w = W.wmix(n=1_000_000 // f)
+        a = [dev(w[k]) for k in ("z", "Om", "OL", "Or", "Ow13", "Ow23", "H0")]
+        timed(lambda: cb.cosmo_eval_w(*a, which=("DC", "DM", "DL", "MU")), len(w["z"]),
+              "extra-w family (general quartic), D_C, D_M, D_L, mu + d/dz, per-element cosmology f64")
     if want("config5"):
         w = W.config5(n=10_000_000 // f, n_struct=100_000 // f)
         a = [dev(x) for x in (w.z, w.Om, w.OL, w.Or, w.H0)]
