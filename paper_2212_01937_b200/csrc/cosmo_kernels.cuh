@@ -472,7 +472,14 @@ __global__ void __launch_bounds__(ELEM_THREADS) k_w(const double* __restrict__ z
     const bool live = i < n;
     const int64_t ii = live ? i : n - 1, ic = n_cosmo == 1 ? 0 : ii;
     WCosmo W;
-    w_prep(Om[ic], OL[ic], Or[ic], Ow13[ic], Ow23[ic], H0[ic], W);
+    __shared__ WCosmo sw;
+    if (n_cosmo == 1) {                       // one shared cosmology: factor it once per block, not once per thread
+        if (threadIdx.x == 0) w_prep(Om[0], OL[0], Or[0], Ow13[0], Ow23[0], H0[0], sw);
+        __syncthreads();
+        W = sw;
+    } else {
+        w_prep(Om[ic], OL[ic], Or[ic], Ow13[ic], Ow23[ic], H0[ic], W);
+    }
     double v[4], dz[4];
     const unsigned st = w_eval<VoteWarp>(W, z[ii], VoteWarp(), v, dz);
     if (!live) return;

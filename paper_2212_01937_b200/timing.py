@@ -120,6 +120,9 @@ def main():
         a = [dev(w[k]) for k in ("z", "Om", "OL", "Or", "Ow13", "Ow23", "H0")]
         timed(lambda: cb.cosmo_eval_w(*a, which=("DC", "DM", "DL", "MU")), len(w["z"]),
               "extra-w family (general quartic), D_C, D_M, D_L, mu + d/dz, per-element cosmology f64")
+        one = [dev(np.array([x])) for x in (0.27, 0.55, 8e-5, 0.06, 0.09, 70.0)]
+        timed(lambda: cb.cosmo_eval_w(a[0], *one, which=("DC", "DM", "DL", "MU")), len(w["z"]),
+              "extra-w family (general quartic), D_C, D_M, D_L, mu + d/dz, one shared cosmology f64")
     if want("config5"):
         w = W.config5(n=10_000_000 // f, n_struct=100_000 // f)
         a = [dev(x) for x in (w.z, w.Om, w.OL, w.Or, w.H0)]
