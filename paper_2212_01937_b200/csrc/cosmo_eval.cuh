@@ -115,8 +115,14 @@ template <> struct Num<double> {
     static constexpr double RC_SMALL = 0.03;
 };
 template <> struct Num<float> {
+#if defined(__CUDA_ARCH__) && !defined(CB_F32_IEEE)
+    // MUFU approximations (about 1 ulp each): the FP32 variant's budget is 2e-5
+    static CB_HD float sqrt_(float a) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(a)); return y; }
+    static CB_HD float log_(float a) { return __logf(a); }
+#else
     static CB_HD float sqrt_(float a) { return sqrtf(a); }
     static CB_HD float log_(float a) { return logf(a); }
+#endif
     static CB_HD float exp_(float a) { return expf(a); }
     static CB_HD float atan_(float a) { return atanf(a); }
     static CB_HD void sincos_(float a, float* s, float* c) { *s = sinf(a); *c = cosf(a); }
@@ -130,8 +136,13 @@ template <> struct Num<float> {
         return 1.0f / sqrtf(a);
 #endif
     }
+#if defined(__CUDA_ARCH__) && !defined(CB_F32_IEEE)
+    static CB_HD float rcp_(float b) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(b)); return y; }
+    static CB_HD float sqrtp_(float a) { return sqrt_(a); }
+#else
     static CB_HD float rcp_(float b) { return 1.0f / b; }
     static CB_HD float sqrtp_(float a) { return sqrtf(a); }
+#endif
     static CB_HD float twice_(float a) { return 2.0f * a; }
     static CB_HD int key_(float a) {
 #ifdef __CUDA_ARCH__
