@@ -27,8 +27,7 @@
  *          factorised (the method needs E^2 of degree 3 or 4)
  *       4  D_L <= 0 (closed universe at/after the antipode): mu is NaN, the other outputs are valid
  *       8  the duplication loop hit its iteration cap before Carlson's stopping rule was met
- *      16  gradient ill-conditioned (near-degenerate roots; the 1/prod(r_j - r_k) of PAPER.md:320-345) or not available
- *          (E^2 without a real negative root: values by the complex slow path, gradients NaN): values valid, gradients
+ *      16  gradient ill-conditioned (near-degenerate roots; the 1/prod(r_j - r_k) of PAPER.md:320-345): values valid, gradients
  *          may have lost more than the documented accuracy (set by the VJP calls; the conditioning estimate is per element
  *          in ELEMENTWISE calls only)
  */
@@ -93,7 +92,7 @@ int cosmo_snia_loglike(const double* z, const double* mu_obs, const double* sigm
  *   grad[4][S]    = d log p[s] / d (Om, OL, Or, H0)      (nullable)
  *   grad_z[S][N]  = d log p[s] / d z[s][n]               (nullable)
  * (the paper fixes beta = 3, sigma_mu = 0.14, sigma_z = 0.04; it does not print the gamma shape: DESIGN.md reading R-prior.)
- * Workspace: cosmo_workspace_bytes(N, S, COSMO_OUTER, COSMO_MU, 1).  Samples whose E^2 has no real negative root give NaN. */
+ * Workspace: cosmo_workspace_bytes(N, S, COSMO_OUTER, COSMO_MU, 1). */
 int cosmo_snia_logjoint(const double* z, const double* z_obs, const double* mu_obs, const double* sigma_mu, double sigma_z,
                         double beta, double shape, int64_t N, cosmo_params p, int64_t S, double* logp, double* grad, double* grad_z,
                         void* workspace, size_t ws_bytes, void* stream);

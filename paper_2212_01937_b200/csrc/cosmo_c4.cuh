@@ -3,8 +3,11 @@
 // config 2).  There eqs. (3.8)/(3.9) single out a COMPLEX root r_i, so the R_J parameter
 // u_i5^2 / u_i0^2 is complex while x = u12^2, y = u13^2, z = u14^2 stay real (each u is invariant under the conjugation
 // that swaps the members of both pairs).  This file evaluates the paper's formulae as printed, in complex arithmetic
-// only where it is needed (the p-track of R_J, R_C, and the algebraic coefficients).  FP64 always; forward values only
-// (gradients of these rows are NaN and carry status bit 16).
+// only where it is needed (the p-track of R_J, R_C, and the algebraic coefficients).  FP64 always.  For the gradients it
+// also returns K = int_1^x N_K / E^3 with N_K = Or^2 Re (x - r1)^2 Q2(x): the real part of Carlson's [+1, -1, -1, -3] integral
+// int sqrt(t - r1) / ((t - r2)^(3/2) sqrt((t - r3)(t - r4))) dt = (2/3) d13 d14 dz^3 R_D(u13^2, u14^2, u12^2) + 2 dz X1 Y1 / (X2 Y2 u12)
+// (the same R_D term eq. (3.9) carries), which for r2 = conj(r1) equals Or^(3/2) int (t - r1)^2 Q2 / E^3 dt.  It plays the part
+// the [p_n = -3] integral of the real root plays in the gradient bases of cosmo_prep.cuh.
 #pragma once
 #include "cosmo_eval.cuh"
 
@@ -108,7 +111,7 @@ CB_HD void c4_carlson(double x, double y, double z, cx p, bool want_j, C4Carlson
 // Q2 = x^2 + b x + c, permutation (i, j, k, l) = (1, 2, 3, 4); everything in x = 1 + z (d_i5 = -rho_i).
 // (never inlined: a rare path must not cost the hot kernels registers)
 CB_HD_NOINLINE void eval_c4(double Or, double g1, double h1, double b, double c, double z, bool want_T, bool want_A,
-                   double& I0, double& TT, double& AA) {
+                   double& I0, double& TT, double& AA, double& KK) {
     const double x = 1.0 + z, dz = z;
     const double D1 = 4.0 * Or * h1 - g1 * g1, D2 = 4.0 * c - b * b;       // both > 0 here
     const cx r1 = cx_(-g1 / (2.0 * Or), sqrt(D1) / (2.0 * Or)), r2 = cx_conj(r1);
@@ -126,6 +129,7 @@ CB_HD_NOINLINE void eval_c4(double Or, double g1, double h1, double b, double c,
     const cx p5 = cx_(xa) - (dz * dz) * (d13 * d14 * (r2 / r1));
     c4_carlson(ya, za, xa, p5, want_T, K);
     I0 = ia * 2.0 * dz * K.RF;
+    KK = sqrt(Or) * (((2.0 / 3.0) * dz * dz * dz * K.RDz) * (d13 * d14) + (2.0 * dz) * ((X1 * Y1) / (X2 * Y2 * u12))).re;
     TT = 0.0; AA = 0.0;
     if (want_T) {
         const cx q5 = (cx_(x) / ((cx_(1.0) - r1) * (cx_(x) - r1))) * p5;

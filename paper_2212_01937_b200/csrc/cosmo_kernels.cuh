@@ -122,48 +122,78 @@ struct OuterArgs {
     int vec;                 // N even and pointers 16-byte aligned
 };
 
-// One cosmology row of the OUTER kernels whose E^2 has no real negative root (Cosmo::cubic bit 1): complex slow path,
-// forward values only.  Never inlined and called at the top of the per-cosmology iteration, where almost nothing is live,
-// so that this rare case costs the hot loop no registers.  Parameter gradients of the row and its contribution to grad_z
-// are NaN ("not available", status bit 16); the likelihood value itself is valid.
+// One cosmology row of the OUTER kernels whose E^2 has no real negative root (Cosmo::cubic bit 1): complex slow path
+// (cosmo_c4.cuh), values and gradients, one element at a time.  Never inlined and called at the top of the per-cosmology
+// iteration, where almost nothing is live, so that this rare case costs the hot loop no registers.
 template <typename T, bool kT, bool kA, int MODE>
 __device__ __noinline__ void outer_c4_row(const OuterArgs& a, const Cosmo<T>& C, int64_t row, int64_t n0, const T* zv, const T* mo,
-                                          const T* isig2, const T* lnorm, unsigned which, double* sacc_row, int lane, T* gzacc) {
-    constexpr int NP = (MODE == MODE_SNIA || MODE == MODE_JOINT) ? 5 : 4;
+                                          const T* isig2, const T* lnorm, const T* zo, unsigned which, double* sacc_row, int lane,
+                                          T* gzacc) {
+    constexpr bool kLike = MODE == MODE_SNIA || MODE == MODE_JOINT;
+    constexpr int NP = kLike ? 5 : 4;
     constexpr int KZ = outer_kz(kT, kA);
     const int64_t N = a.N, S = a.S;
-    T ll = T(0);
+    T pacc[5] = {T(0), T(0), T(0), T(0), T(0)};
     for (int k = 0; k < KZ; ++k) {
         const bool live = n0 + k < N;
+        const int64_t col = live ? n0 + k : N - 1;
         Core<T> R;
         R.I0 = R.TT = R.AA = R.K = R.E = R.iE = R.Em1 = T(0);
         R.status = C.status;
         apply_c4<T, kT, kA, MODE != MODE_FWD>(C, zv[k], R);
         Obs<T> O;
         observables<T, kT, kA>(C, zv[k], R, which, O);
-        if (MODE == MODE_SNIA) {
+        if (kLike) {
             const T resid = mo[k] - O.v[3];
-            if (live) ll += Num<T>::fma_(T(-0.5) * resid, resid * isig2[k], lnorm[k]);
-        } else if (live) {
-            if (a.out != nullptr) {
+            T gg[N_PLANES] = {T(0), T(0), T(0), resid * isig2[k], T(0), T(0), T(0), T(0), T(0)};
+            T dz = T(0), gp[4] = {T(0), T(0), T(0), T(0)};
+            backward<T, false, false>(C, zv[k], R, O, gg, dz, gp);
+            T ll = Num<T>::fma_(T(-0.5) * resid, resid * isig2[k], lnorm[k]);
+            if (MODE == MODE_JOINT) {       // same photometric-redshift and prior terms as the fused row of k_outer
+                const T x = T(1) + zv[k], ix = Num<T>::rcp_(x);
+                const T isz = ix * T(1.0 / a.sigma_z);
+                const T rz = (zo[k] - zv[k]) * isz;
+                ll += Num<T>::fma_(T(-0.5) * rz, rz, -Num<T>::log_(x));
+                ll += T(a.prior_norm) + T(a.shape_m1) * Num<T>::log_(zv[k]) - T(a.beta) * zv[k];
+                dz += rz * isz + (rz * rz - T(1)) * ix + T(a.shape_m1) * Num<T>::rcp_(zv[k]) - T(a.beta);
+                if (live && a.gz != nullptr) static_cast<T*>(a.gz)[row * N + col] = dz;
+            }
+            if (live) {
+                pacc[0] += ll;
+                for (int j = 0; j < 4; ++j) pacc[1 + j] += gp[j];
+            }
+        } else {
+            if (live) {
+                if (a.out != nullptr) {
+                    int pl = 0;
+                    for (int w = 0; w < N_PLANES; ++w) {
+                        if (!(which >> w & 1)) continue;
+                        static_cast<T*>(a.out)[((int64_t)pl * S + row) * N + col] = O.v[w];
+                        ++pl;
+                    }
+                }
+                if (a.status != nullptr) a.status[row * N + col] = (uint8_t)O.status;
+            }
+            if (MODE == MODE_VJP) {
+                T g[N_PLANES];
                 int pl = 0;
                 for (int w = 0; w < N_PLANES; ++w) {
+                    g[w] = T(0);
                     if (!(which >> w & 1)) continue;
-                    static_cast<T*>(a.out)[((int64_t)pl * S + row) * N + n0 + k] = O.v[w];
+                    if (live) g[w] = static_cast<const T*>(a.gout)[((int64_t)pl * S + row) * N + col];
                     ++pl;
                 }
+                T dz = T(0);
+                backward<T, kT, kA>(C, zv[k], R, O, g, dz, pacc, nullptr, which);
+                if (live) gzacc[k] += dz;
             }
-            if (a.status != nullptr) a.status[row * N + n0 + k] = (uint8_t)O.status;
         }
-        if (MODE == MODE_VJP) gzacc[k] = T(NAN);
     }
     if (MODE != MODE_FWD) {
-        if (MODE == MODE_SNIA) {
-            const double l = warp_sum((double)ll);
-            if (lane == 0) sacc_row[0] = l;
+        for (int j = 0; j < NP; ++j) {
+            const double v = warp_sum((double)pacc[j]);
+            if (lane == 0) sacc_row[j] = v;
         }
-        if (lane == 0)
-            for (int j = NP - 4; j < NP; ++j) sacc_row[j] = NAN;
     }
 }
 
@@ -224,19 +254,8 @@ __global__ void __launch_bounds__(OUTER_THREADS, CB_MINBLOCKS) k_outer(OuterArgs
             const Cosmo<T>& C = sc[sl];
             const int64_t row = c0 + sl;
             if (MODE == MODE_JOINT) load2(zp + roff, n0, N, vec, zv);      // latent redshifts: one row per sample
-            if (MODE == MODE_JOINT && (C.cubic & 2u)) {                          // no gradients on the complex slow path: NaN row
-                if (lane == 0)
-                    for (int j = 0; j < NP; ++j) sacc[warp][sl][j] = NAN;
-                if (a.gz != nullptr) {
-                    T nn[KZ];
-#pragma unroll
-                    for (int k = 0; k < KZ; ++k) nn[k] = T(NAN);
-                    store2(static_cast<T*>(a.gz) + roff, n0, N, vec, nn);
-                }
-                continue;
-            }
-            if (MODE != MODE_JOINT && (C.cubic & 2u)) {
-                outer_c4_row<T, kT, kA, MODE == MODE_JOINT ? MODE_SNIA : MODE>(a, C, row, n0, zv, mo, isig2, lnorm, kLike ? (unsigned)W_MU : which,
+            if (C.cubic & 2u) {                                  // two complex root pairs: slow path, whole row
+                outer_c4_row<T, kT, kA, MODE>(a, C, row, n0, zv, mo, isig2, lnorm, zo, kLike ? (unsigned)W_MU : which,
                                               kG ? &sacc[warp][sl][0] : nullptr, lane, gzacc);
                 continue;
             }

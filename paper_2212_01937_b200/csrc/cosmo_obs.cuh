@@ -20,15 +20,20 @@ struct Obs {
 };
 
 // Rows whose E^2 has no real negative root (Cosmo::cubic bit 1): replace the fused real path's result by the complex
-// slow path (cosmo_c4.cuh).  Forward values only: K, 1/E are poisoned so that every gradient of such a row is NaN.
+// slow path (cosmo_c4.cuh), including K, E, 1/E and E - 1 in the meaning the gradient bases of such rows expect.
 template <typename T, bool kT, bool kA, bool kGrad>
 CB_HD void apply_c4(const Cosmo<T>& C, T z, Core<T>& R) {
     if (!(C.cubic & 2u)) return;
-    double I0, TT, AA;
-    eval_c4((double)C.Or, (double)C.m, (double)C.rn, (double)C.b, (double)C.c, (double)z, kT, kA, I0, TT, AA);
-    R.I0 = (T)I0; R.TT = (T)TT; R.AA = (T)AA;
-    R.K = T(NAN); R.iE = T(NAN);
-    R.status = C.status | ((T(1) + z > T(0)) ? 0u : (unsigned)ST_UNSUPPORTED) | (kGrad ? (unsigned)ST_GRAD_ILLCOND : 0u);
+    double I0, TT, AA, KK;
+    eval_c4((double)C.Or, (double)C.m, (double)C.rn, (double)C.b, (double)C.c, (double)z, kT, kA, I0, TT, AA, KK);
+    R.I0 = (T)I0; R.TT = (T)TT; R.AA = (T)AA; R.K = (T)KK;
+    {
+        const double x = 1.0 + (double)z, xp1 = x + 1.0, c2 = fma(xp1, x, 1.0);
+        const double Ev = sqrt(fma(fma((double)C.Or, x, (double)C.m), x, (double)C.rn) * fma(x + (double)C.b, x, (double)C.c));
+        const double t = fma((double)C.Or, fma(c2, x, 1.0), fma((double)C.Om, c2, (double)C.Ok * xp1));     // (E^2 - 1)/z
+        R.E = (T)Ev; R.iE = (T)(1.0 / Ev); R.Em1 = (T)((double)z * t / (Ev + 1.0));
+    }
+    R.status = C.status | ((T(1) + z > T(0)) ? 0u : (unsigned)ST_UNSUPPORTED);
 }
 
 // Comoving volume over the whole sky, V_C = 4 pi dH^3 v, v(k, I0) = int_0^{I0} F(k, I)^2 dI (ref. [59] eq. (13.60)):
@@ -139,10 +144,16 @@ CB_HD void observables(const Cosmo<T>& C, T z, const Core<T>& R, unsigned which,
 // term beyond it (< 2e-15); its parameter derivatives use the same T-basis at that point.  FP64; called after cosmo_prep.
 CB_HD void prep_age(Cosmo<double>& C, bool with_grad) {
     C.Tinf = NAN; C.dTinf[0] = C.dTinf[1] = C.dTinf[2] = NAN;
-    if ((C.cubic & 2u) || C.status) return;
+    if (C.status) return;
     const double X = 1.0e10, z = X - 1.0;
     Core<double> R;
-    eval_core<double, true, false, true, VoteNone>(C, z, VoteNone(), R);
+    if (C.cubic & 2u) {
+        R.I0 = R.TT = R.AA = R.K = R.E = R.iE = R.Em1 = 0.0;
+        R.status = C.status;
+        apply_c4<double, true, false, true>(C, z, R);
+    } else {
+        eval_core<double, true, false, true, VoteNone>(C, z, VoteNone(), R);
+    }
     if (R.status) return;
     const double tail = (C.Or * X > C.Om) ? 0.5 / (sqrt(C.Or) * X * X) : (2.0 / 3.0) / (sqrt(C.Om) * X * sqrt(X));
     C.Tinf = R.TT + tail;
@@ -197,7 +208,7 @@ CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, c
     // - (k-2) Or J'_{k+3}, the Or terms iterated (same scheme as the forward d_abs).
     bool useJ = false;
     T Jp[17];
-    if (kA && !(C.cubic & 2u)) {
+    if (kA) {
         constexpr int KJ = 12;                // levels k = 3 .. 3 + KJ - 1
 #pragma unroll
         for (int p = 0; p < 5; ++p)

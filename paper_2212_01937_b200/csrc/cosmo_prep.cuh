@@ -174,8 +174,12 @@ CB_HD void cosmo_prep(double Om, double OL, double Or, double H0, int want_grad,
     // Eliminating c0 and c2 leaves a 3x3 system in (a, bK, c1), solved by its adjugate: no pivot search, no indexed
     // storage, so the whole solve stays in registers (the ELEMENTWISE kernels do it once per element).
     const double e0 = OL, e2 = Ok, e3 = Om, e4 = Or;
-    const double NK0 = m * m * c, NK1 = m * m * b + 2.0 * Or * m * c, NK2 = m * m + 2.0 * Or * m * b + Or * Or * c,
-                 NK3 = 2.0 * Or * m + Or * Or * b, NK4 = Or * Or;
+    // N_K = P_K(x) (x^2 + b x + c).  Real labelling: P_K = (Or x + m)^2 (the [p_n = -3] integral of the root rn).  Two complex
+    // pairs (C.m, C.rn carry g1, h1 of Q1 = Or x^2 + g1 x + h1 with roots r1 = conj(r2)): P_K = Or^2 Re (x - r1)^2
+    // = Or^2 x^2 + Or g1 x + g1^2/2 - Or h1, the real part of Carlson's [+1, -3] integral of the pair (cosmo_c4.cuh).
+    const bool c4 = (C.cubic & 2u) != 0;
+    const double pk2 = Or * Or, pk1 = c4 ? Or * m : 2.0 * Or * m, pk0 = c4 ? 0.5 * m * m - Or * rn : m * m;
+    const double NK0 = pk0 * c, NK1 = pk0 * b + pk1 * c, NK2 = pk0 + pk1 * b + pk2 * c, NK3 = pk1 + pk2 * b, NK4 = pk2;
     const double k0 = 2.0 / (3.0 * e3), k2 = 2.0 / e3;
     const double al0 = e2 * k0, be0 = NK2 * k0;                              // c0 = al0 a + be0 bK - k0 D2
     const double al2 = -e4 * k2, be2 = -NK4 * k2, de2 = e4 * k2;             // c2 = al2 a + be2 bK + de2 c1 + k2 D4

@@ -148,9 +148,30 @@ def test_two_complex_pairs_slow_path(hc):
     val = val.astype(np.float64)
     for i, tol in ((0, 1e-14), (1, 1e-14), (3, 1e-14), (4, 1e-14), (5, 1e-11)):
         assert (np.abs(out[i] - val[:, i]) / np.abs(val[:, i])).max() <= tol, i
-    g1 = np.zeros((6, n)); g1[0] = 1
-    _, gz, gp, st = run(hc, z, Om, OL, Or, H0, 63, g1)
-    assert np.isnan(gp[:3]).all() and ((st & 16) != 0).all()
+    # gradients: the bases of cosmo_prep.cuh with the pair's [+1, -3] integral (cosmo_c4.cuh) as the K column
+    _, grad, _ = oracle.observables_batch(z, Om, OL, Or, H0, with_grad=True)
+    grad = grad.astype(np.float64)
+    for pl, tols in ((0, (1e-14, 1e-9, 1e-9, 1e-8, 1e-14)), (3, (1e-14, 1e-9, 1e-9, 1e-8, 1e-14)), (4, (1e-14, 1e-9, 1e-9, 1e-8, 1e-14)),
+                     (5, (1e-14, 2e-7, 1e-8, 2e-6, 1e-11))):       # d_abs: the exact basis divides by Or
+        g1 = np.zeros((6, n)); g1[pl] = 1
+        _, gz, gp, st = run(hc, z, Om, OL, Or, H0, 63, g1)
+        assert (st == 0).all()
+        mine = np.vstack([gz[None], gp])
+        for p in range(5):
+            ref = grad[:, pl, p]
+            e = np.abs(mine[p] - ref) / np.maximum(np.abs(ref), 1e-3 * np.abs(val[:, pl]))
+            assert e.max() <= tols[p], (pl, p, e.max())
+    # D_A, V_C and age(z) (T_inf by the same slow path at x = 1e10) on these rows
+    dv, dg, _ = oracle.derived_batch(z, Om, OL, Or, H0)
+    dv, dg = dv.astype(np.float64), dg.astype(np.float64)
+    for k, pl in enumerate((6, 7, 8)):
+        g1 = np.zeros((9, n)); g1[pl] = 1
+        out9, gz, gp, st = run(hc, z, Om, OL, Or, H0, 511, g1)
+        assert (st == 0).all() and (np.abs(out9[pl] - dv[:, k]) <= 1e-13 * np.abs(dv[:, k])).all(), pl
+        mine = np.vstack([gz[None], gp])
+        for p in range(5):
+            e = np.abs(mine[p] - dg[:, k, p]) / np.maximum(np.abs(dg[:, k, p]), 1e-3 * np.abs(dv[:, k]))
+            assert e.max() <= 1e-8, (pl, p, e.max())
 
 
 def test_derived_observables_host(hc):
