@@ -108,15 +108,16 @@ CB_HD void c4_carlson(double x, double y, double z, cx p, bool want_j, C4Carlson
 }
 
 // I0, T, A of eqs. (3.7)-(3.9) with the roots r_1 = conj(r_2) of Q1 = Or x^2 + g1 x + h1 and r_3 = conj(r_4) of
-// Q2 = x^2 + b x + c, permutation (i, j, k, l) = (1, 2, 3, 4); everything in x = 1 + z (d_i5 = -rho_i).
+// Q2 = x^2 + b x + c, permutation (i, j, k, l) = (1, 2, 3, 4); everything in x = 1 + z (d_i5 = -rho_i), between the limits
+// x1 = 1 + z1 and x = 1 + z2 (the hot path calls it with x1 = 1).
 // (never inlined: a rare path must not cost the hot kernels registers)
-CB_HD_NOINLINE void eval_c4(double Or, double g1, double h1, double b, double c, double z, bool want_T, bool want_A,
+CB_HD_NOINLINE void eval_c4(double Or, double g1, double h1, double b, double c, double x1, double x, bool want_T, bool want_A,
                    double& I0, double& TT, double& AA, double& KK) {
-    const double x = 1.0 + z, dz = z;
+    const double dz = x - x1;
     const double D1 = 4.0 * Or * h1 - g1 * g1, D2 = 4.0 * c - b * b;       // both > 0 here
     const cx r1 = cx_(-g1 / (2.0 * Or), sqrt(D1) / (2.0 * Or)), r2 = cx_conj(r1);
     const cx r3 = cx_(-0.5 * b, 0.5 * sqrt(D2)), r4 = cx_conj(r3);
-    const cx X1 = cx_sqrt(cx_(x) - r1), Y1 = cx_sqrt(cx_(1.0) - r1), X3 = cx_sqrt(cx_(x) - r3), Y3 = cx_sqrt(cx_(1.0) - r3);
+    const cx X1 = cx_sqrt(cx_(x) - r1), Y1 = cx_sqrt(cx_(x1) - r1), X3 = cx_sqrt(cx_(x) - r3), Y3 = cx_sqrt(cx_(x1) - r3);
     const cx X2 = cx_conj(X1), Y2 = cx_conj(Y1), X4 = cx_conj(X3), Y4 = cx_conj(Y3);
     const cx u12 = X1 * X2 * Y3 * Y4 + Y1 * Y2 * X3 * X4;
     const cx u13 = X1 * X3 * Y2 * Y4 + Y1 * Y3 * X2 * X4;
@@ -132,7 +133,7 @@ CB_HD_NOINLINE void eval_c4(double Or, double g1, double h1, double b, double c,
     KK = sqrt(Or) * (((2.0 / 3.0) * dz * dz * dz * K.RDz) * (d13 * d14) + (2.0 * dz) * ((X1 * Y1) / (X2 * Y2 * u12))).re;
     TT = 0.0; AA = 0.0;
     if (want_T) {
-        const cx q5 = (cx_(x) / ((cx_(1.0) - r1) * (cx_(x) - r1))) * p5;
+        const cx q5 = (cx_(x * x1) / ((cx_(x1) - r1) * (cx_(x) - r1))) * p5;
         const cx s5 = q5 + (dz * dz) * (r3 * r4 * (r2 / r1));
         const cx br = cx_(K.RF) - ((dz * dz / 3.0) * (d12 * d13 * d14 / (-r1)) * K.RJ + cx_rc(s5, q5));
         TT = ia * ((2.0 * dz) * (br / r1)).re;
@@ -142,7 +143,7 @@ CB_HD_NOINLINE void eval_c4(double Or, double g1, double h1, double b, double c,
         const cx p0 = cx_(xa) - (dz * dz) * (d13 * d14);
         C4Carlson K0;
         c4_carlson(ya, za, xa, p0, true, K0);
-        const cx q0 = p0 / ((cx_(1.0) - r1) * (cx_(x) - r1));
+        const cx q0 = p0 / ((cx_(x1) - r1) * (cx_(x) - r1));
         const cx s0 = q0 + cx_(dz * dz);
         const cx bnd = X1 * X3 * X4 / X2 - Y1 * Y3 * Y4 / Y2;
         const cx sig = r1 + r2 + r3 + r4;

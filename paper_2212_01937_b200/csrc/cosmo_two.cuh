@@ -19,75 +19,84 @@ template <typename Vote>
 CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad, const Vote& vote, Two& O) {
     const double x1 = 1.0 + z1, x2 = 1.0 + z2, dz = z2 - z1, dz2 = dz * dz;
     unsigned st[1] = {C.status};
-    if (!(x1 > 0.0) || !(x2 > 0.0) || (C.cubic & 2u)) st[0] |= ST_UNSUPPORTED;
+    if (!(x1 > 0.0) || !(x2 > 0.0)) st[0] |= ST_UNSUPPORTED;
     if (fmax(x1, x2) >= C.xlim && fmin(x1, x2) < C.xlim) st[0] |= ST_ROOT_ON_PATH;
-    const bool quartA = !(C.cubic & 1u);
-    // ---- S4 radicands with both limits
-    const double L1 = fma(C.Or, x1, C.m), L2 = fma(C.Or, x2, C.m), xm1 = x1 - C.rn, xm2 = x2 - C.rn;
-    const double q21 = fma(x1 + C.b, x1, C.c), q22 = fma(x2 + C.b, x2, C.c);
-    const double a1 = L2 * xm2 * q21, a2 = L1 * xm1 * q22;
-    const double ra = sqrt(a1), rb = sqrt(a2), U12 = ra + rb;
-    double xa[1] = {U12 * U12}, mp[1], s[1], p5[1], p0[1];
-    const double hd = 0.5 * dz2 * C.theta, hs = dz2 * C.sDr;
-    mp[0] = xa[0] - hd;
-    s[0] = dz2 * dz2 * C.sD;
-    const double xa0 = xa[0], m0 = mp[0], s0 = s[0];
-    p5[0] = fma(dz2, C.p5c, xa0);
-    p0[0] = quartA ? fma(-C.Or * dz2, C.Q2n, xa0) : xa0;
-    const double p5_0 = p5[0], p0_0 = p0[0];
-    const double pm5 = p5_0 - m0, pm0 = p0_0 - m0;
-    const double dl5[1] = {(p5_0 - xa0) * fma(pm5, pm5, -s0)}, dl0[1] = {(p0_0 - xa0) * fma(pm0, pm0, -s0)};
-    const double Qc[1] = {carlson_Qc<double>(hd, hs, true)}, Q5v[1] = {carlson_Qj<double>(xa0, m0, hs, p5_0)},
-                 Q0v[1] = {carlson_Qj<double>(xa0, m0, hs, p0_0)};
-    double f, tailD[1], sum5[1], sum0[1];
-    carlson_dup<double, true, true, true, 1, Vote>(xa, mp, s, p5, p0, dl5, dl0, Qc, Q5v, Q0v, st, vote, f, tailD, sum5, sum0);
-    const double RF = carlson_rf_series<double>(xa[0], mp[0], f, hd, s0);
-    const double RD = carlson_rd_series<double>(xa[0], mp[0], f, hd, s0, tailD[0]);
-    const double RJ5 = carlson_rj_series<double>(xa[0], mp[0], p5[0], f, xa0, m0, s0, p5_0, sum5[0]);
-    const double RJ0 = carlson_rj_series<double>(xa[0], mp[0], p0[0], f, xa0, m0, s0, p0_0, sum0[0]);
-    // E at both limits; E2 - E1 without cancellation
-    const double E1 = sqrt(L1 * xm1 * q21), E2 = ra * rb / E1;
-    const double s12 = x1 + x2, p12 = x1 * x2, sq = fma(x2, x2, x1 * x1);          // x1+x2, x1 x2, x1^2+x2^2
-    const double dE = dz * (C.Or * s12 * sq + C.Om * (sq + p12) + C.Ok * s12) / (E1 + E2);
-    // ---- S6 reductions
-    const double I0 = 2.0 * dz * RF;                                                // eq. (3.7)
-    const double K = 2.0 * dz * fma(dz2 * CB_KT.third * C.W, RD, sqrt(L1 * L2 / (xm1 * xm2)) / U12);
-    const double qh = p12 * p5_0 * C.m * C.m / (L1 * L2);
-    const double TT = 2.0 * dz * (dz2 * CB_KT.third * C.Gp * RJ5 + rc<double>(fma(dz2, C.OL, qh), qh) - C.OrM * RF);   // eq. (3.8)
-    double AA;
-    const double bnd = sqrt(xm1 * xm2) / U12;
-    if (quartA) {                                                                   // eq. (3.9), (i,j,k,l) = (rn, pair, pair, big)
-        const double q0 = p0_0 / (xm1 * xm2);
-        const double B0 = fma(dz2 * CB_KT.third * C.Q2n * C.mOrn, RJ0, rc<double>(fma(C.Or, dz2, q0), q0));
-        const double F1 = sqrt(xm1 * q21 / L1), F2 = sqrt(xm2 * q22 / L2);
-        const double c2 = C.b - C.rn, c1 = fma(-C.rn, C.b, C.c);
-        const double dC = (sq + p12) + fma(c2, s12, c1);                            // (C(x2) - C(x1)) / dz, C = (x - rn) Q2
-        const double t1 = dz * fma(L1, dC, -xm1 * q21 * C.Or) / (L1 * L2 * (F1 + F2));
-        const double t2 = dz * C.aF * RF;
-        const double t3 = dz * C.WoOr * fma(dz2 * CB_KT.third * C.Q2n, RD, bnd / sqrt(L1 * L2));
-        const double t4 = dz * C.sig * B0;
-        const double A39 = (t1 + t2) + (t3 + t4);
-        // radiation-perturbative assembly (see eval_core_k): u_j = int x^j dx/E between the limits
-        constexpr int KS = 8;
-        double u[KS + 4], bk[KS + 1];
-        u[0] = I0;
-        u[1] = fma(2.0 * dz, B0, C.rn * I0);
-        double xk1 = 1.0, xk2 = 1.0;
-        for (int j = 0; j <= KS; ++j) { bk[j] = fma(xk2 - xk1, E2, xk1 * dE); xk1 *= x1; xk2 *= x2; }    // x2^j E2 - x1^j E1
-        for (int j = 2; j < KS + 4; ++j) u[j] = 0.0;
-        double prev = 0.0;
-        for (int sw = 0; sw < KS; ++sw) {
-            if (sw == KS - 1) prev = u[2];
-            for (int j = 0; j <= KS - sw; ++j) {
-                double acc = bk[j] - (j + 2) * C.Or * u[j + 3] - (j + 1) * C.Ok * u[j + 1];
-                if (j >= 1) acc -= j * C.OL * u[j - 1];
-                u[j + 2] = acc * C.iOm / (j + 1.5);
+    double I0, K, TT, AA, E1, E2, dE;
+    if (C.cubic & 2u) {
+        // two complex pairs (C.m, C.rn carry g1, h1): eqs. (3.7)-(3.9) as printed with a complex r_i, cosmo_c4.cuh
+        eval_c4(C.Or, C.m, C.rn, C.b, C.c, x1, x2, true, true, I0, TT, AA, K);
+        E1 = sqrt(fma(fma(C.Or, x1, C.m), x1, C.rn) * fma(x1 + C.b, x1, C.c));
+        E2 = sqrt(fma(fma(C.Or, x2, C.m), x2, C.rn) * fma(x2 + C.b, x2, C.c));
+        const double s12 = x1 + x2, p12 = x1 * x2, sq = fma(x2, x2, x1 * x1);
+        dE = dz * (C.Or * s12 * sq + C.Om * (sq + p12) + C.Ok * s12) / (E1 + E2);
+    } else {
+        const bool quartA = !(C.cubic & 1u);
+        // ---- S4 radicands with both limits
+        const double L1 = fma(C.Or, x1, C.m), L2 = fma(C.Or, x2, C.m), xm1 = x1 - C.rn, xm2 = x2 - C.rn;
+        const double q21 = fma(x1 + C.b, x1, C.c), q22 = fma(x2 + C.b, x2, C.c);
+        const double a1 = L2 * xm2 * q21, a2 = L1 * xm1 * q22;
+        const double ra = sqrt(a1), rb = sqrt(a2), U12 = ra + rb;
+        double xa[1] = {U12 * U12}, mp[1], s[1], p5[1], p0[1];
+        const double hd = 0.5 * dz2 * C.theta, hs = dz2 * C.sDr;
+        mp[0] = xa[0] - hd;
+        s[0] = dz2 * dz2 * C.sD;
+        const double xa0 = xa[0], m0 = mp[0], s0 = s[0];
+        p5[0] = fma(dz2, C.p5c, xa0);
+        p0[0] = quartA ? fma(-C.Or * dz2, C.Q2n, xa0) : xa0;
+        const double p5_0 = p5[0], p0_0 = p0[0];
+        const double pm5 = p5_0 - m0, pm0 = p0_0 - m0;
+        const double dl5[1] = {(p5_0 - xa0) * fma(pm5, pm5, -s0)}, dl0[1] = {(p0_0 - xa0) * fma(pm0, pm0, -s0)};
+        const double Qc[1] = {carlson_Qc<double>(hd, hs, true)}, Q5v[1] = {carlson_Qj<double>(xa0, m0, hs, p5_0)},
+                     Q0v[1] = {carlson_Qj<double>(xa0, m0, hs, p0_0)};
+        double f, tailD[1], sum5[1], sum0[1];
+        carlson_dup<double, true, true, true, 1, Vote>(xa, mp, s, p5, p0, dl5, dl0, Qc, Q5v, Q0v, st, vote, f, tailD, sum5, sum0);
+        const double RF = carlson_rf_series<double>(xa[0], mp[0], f, hd, s0);
+        const double RD = carlson_rd_series<double>(xa[0], mp[0], f, hd, s0, tailD[0]);
+        const double RJ5 = carlson_rj_series<double>(xa[0], mp[0], p5[0], f, xa0, m0, s0, p5_0, sum5[0]);
+        const double RJ0 = carlson_rj_series<double>(xa[0], mp[0], p0[0], f, xa0, m0, s0, p0_0, sum0[0]);
+        // E at both limits; E2 - E1 without cancellation
+        E1 = sqrt(L1 * xm1 * q21); E2 = ra * rb / E1;
+        const double s12 = x1 + x2, p12 = x1 * x2, sq = fma(x2, x2, x1 * x1);          // x1+x2, x1 x2, x1^2+x2^2
+        dE = dz * (C.Or * s12 * sq + C.Om * (sq + p12) + C.Ok * s12) / (E1 + E2);
+        // ---- S6 reductions
+        I0 = 2.0 * dz * RF;                                                // eq. (3.7)
+        K = 2.0 * dz * fma(dz2 * CB_KT.third * C.W, RD, sqrt(L1 * L2 / (xm1 * xm2)) / U12);
+        const double qh = p12 * p5_0 * C.m * C.m / (L1 * L2);
+        TT = 2.0 * dz * (dz2 * CB_KT.third * C.Gp * RJ5 + rc<double>(fma(dz2, C.OL, qh), qh) - C.OrM * RF);   // eq. (3.8)
+        const double bnd = sqrt(xm1 * xm2) / U12;
+        if (quartA) {                                                                   // eq. (3.9), (i,j,k,l) = (rn, pair, pair, big)
+            const double q0 = p0_0 / (xm1 * xm2);
+            const double B0 = fma(dz2 * CB_KT.third * C.Q2n * C.mOrn, RJ0, rc<double>(fma(C.Or, dz2, q0), q0));
+            const double F1 = sqrt(xm1 * q21 / L1), F2 = sqrt(xm2 * q22 / L2);
+            const double c2 = C.b - C.rn, c1 = fma(-C.rn, C.b, C.c);
+            const double dC = (sq + p12) + fma(c2, s12, c1);                            // (C(x2) - C(x1)) / dz, C = (x - rn) Q2
+            const double t1 = dz * fma(L1, dC, -xm1 * q21 * C.Or) / (L1 * L2 * (F1 + F2));
+            const double t2 = dz * C.aF * RF;
+            const double t3 = dz * C.WoOr * fma(dz2 * CB_KT.third * C.Q2n, RD, bnd / sqrt(L1 * L2));
+            const double t4 = dz * C.sig * B0;
+            const double A39 = (t1 + t2) + (t3 + t4);
+            // radiation-perturbative assembly (see eval_core_k): u_j = int x^j dx/E between the limits
+            constexpr int KS = 8;
+            double u[KS + 4], bk[KS + 1];
+            u[0] = I0;
+            u[1] = fma(2.0 * dz, B0, C.rn * I0);
+            double xk1 = 1.0, xk2 = 1.0;
+            for (int j = 0; j <= KS; ++j) { bk[j] = fma(xk2 - xk1, E2, xk1 * dE); xk1 *= x1; xk2 *= x2; }    // x2^j E2 - x1^j E1
+            for (int j = 2; j < KS + 4; ++j) u[j] = 0.0;
+            double prev = 0.0;
+            for (int sw = 0; sw < KS; ++sw) {
+                if (sw == KS - 1) prev = u[2];
+                for (int j = 0; j <= KS - sw; ++j) {
+                    double acc = bk[j] - (j + 2) * C.Or * u[j + 3] - (j + 1) * C.Ok * u[j + 1];
+                    if (j >= 1) acc -= j * C.OL * u[j - 1];
+                    u[j + 2] = acc * C.iOm / (j + 1.5);
+                }
             }
+            AA = (fabs(u[2] - prev) <= 1e-14 * fabs(u[2])) ? u[2] : A39;
+        } else {                                                                        // eq. (B.3), i = rn
+            AA = CB_KT.two_thirds * dz * (dE / (C.m * dz) + C.aF * RF + 2.0 * C.sig * fma(dz2 * CB_KT.third * C.Q2n * C.m, RD, bnd));
+            if (dz == 0.0) AA = 0.0;
         }
-        AA = (fabs(u[2] - prev) <= 1e-14 * fabs(u[2])) ? u[2] : A39;
-    } else {                                                                        // eq. (B.3), i = rn
-        AA = CB_KT.two_thirds * dz * (dE / (C.m * dz) + C.aF * RF + 2.0 * C.sig * fma(dz2 * CB_KT.third * C.Q2n * C.m, RD, bnd));
-        if (dz == 0.0) AA = 0.0;
     }
     // ---- S7
     double F, Fi, Fk;

@@ -634,6 +634,30 @@ def test_two_limit(cb):
     assert np.allclose(o2.cpu().numpy(), o1.cpu().numpy()[:, 0], rtol=1e-13, atol=0)
 
 
+def test_two_limit_two_complex_pairs(cb):
+    """cosmo_eval2 on cosmologies whose E^2 has no real negative root (complex slow path between the two limits)"""
+    rng = np.random.default_rng(7)
+    n = 257
+    Om = rng.uniform(0.050, 0.056, n); Or = rng.uniform(9.3e-4, 1e-3, n); OL = rng.uniform(0.01, 0.12, n); H0 = rng.uniform(60, 80, n)
+    z1 = rng.uniform(0, 3, n); z2 = z1 + 10 ** rng.uniform(-3, 0.8, n)
+    z1[:16], z2[:16] = z2[:16].copy(), z1[:16].copy()
+    which = ("DC", "DM", "TL", "DABS", "DA")
+    g = rng.standard_normal((5, n))
+    out, g1, g2, gp, st = cb.cosmo_eval2(dev(z1), dev(z2), dev(Om), dev(OL), dev(Or), dev(H0), which, grad_out=dev(g))
+    out, g1, g2, gp, st = out.cpu().numpy(), g1.cpu().numpy(), g2.cpu().numpy(), gp.cpu().numpy(), st.cpu().numpy()
+    v, gr, so = oracle.observables2_batch(z1, z2, Om, OL, Or, H0)
+    v, gr = v.astype(np.float64), gr.astype(np.float64)
+    assert (so == 0).all() and (st == 0).all()
+    order = [oracle.OBS2.index(w) for w in which]
+    for k, o in enumerate(order):
+        assert relerr(out[k], v[:, o]).max() <= TOL_VAL, which[k]
+    mine = [g1, g2] + [gp[t] for t in range(4)]
+    for c in range(6):
+        ref = sum(g[k] * gr[:, o, c] for k, o in enumerate(order))
+        sab = sum(np.abs(g[k] * gr[:, o, c]) for k, o in enumerate(order))
+        assert (np.abs(mine[c] - ref) <= (2e-7 if c == 4 else TOL_GRAD) * sab).all(), c
+
+
 # ---------------------------------------------------------------- extra constant-w components (SURVEY NEXT-3, PAPER.md:82 fn.4)
 def test_extra_w_components(cb):
     """cosmo_eval_w (general quartic E^2 with w = -1/3 and w = -2/3 components; chi family + d/dz) against oracle.w_chi_batch:

@@ -214,6 +214,29 @@ def test_two_limit_host(hc):
             assert e.max() <= tol, (nm, oracle.WRT2[k], e.max())
 
 
+def test_two_limit_two_complex_pairs_host(hc):
+    """the two-limit forms on cosmologies without a real negative root (cosmo_c4.cuh between x1 and x2), both orders of the limits"""
+    rng = np.random.default_rng(7)
+    n = 80
+    Om = rng.uniform(0.050, 0.056, n); Or = rng.uniform(9.3e-4, 1e-3, n); OL = rng.uniform(0.01, 0.12, n); H0 = rng.uniform(60, 80, n)
+    z1 = rng.uniform(0, 3, n); z2 = z1 + 10 ** rng.uniform(-3, 0.8, n)
+    z1[:8], z2[:8] = z2[:8].copy(), z1[:8].copy()
+    val = np.zeros((5, n)); g1 = np.zeros((5, n)); g2 = np.zeros((5, n)); gp = np.zeros((5, 4, n)); st = np.zeros(n, dtype=np.uint8)
+    dp = lambda a: a.ctypes.data_as(DP)
+    hc.hostcheck_two(C.c_int64(n), dp(z1), dp(z2), dp(Om), dp(OL), dp(Or), dp(H0), dp(val), dp(g1), dp(g2), dp(gp),
+                     st.ctypes.data_as(C.POINTER(C.c_uint8)))
+    v, g, so = oracle.observables2_batch(z1, z2, Om, OL, Or, H0)
+    v, g = v.astype(np.float64), g.astype(np.float64)
+    assert (so == 0).all() and (st == 0).all()
+    for o, nm in enumerate(oracle.OBS2):
+        assert (np.abs(val[o] - v[:, o]) / np.abs(v[:, o])).max() <= 1e-11, nm
+        mine = [g1[o], g2[o]] + [gp[o, t] for t in range(4)]
+        for k in range(6):
+            e = np.abs(mine[k] - g[:, o, k]) / np.maximum(np.abs(g[:, o, k]), 1e-3 * np.abs(v[:, o]))
+            tol = 2e-7 if (nm == "DABS" and k == 4) else 1e-8       # d(d_abs)/dOr: DESIGN.md section 6
+            assert e.max() <= tol, (nm, oracle.WRT2[k], e.max())
+
+
 def test_extra_w_components_host(hc):
     """chi family on the general quartic (cosmo_w.cuh; PAPER.md:82 fn.4) against oracle.w_chi_batch"""
     w = W.wmix(n=6000)
