@@ -248,7 +248,7 @@ def run_ours(args):
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": (achieved / peak_tflops) if (achieved and peak_tflops) else None,
                 "traffic": RL.DRAM_TRAFFIC_BYTES_PER_LAUNCH["config3_vjp_mu_f64"] if (N, S) == (1_000_000, 64) else None,
-                "traffic_unit": "bytes/launch (ncu dram read+write, profiles/r01b_k_outer_vjp.md)",
+                "traffic_unit": "bytes/launch (ncu dram read+write, profiles/r01c_k_outer_vjp.md)",
                 "algorithmic_bytes": RL.BYTES_PER_EVAL_C3 * evals,
                 "fp64_pipe_frac": (RL.FP64_PIPE_INST_PER_EVAL["config3_vjp_mu_f64"] * evals / (k_ms * 1e-3)) / (peak_tflops * 0.5e12)
                 if (k_ms > 0 and peak_tflops) else None,

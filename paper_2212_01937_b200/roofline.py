@@ -9,7 +9,8 @@ probe (cosmo_probe_fma_f64); the nominal figure beside it is 148 SMs x 64 FP64 F
 """
 
 # FP64 work per eval of the config-3 fused forward+VJP kernel k_outer<double,false,false,VJP,MU> as committed, from the
-# ncu capture profiles/r01b_k_outer_vjp.md (6.4e7 evals/launch):
+# ncu captures profiles/r01b_k_outer_vjp.md and (re-captured for the committed build, same counts) profiles/r01c_k_outer_vjp.md
+# (6.4e7 evals/launch):
 #   DFMA 137.4, DMUL 98.7, DADD 24.5 thread-instructions per eval -> 2*137.4 + 98.7 + 24.5 = 397.9 flops
 #   FP64-pipe instructions per eval (the above + 5.3 DSETP) = 265.9
 # (earlier builds: profiles/r01_final_k_outer_vjp.md 430.6 flops / 300.1 pipe instructions; first working version,
@@ -23,7 +24,7 @@ FP64_PIPE_INST_PER_EVAL = {
 }
 # dram__bytes_read.sum + dram__bytes_write.sum of that kernel, per launch (same capture)
 DRAM_TRAFFIC_BYTES_PER_LAUNCH = {
-    "config3_vjp_mu_f64": 544.14e6 + 635.88e6,
+    "config3_vjp_mu_f64": 544.13e6 + 635.70e6,
 }
 
 # nominal B200 FP64 vector peak (context only; the denominator is the measured probe)
