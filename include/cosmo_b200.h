@@ -28,8 +28,8 @@
  *       4  D_L <= 0 (closed universe at/after the antipode): mu is NaN, the other outputs are valid
  *       8  the duplication loop hit its iteration cap before Carlson's stopping rule was met
  *      16  gradient ill-conditioned (near-degenerate roots; the 1/prod(r_j - r_k) of PAPER.md:320-345): values valid, gradients
- *          may have lost more than the documented accuracy (set by the VJP calls; the conditioning estimate is per element
- *          in ELEMENTWISE calls only)
+ *          may have lost more than the documented accuracy or be NaN (set by the VJP calls: per cosmology when the root pair's
+ *          gap has closed, e.g. OL -> 0, in every mode; plus a per-element conditioning estimate in ELEMENTWISE calls)
  */
 #ifndef COSMO_B200_H
 #define COSMO_B200_H

@@ -103,7 +103,7 @@ CB_HD void observables_k(const Cosmo<T>& C, const T (&z)[K], const Core<T> (&R)[
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         const T x = T(1) + z[k];
-        unsigned st = R[k].status;
+        unsigned st = R[k].status | ((C.cubic & 4u) << 2);      // ST_GRAD_ILLCOND of the cosmology (set by cosmo_prep with want_grad)
         O[k].v[0] = C.dH * I0[k];
         O[k].v[1] = C.dH * O[k].F;
         O[k].v[2] = x * O[k].v[1];

@@ -203,6 +203,11 @@ CB_HD void cosmo_prep(double Om, double OL, double Or, double H0, int want_grad,
         out5[3] = c1v;
         out5[4] = al2 * av + be2 * bv + de2 * c1v + g2;
     };
+    // The bases become linearly dependent as the gap g of the pair x^2 + b x + c closes (the 1/prod(r_j - r_k) of appendix A,
+    // PAPER.md:320-345; OL -> 0 is the commonest way there: the pair tends to +-sqrt(-OL/Ok) and at OL = 0 the system is singular).
+    // Measured error ~ 1e-13/g^2: below g^2 = 1e-5, or with a singular system, every gradient of this
+    // cosmology carries status bit 16 (observables() ORs it in), in ELEMENTWISE and OUTER calls alike.
+    if (!(fabs(D2) >= 1e-5) || !isfinite(idet)) C.cubic |= 4u;      // (not in C.status: that would stop the duplication loop)
     // I0: D_theta = dE^2/dtheta with Ok eliminated: x^3 - x^2, 1 - x^2, x^4 - x^2
     solve5(0.0, 0.0, -1.0, 1.0, 0.0, C.GI[0]);
     solve5(1.0, 0.0, -1.0, 0.0, 0.0, C.GI[1]);

@@ -102,7 +102,7 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
     double F, Fi, Fk;
     sinn<double>(C.Ok, I0, F, Fi, Fk);
     O.v[0] = C.dH * I0; O.v[1] = C.dH * F; O.v[2] = C.tH * TT; O.v[3] = C.dH * AA; O.v[4] = O.v[1] / x2;
-    O.status = st[0];
+    O.status = st[0] | (with_grad ? (C.cubic & 4u) << 2 : 0u);
     if (st[0] & (ST_ROOT_ON_PATH | ST_UNSUPPORTED)) {
         for (int i = 0; i < 5; ++i) O.v[i] = NAN;
     }

@@ -94,7 +94,8 @@ struct Cosmo {
     T Tinf, dTinf[3];  // int_1^inf dx/(x E) and its derivatives wrt (Om, OL, Or): age(z) = tH (Tinf - T(z))  (W_AGE only)
     T GJ[5][5];        // J'_p = int x^p dx / E^3, p = 0..4, over the basis (I0, K, b0, b1, b2)  (d_abs gradient)
     unsigned status;
-    unsigned cubic;    // bit 0: Or == 0 (cubic case, appendix B.1);  bit 1: two complex pairs (cosmo_c4.cuh; m, rn hold g1, h1)
+    unsigned cubic;    // bit 0: Or == 0 (cubic case, appendix B.1);  bit 1: two complex pairs (cosmo_c4.cuh; m, rn hold g1, h1);
+                       // bit 2: gradient bases ill-conditioned (reported as status bit 16)
 };
 
 constexpr int COSMO_NFIELDS = 115;   // floating-point members of Cosmo<T>, in declaration order

@@ -410,6 +410,24 @@ def test_two_complex_pairs_outer_and_likelihood(cb):
         assert (np.abs(gzl[s] - rgz) <= TOL_GRAD * np.maximum(np.abs(rgz), 1.0)).all(), s
 
 
+def test_vanishing_lambda_outer_flags_row(cb):
+    """OUTER VJP with one OL = 0 cosmology (Einstein-de Sitter-like: the gradient bases are singular): its row carries status
+    bit 16 and exact values; the other rows are clean and their gradients meet the tolerance"""
+    Om = np.array([0.3, 1.0, 0.28]); OL = np.array([0.7, 0.0, 0.65]); Or = np.array([9e-5, 0.0, 0.0]); H0 = np.array([70.0, 68.0, 72.0])
+    z = np.linspace(0.01, 3.0, 777)
+    g = np.random.default_rng(4).standard_normal((1, 3, len(z)))
+    gz, gp, out, st = cb.cosmo_vjp(dev(z), dev(Om), dev(OL), dev(Or), dev(H0), dev(g), cb.OUTER, ("DC",), want_out=True)
+    gp, st, out = gp.cpu().numpy(), st.cpu().numpy(), out.cpu().numpy()
+    assert (st[1] == 16).all() and (st[[0, 2]] == 0).all()
+    eds = 2.0 * (299792.458 / 68.0) * (1.0 - 1.0 / np.sqrt(1.0 + z))          # closed form, PAPER.md:233 context (EdS)
+    assert relerr(out[0, 1], eds).max() <= 1e-13
+    for s in (0, 2):
+        _, grad, _ = oracle_batch(z, Om[s:s + 1], OL[s:s + 1], Or[s:s + 1], H0[s:s + 1], True)
+        for p in range(4):
+            t = g[0, s] * grad[:, 0, 1 + p]
+            assert abs(gp[p, s] - t.sum()) <= TOL_GRAD * np.abs(t).sum(), (s, p)
+
+
 # ---------------------------------------------------------------- full sizes of configs 4 and 5 (sampled oracle + properties)
 def test_config4_full_size_sampled(cb):
     """BASELINE.json config 4 at full size (10^6 SNe x 256 samples); oracle on full N for 2 samples, properties for all"""

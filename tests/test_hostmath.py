@@ -265,6 +265,29 @@ def test_host_math_fp32(hc):
         assert (np.abs(out[i] - val[:, i]) / np.abs(val[:, i])).max() <= 2e-5, i
 
 
+def test_vanishing_lambda_flags_gradients(hc):
+    """OL -> 0 closes the gap of the pair (+-sqrt(-OL/Ok)): values stay exact, the gradient bases degenerate (singular at
+    OL = 0), and every such cosmology carries status bit 16 instead of silently losing digits"""
+    rng = np.random.default_rng(3)
+    n = 120
+    z = rng.uniform(0.01, 5, n); Om = rng.uniform(0.1, 0.6, n); H0 = np.full(n, 70.0)
+    for OLv, flagged in ((0.0, True), (1e-9, True), (1e-3, False)):
+        for Orv in (0.0, 9e-5):
+            OL = np.full(n, OLv); Or = np.full(n, Orv)
+            g1 = np.zeros((6, n)); g1[0] = 1
+            out, gz, gp, st = run(hc, z, Om, OL, Or, H0, 63, g1)
+            val, grad, _ = oracle.observables_batch(z, Om, OL, Or, H0, with_grad=True)
+            val, grad = val.astype(np.float64), grad.astype(np.float64)
+            assert (((st & 16) != 0) == flagged).all() and ((st & 15) == 0).all(), (OLv, Orv)
+            for i in range(6):
+                assert (np.abs(out[i] - val[:, i]) <= 1e-11 * np.abs(val[:, i])).all(), (OLv, Orv, i)
+            assert (np.abs(gz - grad[:, 0, 0]) <= 1e-12 * np.abs(grad[:, 0, 0])).all()            # d/dz is closed-form: always fine
+            if not flagged:
+                for p in range(3):
+                    e = np.abs(gp[p] - grad[:, 0, 1 + p]) / np.maximum(np.abs(grad[:, 0, 1 + p]), 1e-3 * np.abs(val[:, 0]))
+                    assert e.max() <= 1e-8, (OLv, Orv, p, e.max())
+
+
 def test_invalid_rows_status(hc):
     for z, Om, OL, Or, H0, bit in W.invalid_rows():
         out, _, _, st = run(hc, [z], Om, OL, Or, H0)
