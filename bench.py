@@ -64,11 +64,13 @@ def run_reference(args):
     import oracle
     n_s, S_s = 20_000, 4
     rates = []
+    # torchrun exports OMP_NUM_THREADS=1 to every rank; here the other ranks have exited, so rank 0 uses the host's cores as at N=1
+    threads = len(os.sched_getaffinity(0)) if int(os.environ.get("WORLD_SIZE", "1")) > 1 else None
     for _ in range(args.warmup):
-        oracle_rate(2000, 1)
+        oracle_rate(2000, 1, threads)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        r, cores, sample = oracle_rate(n_s, S_s)
+        r, cores, sample = oracle_rate(n_s, S_s, threads)
         rates.append(r)
     dt = time.perf_counter() - t0
     value = args.steps * n_s * S_s / dt
