@@ -391,8 +391,12 @@ __global__ void k_reduce_gz(const T* __restrict__ part, int ny, int64_t N, T* __
 }
 
 // ELEMENTWISE with one cosmology per redshift: S1-S8 per thread, no reductions.
+// Register budget: left alone the all-outputs variants take 255 registers (8 warps/SM) and wait on latency at a third of the
+// FP64 pipe; capping them at 128 (VJP) / 80 (forward) registers trades spills (written back to DRAM, profiles/r01c_timings.md)
+// for 16 / 24 warps per SM.  Measured on
+// config 5 (profiles/r01c_timings.md): forward 3.31 -> 2.15 ms, forward + VJP 4.75 -> 3.95 ms; config 2 forward 0.26 -> 0.18 ms.
 template <typename T, bool kT, bool kA, bool kG>
-__global__ void __launch_bounds__(ELEM_THREADS) k_elem(const T* __restrict__ z, const double* __restrict__ Om,
+__global__ void __launch_bounds__(ELEM_THREADS, kG ? 4 : 6) k_elem(const T* __restrict__ z, const double* __restrict__ Om,
                                                        const double* __restrict__ OL, const double* __restrict__ Or,
                                                        const double* __restrict__ H0, int64_t N, unsigned which,
                                                        const T* __restrict__ gout, T* __restrict__ out, T* __restrict__ gz,
@@ -445,7 +449,8 @@ __global__ void __launch_bounds__(ELEM_THREADS) k_elem(const T* __restrict__ z, 
 }
 
 // Two-limit evaluation (cosmo_two.cuh), one thread per (z1, z2, cosmology); n_cosmo in {1, n}.  which: DC, DM, TL, DABS, DA.
-__global__ void __launch_bounds__(ELEM_THREADS) k_two(const double* __restrict__ z1, const double* __restrict__ z2,
+// (128-register cap as for k_elem: 0.40 -> 0.28 ms forward, 0.75 -> 0.56 ms forward + VJP per 10^6 pairs)
+__global__ void __launch_bounds__(ELEM_THREADS, 4) k_two(const double* __restrict__ z1, const double* __restrict__ z2,
                                                       const double* __restrict__ Om, const double* __restrict__ OL,
                                                       const double* __restrict__ Or, const double* __restrict__ H0, int64_t n,
                                                       int64_t n_cosmo, unsigned which, const double* __restrict__ gout,
