@@ -244,3 +244,35 @@ def test_loglike_special_cases_and_brute_force():
     assert abs(mp.mpf(float(out[0])) - ll) < 1e-12
     for p in range(4):
         assert abs(mp.mpf(float(out[1 + p])) - gr[p]) < 1e-10 * max(1, abs(gr[p]))
+
+
+def test_loglike_against_scipy_density_and_finite_differences():
+    """Pins of oracle.snia_loglike that do not retype its formula (mu_obs | mu ~ N(mu, sigma^2)):
+    the value against SciPy's normal log-density summed over objects, and all four parameter gradients against Richardson-
+    extrapolated central differences of the VALUE (so a wrong sign, a missing 1/sigma^2 or a wrong d mu/d theta fails)."""
+    from scipy import stats
+    rng = np.random.default_rng(17)
+    n = 25
+    z = rng.uniform(0.02, 1.5, n)
+    sig = rng.uniform(0.05, 0.25, n)
+    th = [0.31, 0.66, 9e-5, 68.5]
+    one = lambda v: np.array([float(v)])
+    mu_of = lambda t: oracle.observables_batch(z, one(t[0]), one(t[1]), one(t[2]), one(t[3]), with_grad=False)[0][:, 3].astype(np.float64)
+    mu_obs = mu_of(th) + rng.normal(0, 0.15, n)
+    out = oracle.snia_loglike(z, mu_obs, sig, *th)
+    ref = stats.norm.logpdf(mu_obs, loc=mu_of(th), scale=sig).sum()
+    assert abs(float(out[0]) - ref) <= 1e-12 * abs(ref)
+    f = lambda t: oracle.snia_loglike(z, mu_obs, sig, *t, with_grad=False)[0]          # long double
+    for p, h in enumerate((2e-4, 2e-4, 2e-5, 2e-2)):
+        def cd(hh):
+            tp, tm = list(th), list(th)
+            tp[p] += hh; tm[p] -= hh
+            return (f(tp) - f(tm)) / np.longdouble(2 * hh)
+        fd = (4 * cd(h / 2) - cd(h)) / 3                                                # Richardson: O(h^4)
+        g = out[1 + p]
+        assert abs(float(fd - g)) <= 1e-9 * max(abs(float(g)), 1.0), (p, float(fd), float(g))
+    # a single object: the gradient is (residual / sigma^2) * d mu / d theta of the (separately pinned) observables
+    o1 = oracle.snia_loglike(z[:1], mu_obs[:1], sig[:1], *th)
+    _, g1, _ = oracle.observables(z[0], *th)
+    for p in range(4):
+        assert abs(float(o1[1 + p]) - (mu_obs[0] - mu_of(th)[0]) / sig[0] ** 2 * float(g1[3, 1 + p])) <= 1e-9 * abs(float(o1[1 + p]))
