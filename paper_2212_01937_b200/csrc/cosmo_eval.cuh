@@ -476,9 +476,9 @@ CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Cor
                 u[0] = R[k].I0;
                 u[1] = N::fma_(T(2) * z[k], B0, C.rn * R[k].I0);
                 {
-                    T xk = T(1);
+                    T dk = T(0);           // x^j - 1 = x (x^(j-1) - 1) + z: no cancellation at small z
 #pragma unroll
-                    for (int j = 0; j <= KS; ++j) { bk[j] = N::fma_(xk - T(1), R[k].E, R[k].Em1); xk *= x; }
+                    for (int j = 0; j <= KS; ++j) { bk[j] = N::fma_(dk, R[k].E, R[k].Em1); dk = N::fma_(x, dk, z[k]); }
 #pragma unroll
                     for (int j = 2; j < KS + 4; ++j) u[j] = T(0);
                 }

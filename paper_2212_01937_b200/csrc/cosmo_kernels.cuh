@@ -122,14 +122,16 @@ struct OuterArgs {
     int vec;                 // N even and pointers 16-byte aligned
 };
 
-// One cosmology row of the OUTER kernels whose E^2 has no real negative root (Cosmo::cubic bit 1): complex slow path
-// (cosmo_c4.cuh), values and gradients, one element at a time.  Never inlined and called at the top of the per-cosmology
-// iteration, where almost nothing is live, so that this rare case costs the hot loop no registers.
+// One cosmology row of the OUTER kernels that cannot take the fused loop: E^2 without a real negative root (Cosmo::cubic bit 1:
+// complex slow path, cosmo_c4.cuh) or gradient bases that need the per-element conditioning check (bits 2, 3: backward_robust).
+// One element at a time.  Never inlined and called at the top of the per-cosmology iteration, where almost nothing is live, so
+// that these rare cases cost the hot loop no registers.
 template <typename T, bool kT, bool kA, int MODE>
-__device__ __noinline__ void outer_c4_row(const OuterArgs& a, const Cosmo<T>& C, int64_t row, int64_t n0, const T* zv, const T* mo,
-                                          const T* isig2, const T* lnorm, const T* zo, unsigned which, double* sacc_row, int lane,
-                                          T* gzacc) {
+__device__ __noinline__ void outer_slow_row(const OuterArgs& a, const Cosmo<T>& C, int64_t row, int64_t n0, const T* zv, const T* mo,
+                                            const T* isig2, const T* lnorm, const T* zo, unsigned which, double* sacc_row, int lane,
+                                            T* gzacc) {
     constexpr bool kLike = MODE == MODE_SNIA || MODE == MODE_JOINT;
+    constexpr bool kG = MODE != MODE_FWD;
     constexpr int NP = kLike ? 5 : 4;
     constexpr int KZ = outer_kz(kT, kA);
     const int64_t N = a.N, S = a.S;
@@ -140,14 +142,15 @@ __device__ __noinline__ void outer_c4_row(const OuterArgs& a, const Cosmo<T>& C,
         Core<T> R;
         R.I0 = R.TT = R.AA = R.K = R.E = R.iE = R.Em1 = T(0);
         R.status = C.status;
-        apply_c4<T, kT, kA, MODE != MODE_FWD>(C, zv[k], R);
+        if (C.cubic & 2u) apply_c4<T, kT, kA, kG>(C, zv[k], R);
+        else eval_core<T, kT, kA, kG, VoteWarp>(C, zv[k], VoteWarp(), R);
         Obs<T> O;
         observables<T, kT, kA>(C, zv[k], R, which, O);
         if (kLike) {
             const T resid = mo[k] - O.v[3];
             T gg[N_PLANES] = {T(0), T(0), T(0), resid * isig2[k], T(0), T(0), T(0), T(0), T(0)};
             T dz = T(0), gp[4] = {T(0), T(0), T(0), T(0)};
-            backward<T, false, false>(C, zv[k], R, O, gg, dz, gp);
+            backward_robust<T, false, false>(C, zv[k], R, O, gg, dz, gp, W_MU);
             T ll = Num<T>::fma_(T(-0.5) * resid, resid * isig2[k], lnorm[k]);
             if (MODE == MODE_JOINT) {       // same photometric-redshift and prior terms as the fused row of k_outer
                 const T x = T(1) + zv[k], ix = Num<T>::rcp_(x);
@@ -163,17 +166,7 @@ __device__ __noinline__ void outer_c4_row(const OuterArgs& a, const Cosmo<T>& C,
                 for (int j = 0; j < 4; ++j) pacc[1 + j] += gp[j];
             }
         } else {
-            if (live) {
-                if (a.out != nullptr) {
-                    int pl = 0;
-                    for (int w = 0; w < N_PLANES; ++w) {
-                        if (!(which >> w & 1)) continue;
-                        static_cast<T*>(a.out)[((int64_t)pl * S + row) * N + col] = O.v[w];
-                        ++pl;
-                    }
-                }
-                if (a.status != nullptr) a.status[row * N + col] = (uint8_t)O.status;
-            }
+            unsigned stg = 0u;
             if (MODE == MODE_VJP) {
                 T g[N_PLANES];
                 int pl = 0;
@@ -184,8 +177,19 @@ __device__ __noinline__ void outer_c4_row(const OuterArgs& a, const Cosmo<T>& C,
                     ++pl;
                 }
                 T dz = T(0);
-                backward<T, kT, kA>(C, zv[k], R, O, g, dz, pacc, nullptr, which);
+                stg = backward_robust<T, kT, kA>(C, zv[k], R, O, g, dz, pacc, which);
                 if (live) gzacc[k] += dz;
+            }
+            if (live) {
+                if (a.out != nullptr) {
+                    int pl = 0;
+                    for (int w = 0; w < N_PLANES; ++w) {
+                        if (!(which >> w & 1)) continue;
+                        static_cast<T*>(a.out)[((int64_t)pl * S + row) * N + col] = O.v[w];
+                        ++pl;
+                    }
+                }
+                if (a.status != nullptr) a.status[row * N + col] = (uint8_t)(O.status | stg);
             }
         }
     }
@@ -254,9 +258,10 @@ __global__ void __launch_bounds__(OUTER_THREADS, CB_MINBLOCKS) k_outer(OuterArgs
             const Cosmo<T>& C = sc[sl];
             const int64_t row = c0 + sl;
             if (MODE == MODE_JOINT) load2(zp + roff, n0, N, vec, zv);      // latent redshifts: one row per sample
-            if (C.cubic & 2u) {                                  // two complex root pairs: slow path, whole row
-                outer_c4_row<T, kT, kA, MODE>(a, C, row, n0, zv, mo, isig2, lnorm, zo, kLike ? (unsigned)W_MU : which,
-                                              kG ? &sacc[warp][sl][0] : nullptr, lane, gzacc);
+            // two complex root pairs, or (with gradients) bases that need the per-element conditioning check: whole row apart
+            if ((C.cubic & 2u) || (kG && (C.cubic & 12u))) {
+                outer_slow_row<T, kT, kA, MODE>(a, C, row, n0, zv, mo, isig2, lnorm, zo, kLike ? (unsigned)W_MU : which,
+                                                kG ? &sacc[warp][sl][0] : nullptr, lane, gzacc);
                 continue;
             }
             T pacc[NP];
@@ -314,7 +319,12 @@ __global__ void __launch_bounds__(OUTER_THREADS, CB_MINBLOCKS) k_outer(OuterArgs
                 }
                 // straight into the accumulators: elements past N carry zero upstream gradients (see the load) and their
                 // grad_z is never stored
-                if (MODE == MODE_VJP) backward<T, kT, kA>(C, zv[k], R[k], O, g[k], gzacc[k], pacc, nullptr, which);
+                if (MODE == MODE_VJP) {
+                    // the chi-family bases of a screened cosmology run unchecked (cosmo_prep, Cosmo::cubic bit 3); the larger t_L / d_abs
+                    // bases are checked element by element
+                    if (kT || kA) stv[k] |= (uint8_t)backward_robust<T, kT, kA>(C, zv[k], R[k], O, g[k], gzacc[k], pacc, which);
+                    else backward<T, kT, kA>(C, zv[k], R[k], O, g[k], gzacc[k], pacc, nullptr, which);
+                }
             }
             if (MODE == MODE_JOINT && a.gz != nullptr) store2(static_cast<T*>(a.gz) + roff, n0, N, vec, gzacc);
             if (!kLike && a.out != nullptr) {
@@ -439,9 +449,8 @@ __global__ void __launch_bounds__(ELEM_THREADS, kG ? 4 : 6) k_elem(const T* __re
             ++pl;
         }
         T dz = T(0), gp[4] = {T(0), T(0), T(0), T(0)};
-        T cond = T(0);
-        backward<T, kT, kA, true>(C, zv, R, O, g, dz, gp, &cond);
-        if (status != nullptr) status[i] = (uint8_t)(O.status | ((cond > T(sizeof(T) == 8 ? GRAD_COND_LIMIT : 30.0) || !(cond == cond)) ? ST_GRAD_ILLCOND : 0u));
+        const unsigned stg = backward_robust<T, kT, kA>(C, zv, R, O, g, dz, gp, which);
+        if (status != nullptr) status[i] = (uint8_t)(O.status | stg);
         gz[i] = dz;
 #pragma unroll
         for (int j = 0; j < 4; ++j) gparams[(int64_t)j * N + i] = (double)gp[j];

@@ -103,7 +103,7 @@ CB_HD void observables_k(const Cosmo<T>& C, const T (&z)[K], const Core<T> (&R)[
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         const T x = T(1) + z[k];
-        unsigned st = R[k].status | ((C.cubic & 4u) << 2);      // ST_GRAD_ILLCOND of the cosmology (set by cosmo_prep with want_grad)
+        unsigned st = R[k].status;
         O[k].v[0] = C.dH * I0[k];
         O[k].v[1] = C.dH * O[k].F;
         O[k].v[2] = x * O[k].v[1];
@@ -125,7 +125,11 @@ CB_HD void observables_k(const Cosmo<T>& C, const T (&z)[K], const Core<T> (&R)[
             volume<T>(C.Ok, I0[k], v, O[k].Vk);
             O[k].v[7] = T(12.566370614359172954) * C.dH * C.dH * C.dH * v;
         }
-        if (kT && (which & W_AGE)) O[k].v[8] = C.tH * (C.Tinf - TT);
+        if (kT && (which & W_AGE)) {
+            O[k].v[8] = C.tH * (C.Tinf - TT);
+            // the age's parameter gradient needs the T-basis at x -> infinity (prep_age): not available where that basis is singular
+            if (!(C.dTinf[0] == C.dTinf[0]) && !bad[k]) st |= ST_GRAD_ILLCOND;
+        }
         O[k].status = st;
     }
 }
@@ -171,55 +175,70 @@ CB_HD void prep_age(Cosmo<double>& C, bool with_grad) {
     C.dTinf[2] -= 0.5 * rem;
 }
 
-// VJP of one element: g[N_PLANES] upstream (entries outside `which` must be 0).  Adds to gz and gp[0..3] = (Om, OL, Or, H0).
-// kCond: also return in *cond the cancellation factor max_theta sum_j |G_j basis_j| / max(|dI0/dtheta|, 1e-3 |I0|) of the
-// chi-family gradient (status bit 16 of the ELEMENTWISE calls is derived from it).
-// `which`: planes that can carry a non-zero upstream gradient; where the caller knows it at compile time the terms of the
-// other planes fold away (x * 0 is not foldable in IEEE arithmetic, so a zero g alone does not remove them).
-template <typename T, bool kT, bool kA, bool kCond = false>
-CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, const T g[N_PLANES], T& gz, T gp[4], T* cond = nullptr,
-                    unsigned which = W_ALL) {
+// ---- S8, first half: the parameter derivatives of the three integrals.
+// Raw gradient integrals of one element over [1, 1+z] (Leibniz' rule: d X / d theta = -1/2 of these), theta = (Om, OL, Or),
+// D_theta = dE^2/dtheta with Ok eliminated = x^3 - x^2, 1 - x^2, x^4 - x^2:
+//   dI[t] = int D_theta / E^3 dx,   dT[t] = int D_theta / (x E^3) dx,   dA[t] = int x^2 D_theta / E^3 dx
+template <typename T>
+struct GradInt { T dI[3], dT[3], dA[3]; };
+
+// From the gradient bases of cosmo_prep.cuh on the forward intermediates (the closed combination of
+// eqs. (2.10)-(2.12) + appendix A).
+// kCond: also return in *cond the cancellation factor of the evaluation, max over the requested families and theta of
+// (sum_j |G_j basis_j|) / max(|result|, 1e-3 |forward integral|): the relative error of the result is ~ 2e-16 x cond in FP64.  It
+// grows like 1 / prod(r_j - r_k) where roots of E^2 approach each other away from the path ("limits have to be
+// explicitly implemented when arguments are repeated"); callers switch to grad_quad() above GRAD_COND_LIMIT.
+template <typename T, bool kT, bool kA, bool kCond>
+CB_HD void grad_basis(const Cosmo<T>& C, T z, const Core<T>& R, GradInt<T>& D, T* cond = nullptr) {
     using N = Num<T>;
     const T x = T(1) + z;
     const T iE = R.iE;
-    const T rxd = N::rcp_(x * O.v[1]);                   // 1/(x D_M): one reciprocal serves 1/x and 1/D_M
-    const T ix = O.v[1] * rxd;
     // boundary terms b_k = x^k / E - 1 (cancellation-free)
     const T xp1 = x + T(1);
     const T n1 = z, n2 = z * xp1, n3 = z * N::fma_(xp1, x, T(1)), n4 = n2 * N::fma_(x, x, T(1));
     const T bt0 = -R.Em1 * iE, bt1 = (n1 - R.Em1) * iE, bt2 = (n2 - R.Em1) * iE;
-    T gM = T(0);
-    if (which & W_DM) gM = g[1];
-    if (which & W_DL) gM = N::fma_(x, g[2], gM);
-    if ((which & W_MU) && g[3] != T(0)) gM = N::fma_(T(CB_KT.five_over_ln10) * g[3], x * rxd, gM);
-    if ((which & W_DA) && g[6] != T(0)) gM = N::fma_(g[6], ix, gM);     // D_A = D_M / (1+z)
-    T aI = C.dH * ((which & W_DC) ? N::fma_(gM, O.Fi, g[0]) : gM * O.Fi);
-    T aK = -gM * C.dH * O.Fk;
-    if ((which & W_VC) && g[7] != T(0)) {                                                 // V_C = 4 pi dH^3 v(Ok, I0): dv = F^2 dI0 + v_k dOk
-        const T c4pi = T(12.566370614359172954) * C.dH * C.dH * C.dH * g[7];
-        aI = N::fma_(c4pi, O.F * O.F, aI);
-        aK = N::fma_(-c4pi, O.Vk, aK);
-    }
-    T btA = T(0);
-    if (kA) btA = (((C.cubic & 1u) ? n4 : n3) - R.Em1) * iE;
-    // d_abs gradient where radiation is a perturbation: the exact basis above then multiplies the forward A by ~3/Or
-    // (the x^5, x^6 rows), which loses Om/Or digits.  Instead J'_p = int x^p dx/E^3, p <= 4, come from the basis and
-    // J'_5.. follow from d(x^k / E) = N_k / E^3:  Om (k - 3/2) J'_{k+2} = [x^k/E] - k OL J'_{k-1} - (k-1) Ok J'_{k+1}
-    // - (k-2) Or J'_{k+3}, the Or terms iterated (same scheme as the forward d_abs).
-    bool useJ = false;
-    T Jp[17];
-    if (kA) {
-        constexpr int KJ = 12;                // levels k = 3 .. 3 + KJ - 1
+    T cmax = T(0);
 #pragma unroll
-        for (int p = 0; p < 5; ++p)
+    for (int t = 0; t < 3; ++t) {
+        D.dI[t] = C.GI[t][0] * R.I0 + C.GI[t][1] * R.K + C.GI[t][2] * bt0 + C.GI[t][3] * bt1 + C.GI[t][4] * bt2;
+        D.dT[t] = T(0); D.dA[t] = T(0);
+        if (kCond) {
+            const T sa = N::abs_(C.GI[t][0] * R.I0) + N::abs_(C.GI[t][1] * R.K) + N::abs_(C.GI[t][2] * bt0) + N::abs_(C.GI[t][3] * bt1)
+                         + N::abs_(C.GI[t][4] * bt2);
+            const T c = sa / N::max_(N::abs_(D.dI[t]), T(1e-3) * N::abs_(R.I0));
+            cmax = (c > cmax || !(c == c)) ? c : cmax;          // a NaN sticks
+        }
+        if (kT) {
+            D.dT[t] = C.GT[t][0] * R.I0 + C.GT[t][1] * R.K + C.GT[t][2] * bt0 + C.GT[t][3] * bt1 + C.GT[t][4] * bt2 + C.GT[t][5] * R.TT;
+            if (kCond) {
+                const T sa = N::abs_(C.GT[t][0] * R.I0) + N::abs_(C.GT[t][1] * R.K) + N::abs_(C.GT[t][2] * bt0) + N::abs_(C.GT[t][3] * bt1)
+                             + N::abs_(C.GT[t][4] * bt2) + N::abs_(C.GT[t][5] * R.TT);
+                const T c = sa / N::max_(N::abs_(D.dT[t]), T(1e-3) * N::abs_(R.TT));
+                cmax = (c > cmax || !(c == c)) ? c : cmax;
+            }
+        }
+    }
+    if (kA) {
+        const T btA = (((C.cubic & 1u) ? n4 : n3) - R.Em1) * iE;
+        // d_abs gradient where radiation is a perturbation: the exact basis below multiplies the forward A by ~3/Or
+        // (the x^5, x^6 rows), which loses Om/Or digits.  Instead J'_p = int x^p dx/E^3, p <= 4, come from the basis and
+        // J'_5.. follow from d(x^k / E) = N_k / E^3:  Om (k - 3/2) J'_{k+2} = [x^k/E] - k OL J'_{k-1} - (k-1) Ok J'_{k+1}
+        // - (k-2) Or J'_{k+3}, the Or terms iterated (same scheme as the forward d_abs).
+        constexpr int KJ = 12;                // levels k = 3 .. 3 + KJ - 1
+        T Jp[17], Sp[7];
+#pragma unroll
+        for (int p = 0; p < 5; ++p) {
             Jp[p] = C.GJ[p][0] * R.I0 + C.GJ[p][1] * R.K + C.GJ[p][2] * bt0 + C.GJ[p][3] * bt1 + C.GJ[p][4] * bt2;
+            if (kCond) Sp[p] = N::abs_(C.GJ[p][0] * R.I0) + N::abs_(C.GJ[p][1] * R.K) + N::abs_(C.GJ[p][2] * bt0) + N::abs_(C.GJ[p][3] * bt1)
+                               + N::abs_(C.GJ[p][4] * bt2);
+        }
 #pragma unroll
         for (int p = 5; p < 17; ++p) Jp[p] = T(0);
         T bk[KJ];
         {
-            T xk = x * x * x;
+            T dk = n3;             // x^k - 1 = x (x^(k-1) - 1) + z, from x^3 - 1: no cancellation at small z
 #pragma unroll
-            for (int j = 0; j < KJ; ++j) { bk[j] = N::fma_(xk - T(1), iE, bt0); xk *= x; }     // x^k/E - 1 = (x^k - 1)/E + (1/E - 1)
+            for (int j = 0; j < KJ; ++j) { bk[j] = N::fma_(dk, iE, bt0); dk = N::fma_(x, dk, z); }     // x^k/E - 1 = (x^k - 1)/E + (1/E - 1)
         }
         T prev5 = T(0), prev6 = T(0);
 #pragma unroll
@@ -233,30 +252,129 @@ CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, c
             }
         }
         const T tol = T(sizeof(T) == 8 ? 1e-12 : 1e-5);
-        useJ = N::abs_(Jp[5] - prev5) <= tol * N::abs_(Jp[5]) && N::abs_(Jp[6] - prev6) <= tol * N::abs_(Jp[6]);
+        const bool useJ = N::abs_(Jp[5] - prev5) <= tol * N::abs_(Jp[5]) && N::abs_(Jp[6] - prev6) <= tol * N::abs_(Jp[6]);
+        if (kCond) {      // error bounds of J'_5, J'_6 through the first two levels of the recursion (the Or terms are small where it is used)
+            Sp[5] = (N::abs_(bk[0]) + T(3) * C.OL * Sp[2] + T(2) * N::abs_(C.Ok) * Sp[4]) * C.iOm * T(1.0 / 1.5);
+            Sp[6] = (N::abs_(bk[1]) + T(4) * C.OL * Sp[3] + T(3) * N::abs_(C.Ok) * Sp[5]) * C.iOm * T(1.0 / 2.5);
+        }
+#pragma unroll
+        for (int t = 0; t < 3; ++t) {
+            const int a = t == 0 ? 5 : (t == 1 ? 2 : 6);      // x^2 D_theta = x^5, x^2, x^6 minus x^4
+            T dA = C.GA[t][0] * R.I0 + C.GA[t][1] * R.K + C.GA[t][2] * bt0 + C.GA[t][3] * bt1 + C.GA[t][4] * bt2 + C.GA[t][5] * btA
+                   + C.GA[t][6] * R.AA;
+            T sa = T(0);
+            if (kCond) sa = N::abs_(C.GA[t][0] * R.I0) + N::abs_(C.GA[t][1] * R.K) + N::abs_(C.GA[t][2] * bt0) + N::abs_(C.GA[t][3] * bt1)
+                            + N::abs_(C.GA[t][4] * bt2) + N::abs_(C.GA[t][5] * btA) + N::abs_(C.GA[t][6] * R.AA);
+            if (useJ) { dA = Jp[a] - Jp[4]; if (kCond) sa = Sp[a] + Sp[4]; }
+            D.dA[t] = dA;
+            if (kCond) {
+                const T c = sa / N::max_(N::abs_(dA), T(1e-3) * N::abs_(R.AA));
+                cmax = (c > cmax || !(c == c)) ? c : cmax;
+            }
+        }
+    }
+    if (kCond) *cond = cmax;
+}
+
+// The same nine integrals by Gauss-Legendre quadrature of their definition (Leibniz' rule on eqs. (2.3)-(2.5), the
+// route PAPER.md:285 fn.23 names), for the elements where grad_basis() is ill-conditioned: E^2 has (nearly) repeated roots away
+// from the path, or z is tiny.  There the integrand is smooth on the path, so a 12-point rule on panels that grow geometrically (ratio
+// <= 2) in the distance x - c from the root pair's centre c (0 when the pair is not left of the path) converges to rounding
+// (measured against the oracle on every element of config 5 with cond > 1e3: <= 4e-14).  E^2 is evaluated as printed,
+// eq. (2.2), so every root structure -- Einstein-de Sitter's triple root included -- takes the same code.  FP64 in every variant;
+// never inlined (rare path).  Returns 0, or ST_GRAD_ILLCOND when the pair's centre lies on the path (peaked integrand: not served).
+CB_HD_NOINLINE unsigned grad_quad(double Om, double OL, double Or, double x0, double z1, double dz, bool wantT, bool wantA, double out[9]) {
+    // nodes xi_i, 1 - xi_i on (0, 1) and weights of the 12-point Gauss-Legendre rule
+    const double XI[6] = {0.0092196828766403746547, 0.047941371814762571661, 0.11504866290284765648, 0.20634102285669127635,
+                          0.31608425050090990312, 0.43738329574426554226};
+    const double WI[6] = {0.023587668193255913597, 0.05346966299765921548, 0.080039164271673113167, 0.10158371336153296087,
+                          0.11674626826917740438, 0.1245735229067013925};
+    for (int i = 0; i < 9; ++i) out[i] = 0.0;
+    const double Ok = 1.0 - Om - OL - Or, X1 = 1.0 + z1, X2 = X1 + dz;
+    const double lo = fmin(X1, X2), hi = fmax(X1, X2);
+    unsigned st = (x0 >= lo && x0 <= hi) ? (unsigned)ST_GRAD_ILLCOND : 0u;
+    const double c = (x0 > 0.0 && x0 < lo) ? x0 : 0.0;
+    if (!(lo > 0.0) || dz == 0.0) return st;
+    const double lr = log((X2 - c) / (X1 - c));
+    int np = (int)ceil(fabs(lr) * 1.4426950408889634);       // panels of ratio <= 2
+    if (np < 1) np = 1;
+    if (np > 64) np = 64;
+    const double r = exp(lr / np);
+    double wd = (np == 1) ? dz : dz * (r - 1.0) / (exp(lr) - 1.0);    // widths sum to dz; one panel: dz itself
+    double tlo = z1;                                                   // x - 1 at the panel's lower end
+    for (int k = 0; k < np; ++k) {
+        for (int i = 0; i < 12; ++i) {
+            const double xi = i < 6 ? XI[i] : 1.0 - XI[11 - i], w = (i < 6 ? WI[i] : WI[11 - i]) * wd;
+            const double t = fma(wd, xi, tlo), x = 1.0 + t;       // t = x - 1 is formed directly: D_theta has the factor (x - 1)
+            const double e2 = fma(fma(fma(Or, x, Om), x, Ok), x * x, OL);
+            const double ie = 1.0 / sqrt(e2), f = w * ie * ie * ie * t;
+            const double x2 = x * x, xp1 = x + 1.0;
+            const double dm = f * x2, dl = -f * xp1, dr = dm * xp1;       // w D_theta / E^3
+            out[0] += dm; out[1] += dl; out[2] += dr;
+            if (wantT) { const double ix = 1.0 / x; out[3] += dm * ix; out[4] += dl * ix; out[5] += dr * ix; }
+            if (wantA) { out[6] += dm * x2; out[7] += dl * x2; out[8] += dr * x2; }
+        }
+        tlo += wd;
+        wd *= r;
+    }
+    return st;
+}
+
+// Above this cancellation factor the gradient integrals are taken from grad_quad() instead of grad_basis() (FP64: basis error
+// ~ 2e-16 x 1e6; measured on config 5: basis <= 4e-10 below it, quadrature <= 4e-14 above it)
+template <typename T>
+CB_HD unsigned grad_robust_fix(const Cosmo<T>& C, T z, bool wantT, bool wantA, T cond, GradInt<T>& D) {
+    const T limit = T(sizeof(T) == 8 ? GRAD_COND_LIMIT : GRAD_COND_LIMIT_F32);
+    if (cond <= limit && !(C.cubic & 4u)) return 0u;
+    double q[9];
+    const unsigned st = grad_quad((double)C.Om, (double)C.OL, (double)C.Or, -0.5 * (double)C.b, 0.0, (double)z, wantT, wantA, q);
+#pragma unroll
+    for (int t = 0; t < 3; ++t) { D.dI[t] = (T)q[t]; D.dT[t] = (T)q[3 + t]; D.dA[t] = (T)q[6 + t]; }
+    return st;
+}
+
+// ---- S8, second half.  VJP of one element: g[N_PLANES] upstream (entries outside `which` must be 0); D = its gradient integrals.
+// Adds to gz and gp[0..3] = (Om, OL, Or, H0).
+// `which`: planes that can carry a non-zero upstream gradient; where the caller knows it at compile time the terms of the
+// other planes fold away (x * 0 is not foldable in IEEE arithmetic, so a zero g alone does not remove them).
+template <typename T, bool kT, bool kA>
+CB_HD void backward_chain(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, const GradInt<T>& D, const T g[N_PLANES], T& gz,
+                          T gp[4], unsigned which = W_ALL) {
+    using N = Num<T>;
+    const T x = T(1) + z;
+    const T iE = R.iE;
+    T ix, xiDL;                                            // 1/x and x/D_L = 1/D_M
+    if (which & W_MU) {                                    // one reciprocal serves 1/x and 1/D_M
+        const T rxd = N::rcp_(x * O.v[1]);
+        ix = O.v[1] * rxd;
+        xiDL = x * rxd;
+        // z = 0: D_M = 0 and mu is undefined (status 4), but the other planes' gradients are finite and must not see 0 * inf
+        if (which != W_MU && O.v[1] == T(0)) ix = N::rcp_(x);
+    } else {
+        ix = N::rcp_(x);
+        xiDL = T(0);
+    }
+    T gM = T(0);
+    if (which & W_DM) gM = g[1];
+    if (which & W_DL) gM = N::fma_(x, g[2], gM);
+    if ((which & W_MU) && g[3] != T(0)) gM = N::fma_(T(CB_KT.five_over_ln10) * g[3], xiDL, gM);
+    if ((which & W_DA) && g[6] != T(0)) gM = N::fma_(g[6], ix, gM);     // D_A = D_M / (1+z)
+    T aI = C.dH * ((which & W_DC) ? N::fma_(gM, O.Fi, g[0]) : gM * O.Fi);
+    T aK = -gM * C.dH * O.Fk;
+    if ((which & W_VC) && g[7] != T(0)) {                                                 // V_C = 4 pi dH^3 v(Ok, I0): dv = F^2 dI0 + v_k dOk
+        const T c4pi = T(12.566370614359172954) * C.dH * C.dH * C.dH * g[7];
+        aI = N::fma_(c4pi, O.F * O.F, aI);
+        aK = N::fma_(-c4pi, O.Vk, aK);
     }
     const T aIh = T(-0.5) * aI;
 #pragma unroll
     for (int t = 0; t < 3; ++t) {
-        T dI = C.GI[t][0] * R.I0 + C.GI[t][1] * R.K + C.GI[t][2] * bt0 + C.GI[t][3] * bt1 + C.GI[t][4] * bt2;
-        if (kCond) {
-            const T sa = N::abs_(C.GI[t][0] * R.I0) + N::abs_(C.GI[t][1] * R.K) + N::abs_(C.GI[t][2] * bt0) + N::abs_(C.GI[t][3] * bt1)
-                         + N::abs_(C.GI[t][4] * bt2);
-            const T c = sa / N::max_(N::abs_(dI), T(1e-3) * N::abs_(R.I0));
-            if (t == 0 || c > *cond) *cond = c;
-        }
-        T acc = N::fma_(aIh, dI, aK);
+        T acc = N::fma_(aIh, D.dI[t], aK);
         if (kT) {
-            T dT = C.GT[t][0] * R.I0 + C.GT[t][1] * R.K + C.GT[t][2] * bt0 + C.GT[t][3] * bt1 + C.GT[t][4] * bt2 + C.GT[t][5] * R.TT;
-            acc = N::fma_((g[4] - g[8]) * C.tH, T(-0.5) * dT, acc);       // t_L = tH T, age = tH (Tinf - T)
+            acc = N::fma_((g[4] - g[8]) * C.tH, T(-0.5) * D.dT[t], acc);       // t_L = tH T, age = tH (Tinf - T)
             acc = N::fma_(g[8] * C.tH, C.dTinf[t], acc);
         }
-        if (kA) {
-            T dA = C.GA[t][0] * R.I0 + C.GA[t][1] * R.K + C.GA[t][2] * bt0 + C.GA[t][3] * bt1 + C.GA[t][4] * bt2 + C.GA[t][5] * btA
-                   + C.GA[t][6] * R.AA;
-            if (useJ) dA = (t == 0 ? Jp[5] : (t == 1 ? Jp[2] : Jp[6])) - Jp[4];      // x^2 D_theta = x^5, x^2, x^6 minus x^4
-            acc = N::fma_(g[5] * C.dH, T(-0.5) * dA, acc);
-        }
+        if (kA) acc = N::fma_(g[5] * C.dH, T(-0.5) * D.dA[t], acc);
         gp[t] += acc;
     }
     T h = T(0);
@@ -276,6 +394,30 @@ CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, c
     if ((which & W_DA) && g[6] != T(0)) dz -= g[6] * O.v[6] * ix;
     if (kA) dz += g[5] * C.dH * x * x * iE;
     gz += dz;
+}
+
+// VJP of one element from the gradient bases alone (the hot OUTER loop: its cosmologies are screened by cosmo_prep, Cosmo::cubic
+// bits 2, 3); kCond as grad_basis.
+template <typename T, bool kT, bool kA, bool kCond = false>
+CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, const T g[N_PLANES], T& gz, T gp[4], T* cond = nullptr,
+                    unsigned which = W_ALL) {
+    GradInt<T> D;
+    grad_basis<T, kT, kA, kCond>(C, z, R, D, cond);
+    backward_chain<T, kT, kA>(C, z, R, O, D, g, gz, gp, which);
+}
+
+// VJP of one element with the conditioning check: bases where they are accurate, quadrature elsewhere.  Returns status bits to OR in.
+template <typename T, bool kT, bool kA>
+CB_HD unsigned backward_robust(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, const T g[N_PLANES], T& gz, T gp[4],
+                               unsigned which = W_ALL) {
+    GradInt<T> D;
+    T cond = T(0);
+    grad_basis<T, kT, kA, true>(C, z, R, D, &cond);
+    const bool valid = !(R.status & (ST_ROOT_ON_PATH | ST_UNSUPPORTED));
+    unsigned st = 0u;
+    if (valid) st = grad_robust_fix<T>(C, z, kT && (which & (W_TL | W_AGE)), kA && (which & W_DABS), cond, D);
+    backward_chain<T, kT, kA>(C, z, R, O, D, g, gz, gp, which);
+    return st;
 }
 
 }  // namespace cb

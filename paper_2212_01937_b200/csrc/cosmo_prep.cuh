@@ -56,6 +56,9 @@ CB_HD void cosmo_prep(double Om, double OL, double Or, double H0, int want_grad,
             t = fmin(t0, fmin(t1, t2));
         }
         rn = t - c2 * (1.0 / 3.0);
+        // OL = 0 exactly: x = 0 is a root (double when Or = 0) and the closed form, at its discriminant's zero, may return the
+        // simple positive root of a closed matter model instead
+        if (c0 == 0.0) rn = 0.0;
         for (int it = 0; it < 3; ++it) {
             double Cv = fma(fma(rn + c2, rn, c1), rn, c0);
             double Cp = fma(fma(3.0, rn, 2.0 * c2), rn, c1);
@@ -95,29 +98,54 @@ CB_HD void cosmo_prep(double Om, double OL, double Or, double H0, int want_grad,
         double e3 = Or * b + g1, e2 = Or * c + g1 * b + h1, e1 = g1 * c + h1 * b, e0 = h1 * c;
         double scale = fabs(Om) + fabs(Ok) + fabs(OL) + fabs(Or);
         double res = fabs(e3 - Om) + fabs(e2 - Ok) + fabs(e1) + fabs(e0 - OL);
-        if (!(res <= 1e-9 * scale) || !(m > 0.0) || !(rn <= 1e-12)) st |= ST_UNSUPPORTED;   // also catches NaN
+        if (!(res <= 1e-13 * scale) || !(m > 0.0) || !(rn <= 1e-12)) st |= ST_UNSUPPORTED;   // also catches NaN
     }
-    // --- no real negative root (two complex pairs): factor P = (Or x^2 + g1 x + h1)(x^2 + b x + c) by Bairstow from the
-    // small pair x^2 ~ -OL/Ok; such rows are evaluated by the complex slow path of cosmo_c4.cuh (C.m, C.rn carry g1, h1)
-    if ((st & ST_UNSUPPORTED) && Or > 0.0 && Om > 0.0 && OL >= 0.0 && H0 > 0.0 && Ok > 0.0 && isfinite(Ok)) {
-        double bb = 0.0, cc = OL / Ok;
-        for (int it = 0; it < 12; ++it) {
-            double q2 = Or, q1 = Om - bb * q2, q0 = Ok - bb * q1 - cc * q2;
-            double r1 = -bb * q0 - cc * q1, r0 = OL - cc * q0;
-            double s1 = q1 - bb * q2, s0 = q0 - cc * q2;
-            double u1 = s0 - bb * s1, u0 = -cc * s1;
-            double det = u1 * s0 - u0 * s1;
-            if (det == 0.0 || !isfinite(det)) break;
-            bb += (r1 * s0 - r0 * s1) / det;
-            cc += (u1 * r0 - u0 * r1) / det;
-        }
-        const double g1 = Om - bb * Or, h1 = Ok - bb * g1 - cc * Or;
-        const double e1 = g1 * cc + h1 * bb, e0 = h1 * cc;
-        const double scale = fabs(Om) + fabs(Ok) + fabs(OL) + fabs(Or);
-        if (fabs(e1) + fabs(e0 - OL) <= 1e-9 * scale && 4.0 * Or * h1 - g1 * g1 > 0.0 && 4.0 * cc - bb * bb > 0.0) {
-            st &= ~ST_UNSUPPORTED;
-            C.cubic |= 2u;
-            m = g1; rn = h1; b = bb; c = cc;
+    // --- the labelled solve failed (the two negative roots nearly coincide, or there is no real negative root at all): factor
+    // P = (Or x^2 + g1 x + h1)(x^2 + b x + c) by Bairstow.  Starts: the small pair x^2 ~ -OL/Ok (Ok > 0), the quadratic the failed solve
+    // ended with, and the pair of Or x^4 + OL = 0 with positive real part (large Or); the first that reproduces the coefficients is
+    // classified: two negative real roots in one factor -> the real labelling (m, rn from that factor); two complex pairs -> the
+    // complex slow path of cosmo_c4.cuh (C.m, C.rn carry g1, h1).
+    if ((st & ST_UNSUPPORTED) && Or > 0.0 && Om > 0.0 && OL >= 0.0 && H0 > 0.0 && isfinite(Ok) && isfinite(H0)) {
+        const double rho2 = sqrt(OL / Or);
+        const double sb[3] = {0.0, b, -sqrt(2.0 * rho2)}, sc[3] = {OL / Ok, c, rho2};
+        for (int start = (Ok > 0.0 ? 0 : 1); start < 3 && (st & ST_UNSUPPORTED); ++start) {
+            double bb = sb[start], cc = sc[start];
+            if (!isfinite(bb) || !isfinite(cc)) continue;
+            for (int it = 0; it < 24; ++it) {
+                double q2 = Or, q1 = Om - bb * q2, q0 = Ok - bb * q1 - cc * q2;
+                double r1 = -bb * q0 - cc * q1, r0 = OL - cc * q0;
+                double s1 = q1 - bb * q2, s0 = q0 - cc * q2;
+                double u1 = s0 - bb * s1, u0 = -cc * s1;
+                double det = u1 * s0 - u0 * s1;
+                if (det == 0.0 || !isfinite(det)) break;
+                bb += (r1 * s0 - r0 * s1) / det;
+                cc += (u1 * r0 - u0 * r1) / det;
+            }
+            double g1 = Om - bb * Or, h1 = Ok - bb * g1 - cc * Or;
+            const double e1 = g1 * cc + h1 * bb, e0 = h1 * cc;
+            const double scale = fabs(Om) + fabs(Ok) + fabs(OL) + fabs(Or);
+            if (!(fabs(e1) + fabs(e0 - OL) <= 1e-13 * scale)) continue;
+            double d1 = g1 * g1 - 4.0 * Or * h1, d2 = bb * bb - 4.0 * cc;
+            // a factor with two non-positive real roots becomes Q1 = (Or x + m)(x - rn)
+            if (d2 >= 0.0 && bb >= 0.0 && cc >= 0.0 && !(d1 >= 0.0 && g1 >= 0.0 && h1 >= 0.0)) {
+                const double tb = g1 / Or, tc = h1 / Or;
+                g1 = Or * bb; h1 = Or * cc; bb = tb; cc = tc;
+                d1 = g1 * g1 - 4.0 * Or * h1; d2 = bb * bb - 4.0 * cc;
+            }
+            if (d1 >= 0.0 && g1 >= 0.0 && h1 >= 0.0) {
+                const double sq = sqrt(d1);
+                m = 0.5 * (g1 + sq);
+                rn = -h1 / m;
+                b = bb; c = cc;
+                st &= ~ST_UNSUPPORTED;
+            } else if (d1 < 0.0 && d2 < 0.0) {
+                // Q1 takes the pair further to the left (the counterpart of {big, neg} on the real path: r_i of eqs. (3.8)/(3.9),
+                // PAPER.md:225 "biggest roots"), Q2 the other one
+                if (bb * Or > g1) { const double tb = g1 / Or, tc = h1 / Or; g1 = Or * bb; h1 = Or * cc; bb = tb; cc = tc; }
+                st &= ~ST_UNSUPPORTED;
+                C.cubic |= 2u;
+                m = g1; rn = h1; b = bb; c = cc;
+            }
         }
     }
     C.m = m; C.rn = rn; C.b = b; C.c = c;
@@ -205,13 +233,23 @@ CB_HD void cosmo_prep(double Om, double OL, double Or, double H0, int want_grad,
     };
     // The bases become linearly dependent as the gap g of the pair x^2 + b x + c closes (the 1/prod(r_j - r_k) of appendix A,
     // PAPER.md:320-345; OL -> 0 is the commonest way there: the pair tends to +-sqrt(-OL/Ok) and at OL = 0 the system is singular).
-    // Measured error ~ 1e-13/g^2: below g^2 = 1e-5, or with a singular system, every gradient of this
-    // cosmology carries status bit 16 (observables() ORs it in), in ELEMENTWISE and OUTER calls alike.
-    if (!(fabs(D2) >= 1e-5) || !isfinite(idet)) C.cubic |= 4u;      // (not in C.status: that would stop the duplication loop)
+    // The per-element cancellation factor (grad_basis) decides where they are still accurate; a singular system is marked here
+    // (bit 2: quadrature for every element; not in C.status: that would stop the duplication loop).
+    if (!isfinite(idet)) C.cubic |= 4u;
     // I0: D_theta = dE^2/dtheta with Ok eliminated: x^3 - x^2, 1 - x^2, x^4 - x^2
     solve5(0.0, 0.0, -1.0, 1.0, 0.0, C.GI[0]);
     solve5(1.0, 0.0, -1.0, 0.0, 0.0, C.GI[1]);
     solve5(0.0, 0.0, -1.0, 0.0, 1.0, C.GI[2]);
+    {   // screening for the OUTER kernels, which run the chi-family bases unchecked: at small z the basis values are ~ (1, kf, E'(1),
+        // 1 - E'(1), 2 - E'(1)) x I0 and the result is compared with >= 1e-3 I0, so 1e3 sum_j |G_j| w_j bounds the cancellation factor
+        // there (it falls with z).  Above the limit the cosmology takes the checked row (bit 3).
+        double gmax = 0.0;
+        for (int t = 0; t < 3; ++t) {
+            const double g = fabs(C.GI[t][0]) + fabs(C.GI[t][1]) * fabs(C.kf) + 2.0 * (fabs(C.GI[t][2]) + fabs(C.GI[t][3]) + fabs(C.GI[t][4]));
+            gmax = (g > gmax || !(g == g)) ? g : gmax;
+        }
+        if (!(1.0e3 * gmax <= GRAD_COND_LIMIT)) C.cubic |= 8u | (isfinite(gmax) ? 0u : 4u);
+    }
     // T: D_theta / x - aT E^2 / x with aT = D_theta(0)/OL (the 1/x pole goes to the forward T): x^2 - x, 1/x - x, x^3 - x
     const double aT = 1.0 / OL;
     solve5(0.0, -1.0, 1.0, 0.0, 0.0, C.GT[0]);

@@ -80,8 +80,8 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
             double u[KS + 4], bk[KS + 1];
             u[0] = I0;
             u[1] = fma(2.0 * dz, B0, C.rn * I0);
-            double xk1 = 1.0, xk2 = 1.0;
-            for (int j = 0; j <= KS; ++j) { bk[j] = fma(xk2 - xk1, E2, xk1 * dE); xk1 *= x1; xk2 *= x2; }    // x2^j E2 - x1^j E1
+            double xk1 = 1.0, dk = 0.0;      // dk = x2^j - x1^j = x2 (x2^(j-1) - x1^(j-1)) + x1^(j-1) dz: no cancellation as z2 -> z1
+            for (int j = 0; j <= KS; ++j) { bk[j] = fma(dk, E2, xk1 * dE); dk = fma(x2, dk, xk1 * dz); xk1 *= x1; }    // x2^j E2 - x1^j E1
             for (int j = 2; j < KS + 4; ++j) u[j] = 0.0;
             double prev = 0.0;
             for (int sw = 0; sw < KS; ++sw) {
@@ -102,7 +102,7 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
     double F, Fi, Fk;
     sinn<double>(C.Ok, I0, F, Fi, Fk);
     O.v[0] = C.dH * I0; O.v[1] = C.dH * F; O.v[2] = C.tH * TT; O.v[3] = C.dH * AA; O.v[4] = O.v[1] / x2;
-    O.status = st[0] | (with_grad ? (C.cubic & 4u) << 2 : 0u);
+    O.status = st[0];
     if (st[0] & (ST_ROOT_ON_PATH | ST_UNSUPPORTED)) {
         for (int i = 0; i < 5; ++i) O.v[i] = NAN;
     }
@@ -111,15 +111,23 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
     const double iE1 = 1.0 / E1, iE2 = 1.0 / E2, diE = -dE * iE1 * iE2;            // 1/E2 - 1/E1
     double btv[16];
     {
-        double xk1 = 1.0, xk2 = 1.0;
-        for (int k = 0; k < 16; ++k) { btv[k] = fma(xk2 - xk1, iE2, xk1 * diE); xk1 *= x1; xk2 *= x2; }
+        double xk1 = 1.0, dk = 0.0;
+        for (int k = 0; k < 16; ++k) { btv[k] = fma(dk, iE2, xk1 * diE); dk = fma(x2, dk, xk1 * dz); xk1 *= x1; }
     }
-    double dI[3], dT[3], dA[3];
-    double Jp[17];
+    // raw gradient integrals int D_theta p_X / E^3 dx between the limits (cosmo_obs.cuh, GradInt) with their cancellation factor
+    double rI[3], rT[3], rA[3], cond = 0.0;
+    auto worse = [&](double sa, double val, double fwd) {
+        const double c = sa / fmax(fabs(val), 1e-3 * fabs(fwd));
+        if (c > cond || !(c == c)) cond = c;
+    };
+    double Jp[17], Sp[7];
     bool useJ = false;
     {
         constexpr int KJ = 12;
-        for (int p = 0; p < 5; ++p) Jp[p] = C.GJ[p][0] * I0 + C.GJ[p][1] * K + C.GJ[p][2] * btv[0] + C.GJ[p][3] * btv[1] + C.GJ[p][4] * btv[2];
+        for (int p = 0; p < 5; ++p) {
+            Jp[p] = C.GJ[p][0] * I0 + C.GJ[p][1] * K + C.GJ[p][2] * btv[0] + C.GJ[p][3] * btv[1] + C.GJ[p][4] * btv[2];
+            Sp[p] = fabs(C.GJ[p][0] * I0) + fabs(C.GJ[p][1] * K) + fabs(C.GJ[p][2] * btv[0]) + fabs(C.GJ[p][3] * btv[1]) + fabs(C.GJ[p][4] * btv[2]);
+        }
         for (int p = 5; p < 17; ++p) Jp[p] = 0.0;
         double prev5 = 0.0, prev6 = 0.0;
         for (int sw = 0; sw < KJ - 1; ++sw) {
@@ -131,19 +139,38 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
             }
         }
         useJ = fabs(Jp[5] - prev5) <= 1e-12 * fabs(Jp[5]) && fabs(Jp[6] - prev6) <= 1e-12 * fabs(Jp[6]);
+        Sp[5] = (fabs(btv[3]) + 3.0 * C.OL * Sp[2] + 2.0 * fabs(C.Ok) * Sp[4]) * C.iOm / 1.5;
+        Sp[6] = (fabs(btv[4]) + 4.0 * C.OL * Sp[3] + 3.0 * fabs(C.Ok) * Sp[5]) * C.iOm / 2.5;
     }
     const double btA = (C.cubic & 1u) ? btv[4] : btv[3];
     for (int t = 0; t < 3; ++t) {
-        dI[t] = -0.5 * (C.GI[t][0] * I0 + C.GI[t][1] * K + C.GI[t][2] * btv[0] + C.GI[t][3] * btv[1] + C.GI[t][4] * btv[2]);
-        dT[t] = -0.5 * (C.GT[t][0] * I0 + C.GT[t][1] * K + C.GT[t][2] * btv[0] + C.GT[t][3] * btv[1] + C.GT[t][4] * btv[2] + C.GT[t][5] * TT);
+        rI[t] = C.GI[t][0] * I0 + C.GI[t][1] * K + C.GI[t][2] * btv[0] + C.GI[t][3] * btv[1] + C.GI[t][4] * btv[2];
+        worse(fabs(C.GI[t][0] * I0) + fabs(C.GI[t][1] * K) + fabs(C.GI[t][2] * btv[0]) + fabs(C.GI[t][3] * btv[1]) + fabs(C.GI[t][4] * btv[2]),
+              rI[t], I0);
+        rT[t] = C.GT[t][0] * I0 + C.GT[t][1] * K + C.GT[t][2] * btv[0] + C.GT[t][3] * btv[1] + C.GT[t][4] * btv[2] + C.GT[t][5] * TT;
+        worse(fabs(C.GT[t][0] * I0) + fabs(C.GT[t][1] * K) + fabs(C.GT[t][2] * btv[0]) + fabs(C.GT[t][3] * btv[1]) + fabs(C.GT[t][4] * btv[2])
+              + fabs(C.GT[t][5] * TT), rT[t], TT);
+        const int ia = t == 0 ? 5 : (t == 1 ? 2 : 6);
         double a = C.GA[t][0] * I0 + C.GA[t][1] * K + C.GA[t][2] * btv[0] + C.GA[t][3] * btv[1] + C.GA[t][4] * btv[2] + C.GA[t][5] * btA
                    + C.GA[t][6] * AA;
-        if (useJ) a = (t == 0 ? Jp[5] : (t == 1 ? Jp[2] : Jp[6])) - Jp[4];
-        dA[t] = -0.5 * a;
-        O.gp[0][t] = C.dH * dI[t];
-        O.gp[1][t] = C.dH * (Fi * dI[t] - Fk);
-        O.gp[2][t] = C.tH * dT[t];
-        O.gp[3][t] = C.dH * dA[t];
+        double sa = fabs(C.GA[t][0] * I0) + fabs(C.GA[t][1] * K) + fabs(C.GA[t][2] * btv[0]) + fabs(C.GA[t][3] * btv[1]) + fabs(C.GA[t][4] * btv[2])
+                    + fabs(C.GA[t][5] * btA) + fabs(C.GA[t][6] * AA);
+        if (useJ) { a = Jp[ia] - Jp[4]; sa = Sp[ia] + Sp[4]; }
+        rA[t] = a;
+        worse(sa, a, AA);
+    }
+    // ill-conditioned bases (near-repeated roots away from the path, tiny ranges): quadrature of the same integrals (grad_quad)
+    if ((!(cond <= GRAD_COND_LIMIT) || (C.cubic & 4u)) && !(st[0] & (ST_ROOT_ON_PATH | ST_UNSUPPORTED))) {
+        double q[9];
+        O.status |= grad_quad(C.Om, C.OL, C.Or, -0.5 * C.b, z1, dz, true, true, q);
+        for (int t = 0; t < 3; ++t) { rI[t] = q[t]; rT[t] = q[3 + t]; rA[t] = q[6 + t]; }
+    }
+    for (int t = 0; t < 3; ++t) {
+        const double dI = -0.5 * rI[t], dT = -0.5 * rT[t], dA = -0.5 * rA[t];
+        O.gp[0][t] = C.dH * dI;
+        O.gp[1][t] = C.dH * (Fi * dI - Fk);
+        O.gp[2][t] = C.tH * dT;
+        O.gp[3][t] = C.dH * dA;
         O.gp[4][t] = O.gp[1][t] / x2;
     }
     const double iH0 = C.dH * (1.0 / C_KM_S);

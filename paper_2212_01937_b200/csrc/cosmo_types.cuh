@@ -62,9 +62,10 @@ enum : unsigned { W_DC = 1, W_DM = 2, W_DL = 4, W_MU = 8, W_TL = 16, W_DABS = 32
 constexpr int N_PLANES = 9;                        // number of `which` bits
 // status bits (include/cosmo_b200.h)
 enum : unsigned { ST_ROOT_ON_PATH = 1, ST_UNSUPPORTED = 2, ST_DL_NONPOS = 4, ST_ITER_CAP = 8, ST_GRAD_ILLCOND = 16 };
-// cancellation factor of the chi-family gradient above which 1e-8 is no longer guaranteed (calibrated against the oracle
-// on config 5: < 1e7 -> max error 4e-9)
-constexpr double GRAD_COND_LIMIT = 3.0e6;
+// cancellation factor of the gradient bases (cosmo_obs.cuh, grad_basis) above which an element's gradient integrals are taken from
+// quadrature instead (grad_quad).  FP64: basis error ~ 2e-16 x cond (measured on config 5: <= 4e-10 below 1e6).
+constexpr double GRAD_COND_LIMIT = 1.0e6;
+constexpr double GRAD_COND_LIMIT_F32 = 30.0;
 
 constexpr int NIT_CAP = 14;   // duplication steps never exceed this (status bit 8 when hit)
 
@@ -95,7 +96,9 @@ struct Cosmo {
     T GJ[5][5];        // J'_p = int x^p dx / E^3, p = 0..4, over the basis (I0, K, b0, b1, b2)  (d_abs gradient)
     unsigned status;
     unsigned cubic;    // bit 0: Or == 0 (cubic case, appendix B.1);  bit 1: two complex pairs (cosmo_c4.cuh; m, rn hold g1, h1);
-                       // bit 2: gradient bases ill-conditioned (reported as status bit 16)
+                       // bit 2: gradient bases unusable (a root pair's gap has closed, e.g. OL = 0): quadrature for every element;
+                       // bit 3: bases large enough that some redshift may exceed GRAD_COND_LIMIT: the OUTER kernels take the
+                       //        checked row for this cosmology (the ELEMENTWISE kernels check every element anyway)
 };
 
 constexpr int COSMO_NFIELDS = 115;   // floating-point members of Cosmo<T>, in declaration order

@@ -265,27 +265,59 @@ def test_host_math_fp32(hc):
         assert (np.abs(out[i] - val[:, i]) / np.abs(val[:, i])).max() <= 2e-5, i
 
 
-def test_vanishing_lambda_flags_gradients(hc):
-    """OL -> 0 closes the gap of the pair (+-sqrt(-OL/Ok)): values stay exact, the gradient bases degenerate (singular at
-    OL = 0), and every such cosmology carries status bit 16 instead of silently losing digits"""
+def test_vanishing_lambda_gradients(hc):
+    """OL -> 0 closes the gap of the pair (+-sqrt(-OL/Ok)) and the gradient bases degenerate (singular at OL = 0, the 1/prod(r_j - r_k)
+    of PAPER.md:320-345): such elements take the quadrature of the Leibniz integrals instead (cosmo_obs.cuh, grad_quad; PAPER.md:145
+    "limits have to be explicitly implemented when arguments are repeated").  Every gradient of every plane meets the tolerance and
+    nothing is flagged -- Einstein-de Sitter (a triple root), open and closed matter models included."""
     rng = np.random.default_rng(3)
     n = 120
-    z = rng.uniform(0.01, 5, n); Om = rng.uniform(0.1, 0.6, n); H0 = np.full(n, 70.0)
-    for OLv, flagged in ((0.0, True), (1e-9, True), (1e-3, False)):
-        for Orv in (0.0, 9e-5):
-            OL = np.full(n, OLv); Or = np.full(n, Orv)
-            g1 = np.zeros((6, n)); g1[0] = 1
+    z = rng.uniform(0.01, 5, n); H0 = np.full(n, 70.0)
+    cases = [(rng.uniform(0.1, 1.6, n), np.full(n, OLv), np.full(n, Orv)) for OLv in (0.0, 1e-12, 1e-9, 1e-6, 1e-3) for Orv in (0.0, 9e-5)]
+    cases.append((np.ones(n), np.zeros(n), np.zeros(n)))                                   # Einstein-de Sitter
+    eps = 10.0 ** rng.uniform(-12, -2, n)
+    cases.append((1.0 - eps, eps, np.zeros(n)))                                            # flat, OL -> 0: three roots close in on x = 0
+    for Om, OL, Or in cases:
+        val, grad, _ = oracle.observables_batch(z, Om, OL, Or, H0, with_grad=True)
+        val, grad = val.astype(np.float64), grad.astype(np.float64)
+        for pl in (0, 1, 3, 4, 5):
+            g1 = np.zeros((6, n)); g1[pl] = 1
             out, gz, gp, st = run(hc, z, Om, OL, Or, H0, 63, g1)
-            val, grad, _ = oracle.observables_batch(z, Om, OL, Or, H0, with_grad=True)
-            val, grad = val.astype(np.float64), grad.astype(np.float64)
-            assert (((st & 16) != 0) == flagged).all() and ((st & 15) == 0).all(), (OLv, Orv)
-            for i in range(6):
-                assert (np.abs(out[i] - val[:, i]) <= 1e-11 * np.abs(val[:, i])).all(), (OLv, Orv, i)
-            assert (np.abs(gz - grad[:, 0, 0]) <= 1e-12 * np.abs(grad[:, 0, 0])).all()            # d/dz is closed-form: always fine
-            if not flagged:
-                for p in range(3):
-                    e = np.abs(gp[p] - grad[:, 0, 1 + p]) / np.maximum(np.abs(grad[:, 0, 1 + p]), 1e-3 * np.abs(val[:, 0]))
-                    assert e.max() <= 1e-8, (OLv, Orv, p, e.max())
+            assert (st == 0).all(), (OL[0], Or[0], pl)
+            assert (np.abs(out[pl] - val[:, pl]) <= 1e-11 * np.abs(val[:, pl])).all(), (OL[0], Or[0], pl)
+            mine = np.vstack([gz[None], gp])
+            for p in range(5):
+                e = np.abs(mine[p] - grad[:, pl, p]) / np.maximum(np.abs(grad[:, pl, p]), 1e-3 * np.abs(val[:, pl]))
+                assert e.max() <= 1e-8, (OL[0], Or[0], pl, p, e.max())
+    # closed forms at Einstein-de Sitter (E^2 = x^3): I0 = 2 (1 - x^-1/2), dI0/dOm = -1/2 int (x^3 - x^2) x^-9/2 dx = -(1/x - 1) - (x^-3/2 - 1)/3 ... by hand:
+    zz = np.array([0.5, 2.0]); x = 1 + zz
+    g1 = np.zeros((6, 2)); g1[0] = 1
+    _, _, gp, st = run(hc, zz, 1.0, 0.0, 0.0, 70.0, 63, g1)
+    dH = 299792.458 / 70.0
+    F = lambda p: (x ** (p - 3.5) - 1) / (p - 3.5)                     # int_1^x t^p t^-9/2 dt
+    ref = [-0.5 * dH * (F(3) - F(2)), -0.5 * dH * (F(0) - F(2)), -0.5 * dH * (F(4) - F(2))]
+    for p in range(3):
+        assert np.allclose(gp[p], ref[p], rtol=1e-12, atol=0), p
+
+
+def test_gradient_at_z_zero(hc):
+    """z = 0: every integral vanishes, D_M = 0 and mu is undefined (status 4), but d/dz of the other planes is the integrand at z = 0
+    (d t_L/dz = t_H, d D_C/dz = d_H, E(0) = 1) and their parameter gradients are exactly zero -- no 0 x inf"""
+    z = np.array([0.0, 0.0]); Om = np.array([0.3, 0.25]); OL = np.array([0.7, 0.6]); Or = np.array([0.0, 9e-5]); H0 = np.array([70.0, 67.0])
+    dH, tH = 299792.458 / H0, 977.7922216807891 / H0
+    expect = {0: dH, 1: dH, 2: dH, 4: tH, 5: dH, 6: dH, 8: -tH}        # D_L = (1+z) D_M, D_A = D_M/(1+z): slope d_H at z = 0
+    for pl, dz_ref in expect.items():
+        g1 = np.zeros((9, 2)); g1[pl] = 1
+        out, gz, gp, st = run(hc, z, Om, OL, Or, H0, 511 & ~8, g1)
+        assert np.isfinite(gz).all() and np.isfinite(gp).all(), pl
+        assert np.allclose(gz, dz_ref, rtol=1e-14), (pl, gz, dz_ref)
+        if pl != 8:
+            assert (gp[:3] == 0).all() and (out[pl] == 0).all(), pl
+    # with the mu plane selected but no upstream gradient on it the others stay finite
+    g1 = np.zeros((9, 2)); g1[0] = 1; g1[4] = 1
+    out, gz, gp, st = run(hc, z, Om, OL, Or, H0, 511, g1)
+    assert np.isfinite(gz).all() and np.isfinite(gp).all() and ((st & 4) != 0).all()
+    assert np.allclose(gz, dH + tH, rtol=1e-14)
 
 
 def test_invalid_rows_status(hc):
