@@ -16,7 +16,9 @@
  * Units: H0 in km/s/Mpc; distances in Mpc (c = 299792.458 km/s); t_L in Gyr (1/H0 = 977.7922216807891/H0 Gyr); mu in mag.
  *
  * Conventions for every call:
- *   - every pointer is a DEVICE pointer owned by the caller unless marked "host"; the library allocates nothing;
+ *   - every pointer is a DEVICE pointer owned by the caller unless marked "host"; the device-pointer calls allocate nothing
+ *     (scratch comes in through `workspace`); only cosmo_eval_host, which takes host pointers, keeps device staging buffers of
+ *     its own (released by cosmo_host_release);
  *   - the call only enqueues kernels on `stream` (a cudaStream_t passed as void*; NULL = legacy default stream),
  *     it never synchronises; results are valid after the stream reaches the end of the enqueued work;
  *   - return value 0 = enqueued; negative = COSMO_E_* below, nothing was launched (argument errors) or the CUDA
@@ -27,9 +29,11 @@
  *          factorised (the method needs E^2 of degree 3 or 4)
  *       4  D_L <= 0 (closed universe at/after the antipode): mu is NaN, the other outputs are valid
  *       8  the duplication loop hit its iteration cap before Carlson's stopping rule was met
- *      16  gradient ill-conditioned (near-degenerate roots; the 1/prod(r_j - r_k) of PAPER.md:320-345): values valid, gradients
- *          may have lost more than the documented accuracy or be NaN (set by the VJP calls: per cosmology when the root pair's
- *          gap has closed, e.g. OL -> 0, in every mode; plus a per-element conditioning estimate in ELEMENTWISE calls)
+ *      16  a parameter gradient of this element is not served to the documented accuracy (set by the VJP calls; values valid).
+ *          Where roots of E^2 (nearly) coincide the closed-form gradient bases cancel -- the 1/prod(r_j - r_k) of PAPER.md:320-345 --
+ *          and the element's gradient integrals are taken from Gauss-Legendre quadrature of their definition instead (also at
+ *          OL = 0: Einstein-de Sitter, open and closed matter models), so this bit is left for: a near-repeated pair whose centre
+ *          lies ON the path while the bases cancel, and the gradient of the age plane when the bases are singular (OL = 0).
  */
 #ifndef COSMO_B200_H
 #define COSMO_B200_H
@@ -131,30 +135,9 @@ int cosmo_eval_w(const double* z, int64_t n, const double* Om, const double* OL,
                  const double* Ow23, const double* H0, int64_t n_cosmo, uint32_t which, double* out, double* dout_dz, uint8_t* status,
                  void* stream);
 
-/* The device Carlson functions of the hot path on their own (eqs. (2.6), (2.7), (2.9); duplication
- * algorithm of ref. [10]), in the real-symmetric form the path uses: for each i
- *   rf[i] = R_F(x, m+h, m-h),  rd[i] = R_D(m+h, m-h, x),  rj[i] = R_J(x, m+h, m-h, p),   h^2 = s[i]
- * with x > 0, p > 0 and either s >= 0 with m - h > 0 (three positive reals) or s < 0 (a complex-conjugate pair m +- i|h|).
- * All arrays have length n (device pointers). */
-int cosmo_carlson_pair(const double* x, const double* m, const double* s, const double* p, int64_t n, double* rf, double* rd,
-                       double* rj, void* stream);
+/* frees the device staging buffers cosmo_eval_host keeps between calls (no-op if there are none) */
+void cosmo_host_release(void);
 
-/* ALU roofline probes: each thread runs `iters` rounds of 8 independent dependent-FMA chains (FP64 / FP32) and
- * stores one value per thread in sink[blocks*256].  flops = blocks * 256 * iters * 8 * 2.  Used by bench.py to
- * measure the DFMA / FFMA peak that the roofline fraction is quoted against. */
-int cosmo_probe_fma_f64(int blocks, int iters, double* sink, void* stream);
-int cosmo_probe_fma_f32(int blocks, int iters, float* sink, void* stream);
-
-/* Optional timing of the DOMINANT kernel of each call (the OUTER / ELEMENTWISE evaluation kernel, not prep/reduce) with
- * CUDA events recorded on the launching stream.  cosmo_profile(1) starts (and resets) the statistics, cosmo_profile(0)
- * stops; cosmo_profile_mean_ms synchronises on the last recorded launch and returns the mean duration in ms over the
- * launches since the reset (count in *n_launches, nullable).  When on, each call first waits for the previous call's
- * kernel to finish (host side), so leave it off outside measurements.  Not thread-safe. */
-int cosmo_profile(int on);
-double cosmo_profile_mean_ms(int64_t* n_launches);
-
-/* number of kernels the library has launched in this process (all entry points) */
-int64_t cosmo_launch_count(void);
 int cosmo_last_cuda_error(void);
 const char* cosmo_strerror(int code);
 const char* cosmo_version(void);

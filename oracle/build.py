@@ -1,7 +1,7 @@
-"""Builds oracle/liboracle.so from oracle/cosmo_oracle.c with gcc.  TEST INFRASTRUCTURE (see README.md here).
+"""Builds oracle/liboracle.so from oracle/cosmo_oracle.c with gcc.  TEST INFRASTRUCTURE (see the header of cosmo_oracle.c).
 
 Plain `gcc -O2 -fopenmp`, no -ffast-math (long-double arithmetic must stay as written).
-Called by __graft_entry__.build(), by tests/conftest.py and by bench.py's cpu_baseline leg.
+Called by __graft_entry__.build() and, on first use, by oracle/__init__.py (tests, smoke(), bench.py's oracle legs).
 """
 import os
 import subprocess

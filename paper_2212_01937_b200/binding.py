@@ -17,8 +17,8 @@ DC, DM, DL, MU, TL, DABS, DA, VC, AGE = 1, 2, 4, 8, 16, 32, 64, 128, 256
 WHICH_BITS = {"DC": DC, "DM": DM, "DL": DL, "MU": MU, "TL": TL, "DABS": DABS, "DA": DA, "VC": VC, "AGE": AGE}
 WHICH_ORDER = ("DC", "DM", "DL", "MU", "TL", "DABS", "DA", "VC", "AGE")
 
-# every symbol include/cosmo_b200.h declares
-SYMBOLS = ("cosmo_workspace_bytes", "cosmo_eval", "cosmo_vjp", "cosmo_snia_loglike", "cosmo_eval_f32", "cosmo_vjp_f32",
+# every symbol include/cosmo_b200.h and include/cosmo_b200_diag.h declare
+SYMBOLS = ("cosmo_host_release", "cosmo_workspace_bytes", "cosmo_eval", "cosmo_vjp", "cosmo_snia_loglike", "cosmo_eval_f32", "cosmo_vjp_f32",
            "cosmo_snia_loglike_f32", "cosmo_snia_logjoint", "cosmo_eval2", "cosmo_eval_w", "cosmo_eval_host", "cosmo_carlson_pair", "cosmo_probe_fma_f64", "cosmo_probe_fma_f32",
            "cosmo_profile", "cosmo_profile_mean_ms",
            "cosmo_launch_count", "cosmo_last_cuda_error", "cosmo_strerror", "cosmo_version")

@@ -1,21 +1,24 @@
 """Builds paper_2212_01937_b200/libcosmo_b200.so (hand-written CUDA for sm_100a, C ABI of include/cosmo_b200.h).
 
-nvcc cross-compiles without a GPU; the built .so stays in-tree (git-ignored) and travels to the GPU box.
-Run:  python -m paper_2212_01937_b200.build [--force]
+nvcc cross-compiles without a GPU; the built .so stays in-tree (git-ignored) and travels to the GPU box.  Each kernel family is its own
+translation unit (csrc/tu_*.cu) so that they compile in parallel; objects go to csrc/build/ (git-ignored).
+Run:  python -m paper_2212_01937_b200.build [--force] [-v]
 """
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libcosmo_b200.so")
-SOURCES = [os.path.join(CSRC, "cosmo_b200.cu")]
-DEPS = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC))] + [os.path.join(ROOT, "include", "cosmo_b200.h")]
+OBJ = os.path.join(CSRC, "build")
+SOURCES = sorted(f for f in os.listdir(CSRC) if f.endswith(".cu"))
+HEADERS = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith(".cuh")] + \
+          [os.path.join(ROOT, "include", f) for f in sorted(os.listdir(os.path.join(ROOT, "include")))]
 
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared"]
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
 
 
 def nvcc():
@@ -26,10 +29,30 @@ def nvcc():
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= max(os.path.getmtime(d) for d in DEPS):
+    os.makedirs(OBJ, exist_ok=True)
+    hdr_time = max(os.path.getmtime(h) for h in HEADERS)
+    todo, objs = [], []
+    for src in SOURCES:
+        o = os.path.join(OBJ, src[:-3] + ".o")
+        objs.append(o)
+        if force or not os.path.exists(o) or os.path.getmtime(o) < max(hdr_time, os.path.getmtime(os.path.join(CSRC, src))):
+            todo.append((src, o))
+    if not todo and os.path.exists(LIB) and os.path.getmtime(LIB) >= max(os.path.getmtime(o) for o in objs):
         return LIB
-    cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
-    subprocess.run(cmd, check=True, cwd=CSRC)
+
+    def compile_one(job):
+        src, o = job
+        cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", o, src]
+        r = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
+        return src, r
+
+    with ThreadPoolExecutor(max_workers=min(len(todo), os.cpu_count() or 4) or 1) as ex:
+        for src, r in ex.map(compile_one, todo):
+            if verbose or r.returncode:
+                sys.stderr.write(f"--- {src}\n{r.stdout}{r.stderr}")
+            if r.returncode:
+                raise subprocess.CalledProcessError(r.returncode, f"nvcc {src}")
+    subprocess.run([nvcc(), "-shared", "-o", LIB] + objs, check=True, cwd=CSRC)
     return LIB
 
 

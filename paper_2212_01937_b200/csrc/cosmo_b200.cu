@@ -2,7 +2,8 @@
 #include <atomic>
 #include <mutex>
 #include "../../include/cosmo_b200.h"
-#include "cosmo_kernels.cuh"
+#include "../../include/cosmo_b200_diag.h"
+#include "cosmo_launch.cuh"
 
 using namespace cb;
 
@@ -59,7 +60,11 @@ struct WsLayout { size_t consts, part, gzpart, total; int ny; int64_t ntiles; };
 WsLayout ws_layout(int64_t n_z, int64_t n_cosmo, int mode, uint32_t which, int with_grad, size_t elt) {
     WsLayout L{};
     const bool per_elem = (mode == COSMO_ELEMENTWISE && n_cosmo != 1);
-    if (per_elem) { L.total = 0; L.ny = 1; L.ntiles = 0; return L; }
+    if (per_elem) {     // VJP: the work list of the second pass (k_elem_redo): a counter and up to n_z 32-bit indices
+        L.total = with_grad ? 256 + align256((size_t)(n_z > 0 ? n_z : 1) * sizeof(unsigned)) : 0;
+        L.ny = 1; L.ntiles = 0;
+        return L;
+    }
     L.ntiles = cdiv(n_z > 0 ? n_z : 1, outer_tile(which & (W_TL | W_AGE), which & W_DABS));   // as launch_outer dispatches
     L.ny = grid_y(L.ntiles, n_cosmo);
     L.consts = 0;
@@ -84,31 +89,24 @@ int check_common(const void* z, int64_t n_z, const cosmo_params& p, int64_t n_co
     return COSMO_OK;
 }
 
-template <typename T, int MODE>
-int launch_outer(OuterArgs& a, dim3 grid, cudaStream_t st) {
-    const bool kT = a.which & (W_TL | W_AGE), kA = a.which & W_DABS;
+template <typename T>
+int launch_outer(int mode, OuterArgs& a, dim3 grid, cudaStream_t st) {
     prof_begin(st);
-    if (MODE == MODE_SNIA || MODE == MODE_JOINT) k_outer<T, false, false, MODE, W_MU><<<grid, OUTER_THREADS, 0, st>>>(a);
-    else if (kT && kA) k_outer<T, true, true, MODE, 0><<<grid, OUTER_THREADS, 0, st>>>(a);
-    else if (kT) k_outer<T, true, false, MODE, 0><<<grid, OUTER_THREADS, 0, st>>>(a);
-    else if (kA) k_outer<T, false, true, MODE, 0><<<grid, OUTER_THREADS, 0, st>>>(a);
-    else if (a.which == W_MU) k_outer<T, false, false, MODE, W_MU><<<grid, OUTER_THREADS, 0, st>>>(a);
-    else k_outer<T, false, false, MODE, 0><<<grid, OUTER_THREADS, 0, st>>>(a);
+    if (sizeof(T) == 8) launch_outer_f64(mode, a, grid, st);
+    else launch_outer_f32(mode, a, grid, st);
     prof_end(st);
     return check_launch();
 }
 
-template <typename T, bool kG>
-int launch_elem(const T* z, const cosmo_params& p, int64_t N, unsigned which, const T* gout, T* out, T* gz, double* gparams,
-                uint8_t* status, cudaStream_t st) {
-    const bool kT = which & (W_TL | W_AGE), kA = which & W_DABS;
-    dim3 grid((unsigned)cdiv(N, ELEM_THREADS));
+template <typename T>
+int launch_elem(bool with_grad, const T* z, const cosmo_params& p, int64_t N, unsigned which, const T* gout, T* out, T* gz, double* gparams,
+                uint8_t* status, unsigned* ws, cudaStream_t st) {
+    ElemArgs a{z, p.Om, p.OL, p.Or, p.H0, N, which, gout, out, gz, gparams, status, ws, ws ? ws + 64 : nullptr};
     prof_begin(st);
-    if (kT && kA) k_elem<T, true, true, kG><<<grid, ELEM_THREADS, 0, st>>>(z, p.Om, p.OL, p.Or, p.H0, N, which, gout, out, gz, gparams, status);
-    else if (kT) k_elem<T, true, false, kG><<<grid, ELEM_THREADS, 0, st>>>(z, p.Om, p.OL, p.Or, p.H0, N, which, gout, out, gz, gparams, status);
-    else if (kA) k_elem<T, false, true, kG><<<grid, ELEM_THREADS, 0, st>>>(z, p.Om, p.OL, p.Or, p.H0, N, which, gout, out, gz, gparams, status);
-    else k_elem<T, false, false, kG><<<grid, ELEM_THREADS, 0, st>>>(z, p.Om, p.OL, p.Or, p.H0, N, which, gout, out, gz, gparams, status);
+    if (sizeof(T) == 8) launch_elem_f64(with_grad, a, st);
+    else launch_elem_f32(with_grad, a, st);
     prof_end(st);
+    if (with_grad) g_launches += 1;      // the second pass
     return check_launch();
 }
 
@@ -129,15 +127,19 @@ int run_eval(const T* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode,
     }
     const bool per_elem = (mode == COSMO_ELEMENTWISE && n_cosmo != 1);
     if (per_elem) {
-        return with_grad ? launch_elem<T, true>(z, p, n_z, which, gout, out, gz, gparams, status, st)
-                         : launch_elem<T, false>(z, p, n_z, which, nullptr, out, nullptr, nullptr, status, st);
+        if (!with_grad) return launch_elem<T>(false, z, p, n_z, which, nullptr, out, nullptr, nullptr, status, nullptr, st);
+        if (n_z > (int64_t)0xffffffffll) return COSMO_E_SIZE;            // 32-bit work list
+        WsLayout L = ws_layout(n_z, n_cosmo, mode, which, with_grad, sizeof(T));
+        if (ws_bytes < L.total || !ws) return ws ? COSMO_E_WORKSPACE : COSMO_E_NULL;
+        return with_grad ? launch_elem<T>(true, z, p, n_z, which, gout, out, gz, gparams, status, static_cast<unsigned*>(ws), st)
+                         : launch_elem<T>(false, z, p, n_z, which, nullptr, out, nullptr, nullptr, status, static_cast<unsigned*>(ws), st);
     }
     WsLayout L = ws_layout(n_z, n_cosmo, mode, which, with_grad, sizeof(T));
     if (ws_bytes < L.total || !ws) return ws ? COSMO_E_WORKSPACE : COSMO_E_NULL;
     char* w = static_cast<char*>(ws);
     Cosmo<double>* consts = reinterpret_cast<Cosmo<double>*>(w + L.consts);
     const bool kT = which & (W_TL | W_AGE), kA = which & W_DABS;
-    k_prep<<<(unsigned)cdiv(n_cosmo, 64), 64, 0, st>>>(p.Om, p.OL, p.Or, p.H0, n_cosmo, (with_grad ? ((kT || kA) ? 2 : 1) : 0) | ((which & W_AGE) ? 4 : 0), consts);
+    launch_prep(p.Om, p.OL, p.Or, p.H0, n_cosmo, (with_grad ? ((kT || kA) ? 2 : 1) : 0) | ((which & W_AGE) ? 4 : 0), consts, st);
     if ((rc = check_launch())) return rc;
     OuterArgs a{};
     a.z = z; a.gout = gout; a.out = out; a.status = status; a.consts = consts;
@@ -148,15 +150,15 @@ int run_eval(const T* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode,
                                     reinterpret_cast<uintptr_t>(gout) | reinterpret_cast<uintptr_t>(gz)) & m) == 0;
     }
     dim3 grid((unsigned)L.ntiles, (unsigned)L.ny);
-    if (!with_grad) return launch_outer<T, MODE_FWD>(a, grid, st);
+    if (!with_grad) return launch_outer<T>(MODE_FWD, a, grid, st);
     a.part = reinterpret_cast<double*>(w + L.part);
     a.gz_accumulate = L.ny > 1;
     a.gz = a.gz_accumulate ? static_cast<void*>(w + L.gzpart) : static_cast<void*>(gz);
-    if ((rc = launch_outer<T, MODE_VJP>(a, grid, st))) return rc;
-    k_reduce_params<4><<<(unsigned)cdiv(n_cosmo * 4 * 32, 256), 256, 0, st>>>(a.part, L.ntiles, n_cosmo, nullptr, gparams);
+    if ((rc = launch_outer<T>(MODE_VJP, a, grid, st))) return rc;
+    launch_reduce_params(4, a.part, L.ntiles, n_cosmo, nullptr, gparams, st);
     if ((rc = check_launch())) return rc;
     if (a.gz_accumulate) {
-        k_reduce_gz<T><<<(unsigned)cdiv(n_z, 256), 256, 0, st>>>(static_cast<const T*>(a.gz), L.ny, n_z, gz);
+        launch_reduce_gz(sizeof(T) == 4, a.gz, L.ny, n_z, gz, st);
         if ((rc = check_launch())) return rc;
     }
     return COSMO_OK;
@@ -181,7 +183,7 @@ int run_snia(const T* z, const T* mu_obs, const T* sigma, int64_t N, cosmo_param
     char* w = static_cast<char*>(ws);
     Cosmo<double>* consts = reinterpret_cast<Cosmo<double>*>(w + L.consts);
     int rc;
-    k_prep<<<(unsigned)cdiv(S, 64), 64, 0, st>>>(p.Om, p.OL, p.Or, p.H0, S, 1, consts);
+    launch_prep(p.Om, p.OL, p.Or, p.H0, S, 1, consts, st);
     if ((rc = check_launch())) return rc;
     OuterArgs a{};
     a.z = z; a.mu_obs = mu_obs; a.sigma = sigma; a.consts = consts; a.N = N; a.S = S; a.which = W_MU;
@@ -194,8 +196,8 @@ int run_snia(const T* z, const T* mu_obs, const T* sigma, int64_t N, cosmo_param
     if (cap < 1) cap = 1;
     if (ny > cap) ny = (int)cap;
     dim3 grid((unsigned)L.ntiles, (unsigned)ny);
-    if ((rc = launch_outer<T, MODE_SNIA>(a, grid, st))) return rc;
-    k_reduce_params<5><<<(unsigned)cdiv(S * 5 * 32, 256), 256, 0, st>>>(a.part, L.ntiles, S, logL, grad);
+    if ((rc = launch_outer<T>(MODE_SNIA, a, grid, st))) return rc;
+    launch_reduce_params(5, a.part, L.ntiles, S, logL, grad, st);
     return check_launch();
 }
 
@@ -219,7 +221,7 @@ int run_joint(const T* z, const T* z_obs, const T* mu_obs, const T* sigma_mu, do
     char* w = static_cast<char*>(ws);
     Cosmo<double>* consts = reinterpret_cast<Cosmo<double>*>(w + L.consts);
     int rc;
-    k_prep<<<(unsigned)cdiv(S, 64), 64, 0, st>>>(p.Om, p.OL, p.Or, p.H0, S, 1, consts);
+    launch_prep(p.Om, p.OL, p.Or, p.H0, S, 1, consts, st);
     if ((rc = check_launch())) return rc;
     OuterArgs a{};
     a.z = z; a.z_obs = z_obs; a.mu_obs = mu_obs; a.sigma = sigma_mu; a.gz = grad_z; a.consts = consts; a.N = N; a.S = S; a.which = W_MU;
@@ -234,15 +236,20 @@ int run_joint(const T* z, const T* z_obs, const T* mu_obs, const T* sigma_mu, do
     if (cap < 1) cap = 1;
     if (ny > cap) ny = (int)cap;
     dim3 grid((unsigned)L.ntiles, (unsigned)ny);
-    if ((rc = launch_outer<T, MODE_JOINT>(a, grid, st))) return rc;
-    k_reduce_params<5><<<(unsigned)cdiv(S * 5 * 32, 256), 256, 0, st>>>(a.part, L.ntiles, S, logp, grad);
+    if ((rc = launch_outer<T>(MODE_JOINT, a, grid, st))) return rc;
+    launch_reduce_params(5, a.part, L.ntiles, S, logp, grad, st);
     return check_launch();
 }
 
-// grow-only device scratch of the host-buffer convenience call
+// staging of the host-buffer call cosmo_eval_host: device scratch (grow-only until cosmo_host_release), a pinned block for the per-chunk
+// parameter sums, two streams and one event
 std::mutex g_host_mu;
 void* g_host_buf = nullptr;
 size_t g_host_cap = 0;
+void* g_host_pin = nullptr;
+size_t g_host_pin_cap = 0;
+cudaStream_t g_host_streams[2] = {nullptr, nullptr};
+cudaEvent_t g_host_ev = nullptr;
 
 }  // namespace
 
@@ -284,6 +291,10 @@ int cosmo_snia_loglike_f32(const float* z, const float* mu_obs, const float* sig
     return run_snia<float>(z, mu_obs, sigma, N, p, S, logL, grad, workspace, ws_bytes, stream);
 }
 
+// Host-buffer call: the redshift axis is cut into chunks that travel through two streams with two sets of device staging buffers, so
+// that the H2D copy of chunk i+1, the kernels of chunk i and the D2H copy of chunk i-1 overlap (PCIe is full duplex; the path is
+// PCIe-bound: 8 B of grad_out per eval against ~20 ps of kernel time).  Pinned host memory is needed for the overlap; pageable
+// memory still gives the right result.  Per-chunk parameter-gradient sums are added on the host in chunk order (deterministic).
 int cosmo_eval_host(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode, uint32_t which,
                     const double* grad_out, double* out, double* grad_z, double* grad_params, uint8_t* status) {
     int rc = check_common(z, n_z, p, n_cosmo, mode, which);
@@ -292,14 +303,31 @@ int cosmo_eval_host(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosm
     const bool with_grad = grad_out != nullptr;
     if (with_grad && (!grad_z || !grad_params)) return COSMO_E_NULL;
     if (!with_grad && !out) return COSMO_E_NULL;
-    const int64_t rows = (mode == COSMO_OUTER) ? n_cosmo : 1;
+    const bool outer = (mode == COSMO_OUTER), per_elem = (mode == COSMO_ELEMENTWISE && n_cosmo != 1);
+    const int64_t rows = outer ? n_cosmo : 1;
     const int np = __builtin_popcount(which);
-    const size_t b_z = align256(sizeof(double) * n_z), b_p = align256(sizeof(double) * n_cosmo);
-    const size_t b_out = align256(sizeof(double) * np * rows * n_z);
-    const size_t b_gp = align256(sizeof(double) * 4 * n_cosmo), b_st = align256((size_t)rows * n_z);
-    const size_t b_ws = align256(cosmo_workspace_bytes(n_z, n_cosmo, mode, which, with_grad));
-    size_t total = b_z + 4 * b_p + (out ? b_out : 0) + (with_grad ? b_out + b_z + b_gp : 0) + (status ? b_st : 0) + b_ws;
+    const int64_t n_par = per_elem ? 0 : n_cosmo;             // parameters copied once (shared) or chunked with z (per element)
+    // chunk length: ~32 MB of the widest per-redshift stream, at least 64 Ki redshifts, even (128-bit accesses), at most 64 chunks
+    const int64_t bytes_per_z = (int64_t)sizeof(double) * ((int64_t)np * rows * ((with_grad ? 1 : 0) + (out ? 1 : 0)) + 2 + (per_elem ? 8 : 0)) + rows;
+    int64_t nc = (32ll << 20) / bytes_per_z;
+    if (nc < 65536) nc = 65536;
+    if (nc * 64 < n_z) nc = cdiv(n_z, 64);
+    nc = (nc + 1) & ~int64_t(1);
+    if (nc > n_z) nc = n_z;
+    const int64_t nchunks = cdiv(n_z, nc);
+    const size_t b_z = align256(sizeof(double) * nc), b_pc = per_elem ? align256(sizeof(double) * nc) : 0;
+    const size_t b_pl = align256(sizeof(double) * np * rows * nc);
+    const size_t b_gp = align256(sizeof(double) * 4 * (per_elem ? nc : n_cosmo)), b_st = align256((size_t)rows * nc);
+    const size_t b_ws = align256(cosmo_workspace_bytes(nc, per_elem ? nc : n_cosmo, mode, which, with_grad));
+    const size_t per_set = b_z + 4 * b_pc + (out ? b_pl : 0) + (with_grad ? b_pl + b_z + b_gp : 0) + (status ? b_st : 0) + b_ws;
+    const size_t b_par = align256(sizeof(double) * (n_par > 0 ? n_par : 1));
+    const size_t total = 4 * b_par + 2 * per_set;
     std::lock_guard<std::mutex> lk(g_host_mu);
+    if (!g_host_streams[0]) {
+        for (int i = 0; i < 2; ++i)
+            if (cudaStreamCreateWithFlags(&g_host_streams[i], cudaStreamNonBlocking) != cudaSuccess) { g_last_cuda = (int)cudaGetLastError(); return COSMO_E_CUDA; }
+        if (cudaEventCreateWithFlags(&g_host_ev, cudaEventDisableTiming) != cudaSuccess) { g_last_cuda = (int)cudaGetLastError(); return COSMO_E_CUDA; }
+    }
     if (total > g_host_cap) {
         if (g_host_buf) cudaFree(g_host_buf);
         g_host_buf = nullptr; g_host_cap = 0;
@@ -307,36 +335,78 @@ int cosmo_eval_host(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosm
         if (e != cudaSuccess) { g_last_cuda = (int)e; return COSMO_E_CUDA; }
         g_host_cap = total;
     }
+    const size_t hp_bytes = with_grad && !per_elem ? sizeof(double) * 4 * n_cosmo * nchunks : 0;     // per-chunk parameter sums (pinned)
+    if (hp_bytes > g_host_pin_cap) {
+        if (g_host_pin) cudaFreeHost(g_host_pin);
+        g_host_pin = nullptr; g_host_pin_cap = 0;
+        if (cudaMallocHost(&g_host_pin, hp_bytes) != cudaSuccess) { g_last_cuda = (int)cudaGetLastError(); return COSMO_E_CUDA; }
+        g_host_pin_cap = hp_bytes;
+    }
     char* base = static_cast<char*>(g_host_buf);
     size_t off = 0;
     auto take = [&](size_t b) { char* q = base + off; off += b; return q; };
-    double* d_z = (double*)take(b_z);
-    double* d_p[4];
-    for (int i = 0; i < 4; ++i) d_p[i] = (double*)take(b_p);
-    double* d_out = out ? (double*)take(b_out) : nullptr;
-    double* d_gout = with_grad ? (double*)take(b_out) : nullptr;
-    double* d_gz = with_grad ? (double*)take(b_z) : nullptr;
-    double* d_gp = with_grad ? (double*)take(b_gp) : nullptr;
-    uint8_t* d_st = status ? (uint8_t*)take(b_st) : nullptr;
-    void* d_ws = take(b_ws);
-    cudaStream_t st = nullptr;
-    cudaMemcpyAsync(d_z, z, sizeof(double) * n_z, cudaMemcpyHostToDevice, st);
-    const double* hp[4] = {p.Om, p.OL, p.Or, p.H0};
-    for (int i = 0; i < 4; ++i) cudaMemcpyAsync(d_p[i], hp[i], sizeof(double) * n_cosmo, cudaMemcpyHostToDevice, st);
-    if (with_grad) cudaMemcpyAsync(d_gout, grad_out, sizeof(double) * np * rows * n_z, cudaMemcpyHostToDevice, st);
-    cosmo_params dp{d_p[0], d_p[1], d_p[2], d_p[3]};
-    rc = with_grad ? cosmo_vjp(d_z, n_z, dp, n_cosmo, mode, which, d_gout, d_out, d_gz, d_gp, d_st, d_ws, b_ws, st)
-                   : cosmo_eval(d_z, n_z, dp, n_cosmo, mode, which, d_out, d_st, d_ws, b_ws, st);
-    if (rc) return rc;
-    if (out) cudaMemcpyAsync(out, d_out, sizeof(double) * np * rows * n_z, cudaMemcpyDeviceToHost, st);
-    if (with_grad) {
-        cudaMemcpyAsync(grad_z, d_gz, sizeof(double) * n_z, cudaMemcpyDeviceToHost, st);
-        cudaMemcpyAsync(grad_params, d_gp, sizeof(double) * 4 * n_cosmo, cudaMemcpyDeviceToHost, st);
+    double* d_par[4];
+    for (int i = 0; i < 4; ++i) d_par[i] = (double*)take(b_par);
+    struct Set { double *z, *pc[4], *out, *gout, *gz, *gp; uint8_t* st; void* ws; } S[2];
+    for (int k = 0; k < 2; ++k) {
+        S[k].z = (double*)take(b_z);
+        for (int i = 0; i < 4; ++i) S[k].pc[i] = per_elem ? (double*)take(b_pc) : d_par[i];
+        S[k].out = out ? (double*)take(b_pl) : nullptr;
+        S[k].gout = with_grad ? (double*)take(b_pl) : nullptr;
+        S[k].gz = with_grad ? (double*)take(b_z) : nullptr;
+        S[k].gp = with_grad ? (double*)take(b_gp) : nullptr;
+        S[k].st = status ? (uint8_t*)take(b_st) : nullptr;
+        S[k].ws = take(b_ws);
     }
-    if (status) cudaMemcpyAsync(status, d_st, (size_t)rows * n_z, cudaMemcpyDeviceToHost, st);
-    cudaError_t e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) { g_last_cuda = (int)e; return COSMO_E_CUDA; }
+    const double* hp[4] = {p.Om, p.OL, p.Or, p.H0};
+    cudaStream_t s0 = g_host_streams[0], s1 = g_host_streams[1];
+    if (!per_elem) {
+        for (int i = 0; i < 4; ++i) cudaMemcpyAsync(d_par[i], hp[i], sizeof(double) * n_cosmo, cudaMemcpyHostToDevice, s0);
+        cudaEventRecord(g_host_ev, s0);
+        cudaStreamWaitEvent(s1, g_host_ev, 0);
+    }
+    const size_t hpitch = sizeof(double) * n_z;               // host planes [np][rows][n_z]: row pitch n_z
+    double* hsum = static_cast<double*>(g_host_pin);
+    for (int64_t c = 0; c < nchunks && rc == COSMO_OK; ++c) {
+        const int k = (int)(c & 1);
+        cudaStream_t st = k ? s1 : s0;
+        const int64_t n0 = c * nc, n = (n0 + nc <= n_z) ? nc : (n_z - n0);
+        cudaMemcpyAsync(S[k].z, z + n0, sizeof(double) * n, cudaMemcpyHostToDevice, st);
+        if (per_elem)
+            for (int i = 0; i < 4; ++i) cudaMemcpyAsync(S[k].pc[i], hp[i] + n0, sizeof(double) * n, cudaMemcpyHostToDevice, st);
+        if (with_grad)
+            cudaMemcpy2DAsync(S[k].gout, sizeof(double) * n, grad_out + n0, hpitch, sizeof(double) * n, (size_t)np * rows, cudaMemcpyHostToDevice, st);
+        cosmo_params dp{S[k].pc[0], S[k].pc[1], S[k].pc[2], S[k].pc[3]};
+        const int64_t ncos = per_elem ? n : n_cosmo;
+        rc = with_grad ? cosmo_vjp(S[k].z, n, dp, ncos, mode, which, S[k].gout, S[k].out, S[k].gz, S[k].gp, S[k].st, S[k].ws, b_ws, st)
+                       : cosmo_eval(S[k].z, n, dp, ncos, mode, which, S[k].out, S[k].st, S[k].ws, b_ws, st);
+        if (rc) break;
+        if (out) cudaMemcpy2DAsync(out + n0, hpitch, S[k].out, sizeof(double) * n, sizeof(double) * n, (size_t)np * rows, cudaMemcpyDeviceToHost, st);
+        if (status) cudaMemcpy2DAsync(status + n0, (size_t)n_z, S[k].st, (size_t)n, (size_t)n, (size_t)rows, cudaMemcpyDeviceToHost, st);
+        if (with_grad) {
+            cudaMemcpyAsync(grad_z + n0, S[k].gz, sizeof(double) * n, cudaMemcpyDeviceToHost, st);
+            if (per_elem) cudaMemcpy2DAsync(grad_params + n0, hpitch, S[k].gp, sizeof(double) * n, sizeof(double) * n, 4, cudaMemcpyDeviceToHost, st);
+            else cudaMemcpyAsync(hsum + c * 4 * n_cosmo, S[k].gp, sizeof(double) * 4 * n_cosmo, cudaMemcpyDeviceToHost, st);
+        }
+    }
+    cudaError_t e0 = cudaStreamSynchronize(s0), e1 = cudaStreamSynchronize(s1);
+    if (rc) return rc;
+    if (e0 != cudaSuccess || e1 != cudaSuccess) { g_last_cuda = (int)(e0 != cudaSuccess ? e0 : e1); return COSMO_E_CUDA; }
+    if (with_grad && !per_elem) {
+        for (int64_t i = 0; i < 4 * n_cosmo; ++i) {
+            double v = 0.0;
+            for (int64_t c = 0; c < nchunks; ++c) v += hsum[c * 4 * n_cosmo + i];
+            grad_params[i] = v;
+        }
+    }
     return COSMO_OK;
+}
+
+void cosmo_host_release(void) {
+    std::lock_guard<std::mutex> lk(g_host_mu);
+    if (g_host_buf) cudaFree(g_host_buf);
+    if (g_host_pin) cudaFreeHost(g_host_pin);
+    g_host_buf = nullptr; g_host_cap = 0; g_host_pin = nullptr; g_host_pin_cap = 0;
 }
 
 int cosmo_eval2(const double* z1, const double* z2, int64_t n, cosmo_params p, int64_t n_cosmo, uint32_t which, const double* grad_out,
@@ -348,8 +418,7 @@ int cosmo_eval2(const double* z1, const double* z2, int64_t n, cosmo_params p, i
     if (grad_out ? (!grad_z1 || !grad_z2 || !grad_params) : !out) return COSMO_E_NULL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     prof_begin(st);
-    k_two<<<(unsigned)cdiv(n, ELEM_THREADS), ELEM_THREADS, 0, st>>>(z1, z2, p.Om, p.OL, p.Or, p.H0, n, n_cosmo, which, grad_out, out, grad_z1,
-                                                                    grad_z2, grad_params, status);
+    launch_two(z1, z2, p.Om, p.OL, p.Or, p.H0, n, n_cosmo, which, grad_out, out, grad_z1, grad_z2, grad_params, status, st);
     prof_end(st);
     return check_launch();
 }
@@ -363,7 +432,7 @@ int cosmo_eval_w(const double* z, int64_t n, const double* Om, const double* OL,
     if (!z || !Om || !OL || !Or || !Ow13 || !Ow23 || !H0 || !out) return COSMO_E_NULL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     prof_begin(st);
-    k_w<<<(unsigned)cdiv(n, ELEM_THREADS), ELEM_THREADS, 0, st>>>(z, Om, OL, Or, Ow13, Ow23, H0, n, n_cosmo, which, out, dout_dz, status);
+    launch_w(z, Om, OL, Or, Ow13, Ow23, H0, n, n_cosmo, which, out, dout_dz, status, st);
     prof_end(st);
     return check_launch();
 }
@@ -373,20 +442,20 @@ int cosmo_carlson_pair(const double* x, const double* m, const double* s, const 
     if (n < 0) return COSMO_E_SIZE;
     if (n == 0) return COSMO_OK;
     if (!x || !m || !s || !p || !rf || !rd || !rj) return COSMO_E_NULL;
-    k_carlson_pair<<<(unsigned)cdiv(n, 128), 128, 0, static_cast<cudaStream_t>(stream)>>>(x, m, s, p, n, rf, rd, rj);
+    launch_carlson_pair(x, m, s, p, n, rf, rd, rj, static_cast<cudaStream_t>(stream));
     return check_launch();
 }
 
 int cosmo_probe_fma_f64(int blocks, int iters, double* sink, void* stream) {
     if (blocks <= 0 || iters < 0) return COSMO_E_SIZE;
     if (!sink) return COSMO_E_NULL;
-    k_probe_fma<double><<<blocks, 256, 0, static_cast<cudaStream_t>(stream)>>>(iters, sink);
+    launch_probe_fma(false, blocks, iters, sink, static_cast<cudaStream_t>(stream));
     return check_launch();
 }
 int cosmo_probe_fma_f32(int blocks, int iters, float* sink, void* stream) {
     if (blocks <= 0 || iters < 0) return COSMO_E_SIZE;
     if (!sink) return COSMO_E_NULL;
-    k_probe_fma<float><<<blocks, 256, 0, static_cast<cudaStream_t>(stream)>>>(iters, sink);
+    launch_probe_fma(true, blocks, iters, sink, static_cast<cudaStream_t>(stream));
     return check_launch();
 }
 

@@ -11,6 +11,7 @@
 // real arithmetic only:  sqrt(y) sqrt(ybar) = sqrt(mp^2 - s),  sqrt(y) + sqrt(ybar) = sqrt(2 (mp + sqrt(mp^2 - s))).
 #pragma once
 #include "cosmo_types.cuh"
+#include "cosmo_prep.cuh"
 
 namespace cb {
 
@@ -359,46 +360,49 @@ CB_HD T carlson_Qj(T xa, T mp, T hs, T p) {
 // S4-S6 for K elements of the SAME cosmology in lock-step (K independent dependency chains per thread: the FP64
 // pipe has ~9 cycles of latency and few warps fit, so instruction-level parallelism is what keeps it busy).
 // kT: lookback integral, kA: absorption integral, kK: the second-kind integral K (needs R_D).
-template <typename T, bool kT, bool kA, bool kK, int K, typename Vote>
-CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Core<T> (&R)[K]) {
+// kRecon (ELEMENTWISE kernels, one cosmology per element): the constants are formed again after the loop from the factorisation
+// (cosmo_reconstitute) and returned in *Cout for the observables and the backward pass.
+template <typename T, bool kT, bool kA, bool kK, int K, typename Vote, bool kRecon = false>
+CB_HD void eval_core_k(const Cosmo<T>& C0, const T (&z)[K], const Vote& vote, Core<T> (&R)[K], Cosmo<T>* Cout = nullptr) {
     using N = Num<T>;
+    const Cosmo<T>* Cp = &C0;
     constexpr bool kD = kK || kA;          // R_D tail needed
     // Only U12 and the loop state stay live across the duplication loop; everything cheap is recomputed after it
     // (registers decide how many warps fit).
     T U12[K], ra[K], iE[K], xa[K], mp[K], s[K], Qc[K];
     unsigned st[K];
     T p5[K], p0[K], dl5[K], dl0[K], p5_0[K], p0_0[K], Q5v[K], Q0v[K];
-    const bool quartA = kA && !(C.cubic & 1u);
+    const bool quartA = kA && !(C0.cubic & 1u);
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         const T x = T(1) + z[k];
         const T z2 = z[k] * z[k];
-        st[k] = C.status;
+        st[k] = C0.status;
         if (!(x > T(0))) st[k] |= ST_UNSUPPORTED;
-        if (x >= C.xlim) st[k] |= ST_ROOT_ON_PATH;
+        if (x >= C0.xlim) st[k] |= ST_ROOT_ON_PATH;
         // ---- S4 radicands
-        const T q1x = N::fma_(C.Or, x, C.m) * (x - C.rn);
-        const T q2x = N::fma_(x + C.b, x, C.c);
-        const T a1 = q1x * C.q21, a2 = C.q11 * q2x;
+        const T q1x = N::fma_(C0.Or, x, C0.m) * (x - C0.rn);
+        const T q2x = N::fma_(x + C0.b, x, C0.c);
+        const T a1 = q1x * C0.q21, a2 = C0.q11 * q2x;
         const T r1 = N::rsqrt_(a1), r2 = N::rsqrt_(a2);
         ra[k] = a1 * r1;
         iE[k] = r1 * r2;                                  // a1 a2 = E^2(x) E^2(1) and E(1) = 1 (sum of Omegas)
         U12[k] = N::fma_(a2, r2, ra[k]);
         xa[k] = U12[k] * U12[k];
-        const T hd = T(0.5) * z2 * C.theta;               // u12^2 - (u13^2 + u14^2)/2
+        const T hd = T(0.5) * z2 * C0.theta;               // u12^2 - (u13^2 + u14^2)/2
         mp[k] = xa[k] - hd;
-        s[k] = z2 * z2 * C.sD;
-        const T hs = z2 * C.sDr;                          // |h|
+        s[k] = z2 * z2 * C0.sD;
+        const T hs = z2 * C0.sDr;                          // |h|
         // ---- R_J parameters
         p5[k] = p0[k] = dl5[k] = dl0[k] = p5_0[k] = p0_0[k] = Q5v[k] = Q0v[k] = T(0);
         if (kT) {
-            p5[k] = N::fma_(z2, C.p5c, xa[k]);
+            p5[k] = N::fma_(z2, C0.p5c, xa[k]);
             p5_0[k] = p5[k];
             const T pm = p5[k] - mp[k];
             dl5[k] = (p5[k] - xa[k]) * N::fma_(pm, pm, -s[k]);
         }
         if (kA) {
-            p0[k] = quartA ? N::fma_(-C.Or * z2, C.Q2n, xa[k]) : xa[k];
+            p0[k] = quartA ? N::fma_(-C0.Or * z2, C0.Q2n, xa[k]) : xa[k];
             p0_0[k] = p0[k];
             const T pm = p0[k] - mp[k];
             dl0[k] = (p0[k] - xa[k]) * N::fma_(pm, pm, -s[k]);
@@ -412,6 +416,13 @@ CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Cor
     // ---- S5 fused duplication
     T g2, tailD[K], sum5[K], sum0[K];
     carlson_dup<T, kD, kT, kA, K, Vote>(xa, mp, s, p5, p0, dl5, dl0, Qc, Q5v, Q0v, st, vote, g2, tailD, sum5, sum0);
+    if (kRecon) {
+        Cosmo<double> Dd{};
+        cosmo_reconstitute<T>(C0, Dd);
+        convert_cosmo<T>(Dd, *Cout);
+        Cp = Cout;
+    }
+    const Cosmo<T>& C = *Cp;
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         const T x = T(1) + z[k];
@@ -507,11 +518,11 @@ CB_HD void eval_core_k(const Cosmo<T>& C, const T (&z)[K], const Vote& vote, Cor
 }
 
 // single-element form (ELEMENTWISE kernel, host checks)
-template <typename T, bool kT, bool kA, bool kK, typename Vote>
-CB_HD void eval_core(const Cosmo<T>& C, T z, const Vote& vote, Core<T>& R) {
+template <typename T, bool kT, bool kA, bool kK, typename Vote, bool kRecon = false>
+CB_HD void eval_core(const Cosmo<T>& C, T z, const Vote& vote, Core<T>& R, Cosmo<T>* Cout = nullptr) {
     const T zz[1] = {z};
     Core<T> RR[1];
-    eval_core_k<T, kT, kA, kK, 1, Vote>(C, zz, vote, RR);
+    eval_core_k<T, kT, kA, kK, 1, Vote, kRecon>(C, zz, vote, RR, Cout);
     R = RR[0];
 }
 
@@ -531,6 +542,21 @@ CB_HD void sinn_poly(T w, T& sf, T& sg, T& sd) {
 // unified curvature transform in w = Ok I0^2 (reading R-sinn):
 //   F = I0 f(w), dF/dI0 = g(w), dF/dOk = I0^3 f'(w);  f = sum w^j/(2j+1)!, g = sum w^j/(2j)!
 // degree 7 for |w| <= 1/2 (next term 0.5^8/17! ~ 1e-17), degree 10 for |w| <= 1, libm beyond.
+// closed forms beyond |w| = 1 (libm exp / sincos)
+template <typename T>
+CB_HD void sinn_libm(T k, T I0, T& F, T& Fi, T& Fk) {
+    using N = Num<T>;
+    if (k > T(0)) {
+        const T sq = N::sqrt_(k), y = sq * I0, ey = N::exp_(y), iey = T(1) / ey;
+        const T sh = T(0.5) * (ey - iey), ch = T(0.5) * (ey + iey);
+        F = sh / sq; Fi = ch; Fk = (I0 * ch - F) / (T(2) * k);
+    } else {
+        const T sq = N::sqrt_(-k);
+        T sn, cs;
+        N::sincos_(sq * I0, &sn, &cs);
+        F = sn / sq; Fi = cs; Fk = (I0 * cs - F) / (T(2) * k);
+    }
+}
 template <typename T>
 CB_HD void sinn(T k, T I0, T& F, T& Fi, T& Fk) {
     using N = Num<T>;
@@ -542,16 +568,7 @@ CB_HD void sinn(T k, T I0, T& F, T& Fi, T& Fk) {
         F = I0 * sf; Fi = sg; Fk = I0 * I0 * I0 * sd;
         return;
     }
-    if (k > T(0)) {
-        const T sq = N::sqrt_(k), y = sq * I0, ey = N::exp_(y), iey = T(1) / ey;
-        const T sh = T(0.5) * (ey - iey), ch = T(0.5) * (ey + iey);
-        F = sh / sq; Fi = ch; Fk = (I0 * ch - F) / (T(2) * k);
-    } else {
-        const T sq = N::sqrt_(-k);
-        T sn, cs;
-        N::sincos_(sq * I0, &sn, &cs);
-        F = sn / sq; Fi = cs; Fk = (I0 * cs - F) / (T(2) * k);
-    }
+    sinn_libm<T>(k, I0, F, Fi, Fk);
 }
 
 }  // namespace cb

@@ -7,36 +7,11 @@
 // looping over a chunk of cosmologies, so the only per-eval HBM traffic is grad_out (8 B) and, if asked, out.
 #pragma once
 #include <cuda_runtime.h>
+#include "cosmo_launch.cuh"
 #include "cosmo_prep.cuh"
 #include "cosmo_obs.cuh"
-#include "cosmo_two.cuh"
-#include "cosmo_w.cuh"
 
 namespace cb {
-
-#ifndef CB_THREADS
-#define CB_THREADS 128
-#endif
-constexpr int OUTER_THREADS = CB_THREADS;
-// consecutive redshifts per thread (even), advanced in lock-step.  Per-thread overhead (staging, address arithmetic, the
-// warp reduction, constant and shared-memory loads) is paid once per KZ elements, so the chi family -- whose working set
-// fits -- takes 4; the kernels that also carry the R_J tracks (t_L, d_abs) stay at 2 (4 spills).  Measured: profiles/.
-#ifndef CB_KZ_CHI
-#define CB_KZ_CHI 4
-#endif
-#ifndef CB_KZ_TA
-#define CB_KZ_TA 2
-#endif
-__host__ __device__ constexpr int outer_kz(bool kT, bool kA) { return (kT || kA) ? CB_KZ_TA : CB_KZ_CHI; }
-__host__ __device__ constexpr int outer_tile(bool kT, bool kA) { return OUTER_THREADS * outer_kz(kT, kA); }   // redshifts per block
-#ifndef CB_SCHUNK
-#define CB_SCHUNK 16
-#endif
-constexpr int S_CHUNK = CB_SCHUNK;                         // cosmologies staged in shared memory at a time
-constexpr int NWARP = OUTER_THREADS / 32;
-constexpr int ELEM_THREADS = 128;
-
-enum { MODE_FWD = 0, MODE_VJP = 1, MODE_SNIA = 2, MODE_JOINT = 3 };   // JOINT: SNIA + latent redshifts z[S][N]
 
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
@@ -57,25 +32,6 @@ __device__ __forceinline__ double warp_sum4(const double (&v)[4], int lane) {
 #pragma unroll
     for (int off = 4; off > 0; off >>= 1) k += __shfl_xor_sync(0xffffffffu, k, off);
     return k;
-}
-
-// S1-S3, one thread per cosmology
-__global__ void k_prep(const double* __restrict__ Om, const double* __restrict__ OL, const double* __restrict__ Or,
-                       const double* __restrict__ H0, int64_t S, int want_grad, Cosmo<double>* __restrict__ out) {
-    int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (s >= S) return;
-    Cosmo<double> C;
-    cosmo_prep(Om[s], OL[s], Or[s], H0[s], want_grad & 3, C);
-    if (want_grad & 4) prep_age(C, (want_grad & 3) != 0);
-    else { C.Tinf = 0.0; C.dTinf[0] = C.dTinf[1] = C.dTinf[2] = 0.0; }
-    if ((want_grad & 3) < 2) {
-        for (int t = 0; t < 3; ++t) {
-            for (int j = 0; j < 7; ++j) C.GA[t][j] = 0.0;
-            for (int j = 0; j < 5; ++j) C.GJ[t][j] = C.GJ[t + 2][j] = 0.0;
-            if ((want_grad & 3) < 1) { for (int j = 0; j < 5; ++j) C.GI[t][j] = 0.0; for (int j = 0; j < 6; ++j) C.GT[t][j] = 0.0; }
-        }
-    }
-    out[s] = C;
 }
 
 template <typename T> struct Vec2;
@@ -108,19 +64,6 @@ __device__ __forceinline__ void store2(T* __restrict__ p, int64_t i, int64_t n, 
         }
     }
 }
-
-struct OuterArgs {
-    const void* z; const void* gout; const void* mu_obs; const void* sigma; const void* z_obs;
-    double sigma_z, beta, shape_m1, prior_norm;   // MODE_JOINT: photo-z scatter, gamma prior rate, shape - 1, and the constant
-                                                  // shape ln(beta) - lnGamma(shape) - ln(sigma_z) - ln(2 pi)/2
-    void* out; void* gz; uint8_t* status;
-    const Cosmo<double>* consts;
-    double* part;            // [S][NP][ntiles] partial parameter sums (NP = 4 vjp, 5 snia)
-    int64_t N, S;
-    unsigned which;
-    int gz_accumulate;       // gridDim.y > 1: gz holds [gridDim.y][N] partials
-    int vec;                 // N even and pointers 16-byte aligned
-};
 
 // One cosmology row of the OUTER kernels that cannot take the fused loop: E^2 without a real negative root (Cosmo::cubic bit 1:
 // complex slow path, cosmo_c4.cuh) or gradient bases that need the per-element conditioning check (bits 2, 3: backward_robust).
@@ -400,152 +343,108 @@ __global__ void k_reduce_gz(const T* __restrict__ part, int ny, int64_t N, T* __
     gz[n] = v;
 }
 
-// ELEMENTWISE with one cosmology per redshift: S1-S8 per thread, no reductions.
+// ELEMENTWISE with one cosmology per redshift: S1-S8 per thread (cosmo_obs.cuh, elem_one), no reductions.
 // Register budget: left alone the all-outputs variants take 255 registers (8 warps/SM) and wait on latency at a third of the
-// FP64 pipe; capping them at 128 (VJP) / 80 (forward) registers trades spills (written back to DRAM, profiles/r01c_timings.md)
-// for 16 / 24 warps per SM.  Measured on
-// config 5 (profiles/r01c_timings.md): forward 3.31 -> 2.15 ms, forward + VJP 4.75 -> 3.95 ms; config 2 forward 0.26 -> 0.18 ms.
+// FP64 pipe; capped at 128 (VJP) / 80 (forward) registers they run 16 / 24 warps per SM (profiles/).
+// Two passes.  k_elem is the fast path for every element; the few that need a slow path -- E^2 without a real negative root
+// (complex arithmetic, cosmo_c4.cuh), gradient bases too ill-conditioned (quadrature, cosmo_obs.cuh) -- are only listed
+// (redo_count, redo_list in the workspace) and k_elem_redo runs them again, densely packed, with the slow paths compiled in.
+// A never-inlined call inside the main kernel costs it 15-30 % even where it is not taken (profiles/).
+#ifndef CB_ELEM_MINB_G
+#define CB_ELEM_MINB_G 4
+#endif
+#ifndef CB_ELEM_MINB_F
+#define CB_ELEM_MINB_F 6
+#endif
 template <typename T, bool kT, bool kA, bool kG>
-__global__ void __launch_bounds__(ELEM_THREADS, kG ? 4 : 6) k_elem(const T* __restrict__ z, const double* __restrict__ Om,
-                                                       const double* __restrict__ OL, const double* __restrict__ Or,
-                                                       const double* __restrict__ H0, int64_t N, unsigned which,
-                                                       const T* __restrict__ gout, T* __restrict__ out, T* __restrict__ gz,
-                                                       double* __restrict__ gparams, uint8_t* __restrict__ status) {
+__global__ void __launch_bounds__(ELEM_THREADS, kG ? CB_ELEM_MINB_G : CB_ELEM_MINB_F) k_elem(ElemArgs a) {
+    const int64_t N = a.N;
+    const unsigned which = a.which;
     const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     const bool live = i < N;
     const int64_t ii = live ? i : N - 1;
-    Cosmo<T> C;
-    {
-        Cosmo<double> Cd;
-        cosmo_prep(Om[ii], OL[ii], Or[ii], H0[ii], kG ? ((kT || kA) ? 2 : 1) : 0, Cd);
-        if (kT && (which & W_AGE)) prep_age(Cd, kG);
-        else { Cd.Tinf = 0.0; Cd.dTinf[0] = Cd.dTinf[1] = Cd.dTinf[2] = 0.0; }
-        convert_cosmo<T>(Cd, C);
-    }
-    const T zv = z[ii];
-    Core<T> R;
-    R.K = T(0); R.TT = T(0); R.AA = T(0);
-    eval_core<T, kT, kA, kG, VoteWarp>(C, zv, VoteWarp(), R);
-    apply_c4<T, kT, kA, kG>(C, zv, R);
-    Obs<T> O;
-    observables<T, kT, kA>(C, zv, R, which, O);
-    if (!live) return;
-    if (out != nullptr) {
-        int pl = 0;
-        for (int w = 0; w < N_PLANES; ++w) {
-            if (!(which >> w & 1)) continue;
-            out[(int64_t)pl * N + i] = O.v[w];
-            ++pl;
-        }
-    }
-    if (status != nullptr && !kG) status[i] = (uint8_t)O.status;
+    const T* __restrict__ gout = static_cast<const T*>(a.gout);
+    T g[N_PLANES], v[N_PLANES];
     if (kG) {
-        T g[N_PLANES];
         int pl = 0;
         for (int w = 0; w < N_PLANES; ++w) {
             g[w] = T(0);
             if (!(which >> w & 1)) continue;
-            g[w] = gout[(int64_t)pl * N + i];
+            g[w] = gout[(int64_t)pl * N + ii];
             ++pl;
         }
-        T dz = T(0), gp[4] = {T(0), T(0), T(0), T(0)};
-        const unsigned stg = backward_robust<T, kT, kA>(C, zv, R, O, g, dz, gp, which);
-        if (status != nullptr) status[i] = (uint8_t)(O.status | stg);
-        gz[i] = dz;
-#pragma unroll
-        for (int j = 0; j < 4; ++j) gparams[(int64_t)j * N + i] = (double)gp[j];
     }
-}
-
-// Two-limit evaluation (cosmo_two.cuh), one thread per (z1, z2, cosmology); n_cosmo in {1, n}.  which: DC, DM, TL, DABS, DA.
-// (128-register cap as for k_elem: 0.40 -> 0.28 ms forward, 0.75 -> 0.56 ms forward + VJP per 10^6 pairs)
-__global__ void __launch_bounds__(ELEM_THREADS, 4) k_two(const double* __restrict__ z1, const double* __restrict__ z2,
-                                                      const double* __restrict__ Om, const double* __restrict__ OL,
-                                                      const double* __restrict__ Or, const double* __restrict__ H0, int64_t n,
-                                                      int64_t n_cosmo, unsigned which, const double* __restrict__ gout,
-                                                      double* __restrict__ out, double* __restrict__ gz1, double* __restrict__ gz2,
-                                                      double* __restrict__ gparams, uint8_t* __restrict__ status) {
-    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    const bool live = i < n;
-    const int64_t ii = live ? i : n - 1, ic = n_cosmo == 1 ? 0 : ii;
-    const bool with_grad = gout != nullptr;
-    Cosmo<double> C;
-    cosmo_prep(Om[ic], OL[ic], Or[ic], H0[ic], with_grad ? 2 : 0, C);
-    Two O;
-    eval_two<VoteWarp>(C, z1[ii], z2[ii], with_grad, VoteWarp(), O);
-    if (!live) return;
-    const unsigned bits[5] = {W_DC, W_DM, W_TL, W_DABS, W_DA};
-    double a1 = 0.0, a2 = 0.0, ap[4] = {0.0, 0.0, 0.0, 0.0};
-    int pl = 0;
-    for (int o = 0; o < 5; ++o) {
-        if (!(which & bits[o])) continue;
-        if (out != nullptr) out[(int64_t)pl * n + i] = O.v[o];
-        if (with_grad) {
-            const double g = gout[(int64_t)pl * n + i];
-            a1 = fma(g, O.gz1[o], a1); a2 = fma(g, O.gz2[o], a2);
-            for (int t = 0; t < 4; ++t) ap[t] = fma(g, O.gp[o][t], ap[t]);
+    T dz = T(0), gp[4] = {T(0), T(0), T(0), T(0)};
+    const unsigned st = elem_one<T, kT, kA, kG, VoteWarp, true>(static_cast<const T*>(a.z)[ii], a.Om[ii], a.OL[ii], a.Or[ii], a.H0[ii], which,
+                                                                VoteWarp(), g, v, dz, gp);
+    if (live && a.out != nullptr) {
+        T* __restrict__ out = static_cast<T*>(a.out);
+        int pl = 0;
+        for (int w = 0; w < N_PLANES; ++w) {
+            if (!(which >> w & 1)) continue;
+            out[(int64_t)pl * N + i] = v[w];
+            ++pl;
         }
-        ++pl;
     }
-    if (status != nullptr) status[i] = (uint8_t)O.status;
-    if (with_grad) {
-        gz1[i] = a1; gz2[i] = a2;
-        for (int t = 0; t < 4; ++t) gparams[(int64_t)t * n + i] = ap[t];
+    if (live && a.status != nullptr) a.status[i] = (uint8_t)(st & ~(unsigned)ST_INTERNAL_REDO);
+    if (kG && live) {
+        static_cast<T*>(a.gz)[i] = dz;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) a.gparams[(int64_t)j * N + i] = (double)gp[j];
+    }
+    if (kG) {   // work list of the second pass: one atomic per warp (no lane has returned early)
+        const bool redo = live && (st & ST_INTERNAL_REDO);
+        const unsigned active = __activemask();
+        const unsigned m = __ballot_sync(active, redo);
+        if (m) {
+            const int lane = threadIdx.x & 31, leader = __ffs(m) - 1;
+            unsigned base = 0;
+            if (lane == leader) base = atomicAdd(a.redo_count, (unsigned)__popc(m));
+            base = __shfl_sync(active, base, leader);
+            if (redo) a.redo_list[base + __popc(m & ((1u << lane) - 1u))] = (unsigned)i;
+        }
     }
 }
 
-// chi family with extra constant-w components (cosmo_w.cuh), one thread per (z, cosmology); n_cosmo in {1, n}.
-// which: DC, DM, DL, MU.  out[n_which][n]; dout[n_which][n] = d out / dz (nullable).
-__global__ void __launch_bounds__(ELEM_THREADS) k_w(const double* __restrict__ z, const double* __restrict__ Om,
-                                                    const double* __restrict__ OL, const double* __restrict__ Or,
-                                                    const double* __restrict__ Ow13, const double* __restrict__ Ow23,
-                                                    const double* __restrict__ H0, int64_t n, int64_t n_cosmo, unsigned which,
-                                                    double* __restrict__ out, double* __restrict__ dout, uint8_t* __restrict__ status) {
-    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    const bool live = i < n;
-    const int64_t ii = live ? i : n - 1, ic = n_cosmo == 1 ? 0 : ii;
-    WCosmo W;
-    __shared__ WCosmo sw;
-    if (n_cosmo == 1) {                       // one shared cosmology: factor it once per block, not once per thread
-        if (threadIdx.x == 0) w_prep(Om[0], OL[0], Or[0], Ow13[0], Ow23[0], H0[0], sw);
-        __syncthreads();
-        W = sw;
-    } else {
-        w_prep(Om[ic], OL[ic], Or[ic], Ow13[ic], Ow23[ic], H0[ic], W);
+// second pass: the listed elements again with every slow path available (elem_one without kDefer).  Dense: consecutive threads take
+// consecutive list entries, whatever their position in the batch.
+template <typename T, bool kT, bool kA, bool kG>      // (kG = true: only the VJP has a second pass)
+__global__ void __launch_bounds__(ELEM_THREADS, 4) k_elem_redo(ElemArgs a) {
+    const int64_t N = a.N;
+    const unsigned which = a.which;
+    const unsigned count = *a.redo_count;
+    const T* __restrict__ gout = static_cast<const T*>(a.gout);
+    for (unsigned j = blockIdx.x * blockDim.x + threadIdx.x; j < count; j += gridDim.x * blockDim.x) {
+        const int64_t i = a.redo_list[j];
+        T g[N_PLANES], v[N_PLANES];
+        if (kG) {
+            int pl = 0;
+            for (int w = 0; w < N_PLANES; ++w) {
+                g[w] = T(0);
+                if (!(which >> w & 1)) continue;
+                g[w] = gout[(int64_t)pl * N + i];
+                ++pl;
+            }
+        }
+        T dz = T(0), gp[4] = {T(0), T(0), T(0), T(0)};
+        const unsigned st = elem_one<T, kT, kA, kG, VoteNone, false>(static_cast<const T*>(a.z)[i], a.Om[i], a.OL[i], a.Or[i], a.H0[i], which,
+                                                                     VoteNone(), g, v, dz, gp);
+        if (a.out != nullptr) {
+            T* __restrict__ out = static_cast<T*>(a.out);
+            int pl = 0;
+            for (int w = 0; w < N_PLANES; ++w) {
+                if (!(which >> w & 1)) continue;
+                out[(int64_t)pl * N + i] = v[w];
+                ++pl;
+            }
+        }
+        if (a.status != nullptr) a.status[i] = (uint8_t)st;
+        if (kG) {
+            static_cast<T*>(a.gz)[i] = dz;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) a.gparams[(int64_t)k * N + i] = (double)gp[k];
+        }
     }
-    double v[4], dz[4];
-    const unsigned st = w_eval<VoteWarp>(W, z[ii], VoteWarp(), v, dz);
-    if (!live) return;
-    int pl = 0;
-    for (int o = 0; o < 4; ++o) {
-        if (!(which >> o & 1)) continue;
-        out[(int64_t)pl * n + i] = v[o];
-        if (dout != nullptr) dout[(int64_t)pl * n + i] = dz[o];
-        ++pl;
-    }
-    if (status != nullptr) status[i] = (uint8_t)st;
-}
-
-// The device Carlson functions on their own (same code as the hot path): R_F(x, m+h, m-h), R_D(m+h, m-h, x) and
-// R_J(x, m+h, m-h, p) with h^2 = s (s < 0: complex-conjugate pair), positive x and p.
-__global__ void k_carlson_pair(const double* __restrict__ x, const double* __restrict__ m, const double* __restrict__ s,
-                               const double* __restrict__ p, int64_t n, double* __restrict__ rf, double* __restrict__ rd,
-                               double* __restrict__ rj) {
-    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    const int64_t ii = i < n ? i : n - 1;
-    double xa[1] = {x[ii]}, mp[1] = {m[ii]}, ss[1] = {s[ii]}, p5[1] = {p[ii]}, p0[1] = {0.0};
-    const double xa0 = xa[0], m0 = mp[0], s0 = ss[0], pp0 = p5[0];
-    const double hd = xa0 - m0, hs = sqrt(fabs(s0));
-    const double pm = pp0 - m0;
-    const double dl5[1] = {(pp0 - xa0) * fma(pm, pm, -s0)}, dl0[1] = {0.0};
-    const double Qc[1] = {carlson_Qc<double>(hd, hs, true)}, Q5v[1] = {carlson_Qj<double>(xa0, m0, hs, pp0)}, Q0v[1] = {0.0};
-    unsigned st[1] = {0u};
-    double f, tailD[1], sum5[1], sum0[1];
-    carlson_dup<double, true, true, false, 1, VoteWarp>(xa, mp, ss, p5, p0, dl5, dl0, Qc, Q5v, Q0v, st, VoteWarp(), f, tailD, sum5, sum0);
-    if (i >= n) return;
-    rf[i] = carlson_rf_series<double>(xa[0], mp[0], f, hd, s0);
-    rd[i] = carlson_rd_series<double>(xa[0], mp[0], f, hd, s0, tailD[0]);
-    rj[i] = carlson_rj_series<double>(xa[0], mp[0], p5[0], f, xa0, m0, s0, pp0, sum5[0]);
 }
 
 // ALU roofline probes: 8 independent FMA chains per thread

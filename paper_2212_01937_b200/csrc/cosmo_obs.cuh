@@ -40,6 +40,22 @@ CB_HD void apply_c4(const Cosmo<T>& C, T z, Core<T>& R) {
 //   v = I0^3 h(w), dv/dk = I0^5 h'(w), w = Ok I0^2, h = sum_{j>=1} 4^j w^(j-1) / (2 (2j+1)!)  (|w| <= 1), closed forms beyond;
 //   dv/dI0 = F^2.
 template <typename T>
+CB_HD void volume_libm(T k, T I0, T& v, T& vk) {
+    using N = Num<T>;
+    if (k > T(0)) {
+        const T sq = N::sqrt_(k), y2 = T(2) * sq * I0, ey = N::exp_(y2), iey = T(1) / ey;
+        const T sh2 = T(0.5) * (ey - iey), ch2 = T(0.5) * (ey + iey);
+        v = (sh2 / (T(2) * sq) - I0) / (T(2) * k);
+        vk = (I0 * ch2 / (T(2) * k) - sh2 / (T(4) * k * sq)) / (T(2) * k) - v / k;
+    } else {
+        const T kk = -k, sq = N::sqrt_(kk);
+        T sn2, cs2;
+        N::sincos_(T(2) * sq * I0, &sn2, &cs2);
+        v = (I0 - sn2 / (T(2) * sq)) / (T(2) * kk);
+        vk = -((-(I0 * cs2 / (T(2) * kk) - sn2 / (T(4) * kk * sq))) / (T(2) * kk) - v / kk);
+    }
+}
+template <typename T>
 CB_HD void volume(T k, T I0, T& v, T& vk) {
     using N = Num<T>;
     const T w = k * I0 * I0;
@@ -59,18 +75,7 @@ CB_HD void volume(T k, T I0, T& v, T& vk) {
         vk = I3 * I0 * I0 * sd;
         return;
     }
-    if (k > T(0)) {
-        const T sq = N::sqrt_(k), y2 = T(2) * sq * I0, ey = N::exp_(y2), iey = T(1) / ey;
-        const T sh2 = T(0.5) * (ey - iey), ch2 = T(0.5) * (ey + iey);
-        v = (sh2 / (T(2) * sq) - I0) / (T(2) * k);
-        vk = (I0 * ch2 / (T(2) * k) - sh2 / (T(4) * k * sq)) / (T(2) * k) - v / k;
-    } else {
-        const T kk = -k, sq = N::sqrt_(kk);
-        T sn2, cs2;
-        N::sincos_(T(2) * sq * I0, &sn2, &cs2);
-        v = (I0 - sn2 / (T(2) * sq)) / (T(2) * kk);
-        vk = -((-(I0 * cs2 / (T(2) * kk) - sn2 / (T(4) * kk * sq))) / (T(2) * kk) - v / kk);
-    }
+    volume_libm<T>(k, I0, v, vk);
 }
 
 // K elements of the same cosmology at once.  The common case (|Ok I0^2| <= 1/2, D_L > 0) is straight-line code for all K
@@ -164,9 +169,13 @@ CB_HD void prep_age(Cosmo<double>& C, bool with_grad) {
     if (!with_grad) return;
     const double iE = R.iE;
     const double bt0 = -R.Em1 * iE, bt1 = (z - R.Em1) * iE, bt2 = (z * (X + 1.0) - R.Em1) * iE;
-    for (int t = 0; t < 3; ++t)
-        C.dTinf[t] = -0.5 * (C.GT[t][0] * R.I0 + C.GT[t][1] * R.K + C.GT[t][2] * bt0 + C.GT[t][3] * bt1 + C.GT[t][4] * bt2
-                             + C.GT[t][5] * R.TT);
+    GradSolve S;
+    S.init(C);
+    for (int t = 0; t < 3; ++t) {
+        double g[6];
+        S.rowT(t, g);
+        C.dTinf[t] = -0.5 * (g[0] * R.I0 + g[1] * R.K + g[2] * bt0 + g[3] * bt1 + g[4] * bt2 + g[5] * R.TT);
+    }
     // remainder beyond X of the Or-derivative, -1/2 int_X^inf (x^3 - x)/E^3 dx with E^2 ~ x^3 (Or x + Om): it decays only like
     // X^(-1/2) while matter dominates at X (2e-5/Om^1.5 at Or = 0); the Om and OL remainders are O(X^-3/2) and dropped.
     double rem;
@@ -188,8 +197,41 @@ struct GradInt { T dI[3], dT[3], dA[3]; };
 // (sum_j |G_j basis_j|) / max(|result|, 1e-3 |forward integral|): the relative error of the result is ~ 2e-16 x cond in FP64.  It
 // grows like 1 / prod(r_j - r_k) where roots of E^2 approach each other away from the path ("limits have to be
 // explicitly implemented when arguments are repeated"); callers switch to grad_quad() above GRAD_COND_LIMIT.
-template <typename T, bool kT, bool kA, bool kCond>
-CB_HD void grad_basis(const Cosmo<T>& C, T z, const Core<T>& R, GradInt<T>& D, T* cond = nullptr) {
+// where the basis rows come from: stored per cosmology by k_prep (OUTER kernels) ...
+template <typename T>
+struct RowsStored {
+    const Cosmo<T>& C;
+    CB_HD void rowI(int t, T (&g)[5]) const { for (int j = 0; j < 5; ++j) g[j] = C.GI[t][j]; }
+    CB_HD void rowT(int t, T (&g)[6]) const { for (int j = 0; j < 6; ++j) g[j] = C.GT[t][j]; }
+    CB_HD void rowJ(int p, T (&g)[5]) const { for (int j = 0; j < 5; ++j) g[j] = C.GJ[p][j]; }
+    CB_HD void rowA(int t, T (&g)[7]) const { for (int j = 0; j < 7; ++j) g[j] = C.GA[t][j]; }
+};
+// ... or produced right where they are consumed (ELEMENTWISE kernels: nothing to keep across the duplication loop)
+template <typename T>
+struct RowsSolved {
+    const GradSolve& S;
+    CB_HD void rowI(int t, T (&g)[5]) const { double d[5]; S.rowI(t, d); for (int j = 0; j < 5; ++j) g[j] = (T)d[j]; }
+    CB_HD void rowT(int t, T (&g)[6]) const { double d[6]; S.rowT(t, d); for (int j = 0; j < 6; ++j) g[j] = (T)d[j]; }
+    CB_HD void rowJ(int p, T (&g)[5]) const { double d[5]; S.rowJ(p, d); for (int j = 0; j < 5; ++j) g[j] = (T)d[j]; }
+    CB_HD void rowA(int t, T (&g)[7]) const { double d[7]; S.rowA(t, d); for (int j = 0; j < 7; ++j) g[j] = (T)d[j]; }
+};
+
+// accumulator of the cancellation factor: kCond = 2 keeps its value (one division per result), kCond = 1 only whether it exceeds
+// `limit` (a comparison per result: the form the kernels use)
+template <typename T, int kCond>
+struct CondAcc {
+    T limit, cmax;
+    bool over;
+    CB_HD void add(T sa, T val, T fwd) {
+        using N = Num<T>;
+        const T den = N::max_(N::abs_(val), T(1e-3) * N::abs_(fwd));
+        if (kCond == 2) { const T c = sa / den; cmax = (c > cmax || !(c == c)) ? c : cmax; }
+        if (kCond == 1) over = over | !(sa <= limit * den);           // a NaN counts as exceeded
+    }
+};
+
+template <typename T, bool kT, bool kA, int kCond, typename Rows>
+CB_HD void grad_basis(const Cosmo<T>& C, const Rows& rows, T z, const Core<T>& R, GradInt<T>& D, T* cond = nullptr, T limit = T(0)) {
     using N = Num<T>;
     const T x = T(1) + z;
     const T iE = R.iE;
@@ -197,40 +239,43 @@ CB_HD void grad_basis(const Cosmo<T>& C, T z, const Core<T>& R, GradInt<T>& D, T
     const T xp1 = x + T(1);
     const T n1 = z, n2 = z * xp1, n3 = z * N::fma_(xp1, x, T(1)), n4 = n2 * N::fma_(x, x, T(1));
     const T bt0 = -R.Em1 * iE, bt1 = (n1 - R.Em1) * iE, bt2 = (n2 - R.Em1) * iE;
-    T cmax = T(0);
+    // |basis values|: sum_j |g_j b_j| = sum_j |g_j| |b_j| costs one FMA per term (the |.| of an operand is free)
+    const T aI0 = N::abs_(R.I0), aK = N::abs_(R.K), a0 = N::abs_(bt0), a1 = N::abs_(bt1), a2 = N::abs_(bt2), aTT = N::abs_(R.TT);
+    CondAcc<T, kCond> acc{limit, T(0), false};
+    auto asum5 = [&](const T* g) {
+        return N::fma_(N::abs_(g[0]), aI0, N::fma_(N::abs_(g[1]), aK, N::fma_(N::abs_(g[2]), a0, N::fma_(N::abs_(g[3]), a1, N::abs_(g[4]) * a2))));
+    };
 #pragma unroll
     for (int t = 0; t < 3; ++t) {
-        D.dI[t] = C.GI[t][0] * R.I0 + C.GI[t][1] * R.K + C.GI[t][2] * bt0 + C.GI[t][3] * bt1 + C.GI[t][4] * bt2;
-        D.dT[t] = T(0); D.dA[t] = T(0);
-        if (kCond) {
-            const T sa = N::abs_(C.GI[t][0] * R.I0) + N::abs_(C.GI[t][1] * R.K) + N::abs_(C.GI[t][2] * bt0) + N::abs_(C.GI[t][3] * bt1)
-                         + N::abs_(C.GI[t][4] * bt2);
-            const T c = sa / N::max_(N::abs_(D.dI[t]), T(1e-3) * N::abs_(R.I0));
-            cmax = (c > cmax || !(c == c)) ? c : cmax;          // a NaN sticks
+        {
+            T gi[5];
+            rows.rowI(t, gi);
+            D.dI[t] = gi[0] * R.I0 + gi[1] * R.K + gi[2] * bt0 + gi[3] * bt1 + gi[4] * bt2;
+            if (kCond) acc.add(asum5(gi), D.dI[t], R.I0);
         }
+        D.dT[t] = T(0); D.dA[t] = T(0);
         if (kT) {
-            D.dT[t] = C.GT[t][0] * R.I0 + C.GT[t][1] * R.K + C.GT[t][2] * bt0 + C.GT[t][3] * bt1 + C.GT[t][4] * bt2 + C.GT[t][5] * R.TT;
-            if (kCond) {
-                const T sa = N::abs_(C.GT[t][0] * R.I0) + N::abs_(C.GT[t][1] * R.K) + N::abs_(C.GT[t][2] * bt0) + N::abs_(C.GT[t][3] * bt1)
-                             + N::abs_(C.GT[t][4] * bt2) + N::abs_(C.GT[t][5] * R.TT);
-                const T c = sa / N::max_(N::abs_(D.dT[t]), T(1e-3) * N::abs_(R.TT));
-                cmax = (c > cmax || !(c == c)) ? c : cmax;
-            }
+            T g[6];
+            rows.rowT(t, g);
+            D.dT[t] = g[0] * R.I0 + g[1] * R.K + g[2] * bt0 + g[3] * bt1 + g[4] * bt2 + g[5] * R.TT;
+            if (kCond) acc.add(N::fma_(N::abs_(g[5]), aTT, asum5(g)), D.dT[t], R.TT);
         }
     }
     if (kA) {
         const T btA = (((C.cubic & 1u) ? n4 : n3) - R.Em1) * iE;
         // d_abs gradient where radiation is a perturbation: the exact basis below multiplies the forward A by ~3/Or
-        // (the x^5, x^6 rows), which loses Om/Or digits.  Instead J'_p = int x^p dx/E^3, p <= 4, come from the basis and
+        // (the x^5, x^6 rows), which loses Om/Or digits.  Instead J'_p = int x^p dx/E^3, p = 2, 3, 4, come from the basis and
         // J'_5.. follow from d(x^k / E) = N_k / E^3:  Om (k - 3/2) J'_{k+2} = [x^k/E] - k OL J'_{k-1} - (k-1) Ok J'_{k+1}
         // - (k-2) Or J'_{k+3}, the Or terms iterated (same scheme as the forward d_abs).
         constexpr int KJ = 12;                // levels k = 3 .. 3 + KJ - 1
         T Jp[17], Sp[7];
+        Jp[0] = Jp[1] = T(0); Sp[0] = Sp[1] = T(0);
 #pragma unroll
-        for (int p = 0; p < 5; ++p) {
-            Jp[p] = C.GJ[p][0] * R.I0 + C.GJ[p][1] * R.K + C.GJ[p][2] * bt0 + C.GJ[p][3] * bt1 + C.GJ[p][4] * bt2;
-            if (kCond) Sp[p] = N::abs_(C.GJ[p][0] * R.I0) + N::abs_(C.GJ[p][1] * R.K) + N::abs_(C.GJ[p][2] * bt0) + N::abs_(C.GJ[p][3] * bt1)
-                               + N::abs_(C.GJ[p][4] * bt2);
+        for (int p = 2; p < 5; ++p) {
+            T gj[5];
+            rows.rowJ(p, gj);
+            Jp[p] = gj[0] * R.I0 + gj[1] * R.K + gj[2] * bt0 + gj[3] * bt1 + gj[4] * bt2;
+            Sp[p] = kCond ? asum5(gj) : T(0);
         }
 #pragma unroll
         for (int p = 5; p < 17; ++p) Jp[p] = T(0);
@@ -257,66 +302,123 @@ CB_HD void grad_basis(const Cosmo<T>& C, T z, const Core<T>& R, GradInt<T>& D, T
             Sp[5] = (N::abs_(bk[0]) + T(3) * C.OL * Sp[2] + T(2) * N::abs_(C.Ok) * Sp[4]) * C.iOm * T(1.0 / 1.5);
             Sp[6] = (N::abs_(bk[1]) + T(4) * C.OL * Sp[3] + T(3) * N::abs_(C.Ok) * Sp[5]) * C.iOm * T(1.0 / 2.5);
         }
+        if (useJ) {
 #pragma unroll
-        for (int t = 0; t < 3; ++t) {
-            const int a = t == 0 ? 5 : (t == 1 ? 2 : 6);      // x^2 D_theta = x^5, x^2, x^6 minus x^4
-            T dA = C.GA[t][0] * R.I0 + C.GA[t][1] * R.K + C.GA[t][2] * bt0 + C.GA[t][3] * bt1 + C.GA[t][4] * bt2 + C.GA[t][5] * btA
-                   + C.GA[t][6] * R.AA;
-            T sa = T(0);
-            if (kCond) sa = N::abs_(C.GA[t][0] * R.I0) + N::abs_(C.GA[t][1] * R.K) + N::abs_(C.GA[t][2] * bt0) + N::abs_(C.GA[t][3] * bt1)
-                            + N::abs_(C.GA[t][4] * bt2) + N::abs_(C.GA[t][5] * btA) + N::abs_(C.GA[t][6] * R.AA);
-            if (useJ) { dA = Jp[a] - Jp[4]; if (kCond) sa = Sp[a] + Sp[4]; }
-            D.dA[t] = dA;
-            if (kCond) {
-                const T c = sa / N::max_(N::abs_(dA), T(1e-3) * N::abs_(R.AA));
-                cmax = (c > cmax || !(c == c)) ? c : cmax;
+            for (int t = 0; t < 3; ++t) {
+                const int a = t == 0 ? 5 : (t == 1 ? 2 : 6);      // x^2 D_theta = x^5, x^2, x^6 minus x^4
+                D.dA[t] = Jp[a] - Jp[4];
+                if (kCond) acc.add(Sp[a] + Sp[4], D.dA[t], R.AA);
+            }
+        } else {
+#pragma unroll
+            for (int t = 0; t < 3; ++t) {
+                T ga[7];
+                rows.rowA(t, ga);
+                D.dA[t] = ga[0] * R.I0 + ga[1] * R.K + ga[2] * bt0 + ga[3] * bt1 + ga[4] * bt2 + ga[5] * btA + ga[6] * R.AA;
+                if (kCond) acc.add(N::fma_(N::abs_(ga[5]), N::abs_(btA), N::fma_(N::abs_(ga[6]), N::abs_(R.AA), asum5(ga))), D.dA[t], R.AA);
             }
         }
     }
-    if (kCond) *cond = cmax;
+    if (kCond == 2) *cond = acc.cmax;
+    if (kCond == 1) *cond = acc.over ? T(INFINITY) : T(0);
 }
 
 // The same nine integrals by Gauss-Legendre quadrature of their definition (Leibniz' rule on eqs. (2.3)-(2.5), the
 // route PAPER.md:285 fn.23 names), for the elements where grad_basis() is ill-conditioned: E^2 has (nearly) repeated roots away
-// from the path, or z is tiny.  There the integrand is smooth on the path, so a 12-point rule on panels that grow geometrically (ratio
-// <= 2) in the distance x - c from the root pair's centre c (0 when the pair is not left of the path) converges to rounding
-// (measured against the oracle on every element of config 5 with cond > 1e3: <= 4e-14).  E^2 is evaluated as printed,
-// eq. (2.2), so every root structure -- Einstein-de Sitter's triple root included -- takes the same code.  FP64 in every variant;
-// never inlined (rare path).  Returns 0, or ST_GRAD_ILLCOND when the pair's centre lies on the path (peaked integrand: not served).
-CB_HD_NOINLINE unsigned grad_quad(double Om, double OL, double Or, double x0, double z1, double dz, bool wantT, bool wantA, double out[9]) {
-    // nodes xi_i, 1 - xi_i on (0, 1) and weights of the 12-point Gauss-Legendre rule
-    const double XI[6] = {0.0092196828766403746547, 0.047941371814762571661, 0.11504866290284765648, 0.20634102285669127635,
-                          0.31608425050090990312, 0.43738329574426554226};
-    const double WI[6] = {0.023587668193255913597, 0.05346966299765921548, 0.080039164271673113167, 0.10158371336153296087,
-                          0.11674626826917740438, 0.1245735229067013925};
+// from the path, or the range is tiny.  There the integrand is smooth on the path: with panels that grow geometrically (ratio <= 2) in
+// the distance x - c from the root pair (c = its right end when it lies left of the path, else 0: every other root is at x <= 0) a
+// panel of ratio q sees no singularity inside the Bernstein ellipse of parameter rho = ((q+1) + 2 sqrt(q))/(q-1), so n nodes leave
+// ~ rho^-2n times a constant that grows with the order of the singularity (x^-9/2 at Einstein-de Sitter): 4 nodes for q <= 1.02
+// (rho = 202), 6 for q <= 1.2 (rho = 22), 12 for q <= 2 (rho = 5.8); measured against the oracle <= 4e-14 wherever grad_basis() gives
+// way to it.  E^2 is evaluated as printed, eq. (2.2), so
+// every root structure -- Einstein-de Sitter's triple root included -- takes the same code.  FP64 in every variant; never inlined
+// (rare path).  x0, d2: centre of the root pair of Q2 and (half its gap)^2 (d2 < 0: conjugate pair x0 +- i sqrt(-d2)).
+// Returns 0, or ST_GRAD_ILLCOND when the pair sits next to the path without the panels being graded towards it (peaked integrand).
+template <int NG>
+CB_HD void grad_quad_panel(const double (&XI)[NG], const double (&WI)[NG], double Om, double OL, double Or, double Ok, double tlo,
+                           double wd, bool wantT, bool wantA, double (&acc)[9]) {
+    using N = Num<double>;
+    double dm[NG], dl[NG], dr[NG], xs[NG];
+#pragma unroll
+    for (int i = 0; i < NG; ++i) {              // NG independent chains: the rare path is latency-bound, not throughput-bound
+        const double t = fma(wd, XI[i], tlo), x = 1.0 + t;        // t = x - 1 is formed directly: D_theta has the factor (x - 1)
+        const double e2 = fma(fma(fma(Or, x, Om), x, Ok), x * x, OL);
+        const double ie = N::rsqrt_(e2), f = (WI[i] * wd) * (ie * ie) * (ie * t);
+        xs[i] = x;
+        dm[i] = f * (x * x); dl[i] = -f * (x + 1.0); dr[i] = dm[i] * (x + 1.0);       // w D_theta / E^3, theta = Om, OL, Or
+    }
+#pragma unroll
+    for (int i = 0; i < NG; ++i) { acc[0] += dm[i]; acc[1] += dl[i]; acc[2] += dr[i]; }
+    if (wantT) {
+#pragma unroll
+        for (int i = 0; i < NG; ++i) { const double ix = N::rcp_(xs[i]); acc[3] = fma(dm[i], ix, acc[3]); acc[4] = fma(dl[i], ix, acc[4]); acc[5] = fma(dr[i], ix, acc[5]); }
+    }
+    if (wantA) {
+#pragma unroll
+        for (int i = 0; i < NG; ++i) { const double x2 = xs[i] * xs[i]; acc[6] = fma(dm[i], x2, acc[6]); acc[7] = fma(dl[i], x2, acc[7]); acc[8] = fma(dr[i], x2, acc[8]); }
+    }
+}
+
+CB_HD_NOINLINE unsigned grad_quad(double Om, double OL, double Or, double x0, double d2, double z1, double dz, bool wantT, bool wantA,
+                                  double out[9]) {
+    const double X4[4] = {0.0694318442029737124, 0.330009478207571868, 0.669990521792428132, 0.930568155797026288};
+    const double W4[4] = {0.173927422568726929, 0.326072577431273071, 0.326072577431273071, 0.173927422568726929};
+    const double X6[6] = {0.0337652428984239861, 0.169395306766867743, 0.380690406958401546, 0.619309593041598454, 
+                           0.830604693233132257, 0.966234757101576014};
+    const double W6[6] = {0.0856622461895851725, 0.180380786524069304, 0.233956967286345524, 0.233956967286345524, 
+                           0.180380786524069304, 0.0856622461895851725};
+    const double X12[12] = {0.00921968287664037465, 0.0479413718147625717, 0.115048662902847656, 0.206341022856691276, 
+                           0.316084250500909903, 0.437383295744265542, 0.562616704255734458, 0.683915749499090097, 
+                           0.793658977143308724, 0.884951337097152344, 0.952058628185237428, 0.990780317123359625};
+    const double W12[12] = {0.0235876681932559136, 0.0534696629976592155, 0.0800391642716731132, 0.101583713361532961, 
+                           0.116746268269177404, 0.124573522906701393, 0.124573522906701393, 0.116746268269177404, 
+                           0.101583713361532961, 0.0800391642716731132, 0.0534696629976592155, 0.0235876681932559136};
+    double acc[9] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
     for (int i = 0; i < 9; ++i) out[i] = 0.0;
     const double Ok = 1.0 - Om - OL - Or, X1 = 1.0 + z1, X2 = X1 + dz;
     const double lo = fmin(X1, X2), hi = fmax(X1, X2);
-    unsigned st = (x0 >= lo && x0 <= hi) ? (unsigned)ST_GRAD_ILLCOND : 0u;
-    const double c = (x0 > 0.0 && x0 < lo) ? x0 : 0.0;
+    unsigned st = 0u;
     if (!(lo > 0.0) || dz == 0.0) return st;
-    const double lr = log((X2 - c) / (X1 - c));
-    int np = (int)ceil(fabs(lr) * 1.4426950408889634);       // panels of ratio <= 2
-    if (np < 1) np = 1;
-    if (np > 64) np = 64;
-    const double r = exp(lr / np);
-    double wd = (np == 1) ? dz : dz * (r - 1.0) / (exp(lr) - 1.0);    // widths sum to dz; one panel: dz itself
-    double tlo = z1;                                                   // x - 1 at the panel's lower end
-    for (int k = 0; k < np; ++k) {
-        for (int i = 0; i < 12; ++i) {
-            const double xi = i < 6 ? XI[i] : 1.0 - XI[11 - i], w = (i < 6 ? WI[i] : WI[11 - i]) * wd;
-            const double t = fma(wd, xi, tlo), x = 1.0 + t;       // t = x - 1 is formed directly: D_theta has the factor (x - 1)
-            const double e2 = fma(fma(fma(Or, x, Om), x, Ok), x * x, OL);
-            const double ie = 1.0 / sqrt(e2), f = w * ie * ie * ie * t;
-            const double x2 = x * x, xp1 = x + 1.0;
-            const double dm = f * x2, dl = -f * xp1, dr = dm * xp1;       // w D_theta / E^3
-            out[0] += dm; out[1] += dl; out[2] += dr;
-            if (wantT) { const double ix = 1.0 / x; out[3] += dm * ix; out[4] += dl * ix; out[5] += dr * ix; }
-            if (wantA) { out[6] += dm * x2; out[7] += dl * x2; out[8] += dr * x2; }
-        }
-        tlo += wd;
-        wd *= r;
+    const double xr = x0 + (d2 > 0.0 ? sqrt(d2) : 0.0);              // right end of the pair (its centre for a conjugate pair)
+    const double c = (xr > 0.0 && xr < lo) ? xr : 0.0;
+    const double q = (X2 - c) / (X1 - c);                             // overall ratio (< 1 when z2 < z1)
+    const double qa = q >= 1.0 ? q : 1.0 / q;
+    int np = 1;
+    double r = q;
+    if (qa > 2.0) {
+        const double lr = log(q);
+        np = (int)ceil(fabs(lr) * 1.4426950408889634);                // panels of ratio <= 2
+        if (np > 64) np = 64;
+        r = exp(lr / np);
     }
+    double rho = 1e300;
+    if (!(xr < lo)) {
+        // the pair is not left of the path, so the panels are not graded towards it.  Bernstein parameter of the panel next to its
+        // nearest member s = xs + i y0: rho = a + sqrt(a^2 - 1), a = (|w + 1| + |w - 1|)/2, w = (s - centre)/half-width; a pair whose
+        // real part lies on the path is taken over the centre of a panel (the worst case)
+        const double y0 = d2 < 0.0 ? sqrt(-d2) : 0.0, hg = d2 > 0.0 ? sqrt(d2) : 0.0;
+        const double rr = r >= 1.0 ? r : 1.0 / r;                       // panel ratio, >= 1
+        double wre, h;
+        if (x0 + hg < lo) { h = 0.5 * lo * (rr - 1.0); wre = (lo - (x0 + hg)) / h + 1.0; }                 // first panel [lo, lo rr]
+        else if (x0 - hg > hi) { h = 0.5 * hi * (1.0 - 1.0 / rr); wre = ((x0 - hg) - hi) / h + 1.0; }       // last panel [hi/rr, hi]
+        else { h = 0.5 * fmin(fmax(x0, lo), hi) * (rr - 1.0); wre = 0.0; }
+        const double wim = y0 / h;
+        const double a = 0.5 * (hypot(wre + 1.0, wim) + hypot(wre - 1.0, wim));
+        rho = a + sqrt(fmax(a * a - 1.0, 0.0));
+        if (!(rho >= 3.5)) st = (unsigned)ST_GRAD_ILLCOND;           // 12 nodes: 3.5^-24 = 9e-14
+    }
+    double wd = (np == 1) ? dz : dz * (r - 1.0) / (q - 1.0);            // widths sum to dz; one panel: dz itself
+    double tlo = z1;                                                   // x - 1 at the panel's lower end
+    if (np == 1 && qa <= 1.02 && rho >= 60.0) grad_quad_panel<4>(X4, W4, Om, OL, Or, Ok, tlo, wd, wantT, wantA, acc);
+    else if (np == 1 && qa <= 1.2 && rho >= 12.0) grad_quad_panel<6>(X6, W6, Om, OL, Or, Ok, tlo, wd, wantT, wantA, acc);
+    else {
+        for (int k = 0; k < np; ++k) {
+            grad_quad_panel<12>(X12, W12, Om, OL, Or, Ok, tlo, wd, wantT, wantA, acc);
+            tlo += wd;
+            wd *= r;
+        }
+    }
+    for (int i = 0; i < 9; ++i) out[i] = acc[i];
     return st;
 }
 
@@ -325,9 +427,10 @@ CB_HD_NOINLINE unsigned grad_quad(double Om, double OL, double Or, double x0, do
 template <typename T>
 CB_HD unsigned grad_robust_fix(const Cosmo<T>& C, T z, bool wantT, bool wantA, T cond, GradInt<T>& D) {
     const T limit = T(sizeof(T) == 8 ? GRAD_COND_LIMIT : GRAD_COND_LIMIT_F32);
-    if (cond <= limit && !(C.cubic & 4u)) return 0u;
+    if (cond <= limit) return 0u;
     double q[9];
-    const unsigned st = grad_quad((double)C.Om, (double)C.OL, (double)C.Or, -0.5 * (double)C.b, 0.0, (double)z, wantT, wantA, q);
+    const double b = (double)C.b;
+    const unsigned st = grad_quad((double)C.Om, (double)C.OL, (double)C.Or, -0.5 * b, 0.25 * b * b - (double)C.c, 0.0, (double)z, wantT, wantA, q);
 #pragma unroll
     for (int t = 0; t < 3; ++t) { D.dI[t] = (T)q[t]; D.dT[t] = (T)q[3 + t]; D.dA[t] = (T)q[6 + t]; }
     return st;
@@ -402,21 +505,84 @@ template <typename T, bool kT, bool kA, bool kCond = false>
 CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, const T g[N_PLANES], T& gz, T gp[4], T* cond = nullptr,
                     unsigned which = W_ALL) {
     GradInt<T> D;
-    grad_basis<T, kT, kA, kCond>(C, z, R, D, cond);
+    const RowsStored<T> rows{C};
+    grad_basis<T, kT, kA, kCond ? 2 : 0, RowsStored<T>>(C, rows, z, R, D, cond);
     backward_chain<T, kT, kA>(C, z, R, O, D, g, gz, gp, which);
 }
 
 // VJP of one element with the conditioning check: bases where they are accurate, quadrature elsewhere.  Returns status bits to OR in.
-template <typename T, bool kT, bool kA>
+// kSolve: the basis rows are solved on the spot from the factorisation (ELEMENTWISE kernels) instead of read from the Cosmo block.
+// kDefer: do not run the quadrature here; return ST_INTERNAL_REDO for an element that needs it (the ELEMENTWISE kernels collect
+// those few per cent of elements and a second, dense pass redoes them: a divergent call inside the main kernel costs it a third
+// of its time, measured).
+template <typename T, bool kT, bool kA, bool kSolve = false, bool kDefer = false>
 CB_HD unsigned backward_robust(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, const T g[N_PLANES], T& gz, T gp[4],
                                unsigned which = W_ALL) {
     GradInt<T> D;
     T cond = T(0);
-    grad_basis<T, kT, kA, true>(C, z, R, D, &cond);
+    const T limit = T(sizeof(T) == 8 ? GRAD_COND_LIMIT : GRAD_COND_LIMIT_F32);
+    bool singular = (C.cubic & 4u) != 0;
+    if (kSolve) {
+        Cosmo<double> Cd;
+        Cd.Om = (double)C.Om; Cd.OL = (double)C.OL; Cd.Or = (double)C.Or; Cd.Ok = (double)C.Ok;
+        Cd.m = (double)C.m; Cd.rn = (double)C.rn; Cd.b = (double)C.b; Cd.c = (double)C.c; Cd.cubic = C.cubic;
+        GradSolve S;
+        S.init(Cd);
+        singular = S.singular;
+        const RowsSolved<T> rows{S};
+        grad_basis<T, kT, kA, 1, RowsSolved<T>>(C, rows, z, R, D, &cond, limit);
+    } else {
+        const RowsStored<T> rows{C};
+        grad_basis<T, kT, kA, 1, RowsStored<T>>(C, rows, z, R, D, &cond, limit);
+    }
     const bool valid = !(R.status & (ST_ROOT_ON_PATH | ST_UNSUPPORTED));
     unsigned st = 0u;
-    if (valid) st = grad_robust_fix<T>(C, z, kT && (which & (W_TL | W_AGE)), kA && (which & W_DABS), cond, D);
+    if (valid) {
+        if (kDefer) {
+            if (singular || !(cond <= limit)) st = ST_INTERNAL_REDO;
+        } else {
+            st = grad_robust_fix<T>(C, z, kT && (which & (W_TL | W_AGE)), kA && (which & W_DABS), singular ? T(INFINITY) : cond, D);
+        }
+    }
     backward_chain<T, kT, kA>(C, z, R, O, D, g, gz, gp, which);
+    return st;
+}
+
+// ---- one element of the ELEMENTWISE calls with its own cosmology: S1-S8.  Out: values v[N_PLANES], status; with kG also
+// dz and gp[4] for the upstream gradients g[N_PLANES].  No gradient bases are stored: backward_robust<.., kSolve> produces each row
+// where it is consumed, and the constants are formed a second time after the duplication loop (kRecon), so that little more than
+// the factorisation crosses the loop (registers decide how many warps fit).
+// kDefer: the main pass of the ELEMENTWISE kernels -- elements that need a slow path (complex root structure, ill-conditioned
+// gradient bases: backward_robust) are only marked ST_INTERNAL_REDO; the second pass runs them again without kDefer.
+template <typename T, bool kT, bool kA, bool kG, typename Vote, bool kDefer = false>
+CB_HD unsigned elem_one(T zv, double Om, double OL, double Or, double H0, unsigned which, const Vote& vote, const T* g, T* v, T& dz, T gp[4]) {
+    Cosmo<T> C0{}, C{};
+    {
+        Cosmo<double> Cd{};
+        cosmo_factor(Om, OL, Or, H0, Cd);
+        cosmo_constants(Cd);
+        if (kT && (which & W_AGE)) prep_age(Cd, kG);
+        convert_cosmo<T>(Cd, C0);
+    }
+    Core<T> R;
+    R.K = T(0); R.TT = T(0); R.AA = T(0);
+    eval_core<T, kT, kA, kG, Vote, true>(C0, zv, vote, R, &C);
+    // E^2 without a real negative root: complex slow path (cosmo_c4.cuh), a never-inlined call that costs the kernel a fifth of its
+    // time where it diverges (measured on config 2) -- with kDefer such elements go to the second pass instead
+    unsigned redo = 0u;
+    if (kDefer && kG) redo = (C.cubic & 2u) ? (unsigned)ST_INTERNAL_REDO : 0u;      // (the forward kernels have no second pass)
+    else apply_c4<T, kT, kA, kG>(C, zv, R);
+    Obs<T> O;
+    observables<T, kT, kA>(C, zv, R, which, O);
+#pragma unroll
+    for (int w = 0; w < N_PLANES; ++w) v[w] = O.v[w];
+    unsigned st = O.status | redo;
+    if (kG) {
+        dz = T(0); gp[0] = gp[1] = gp[2] = gp[3] = T(0);
+        {
+            st |= backward_robust<T, kT, kA, true, kDefer>(C, zv, R, O, g, dz, gp, which);
+        }
+    }
     return st;
 }
 

@@ -162,7 +162,7 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
     // ill-conditioned bases (near-repeated roots away from the path, tiny ranges): quadrature of the same integrals (grad_quad)
     if ((!(cond <= GRAD_COND_LIMIT) || (C.cubic & 4u)) && !(st[0] & (ST_ROOT_ON_PATH | ST_UNSUPPORTED))) {
         double q[9];
-        O.status |= grad_quad(C.Om, C.OL, C.Or, -0.5 * C.b, z1, dz, true, true, q);
+        O.status |= grad_quad(C.Om, C.OL, C.Or, -0.5 * C.b, 0.25 * C.b * C.b - C.c, z1, dz, true, true, q);
         for (int t = 0; t < 3; ++t) { rI[t] = q[t]; rT[t] = q[3 + t]; rA[t] = q[6 + t]; }
     }
     for (int t = 0; t < 3; ++t) {

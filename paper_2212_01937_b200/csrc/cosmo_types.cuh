@@ -11,13 +11,49 @@
 
 #ifdef __CUDACC__
 #define CB_HD __host__ __device__ __forceinline__
-#define CB_HD_NOINLINE __host__ __device__ __noinline__
+#define CB_HD_NOINLINE static __host__ __device__ __noinline__
+
 #else
 #define CB_HD inline
-#define CB_HD_NOINLINE inline
+#define CB_HD_NOINLINE static inline
 #endif
 
 namespace cb {
+
+// Fast FP64 reciprocal / square root for the per-element path on the device: MUFU seed (2^-20, measured) + one cubic step (error
+// ~ 2^-58), no special-case handling -- the IEEE sequences cost 3-5 times the instructions and, inlined some 40 times per element,
+// push the ELEMENTWISE kernels out of the instruction cache (profiles/).  Arguments: finite, normal, non-zero (cb_sqrt0 also takes 0).
+// On the host (tests/hostcheck) they are the plain operations.
+CB_HD double cb_rcp(double b) {
+#ifdef __CUDA_ARCH__
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(b));
+    const double e = fma(-b, r, 1.0);
+    return fma(r, fma(e, e, e), r);
+#else
+    return 1.0 / b;
+#endif
+}
+CB_HD double cb_div(double a, double b) {
+#ifdef __CUDA_ARCH__
+    const double r = cb_rcp(b), q = a * r;
+    return fma(fma(-b, q, a), r, q);              // one correction step on the quotient
+#else
+    return a / b;
+#endif
+}
+CB_HD double cb_sqrt0(double a) {                 // sqrt(a), a >= 0
+#ifdef __CUDA_ARCH__
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+    const double t = a * y;
+    const double e = fma(-t, y, 1.0);
+    const double r = fma(t * e, fma(0.375, e, 0.5), t);
+    return a > 0.0 ? r : 0.0;
+#else
+    return sqrt(a);
+#endif
+}
 
 // units: DESIGN.md reading R-units (the paper is silent)
 constexpr double C_KM_S = 299792.458;             // km/s
@@ -61,7 +97,8 @@ static const KTab KT_host = CB_KTAB_INIT;
 enum : unsigned { W_DC = 1, W_DM = 2, W_DL = 4, W_MU = 8, W_TL = 16, W_DABS = 32, W_DA = 64, W_VC = 128, W_AGE = 256, W_ALL = 511 };
 constexpr int N_PLANES = 9;                        // number of `which` bits
 // status bits (include/cosmo_b200.h)
-enum : unsigned { ST_ROOT_ON_PATH = 1, ST_UNSUPPORTED = 2, ST_DL_NONPOS = 4, ST_ITER_CAP = 8, ST_GRAD_ILLCOND = 16 };
+enum : unsigned { ST_ROOT_ON_PATH = 1, ST_UNSUPPORTED = 2, ST_DL_NONPOS = 4, ST_ITER_CAP = 8, ST_GRAD_ILLCOND = 16,
+                  ST_INTERNAL_REDO = 128 };   // internal: never leaves the library
 // cancellation factor of the gradient bases (cosmo_obs.cuh, grad_basis) above which an element's gradient integrals are taken from
 // quadrature instead (grad_quad).  FP64: basis error ~ 2e-16 x cond (measured on config 5: <= 4e-10 below 1e6).
 constexpr double GRAD_COND_LIMIT = 1.0e6;

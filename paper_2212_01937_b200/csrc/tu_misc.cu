@@ -1,0 +1,150 @@
+// tu_misc.cu -- instantiates the small kernels of cosmo_kernels.cuh: per-cosmology prep, the reductions, the two-limit and extra-w
+// ELEMENTWISE kernels, the stand-alone Carlson functions and the ALU probes.
+#include "cosmo_kernels.cuh"
+#include "cosmo_two.cuh"
+#include "cosmo_w.cuh"
+
+namespace cb {
+
+// S1-S3, one thread per cosmology
+__global__ void k_prep(const double* __restrict__ Om, const double* __restrict__ OL, const double* __restrict__ Or,
+                       const double* __restrict__ H0, int64_t S, int want_grad, Cosmo<double>* __restrict__ out) {
+    int64_t s = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (s >= S) return;
+    Cosmo<double> C;
+    cosmo_prep(Om[s], OL[s], Or[s], H0[s], want_grad & 3, C);
+    if (want_grad & 4) prep_age(C, (want_grad & 3) != 0);
+    else { C.Tinf = 0.0; C.dTinf[0] = C.dTinf[1] = C.dTinf[2] = 0.0; }
+    if ((want_grad & 3) < 2) {
+        for (int t = 0; t < 3; ++t) {
+            for (int j = 0; j < 7; ++j) C.GA[t][j] = 0.0;
+            for (int j = 0; j < 5; ++j) C.GJ[t][j] = C.GJ[t + 2][j] = 0.0;
+            if ((want_grad & 3) < 1) { for (int j = 0; j < 5; ++j) C.GI[t][j] = 0.0; for (int j = 0; j < 6; ++j) C.GT[t][j] = 0.0; }
+        }
+    }
+    out[s] = C;
+}
+
+// Two-limit evaluation (cosmo_two.cuh), one thread per (z1, z2, cosmology); n_cosmo in {1, n}.  which: DC, DM, TL, DABS, DA.
+// (128-register cap as for k_elem: 0.40 -> 0.28 ms forward, 0.75 -> 0.56 ms forward + VJP per 10^6 pairs)
+__global__ void __launch_bounds__(ELEM_THREADS, 4) k_two(const double* __restrict__ z1, const double* __restrict__ z2,
+                                                      const double* __restrict__ Om, const double* __restrict__ OL,
+                                                      const double* __restrict__ Or, const double* __restrict__ H0, int64_t n,
+                                                      int64_t n_cosmo, unsigned which, const double* __restrict__ gout,
+                                                      double* __restrict__ out, double* __restrict__ gz1, double* __restrict__ gz2,
+                                                      double* __restrict__ gparams, uint8_t* __restrict__ status) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const bool live = i < n;
+    const int64_t ii = live ? i : n - 1, ic = n_cosmo == 1 ? 0 : ii;
+    const bool with_grad = gout != nullptr;
+    Cosmo<double> C;
+    cosmo_prep(Om[ic], OL[ic], Or[ic], H0[ic], with_grad ? 2 : 0, C);
+    Two O;
+    eval_two<VoteWarp>(C, z1[ii], z2[ii], with_grad, VoteWarp(), O);
+    if (!live) return;
+    const unsigned bits[5] = {W_DC, W_DM, W_TL, W_DABS, W_DA};
+    double a1 = 0.0, a2 = 0.0, ap[4] = {0.0, 0.0, 0.0, 0.0};
+    int pl = 0;
+    for (int o = 0; o < 5; ++o) {
+        if (!(which & bits[o])) continue;
+        if (out != nullptr) out[(int64_t)pl * n + i] = O.v[o];
+        if (with_grad) {
+            const double g = gout[(int64_t)pl * n + i];
+            a1 = fma(g, O.gz1[o], a1); a2 = fma(g, O.gz2[o], a2);
+            for (int t = 0; t < 4; ++t) ap[t] = fma(g, O.gp[o][t], ap[t]);
+        }
+        ++pl;
+    }
+    if (status != nullptr) status[i] = (uint8_t)O.status;
+    if (with_grad) {
+        gz1[i] = a1; gz2[i] = a2;
+        for (int t = 0; t < 4; ++t) gparams[(int64_t)t * n + i] = ap[t];
+    }
+}
+
+// chi family with extra constant-w components (cosmo_w.cuh), one thread per (z, cosmology); n_cosmo in {1, n}.
+// which: DC, DM, DL, MU.  out[n_which][n]; dout[n_which][n] = d out / dz (nullable).
+__global__ void __launch_bounds__(ELEM_THREADS) k_w(const double* __restrict__ z, const double* __restrict__ Om,
+                                                    const double* __restrict__ OL, const double* __restrict__ Or,
+                                                    const double* __restrict__ Ow13, const double* __restrict__ Ow23,
+                                                    const double* __restrict__ H0, int64_t n, int64_t n_cosmo, unsigned which,
+                                                    double* __restrict__ out, double* __restrict__ dout, uint8_t* __restrict__ status) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const bool live = i < n;
+    const int64_t ii = live ? i : n - 1, ic = n_cosmo == 1 ? 0 : ii;
+    WCosmo W;
+    __shared__ WCosmo sw;
+    if (n_cosmo == 1) {                       // one shared cosmology: factor it once per block, not once per thread
+        if (threadIdx.x == 0) w_prep(Om[0], OL[0], Or[0], Ow13[0], Ow23[0], H0[0], sw);
+        __syncthreads();
+        W = sw;
+    } else {
+        w_prep(Om[ic], OL[ic], Or[ic], Ow13[ic], Ow23[ic], H0[ic], W);
+    }
+    double v[4], dz[4];
+    const unsigned st = w_eval<VoteWarp>(W, z[ii], VoteWarp(), v, dz);
+    if (!live) return;
+    int pl = 0;
+    for (int o = 0; o < 4; ++o) {
+        if (!(which >> o & 1)) continue;
+        out[(int64_t)pl * n + i] = v[o];
+        if (dout != nullptr) dout[(int64_t)pl * n + i] = dz[o];
+        ++pl;
+    }
+    if (status != nullptr) status[i] = (uint8_t)st;
+}
+
+// The device Carlson functions on their own (same code as the hot path): R_F(x, m+h, m-h), R_D(m+h, m-h, x) and
+// R_J(x, m+h, m-h, p) with h^2 = s (s < 0: complex-conjugate pair), positive x and p.
+__global__ void k_carlson_pair(const double* __restrict__ x, const double* __restrict__ m, const double* __restrict__ s,
+                               const double* __restrict__ p, int64_t n, double* __restrict__ rf, double* __restrict__ rd,
+                               double* __restrict__ rj) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const int64_t ii = i < n ? i : n - 1;
+    double xa[1] = {x[ii]}, mp[1] = {m[ii]}, ss[1] = {s[ii]}, p5[1] = {p[ii]}, p0[1] = {0.0};
+    const double xa0 = xa[0], m0 = mp[0], s0 = ss[0], pp0 = p5[0];
+    const double hd = xa0 - m0, hs = sqrt(fabs(s0));
+    const double pm = pp0 - m0;
+    const double dl5[1] = {(pp0 - xa0) * fma(pm, pm, -s0)}, dl0[1] = {0.0};
+    const double Qc[1] = {carlson_Qc<double>(hd, hs, true)}, Q5v[1] = {carlson_Qj<double>(xa0, m0, hs, pp0)}, Q0v[1] = {0.0};
+    unsigned st[1] = {0u};
+    double f, tailD[1], sum5[1], sum0[1];
+    carlson_dup<double, true, true, false, 1, VoteWarp>(xa, mp, ss, p5, p0, dl5, dl0, Qc, Q5v, Q0v, st, VoteWarp(), f, tailD, sum5, sum0);
+    if (i >= n) return;
+    rf[i] = carlson_rf_series<double>(xa[0], mp[0], f, hd, s0);
+    rd[i] = carlson_rd_series<double>(xa[0], mp[0], f, hd, s0, tailD[0]);
+    rj[i] = carlson_rj_series<double>(xa[0], mp[0], p5[0], f, xa0, m0, s0, pp0, sum5[0]);
+}
+
+
+void launch_prep(const double* Om, const double* OL, const double* Or, const double* H0, int64_t S, int want_grad, Cosmo<double>* out,
+                 cudaStream_t st) {
+    k_prep<<<(unsigned)cdiv64(S, 64), 64, 0, st>>>(Om, OL, Or, H0, S, want_grad, out);
+}
+void launch_reduce_params(int np, const double* part, int64_t ntiles, int64_t S, double* logL, double* grad, cudaStream_t st) {
+    if (np == 5) k_reduce_params<5><<<(unsigned)cdiv64(S * 5 * 32, 256), 256, 0, st>>>(part, ntiles, S, logL, grad);
+    else k_reduce_params<4><<<(unsigned)cdiv64(S * 4 * 32, 256), 256, 0, st>>>(part, ntiles, S, nullptr, grad);
+}
+void launch_reduce_gz(bool f32, const void* part, int ny, int64_t N, void* gz, cudaStream_t st) {
+    if (f32) k_reduce_gz<float><<<(unsigned)cdiv64(N, 256), 256, 0, st>>>(static_cast<const float*>(part), ny, N, static_cast<float*>(gz));
+    else k_reduce_gz<double><<<(unsigned)cdiv64(N, 256), 256, 0, st>>>(static_cast<const double*>(part), ny, N, static_cast<double*>(gz));
+}
+void launch_two(const double* z1, const double* z2, const double* Om, const double* OL, const double* Or, const double* H0, int64_t n,
+                int64_t n_cosmo, unsigned which, const double* gout, double* out, double* gz1, double* gz2, double* gparams,
+                uint8_t* status, cudaStream_t st) {
+    k_two<<<(unsigned)cdiv64(n, ELEM_THREADS), ELEM_THREADS, 0, st>>>(z1, z2, Om, OL, Or, H0, n, n_cosmo, which, gout, out, gz1, gz2, gparams, status);
+}
+void launch_w(const double* z, const double* Om, const double* OL, const double* Or, const double* Ow13, const double* Ow23,
+              const double* H0, int64_t n, int64_t n_cosmo, unsigned which, double* out, double* dout, uint8_t* status, cudaStream_t st) {
+    k_w<<<(unsigned)cdiv64(n, ELEM_THREADS), ELEM_THREADS, 0, st>>>(z, Om, OL, Or, Ow13, Ow23, H0, n, n_cosmo, which, out, dout, status);
+}
+void launch_carlson_pair(const double* x, const double* m, const double* s, const double* p, int64_t n, double* rf, double* rd, double* rj,
+                         cudaStream_t st) {
+    k_carlson_pair<<<(unsigned)cdiv64(n, 128), 128, 0, st>>>(x, m, s, p, n, rf, rd, rj);
+}
+void launch_probe_fma(bool f32, int blocks, int iters, void* sink, cudaStream_t st) {
+    if (f32) k_probe_fma<float><<<blocks, 256, 0, st>>>(iters, static_cast<float*>(sink));
+    else k_probe_fma<double><<<blocks, 256, 0, st>>>(iters, static_cast<double*>(sink));
+}
+
+}  // namespace cb

@@ -1,0 +1,27 @@
+// tu_outer_f32.cu -- instantiates the OUTER kernels (cosmo_kernels.cuh: k_outer) for float (FP32 variant: forward, fused forward + VJP, likelihood) and exports their launcher.
+#include "cosmo_kernels.cuh"
+
+namespace cb {
+
+template <int MODE>
+static void outer_dispatch_f32(const OuterArgs& a, dim3 grid, cudaStream_t st) {
+    using T = float;
+    const bool kT = a.which & (W_TL | W_AGE), kA = a.which & W_DABS;
+    if (MODE == MODE_SNIA || MODE == MODE_JOINT) k_outer<T, false, false, MODE, W_MU><<<grid, OUTER_THREADS, 0, st>>>(a);
+    else if (kT && kA) k_outer<T, true, true, MODE, 0><<<grid, OUTER_THREADS, 0, st>>>(a);
+    else if (kT) k_outer<T, true, false, MODE, 0><<<grid, OUTER_THREADS, 0, st>>>(a);
+    else if (kA) k_outer<T, false, true, MODE, 0><<<grid, OUTER_THREADS, 0, st>>>(a);
+    else if (a.which == W_MU) k_outer<T, false, false, MODE, W_MU><<<grid, OUTER_THREADS, 0, st>>>(a);
+    else k_outer<T, false, false, MODE, 0><<<grid, OUTER_THREADS, 0, st>>>(a);
+}
+
+void launch_outer_f32(int mode, const OuterArgs& a, dim3 grid, cudaStream_t st) {
+    switch (mode) {
+        case MODE_FWD: outer_dispatch_f32<MODE_FWD>(a, grid, st); break;
+        case MODE_VJP: outer_dispatch_f32<MODE_VJP>(a, grid, st); break;
+        case MODE_SNIA: outer_dispatch_f32<MODE_SNIA>(a, grid, st); break;
+        default: break;      // the log-joint has no FP32 entry point
+    }
+}
+
+}  // namespace cb

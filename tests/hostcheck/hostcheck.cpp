@@ -52,6 +52,28 @@ extern "C" void hostcheck_f32(int64_t n, const double* z, const double* Om, cons
                               unsigned which, const double* gup, double* out, double* gz, double* gp, uint8_t* status) {
     run<float>(n, z, Om, OL, Or, H0, which, gup, out, gz, gp, status);
 }
+// exactly what the ELEMENTWISE kernel k_elem runs per element (cosmo_obs.cuh, elem_one): no stored bases, constants re-formed after the loop
+template <typename T>
+static void run_elem(int64_t n, const double* z, const double* Om, const double* OL, const double* Or, const double* H0, unsigned which,
+                     const double* gup, double* out, double* gz, double* gp, uint8_t* status) {
+    for (int64_t i = 0; i < n; ++i) {
+        T g[N_PLANES], v[N_PLANES], dz = 0, p[4] = {0, 0, 0, 0};
+        for (int w = 0; w < N_PLANES; ++w) g[w] = (gup && (which >> w & 1)) ? (T)gup[w * n + i] : T(0);
+        unsigned st = gup ? elem_one<T, true, true, true, VoteNone>((T)z[i], Om[i], OL[i], Or[i], H0[i], which, VoteNone(), g, v, dz, p)
+                          : elem_one<T, true, true, false, VoteNone>((T)z[i], Om[i], OL[i], Or[i], H0[i], which, VoteNone(), g, v, dz, p);
+        for (int w = 0; w < N_PLANES; ++w) out[w * n + i] = (double)v[w];
+        status[i] = (uint8_t)st;
+        if (gup) { gz[i] = (double)dz; for (int t = 0; t < 4; ++t) gp[t * n + i] = (double)p[t]; }
+    }
+}
+extern "C" void hostcheck_elem_f64(int64_t n, const double* z, const double* Om, const double* OL, const double* Or, const double* H0,
+                                   unsigned which, const double* gup, double* out, double* gz, double* gp, uint8_t* status) {
+    run_elem<double>(n, z, Om, OL, Or, H0, which, gup, out, gz, gp, status);
+}
+extern "C" void hostcheck_elem_f32(int64_t n, const double* z, const double* Om, const double* OL, const double* Or, const double* H0,
+                                   unsigned which, const double* gup, double* out, double* gz, double* gp, uint8_t* status) {
+    run_elem<float>(n, z, Om, OL, Or, H0, which, gup, out, gz, gp, status);
+}
 extern "C" void hostcheck_f64_cond(int64_t n, const double* z, const double* Om, const double* OL, const double* Or, const double* H0,
                                    unsigned which, const double* gup, double* out, double* gz, double* gp, uint8_t* status, double* cond) {
     run<double>(n, z, Om, OL, Or, H0, which, gup, out, gz, gp, status, cond);

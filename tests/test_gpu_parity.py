@@ -1,14 +1,15 @@
 """GPU parity: the CUDA path (through the C ABI binding) against the oracle, element by element, on the same seeded
 inputs.  Tolerances are BASELINE.json's: FP64 values <= 1e-11, FP64 gradients <= 1e-8, FP32 <= 2e-5 (relative; the
-denominator of a gradient error is max(|ref|, 1e-3 |forward value|), reading R-tol).  Known, documented
-exceptions: d_abs at Or ~ 1e-5 (cancellation Om/Or inherent to eq. (3.9)),
-elements whose integral itself is ill-conditioned (loitering, antipode) and near-degenerate root pairs in gradients.
+denominator of a gradient error is max(|ref|, 1e-3 |forward value|), reading R-tol).  They are asserted as MAXIMA.  Rows
+whose result is ill-conditioned for any evaluation in that precision (loitering next to the no-Big-Bang boundary, D_M -> 0 at the
+antipode of a closed model) get the tolerance their conditioning allows, row by row (tests/tolerances.py), and are counted.
 """
 import numpy as np
 import pytest
 
 import oracle
 from paper_2212_01937_b200 import workloads as W
+import tolerances as TT
 
 pytestmark = pytest.mark.gpu
 
@@ -69,11 +70,14 @@ def test_golden_table(cb, goldens):
 
 # ---------------------------------------------------------------- config 2
 def test_config2_forward(cb):
-    w = W.config2(n=200_000)
+    """BASELINE.json config 2 at its full size (10^6 per-element cosmologies); oracle on a stride-16 sample plus every row whose
+    E^2 has no real negative root"""
+    w = W.config2()
     out, st = cb.cosmo_eval(dev(w.z), dev(w.Om), dev(w.OL), dev(w.Or), dev(w.H0), cb.ELEMENTWISE, w.which)
     out = out.cpu().numpy()
     st = st.cpu().numpy()[0]
     assert (st == 0).all()
+    assert np.isfinite(out).all()
     # rows whose E^2 has NO real negative root (two complex pairs, ~1e-4 of the config) take the complex slow path
     # (cosmo_c4.cuh): include every one of them in the comparison
     Ok = 1 - w.Om - w.OL - w.Or
@@ -82,7 +86,7 @@ def test_config2_forward(cb):
         t1 = np.where(disc > 0, (3 * w.Om + np.sqrt(np.abs(disc))) / (8 * w.Or), np.nan)
         gmin = w.Or * t1 ** 4 - w.Om * t1 ** 3 + Ok * t1 ** 2 + w.OL
     c4 = np.nonzero((disc <= 0) | (gmin > 0))[0]
-    assert len(c4) > 5
+    assert len(c4) > 50
     idx = np.union1d(np.arange(0, w.n_z, 16), c4)
     val, _, sto = oracle_batch(w.z[idx], w.Om[idx], w.OL[idx], w.Or[idx], w.H0[idx], False)
     assert (sto == 0).all()
@@ -127,36 +131,35 @@ def test_config3_small_full(cb, n, S):
 
 
 def test_config3_all_planes_outer(cb):
-    """OUTER VJP with every output plane (exercises the R_J tails and the T / d_abs gradient bases)"""
+    """OUTER VJP with every output plane (exercises the R_J tails and the T / d_abs gradient bases), d_abs gradients included"""
     w = W.config3(n=3000, S=3, which=("DC", "DM", "DL", "MU", "TL", "DABS"))
     gz, gp, out, st = cb.cosmo_vjp(dev(w.z), dev(w.Om), dev(w.OL), dev(w.Or), dev(w.H0), dev(w.grad_out), cb.OUTER, w.which,
                                    want_out=True)
     gz, gp, out = gz.cpu().numpy(), gp.cpu().numpy(), out.cpu().numpy()
-    gz_ref = np.zeros(w.n_z)
-    for s in range(3):
-        val, grad, _ = oracle_batch(w.z, w.Om[s:s + 1], w.OL[s:s + 1], w.Or[s:s + 1], w.H0[s:s + 1], True)
-        gp_ref = np.zeros(4)
-        gp_abs = np.zeros(4)
+    assert (st.cpu().numpy() == 0).all()
+    gz_ref = np.zeros(w.n_z); gz_abs = np.zeros(w.n_z)
+    for s_ in range(3):
+        val, grad, _ = oracle_batch(w.z, w.Om[s_:s_ + 1], w.OL[s_:s_ + 1], w.Or[s_:s_ + 1], w.H0[s_:s_ + 1], True)
+        gp_ref = np.zeros(4); gp_abs = np.zeros(4)
         for k, name in enumerate(w.which):
-            tol = TOL_VAL
-            assert relerr(out[k, s], val[:, OBS[name]]).max() <= tol, name
-            g = w.grad_out[k, s]
-            gz_ref += g * grad[:, OBS[name], 0]
-            if name == "DABS":
-                continue     # d(d_abs)/dOr: documented accuracy limit
-            for p in range(4):
-                gp_ref[p] += (g * grad[:, OBS[name], 1 + p]).sum()
-                gp_abs[p] += np.abs(g * grad[:, OBS[name], 1 + p]).sum()
-        # compare without the DABS plane: rerun is cheaper than subtracting
-    w2 = W.config3(n=3000, S=3, which=("DC", "DM", "DL", "MU", "TL"))
-    gz2, gp2, _, _ = cb.cosmo_vjp(dev(w2.z), dev(w2.Om), dev(w2.OL), dev(w2.Or), dev(w2.H0), dev(w2.grad_out), cb.OUTER, w2.which)
-    gp2 = gp2.cpu().numpy()
-    for s in range(3):
-        val, grad, _ = oracle_batch(w2.z, w2.Om[s:s + 1], w2.OL[s:s + 1], w2.Or[s:s + 1], w2.H0[s:s + 1], True)
-        for p in range(4):
-            terms = sum(w2.grad_out[k, s] * grad[:, OBS[name], 1 + p] for k, name in enumerate(w2.which))
-            abs_terms = sum(np.abs(w2.grad_out[k, s] * grad[:, OBS[name], 1 + p]) for k, name in enumerate(w2.which))
-            assert abs(gp2[p, s] - terms.sum()) <= TOL_GRAD * abs_terms.sum(), (s, p)
+            assert relerr(out[k, s_], val[:, OBS[name]]).max() <= TOL_VAL, name
+            g = w.grad_out[k, s_]
+            gz_ref += g * grad[:, OBS[name], 0]; gz_abs += np.abs(g * grad[:, OBS[name], 0])
+            for p_ in range(4):
+                gp_ref[p_] += (g * grad[:, OBS[name], 1 + p_]).sum()
+                gp_abs[p_] += np.abs(g * grad[:, OBS[name], 1 + p_]).sum()
+        assert (np.abs(gp[:, s_] - gp_ref) <= TOL_GRAD * gp_abs).all(), (s_, np.abs(gp[:, s_] - gp_ref) / gp_abs)
+    assert (np.abs(gz - gz_ref) <= TOL_GRAD * gz_abs).all()
+    # each plane on its own (one-hot upstream): the d_abs gradients are not hidden behind the larger chi-family terms
+    for k, name in enumerate(w.which):
+        g1 = np.zeros_like(w.grad_out); g1[k] = 1.0
+        _, gp1, _, _ = cb.cosmo_vjp(dev(w.z), dev(w.Om), dev(w.OL), dev(w.Or), dev(w.H0), dev(g1), cb.OUTER, w.which)
+        gp1 = gp1.cpu().numpy()
+        for s_ in range(3):
+            _, grad, _ = oracle_batch(w.z, w.Om[s_:s_ + 1], w.OL[s_:s_ + 1], w.Or[s_:s_ + 1], w.H0[s_:s_ + 1], True)
+            for p_ in range(4):
+                t = grad[:, OBS[name], 1 + p_]
+                assert abs(gp1[p_, s_] - t.sum()) <= TOL_GRAD * np.abs(t).sum(), (name, s_, p_)
 
 
 def test_config3_full_size_sampled(cb):
@@ -233,62 +236,68 @@ def test_config4_exact_data_gives_normalisation(cb):
 
 
 # ---------------------------------------------------------------- config 5 (stress) and edge cases
-def test_config5_forward_and_vjp(cb):
-    w = W.config5(n=120_000, n_struct=8000)
-    n = w.n_z
-    gz, gp, out, st = cb.cosmo_vjp(dev(w.z), dev(w.Om), dev(w.OL), dev(w.Or), dev(w.H0), dev(w.grad_out), cb.ELEMENTWISE, w.which,
-                                   want_out=True)
-    gz, gp, out, st = gz.cpu().numpy(), gp.cpu().numpy(), out.cpu().numpy(), st.cpu().numpy()[0]
-    idx = np.concatenate([np.arange(0, 120_000, 16), np.arange(120_000, n, 4)])
-    val, grad, sto = oracle_batch(w.z[idx], w.Om[idx], w.OL[idx], w.Or[idx], w.H0[idx], True)
-    assert (sto >= 0).all()
-    assert ((st[idx] & 3) == 0).all()
-    assert (((st[idx] & 4) != 0) == (sto == 1)).all()
-    rnd = idx < 120_000
+def _config5_checks(w, idx, out, st, grads_by_plane, val, grad, sto, label):
+    """values of all six planes and (when given) the five derivative columns of each plane, as MAXIMA against the per-row tolerance
+    (tests/tolerances.py); prints how many rows carry an inflated tolerance"""
+    z, Om, OL, Or, H0 = w.z[idx], w.Om[idx], w.OL[idx], w.Or[idx], w.H0[idx]
+    assert (sto >= 0).all() and ((st & 3) == 0).all()
+    assert (((st & 4) != 0) == (sto == 1)).all()
+    assert ((st & 24) == 0).all()                      # no iteration cap, no ill-conditioned-gradient flag anywhere
+    I0 = val[:, OBS["DC"]] / (299792.458 / H0)
+    tau, amp = TT.row_conditioning(z, Om, OL, Or, H0, I0, TOL_VAL)
+    n_loiter, n_anti = int((tau > TOL_VAL).sum()), int((amp > 10).sum())
+    print(f"[{label}] rows {len(idx)}: loitering (tolerance > 1e-11 on the integrals) {n_loiter}, |a cot a| > 10 {n_anti}")
+    blocks = w.extra["blocks"]
+    rnd = idx < blocks["random"][1]
+    assert (tau[rnd] == TOL_VAL).all()                 # the random block has no loitering rows: plain 1e-11 / 1e-8 there
     for k, name in enumerate(w.which):
         ref = val[:, OBS[name]]
         m = np.isfinite(ref)
-        e = relerr(out[k, 0, idx], ref)
-        if name in ("DC", "TL"):
-            assert e[m & rnd].max() <= TOL_VAL, (name, e[m & rnd].max())
-            # structured blocks include loitering rows whose integral is ill-conditioned by ~1/delta
-            assert e[m].max() <= 1e-9 and np.mean(e[m] <= TOL_VAL) > 0.995, name
-        elif name in ("DM", "DL", "MU"):
-            # D_M -> 0 at the antipode: bound the ABSOLUTE error by TOL x d_H-scale instead
-            scale = np.abs(val[:, OBS["DC"]]) if name != "MU" else np.ones_like(ref)
-            if name == "DL":
-                scale = scale * (1 + w.z[idx])
-            ae = np.abs(out[k, 0, idx] - ref)[m]
-            assert np.mean(ae <= 2e-11 * np.maximum(scale[m], np.abs(ref[m]))) > 0.995, name
-        else:
-            assert np.mean(e[m] <= 3e-11) > 0.9, name
-    # status bit 16 (gradient ill-conditioned: near-degenerate roots): rare on the random block, and
-    # every element WITHOUT it meets the gradient tolerance for the chi-family
-    assert np.mean((st[idx][rnd] & 16) != 0) < 0.02
-    g = w.grad_out[:, 0, idx]
-    mine = np.vstack([gz[idx][None], gp[:, idx]])
-    fin = np.isfinite(val).all(axis=1)
-    ref = np.zeros((5, len(idx)))
-    ref_abs = np.zeros((5, len(idx)))
-    for k, name in enumerate(w.which):
+        e = relerr(out[k], ref)
+        tol = TT.value_tolerance(name, tau, amp, val[:, OBS["MU"]])
+        assert (e[m] <= tol[m]).all(), (label, name, float((e[m] / tol[m]).max()))
+        if grads_by_plane is None:
+            continue
+        mine = grads_by_plane[name]                    # [5][rows]: d/dz, d/dOm, d/dOL, d/dOr, d/dH0
+        tg = TT.grad_tolerance(name, tau, amp, TOL_VAL, TOL_GRAD)
         for p in range(5):
-            t = g[k] * grad[:, OBS[name], p]
-            ref[p] += np.where(np.isfinite(t), t, 0.0)
-            ref_abs[p] += np.abs(np.where(np.isfinite(t), t, 0.0))
-    for p in (0, 4):    # d/dz and d/dH0 are closed-form: tight everywhere finite
-        e = np.abs(mine[p] - ref[p])[fin & rnd] / ref_abs[p][fin & rnd]
-        assert e.max() <= 1e-9, (p, e.max())
-    # chi-family parameter gradients alone (one-hot upstream on D_C), all blocks, unflagged elements
-    g1 = np.zeros_like(w.grad_out)
-    g1[0] = 1.0
-    _, gp1, _, st1 = cb.cosmo_vjp(dev(w.z), dev(w.Om), dev(w.OL), dev(w.Or), dev(w.H0), dev(g1), cb.ELEMENTWISE, w.which)
-    gp1, st1 = gp1.cpu().numpy()[:, idx], st1.cpu().numpy()[0][idx]
-    okm = fin & ((st1 & 16) == 0)
-    assert okm.mean() > 0.6
-    for p in range(3):
-        r = grad[:, OBS["DC"], 1 + p]
-        e = np.abs(gp1[p] - r) / np.maximum(np.abs(r), 1e-3 * np.abs(val[:, OBS["DC"]]))
-        assert e[okm].max() <= TOL_GRAD, (p, e[okm].max())
+            r = grad[:, OBS[name], p]
+            mm = m & np.isfinite(r)
+            eg = np.abs(mine[p] - r) / np.maximum(np.abs(r), 1e-3 * np.abs(ref))
+            assert np.isfinite(mine[p][mm]).all(), (label, name, p)
+            assert (eg[mm] <= tg[mm]).all(), (label, name, oracle.WRT[p], float((eg[mm] / tg[mm]).max()))
+
+
+def test_config5_forward_and_vjp(cb):
+    """config 5 at a size the oracle covers densely: all six planes, every derivative column of every plane (one-hot upstream per
+    plane), random AND structured rows (loitering, near-degenerate real pair, conjugate pair with Re x > 1)"""
+    w = W.config5(n=120_000, n_struct=8000)
+    n = w.n_z
+    a = [dev(x) for x in (w.z, w.Om, w.OL, w.Or, w.H0)]
+    idx = np.concatenate([np.arange(0, 120_000, 16), np.arange(120_000, n, 4)])
+    val, grad, sto = oracle_batch(w.z[idx], w.Om[idx], w.OL[idx], w.Or[idx], w.H0[idx], True)
+    by_plane = {}
+    out = st = None
+    for k, name in enumerate(w.which):
+        g1 = np.zeros_like(w.grad_out); g1[k] = 1.0
+        gz, gp, out, st = cb.cosmo_vjp(*a, dev(g1), cb.ELEMENTWISE, w.which, want_out=True)
+        by_plane[name] = np.vstack([gz.cpu().numpy()[None, idx], gp.cpu().numpy()[:, idx]])
+    out, st = out.cpu().numpy()[:, 0][:, idx], st.cpu().numpy()[0][idx]
+    _config5_checks(w, idx, out, st, by_plane, val, grad, sto, "config5 120k+24k")
+    # the forward-only call gives the same values
+    out_f, st_f = cb.cosmo_eval(*a, cb.ELEMENTWISE, w.which)
+    assert np.allclose(out_f.cpu().numpy()[:, 0][:, idx], out, rtol=1e-13, atol=0, equal_nan=True)
+    # a random upstream over all planes at once (the config's grad_out ~ N(0,1)): sums of the per-plane gradients
+    gz, gp, _, _ = cb.cosmo_vjp(*a, dev(w.grad_out), cb.ELEMENTWISE, w.which)
+    mine = np.vstack([gz.cpu().numpy()[None, idx], gp.cpu().numpy()[:, idx]])
+    fin = np.isfinite(val).all(axis=1)
+    I0 = val[:, OBS["DC"]] / (299792.458 / w.H0[idx])
+    tau, amp = TT.row_conditioning(w.z[idx], w.Om[idx], w.OL[idx], w.Or[idx], w.H0[idx], I0, TOL_VAL)
+    for p in range(5):
+        ref = sum(w.grad_out[k, 0, idx] * grad[:, OBS[nm], p] for k, nm in enumerate(w.which))
+        sab = sum(np.abs(w.grad_out[k, 0, idx] * grad[:, OBS[nm], p]) for k, nm in enumerate(w.which))
+        tg = TT.grad_tolerance("MU", tau, amp, TOL_VAL, TOL_GRAD)          # the loosest of the planes' row tolerances
+        assert (np.abs(mine[p] - ref)[fin] <= (tg * sab)[fin]).all(), p
 
 
 def test_empty_and_ragged(cb):
@@ -410,22 +419,84 @@ def test_two_complex_pairs_outer_and_likelihood(cb):
         assert (np.abs(gzl[s] - rgz) <= TOL_GRAD * np.maximum(np.abs(rgz), 1.0)).all(), s
 
 
-def test_vanishing_lambda_outer_flags_row(cb):
-    """OUTER VJP with one OL = 0 cosmology (Einstein-de Sitter-like: the gradient bases are singular): its row carries status
-    bit 16 and exact values; the other rows are clean and their gradients meet the tolerance"""
-    Om = np.array([0.3, 1.0, 0.28]); OL = np.array([0.7, 0.0, 0.65]); Or = np.array([9e-5, 0.0, 0.0]); H0 = np.array([70.0, 68.0, 72.0])
+def test_degenerate_cosmologies_outer_parity(cb):
+    """OUTER VJP with cosmologies whose root pair's gap has closed (OL = 0: Einstein-de Sitter, open and closed matter models, with
+    and without radiation; OL tiny): the gradient bases are singular there and the rows take the checked path with
+    quadrature of the Leibniz integrals.  All four parameter gradients meet the tolerance and nothing is flagged."""
+    Om = np.array([0.3, 1.0, 0.3, 1.4, 0.28, 0.3, 1.0 - 1e-7, 0.25]); OL = np.array([0.7, 0.0, 0.0, 0.0, 0.65, 1e-9, 1e-7, 0.0])
+    Or = np.array([9e-5, 0.0, 0.0, 0.0, 0.0, 9e-5, 0.0, 1e-3]); H0 = np.array([70.0, 68.0, 71.0, 66.0, 72.0, 70.0, 69.0, 73.0])
+    S = len(Om)
     z = np.linspace(0.01, 3.0, 777)
-    g = np.random.default_rng(4).standard_normal((1, 3, len(z)))
-    gz, gp, out, st = cb.cosmo_vjp(dev(z), dev(Om), dev(OL), dev(Or), dev(H0), dev(g), cb.OUTER, ("DC",), want_out=True)
-    gp, st, out = gp.cpu().numpy(), st.cpu().numpy(), out.cpu().numpy()
-    assert (st[1] == 16).all() and (st[[0, 2]] == 0).all()
+    rng = np.random.default_rng(4)
+    for which in (("DC",), ("MU",), ("DM", "TL", "DABS")):
+        g = rng.standard_normal((len(which), S, len(z)))
+        gz, gp, out, st = cb.cosmo_vjp(dev(z), dev(Om), dev(OL), dev(Or), dev(H0), dev(g), cb.OUTER, which, want_out=True)
+        gz, gp, st, out = gz.cpu().numpy(), gp.cpu().numpy(), st.cpu().numpy(), out.cpu().numpy()
+        assert (st == 0).all(), which
+        gz_ref = np.zeros(len(z)); gz_abs = np.zeros(len(z))
+        for s_ in range(S):
+            val, grad, _ = oracle_batch(z, Om[s_:s_ + 1], OL[s_:s_ + 1], Or[s_:s_ + 1], H0[s_:s_ + 1], True)
+            for p in range(4):
+                t = sum(g[k, s_] * grad[:, OBS[nm], 1 + p] for k, nm in enumerate(which))
+                ta = sum(np.abs(g[k, s_] * grad[:, OBS[nm], 1 + p]) for k, nm in enumerate(which))
+                assert abs(gp[p, s_] - t.sum()) <= TOL_GRAD * ta.sum(), (which, s_, p, abs(gp[p, s_] - t.sum()) / ta.sum())
+            for k, nm in enumerate(which):
+                assert relerr(out[k, s_], val[:, OBS[nm]]).max() <= TOL_VAL, (which, s_, nm)
+                gz_ref += g[k, s_] * grad[:, OBS[nm], 0]; gz_abs += np.abs(g[k, s_] * grad[:, OBS[nm], 0])
+        assert (np.abs(gz - gz_ref) <= TOL_GRAD * gz_abs).all()
     eds = 2.0 * (299792.458 / 68.0) * (1.0 - 1.0 / np.sqrt(1.0 + z))          # closed form, PAPER.md:233 context (EdS)
-    assert relerr(out[0, 1], eds).max() <= 1e-13
-    for s in (0, 2):
-        _, grad, _ = oracle_batch(z, Om[s:s + 1], OL[s:s + 1], Or[s:s + 1], H0[s:s + 1], True)
-        for p in range(4):
-            t = g[0, s] * grad[:, 0, 1 + p]
-            assert abs(gp[p, s] - t.sum()) <= TOL_GRAD * np.abs(t).sum(), (s, p)
+    o, _ = cb.cosmo_eval(dev(z), dev(Om[1:2]), dev(OL[1:2]), dev(Or[1:2]), dev(H0[1:2]), cb.ELEMENTWISE, ("DC",))
+    assert relerr(o[0, 0].cpu().numpy(), eds).max() <= 1e-13
+    # the same cosmologies, element by element (ELEMENTWISE kernel), every derivative column of every plane
+    zz = np.tile(z[::7], S); rep = lambda v: np.repeat(v, len(z[::7]))
+    which = ("DC", "DM", "MU", "TL", "DABS")
+    val, grad, _ = oracle_batch(zz, rep(Om), rep(OL), rep(Or), rep(H0), True)
+    for k, nm in enumerate(which):
+        g1 = np.zeros((len(which), 1, len(zz))); g1[k] = 1.0
+        gz, gp, out, st = cb.cosmo_vjp(dev(zz), dev(rep(Om)), dev(rep(OL)), dev(rep(Or)), dev(rep(H0)), dev(g1), cb.ELEMENTWISE, which)
+        assert (st.cpu().numpy() == 0).all()
+        mine = np.vstack([gz.cpu().numpy()[None], gp.cpu().numpy()])
+        for p in range(5):
+            r = grad[:, OBS[nm], p]
+            e = np.abs(mine[p] - r) / np.maximum(np.abs(r), 1e-3 * np.abs(val[:, OBS[nm]]))
+            assert e.max() <= TOL_GRAD, (nm, p, e.max())
+
+
+@pytest.mark.parametrize("mode", ["outer", "elementwise"])
+def test_vjp_at_z_zero(cb, mode):
+    """z = 0 among the redshifts: the integrals vanish, D_M = 0, mu is undefined there (status 4) -- and the gradients of the other
+    planes are the integrands at z = 0, finite, without poisoning the sums of the row (0 x inf)"""
+    z = np.array([0.0, 0.3, 0.0, 1.2, 2.0])
+    which = ("DC", "DM", "TL", "DABS", "DA", "AGE")
+    rng = np.random.default_rng(8)
+    if mode == "outer":
+        Om = np.array([0.3, 0.27]); OL = np.array([0.7, 0.6]); Or = np.array([9e-5, 0.0]); H0 = np.array([70.0, 66.0])
+        g = rng.standard_normal((len(which), 2, len(z)))
+        gz, gp, out, st = cb.cosmo_vjp(dev(z), dev(Om), dev(OL), dev(Or), dev(H0), dev(g), cb.OUTER, which, want_out=True)
+        rows = [(s_, slice(None)) for s_ in range(2)]
+        zz, pp = [z, z], [(Om[s_:s_ + 1], OL[s_:s_ + 1], Or[s_:s_ + 1], H0[s_:s_ + 1]) for s_ in range(2)]
+    else:
+        Om = np.full(5, 0.3); OL = np.full(5, 0.7); Or = np.array([0.0, 9e-5, 9e-5, 0.0, 1e-3]); H0 = np.full(5, 70.0)
+        g = rng.standard_normal((len(which), 1, len(z)))
+        gz, gp, out, st = cb.cosmo_vjp(dev(z), dev(Om), dev(OL), dev(Or), dev(H0), dev(g), cb.ELEMENTWISE, which, want_out=True)
+        zz, pp = [z], [(Om, OL, Or, H0)]
+    gz, gp, out, st = gz.cpu().numpy(), gp.cpu().numpy(), out.cpu().numpy(), st.cpu().numpy()
+    assert np.isfinite(gz).all() and np.isfinite(gp).all() and (st == 0).all()
+    assert (out[:5, :, [0, 2]] == 0).all()
+    gz_ref = np.zeros(len(z))
+    for r, (zr, pr) in enumerate(zip(zz, pp)):
+        val, grad, _ = oracle_batch(zr, *pr, True)
+        dv, dg, _ = oracle.derived_batch(zr, *pr)
+        dv, dg = dv.astype(np.float64), dg.astype(np.float64)
+        refs = [grad[:, 0], grad[:, 1], grad[:, 4], grad[:, 5], dg[:, 0], dg[:, 2]]
+        gz_ref += sum(g[k, r] * refs[k][:, 0] for k in range(len(which)))
+        gp_ref = np.stack([sum(g[k, r] * refs[k][:, 1 + p] for k in range(len(which))) for p in range(4)])
+        gp_abs = np.stack([sum(np.abs(g[k, r] * refs[k][:, 1 + p]) for k in range(len(which))) for p in range(4)])
+        if mode == "outer":
+            assert (np.abs(gp[:, r] - gp_ref.sum(axis=1)) <= TOL_GRAD * gp_abs.sum(axis=1)).all(), r
+        else:
+            assert (np.abs(gp - gp_ref) <= TOL_GRAD * np.maximum(gp_abs, 1e-300)).all()
+    assert np.allclose(gz, gz_ref, rtol=1e-9, atol=0)
 
 
 # ---------------------------------------------------------------- full sizes of configs 4 and 5 (sampled oracle + properties)
@@ -456,41 +527,46 @@ def test_config4_full_size_sampled(cb):
 
 
 def test_config5_full_size_sampled(cb):
-    """BASELINE.json config 5 at full size (10^7 + 3 x 10^5 rows, all six outputs, forward + VJP); oracle on a sample"""
+    """BASELINE.json config 5 at full size (10^7 + 3 x 10^5 rows, all six outputs, forward + VJP); oracle on a sample of the random
+    block and of every structured block; values and gradients as maxima against the per-row tolerances"""
     import torch
     w = W.config5()
     n = w.n_z
-    g = torch.randn((6, 1, n), dtype=torch.float64, device="cuda", generator=torch.Generator("cuda").manual_seed(5))
-    gz, gp, out, st = cb.cosmo_vjp(dev(w.z), dev(w.Om), dev(w.OL), dev(w.Or), dev(w.H0), g, cb.ELEMENTWISE, w.which, want_out=True)
-    st = st[0]
-    assert int(((st & 3) != 0).sum()) == 0            # every row is a valid cosmology
+    a = [dev(x) for x in (w.z, w.Om, w.OL, w.Or, w.H0)]
     rng = np.random.default_rng(55)
     idx = np.sort(np.concatenate([rng.choice(10_000_000, 6000, replace=False), 10_000_000 + rng.choice(300_000, 3000, replace=False)]))
     ti = torch.from_numpy(idx).cuda()
-    o = out[:, 0, :][:, ti].cpu().numpy()
-    s_ = st[ti].cpu().numpy()
     val, grad, sto = oracle_batch(w.z[idx], w.Om[idx], w.OL[idx], w.Or[idx], w.H0[idx], True)
-    assert (sto >= 0).all() and (((s_ & 4) != 0) == (sto == 1)).all()
-    rnd = idx < 10_000_000
-    for k, name in enumerate(w.which):
-        ref = val[:, OBS[name]]
-        m = np.isfinite(ref) & rnd
-        if name in ("DC", "TL", "DABS"):
-            e = relerr(o[k], ref)[m]
-            assert np.mean(e <= TOL_VAL) > 0.998 and e.max() <= 1e-9, (name, e.max())
-        else:
-            scale = np.abs(val[:, OBS["DC"]]) * ((1 + w.z[idx]) if name == "DL" else 1.0) if name != "MU" else np.ones_like(ref)
-            ae = np.abs(o[k] - ref)[m]
-            assert np.mean(ae <= 2e-11 * np.maximum(scale[m], np.abs(ref[m]))) > 0.995, name
-    # closed-form gradients (d/dz, d/dH0) on the sampled random rows
+    # one-hot upstream on D_C and on d_abs (the extremes of the gradient bases), then the config's random upstream
+    by_plane = {}
+    for name in ("DC", "DABS"):
+        g1 = torch.zeros((6, 1, n), dtype=torch.float64, device="cuda")
+        g1[w.which.index(name)] = 1.0
+        gz, gp, out, st = cb.cosmo_vjp(*a, g1, cb.ELEMENTWISE, w.which, want_out=True)
+        by_plane[name] = np.vstack([gz[ti].cpu().numpy()[None], gp[:, ti].cpu().numpy()])
+        assert int(((st[0] & 3) != 0).sum()) == 0            # every row is a valid cosmology
+        assert int(((st[0] & 24) != 0).sum()) == 0           # nothing flagged, anywhere in the 1.03e7 rows
+    o = out[:, 0, :][:, ti].cpu().numpy()
+    s_ = st[0][ti].cpu().numpy()
+    sub = type("W", (), {})()
+    sub.z, sub.Om, sub.OL, sub.Or, sub.H0, sub.extra = w.z, w.Om, w.OL, w.Or, w.H0, w.extra
+    for name in ("DC", "DABS"):
+        sub.which = (name,)
+        _config5_checks(sub, idx, o[[w.which.index(name)]], s_, {name: by_plane[name]}, val, grad, sto, f"config5 full size, d {name}")
+    sub.which = w.which
+    _config5_checks(sub, idx, o, s_, None, val, grad, sto, "config5 full size, values")
+    g = torch.randn((6, 1, n), dtype=torch.float64, device="cuda", generator=torch.Generator("cuda").manual_seed(5))
+    gz, gp, _, _ = cb.cosmo_vjp(*a, g, cb.ELEMENTWISE, w.which)
     gs = g[:, 0, :][:, ti].cpu().numpy()
-    fin = np.isfinite(val).all(axis=1) & rnd
-    for p, mine in ((0, gz[ti].cpu().numpy()), (4, gp[3][ti].cpu().numpy())):
-        ref = np.zeros(len(idx)); ref_abs = np.zeros(len(idx))
-        for k, name in enumerate(w.which):
-            t = gs[k] * grad[:, OBS[name], p]
-            ref += np.where(np.isfinite(t), t, 0.0); ref_abs += np.abs(np.where(np.isfinite(t), t, 0.0))
-        assert (np.abs(mine - ref)[fin] <= 1e-9 * ref_abs[fin]).all(), p
+    mine = np.vstack([gz[ti].cpu().numpy()[None], gp[:, ti].cpu().numpy()])
+    fin = np.isfinite(val).all(axis=1)
+    I0 = val[:, OBS["DC"]] / (299792.458 / w.H0[idx])
+    tau, amp = TT.row_conditioning(w.z[idx], w.Om[idx], w.OL[idx], w.Or[idx], w.H0[idx], I0, TOL_VAL)
+    tg = TT.grad_tolerance("MU", tau, amp, TOL_VAL, TOL_GRAD)
+    for p in range(5):
+        ref = sum(gs[k] * grad[:, OBS[nm], p] for k, nm in enumerate(w.which))
+        sab = sum(np.abs(gs[k] * grad[:, OBS[nm], p]) for k, nm in enumerate(w.which))
+        assert (np.abs(mine[p] - ref)[fin] <= (tg * sab)[fin]).all(), p
 
 
 # ---------------------------------------------------------------- OUTER and ELEMENTWISE are the same arithmetic
@@ -644,7 +720,7 @@ def test_two_limit(cb):
     for c in range(6):
         ref = sum(g[k, idx] * gr[:, o, c] for k, o in enumerate(order))
         sab = sum(np.abs(g[k, idx] * gr[:, o, c]) for k, o in enumerate(order))
-        assert (np.abs(mine[c] - ref) <= (5e-8 if c == 4 else TOL_GRAD) * sab).all(), c
+        assert (np.abs(mine[c] - ref) <= TOL_GRAD * sab).all(), c
     # one cosmology for all pairs, forward only; z1 = 0 reproduces the one-limit call
     p = [dev(np.array([v_])) for v_ in (0.3, 0.7, 9e-5, 70.0)]
     o2, *_ = cb.cosmo_eval2(dev(np.zeros(1000)), dev(z2[:1000]), *p, ("DC", "TL"))
@@ -673,7 +749,7 @@ def test_two_limit_two_complex_pairs(cb):
     for c in range(6):
         ref = sum(g[k] * gr[:, o, c] for k, o in enumerate(order))
         sab = sum(np.abs(g[k] * gr[:, o, c]) for k, o in enumerate(order))
-        assert (np.abs(mine[c] - ref) <= (2e-7 if c == 4 else TOL_GRAD) * sab).all(), c
+        assert (np.abs(mine[c] - ref) <= TOL_GRAD * sab).all(), c
 
 
 # ---------------------------------------------------------------- extra constant-w components (PAPER.md:82 fn.4)
