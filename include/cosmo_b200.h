@@ -66,7 +66,8 @@ enum {
  * (reading R-fp32). */
 typedef struct { const double *Om, *OL, *Or, *H0; } cosmo_params;
 
-/* Bytes of scratch the calls below need (device memory, 256-byte aligned, contents undefined on entry and exit). */
+/* Bytes of scratch the calls below need (device memory, 256-byte aligned, contents undefined on entry and exit).  ELEMENTWISE calls
+ * with one cosmology per redshift need none for the forward and a work list of n_z 32-bit indices for the VJP (n_z < 2^32). */
 size_t cosmo_workspace_bytes(int64_t n_z, int64_t n_cosmo, int mode, uint32_t which, int with_grad);
 
 /* Forward.  z[n_z]; out[n_which][rows][n_z]; status: nullable, [rows][n_z] bytes. */
@@ -120,9 +121,13 @@ int cosmo_eval_host(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosm
  * (z1[i], z2[i], cosmology) per element; n_cosmo in {1, n}.  `which` may hold COSMO_DC (comoving distance between z1 and z2),
  * COSMO_DM (transverse distance between them, d_H sinn(...)), COSMO_TL (t(z1,z2)), COSMO_DABS, COSMO_DA (= D_M12/(1+z2));
  * planes out[n_which][n] in ascending bit order.  grad_out == NULL: forward (out required).  Otherwise also the VJP:
- * grad_z1[n], grad_z2[n], grad_params[4][n] (per element, order Om, OL, Or, H0; out nullable).  status as above. */
+ * grad_z1[n], grad_z2[n], grad_params[4][n] (per element, order Om, OL, Or, H0; out nullable).  status as above.
+ * workspace: cosmo_eval2_workspace_bytes(n, grad_out != NULL) bytes of device scratch. */
 int cosmo_eval2(const double* z1, const double* z2, int64_t n, cosmo_params p, int64_t n_cosmo, uint32_t which, const double* grad_out,
-                double* out, double* grad_z1, double* grad_z2, double* grad_params, uint8_t* status, void* stream);
+                double* out, double* grad_z1, double* grad_z2, double* grad_params, uint8_t* status, void* workspace, size_t ws_bytes,
+                void* stream);
+/* scratch of cosmo_eval2: 0 for the forward call (workspace may be NULL), a work list of up to n indices with the VJP (n < 2^32) */
+size_t cosmo_eval2_workspace_bytes(int64_t n, int with_grad);
 
 /* EXTRA CONSTANT-w COMPONENTS (PAPER.md:82 fn.4: E^2 must be a polynomial of degree <= 4, which admits w in
  * {-1, -2/3, -1/3, 0, 1/3}):  E^2(x) = Or x^4 + Om x^3 + (Ok + Ow13) x^2 + Ow23 x + OL with Ok = 1 - Om - OL - Or - Ow13 - Ow23

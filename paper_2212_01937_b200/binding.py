@@ -18,7 +18,7 @@ WHICH_BITS = {"DC": DC, "DM": DM, "DL": DL, "MU": MU, "TL": TL, "DABS": DABS, "D
 WHICH_ORDER = ("DC", "DM", "DL", "MU", "TL", "DABS", "DA", "VC", "AGE")
 
 # every symbol include/cosmo_b200.h and include/cosmo_b200_diag.h declare
-SYMBOLS = ("cosmo_host_release", "cosmo_workspace_bytes", "cosmo_eval", "cosmo_vjp", "cosmo_snia_loglike", "cosmo_eval_f32", "cosmo_vjp_f32",
+SYMBOLS = ("cosmo_host_release", "cosmo_eval2_workspace_bytes", "cosmo_workspace_bytes", "cosmo_eval", "cosmo_vjp", "cosmo_snia_loglike", "cosmo_eval_f32", "cosmo_vjp_f32",
            "cosmo_snia_loglike_f32", "cosmo_snia_logjoint", "cosmo_eval2", "cosmo_eval_w", "cosmo_eval_host", "cosmo_carlson_pair", "cosmo_probe_fma_f64", "cosmo_probe_fma_f32",
            "cosmo_profile", "cosmo_profile_mean_ms",
            "cosmo_launch_count", "cosmo_last_cuda_error", "cosmo_strerror", "cosmo_version")
@@ -67,7 +67,9 @@ def lib():
         f.restype = ci
     L.cosmo_snia_logjoint.argtypes = [vp, vp, vp, vp, C.c_double, C.c_double, C.c_double, i64, CosmoParams, i64, vp, vp, vp, vp, sz, vp]
     L.cosmo_snia_logjoint.restype = ci
-    L.cosmo_eval2.argtypes = [vp, vp, i64, CosmoParams, i64, u32, vp, vp, vp, vp, vp, vp, vp]
+    L.cosmo_eval2.argtypes = [vp, vp, i64, CosmoParams, i64, u32, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    L.cosmo_eval2_workspace_bytes.argtypes = [i64, ci]
+    L.cosmo_eval2_workspace_bytes.restype = sz
     L.cosmo_eval2.restype = ci
     L.cosmo_eval_w.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, i64, u32, vp, vp, vp, vp]
     L.cosmo_eval_w.restype = ci
@@ -240,7 +242,7 @@ def cosmo_snia_logjoint(z, z_obs, mu_obs, sigma_mu, sigma_z, beta, shape, Om, OL
     return logp, grad, gz
 
 
-def cosmo_eval2(z1, z2, Om, OL, Or, H0, which=("DC",), grad_out=None, want_out=True):
+def cosmo_eval2(z1, z2, Om, OL, Or, H0, which=("DC",), grad_out=None, want_out=True, workspace=None):
     """Two-limit forms between z1 and z2 (elementwise).  Returns (out[n_which, n] or None, grad_z1, grad_z2, grad_params[4, n], status);
     the gradients are None without grad_out.  which from DC, DM, TL, DABS, DA."""
     torch = _torch()
@@ -257,8 +259,10 @@ def cosmo_eval2(z1, z2, Om, OL, Or, H0, which=("DC",), grad_out=None, want_out=T
         g1 = torch.empty(n, dtype=torch.float64, device=z1.device)
         g2 = torch.empty(n, dtype=torch.float64, device=z1.device)
         gp = torch.empty((4, n), dtype=torch.float64, device=z1.device)
+    ws_b = int(lib().cosmo_eval2_workspace_bytes(n, int(grad_out is not None)))
+    ws = _workspace(torch, ws_b, z1.device, workspace) if ws_b else None
     _check(lib().cosmo_eval2(_ptr(z1), _ptr(z2), n, P, n_cosmo, mask, _ptr(grad_out), _ptr(out), _ptr(g1), _ptr(g2), _ptr(gp), _ptr(status),
-                             _stream(torch)))
+                             _ptr(ws), ws_b, _stream(torch)))
     return out, g1, g2, gp, status
 
 

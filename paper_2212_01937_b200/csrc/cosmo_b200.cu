@@ -255,6 +255,11 @@ cudaEvent_t g_host_ev = nullptr;
 
 extern "C" {
 
+size_t cosmo_eval2_workspace_bytes(int64_t n, int with_grad) {
+    if (n < 0 || !with_grad) return 0;
+    return 256 + align256((size_t)(n > 0 ? n : 1) * sizeof(unsigned));       // counter + work list of the second pass
+}
+
 size_t cosmo_workspace_bytes(int64_t n_z, int64_t n_cosmo, int mode, uint32_t which, int with_grad) {
     if (n_z < 0 || n_cosmo < 0) return 0;
     WsLayout L = ws_layout(n_z, n_cosmo, mode, which, with_grad, sizeof(double));
@@ -410,16 +415,24 @@ void cosmo_host_release(void) {
 }
 
 int cosmo_eval2(const double* z1, const double* z2, int64_t n, cosmo_params p, int64_t n_cosmo, uint32_t which, const double* grad_out,
-                double* out, double* grad_z1, double* grad_z2, double* grad_params, uint8_t* status, void* stream) {
+                double* out, double* grad_z1, double* grad_z2, double* grad_params, uint8_t* status, void* workspace, size_t ws_bytes,
+                void* stream) {
     if (n < 0 || !(n_cosmo == 1 || n_cosmo == n)) return COSMO_E_SIZE;
     if (which == 0 || (which & ~uint32_t(W_DC | W_DM | W_TL | W_DABS | W_DA))) return COSMO_E_WHICH;
     if (n == 0) return COSMO_OK;
     if (!z1 || !z2 || !p.Om || !p.OL || !p.Or || !p.H0) return COSMO_E_NULL;
     if (grad_out ? (!grad_z1 || !grad_z2 || !grad_params) : !out) return COSMO_E_NULL;
+    if (grad_out) {
+        if (n > (int64_t)0xffffffffll) return COSMO_E_SIZE;              // 32-bit work list
+        if (!workspace) return COSMO_E_NULL;
+        if (ws_bytes < cosmo_eval2_workspace_bytes(n, 1)) return COSMO_E_WORKSPACE;
+    }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     prof_begin(st);
-    launch_two(z1, z2, p.Om, p.OL, p.Or, p.H0, n, n_cosmo, which, grad_out, out, grad_z1, grad_z2, grad_params, status, st);
+    launch_two(z1, z2, p.Om, p.OL, p.Or, p.H0, n, n_cosmo, which, grad_out, out, grad_z1, grad_z2, grad_params, status,
+               grad_out ? static_cast<unsigned*>(workspace) : nullptr, st);
     prof_end(st);
+    if (grad_out) g_launches += 1;
     return check_launch();
 }
 

@@ -334,28 +334,28 @@ CB_HD void grad_basis(const Cosmo<T>& C, const Rows& rows, T z, const Core<T>& R
 // every root structure -- Einstein-de Sitter's triple root included -- takes the same code.  FP64 in every variant; never inlined
 // (rare path).  x0, d2: centre of the root pair of Q2 and (half its gap)^2 (d2 < 0: conjugate pair x0 +- i sqrt(-d2)).
 // Returns 0, or ST_GRAD_ILLCOND when the pair sits next to the path without the panels being graded towards it (peaked integrand).
-template <int NG>
-CB_HD void grad_quad_panel(const double (&XI)[NG], const double (&WI)[NG], double Om, double OL, double Or, double Ok, double tlo,
-                           double wd, bool wantT, bool wantA, double (&acc)[9]) {
-    using N = Num<double>;
-    double dm[NG], dl[NG], dr[NG], xs[NG];
+template <int NG, typename T>
+CB_HD void grad_quad_panel(const double (&XI)[NG], const double (&WI)[NG], T Om, T OL, T Or, T Ok, T tlo, T wd, bool wantT, bool wantA,
+                           T (&acc)[9]) {
+    using N = Num<T>;
+    T dm[NG], dl[NG], dr[NG], xs[NG];
 #pragma unroll
     for (int i = 0; i < NG; ++i) {              // NG independent chains: the rare path is latency-bound, not throughput-bound
-        const double t = fma(wd, XI[i], tlo), x = 1.0 + t;        // t = x - 1 is formed directly: D_theta has the factor (x - 1)
-        const double e2 = fma(fma(fma(Or, x, Om), x, Ok), x * x, OL);
-        const double ie = N::rsqrt_(e2), f = (WI[i] * wd) * (ie * ie) * (ie * t);
+        const T t = N::fma_(wd, T(XI[i]), tlo), x = T(1) + t;        // t = x - 1 is formed directly: D_theta has the factor (x - 1)
+        const T e2 = N::fma_(N::fma_(N::fma_(Or, x, Om), x, Ok), x * x, OL);
+        const T ie = N::rsqrt_(e2), f = (T(WI[i]) * wd) * (ie * ie) * (ie * t);
         xs[i] = x;
-        dm[i] = f * (x * x); dl[i] = -f * (x + 1.0); dr[i] = dm[i] * (x + 1.0);       // w D_theta / E^3, theta = Om, OL, Or
+        dm[i] = f * (x * x); dl[i] = -f * (x + T(1)); dr[i] = dm[i] * (x + T(1));       // w D_theta / E^3, theta = Om, OL, Or
     }
 #pragma unroll
     for (int i = 0; i < NG; ++i) { acc[0] += dm[i]; acc[1] += dl[i]; acc[2] += dr[i]; }
     if (wantT) {
 #pragma unroll
-        for (int i = 0; i < NG; ++i) { const double ix = N::rcp_(xs[i]); acc[3] = fma(dm[i], ix, acc[3]); acc[4] = fma(dl[i], ix, acc[4]); acc[5] = fma(dr[i], ix, acc[5]); }
+        for (int i = 0; i < NG; ++i) { const T ix = N::rcp_(xs[i]); acc[3] = N::fma_(dm[i], ix, acc[3]); acc[4] = N::fma_(dl[i], ix, acc[4]); acc[5] = N::fma_(dr[i], ix, acc[5]); }
     }
     if (wantA) {
 #pragma unroll
-        for (int i = 0; i < NG; ++i) { const double x2 = xs[i] * xs[i]; acc[6] = fma(dm[i], x2, acc[6]); acc[7] = fma(dl[i], x2, acc[7]); acc[8] = fma(dr[i], x2, acc[8]); }
+        for (int i = 0; i < NG; ++i) { const T x2 = xs[i] * xs[i]; acc[6] = N::fma_(dm[i], x2, acc[6]); acc[7] = N::fma_(dl[i], x2, acc[7]); acc[8] = N::fma_(dr[i], x2, acc[8]); }
     }
 }
 
@@ -409,16 +409,61 @@ CB_HD_NOINLINE unsigned grad_quad(double Om, double OL, double Or, double x0, do
     }
     double wd = (np == 1) ? dz : dz * (r - 1.0) / (q - 1.0);            // widths sum to dz; one panel: dz itself
     double tlo = z1;                                                   // x - 1 at the panel's lower end
-    if (np == 1 && qa <= 1.02 && rho >= 60.0) grad_quad_panel<4>(X4, W4, Om, OL, Or, Ok, tlo, wd, wantT, wantA, acc);
-    else if (np == 1 && qa <= 1.2 && rho >= 12.0) grad_quad_panel<6>(X6, W6, Om, OL, Or, Ok, tlo, wd, wantT, wantA, acc);
+    if (np == 1 && qa <= 1.02 && rho >= 60.0) grad_quad_panel<4, double>(X4, W4, Om, OL, Or, Ok, tlo, wd, wantT, wantA, acc);
+    else if (np == 1 && qa <= 1.2 && rho >= 12.0) grad_quad_panel<6, double>(X6, W6, Om, OL, Or, Ok, tlo, wd, wantT, wantA, acc);
     else {
         for (int k = 0; k < np; ++k) {
-            grad_quad_panel<12>(X12, W12, Om, OL, Or, Ok, tlo, wd, wantT, wantA, acc);
+            grad_quad_panel<12, double>(X12, W12, Om, OL, Or, Ok, tlo, wd, wantT, wantA, acc);
             tlo += wd;
             wd *= r;
         }
     }
     for (int i = 0; i < 9; ++i) out[i] = acc[i];
+    return st;
+}
+
+// FP32 variant: the gradient integrals of EVERY element by the same quadrature in FP32 arithmetic (6 nodes per panel of ratio <= 2:
+// rho^-12 = 6e-10).  The gradient bases lose cond x 6e-8 in FP32 and cond reaches 1e3-1e5 at small z, while the quadrature sums terms of
+// one sign pattern and is as accurate as FP32 allows (~1e-6) at every z; it is also FP32 work, which the bases' FP64 rows are not.
+// x0, d2 as grad_quad.  Inlined (it is this variant's main path).
+CB_HD unsigned grad_quad_f32(float Om, float OL, float Or, float x0, float d2, float z, bool wantT, bool wantA, float (&acc)[9]) {
+    const double X6[6] = {0.0337652428984239861, 0.169395306766867743, 0.380690406958401546, 0.619309593041598454, 0.830604693233132257,
+                          0.966234757101576014};
+    const double W6[6] = {0.0856622461895851725, 0.180380786524069303, 0.233956967286345524, 0.233956967286345524, 0.180380786524069303,
+                          0.0856622461895851725};
+#pragma unroll
+    for (int i = 0; i < 9; ++i) acc[i] = 0.0f;
+    const float Ok = 1.0f - Om - OL - Or, X2 = 1.0f + z;
+    if (!(X2 > 0.0f) || z == 0.0f) return 0u;
+    const float lo = fminf(1.0f, X2), hi = fmaxf(1.0f, X2);
+    const float hg = d2 > 0.0f ? sqrtf(d2) : 0.0f, xr = x0 + hg;
+    const float c = (xr > 0.0f && xr < lo) ? xr : 0.0f;
+    const float q = (X2 - c) / (1.0f - c), qa = q >= 1.0f ? q : 1.0f / q;
+    int np = 1;
+    float r = q;
+    if (qa > 2.0f) {
+        const float lr = logf(q);
+        np = (int)ceilf(fabsf(lr) * 1.44269504f);
+        if (np > 64) np = 64;
+        r = expf(lr / (float)np);
+    }
+    unsigned st = 0u;
+    if (!(xr < lo)) {       // pair not left of the path: Bernstein parameter of the panel next to it (see grad_quad); 6 nodes need rho >= 5
+        const float y0 = d2 < 0.0f ? sqrtf(-d2) : 0.0f, rr = r >= 1.0f ? r : 1.0f / r;
+        float wre, h;
+        if (x0 + hg < lo) { h = 0.5f * lo * (rr - 1.0f); wre = (lo - (x0 + hg)) / h + 1.0f; }
+        else if (x0 - hg > hi) { h = 0.5f * hi * (1.0f - 1.0f / rr); wre = ((x0 - hg) - hi) / h + 1.0f; }
+        else { h = 0.5f * fminf(fmaxf(x0, lo), hi) * (rr - 1.0f); wre = 0.0f; }
+        const float wim = y0 / h;
+        const float a = 0.5f * (hypotf(wre + 1.0f, wim) + hypotf(wre - 1.0f, wim));
+        if (!(a + sqrtf(fmaxf(a * a - 1.0f, 0.0f)) >= 5.0f)) st = (unsigned)ST_GRAD_ILLCOND;
+    }
+    float wd = (np == 1) ? z : z * (r - 1.0f) / (q - 1.0f), tlo = 0.0f;
+    for (int k = 0; k < np; ++k) {
+        grad_quad_panel<6, float>(X6, W6, Om, OL, Or, Ok, tlo, wd, wantT, wantA, acc);
+        tlo += wd;
+        wd *= r;
+    }
     return st;
 }
 
@@ -579,7 +624,32 @@ CB_HD unsigned elem_one(T zv, double Om, double OL, double Or, double H0, unsign
     unsigned st = O.status | redo;
     if (kG) {
         dz = T(0); gp[0] = gp[1] = gp[2] = gp[3] = T(0);
-        {
+        if (sizeof(T) == 4) {       // FP32 variant: gradient integrals by FP32 quadrature (grad_quad_f32), no bases
+            float q[9];
+            GradInt<T> D;
+            const float b = (float)C.b;
+            const unsigned sq = grad_quad_f32((float)C.Om, (float)C.OL, (float)C.Or, -0.5f * b, 0.25f * b * b - (float)C.c, (float)zv,
+                                              kT && (which & (W_TL | W_AGE)), kA && (which & W_DABS), q);
+#pragma unroll
+            for (int t = 0; t < 3; ++t) { D.dI[t] = (T)q[t]; D.dT[t] = (T)q[3 + t]; D.dA[t] = (T)q[6 + t]; }
+            const bool peaked = sq != 0u && !(R.status & (ST_ROOT_ON_PATH | ST_UNSUPPORTED));
+            // a root pair next to the path (peaked integrand: the 6-node panels do not resolve it; loitering models, where FP32 cannot
+            // even hold the pair's gap): such elements are evaluated by the FP64 path, values included (second pass of the kernel when kDefer)
+            if (peaked && kDefer) st |= ST_INTERNAL_REDO;
+            if (peaked && !kDefer) {
+                double gd[N_PLANES], vd[N_PLANES], dzd = 0.0, gpd[4] = {0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+                for (int w = 0; w < N_PLANES; ++w) gd[w] = (double)g[w];
+                st = elem_one<double, kT, kA, kG, VoteNone, false>((double)zv, Om, OL, Or, H0, which, VoteNone(), gd, vd, dzd, gpd);
+#pragma unroll
+                for (int w = 0; w < N_PLANES; ++w) v[w] = (T)vd[w];
+                dz = (T)dzd;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) gp[j] = (T)gpd[j];
+            } else {
+                backward_chain<T, kT, kA>(C, zv, R, O, D, g, dz, gp, which);
+            }
+        } else {
             st |= backward_robust<T, kT, kA, true, kDefer>(C, zv, R, O, g, dz, gp, which);
         }
     }

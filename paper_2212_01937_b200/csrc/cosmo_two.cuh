@@ -15,14 +15,19 @@ struct Two {
     unsigned status;
 };
 
-template <typename Vote>
+// kDefer (main pass of k_two's VJP): an element that needs a slow path -- complex root structure (cosmo_c4.cuh) or quadrature of the
+// gradient integrals -- is only marked ST_INTERNAL_REDO; the second pass runs it again without kDefer (as the ELEMENTWISE kernels do).
+template <typename Vote, bool kDefer = false>
 CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad, const Vote& vote, Two& O) {
     const double x1 = 1.0 + z1, x2 = 1.0 + z2, dz = z2 - z1, dz2 = dz * dz;
     unsigned st[1] = {C.status};
     if (!(x1 > 0.0) || !(x2 > 0.0)) st[0] |= ST_UNSUPPORTED;
     if (fmax(x1, x2) >= C.xlim && fmin(x1, x2) < C.xlim) st[0] |= ST_ROOT_ON_PATH;
     double I0, K, TT, AA, E1, E2, dE;
-    if (C.cubic & 2u) {
+    if (kDefer && (C.cubic & 2u)) {
+        I0 = K = TT = AA = E1 = E2 = dE = NAN;
+        st[0] |= ST_INTERNAL_REDO;
+    } else if (C.cubic & 2u) {
         // two complex pairs (C.m, C.rn carry g1, h1): eqs. (3.7)-(3.9) as printed with a complex r_i, cosmo_c4.cuh
         eval_c4(C.Or, C.m, C.rn, C.b, C.c, x1, x2, true, true, I0, TT, AA, K);
         E1 = sqrt(fma(fma(C.Or, x1, C.m), x1, C.rn) * fma(x1 + C.b, x1, C.c));
@@ -115,18 +120,24 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
         for (int k = 0; k < 16; ++k) { btv[k] = fma(dk, iE2, xk1 * diE); dk = fma(x2, dk, xk1 * dz); xk1 *= x1; }
     }
     // raw gradient integrals int D_theta p_X / E^3 dx between the limits (cosmo_obs.cuh, GradInt) with their cancellation factor
-    double rI[3], rT[3], rA[3], cond = 0.0;
-    auto worse = [&](double sa, double val, double fwd) {
-        const double c = sa / fmax(fabs(val), 1e-3 * fabs(fwd));
-        if (c > cond || !(c == c)) cond = c;
-    };
+    double rI[3], rT[3], rA[3];
+    bool over = false;                   // cancellation factor above GRAD_COND_LIMIT somewhere (a NaN counts)
+    auto worse = [&](double sa, double val, double fwd) { over = over | !(sa <= GRAD_COND_LIMIT * fmax(fabs(val), 1e-3 * fabs(fwd))); };
+    // basis rows solved on the spot from the factorisation (cosmo_prep.cuh, GradSolve): nothing stored per cosmology
+    GradSolve S;
+    S.init(C);
+    const double aI0 = fabs(I0), aK = fabs(K), a0 = fabs(btv[0]), a1 = fabs(btv[1]), a2 = fabs(btv[2]);
+    auto dot5 = [&](const double* g) { return g[0] * I0 + g[1] * K + g[2] * btv[0] + g[3] * btv[1] + g[4] * btv[2]; };
+    auto abs5 = [&](const double* g) { return fabs(g[0]) * aI0 + fabs(g[1]) * aK + fabs(g[2]) * a0 + fabs(g[3]) * a1 + fabs(g[4]) * a2; };
     double Jp[17], Sp[7];
     bool useJ = false;
     {
         constexpr int KJ = 12;
-        for (int p = 0; p < 5; ++p) {
-            Jp[p] = C.GJ[p][0] * I0 + C.GJ[p][1] * K + C.GJ[p][2] * btv[0] + C.GJ[p][3] * btv[1] + C.GJ[p][4] * btv[2];
-            Sp[p] = fabs(C.GJ[p][0] * I0) + fabs(C.GJ[p][1] * K) + fabs(C.GJ[p][2] * btv[0]) + fabs(C.GJ[p][3] * btv[1]) + fabs(C.GJ[p][4] * btv[2]);
+        Jp[0] = Jp[1] = 0.0; Sp[0] = Sp[1] = 0.0;
+        for (int p = 2; p < 5; ++p) {
+            double g[5];
+            S.rowJ(p, g);
+            Jp[p] = dot5(g); Sp[p] = abs5(g);
         }
         for (int p = 5; p < 17; ++p) Jp[p] = 0.0;
         double prev5 = 0.0, prev6 = 0.0;
@@ -144,23 +155,27 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
     }
     const double btA = (C.cubic & 1u) ? btv[4] : btv[3];
     for (int t = 0; t < 3; ++t) {
-        rI[t] = C.GI[t][0] * I0 + C.GI[t][1] * K + C.GI[t][2] * btv[0] + C.GI[t][3] * btv[1] + C.GI[t][4] * btv[2];
-        worse(fabs(C.GI[t][0] * I0) + fabs(C.GI[t][1] * K) + fabs(C.GI[t][2] * btv[0]) + fabs(C.GI[t][3] * btv[1]) + fabs(C.GI[t][4] * btv[2]),
-              rI[t], I0);
-        rT[t] = C.GT[t][0] * I0 + C.GT[t][1] * K + C.GT[t][2] * btv[0] + C.GT[t][3] * btv[1] + C.GT[t][4] * btv[2] + C.GT[t][5] * TT;
-        worse(fabs(C.GT[t][0] * I0) + fabs(C.GT[t][1] * K) + fabs(C.GT[t][2] * btv[0]) + fabs(C.GT[t][3] * btv[1]) + fabs(C.GT[t][4] * btv[2])
-              + fabs(C.GT[t][5] * TT), rT[t], TT);
+        double g[7];
+        S.rowI(t, g);
+        rI[t] = dot5(g);
+        worse(abs5(g), rI[t], I0);
+        S.rowT(t, g);
+        rT[t] = dot5(g) + g[5] * TT;
+        worse(abs5(g) + fabs(g[5] * TT), rT[t], TT);
         const int ia = t == 0 ? 5 : (t == 1 ? 2 : 6);
-        double a = C.GA[t][0] * I0 + C.GA[t][1] * K + C.GA[t][2] * btv[0] + C.GA[t][3] * btv[1] + C.GA[t][4] * btv[2] + C.GA[t][5] * btA
-                   + C.GA[t][6] * AA;
-        double sa = fabs(C.GA[t][0] * I0) + fabs(C.GA[t][1] * K) + fabs(C.GA[t][2] * btv[0]) + fabs(C.GA[t][3] * btv[1]) + fabs(C.GA[t][4] * btv[2])
-                    + fabs(C.GA[t][5] * btA) + fabs(C.GA[t][6] * AA);
-        if (useJ) { a = Jp[ia] - Jp[4]; sa = Sp[ia] + Sp[4]; }
-        rA[t] = a;
-        worse(sa, a, AA);
+        if (useJ) {
+            rA[t] = Jp[ia] - Jp[4];
+            worse(Sp[ia] + Sp[4], rA[t], AA);
+        } else {
+            S.rowA(t, g);
+            rA[t] = dot5(g) + g[5] * btA + g[6] * AA;
+            worse(abs5(g) + fabs(g[5] * btA) + fabs(g[6] * AA), rA[t], AA);
+        }
     }
     // ill-conditioned bases (near-repeated roots away from the path, tiny ranges): quadrature of the same integrals (grad_quad)
-    if ((!(cond <= GRAD_COND_LIMIT) || (C.cubic & 4u)) && !(st[0] & (ST_ROOT_ON_PATH | ST_UNSUPPORTED))) {
+    if (kDefer) {
+        if ((over || S.singular) && !(st[0] & (ST_ROOT_ON_PATH | ST_UNSUPPORTED))) O.status |= ST_INTERNAL_REDO;
+    } else if ((over || S.singular) && !(st[0] & (ST_ROOT_ON_PATH | ST_UNSUPPORTED))) {
         double q[9];
         O.status |= grad_quad(C.Om, C.OL, C.Or, -0.5 * C.b, 0.25 * C.b * C.b - C.c, z1, dz, true, true, q);
         for (int t = 0; t < 3; ++t) { rI[t] = q[t]; rT[t] = q[3 + t]; rA[t] = q[6 + t]; }

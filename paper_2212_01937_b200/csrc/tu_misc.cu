@@ -26,40 +26,71 @@ __global__ void k_prep(const double* __restrict__ Om, const double* __restrict__
 }
 
 // Two-limit evaluation (cosmo_two.cuh), one thread per (z1, z2, cosmology); n_cosmo in {1, n}.  which: DC, DM, TL, DABS, DA.
-// (128-register cap as for k_elem: 0.40 -> 0.28 ms forward, 0.75 -> 0.56 ms forward + VJP per 10^6 pairs)
-__global__ void __launch_bounds__(ELEM_THREADS, 4) k_two(const double* __restrict__ z1, const double* __restrict__ z2,
-                                                      const double* __restrict__ Om, const double* __restrict__ OL,
-                                                      const double* __restrict__ Or, const double* __restrict__ H0, int64_t n,
-                                                      int64_t n_cosmo, unsigned which, const double* __restrict__ gout,
-                                                      double* __restrict__ out, double* __restrict__ gz1, double* __restrict__ gz2,
-                                                      double* __restrict__ gparams, uint8_t* __restrict__ status) {
-    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    const bool live = i < n;
-    const int64_t ii = live ? i : n - 1, ic = n_cosmo == 1 ? 0 : ii;
-    const bool with_grad = gout != nullptr;
-    Cosmo<double> C;
-    cosmo_prep(Om[ic], OL[ic], Or[ic], H0[ic], with_grad ? 2 : 0, C);
+// (128-register cap as for k_elem.)  kG: with the VJP; its slow paths go to the second pass k_two<.., kRedo> through a work list, as in
+// k_elem; the forward kernel keeps the complex path inline.
+#ifndef CB_TWO_DEFER_MIN
+#define CB_TWO_DEFER_MIN 3000000
+#endif
+constexpr int64_t TWO_DEFER_MIN = CB_TWO_DEFER_MIN;
+struct TwoArgs {
+    const double *z1, *z2, *Om, *OL, *Or, *H0;
+    int64_t n, n_cosmo; unsigned which;
+    const double* gout; double *out, *gz1, *gz2, *gparams; uint8_t* status;
+    unsigned *redo_count, *redo_list;
+};
+
+template <bool kG, bool kDefer, bool kRedo>
+__device__ __forceinline__ unsigned two_one(const TwoArgs& a, int64_t i, bool live) {
+    const int64_t n = a.n, ii = live ? i : n - 1, ic = a.n_cosmo == 1 ? 0 : ii;
+    Cosmo<double> C{};
+    cosmo_factor(a.Om[ic], a.OL[ic], a.Or[ic], a.H0[ic], C);
+    cosmo_constants(C);
     Two O;
-    eval_two<VoteWarp>(C, z1[ii], z2[ii], with_grad, VoteWarp(), O);
-    if (!live) return;
+    if (kRedo) eval_two<VoteNone, false>(C, a.z1[ii], a.z2[ii], kG, VoteNone(), O);
+    else eval_two<VoteWarp, kDefer>(C, a.z1[ii], a.z2[ii], kG, VoteWarp(), O);
+    if (!live) return 0u;
     const unsigned bits[5] = {W_DC, W_DM, W_TL, W_DABS, W_DA};
     double a1 = 0.0, a2 = 0.0, ap[4] = {0.0, 0.0, 0.0, 0.0};
     int pl = 0;
     for (int o = 0; o < 5; ++o) {
-        if (!(which & bits[o])) continue;
-        if (out != nullptr) out[(int64_t)pl * n + i] = O.v[o];
-        if (with_grad) {
-            const double g = gout[(int64_t)pl * n + i];
+        if (!(a.which & bits[o])) continue;
+        if (a.out != nullptr) a.out[(int64_t)pl * n + i] = O.v[o];
+        if (kG) {
+            const double g = a.gout[(int64_t)pl * n + i];
             a1 = fma(g, O.gz1[o], a1); a2 = fma(g, O.gz2[o], a2);
             for (int t = 0; t < 4; ++t) ap[t] = fma(g, O.gp[o][t], ap[t]);
         }
         ++pl;
     }
-    if (status != nullptr) status[i] = (uint8_t)O.status;
-    if (with_grad) {
-        gz1[i] = a1; gz2[i] = a2;
-        for (int t = 0; t < 4; ++t) gparams[(int64_t)t * n + i] = ap[t];
+    if (a.status != nullptr) a.status[i] = (uint8_t)(O.status & ~(unsigned)ST_INTERNAL_REDO);
+    if (kG) {
+        a.gz1[i] = a1; a.gz2[i] = a2;
+        for (int t = 0; t < 4; ++t) a.gparams[(int64_t)t * n + i] = ap[t];
     }
+    return O.status;
+}
+
+template <bool kG, bool kDefer>
+__global__ void __launch_bounds__(ELEM_THREADS, 4) k_two(TwoArgs a) {
+    const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    const bool live = i < a.n;
+    const unsigned st = two_one<kG, kDefer, false>(a, i, live);
+    if (kDefer) {       // work list of the second pass: one atomic per warp
+        const bool redo = live && (st & ST_INTERNAL_REDO);
+        const unsigned active = __activemask();
+        const unsigned m = __ballot_sync(active, redo);
+        if (m) {
+            const int lane = threadIdx.x & 31, leader = __ffs(m) - 1;
+            unsigned base = 0;
+            if (lane == leader) base = atomicAdd(a.redo_count, (unsigned)__popc(m));
+            base = __shfl_sync(active, base, leader);
+            if (redo) a.redo_list[base + __popc(m & ((1u << lane) - 1u))] = (unsigned)i;
+        }
+    }
+}
+__global__ void __launch_bounds__(ELEM_THREADS, 4) k_two_redo(TwoArgs a) {
+    const unsigned count = *a.redo_count;
+    for (unsigned j = blockIdx.x * blockDim.x + threadIdx.x; j < count; j += gridDim.x * blockDim.x) two_one<true, false, true>(a, (int64_t)a.redo_list[j], true);
 }
 
 // chi family with extra constant-w components (cosmo_w.cuh), one thread per (z, cosmology); n_cosmo in {1, n}.
@@ -131,8 +162,16 @@ void launch_reduce_gz(bool f32, const void* part, int ny, int64_t N, void* gz, c
 }
 void launch_two(const double* z1, const double* z2, const double* Om, const double* OL, const double* Or, const double* H0, int64_t n,
                 int64_t n_cosmo, unsigned which, const double* gout, double* out, double* gz1, double* gz2, double* gparams,
-                uint8_t* status, cudaStream_t st) {
-    k_two<<<(unsigned)cdiv64(n, ELEM_THREADS), ELEM_THREADS, 0, st>>>(z1, z2, Om, OL, Or, H0, n, n_cosmo, which, gout, out, gz1, gz2, gparams, status);
+                uint8_t* status, unsigned* ws, cudaStream_t st) {
+    TwoArgs a{z1, z2, Om, OL, Or, H0, n, n_cosmo, which, gout, out, gz1, gz2, gparams, status, ws, ws ? ws + 64 : nullptr};
+    const unsigned grid = (unsigned)cdiv64(n, ELEM_THREADS);
+    if (gout == nullptr) { k_two<false, false><<<grid, ELEM_THREADS, 0, st>>>(a); return; }
+    // The second pass costs the latency of one slow element (tens of microseconds) whatever the batch size, the inline slow paths
+    // ~10 % of the main kernel: two passes from a few million elements on (measured, profiles/)
+    if (n < TWO_DEFER_MIN) { k_two<true, false><<<grid, ELEM_THREADS, 0, st>>>(a); return; }
+    cudaMemsetAsync(a.redo_count, 0, sizeof(unsigned), st);
+    k_two<true, true><<<grid, ELEM_THREADS, 0, st>>>(a);
+    k_two_redo<<<148 * 4, ELEM_THREADS, 0, st>>>(a);
 }
 void launch_w(const double* z, const double* Om, const double* OL, const double* Or, const double* Ow13, const double* Ow23,
               const double* H0, int64_t n, int64_t n_cosmo, unsigned which, double* out, double* dout, uint8_t* status, cudaStream_t st) {

@@ -96,8 +96,9 @@ extern "C" void hostcheck_factor(double Om, double OL, double Or, double* out5) 
 extern "C" void hostcheck_two(int64_t n, const double* z1, const double* z2, const double* Om, const double* OL, const double* Or,
                               const double* H0, double* val, double* gz1, double* gz2, double* gp, uint8_t* status) {
     for (int64_t i = 0; i < n; ++i) {
-        Cosmo<double> C;
-        cosmo_prep(Om[i], OL[i], Or[i], H0[i], 2, C);
+        Cosmo<double> C{};
+        cosmo_factor(Om[i], OL[i], Or[i], H0[i], C);
+        cosmo_constants(C);
         Two O;
         eval_two<VoteNone>(C, z1[i], z2[i], true, VoteNone(), O);
         for (int o = 0; o < 5; ++o) {
