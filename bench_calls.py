@@ -1,6 +1,7 @@
-"""Times the C-ABI calls on the five BASELINE.json configs (seeded synthetic inputs, device-resident, CUDA events).
+"""Times every C-ABI call on the BASELINE.json configs (seeded synthetic inputs, device-resident, CUDA events).  A measurement
+script beside bench.py, not part of the package.
 
-    python -m paper_2212_01937_b200.timing [--steps 10] [--small]
+    python bench_calls.py [--steps 10] [--small] [--only config2,config5]
 
 One JSON line per config: evals/s of the whole call and the mean duration of its dominant kernel (library hook).
 bench.py stays the headline (config 3); this is the per-config table quoted in DESIGN.md / profiles/.
@@ -8,12 +9,19 @@ bench.py stays the headline (config 3); this is the per-config table quoted in D
 import argparse
 import json
 
+import os
+import sys
+
 import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
 
 
 def main():
     import torch
-    from . import binding as cb, workloads as W
+    from paper_2212_01937_b200 import binding as cb, workloads as W
 
     ap = argparse.ArgumentParser()
     ap.add_argument("--steps", type=int, default=10)

@@ -288,8 +288,10 @@ def cosmo_eval_w(z, Om, OL, Or, Ow13, Ow23, H0, which=("DC",), want_dz=True):
     return out, dz, status
 
 
-def cosmo_eval_host(z, Om, OL, Or, H0, mode=ELEMENTWISE, which=("DC",), grad_out=None, want_out=True, want_status=True):
-    """Host-buffer call (numpy float64 arrays in, numpy out): H2D + kernels + D2H inside the library, synchronous."""
+def cosmo_eval_host(z, Om, OL, Or, H0, mode=ELEMENTWISE, which=("DC",), grad_out=None, want_out=True, want_status=True, out=None,
+                    grad_z=None, grad_params=None, status=None):
+    """Host-buffer call (numpy float64 arrays in, numpy out): H2D + kernels + D2H inside the library, synchronous.  Pass pinned arrays
+    (inputs and, through out / grad_z / grad_params / status, outputs) for full PCIe speed; outputs not passed are allocated here."""
     import numpy as np
     _torch()
     mask = which_mask(which)
@@ -299,13 +301,22 @@ def cosmo_eval_host(z, Om, OL, Or, H0, mode=ELEMENTWISE, which=("DC",), grad_out
     nw = bin(mask).count("1")
     vp = lambda a: C.c_void_p(a.ctypes.data) if a is not None else C.c_void_p(0)
     P = CosmoParams(*[a.ctypes.data for a in arrs[1:]])
-    out = np.empty((nw, rows, n_z)) if (want_out or grad_out is None) else None
-    status = np.empty((rows, n_z), dtype=np.uint8) if want_status else None
+
+    def buf(given, shape, dtype, want):
+        if given is not None:
+            if given.shape != shape or given.dtype != dtype or not given.flags.c_contiguous:
+                raise CosmoError(f"output buffer: expected a C-contiguous {dtype} array of shape {shape}")
+            return given
+        return np.empty(shape, dtype=dtype) if want else None
+    out = buf(out, (nw, rows, n_z), np.float64, want_out or grad_out is None)
+    status = buf(status, (rows, n_z), np.uint8, want_status)
     gz = gp = None
     if grad_out is not None:
         grad_out = np.ascontiguousarray(grad_out, dtype=np.float64)
-        gz = np.empty(n_z)
-        gp = np.empty((4, n_cosmo))
+        if grad_out.size != nw * rows * n_z:
+            raise CosmoError("grad_out must have shape [n_which, rows, n_z]")
+        gz = buf(grad_z, (n_z,), np.float64, True)
+        gp = buf(grad_params, (4, n_cosmo), np.float64, True)
     _check(lib().cosmo_eval_host(vp(arrs[0]), n_z, P, n_cosmo, mode, mask, vp(grad_out), vp(out), vp(gz), vp(gp), vp(status)))
     return out, gz, gp, status
 

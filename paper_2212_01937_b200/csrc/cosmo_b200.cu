@@ -1,5 +1,6 @@
 // cosmo_b200.cu -- launchers and the C ABI declared in include/cosmo_b200.h.  sm_100a only; no CPU path.
 #include <atomic>
+#include <cstdlib>
 #include <mutex>
 #include "../../include/cosmo_b200.h"
 #include "../../include/cosmo_b200_diag.h"
@@ -314,7 +315,8 @@ int cosmo_eval_host(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosm
     const int64_t n_par = per_elem ? 0 : n_cosmo;             // parameters copied once (shared) or chunked with z (per element)
     // chunk length: ~32 MB of the widest per-redshift stream, at least 64 Ki redshifts, even (128-bit accesses), at most 64 chunks
     const int64_t bytes_per_z = (int64_t)sizeof(double) * ((int64_t)np * rows * ((with_grad ? 1 : 0) + (out ? 1 : 0)) + 2 + (per_elem ? 8 : 0)) + rows;
-    int64_t nc = (32ll << 20) / bytes_per_z;
+    static const int64_t chunk_mb = []() { const char* e = getenv("COSMO_HOST_CHUNK_MB"); const long v = e ? atol(e) : 0; return (int64_t)(v > 0 ? v : 32); }();
+    int64_t nc = (chunk_mb << 20) / bytes_per_z;
     if (nc < 65536) nc = 65536;
     if (nc * 64 < n_z) nc = cdiv(n_z, 64);
     nc = (nc + 1) & ~int64_t(1);

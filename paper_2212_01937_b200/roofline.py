@@ -19,16 +19,23 @@ probe (cosmo_probe_fma_f64); the nominal figure beside it is 148 SMs x 64 FP64 F
 FLOPS_PER_EVAL = {
     "config3_vjp_mu_f64": 397.9,
 }
-FP64_PIPE_INST_PER_EVAL = {
+# instructions per eval on the arithmetic pipe of the dtype (FP64: DFMA + DMUL + DADD + DSETP)
+PIPE_INST_PER_EVAL = {
     "config3_vjp_mu_f64": 265.9,
 }
 # dram__bytes_read.sum + dram__bytes_write.sum of that kernel, per launch (same capture)
 DRAM_TRAFFIC_BYTES_PER_LAUNCH = {
     "config3_vjp_mu_f64": 544.13e6 + 635.70e6,
 }
+# where each entry comes from
+SOURCE = {
+    "config3_vjp_mu_f64": "profiles/r01c_k_outer_vjp.md",
+}
 
-# nominal B200 FP64 vector peak (context only; the denominator is the measured probe)
+# nominal B200 vector peaks (context only; the denominator is the measured probe): 148 SMs x lanes x 2 x 1.965 GHz
 NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+NOMINAL_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 
-# algorithmic HBM bytes per eval, config 3 as bench.py runs it (z, params and constants stay on chip)
-BYTES_PER_EVAL_C3 = 8.0 + 8.0 + 1.0 + (8.0 + 8.0) / 64.0   # grad_out read, out + status written, z/grad_z amortised over S
+# algorithmic HBM bytes per eval, config 3 as bench.py runs it (z, params and constants stay on chip): grad_out read, out + status
+# written, z / grad_z amortised over S
+BYTES_PER_EVAL_C3 = {"f64": 8.0 + 8.0 + 1.0 + (8.0 + 8.0) / 64.0, "f32": 4.0 + 4.0 + 1.0 + (4.0 + 4.0) / 64.0}

@@ -14,7 +14,7 @@ from dataclasses import dataclass, field
 
 import numpy as np
 
-__all__ = ["Workload", "config1", "config2", "config3", "config4", "config5", "invalid_rows", "e2_min_on_path"]
+__all__ = ["Workload", "config1", "config2", "config3", "config3_shard", "config4", "config5", "invalid_rows", "e2_min_on_path"]
 
 
 @dataclass
@@ -111,6 +111,19 @@ def config3(n: int = 1_000_000, S: int = 64, seed: int = 3, which=("MU",)) -> Wo
     Om, OL, Or, H0 = _vi_samples(rng, S, 9e-5)
     g = rng.standard_normal((len(which), S, n))
     return Workload("config3", "outer", z, Om, OL, Or, H0, tuple(which), grad_out=g)
+
+
+def config3_shard(n_per_rank: int, world: int, rank: int, S: int = 64, seed: int = 3, which=("MU",)) -> Workload:
+    """Rank `rank`'s part of ONE config-3 job of world x n_per_rank sorted redshifts (multi-GPU runs): the global
+    redshift array is drawn and sorted once and cut contiguously (sharding.shard_bounds); the upstream gradient of a shard is drawn
+    from (seed, shard index), so the job on `world` ranks and the same job on one rank (its shards concatenated) see identical inputs."""
+    from .sharding import shard_bounds
+    rng = np.random.default_rng(seed)
+    z = np.sort(rng.uniform(0.01, 1.5, n_per_rank * world))
+    Om, OL, Or, H0 = _vi_samples(rng, S, 9e-5)
+    lo, hi = shard_bounds(n_per_rank * world, world, rank)
+    g = np.random.default_rng([seed, rank]).standard_normal((len(which), S, hi - lo))
+    return Workload("config3", "outer", z[lo:hi], Om, OL, Or, H0, tuple(which), grad_out=g)
 
 
 def config4(mu_fn, n: int = 1_000_000, S: int = 256, seed: int = 4) -> Workload:

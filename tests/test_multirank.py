@@ -27,13 +27,12 @@ def _worker(rank, world, port, n, S, q):
     dist.init_process_group("gloo", rank=rank, world_size=world)
     import oracle
     from paper_2212_01937_b200 import workloads as W
-    w = W.config3(n=n, S=S)
-    lo, hi = sharding.shard_bounds(n, world, rank)
+    w = W.config3_shard(n, world, rank, S=S)          # exactly what bench.py --gpus N gives rank `rank`
     MU = oracle.OBS.index("MU")
     gp = torch.zeros((4, S), dtype=torch.float64)
     for s in range(S):
-        _, grad, _ = oracle.observables_batch(w.z[lo:hi], w.Om[s:s + 1], w.OL[s:s + 1], w.Or[s:s + 1], w.H0[s:s + 1], with_grad=True, threads=1)
-        g = w.grad_out[0, s, lo:hi]
+        _, grad, _ = oracle.observables_batch(w.z, w.Om[s:s + 1], w.OL[s:s + 1], w.Or[s:s + 1], w.H0[s:s + 1], with_grad=True, threads=1)
+        g = w.grad_out[0, s]
         for p in range(4):
             gp[p, s] = float((g * grad[:, MU, 1 + p].astype(np.float64)).sum())
     sharding.allreduce_sums(gp)
@@ -59,10 +58,15 @@ def test_gloo_two_ranks_match_single():
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
-    w = W.config3(n=n, S=S)
+    # the same job on ONE rank: the shards concatenated (W.config3_shard draws the global redshift array once and cuts it)
+    shards = [W.config3_shard(n, 2, r, S=S) for r in range(2)]
+    z = np.concatenate([w.z for w in shards]); g = np.concatenate([w.grad_out for w in shards], axis=2)
+    one = W.config3_shard(2 * n, 1, 0, S=S)
+    assert np.array_equal(z, one.z) and np.array_equal(shards[0].Om, one.Om) and (np.diff(z) >= 0).all()
+    w = shards[0]
     MU = oracle.OBS.index("MU")
     for s in range(S):
-        _, grad, _ = oracle.observables_batch(w.z, w.Om[s:s + 1], w.OL[s:s + 1], w.Or[s:s + 1], w.H0[s:s + 1], with_grad=True)
+        _, grad, _ = oracle.observables_batch(z, w.Om[s:s + 1], w.OL[s:s + 1], w.Or[s:s + 1], w.H0[s:s + 1], with_grad=True)
         for p in range(4):
-            terms = w.grad_out[0, s] * grad[:, MU, 1 + p].astype(np.float64)
+            terms = g[0, s] * grad[:, MU, 1 + p].astype(np.float64)
             assert abs(got[p, s] - terms.sum()) <= 1e-12 * np.abs(terms).sum()
