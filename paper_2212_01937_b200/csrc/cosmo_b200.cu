@@ -156,12 +156,8 @@ int run_eval(const T* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode,
     a.gz_accumulate = L.ny > 1;
     a.gz = a.gz_accumulate ? static_cast<void*>(w + L.gzpart) : static_cast<void*>(gz);
     if ((rc = launch_outer<T>(MODE_VJP, a, grid, st))) return rc;
-    launch_reduce_params(4, a.part, L.ntiles, n_cosmo, nullptr, gparams, st);
+    launch_reduce_vjp(sizeof(T) == 4, a.part, L.ntiles, n_cosmo, gparams, a.gz_accumulate ? a.gz : nullptr, L.ny, n_z, gz, st);
     if ((rc = check_launch())) return rc;
-    if (a.gz_accumulate) {
-        launch_reduce_gz(sizeof(T) == 4, a.gz, L.ny, n_z, gz, st);
-        if ((rc = check_launch())) return rc;
-    }
     return COSMO_OK;
 }
 

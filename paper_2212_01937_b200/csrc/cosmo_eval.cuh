@@ -227,12 +227,16 @@ CB_HD void carlson_dup(T (&xa)[K], T (&mp)[K], const T (&s)[K], T (&p5)[K], T (&
     g2 = T(1);
     // thresholds as magnitude keys (Num<T>::key_): the rule needs a few significant bits, and integer compares are free
     // beside the FP64 pipe
-    int kF[K], kDd[K], k5[K], k0[K];
+    int kF[K], k5[K], k0[K];
+    T cx[K];
 #pragma unroll
     for (int k = 0; k < K; ++k) {
         tailD[k] = sum5[k] = sum0[k] = T(0);
-        kF[k] = N::key_(T(3) * Qc[k]);
-        kDd[k] = N::key_(T(5) * Qc[k]);
+        // R_F and R_D share the bound Qc and their means differ by 5 A_D - 3 A_F ... : A_D - A_F = 4 (xa - mp)/15, and xa - mp is
+        // invariant under the unscaled step, so the smaller of the two means is known once: one comparison per step serves both
+        const bool dsel = kD && (xa[k] < mp[k]);              // A_D < A_F
+        cx[k] = dsel ? T(3) : T(1);
+        kF[k] = N::key_((dsel ? T(5) : T(3)) * Qc[k]);
         k5[k] = N::key_(T(5) * Q5v[k]);
         k0[k] = N::key_(T(5) * Q0v[k]);
     }
@@ -242,9 +246,10 @@ CB_HD void carlson_dup(T (&xa)[K], T (&mp)[K], const T (&s)[K], T (&p5)[K], T (&
         const bool cap = nit >= NIT_CAP;
 #pragma unroll
         for (int k = 0; k < K; ++k) {
-            const T a3 = N::fma_(T(2), mp[k], xa[k]);                       // 3 A_n of R_F
-            bool mk = kF[k] >= N::key_(a3);
-            if (kD) mk = mk | (kDd[k] >= N::key_(N::fma_(T(2), xa[k], a3)));           // 5 A_n of R_D
+            const T m2 = N::twice_(mp[k]);
+            const T a3 = xa[k] + m2;                                        // 3 A_n of R_F (needed by the R_J tests only)
+            // 3 A_F = xa + 2 mp, or 5 A_D = 3 xa + 2 mp where that mean is the smaller one
+            bool mk = kF[k] >= N::key_(N::fma_(cx[k], xa[k], m2));
             if (kT) mk = mk | (k5[k] >= N::key_(N::fma_(T(2), p5[k], a3)));            // 5 A_n of R_J(p5)
             if (kA) mk = mk | (k0[k] >= N::key_(N::fma_(T(2), p0[k], a3)));
             mk = mk & (st[k] == 0);

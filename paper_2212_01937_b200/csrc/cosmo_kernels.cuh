@@ -184,6 +184,7 @@ __global__ void __launch_bounds__(OUTER_THREADS, CB_MINBLOCKS) k_outer(OuterArgs
     for (int k = 0; k < KZ; ++k) gzacc[k] = T(0);
     const VoteWarp vote;
 
+    cudaGridDependencySynchronize();          // PDL: k_prep's constants (everything above only read the caller's inputs)
     for (int64_t c0 = (int64_t)blockIdx.y * S_CHUNK; c0 < S; c0 += (int64_t)gridDim.y * S_CHUNK) {
         const int ns = (int)((S - c0 < S_CHUNK) ? (S - c0) : S_CHUNK);
         __syncthreads();
@@ -314,6 +315,7 @@ __global__ void __launch_bounds__(OUTER_THREADS, CB_MINBLOCKS) k_outer(OuterArgs
 template <int NP>
 __global__ void k_reduce_params(const double* __restrict__ part, int64_t ntiles, int64_t S, double* __restrict__ logL,
                                 double* __restrict__ grad) {
+    cudaGridDependencySynchronize();          // PDL: the OUTER kernel's partial sums
     // one warp per (s, j)
     const int64_t wid = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) >> 5;
     const int lane = threadIdx.x & 31;
@@ -332,6 +334,32 @@ __global__ void k_reduce_params(const double* __restrict__ part, int64_t ntiles,
             grad[(int64_t)j * S + s] = v;
         }
     }
+}
+
+// the two reductions of an OUTER VJP in ONE launch: blocks [0, nb_gz) sum the grad_z partials of the cosmology groups (if any),
+// the others the per-tile parameter sums (as k_reduce_params<4>)
+template <typename T>
+__global__ void k_reduce_vjp(const double* __restrict__ part, int64_t ntiles, int64_t S, double* __restrict__ grad,
+                             const T* __restrict__ gzpart, int ny, int64_t N, T* __restrict__ gz, unsigned nb_gz) {
+    cudaGridDependencySynchronize();          // PDL: the OUTER kernel's partial sums
+    if (blockIdx.x < nb_gz) {
+        const int64_t n = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+        if (n >= N) return;
+        T v = T(0);
+        for (int y = 0; y < ny; ++y) v += gzpart[(int64_t)y * N + n];
+        gz[n] = v;
+        return;
+    }
+    const int64_t wid = ((blockIdx.x - nb_gz) * (int64_t)blockDim.x + threadIdx.x) >> 5;
+    const int lane = threadIdx.x & 31;
+    if (wid >= S * 4) return;
+    const int64_t s = wid >> 2;
+    const int j = (int)(wid & 3);
+    double v = 0.0;
+    const double* __restrict__ row = part + (s * 4 + j) * ntiles;
+    for (int64_t t = lane; t < ntiles; t += 32) v += row[t];
+    v = warp_sum(v);
+    if (lane == 0) grad[(int64_t)j * S + s] = v;
 }
 
 template <typename T>

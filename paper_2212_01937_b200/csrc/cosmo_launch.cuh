@@ -59,6 +59,8 @@ void launch_outer_f32(int mode, const OuterArgs& a, dim3 grid, cudaStream_t st);
 void launch_elem_f64(bool with_grad, const ElemArgs& a, cudaStream_t st);
 void launch_elem_f32(bool with_grad, const ElemArgs& a, cudaStream_t st);
 void launch_reduce_params(int np, const double* part, int64_t ntiles, int64_t S, double* logL, double* grad, cudaStream_t st);
+void launch_reduce_vjp(bool f32, const double* part, int64_t ntiles, int64_t S, double* grad, const void* gzpart, int ny, int64_t N, void* gz,
+                       cudaStream_t st);
 void launch_reduce_gz(bool f32, const void* part, int ny, int64_t N, void* gz, cudaStream_t st);
 void launch_two(const double* z1, const double* z2, const double* Om, const double* OL, const double* Or, const double* H0, int64_t n,
                 int64_t n_cosmo, unsigned which, const double* gout, double* out, double* gz1, double* gz2, double* gparams,
@@ -70,5 +72,21 @@ void launch_carlson_pair(const double* x, const double* m, const double* s, cons
 void launch_probe_fma(bool f32, int blocks, int iters, void* sink, cudaStream_t st);
 
 inline int64_t cdiv64(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+#ifdef __CUDACC__
+// Launch with programmatic dependent launch (PDL): the kernel may start while its predecessor in the stream is still draining; it
+// must call cudaGridDependencySynchronize() before touching anything the predecessor wrote.  Closes most of the gap that a chain of
+// short launches (prep -> outer -> reduce) otherwise leaves between kernels.
+template <typename... KArgs, typename... Args>
+inline void launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = 0; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+#endif
 
 }  // namespace cb

@@ -153,8 +153,14 @@ void launch_prep(const double* Om, const double* OL, const double* Or, const dou
     k_prep<<<(unsigned)cdiv64(S, 64), 64, 0, st>>>(Om, OL, Or, H0, S, want_grad, out);
 }
 void launch_reduce_params(int np, const double* part, int64_t ntiles, int64_t S, double* logL, double* grad, cudaStream_t st) {
-    if (np == 5) k_reduce_params<5><<<(unsigned)cdiv64(S * 5 * 32, 256), 256, 0, st>>>(part, ntiles, S, logL, grad);
-    else k_reduce_params<4><<<(unsigned)cdiv64(S * 4 * 32, 256), 256, 0, st>>>(part, ntiles, S, nullptr, grad);
+    if (np == 5) launch_pdl(k_reduce_params<5>, dim3((unsigned)cdiv64(S * 5 * 32, 256)), dim3(256), st, part, ntiles, S, logL, grad);
+    else launch_pdl(k_reduce_params<4>, dim3((unsigned)cdiv64(S * 4 * 32, 256)), dim3(256), st, part, ntiles, S, (double*)nullptr, grad);
+}
+void launch_reduce_vjp(bool f32, const double* part, int64_t ntiles, int64_t S, double* grad, const void* gzpart, int ny, int64_t N, void* gz,
+                       cudaStream_t st) {
+    const unsigned nb_gz = gzpart ? (unsigned)cdiv64(N, 256) : 0u, nb_p = (unsigned)cdiv64(S * 4 * 32, 256);
+    if (f32) launch_pdl(k_reduce_vjp<float>, dim3(nb_gz + nb_p), dim3(256), st, part, ntiles, S, grad, static_cast<const float*>(gzpart), ny, N, static_cast<float*>(gz), nb_gz);
+    else launch_pdl(k_reduce_vjp<double>, dim3(nb_gz + nb_p), dim3(256), st, part, ntiles, S, grad, static_cast<const double*>(gzpart), ny, N, static_cast<double*>(gz), nb_gz);
 }
 void launch_reduce_gz(bool f32, const void* part, int ny, int64_t N, void* gz, cudaStream_t st) {
     if (f32) k_reduce_gz<float><<<(unsigned)cdiv64(N, 256), 256, 0, st>>>(static_cast<const float*>(part), ny, N, static_cast<float*>(gz));

@@ -7,12 +7,12 @@ template <int MODE>
 static void outer_dispatch_f64(const OuterArgs& a, dim3 grid, cudaStream_t st) {
     using T = double;
     const bool kT = a.which & (W_TL | W_AGE), kA = a.which & W_DABS;
-    if (MODE == MODE_SNIA || MODE == MODE_JOINT) k_outer<T, false, false, MODE, W_MU><<<grid, OUTER_THREADS, 0, st>>>(a);
-    else if (kT && kA) k_outer<T, true, true, MODE, 0><<<grid, OUTER_THREADS, 0, st>>>(a);
-    else if (kT) k_outer<T, true, false, MODE, 0><<<grid, OUTER_THREADS, 0, st>>>(a);
-    else if (kA) k_outer<T, false, true, MODE, 0><<<grid, OUTER_THREADS, 0, st>>>(a);
-    else if (a.which == W_MU) k_outer<T, false, false, MODE, W_MU><<<grid, OUTER_THREADS, 0, st>>>(a);
-    else k_outer<T, false, false, MODE, 0><<<grid, OUTER_THREADS, 0, st>>>(a);
+    if (MODE == MODE_SNIA || MODE == MODE_JOINT) launch_pdl(k_outer<T, false, false, MODE, W_MU>, grid, dim3(OUTER_THREADS), st, a);
+    else if (kT && kA) launch_pdl(k_outer<T, true, true, MODE, 0>, grid, dim3(OUTER_THREADS), st, a);
+    else if (kT) launch_pdl(k_outer<T, true, false, MODE, 0>, grid, dim3(OUTER_THREADS), st, a);
+    else if (kA) launch_pdl(k_outer<T, false, true, MODE, 0>, grid, dim3(OUTER_THREADS), st, a);
+    else if (a.which == W_MU) launch_pdl(k_outer<T, false, false, MODE, W_MU>, grid, dim3(OUTER_THREADS), st, a);
+    else launch_pdl(k_outer<T, false, false, MODE, 0>, grid, dim3(OUTER_THREADS), st, a);
 }
 
 void launch_outer_f64_like(int mode, const OuterArgs& a, dim3 grid, cudaStream_t st);      // tu_outer_f64_like.cu

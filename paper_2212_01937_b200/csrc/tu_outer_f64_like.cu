@@ -4,8 +4,8 @@
 namespace cb {
 
 void launch_outer_f64_like(int mode, const OuterArgs& a, dim3 grid, cudaStream_t st) {
-    if (mode == MODE_SNIA) k_outer<double, false, false, MODE_SNIA, W_MU><<<grid, OUTER_THREADS, 0, st>>>(a);
-    else k_outer<double, false, false, MODE_JOINT, W_MU><<<grid, OUTER_THREADS, 0, st>>>(a);
+    if (mode == MODE_SNIA) launch_pdl(k_outer<double, false, false, MODE_SNIA, W_MU>, grid, dim3(OUTER_THREADS), st, a);
+    else launch_pdl(k_outer<double, false, false, MODE_JOINT, W_MU>, grid, dim3(OUTER_THREADS), st, a);
 }
 
 }  // namespace cb
