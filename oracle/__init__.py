@@ -41,6 +41,8 @@ def lib():
         _lib.oracle_observables2_batch.restype = None
         _lib.oracle_w_chi_batch.argtypes = [C.c_int64] + [_DP] * 7 + [C.c_int64, _LDP, _LDP, C.POINTER(C.c_int32)]
         _lib.oracle_w_chi_batch.restype = None
+        _lib.oracle_w_observables_batch.argtypes = [C.c_int64] + [_DP] * 7 + [C.c_int64, _LDP, _LDP, C.POINTER(C.c_int32)]
+        _lib.oracle_w_observables_batch.restype = None
         _lib.oracle_snia_logjoint.argtypes = [C.c_int64, _DP, _DP, _DP, _DP] + [C.c_double] * 7 + [C.c_int, _LDP, _LDP]
         _lib.oracle_snia_logjoint.restype = C.c_int
         for name, nin in (("oracle_rf", 6), ("oracle_rc", 4), ("oracle_rd", 6), ("oracle_rj", 8)):
@@ -179,6 +181,28 @@ def w_chi_batch(z, Om, OL, Or, Ow13, Ow23, H0, threads=None):
         L.oracle_set_threads(int(threads))
     L.oracle_w_chi_batch(n, _dp(z), *[_dp(p) for p in ps], n_cosmo, _ldp(val), _ldp(dz), status.ctypes.data_as(C.POINTER(C.c_int32)))
     return val, dz, status
+
+
+WRTW = ("z", "Om", "OL", "Or", "Ow13", "Ow23", "H0")
+
+
+def w_observables_batch(z, Om, OL, Or, Ow13, Ow23, H0, with_grad=True, threads=None):
+    """All six observables (OBS order) with extra constant-w components and their total derivatives (WRTW order):
+    val[n,6], grad[n,6,7] or None, status[n] (0 ok, -1 invalid path, 1 D_L <= 0).  PAPER.md:82 fn.4; SURVEY NEXT-3."""
+    z = np.ascontiguousarray(z, dtype=np.float64)
+    n = z.shape[0]
+    ps = [np.ascontiguousarray(np.atleast_1d(p), dtype=np.float64) for p in (Om, OL, Or, Ow13, Ow23, H0)]
+    n_cosmo = ps[0].shape[0]
+    assert all(p.shape[0] == n_cosmo for p in ps) and n_cosmo in (1, n)
+    val = np.zeros((n, N_OBS), dtype=np.longdouble)
+    grad = np.zeros((n, N_OBS, 7), dtype=np.longdouble) if with_grad else None
+    status = np.zeros(n, dtype=np.int32)
+    L = lib()
+    if threads:
+        L.oracle_set_threads(int(threads))
+    L.oracle_w_observables_batch(n, _dp(z), *[_dp(p) for p in ps], n_cosmo, _ldp(val), _ldp(grad) if with_grad else None,
+                                 status.ctypes.data_as(C.POINTER(C.c_int32)))
+    return val, grad, status
 
 
 def snia_logjoint(z, z_obs, mu_obs, sigma_mu, sigma_z, beta, shape, Om, OL, Or, H0, with_grad=True):

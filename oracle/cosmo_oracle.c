@@ -35,6 +35,9 @@
  *                              that the paper's closed forms equal the quadrature.
  *  (5) oracle_snia_loglike   : the Gaussian mu-likelihood of PAPER.md:283 summed over
  *                              objects, with parameter gradients, by direct summation.
+ *  (6)-(10)                  : further down, each with its own header: the section-4 log-joint, the two-limit forms, the
+ *                              derived observables, the extra constant-w components (chi family; then all six observables
+ *                              with every gradient).
  *
  * Pins (tests/test_oracle_*.py): closed forms (Einstein-de Sitter, de Sitter, Milne,
  * radiation-only, flat LCDM t_L/age/d_abs, Mattig), flat-LCDM 2F1 expression,
@@ -834,6 +837,118 @@ void oracle_w_chi_batch(int64_t n, const double *z, const double *Om, const doub
     for (int64_t i = 0; i < n; ++i) {
         int64_t j = (n_cosmo == 1) ? 0 : i;
         int rc = oracle_w_chi((ld)z[i], (ld)Om[j], (ld)OL[j], (ld)Or[j], (ld)Ow13[j], (ld)Ow23[j], (ld)H0[j], val + i * 4, dz + i * 4);
+        if (status) status[i] = rc;
+    }
+}
+
+/* ======================================================================================
+ * (10) the w family in full (rest): all three integrals of eqs. (2.3)-(2.5) for the polynomial of (9), the six
+ *      observables of (2) and their total derivatives with respect to (z, Om, OL, Or, Ow13, Ow23, H0), Ok = 1 - (sum of the five
+ *      densities) eliminated: by Leibniz' rule
+ *        dE^2/dOm = x^3 - x^2, dE^2/dOL = 1 - x^2, dE^2/dOr = x^4 - x^2, dE^2/dOw13 = x^2 - x^2 = 0, dE^2/dOw23 = x - x^2,
+ *      and dOk/dtheta = -1 for each of the five in the curvature transform.  Same adaptive GK21 in u = ln x, written out for this
+ *      integrand set so that (1) and (9) stay exactly as pinned.
+ *      q[15] = I0, T, A, then d I0 / d(Om, OL, Or, Ow23), d T / d(..), d A / d(..)   (Ow13: identically zero, not stored).
+ * ====================================================================================== */
+#define NVW 15
+static ld w_integrand_full(const poly4_t *p, int nv, ld u, ld f[NVW]) {
+    ld x = expl(u);
+    ld E2 = w_E2(p, x);
+    ld kappa = ((((fabsl(p->a4) * x + fabsl(p->a3)) * x + fabsl(p->a2)) * x + fabsl(p->a1)) * x + fabsl(p->a0)) / fabsl(E2);
+    ld E = sqrtl(E2);
+    f[0] = x / E; f[1] = 1.0L / E; f[2] = x * x * x / E;
+    if (nv > 3) {
+        ld E3 = E2 * E, x2 = x * x, zz = expm1l(u);
+        ld d[4] = { x2 * zz, -zz * (x + 1.0L), x2 * zz * (x + 1.0L), -x * zz };      /* x^3-x^2, 1-x^2, x^4-x^2, x-x^2 */
+        ld w[3] = { -0.5L * x / E3, -0.5L / E3, -0.5L * x2 * x / E3 };
+        for (int k = 0; k < 3; ++k)
+            for (int t = 0; t < 4; ++t) f[3 + 4 * k + t] = w[k] * d[t];
+    }
+    return kappa;
+}
+static void w_panel_full(const poly4_t *p, int nv, ld a, ld b, ld K[NVW], ld G[NVW], ld Kabs[NVW]) {
+    ld h = 0.5L * (b - a), m = 0.5L * (a + b), f[NVW];
+    for (int v = 0; v < nv; ++v) K[v] = G[v] = Kabs[v] = 0.0L;
+    for (int i = 0; i < 21; ++i) {
+        ld kappa = w_integrand_full(p, nv, m + h * GK21_X[i], f);
+        for (int v = 0; v < nv; ++v) { K[v] += GK21_WK[i] * f[v]; G[v] += GK21_WG[i] * f[v]; Kabs[v] += GK21_WK[i] * fabsl(f[v]) * kappa; }
+    }
+    for (int v = 0; v < nv; ++v) { K[v] *= h; G[v] *= h; Kabs[v] *= h; }
+}
+static void w_adapt_full(const poly4_t *p, int nv, ld a, ld b, ld frac, const ld scale[NVW], int depth, ld acc[NVW], int *npanels) {
+    ld K[NVW], G[NVW], Kabs[NVW];
+    w_panel_full(p, nv, a, b, K, G, Kabs);
+    int ok = 1;
+    for (int v = 0; v < nv; ++v) {
+        ld err = fabsl(K[v] - G[v]);
+        if (err > GK_TOL * scale[v] * frac && err > GK_ROUND * LDBL_EPSILON * Kabs[v]) ok = 0;
+        if (err != err) ok = 1;
+    }
+    if (ok || depth >= GK_MAXDEPTH || *npanels >= GK_MAXPANELS) { for (int v = 0; v < nv; ++v) acc[v] += K[v]; ++*npanels; return; }
+    ld m = 0.5L * (a + b);
+    w_adapt_full(p, nv, a, m, 0.5L * frac, scale, depth + 1, acc, npanels);
+    w_adapt_full(p, nv, m, b, 0.5L * frac, scale, depth + 1, acc, npanels);
+}
+
+enum { WWRT_Z = 0, WWRT_OM, WWRT_OL, WWRT_OR, WWRT_OW13, WWRT_OW23, WWRT_H0, N_WWRT };
+
+/* val[N_OBS] (order of (2): DC, DM, DL, MU, TL, DABS), grad[N_OBS][N_WWRT] (nullable).  Returns 0, -1 (invalid path: NaN) or 1 (D_L <= 0). */
+int oracle_w_observables(ld z, ld Om, ld OL, ld Or, ld Ow13, ld Ow23, ld H0, ld val[N_OBS], ld *grad) {
+    ld Ok = 1.0L - Om - OL - Or - Ow13 - Ow23;
+    poly4_t p = { Or, Om, Ok + Ow13, Ow23, OL };
+    for (int i = 0; i < N_OBS; ++i) val[i] = NAN;
+    if (grad) for (int i = 0; i < N_OBS * N_WWRT; ++i) grad[i] = NAN;
+    if (!(z > -1.0L)) return -1;
+    ld U = log1pl(z), q[NVW];
+    int nv = grad ? NVW : 3;
+    for (int v = 0; v < NVW; ++v) q[v] = 0.0L;
+    for (int i = 0; i <= 64; ++i)
+        if (!(w_E2(&p, expl(U * i / 64.0L)) > 0.0L)) return -1;
+    if (z != 0.0L) {
+        ld scale[NVW], K[NVW], G[NVW], Kabs[NVW];
+        w_panel_full(&p, nv, 0.0L, U, K, G, Kabs);
+        for (int v = 0; v < nv; ++v) scale[v] = fabsl(K[v]);
+        int npanels = 0, nseg = (int)ceill(fabsl(U));
+        if (nseg < 1) nseg = 1;
+        for (int s = 0; s < nseg; ++s) w_adapt_full(&p, nv, U * s / nseg, U * (s + 1) / nseg, 1.0L / nseg, scale, 0, q, &npanels);
+    }
+    ld x = 1.0L + z, E = sqrtl(w_E2(&p, x)), dH = C_KM_S / H0, tH = HUBBLE_GYR / H0;
+    ld I0 = q[0], T = q[1], A = q[2], F, Fi, Fk;
+    sinn_transform(Ok, I0, &F, &Fi, &Fk);
+    val[OBS_DC] = dH * I0; val[OBS_DM] = dH * F; val[OBS_DL] = x * dH * F;
+    int status = 0;
+    if (val[OBS_DL] > 0) val[OBS_MU] = 5.0L * log10l(val[OBS_DL]) + 25.0L;
+    else { val[OBS_MU] = NAN; status = 1; }
+    val[OBS_TL] = tH * T; val[OBS_DABS] = dH * A;
+    if (!grad) return status;
+    ld (*g)[N_WWRT] = (ld (*)[N_WWRT])grad;
+    g[OBS_DC][WWRT_Z] = dH / E;
+    g[OBS_DM][WWRT_Z] = dH * Fi / E;
+    g[OBS_DL][WWRT_Z] = dH * F + x * g[OBS_DM][WWRT_Z];
+    g[OBS_TL][WWRT_Z] = tH / (x * E);
+    g[OBS_DABS][WWRT_Z] = dH * x * x / E;
+    const int col[5] = { 0, 1, 2, -1, 3 };             /* Om, OL, Or, Ow13 (no E^2 dependence), Ow23 -> column of q */
+    for (int t = 0; t < 5; ++t) {
+        ld dI = col[t] >= 0 ? q[3 + col[t]] : 0.0L, dT = col[t] >= 0 ? q[7 + col[t]] : 0.0L, dA = col[t] >= 0 ? q[11 + col[t]] : 0.0L;
+        g[OBS_DC][WWRT_OM + t] = dH * dI;
+        g[OBS_DM][WWRT_OM + t] = dH * (Fi * dI - Fk);           /* dOk/dtheta = -1 */
+        g[OBS_DL][WWRT_OM + t] = x * g[OBS_DM][WWRT_OM + t];
+        g[OBS_TL][WWRT_OM + t] = tH * dT;
+        g[OBS_DABS][WWRT_OM + t] = dH * dA;
+    }
+    for (int o = 0; o < N_OBS; ++o) if (o != OBS_MU) g[o][WWRT_H0] = -val[o] / H0;
+    for (int w = 0; w < N_WWRT; ++w)
+        g[OBS_MU][w] = (status == 0) ? 5.0L / logl(10.0L) * g[OBS_DL][w] / val[OBS_DL] : NAN;
+    return status;
+}
+
+void oracle_w_observables_batch(int64_t n, const double *z, const double *Om, const double *OL, const double *Or, const double *Ow13,
+                                const double *Ow23, const double *H0, int64_t n_cosmo, ld *val, ld *grad, int32_t *status) {
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < n; ++i) {
+        int64_t j = (n_cosmo == 1) ? 0 : i;
+        int rc = oracle_w_observables((ld)z[i], (ld)Om[j], (ld)OL[j], (ld)Or[j], (ld)Ow13[j], (ld)Ow23[j], (ld)H0[j], val + i * N_OBS,
+                                      grad ? grad + i * N_OBS * N_WWRT : NULL);
         if (status) status[i] = rc;
     }
 }

@@ -112,3 +112,100 @@ def test_dz_by_finite_differences():
 def test_invalid_path_and_status():
     v, d, s = oracle.w_chi_batch(np.array([5.0]), 0.1, 2.0, 0.0, 0.0, 0.05, H0)      # no Big Bang: E^2 < 0 at x = 2
     assert s[0] == -1 and np.isnan(v).all()
+
+
+# ---------------------------------------------------------------- all six observables with every gradient (oracle.w_observables_batch)
+OBS6 = {n: i for i, n in enumerate(oracle.OBS)}
+WRT = {n: i for i, n in enumerate(oracle.WRTW)}
+TH = 977.7922216807891 / H0
+
+
+def test_full_reduces_to_the_lcdm_oracle():
+    """no extra components: values and the (z, Om, OL, Or, H0) gradients of all six observables equal the pinned LCDM oracle's"""
+    for Om, OL, Or in ((0.3, 0.7, 0.0), (0.3, 0.6, 9e-5), (0.2, 0.9, 1e-3)):
+        v, g, s = oracle.w_observables_batch(Z, Om, OL, Or, 0.0, 0.0, H0)
+        v0, g0, s0 = oracle.observables_batch(Z, [Om], [OL], [Or], [H0], True)
+        assert (s == 0).all()
+        assert rel(v, v0).max() < 1e-17
+        assert rel(g[:, :, [0, 1, 2, 3, 6]], g0).max() < 1e-15
+    # and the chi family agrees with w_chi_batch for a mixture
+    p = (0.27, 0.55, 8e-5, 0.06, 0.09, H0)
+    v, g, _ = oracle.w_observables_batch(Z, *p)
+    vc, dc, _ = oracle.w_chi_batch(Z, *p)
+    assert rel(v[:, :4], vc).max() < 1e-17 and rel(g[:, :4, 0], dc).max() < 1e-17
+
+
+def test_full_single_and_two_component_closed_forms():
+    # E^2 = x (pure w = -2/3): T = 2 (1 - x^-1/2), A = (2/5)(x^5/2 - 1)
+    v, g, _ = oracle.w_observables_batch(Z, 0.0, 0.0, 0.0, 0.0, 1.0, H0)
+    assert rel(v[:, OBS6["TL"]], TH * _mp(lambda mp, z: 2 * (1 - 1 / mp.sqrt(1 + z)))).max() < 5e-16
+    assert rel(v[:, OBS6["DABS"]], DH * _mp(lambda mp, z: mp.mpf(2) / 5 * ((1 + z) ** mp.mpf(2.5) - 1))).max() < 5e-16
+    # E^2 = x^2 (pure w = -1/3, flat): T = 1 - 1/x, A = (x^2 - 1)/2
+    v, g, _ = oracle.w_observables_batch(Z, 0.0, 0.0, 0.0, 1.0, 0.0, H0)
+    assert rel(v[:, OBS6["TL"]], TH * _mp(lambda mp, z: z / (1 + z))).max() < 5e-16
+    assert rel(v[:, OBS6["DABS"]], DH * _mp(lambda mp, z: z * (2 + z) / 2)).max() < 5e-16
+    # E^2 = a x + b, b = 1 - a (w = -2/3 and Lambda): elementary
+    a = 0.35
+    v, g, _ = oracle.w_observables_batch(Z, 0.0, 1.0 - a, 0.0, 0.0, a, H0)
+
+    def T_ab(mp, z):
+        A_, b = mp.mpf(a), 1 - mp.mpf(a)
+        s = lambda x: mp.sqrt(A_ * x + b)
+        G = lambda x: mp.log((s(x) - mp.sqrt(b)) / (s(x) + mp.sqrt(b))) / mp.sqrt(b)
+        return G(1 + z) - G(1)
+
+    def A_ab(mp, z):
+        A_, b = mp.mpf(a), 1 - mp.mpf(a)
+        G = lambda x: 2 * mp.sqrt(A_ * x + b) * (3 * A_ ** 2 * x ** 2 - 4 * A_ * b * x + 8 * b ** 2) / (15 * A_ ** 3)
+        return G(1 + z) - G(1)
+    assert rel(v[:, OBS6["TL"]], TH * _mp(T_ab)).max() < 2e-15
+    assert rel(v[:, OBS6["DABS"]], DH * _mp(A_ab)).max() < 2e-14          # the closed form itself cancels at small z in 30 digits: ok
+    # Leibniz gradient of that case in closed form: d I0 / d Ow23 at fixed sum (OL compensates? no: Ok does): dE^2 = (x - x^2) dOw23
+    # checked against mpmath quadrature below for all parameters
+
+
+def test_full_against_mpmath_quadrature():
+    """independent quadrature (mpmath tanh-sinh, 30 digits) of the three integrals and of all twelve Leibniz gradient integrals"""
+    import mpmath as mp
+    mp.mp.dps = 30
+    Om, OL, Or, O13, O23 = 0.27, 0.55, 8e-5, 0.06, 0.09
+    Ok = 1 - Om - OL - Or - O13 - O23
+    E2 = lambda x: Or * x ** 4 + Om * x ** 3 + (Ok + O13) * x ** 2 + O23 * x + OL
+    D = {"Om": lambda x: x ** 3 - x ** 2, "OL": lambda x: 1 - x ** 2, "Or": lambda x: x ** 4 - x ** 2, "Ow23": lambda x: x - x ** 2}
+    W = {"DC": (lambda x: mp.mpf(1), DH), "TL": (lambda x: 1 / x, TH), "DABS": (lambda x: x ** 2, DH)}
+    zs = np.array([0.05, 0.8, 3.0, 40.0])
+    v, g, s = oracle.w_observables_batch(zs, Om, OL, Or, O13, O23, H0)
+    for i, z in enumerate(zs):
+        for name, (wf, unit) in W.items():
+            ref = unit * mp.quad(lambda x: wf(x) / mp.sqrt(E2(x)), [1, 1 + mp.mpf(float(z))])
+            assert abs(mp.mpf(float(v[i, OBS6[name]])) - ref) <= 1e-15 * abs(ref), (z, name)
+            for th, Df in D.items():
+                ref = -unit / 2 * mp.quad(lambda x: wf(x) * Df(x) / E2(x) ** mp.mpf(1.5), [1, 1 + mp.mpf(float(z))])
+                got = mp.mpf(float(g[i, OBS6[name], WRT[th]]))
+                assert abs(got - ref) <= 1e-14 * abs(ref), (z, name, th)
+            assert g[i, OBS6[name], WRT["Ow13"]] == 0          # Ow13 enters E^2 exactly like curvature: no E^2 dependence at fixed sum
+    # ... but the transverse distance feels it through Ok alone (PAPER.md:95): d D_M / d Ow13 = -d_H dF/dOk != 0
+    assert (np.abs(g[:, OBS6["DM"], WRT["Ow13"]].astype(float)) > 1e-3 * np.abs(v[:, OBS6["DM"]].astype(float)) * zs ** 2 * 0.1).all()
+
+
+def test_full_gradients_by_finite_differences():
+    """Richardson-extrapolated central differences of the VALUES for every observable and every parameter (long double)"""
+    th = [0.27, 0.55, 8e-5, 0.06, 0.09, 68.0]
+    zs = np.array([0.03, 0.7, 2.2, 15.0])
+    v, g, s = oracle.w_observables_batch(zs, *th)
+    f = lambda zz, t: oracle.w_observables_batch(zz, *t, with_grad=False)[0]
+    hs = {"Om": 2e-4, "OL": 2e-4, "Or": 2e-6, "Ow13": 2e-4, "Ow23": 2e-4, "H0": 2e-2}
+    for k, (name, h) in enumerate(hs.items()):
+        def cd(hh):
+            tp, tm = list(th), list(th)
+            tp[k] += hh; tm[k] -= hh
+            return (f(zs, tp) - f(zs, tm)) / np.longdouble(2 * hh)
+        fd = (4 * cd(h / 2) - cd(h)) / 3
+        an = g[:, :, WRT[name]]
+        err = np.abs((fd - an).astype(float)) / np.maximum(np.abs(an.astype(float)), 1e-3 * np.abs(v.astype(float)))
+        assert err.max() <= 2e-9, (name, err.max())
+    h = 1e-4 * (1 + zs)
+    fd = (f(zs + h, th) - f(zs - h, th)) / (2 * h[:, None])
+    fd2 = (f(zs + h / 2, th) - f(zs - h / 2, th)) / h[:, None]
+    fdz = (4 * fd2 - fd) / 3
+    assert (np.abs((fdz - g[:, :, 0]).astype(float)) <= 2e-9 * np.abs(g[:, :, 0].astype(float))).all()
