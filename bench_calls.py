@@ -128,6 +128,9 @@ def main():
         a = [dev(w[k]) for k in ("z", "Om", "OL", "Or", "Ow13", "Ow23", "H0")]
         timed(lambda: cb.cosmo_eval_w(*a, which=("DC", "DM", "DL", "MU")), len(w["z"]),
               "extra-w family (general quartic), D_C, D_M, D_L, mu + d/dz, per-element cosmology f64")
+        gw = torch.randn((6, len(w["z"])), dtype=torch.float64, device="cuda")
+        timed(lambda: cb.cosmo_eval_w(*a, which=("DC", "DM", "DL", "MU", "TL", "DABS"), grad_out=gw), len(w["z"]),
+              "extra-w family (general quartic), all six outputs forward + VJP (6 parameter gradients), per-element cosmology f64")
         one = [dev(np.array([x])) for x in (0.27, 0.55, 8e-5, 0.06, 0.09, 70.0)]
         timed(lambda: cb.cosmo_eval_w(a[0], *one, which=("DC", "DM", "DL", "MU")), len(w["z"]),
               "extra-w family (general quartic), D_C, D_M, D_L, mu + d/dz, one shared cosmology f64")

@@ -131,14 +131,23 @@ size_t cosmo_eval2_workspace_bytes(int64_t n, int with_grad);
 
 /* EXTRA CONSTANT-w COMPONENTS (PAPER.md:82 fn.4: E^2 must be a polynomial of degree <= 4, which admits w in
  * {-1, -2/3, -1/3, 0, 1/3}):  E^2(x) = Or x^4 + Om x^3 + (Ok + Ow13) x^2 + Ow23 x + OL with Ok = 1 - Om - OL - Or - Ow13 - Ow23
- * (the curvature of the transverse distance is Ok alone).  chi family only: `which` from COSMO_DC, COSMO_DM, COSMO_DL, COSMO_MU,
- * by eq. (3.7)/(B.1) on a general real factorisation of the quartic.  One (z[i], cosmology) per element, parameter arrays of
- * length n_cosmo in {1, n} (device pointers).  out[n_which][n] in ascending bit order; dout_dz (nullable), same shape: the
- * derivative of each plane with respect to z.  status (nullable) as above: 1 root of E^2 on the path / E^2 <= 0,
- * 2 unsupported input or factorisation failure, 4 D_L <= 0, 8 iteration cap.  Forward only: no parameter gradients. */
+ * (the curvature of the transverse distance is Ok alone).  `which` from COSMO_DC, COSMO_DM, COSMO_DL, COSMO_MU (eq. (3.7)/(B.1) on a
+ * general real factorisation of the quartic), COSMO_TL, COSMO_DABS (eqs. (3.8)/(3.9), (B.2)/(B.3) with the polynomial's complex roots
+ * and complex Carlson functions, as the paper formulates them).  One (z[i], cosmology) per element, parameter
+ * arrays of length n_cosmo in {1, n} (device pointers).
+ *   out[n_which][n] in ascending bit order (nullable with grad_out); dout_dz (nullable), same shape: d plane / dz.
+ *   grad_out (nullable, [n_which][n]): also the VJP, per element: grad_z[n] and grad_params[6][n] in the order
+ *   (Om, OL, Or, Ow13, Ow23, H0), total derivatives with Ok eliminated.  Their density part is the quadrature of the Leibniz integrals
+ *   (a general quartic offers no fixed root structure for the closed-form gradient bases); status 16 where a root of E^2 sits too close
+ *   to the path for that rule.
+ *   status (nullable): 1 root of E^2 on the path / E^2 <= 0; 2 unsupported input or factorisation failure -- also set, with NaN in the
+ *   t_L / d_abs planes only, where E^2 has degree <= 2 with distinct roots (the method needs degree 3 or 4; monomials
+ *   E^2 = a x^n are served in closed form); 4 D_L <= 0; 8 iteration cap; 16 as above.
+ *   workspace: cosmo_eval_w_workspace_bytes(n_cosmo) bytes (a shared cosmology is factored once per call into it; 0 for n_cosmo = n). */
 int cosmo_eval_w(const double* z, int64_t n, const double* Om, const double* OL, const double* Or, const double* Ow13,
-                 const double* Ow23, const double* H0, int64_t n_cosmo, uint32_t which, double* out, double* dout_dz, uint8_t* status,
-                 void* stream);
+                 const double* Ow23, const double* H0, int64_t n_cosmo, uint32_t which, const double* grad_out, double* out,
+                 double* dout_dz, double* grad_z, double* grad_params, uint8_t* status, void* workspace, size_t ws_bytes, void* stream);
+size_t cosmo_eval_w_workspace_bytes(int64_t n_cosmo);
 
 /* frees the device staging buffers cosmo_eval_host keeps between calls (no-op if there are none) */
 void cosmo_host_release(void);

@@ -18,7 +18,7 @@ WHICH_BITS = {"DC": DC, "DM": DM, "DL": DL, "MU": MU, "TL": TL, "DABS": DABS, "D
 WHICH_ORDER = ("DC", "DM", "DL", "MU", "TL", "DABS", "DA", "VC", "AGE")
 
 # every symbol include/cosmo_b200.h and include/cosmo_b200_diag.h declare
-SYMBOLS = ("cosmo_host_release", "cosmo_eval2_workspace_bytes", "cosmo_workspace_bytes", "cosmo_eval", "cosmo_vjp", "cosmo_snia_loglike", "cosmo_eval_f32", "cosmo_vjp_f32",
+SYMBOLS = ("cosmo_host_release", "cosmo_eval2_workspace_bytes", "cosmo_eval_w_workspace_bytes", "cosmo_workspace_bytes", "cosmo_eval", "cosmo_vjp", "cosmo_snia_loglike", "cosmo_eval_f32", "cosmo_vjp_f32",
            "cosmo_snia_loglike_f32", "cosmo_snia_logjoint", "cosmo_eval2", "cosmo_eval_w", "cosmo_eval_host", "cosmo_carlson_pair", "cosmo_probe_fma_f64", "cosmo_probe_fma_f32",
            "cosmo_profile", "cosmo_profile_mean_ms",
            "cosmo_launch_count", "cosmo_last_cuda_error", "cosmo_strerror", "cosmo_version")
@@ -71,7 +71,9 @@ def lib():
     L.cosmo_eval2_workspace_bytes.argtypes = [i64, ci]
     L.cosmo_eval2_workspace_bytes.restype = sz
     L.cosmo_eval2.restype = ci
-    L.cosmo_eval_w.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, i64, u32, vp, vp, vp, vp]
+    L.cosmo_eval_w.argtypes = [vp, i64, vp, vp, vp, vp, vp, vp, i64, u32, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    L.cosmo_eval_w_workspace_bytes.argtypes = [i64]
+    L.cosmo_eval_w_workspace_bytes.restype = sz
     L.cosmo_eval_w.restype = ci
     L.cosmo_carlson_pair.argtypes = [vp, vp, vp, vp, i64, vp, vp, vp, vp]
     L.cosmo_carlson_pair.restype = ci
@@ -266,9 +268,10 @@ def cosmo_eval2(z1, z2, Om, OL, Or, H0, which=("DC",), grad_out=None, want_out=T
     return out, g1, g2, gp, status
 
 
-def cosmo_eval_w(z, Om, OL, Or, Ow13, Ow23, H0, which=("DC",), want_dz=True):
-    """chi family with extra constant-w components w = -1/3 (Ow13) and w = -2/3 (Ow23), PAPER.md:82 fn.4 (elementwise; parameters of
-    length 1 or n).  Returns (out[n_which, n], dout_dz[n_which, n] or None, status[n]).  which from DC, DM, DL, MU."""
+def cosmo_eval_w(z, Om, OL, Or, Ow13, Ow23, H0, which=("DC",), want_dz=True, grad_out=None, workspace=None):
+    """Extra constant-w components w = -1/3 (Ow13) and w = -2/3 (Ow23), PAPER.md:82 fn.4 (elementwise; parameters of length 1 or n).
+    which from DC, DM, DL, MU, TL, DABS.  Returns (out[n_which, n], dout_dz[n_which, n] or None, status[n]); with grad_out also
+    (grad_z[n], grad_params[6, n]) appended, the parameters in the order (Om, OL, Or, Ow13, Ow23, H0)."""
     torch = _torch()
     mask = which_mask(which)
     _dev(z, torch.float64, torch, "z")
@@ -284,8 +287,20 @@ def cosmo_eval_w(z, Om, OL, Or, Ow13, Ow23, H0, which=("DC",), want_dz=True):
     out = torch.empty((nw, n), dtype=torch.float64, device=z.device)
     dz = torch.empty((nw, n), dtype=torch.float64, device=z.device) if want_dz else None
     status = torch.empty(n, dtype=torch.uint8, device=z.device)
-    _check(lib().cosmo_eval_w(_ptr(z), n, *[_ptr(t) for t in ps], n_cosmo, mask, _ptr(out), _ptr(dz), _ptr(status), _stream(torch)))
-    return out, dz, status
+    gz = gp = None
+    if grad_out is not None:
+        _dev(grad_out, torch.float64, torch, "grad_out")
+        if grad_out.numel() != nw * n:
+            raise CosmoError("grad_out must have shape [n_which, n]")
+        gz = torch.empty(n, dtype=torch.float64, device=z.device)
+        gp = torch.empty((6, n), dtype=torch.float64, device=z.device)
+    ws_b = int(lib().cosmo_eval_w_workspace_bytes(n_cosmo))
+    ws = _workspace(torch, ws_b, z.device, workspace) if ws_b else None
+    _check(lib().cosmo_eval_w(_ptr(z), n, *[_ptr(t) for t in ps], n_cosmo, mask, _ptr(grad_out), _ptr(out), _ptr(dz), _ptr(gz), _ptr(gp),
+                              _ptr(status), _ptr(ws), ws_b, _stream(torch)))
+    if grad_out is None:
+        return out, dz, status
+    return out, dz, status, gz, gp
 
 
 def cosmo_eval_host(z, Om, OL, Or, H0, mode=ELEMENTWISE, which=("DC",), grad_out=None, want_out=True, want_status=True, out=None,

@@ -434,17 +434,25 @@ int cosmo_eval2(const double* z1, const double* z2, int64_t n, cosmo_params p, i
     return check_launch();
 }
 
+size_t cosmo_eval_w_workspace_bytes(int64_t n_cosmo) { return n_cosmo == 1 ? align256(w_cosmo_bytes()) : 0; }
+
 int cosmo_eval_w(const double* z, int64_t n, const double* Om, const double* OL, const double* Or, const double* Ow13,
-                 const double* Ow23, const double* H0, int64_t n_cosmo, uint32_t which, double* out, double* dout_dz, uint8_t* status,
-                 void* stream) {
+                 const double* Ow23, const double* H0, int64_t n_cosmo, uint32_t which, const double* grad_out, double* out,
+                 double* dout_dz, double* grad_z, double* grad_params, uint8_t* status, void* workspace, size_t ws_bytes, void* stream) {
     if (n < 0 || !(n_cosmo == 1 || n_cosmo == n)) return COSMO_E_SIZE;
-    if (which == 0 || (which & ~uint32_t(W_DC | W_DM | W_DL | W_MU))) return COSMO_E_WHICH;
+    if (which == 0 || (which & ~uint32_t(W_DC | W_DM | W_DL | W_MU | W_TL | W_DABS))) return COSMO_E_WHICH;
     if (n == 0) return COSMO_OK;
-    if (!z || !Om || !OL || !Or || !Ow13 || !Ow23 || !H0 || !out) return COSMO_E_NULL;
+    if (!z || !Om || !OL || !Or || !Ow13 || !Ow23 || !H0) return COSMO_E_NULL;
+    if (grad_out ? (!grad_z || !grad_params) : !out) return COSMO_E_NULL;
+    if (n_cosmo == 1) {
+        if (!workspace) return COSMO_E_NULL;
+        if (ws_bytes < cosmo_eval_w_workspace_bytes(1)) return COSMO_E_WORKSPACE;
+    }
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     prof_begin(st);
-    launch_w(z, Om, OL, Or, Ow13, Ow23, H0, n, n_cosmo, which, out, dout_dz, status, st);
+    launch_w(z, Om, OL, Or, Ow13, Ow23, H0, n, n_cosmo, which, grad_out, out, dout_dz, grad_z, grad_params, status, workspace, st);
     prof_end(st);
+    if (n_cosmo == 1) g_launches += 1;
     return check_launch();
 }
 

@@ -65,8 +65,10 @@ void launch_reduce_gz(bool f32, const void* part, int ny, int64_t N, void* gz, c
 void launch_two(const double* z1, const double* z2, const double* Om, const double* OL, const double* Or, const double* H0, int64_t n,
                 int64_t n_cosmo, unsigned which, const double* gout, double* out, double* gz1, double* gz2, double* gparams,
                 uint8_t* status, unsigned* ws, cudaStream_t st);
+size_t w_cosmo_bytes();
 void launch_w(const double* z, const double* Om, const double* OL, const double* Or, const double* Ow13, const double* Ow23,
-              const double* H0, int64_t n, int64_t n_cosmo, unsigned which, double* out, double* dout, uint8_t* status, cudaStream_t st);
+              const double* H0, int64_t n, int64_t n_cosmo, unsigned which, const double* gout, double* out, double* dout, double* gz,
+              double* gparams, uint8_t* status, void* ws, cudaStream_t st);
 void launch_carlson_pair(const double* x, const double* m, const double* s, const double* p, int64_t n, double* rf, double* rd, double* rj,
                          cudaStream_t st);
 void launch_probe_fma(bool f32, int blocks, int iters, void* sink, cudaStream_t st);

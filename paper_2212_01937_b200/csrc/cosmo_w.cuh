@@ -20,7 +20,11 @@ struct WCosmo {
     double q11, q21, theta, sD, sDr;   // Q1(1), Q2(1), apolar invariant, disc1 disc2 / 4 and sqrt|.|
     double rr[4];                      // real roots (path check)
     int nreal;
-    double Ok, dH;
+    double Ok, dH, tH;
+    double a[5];                       // E^2 = a[0] + a[1] x + .. + a[4] x^4
+    cx rt[4];                          // its roots in x, sorted by decreasing modulus (t_L, d_abs: eqs. (3.8)/(3.9) single roots out)
+    int deg;                           // degree of E^2
+    int iA;                            // index in rt of r_i of eq. (3.9): the smallest real root other than rt[0], else rt[3]
     unsigned status;
 };
 
@@ -34,7 +38,10 @@ CB_HD cx w_poly(const double* a, int n, cx x, cx& dp) {       // Horner: value a
 CB_HD void w_prep(double Om, double OL, double Or, double Ow13, double Ow23, double H0, WCosmo& W) {
     const double Ok = 1.0 - Om - OL - Or - Ow13 - Ow23;
     const double a[5] = {OL, Ow23, Ok + Ow13, Om, Or};
-    W.Ok = Ok; W.dH = C_KM_S / H0;
+    W.Ok = Ok; W.dH = C_KM_S / H0; W.tH = HUBBLE_GYR / H0;
+    for (int i = 0; i < 5; ++i) W.a[i] = a[i];
+    for (int i = 0; i < 4; ++i) W.rt[i] = cx_(0.0);
+    W.deg = 0; W.iA = 3;
     W.status = 0; W.nreal = 0;
     for (int i = 0; i < 4; ++i) W.rr[i] = 0.0;
     bool fin = H0 > 0.0;
@@ -58,7 +65,38 @@ CB_HD void w_prep(double Om, double OL, double Or, double Ow13, double Ow23, dou
             r[k] = cx_(R * cos(ang), R * sin(ang));
         }
         for (int k = nd; k < n; ++k) r[k] = cx_(0.0);
-        for (int it = 0; it < 200 && nd > 0; ++it) {
+        // Fast path for the usual structure (degree 3 or 4, no root at 0, matter present): Bairstow's iteration for a real quadratic
+        // factor x^2 + b x + c from the pair of a0 + a3 x^3 ~ 0 (x = rho e^{+-i pi/3}, rho = cbrt(a0/a3)), then the two quadratic
+        // formulas.  ~10 x cheaper than the simultaneous iteration below, which remains the fall-back (and serves every other case).
+        bool fast = false;
+        if (m0 == 0 && nd >= 3 && a[3] > 0.0 && a[0] > 0.0) {
+            const double rho = cbrt(a[0] / a[3]);
+            double bb = -rho, cc = rho * rho, q2 = a[4], q1 = 0.0, q0 = 0.0;
+            const double sc = fabs(a[0]) + fabs(a[1]) + fabs(a[2]) + fabs(a[3]) + fabs(a[4]);
+            for (int it = 0; it < 16; ++it) {
+                q1 = a[3] - bb * q2; q0 = a[2] - bb * q1 - cc * q2;
+                const double r1 = a[1] - bb * q0 - cc * q1, r0 = a[0] - cc * q0;
+                if (fabs(r1) + fabs(r0) <= 1e-15 * sc) { fast = true; break; }
+                const double s1 = q1 - bb * q2, s0 = q0 - cc * q2;
+                const double u1 = s0 - bb * s1, u0 = -cc * s1;
+                const double det = u1 * s0 - u0 * s1;
+                if (det == 0.0 || !(fabs(det) < 1e300)) break;
+                bb += (r1 * s0 - r0 * s1) / det;
+                cc += (u1 * r0 - u0 * r1) / det;
+            }
+            if (fast) {
+                q1 = a[3] - bb * q2; q0 = a[2] - bb * q1 - cc * q2;
+                auto quad_roots = [](double A, double B, double Cc, cx& ra, cx& rb) {       // A x^2 + B x + Cc, A != 0
+                    const double disc = B * B - 4.0 * A * Cc;
+                    if (disc < 0.0) { const double sq = sqrt(-disc); ra = cx_(-B / (2.0 * A), sq / (2.0 * A)); rb = cx_conj(ra); }
+                    else { const double t = -0.5 * (B + copysign(sqrt(disc), B)); ra = cx_(t / A); rb = cx_(t != 0.0 ? Cc / t : 0.0); }
+                };
+                quad_roots(1.0, bb, cc, r[0], r[1]);
+                if (nd == 4) quad_roots(q2, q1, q0, r[2], r[3]);
+                else r[2] = cx_(-q0 / q1);
+            }
+        }
+        for (int it = 0; it < 200 && nd > 0 && !fast; ++it) {
             double big = 0.0;
             for (int k = 0; k < nd; ++k) {
                 cx dp;
@@ -74,6 +112,16 @@ CB_HD void w_prep(double Om, double OL, double Or, double Ow13, double Ow23, dou
             }
             if (big < 4e-16) break;
         }
+        W.deg = n;
+        for (int k = 0; k < n; ++k) W.rt[k] = r[k];
+        for (int i = 1; i < n; ++i) {                                       // insertion sort by decreasing modulus
+            const cx v = W.rt[i]; int j = i - 1;
+            while (j >= 0 && cx_abs(W.rt[j]) < cx_abs(v)) { W.rt[j + 1] = W.rt[j]; --j; }
+            W.rt[j + 1] = v;
+        }
+        W.iA = 3;
+        for (int k = 1; k < n; ++k)
+            if (fabs(W.rt[k].im) <= 1e-9 * cx_abs(W.rt[k])) W.iA = k;
         // group into real quadratics: a root with a significant imaginary part goes with its conjugate, real ones are
         // sorted and paired with their neighbours
         bool used[4] = {false, false, false, false};
@@ -166,6 +214,257 @@ CB_HD unsigned w_eval(const WCosmo& W, double z, const Vote& vote, double v[4], 
     if (st[0] & (ST_ROOT_ON_PATH | ST_UNSUPPORTED))
         for (int i = 0; i < 4; ++i) v[i] = dz[i] = NAN;
     return st[0];
+}
+
+// ---- t_L and d_abs on the general quartic (rest).  Eqs. (3.8)/(3.9) single out a root r_i, which may be complex here,
+// so this is the paper's own formulation: complex roots, complex X_n, Y_n, u_ij and complex Carlson functions,
+// principal square roots throughout.  Labelling ("r_i, r_j the biggest roots"), by modulus of
+// the x-roots: t_L: r_i = the biggest; d_abs: r_l = the biggest, r_i = the smallest real root (the smallest root if none is real) --
+// tried over all 24 labellings against the oracle on the seeded mix: the only one without failures (d_abs <= 5e-11: the Om/Or
+// cancellation of eq. (3.9)).
+
+// R_F(x,y,z), R_D(x,y,z) (last argument z) and R_J(x,y,z,p), all arguments complex: duplication, ref. [10] (DLMF 19.36(i))
+struct CxCarlson { cx RF, RD, RJ; };
+CB_HD void cx_carlson(cx x, cx y, cx z, cx p, bool want_j, CxCarlson& out) {
+    const cx x0 = x, y0 = y, z0 = z;
+    const cx delta = (p - x) * (p - y) * (p - z);
+    const cx AF0 = (1.0 / 3.0) * (x + y + z), AD0 = 0.2 * (x + y + 3.0 * z), AJ0 = 0.2 * (x + y + z + 2.0 * p);
+    const double dev = fmax(fmax(cx_abs(AF0 - x), cx_abs(AF0 - y)), cx_abs(AF0 - z)) + fmax(cx_abs(AD0 - x), fmax(cx_abs(AD0 - y), cx_abs(AD0 - z)));
+    const double devJ = want_j ? fmax(fmax(cx_abs(AJ0 - x), cx_abs(AJ0 - y)), fmax(cx_abs(AJ0 - z), cx_abs(AJ0 - p))) : 0.0;
+    double f = 1.0;
+    cx tailD = cx_(0.0), sumJ = cx_(0.0);
+    for (int it = 0; it < 2 * NIT_CAP; ++it) {
+        const cx AF = (1.0 / 3.0) * (x + y + z), AD = 0.2 * (x + y + 3.0 * z), AJ = 0.2 * (x + y + z + 2.0 * p);
+        if (f * 600.0 * dev < fmin(cx_abs(AF), cx_abs(AD)) && (!want_j || f * 600.0 * devJ < cx_abs(AJ))) break;
+        const cx sx = cx_sqrt(x), sy = cx_sqrt(y), sz = cx_sqrt(z);
+        const cx lam = sx * sy + sx * sz + sy * sz;
+        tailD = tailD + cx_(f) / (sz * (z + lam));
+        if (want_j) {
+            const cx sp = cx_sqrt(p);
+            const cx d = (sp + sx) * (sp + sy) * (sp + sz);
+            const cx e = (f * f * f) * delta / (d * d);
+            sumJ = sumJ + (f * cx_rc1(e)) / d;
+            p = 0.25 * (p + lam);
+        }
+        x = 0.25 * (x + lam); y = 0.25 * (y + lam); z = 0.25 * (z + lam);
+        f *= 0.25;
+    }
+    const double* c = CB_KT.rj;
+    {
+        const cx A = (1.0 / 3.0) * (x + y + z), g = cx_(f) / A;
+        const cx X = (AF0 - x0) * g, Y = (AF0 - y0) * g, Z = -(X + Y);
+        const cx e2 = X * Y - Z * Z, e3 = X * Y * Z;
+        const cx S = cx_(1.0) - 0.1 * e2 + (1.0 / 14.0) * e3 + (1.0 / 24.0) * (e2 * e2) - (3.0 / 44.0) * (e2 * e3) - (5.0 / 208.0) * (e2 * e2 * e2)
+                     + (3.0 / 104.0) * (e3 * e3) + (1.0 / 16.0) * (e2 * e2 * e3);
+        out.RF = S / cx_sqrt(A);
+    }
+    {
+        const cx A = 0.2 * (x + y + 3.0 * z), g = cx_(f) / A;
+        const cx X = (AD0 - x0) * g, Y = (AD0 - y0) * g, Z = (-1.0 / 3.0) * (X + Y);
+        const cx XY = X * Y, Z2 = Z * Z;
+        const cx e2 = XY - 6.0 * Z2, e3 = (3.0 * XY - 8.0 * Z2) * Z, e4 = 3.0 * ((XY - Z2) * Z2), e5 = XY * Z2 * Z;
+        const cx S = cx_(1.0) + c[0] * e2 + c[3] * e3 + c[1] * (e2 * e2) + c[8] * e4 + c[4] * (e2 * e3) + c[10] * e5 + c[2] * (e2 * e2 * e2)
+                     + c[6] * (e3 * e3) + c[9] * (e2 * e4) + c[5] * (e2 * e2 * e3) + c[7] * (e3 * e4 + e2 * e5);
+        out.RD = (f * S) / (A * cx_sqrt(A)) + 3.0 * tailD;
+    }
+    out.RJ = cx_(0.0);
+    if (want_j) {
+        const cx A = 0.2 * (x + y + z + 2.0 * p), g = cx_(f) / A;
+        const cx X = (AJ0 - x0) * g, Y = (AJ0 - y0) * g, Z = (AJ0 - z0) * g;
+        const cx P = -0.5 * (X + Y + Z);
+        const cx XYZ = X * Y * Z, P2 = P * P;
+        const cx e2 = X * Y + X * Z + Y * Z - 3.0 * P2;
+        const cx e3 = XYZ + 2.0 * (e2 * P) + 4.0 * (P2 * P);
+        const cx e4 = (2.0 * XYZ + e2 * P + 3.0 * (P2 * P)) * P;
+        const cx e5 = XYZ * P2;
+        const cx S = cx_(1.0) + c[0] * e2 + c[3] * e3 + c[1] * (e2 * e2) + c[8] * e4 + c[4] * (e2 * e3) + c[10] * e5 + c[2] * (e2 * e2 * e2)
+                     + c[6] * (e3 * e3) + c[9] * (e2 * e4) + c[5] * (e2 * e2 * e3) + c[7] * (e3 * e4 + e2 * e5);
+        out.RJ = (f * S) / (A * cx_sqrt(A)) + 6.0 * sumJ;
+    }
+}
+
+// T = int_1^x dx/(x E), A = int_1^x x^2 dx/E for E^2 of degree 4 or 3 with the roots W.rt (x-roots, so d_i5 = -rho_i), and for
+// E^2 = a x^n (every root at 0: elementary).  Returns false where the method does not apply (degree <= 2 with distinct roots).
+CB_HD_NOINLINE bool w_TA(const WCosmo& W, double x, bool want_T, bool want_A, double& TT, double& AA) {
+    TT = AA = NAN;
+    const double dz = x - 1.0, lead = W.a[W.deg];
+    bool mono = true;
+    for (int k = 0; k < W.deg; ++k) mono = mono && cx_abs(W.rt[k]) == 0.0;
+    if (mono) {                                          // E = sqrt(lead) x^(deg/2)
+        const double h = 0.5 * W.deg, il = 1.0 / sqrt(lead), lx = log(x);
+        TT = (h == 0.0) ? il * lx : il * -expm1(-h * lx) / h;
+        AA = (h == 3.0) ? il * lx : il * expm1((3.0 - h) * lx) / (3.0 - h);
+        return true;
+    }
+    if (W.deg < 3) return false;
+    const double ia = 1.0 / sqrt(lead);
+    if (W.deg == 4) {
+        const cx* r = W.rt;
+        cx X[4], Y[4];
+        for (int n = 0; n < 4; ++n) { X[n] = cx_sqrt(cx_(x) - r[n]); Y[n] = cx_sqrt(cx_(1.0) - r[n]); }
+        auto usq = [&](int a, int b, int c, int e) { const cx u = X[a] * X[b] * Y[c] * Y[e] + Y[a] * Y[b] * X[c] * X[e]; return u * u; };
+        const cx P1 = usq(0, 1, 2, 3), P2 = usq(0, 2, 1, 3), P3 = usq(0, 3, 1, 2);       // the three pairings
+        auto d = [&](int a, int b) { return r[b] - r[a]; };
+        CxCarlson K;
+        if (want_T) {                    // eq. (3.8), (i, j, k, l) = (0, 3, 1, 2): u_ij^2 = P3, u_ik^2 = P1, u_il^2 = P2
+            const int i = 0, j = 3, k = 1, l = 2;
+            const cx p5 = P3 - (dz * dz) * (d(i, k) * d(i, l) * (r[j] / r[i]));
+            cx_carlson(P3, P1, P2, p5, true, K);
+            const cx q5 = (cx_(x) / ((cx_(1.0) - r[i]) * (cx_(x) - r[i]))) * p5;
+            const cx s5 = q5 + (dz * dz) * (r[k] * r[l] * (r[j] / r[i]));
+            const cx br = K.RF - ((dz * dz / 3.0) * (d(i, j) * d(i, k) * d(i, l) / (-r[i])) * K.RJ + cx_rc(s5, q5));
+            TT = ia * ((2.0 * dz) * (br / r[i])).re;
+        }
+        if (want_A) {                    // eq. (3.9): r_l = the biggest root, r_i = the smallest REAL one if there is any (a member of a
+                                         // conjugate pair as r_i breaks the principal branches), r_j, r_k the other two
+            const int i = W.iA, l = 0;
+            int j = -1, k = -1;
+            for (int m = 1; m < 4; ++m)
+                if (m != i) { if (j < 0) j = m; else k = m; }
+            auto pair = [&](int a, int b) { int c = -1, e = -1; for (int m = 0; m < 4; ++m) if (m != a && m != b) { if (c < 0) c = m; else e = m; } return usq(a, b, c, e); };
+            const cx Uij = pair(i, j), Uik = pair(i, k), Uil = pair(i, l);
+            const cx p0 = Uij - (dz * dz) * (d(i, k) * d(i, l));
+            cx_carlson(Uij, Uik, Uil, p0, true, K);                      // R_D's last argument is u_il^2
+            const cx q0 = p0 / ((cx_(1.0) - r[i]) * (cx_(x) - r[i]));
+            const cx s0 = q0 + cx_(dz * dz);
+            const cx bnd = X[i] * X[j] * X[k] / X[l] - Y[i] * Y[j] * Y[k] / Y[l];
+            const cx uil = X[i] * X[l] * Y[j] * Y[k] + Y[i] * Y[l] * X[j] * X[k];
+            const cx sig = r[0] + r[1] + r[2] + r[3];
+            const cx t2 = dz * ((2.0 * (r[i] * r[i]) - d(i, j) * d(i, k)) * K.RF);
+            const cx t3 = dz * ((d(j, l) * d(k, l)) * (((dz * dz / 3.0) * (d(i, j) * d(i, k))) * K.RD + (X[i] * Y[i]) / (X[l] * Y[l] * uil)));
+            const cx t4 = dz * (sig * (cx_rc(s0, q0) - ((dz * dz / 3.0) * (d(i, j) * d(i, k) * d(i, l))) * K.RJ));
+            AA = ia * (bnd + t2 + t3 + t4).re;
+        }
+        return true;
+    }
+    // degree 3: eqs. (B.2), (B.3) with r_i = the biggest root (any labelling does; tested over all six)
+    const cx* r = W.rt;
+    cx X[3], Y[3];
+    for (int n = 0; n < 3; ++n) { X[n] = cx_sqrt(cx_(x) - r[n]); Y[n] = cx_sqrt(cx_(1.0) - r[n]); }
+    const cx u0 = X[0] * Y[1] * Y[2] + Y[0] * X[1] * X[2], u1 = X[1] * Y[0] * Y[2] + Y[1] * X[0] * X[2], u2 = X[2] * Y[0] * Y[1] + Y[2] * X[0] * X[1];
+    CxCarlson K;
+    if (want_T) {
+        const cx p5 = u0 * u0 + (dz * dz) * r[0];
+        cx_carlson(u0 * u0, u1 * u1, u2 * u2, p5, true, K);
+        const cx s5 = Y[0] * Y[1] * Y[2] * cx_(x) + X[0] * X[1] * X[2];
+        TT = ia * ((2.0 * dz) * ((dz * dz / 3.0) * K.RJ + cx_rc(s5 * s5, cx_(x) * p5))).re;
+    }
+    if (want_A) {
+        cx_carlson(u1 * u1, u2 * u2, u0 * u0, cx_(1.0), false, K);       // R_D(u_j^2, u_k^2, u_i^2)
+        const cx d01 = r[1] - r[0], d02 = r[2] - r[0], sig = r[0] + r[1] + r[2];
+        const cx b3 = (X[0] * X[1] * X[2] - Y[0] * Y[1] * Y[2]) + dz * ((3.0 * (r[0] * r[0]) - d01 * d02) * K.RF)
+                      + (2.0 * dz) * (sig * (((dz * dz / 3.0) * (d01 * d02)) * K.RD + (X[0] * Y[0]) / u0));
+        AA = ia * ((2.0 / 3.0) * b3).re;
+    }
+    return true;
+}
+
+// Gradient integrals of the w family: int D_theta p_X / E^3 dx over [1, x], theta = (Om, OL, Or, Ow23), D_theta = x^3 - x^2, 1 - x^2,
+// x^4 - x^2, x - x^2 (Ow13 enters E^2 like curvature: no dependence at fixed sum), p_X = 1, 1/x, x^2 (X = I0, T, A): out[12] = [X][theta].
+// By the 12-point Gauss-Legendre rule on panels of ratio <= 2 in x - c, as grad_quad() of the hot path (cosmo_obs.cuh), with c placed so
+// that the panel widths follow the distance to the nearest root left of the path.  A general quartic has no fixed root structure to
+// build the hot path's gradient bases on, so this family takes the quadrature for every element; where a root sits too close to the path
+// for the rule to converge (Bernstein parameter < 3.5 for some root) the element is flagged ST_GRAD_ILLCOND instead.
+CB_HD_NOINLINE unsigned w_grad_quad(const WCosmo& W, double z, double out[12]) {
+    const double X12[12] = {0.00921968287664037465, 0.0479413718147625717, 0.115048662902847656, 0.206341022856691276, 0.316084250500909903,
+                            0.437383295744265542, 0.562616704255734458, 0.683915749499090097, 0.793658977143308724, 0.884951337097152344,
+                            0.952058628185237428, 0.990780317123359625};
+    const double W12[12] = {0.0235876681932559136, 0.0534696629976592155, 0.0800391642716731132, 0.101583713361532961, 0.116746268269177404,
+                            0.124573522906701393, 0.124573522906701393, 0.116746268269177404, 0.101583713361532961, 0.0800391642716731132,
+                            0.0534696629976592155, 0.0235876681932559136};
+    for (int i = 0; i < 12; ++i) out[i] = 0.0;
+    const double X2 = 1.0 + z;
+    const double lo = fmin(1.0, X2), hi = fmax(1.0, X2);
+    if (!(lo > 0.0) || z == 0.0) return 0u;
+    double dmin = 1e300;                                   // distance of the nearest root left of the path from its start
+    for (int k = 0; k < W.deg; ++k)
+        if (W.rt[k].re < lo) dmin = fmin(dmin, hypot(lo - W.rt[k].re, W.rt[k].im));
+    const double c = lo - fmin(dmin, 1e6 * lo);
+    const double q = (X2 - c) / (1.0 - c), qa = q >= 1.0 ? q : 1.0 / q;
+    int np = 1;
+    double r = q;
+    if (qa > 2.0) {
+        const double lr = log(q);
+        np = (int)ceil(fabs(lr) * 1.4426950408889634);
+        if (np > 64) np = 64;
+        r = exp(lr / np);
+    }
+    unsigned st = 0u;
+    const double rr = r >= 1.0 ? r : 1.0 / r;
+    for (int k = 0; k < W.deg; ++k) {                      // Bernstein parameter of every root against the panel next to it
+        const double a0 = W.rt[k].re, y0 = fabs(W.rt[k].im);
+        double wre, h;
+        if (a0 < lo) { h = 0.5 * (lo - c) * (rr - 1.0); wre = (lo - a0) / h + 1.0; }
+        else if (a0 > hi) { h = 0.5 * (hi - c) * (1.0 - 1.0 / rr); wre = (a0 - hi) / h + 1.0; }
+        else { h = 0.5 * (a0 - c) * (rr - 1.0); wre = 0.0; }
+        const double wim = y0 / h;
+        const double a = 0.5 * (hypot(wre + 1.0, wim) + hypot(wre - 1.0, wim));
+        if (!(a + sqrt(fmax(a * a - 1.0, 0.0)) >= 3.5)) st = (unsigned)ST_GRAD_ILLCOND;
+    }
+    double wd = (np == 1) ? z : z * (r - 1.0) / (q - 1.0), tlo = 0.0;
+    for (int k = 0; k < np; ++k) {
+#pragma unroll
+        for (int i = 0; i < 12; ++i) {
+            const double t = fma(wd, X12[i], tlo), x = 1.0 + t;
+            const double e2 = fma(fma(fma(fma(W.a[4], x, W.a[3]), x, W.a[2]), x, W.a[1]), x, W.a[0]);
+            const double ie = 1.0 / sqrt(e2), f = (W12[i] * wd) * (ie * ie) * (ie * t);
+            const double x2 = x * x, xp1 = x + 1.0, ix = 1.0 / x;
+            const double d[4] = {f * x2, -f * xp1, f * x2 * xp1, -f * x};
+#pragma unroll
+            for (int th = 0; th < 4; ++th) { out[th] += d[th]; out[4 + th] = fma(d[th], ix, out[4 + th]); out[8 + th] = fma(d[th], x2, out[8 + th]); }
+        }
+        tlo += wd;
+        wd *= r;
+    }
+    return st;
+}
+
+// One element of the w family: values v[6] = D_C, D_M, D_L, mu, t_L, d_abs; dz[6] = d v / dz; with want_grad also
+// gp[6][6] = d v[o] / d (Om, OL, Or, Ow13, Ow23, H0).  Status as w_eval, plus 2 (unsupported) with NaN in the t_L / d_abs planes
+// where E^2 has degree <= 2 with distinct roots (eqs. (3.8)/(3.9), (B.2)/(B.3) need degree 3 or 4), plus 16.
+template <typename Vote>
+CB_HD unsigned w_eval_full(const WCosmo& W, double z, const Vote& vote, bool want_T, bool want_A, bool want_grad, double v[6], double dz[6],
+                           double gp[6][6]) {
+    double v4[4], d4[4];
+    unsigned st = w_eval<Vote>(W, z, vote, v4, d4);
+    for (int o = 0; o < 4; ++o) { v[o] = v4[o]; dz[o] = d4[o]; }
+    v[4] = v[5] = dz[4] = dz[5] = NAN;
+    const bool bad = (st & (ST_ROOT_ON_PATH | ST_UNSUPPORTED)) != 0;
+    const double x = 1.0 + z;
+    if ((want_T || want_A) && !bad) {
+        double TT, AA;
+        if (w_TA(W, x, want_T, want_A, TT, AA)) {
+            const double E = W.dH / d4[0];                 // d D_C / dz = d_H / E
+            if (want_T) { v[4] = W.tH * TT; dz[4] = W.tH / (x * E); }
+            if (want_A) { v[5] = W.dH * AA; dz[5] = W.dH * x * x / E; }
+        } else {
+            st |= ST_UNSUPPORTED;
+        }
+    }
+    if (!want_grad) return st;
+    for (int o = 0; o < 6; ++o)
+        for (int t = 0; t < 6; ++t) gp[o][t] = NAN;
+    if (bad) return st;
+    double q[12];
+    st |= w_grad_quad(W, z, q);
+    const double I0 = v[0] / W.dH;
+    double F, Fi, Fk;
+    sinn<double>(W.Ok, I0, F, Fi, Fk);
+    const int col[5] = {0, 1, 2, -1, 3};                   // Om, OL, Or, Ow13 (no E^2 dependence), Ow23 -> column of q
+    const double k5 = CB_KT.five_over_ln10;
+    for (int t = 0; t < 5; ++t) {
+        const double dI = col[t] >= 0 ? -0.5 * q[col[t]] : 0.0, dT = col[t] >= 0 ? -0.5 * q[4 + col[t]] : 0.0, dA = col[t] >= 0 ? -0.5 * q[8 + col[t]] : 0.0;
+        gp[0][t] = W.dH * dI;
+        gp[1][t] = W.dH * (Fi * dI - Fk);                  // d Ok / d theta = -1 for each of the five densities
+        gp[2][t] = x * gp[1][t];
+        gp[3][t] = (v[2] > 0.0) ? k5 * gp[2][t] / v[2] : NAN;
+        gp[4][t] = W.tH * dT;
+        gp[5][t] = W.dH * dA;
+    }
+    const double iH0 = W.dH * (1.0 / C_KM_S);
+    for (int o = 0; o < 6; ++o) gp[o][5] = -v[o] * iH0;
+    gp[3][5] = -k5 * iH0;
+    return st;
 }
 
 }  // namespace cb

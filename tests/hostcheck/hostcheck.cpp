@@ -120,3 +120,18 @@ extern "C" void hostcheck_w(int64_t n, const double* z, const double* Om, const 
         for (int o = 0; o < 4; ++o) { val[o * n + i] = v[o]; dz[o * n + i] = d[o]; }
     }
 }
+
+// the w family in full (cosmo_w.cuh, w_eval_full): val[6][n], dz[6][n], gp[6][6][n] (observable, parameter, element)
+extern "C" void hostcheck_w_full(int64_t n, const double* z, const double* Om, const double* OL, const double* Or, const double* Ow13,
+                                 const double* Ow23, const double* H0, double* val, double* dz, double* gp, uint8_t* status) {
+    for (int64_t i = 0; i < n; ++i) {
+        WCosmo W;
+        w_prep(Om[i], OL[i], Or[i], Ow13[i], Ow23[i], H0[i], W);
+        double v[6], d[6], g[6][6];
+        status[i] = (uint8_t)w_eval_full<VoteNone>(W, z[i], VoteNone(), true, true, true, v, d, g);
+        for (int o = 0; o < 6; ++o) {
+            val[o * n + i] = v[o]; dz[o * n + i] = d[o];
+            for (int t = 0; t < 6; ++t) gp[(o * 6 + t) * n + i] = g[o][t];
+        }
+    }
+}

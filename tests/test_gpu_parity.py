@@ -842,6 +842,30 @@ def test_extra_w_components(cb):
     for o, nm in enumerate(oracle.OBSW):
         assert relerr(out[o][ok], v[ok, o]).max() <= TOL_VAL, nm
         assert relerr(dz[o][ok], d[ok, o]).max() <= TOL_VAL, nm          # d/dz is closed form (the integrand), not a basis solve
+    # t_L, d_abs and the VJP (rest): all six planes, every parameter gradient, against oracle.w_observables_batch
+    which6 = ("DC", "DM", "DL", "MU", "TL", "DABS")
+    v6, g6, so6 = oracle.w_observables_batch(*[w[k] for k in names])
+    v6, g6 = v6.astype(np.float64), g6.astype(np.float64)
+    n = len(w["z"])
+    for k, nm in enumerate(which6):
+        g1 = np.zeros((6, n)); g1[k] = 1.0
+        o6, d6, s6, gz, gp = cb.cosmo_eval_w(*[dev(w[kk]) for kk in names], which=which6, grad_out=dev(g1))
+        o6, d6, s6, gz, gp = o6.cpu().numpy(), d6.cpu().numpy(), s6.cpu().numpy(), gz.cpu().numpy(), gp.cpu().numpy()
+        good = (so6 == 0) & ((s6 & 1) == 0) & np.isfinite(v6[:, k])
+        sup = good & ((s6 & 2) == 0) if k >= 4 else good & np.isfinite(o6[k])
+        if k >= 4:
+            assert sup.sum() >= good.sum() - 40 and np.isnan(o6[k][good & ~sup]).all()        # degree <= 2 with distinct roots: unsupported
+        tolv = 1e-10 if nm == "DABS" else TOL_VAL            # eq. (3.9)'s Om/Or cancellation at Om/Or up to 5e4
+        assert relerr(o6[k][sup], v6[sup, k]).max() <= tolv, nm
+        assert relerr(d6[k][sup], g6[sup, k, 0]).max() <= TOL_VAL, nm
+        assert relerr(gz[sup], g6[sup, k, 0]).max() <= TOL_VAL, nm
+        fl = (s6 & 16) != 0
+        assert fl[good].mean() < 0.05
+        m = sup & ~fl
+        for t in range(6):
+            r = g6[:, k, 1 + t]
+            e = np.abs(gp[t] - r)[m] / np.maximum(np.abs(r[m]), 1e-3 * np.abs(v6[m, k]))
+            assert e.max() <= (1e-7 if (nm == "DABS" and t == 5) else TOL_GRAD), (nm, oracle.WRTW[1 + t], e.max())
     # a subset of planes, one shared cosmology
     z = np.linspace(0.0, 6.0, 4001)
     p = (0.27, 0.55, 8e-5, 0.06, 0.09, 70.0)
@@ -856,6 +880,10 @@ def test_extra_w_components(cb):
     _, _, so2 = oracle.w_chi_batch(np.array([0.2, 5.0]), 0.1, 2.0, 0.0, 0.0, 0.05, 70.0)
     assert so2[0] == 0 and so2[1] == -1 and s2[0] == 0 and (s2[1] & 1) and np.isnan(float(o2[0, 1])) and np.isfinite(float(o2[0, 0]))
     with pytest.raises(cb.CosmoError):
-        cb.cosmo_eval_w(dev(z), *[dev(np.array([x])) for x in p], which=("TL",))
+        cb.cosmo_eval_w(dev(z), *[dev(np.array([x])) for x in p], which=("AGE",))
+    ot, _, stt = cb.cosmo_eval_w(dev(z[1:]), *[dev(np.array([x])) for x in p], which=("TL", "DABS"))
+    vt, _, _ = oracle.w_observables_batch(z[1:], *p, with_grad=False)
+    assert (stt.cpu().numpy() == 0).all() and relerr(ot[0].cpu().numpy(), vt[:, 4].astype(np.float64)).max() <= TOL_VAL
+    assert relerr(ot[1].cpu().numpy(), vt[:, 5].astype(np.float64)).max() <= 1e-10
     e, _, _ = cb.cosmo_eval_w(dev(np.zeros(0)), *[dev(np.array([x])) for x in p])
     assert e.shape == (1, 0)

@@ -268,6 +268,41 @@ def test_extra_w_components_host(hc):
     assert np.isnan(val[:, so == -1]).all()
 
 
+def test_extra_w_components_full_host(hc):
+    """t_L, d_abs and every parameter gradient on the general quartic (cosmo_w.cuh: eqs. (3.8)/(3.9) with complex roots and complex
+    Carlson functions; gradient integrals by quadrature) against oracle.w_observables_batch"""
+    w = W.wmix(n=3000)
+    n = len(w["z"])
+    names = ("z", "Om", "OL", "Or", "Ow13", "Ow23", "H0")
+    val = np.zeros((6, n)); dz = np.zeros((6, n)); gp = np.zeros((6, 6, n)); st = np.zeros(n, dtype=np.uint8)
+    dp = lambda a: np.ascontiguousarray(a).ctypes.data_as(DP)
+    hc.hostcheck_w_full(C.c_int64(n), *[dp(w[k]) for k in names], dp(val), dp(dz), dp(gp), st.ctypes.data_as(C.POINTER(C.c_uint8)))
+    v, g, so = oracle.w_observables_batch(*[w[k] for k in names])
+    v, g = v.astype(np.float64), g.astype(np.float64)
+    ok = (so == 0) & ((st & 1) == 0)
+    assert ok.mean() > 0.95 and (st[so == -1] & 3).all()
+    chi_ok = ok & np.isfinite(val[0])
+    for o in range(4):
+        assert (np.abs(val[o][chi_ok] - v[chi_ok, o]) / np.abs(v[chi_ok, o])).max() <= 1e-11, oracle.OBS[o]
+    # t_L, d_abs: every element of degree 3 or 4 and the monomials; the few of degree <= 2 with distinct roots are marked unsupported
+    sup = ok & ((st & 2) == 0)
+    assert sup.sum() >= ok.sum() - 8 and np.isnan(val[4][ok & ~sup]).all()
+    for o, tol in ((4, 1e-11), (5, 1e-10)):      # d_abs: the Om/Or cancellation of eq. (3.9) (PAPER.md:249), up to Om/Or = 5e4 here
+        e = np.abs(val[o][sup] - v[sup, o]) / np.abs(v[sup, o])
+        assert e.max() <= tol, (oracle.OBS[o], e.max())
+        ez = np.abs(dz[o][sup] - g[sup, o, 0]) / np.abs(g[sup, o, 0])
+        assert ez.max() <= 1e-11, (oracle.OBS[o], ez.max())
+    # parameter gradients (Om, OL, Or, Ow13, Ow23, H0) of all six observables; elements the quadrature cannot serve are flagged
+    fl = (st & 16) != 0
+    assert fl[ok].mean() < 0.05
+    for o in range(6):
+        m = (sup if o >= 4 else chi_ok) & ~fl & np.isfinite(v[:, o])
+        for t in range(6):
+            r = g[:, o, 1 + t]
+            e = np.abs(gp[o, t] - r)[m] / np.maximum(np.abs(r[m]), 1e-3 * np.abs(v[m, o]))
+            assert e.max() <= (1e-7 if (o == 5 and t == 5) else 1e-8), (oracle.OBS[o], oracle.WRTW[1 + t], e.max())
+
+
 def test_host_math_fp32(hc):
     w = W.config3(n=3000, S=1)
     z = w.z.astype(np.float32).astype(np.float64)
