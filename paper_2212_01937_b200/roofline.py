@@ -8,28 +8,46 @@ DESIGN.md "Roofline" the derivation).  `peak` = the DFMA rate bench.py measures 
 probe (cosmo_probe_fma_f64); the nominal figure beside it is 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz.
 """
 
-# FP64 work per eval of the config-3 fused forward+VJP kernel k_outer<double,false,false,VJP,MU> as committed, from the
-# ncu captures profiles/r01b_k_outer_vjp.md and (re-captured for the committed build, same counts) profiles/r01c_k_outer_vjp.md
-# (6.4e7 evals/launch):
-#   DFMA 137.4, DMUL 98.7, DADD 24.5 thread-instructions per eval -> 2*137.4 + 98.7 + 24.5 = 397.9 flops
-#   FP64-pipe instructions per eval (the above + 5.3 DSETP) = 265.9
-# (earlier builds: profiles/r01_final_k_outer_vjp.md 430.6 flops / 300.1 pipe instructions; first working version,
-#  profiles/r01_k_outer_vjp.md: 774.8 / 513.7.  Fewer flops for the same result is the point: compare evals/s across
-#  builds, and the roofline fraction within one.)
+# Arithmetic work per eval of the dominant kernel of each bench.py arm, from Nsight Compute SASS counters of the committed build
+# (profiles/r02_k_outer_vjp.md, profiles/r02_other_kernels.md + .csv).  flops = 2 x FMA + MUL + ADD of the arithmetic type; "pipe"
+# = instructions that occupy that type's pipe.  Fewer flops for the same result is the point of most optimisations here: compare evals/s
+# across builds, and the roofline fraction within one.  (Round 1: config 3 397.9 flops / 265.9 pipe instructions.)
+#   config3_vjp_mu_f64  k_outer<double,0,0,VJP,MU>, 6.4e7 evals/launch: DFMA 135.05, DMUL 98.23, DADD 24.48 per eval
+#   config3_vjp_mu_f32  k_outer<float,0,0,VJP,MU>:  FFMA 78.47, FMUL 80.14, FADD 14.63 per eval (204.4 FP32 instructions in all)
+#   config4_snia_f64    k_outer<double,0,0,SNIA,MU>, 2.56e8 evals/launch: DFMA 150.60, DMUL 105.15, DADD 34.66 per eval
+#   config5_vjp_all_f64 k_elem<double,1,1,1> (+ k_elem_redo on 2.5 % of the elements), 1.03e7 evals: DFMA 1199.9, DMUL 740.8, DADD 213.1 per eval
+#   config5_vjp_all_f32 k_elem<float,1,1,1>: FFMA 578.0, FMUL 412.2, FADD 195.9 per eval (FP32 flops only are counted), plus 376 FP64
+#                       instructions per eval (the per-element root solve, which stays FP64)
 FLOPS_PER_EVAL = {
-    "config3_vjp_mu_f64": 397.9,
+    "config3_vjp_mu_f64": 392.8,
+    "config3_vjp_mu_f32": 251.7,
+    "config4_snia_f64": 441.0,
+    "config5_vjp_all_f64": 3353.7,
+    "config5_vjp_all_f32": 1764.1,
 }
-# instructions per eval on the arithmetic pipe of the dtype (FP64: DFMA + DMUL + DADD + DSETP)
+# instructions per eval on the arithmetic pipe of the dtype
 PIPE_INST_PER_EVAL = {
-    "config3_vjp_mu_f64": 265.9,
+    "config3_vjp_mu_f64": 264.0,
+    "config3_vjp_mu_f32": 204.4,
+    "config4_snia_f64": 297.4,
+    "config5_vjp_all_f64": 2232.0,
+    "config5_vjp_all_f32": 1406.0,
 }
-# dram__bytes_read.sum + dram__bytes_write.sum of that kernel, per launch (same capture)
+# dram__bytes_read.sum + dram__bytes_write.sum of that kernel, per launch (same captures)
 DRAM_TRAFFIC_BYTES_PER_LAUNCH = {
-    "config3_vjp_mu_f64": 544.13e6 + 635.70e6,
+    "config3_vjp_mu_f64": 544.23e6 + 639.98e6,
+    "config3_vjp_mu_f32": 272e6 + 305e6,
+    "config4_snia_f64": 24e6,
+    "config5_vjp_all_f64": 908e6 + 1564e6,
+    "config5_vjp_all_f32": 618e6 + 593e6,
 }
 # where each entry comes from
 SOURCE = {
-    "config3_vjp_mu_f64": "profiles/r01c_k_outer_vjp.md",
+    "config3_vjp_mu_f64": "profiles/r02_k_outer_vjp.md",
+    "config3_vjp_mu_f32": "profiles/r02_other_kernels.csv",
+    "config4_snia_f64": "profiles/r02_other_kernels.csv",
+    "config5_vjp_all_f64": "profiles/r02_other_kernels.csv",
+    "config5_vjp_all_f32": "profiles/r02_other_kernels.csv",
 }
 
 # nominal B200 vector peaks (context only; the denominator is the measured probe): 148 SMs x lanes x 2 x 1.965 GHz
