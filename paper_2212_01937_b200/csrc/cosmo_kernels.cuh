@@ -373,19 +373,23 @@ __global__ void k_reduce_gz(const T* __restrict__ part, int ny, int64_t N, T* __
 
 // ELEMENTWISE with one cosmology per redshift: S1-S8 per thread (cosmo_obs.cuh, elem_one), no reductions.
 // Register budget: left alone the all-outputs variants take 255 registers (8 warps/SM) and wait on latency at a third of the
-// FP64 pipe; capped at 128 (VJP) / 80 (forward) registers they run 16 / 24 warps per SM (profiles/).
+// FP64 pipe; capped at 128 (VJP) / 80 (forward) registers they run 16 / 24 warps per SM (profiles/).  Blocks of 256 threads measured 7-10 %
+// faster than 128 at the same occupancy (2.79 vs 3.09 ms on config 5); block-wide barriers between the phases of an element did not help.
 // Two passes.  k_elem is the fast path for every element; the few that need a slow path -- E^2 without a real negative root
 // (complex arithmetic, cosmo_c4.cuh), gradient bases too ill-conditioned (quadrature, cosmo_obs.cuh) -- are only listed
 // (redo_count, redo_list in the workspace) and k_elem_redo runs them again, densely packed, with the slow paths compiled in.
 // A never-inlined call inside the main kernel costs it 15-30 % even where it is not taken (profiles/).
+#ifndef CB_ELEM_BLOCK
+#define CB_ELEM_BLOCK 256
+#endif
 #ifndef CB_ELEM_MINB_G
-#define CB_ELEM_MINB_G 4
+#define CB_ELEM_MINB_G 2
 #endif
 #ifndef CB_ELEM_MINB_F
-#define CB_ELEM_MINB_F 6
+#define CB_ELEM_MINB_F 3
 #endif
-template <typename T, bool kT, bool kA, bool kG>
-__global__ void __launch_bounds__(ELEM_THREADS, kG ? CB_ELEM_MINB_G : CB_ELEM_MINB_F) k_elem(ElemArgs a) {
+template <typename T, bool kT, bool kA, bool kG, bool kAge>
+__global__ void __launch_bounds__(CB_ELEM_BLOCK, kG ? CB_ELEM_MINB_G : CB_ELEM_MINB_F) k_elem(ElemArgs a) {
     const int64_t N = a.N;
     const unsigned which = a.which;
     const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
@@ -403,7 +407,7 @@ __global__ void __launch_bounds__(ELEM_THREADS, kG ? CB_ELEM_MINB_G : CB_ELEM_MI
         }
     }
     T dz = T(0), gp[4] = {T(0), T(0), T(0), T(0)};
-    const unsigned st = elem_one<T, kT, kA, kG, VoteWarp, true>(static_cast<const T*>(a.z)[ii], a.Om[ii], a.OL[ii], a.Or[ii], a.H0[ii], which,
+    const unsigned st = elem_one<T, kT, kA, kG, VoteWarp, true, kAge>(static_cast<const T*>(a.z)[ii], a.Om[ii], a.OL[ii], a.Or[ii], a.H0[ii], which,
                                                                 VoteWarp(), g, v, dz, gp);
     if (live && a.out != nullptr) {
         T* __restrict__ out = static_cast<T*>(a.out);

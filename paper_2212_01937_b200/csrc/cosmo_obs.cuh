@@ -599,14 +599,15 @@ CB_HD unsigned backward_robust(const Cosmo<T>& C, T z, const Core<T>& R, const O
 // the factorisation crosses the loop (registers decide how many warps fit).
 // kDefer: the main pass of the ELEMENTWISE kernels -- elements that need a slow path (complex root structure, ill-conditioned
 // gradient bases: backward_robust) are only marked ST_INTERNAL_REDO; the second pass runs them again without kDefer.
-template <typename T, bool kT, bool kA, bool kG, typename Vote, bool kDefer = false>
+// kAge: the age plane may be asked for (its T_inf costs a second pass of eq. (3.8) per element: kept out of the other instantiations)
+template <typename T, bool kT, bool kA, bool kG, typename Vote, bool kDefer = false, bool kAge = true>
 CB_HD unsigned elem_one(T zv, double Om, double OL, double Or, double H0, unsigned which, const Vote& vote, const T* g, T* v, T& dz, T gp[4]) {
     Cosmo<T> C0{}, C{};
     {
         Cosmo<double> Cd{};
         cosmo_factor(Om, OL, Or, H0, Cd);
         cosmo_constants(Cd);
-        if (kT && (which & W_AGE)) prep_age(Cd, kG);
+        if (kT && kAge && (which & W_AGE)) prep_age(Cd, kG);
         convert_cosmo<T>(Cd, C0);
     }
     Core<T> R;
@@ -640,7 +641,7 @@ CB_HD unsigned elem_one(T zv, double Om, double OL, double Or, double H0, unsign
                 double gd[N_PLANES], vd[N_PLANES], dzd = 0.0, gpd[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
                 for (int w = 0; w < N_PLANES; ++w) gd[w] = (double)g[w];
-                st = elem_one<double, kT, kA, kG, VoteNone, false>((double)zv, Om, OL, Or, H0, which, VoteNone(), gd, vd, dzd, gpd);
+                st = elem_one<double, kT, kA, kG, VoteNone, false, kAge>((double)zv, Om, OL, Or, H0, which, VoteNone(), gd, vd, dzd, gpd);
 #pragma unroll
                 for (int w = 0; w < N_PLANES; ++w) v[w] = (T)vd[w];
                 dz = (T)dzd;

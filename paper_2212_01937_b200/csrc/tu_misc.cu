@@ -28,6 +28,9 @@ __global__ void k_prep(const double* __restrict__ Om, const double* __restrict__
 // Two-limit evaluation (cosmo_two.cuh), one thread per (z1, z2, cosmology); n_cosmo in {1, n}.  which: DC, DM, TL, DABS, DA.
 // (128-register cap as for k_elem.)  kG: with the VJP; its slow paths go to the second pass k_two<.., kRedo> through a work list, as in
 // k_elem; the forward kernel keeps the complex path inline.
+#ifndef CB_TWO_BLOCK
+#define CB_TWO_BLOCK 256      // as k_elem: 256-thread blocks measured a few per cent faster than 128 at the same occupancy
+#endif
 #ifndef CB_TWO_DEFER_MIN
 #define CB_TWO_DEFER_MIN 3000000
 #endif
@@ -71,7 +74,7 @@ __device__ __forceinline__ unsigned two_one(const TwoArgs& a, int64_t i, bool li
 }
 
 template <bool kG, bool kDefer>
-__global__ void __launch_bounds__(ELEM_THREADS, 4) k_two(TwoArgs a) {
+__global__ void __launch_bounds__(CB_TWO_BLOCK, kG ? 2 : 3) k_two(TwoArgs a) {
     const int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     const bool live = i < a.n;
     const unsigned st = two_one<kG, kDefer, false>(a, i, live);
@@ -192,13 +195,13 @@ void launch_two(const double* z1, const double* z2, const double* Om, const doub
                 int64_t n_cosmo, unsigned which, const double* gout, double* out, double* gz1, double* gz2, double* gparams,
                 uint8_t* status, unsigned* ws, cudaStream_t st) {
     TwoArgs a{z1, z2, Om, OL, Or, H0, n, n_cosmo, which, gout, out, gz1, gz2, gparams, status, ws, ws ? ws + 64 : nullptr};
-    const unsigned grid = (unsigned)cdiv64(n, ELEM_THREADS);
-    if (gout == nullptr) { k_two<false, false><<<grid, ELEM_THREADS, 0, st>>>(a); return; }
+    const unsigned grid = (unsigned)cdiv64(n, CB_TWO_BLOCK);
+    if (gout == nullptr) { k_two<false, false><<<grid, CB_TWO_BLOCK, 0, st>>>(a); return; }
     // The second pass costs the latency of one slow element (tens of microseconds) whatever the batch size, the inline slow paths
     // ~10 % of the main kernel: two passes from a few million elements on (measured, profiles/)
-    if (n < TWO_DEFER_MIN) { k_two<true, false><<<grid, ELEM_THREADS, 0, st>>>(a); return; }
+    if (n < TWO_DEFER_MIN) { k_two<true, false><<<grid, CB_TWO_BLOCK, 0, st>>>(a); return; }
     cudaMemsetAsync(a.redo_count, 0, sizeof(unsigned), st);
-    k_two<true, true><<<grid, ELEM_THREADS, 0, st>>>(a);
+    k_two<true, true><<<grid, CB_TWO_BLOCK, 0, st>>>(a);
     k_two_redo<<<148 * 4, ELEM_THREADS, 0, st>>>(a);
 }
 size_t w_cosmo_bytes() { return sizeof(WCosmo); }
