@@ -59,7 +59,8 @@ enum {
     COSMO_E_WHICH = -3,     /* which == 0 or has unknown bits                    */
     COSMO_E_MODE = -4,      /* unknown mode                                      */
     COSMO_E_WORKSPACE = -5, /* ws_bytes < cosmo_workspace_bytes(...)             */
-    COSMO_E_CUDA = -6       /* kernel launch failed                              */
+    COSMO_E_CUDA = -6,      /* kernel launch failed                              */
+    COSMO_E_STATIC_LIMIT = -7 /* problem too large for the fixed static scratch of cosmo_snia_loglike_static */
 };
 
 /* SoA cosmological parameters, each of length n_cosmo.  Always FP64, also for the _f32 entry points
@@ -89,6 +90,21 @@ int cosmo_vjp(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int
  * Elements with status != 0 contribute NaN. */
 int cosmo_snia_loglike(const double* z, const double* mu_obs, const double* sigma, int64_t N, cosmo_params p, int64_t S,
                        double* logL, double* grad, void* workspace, size_t ws_bytes, void* stream);
+
+/* The same likelihood WITHOUT a workspace and without any allocation, for callers that cannot call cudaMalloc (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it): the scratch is a static device array of COSMO_STATIC_SCRATCH_BYTES (24 MiB)
+ * that every GPU loading the library holds until the process exits.  Same kernels and results as cosmo_snia_loglike (FP64).
+ *   Limit: align256(928 S) + align256(40 S ceil(N / 512)) <= COSMO_STATIC_SCRATCH_BYTES, e.g. S = 256 samples x N <= 1.04e6 supernovae
+ *   (BASELINE.json config 4 fits) or S = 64 x N <= 4.2e6; beyond it the call returns COSMO_E_STATIC_LIMIT and launches nothing.
+ *   The call runs no cudaMalloc / cudaFree / allocating routine; its first use on a device asks the runtime for the array's address
+ *   (cudaGetSymbolAddress, with the CURRENT device: `stream` must belong to it).
+ *   All calls on a GPU share the array and it keeps the last call's contents (every call overwrites what it reads, nothing has to be
+ *   cleared): calls that may overlap on the device -- different streams without ordering between them, different host threads -- race.
+ *   Serialise them, or use cosmo_snia_loglike with one workspace per stream. */
+#define COSMO_STATIC_SCRATCH_BYTES (24u << 20)
+int cosmo_snia_loglike_static(const double* z, const double* mu_obs, const double* sigma, int64_t N, cosmo_params p, int64_t S,
+                              double* logL, double* grad, void* stream);
+size_t cosmo_static_scratch_bytes(void);
 
 /* Log-joint of the paper's section-4 toy model with LATENT redshifts (one step of its variational fit evaluates this
  * and its gradient for S posterior samples): for sample s with redshifts z[s][0..N) and cosmology theta_s

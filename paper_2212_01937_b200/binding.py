@@ -18,7 +18,7 @@ WHICH_BITS = {"DC": DC, "DM": DM, "DL": DL, "MU": MU, "TL": TL, "DABS": DABS, "D
 WHICH_ORDER = ("DC", "DM", "DL", "MU", "TL", "DABS", "DA", "VC", "AGE")
 
 # every symbol include/cosmo_b200.h and include/cosmo_b200_diag.h declare
-SYMBOLS = ("cosmo_host_release", "cosmo_eval2_workspace_bytes", "cosmo_eval_w_workspace_bytes", "cosmo_workspace_bytes", "cosmo_eval", "cosmo_vjp", "cosmo_snia_loglike", "cosmo_eval_f32", "cosmo_vjp_f32",
+SYMBOLS = ("cosmo_host_release", "cosmo_snia_loglike_static", "cosmo_static_scratch_bytes", "cosmo_eval2_workspace_bytes", "cosmo_eval_w_workspace_bytes", "cosmo_workspace_bytes", "cosmo_eval", "cosmo_vjp", "cosmo_snia_loglike", "cosmo_eval_f32", "cosmo_vjp_f32",
            "cosmo_snia_loglike_f32", "cosmo_snia_logjoint", "cosmo_eval2", "cosmo_eval_w", "cosmo_eval_host", "cosmo_carlson_pair", "cosmo_probe_fma_f64", "cosmo_probe_fma_f32",
            "cosmo_profile", "cosmo_profile_mean_ms",
            "cosmo_launch_count", "cosmo_last_cuda_error", "cosmo_strerror", "cosmo_version")
@@ -59,6 +59,9 @@ def lib():
         f = getattr(L, name)
         f.argtypes = [vp, vp, vp, i64, CosmoParams, i64, vp, vp, vp, sz, vp]
         f.restype = ci
+    L.cosmo_snia_loglike_static.argtypes = [vp, vp, vp, i64, CosmoParams, i64, vp, vp, vp]
+    L.cosmo_snia_loglike_static.restype = ci
+    L.cosmo_static_scratch_bytes.restype = sz
     L.cosmo_eval_host.argtypes = [vp, i64, CosmoParams, i64, ci, u32, vp, vp, vp, vp, vp]
     L.cosmo_eval_host.restype = ci
     for name in ("cosmo_probe_fma_f64", "cosmo_probe_fma_f32"):
@@ -224,6 +227,28 @@ def cosmo_snia_loglike(z, mu_obs, sigma, Om, OL, Or, H0, want_grad=True, logL=No
     fn = lib().cosmo_snia_loglike_f32 if f32 else lib().cosmo_snia_loglike
     _check(fn(_ptr(z), _ptr(mu_obs), _ptr(sigma), N, P, S, _ptr(logL), _ptr(grad), _ptr(ws), ws.numel(), _stream(torch)))
     return logL, grad
+
+
+def cosmo_snia_loglike_static(z, mu_obs, sigma, Om, OL, Or, H0, want_grad=True, logL=None, grad=None):
+    """cosmo_snia_loglike without workspace or allocation inside the library (static device scratch of 24 MiB, shared by all calls on the
+    GPU: do not overlap calls).  FP64.  Pass logL / grad to keep this wrapper from allocating the outputs.  Raises CosmoError (-7) when
+    (N, S) exceeds the static scratch.  Returns (logL[S], grad[4, S] or None)."""
+    torch = _torch()
+    for t, nm in ((z, "z"), (mu_obs, "mu_obs"), (sigma, "sigma")):
+        _dev(t, torch.float64, torch, nm)
+    P, S, keep = _params(Om, OL, Or, H0, torch)
+    N = z.numel()
+    if logL is None:
+        logL = torch.empty(S, dtype=torch.float64, device=z.device)
+    if want_grad and grad is None:
+        grad = torch.empty((4, S), dtype=torch.float64, device=z.device)
+    with torch.cuda.device(z.device):          # the static array's address is taken for the CURRENT device
+        _check(lib().cosmo_snia_loglike_static(_ptr(z), _ptr(mu_obs), _ptr(sigma), N, P, S, _ptr(logL), _ptr(grad), _stream(torch)))
+    return logL, grad
+
+
+def static_scratch_bytes() -> int:
+    return int(lib().cosmo_static_scratch_bytes())
 
 
 def cosmo_snia_logjoint(z, z_obs, mu_obs, sigma_mu, sigma_z, beta, shape, Om, OL, Or, H0, want_grad=True, workspace=None):

@@ -512,6 +512,7 @@ const char* cosmo_strerror(int code) {
         case COSMO_E_MODE: return "unknown mode";
         case COSMO_E_WORKSPACE: return "workspace too small (see cosmo_workspace_bytes)";
         case COSMO_E_CUDA: return "CUDA launch or runtime error (see cosmo_last_cuda_error)";
+        case COSMO_E_STATIC_LIMIT: return "problem too large for the fixed static scratch (COSMO_STATIC_SCRATCH_BYTES): use the workspace call";
         default: return "unknown error code";
     }
 }
