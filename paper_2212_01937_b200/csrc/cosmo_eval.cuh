@@ -175,13 +175,13 @@ CB_HD T rc1(T e) {
         for (int j = 8; j >= 0; --j) s = N::fma_(s, -e, T(CB_KT.rc[j]));
         return N::fma_(s, -e, T(1));
     }
-    if (e > T(0)) { T r = N::sqrt_(e); return N::atan_(r) / r; }
-    T r = N::sqrt_(-e);
-    return T(0.5) * N::log_((T(1) + r) / (T(1) - r)) / r;
+    if (e > T(0)) { const T ir = N::rsqrt_(e); return N::atan_(e * ir) * ir; }
+    const T ir = N::rsqrt_(-e), r = -e * ir;
+    return T(0.5) * N::log_((T(1) + r) * N::rcp_(T(1) - r)) * ir;
 }
 // R_C(x, y) for x >= 0, y > 0
 template <typename T>
-CB_HD T rc(T x, T y) { return rc1<T>(y / x - T(1)) / Num<T>::sqrt_(x); }
+CB_HD T rc(T x, T y) { const T ir = Num<T>::rsqrt_(x); return rc1<T>((y - x) * (ir * ir)) * ir; }
 
 // Carlson's degree-7 series in the elementary symmetric functions (R_D / R_J form, ref. [10] as in DLMF 19.36.2)
 template <typename T>
@@ -461,26 +461,28 @@ CB_HD void eval_core_k(const Cosmo<T>& C0, const T (&z)[K], const Vote& vote, Co
         if (kT) {
             // eq. (3.8) with i = big root, j = rn, scaled so that Or -> 0 reproduces (B.2)
             const T RJ5 = carlson_rj_series<T>(xa[k], mp[k], p5[k], g2, xa0, m0, s0, p5_0[k], sum5[k]);
-            const T qh = x * p5_0[k] * C.qhc / lin;
+            const T rlin = N::rcp_(lin);
+            const T qh = x * p5_0[k] * C.qhc * rlin;
             const T sh = N::fma_(z2, C.OL, qh);
             R[k].TT = T(2) * z[k] * (z2 * T(CB_KT.third) * C.Gp * RJ5 + rc<T>(sh, qh) - C.OrM * RF);
         }
         if (kA) {
-            const T bnd = N::sqrt_(xmr * (T(1) - C.rn)) * rU;
+            const T bnd = N::sqrtp_(xmr * (T(1) - C.rn)) * rU;
             if (quartA) {
                 // eq. (3.9) with (i,j,k,l) = (rn, pair, pair, big)
                 const T RJ0 = carlson_rj_series<T>(xa[k], mp[k], p0[k], g2, xa0, m0, s0, p0_0[k], sum0[k]);
-                const T q0 = p0_0[k] / ((T(1) - C.rn) * xmr);
+                const T q0 = p0_0[k] * N::rcp_((T(1) - C.rn) * xmr);
                 const T s0q = N::fma_(C.Or, z2, q0);
                 // third-kind bracket of (3.9): 2 z B0 = int (x - rn) dx / E
                 const T B0 = N::fma_(z2 * T(CB_KT.third) * C.Q2n * C.mOrn, RJ0, rc<T>(s0q, q0));
                 // boundary term [sqrt((x-rn) Q2 / (Or x + m))] between 1 and x, with the factor z taken out analytically
-                const T Fx = N::sqrt_(xmr * q2x / lin);
+                const T rl = N::rcp_(lin);
+                const T Fx = N::sqrtp_(xmr * q2x * rl);
                 const T c2 = C.b - C.rn, c1 = N::fma_(-C.rn, C.b, C.c);
                 const T dC = N::fma_(x, x + T(1), T(1)) + N::fma_(c2, x + T(1), c1);          // (C(x) - C(1)) / z
-                const T t1 = z[k] * (N::fma_(C.Or + C.m, dC, -C.C1 * C.Or)) / (lin * (C.Or + C.m) * (Fx + C.F1));
+                const T t1 = z[k] * (N::fma_(C.Or + C.m, dC, -C.C1 * C.Or)) * rl * N::rcp_((C.Or + C.m) * (Fx + C.F1));
                 const T t2 = z[k] * C.aF * RF;
-                const T t3 = z[k] * C.WoOr * N::fma_(z2 * T(CB_KT.third) * C.Q2n, RD, bnd / N::sqrt_(lin * (C.Or + C.m)));
+                const T t3 = z[k] * C.WoOr * N::fma_(z2 * T(CB_KT.third) * C.Q2n, RD, bnd * N::rsqrt_(lin * (C.Or + C.m)));
                 const T t4 = z[k] * C.sig * B0;
                 const T A39 = (t1 + t2) + (t3 + t4);
                 // The R_D and R_J groups of (3.9) cancel by ~Om/(Or x).  Where radiation is a perturbation
@@ -513,7 +515,7 @@ CB_HD void eval_core_k(const Cosmo<T>& C0, const T (&z)[K], const Vote& vote, Co
                 R[k].AA = conv ? u[2] : A39;
             } else {
                 // eq. (B.3) with i = rn
-                R[k].AA = T(CB_KT.two_thirds) * z[k] * (R[k].Em1 / (C.m * z[k]) + C.aF * RF
+                R[k].AA = T(CB_KT.two_thirds) * z[k] * (R[k].Em1 * N::rcp_(C.m * z[k]) + C.aF * RF
                                                + T(2) * C.sig * N::fma_(z2 * T(CB_KT.third) * C.Q2n * C.m, RD, bnd));
                 if (z[k] == T(0)) R[k].AA = T(0);
             }
