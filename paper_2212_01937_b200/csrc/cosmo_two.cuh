@@ -40,7 +40,7 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
         const double L1 = fma(C.Or, x1, C.m), L2 = fma(C.Or, x2, C.m), xm1 = x1 - C.rn, xm2 = x2 - C.rn;
         const double q21 = fma(x1 + C.b, x1, C.c), q22 = fma(x2 + C.b, x2, C.c);
         const double a1 = L2 * xm2 * q21, a2 = L1 * xm1 * q22;
-        const double ra = sqrt(a1), rb = sqrt(a2), U12 = ra + rb;
+        const double ra = cb_sqrt0(a1), rb = cb_sqrt0(a2), U12 = ra + rb;
         double xa[1] = {U12 * U12}, mp[1], s[1], p5[1], p0[1];
         const double hd = 0.5 * dz2 * C.theta, hs = dz2 * C.sDr;
         mp[0] = xa[0] - hd;
@@ -60,24 +60,25 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
         const double RJ5 = carlson_rj_series<double>(xa[0], mp[0], p5[0], f, xa0, m0, s0, p5_0, sum5[0]);
         const double RJ0 = carlson_rj_series<double>(xa[0], mp[0], p0[0], f, xa0, m0, s0, p0_0, sum0[0]);
         // E at both limits; E2 - E1 without cancellation
-        E1 = sqrt(L1 * xm1 * q21); E2 = ra * rb / E1;
+        E1 = cb_sqrt0(L1 * xm1 * q21); E2 = ra * rb * cb_rcp(E1);
         const double s12 = x1 + x2, p12 = x1 * x2, sq = fma(x2, x2, x1 * x1);          // x1+x2, x1 x2, x1^2+x2^2
-        dE = dz * (C.Or * s12 * sq + C.Om * (sq + p12) + C.Ok * s12) / (E1 + E2);
+        dE = dz * (C.Or * s12 * sq + C.Om * (sq + p12) + C.Ok * s12) * cb_rcp(E1 + E2);
+        const double rx12 = cb_rcp(xm1 * xm2), rL12 = cb_rcp(L1 * L2), rU = cb_rcp(U12);
         // ---- S6 reductions
         I0 = 2.0 * dz * RF;                                                // eq. (3.7)
-        K = 2.0 * dz * fma(dz2 * CB_KT.third * C.W, RD, sqrt(L1 * L2 / (xm1 * xm2)) / U12);
-        const double qh = p12 * p5_0 * C.m * C.m / (L1 * L2);
+        K = 2.0 * dz * fma(dz2 * CB_KT.third * C.W, RD, cb_sqrt0(L1 * L2 * rx12) * rU);
+        const double qh = p12 * p5_0 * C.m * C.m * rL12;
         TT = 2.0 * dz * (dz2 * CB_KT.third * C.Gp * RJ5 + rc<double>(fma(dz2, C.OL, qh), qh) - C.OrM * RF);   // eq. (3.8)
-        const double bnd = sqrt(xm1 * xm2) / U12;
+        const double bnd = cb_sqrt0(xm1 * xm2) * rU;
         if (quartA) {                                                                   // eq. (3.9), (i,j,k,l) = (rn, pair, pair, big)
-            const double q0 = p0_0 / (xm1 * xm2);
+            const double q0 = p0_0 * rx12;
             const double B0 = fma(dz2 * CB_KT.third * C.Q2n * C.mOrn, RJ0, rc<double>(fma(C.Or, dz2, q0), q0));
-            const double F1 = sqrt(xm1 * q21 / L1), F2 = sqrt(xm2 * q22 / L2);
+            const double F1 = cb_sqrt0(xm1 * q21 * L2 * rL12), F2 = cb_sqrt0(xm2 * q22 * L1 * rL12);
             const double c2 = C.b - C.rn, c1 = fma(-C.rn, C.b, C.c);
             const double dC = (sq + p12) + fma(c2, s12, c1);                            // (C(x2) - C(x1)) / dz, C = (x - rn) Q2
-            const double t1 = dz * fma(L1, dC, -xm1 * q21 * C.Or) / (L1 * L2 * (F1 + F2));
+            const double t1 = dz * fma(L1, dC, -xm1 * q21 * C.Or) * rL12 * cb_rcp(F1 + F2);
             const double t2 = dz * C.aF * RF;
-            const double t3 = dz * C.WoOr * fma(dz2 * CB_KT.third * C.Q2n, RD, bnd / sqrt(L1 * L2));
+            const double t3 = dz * C.WoOr * fma(dz2 * CB_KT.third * C.Q2n, RD, bnd * cb_sqrt0(rL12));
             const double t4 = dz * C.sig * B0;
             const double A39 = (t1 + t2) + (t3 + t4);
             // radiation-perturbative assembly (see eval_core_k): u_j = int x^j dx/E between the limits
@@ -89,31 +90,34 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
             for (int j = 0; j <= KS; ++j) { bk[j] = fma(dk, E2, xk1 * dE); dk = fma(x2, dk, xk1 * dz); xk1 *= x1; }    // x2^j E2 - x1^j E1
             for (int j = 2; j < KS + 4; ++j) u[j] = 0.0;
             double prev = 0.0;
+#pragma unroll
             for (int sw = 0; sw < KS; ++sw) {
                 if (sw == KS - 1) prev = u[2];
+#pragma unroll
                 for (int j = 0; j <= KS - sw; ++j) {
                     double acc = bk[j] - (j + 2) * C.Or * u[j + 3] - (j + 1) * C.Ok * u[j + 1];
                     if (j >= 1) acc -= j * C.OL * u[j - 1];
-                    u[j + 2] = acc * C.iOm / (j + 1.5);
+                    u[j + 2] = acc * C.iOm * (1.0 / (j + 1.5));
                 }
             }
             AA = (fabs(u[2] - prev) <= 1e-14 * fabs(u[2])) ? u[2] : A39;
         } else {                                                                        // eq. (B.3), i = rn
-            AA = CB_KT.two_thirds * dz * (dE / (C.m * dz) + C.aF * RF + 2.0 * C.sig * fma(dz2 * CB_KT.third * C.Q2n * C.m, RD, bnd));
+            AA = CB_KT.two_thirds * dz * (dE * cb_rcp(C.m * dz) + C.aF * RF + 2.0 * C.sig * fma(dz2 * CB_KT.third * C.Q2n * C.m, RD, bnd));
             if (dz == 0.0) AA = 0.0;
         }
     }
     // ---- S7
     double F, Fi, Fk;
     sinn<double>(C.Ok, I0, F, Fi, Fk);
-    O.v[0] = C.dH * I0; O.v[1] = C.dH * F; O.v[2] = C.tH * TT; O.v[3] = C.dH * AA; O.v[4] = O.v[1] / x2;
+    const double ix1 = cb_rcp(x1), ix2 = cb_rcp(x2);
+    O.v[0] = C.dH * I0; O.v[1] = C.dH * F; O.v[2] = C.tH * TT; O.v[3] = C.dH * AA; O.v[4] = O.v[1] * ix2;
     O.status = st[0];
     if (st[0] & (ST_ROOT_ON_PATH | ST_UNSUPPORTED)) {
         for (int i = 0; i < 5; ++i) O.v[i] = NAN;
     }
     if (!with_grad) return;
     // ---- S8: the same bases (GI, GT, GA/GJ) on two-limit basis values; b_k = x2^k/E2 - x1^k/E1
-    const double iE1 = 1.0 / E1, iE2 = 1.0 / E2, diE = -dE * iE1 * iE2;            // 1/E2 - 1/E1
+    const double iE1 = cb_rcp(E1), iE2 = cb_rcp(E2), diE = -dE * iE1 * iE2;            // 1/E2 - 1/E1
     double btv[16];
     {
         double xk1 = 1.0, dk = 0.0;
@@ -141,12 +145,14 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
         }
         for (int p = 5; p < 17; ++p) Jp[p] = 0.0;
         double prev5 = 0.0, prev6 = 0.0;
+#pragma unroll
         for (int sw = 0; sw < KJ - 1; ++sw) {
             if (sw == KJ - 2) { prev5 = Jp[5]; prev6 = Jp[6]; }
+#pragma unroll
             for (int j = 0; j < KJ - 1 - sw; ++j) {
                 const int k = 3 + j;
                 const double a = btv[k] - k * C.OL * Jp[k - 1] - (k - 1) * C.Ok * Jp[k + 1] - (k - 2) * C.Or * Jp[k + 3];
-                Jp[k + 2] = a * C.iOm / (k - 1.5);
+                Jp[k + 2] = a * C.iOm * (1.0 / (k - 1.5));
             }
         }
         useJ = fabs(Jp[5] - prev5) <= 1e-12 * fabs(Jp[5]) && fabs(Jp[6] - prev6) <= 1e-12 * fabs(Jp[6]);
@@ -186,15 +192,15 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
         O.gp[1][t] = C.dH * (Fi * dI - Fk);
         O.gp[2][t] = C.tH * dT;
         O.gp[3][t] = C.dH * dA;
-        O.gp[4][t] = O.gp[1][t] / x2;
+        O.gp[4][t] = O.gp[1][t] * ix2;
     }
     const double iH0 = C.dH * (1.0 / C_KM_S);
     for (int o = 0; o < 5; ++o) O.gp[o][3] = -O.v[o] * iH0;
     O.gz1[0] = -C.dH * iE1;            O.gz2[0] = C.dH * iE2;
     O.gz1[1] = -C.dH * Fi * iE1;       O.gz2[1] = C.dH * Fi * iE2;
-    O.gz1[2] = -C.tH * iE1 / x1;       O.gz2[2] = C.tH * iE2 / x2;
+    O.gz1[2] = -C.tH * iE1 * ix1;      O.gz2[2] = C.tH * iE2 * ix2;
     O.gz1[3] = -C.dH * x1 * x1 * iE1;  O.gz2[3] = C.dH * x2 * x2 * iE2;
-    O.gz1[4] = O.gz1[1] / x2;          O.gz2[4] = O.gz2[1] / x2 - O.v[1] / (x2 * x2);
+    O.gz1[4] = O.gz1[1] * ix2;         O.gz2[4] = O.gz2[1] * ix2 - O.v[1] * (ix2 * ix2);
 }
 
 }  // namespace cb
