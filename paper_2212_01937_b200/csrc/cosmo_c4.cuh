@@ -20,18 +20,29 @@ CB_HD cx operator-(cx a, cx b) { return cx_(a.re - b.re, a.im - b.im); }
 CB_HD cx operator-(cx a) { return cx_(-a.re, -a.im); }
 CB_HD cx operator*(cx a, cx b) { return cx_(a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re); }
 CB_HD cx operator*(double s, cx a) { return cx_(s * a.re, s * a.im); }
+// Division, modulus and square root: IEEE operations by default -- the rare two-complex-pairs rows of the hot path carry eq. (3.9)'s
+// Om/Or cancellation and need every bit.  A translation unit that defines CB_CX_FAST before including this header (tu_w.cu: the extra-w
+// family, where complex arithmetic is the main path and the stated d_abs tolerance is 1e-10) gets the MUFU-seeded forms of cosmo_types.cuh.
+#if defined(CB_CX_FAST) && defined(__CUDA_ARCH__)
+CB_HD double cx_rcp_(double a) { return cb_rcp(a); }
+CB_HD double cx_sqrt_(double a) { return cb_sqrt0(a); }
+CB_HD double cx_abs(cx a) { return cb_sqrt0(a.re * a.re + a.im * a.im); }
+#else
+CB_HD double cx_rcp_(double a) { return 1.0 / a; }
+CB_HD double cx_sqrt_(double a) { return sqrt(a); }
+CB_HD double cx_abs(cx a) { return hypot(a.re, a.im); }
+#endif
 CB_HD cx operator/(cx a, cx b) {
-    const double d = 1.0 / (b.re * b.re + b.im * b.im);
+    const double d = cx_rcp_(b.re * b.re + b.im * b.im);
     return cx_((a.re * b.re + a.im * b.im) * d, (a.im * b.re - a.re * b.im) * d);
 }
 CB_HD cx cx_conj(cx a) { return cx_(a.re, -a.im); }
-CB_HD double cx_abs(cx a) { return hypot(a.re, a.im); }
 CB_HD cx cx_sqrt(cx a) {      // principal square root (Re >= 0)
     const double r = cx_abs(a);
     if (r == 0.0) return cx_(0.0);
-    if (a.re >= 0.0) { const double t = sqrt(0.5 * (r + a.re)); return cx_(t, 0.5 * a.im / t); }
-    const double t = sqrt(0.5 * (r - a.re));
-    return cx_(0.5 * fabs(a.im) / t, a.im >= 0.0 ? t : -t);
+    if (a.re >= 0.0) { const double t = cx_sqrt_(0.5 * (r + a.re)); return cx_(t, 0.5 * a.im * cx_rcp_(t)); }
+    const double t = cx_sqrt_(0.5 * (r - a.re));
+    return cx_(0.5 * fabs(a.im) * cx_rcp_(t), a.im >= 0.0 ? t : -t);
 }
 CB_HD cx cx_log(cx a) { return cx_(log(cx_abs(a)), atan2(a.im, a.re)); }
 

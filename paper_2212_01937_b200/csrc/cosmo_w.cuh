@@ -35,7 +35,8 @@ CB_HD cx w_poly(const double* a, int n, cx x, cx& dp) {       // Horner: value a
     return p;
 }
 
-CB_HD void w_prep(double Om, double OL, double Or, double Ow13, double Ow23, double H0, WCosmo& W) {
+// every structure (degrees 0-4, roots at 0, four real roots, ...): never inlined, the kernels reach it through w_prep's fall-back
+CB_HD_NOINLINE void w_prep_general(double Om, double OL, double Or, double Ow13, double Ow23, double H0, WCosmo& W) {
     const double Ok = 1.0 - Om - OL - Or - Ow13 - Ow23;
     const double a[5] = {OL, Ow23, Ok + Ow13, Om, Or};
     W.Ok = Ok; W.dH = C_KM_S / H0; W.tH = HUBBLE_GYR / H0;
@@ -178,6 +179,95 @@ CB_HD void w_prep(double Om, double OL, double Or, double Ow13, double Ow23, dou
     W.sDr = sqrt(fabs(W.sD));
 }
 
+// S1-S3 of the w family.  Fast front end for the usual structure -- degree 3 or 4 with matter and a constant term, and at least one
+// complex-conjugate pair: Bairstow's iteration for a real quadratic factor x^2 + b x + c of E^2 from the pair of a0 + a3 x^3 ~ 0
+// (x = rho e^{+-i pi/3}, rho = cbrt(a0/a3)) splits E^2 into the two real quadratics directly; roots by the quadratic formula; no
+// indexed arrays, fast reciprocals.  Anything else (and any doubt: no convergence, both factors with real roots, where the pairing
+// of the four real roots matters) goes to w_prep_general.
+CB_HD void w_prep(double Om, double OL, double Or, double Ow13, double Ow23, double H0, WCosmo& W) {
+    const double Ok = 1.0 - Om - OL - Or - Ow13 - Ow23;
+    const double a0 = OL, a1 = Ow23, a2 = Ok + Ow13, a3 = Om, a4 = Or;
+    const double sc = fabs(a0) + fabs(a1) + fabs(a2) + fabs(a3) + fabs(a4);
+    bool ok = (H0 > 0.0) && (a0 > 0.0) && (a3 > 0.0) && (a4 >= 0.0) && (sc < 1e300);
+    double bb = 0.0, cc = 0.0, q2 = a4, q1 = 0.0, q0 = 0.0;
+    if (ok) {
+        const double rho = cbrt(a0 * cb_rcp(a3));
+        bb = -rho; cc = rho * rho;
+        bool conv = false;
+        for (int it = 0; it < 16; ++it) {
+            q1 = a3 - bb * q2; q0 = a2 - bb * q1 - cc * q2;
+            const double r1 = a1 - bb * q0 - cc * q1, r0 = a0 - cc * q0;
+            if (fabs(r1) + fabs(r0) <= 1e-15 * sc) { conv = true; break; }
+            const double s1 = q1 - bb * q2, s0 = q0 - cc * q2;
+            const double u1 = s0 - bb * s1, u0 = -cc * s1;
+            const double det = u1 * s0 - u0 * s1;
+            if (det == 0.0 || !(fabs(det) < 1e300)) break;
+            const double idet = cb_rcp(det);
+            bb += (r1 * s0 - r0 * s1) * idet;
+            cc += (u1 * r0 - u0 * r1) * idet;
+        }
+        ok = conv;
+    }
+    const bool quart = a4 > 0.0;
+    const double d2 = bb * bb - 4.0 * cc;                         // disc of x^2 + b x + c
+    const double d1 = q1 * q1 - 4.0 * q2 * q0;                    // disc of q2 x^2 + q1 x + q0 (quartic case)
+    // the pairing is forced only if a conjugate pair exists; three or four real roots: general path (pairs real roots with neighbours)
+    ok = ok && ((d2 < 0.0) || (quart && d1 < 0.0)) && (quart || q1 != 0.0);
+    if (!ok) { w_prep_general(Om, OL, Or, Ow13, Ow23, H0, W); return; }
+    W.Ok = Ok;
+    { const double iH = cb_rcp(H0); W.dH = C_KM_S * iH; W.tH = HUBBLE_GYR * iH; }
+    W.a[0] = a0; W.a[1] = a1; W.a[2] = a2; W.a[3] = a3; W.a[4] = a4;
+    W.status = 0;
+    W.deg = quart ? 4 : 3;
+    W.f1 = quart ? q2 : 0.0; W.g1 = q1; W.h1 = q0; W.f2 = 1.0; W.g2 = bb; W.h2 = cc;
+    // roots of the two factors
+    cx ra, rb, rc_, rd;                                           // (ra, rb) of Q2, (rc_, rd) of Q1 (rd unused for the cubic)
+    int nr = 0;
+    double real0 = 0.0, real1 = 0.0, real2 = 0.0;                 // real roots, ascending where two come from one quadratic
+    if (d2 < 0.0) { const double sq = cb_sqrt0(-d2); ra = cx_(-0.5 * bb, 0.5 * sq); rb = cx_conj(ra); }
+    else {
+        const double t = -0.5 * (bb + copysign(cb_sqrt0(d2), bb));
+        const double x1 = t, x2 = (t != 0.0) ? cc * cb_rcp(t) : 0.0;
+        ra = cx_(x1); rb = cx_(x2);
+        real0 = fmin(x1, x2); real1 = fmax(x1, x2); nr = 2;
+    }
+    if (quart) {
+        const double i2 = cb_rcp(2.0 * q2);
+        if (d1 < 0.0) { rc_ = cx_(-q1 * i2, cb_sqrt0(-d1) * i2); rd = cx_conj(rc_); }
+        else {
+            const double t = -0.5 * (q1 + copysign(cb_sqrt0(d1), q1));
+            const double x1 = t * cb_rcp(q2), x2 = (t != 0.0) ? q0 * cb_rcp(t) : 0.0;
+            rc_ = cx_(x1); rd = cx_(x2);
+            real0 = fmin(x1, x2); real1 = fmax(x1, x2); nr = 2;   // (d2 < 0 here: the only real roots)
+        }
+    } else {
+        const double xl = -q0 * cb_rcp(q1);
+        rc_ = cx_(xl); rd = cx_(0.0);
+        if (nr == 0) { real0 = xl; nr = 1; }
+        else { real2 = fmax(real1, xl); const double lo = fmin(real0, xl), mid = fmax(real0, fmin(real1, xl)); real0 = lo; real1 = mid; nr = 3; }
+    }
+    W.nreal = nr; W.rr[0] = real0; W.rr[1] = real1; W.rr[2] = real2; W.rr[3] = 0.0;
+    // roots by decreasing modulus (sorting network on four scalars; the cubic's fourth slot has modulus -1 and stays last)
+    double ma = ra.re * ra.re + ra.im * ra.im, mb = rb.re * rb.re + rb.im * rb.im, mc = rc_.re * rc_.re + rc_.im * rc_.im,
+           md = quart ? rd.re * rd.re + rd.im * rd.im : -1.0;
+    auto cswap = [](cx& u, double& mu, cx& v, double& mv) { if (mu < mv) { const cx t = u; u = v; v = t; const double m = mu; mu = mv; mv = m; } };
+    cswap(ra, ma, rb, mb); cswap(rc_, mc, rd, md); cswap(ra, ma, rc_, mc); cswap(rb, mb, rd, md); cswap(rb, mb, rc_, mc);
+    W.rt[0] = ra; W.rt[1] = rb; W.rt[2] = rc_; W.rt[3] = rd;
+    W.iA = 3;
+    if (fabs(rb.im) <= 1e-9 * sqrt(mb)) W.iA = 1;
+    if (fabs(rc_.im) <= 1e-9 * sqrt(mc)) W.iA = 2;
+    if (quart && fabs(rd.im) <= 1e-9 * sqrt(md)) W.iA = 3;
+    // the product must reproduce the coefficients
+    const double e4 = W.f1, e3 = W.f1 * W.g2 + W.g1, e2 = W.f1 * W.h2 + W.g1 * W.g2 + W.h1, e1 = W.g1 * W.h2 + W.h1 * W.g2, e0 = W.h1 * W.h2;
+    const double res = fabs(e4 - a4) + fabs(e3 - a3) + fabs(e2 - a2) + fabs(e1 - a1) + fabs(e0 - a0);
+    if (!(res <= 1e-11 * sc)) W.status |= ST_UNSUPPORTED;
+    W.q11 = W.f1 + W.g1 + W.h1;
+    W.q21 = W.f2 + W.g2 + W.h2;
+    W.theta = 2.0 * W.f1 * W.h2 + 2.0 * W.h1 * W.f2 - W.g1 * W.g2;
+    W.sD = 0.25 * (W.g1 * W.g1 - 4.0 * W.f1 * W.h1) * d2;
+    W.sDr = cb_sqrt0(fabs(W.sD));
+}
+
 // values v[4] = D_C, D_M, D_L, mu and dz[4] = their d/dz
 template <typename Vote>
 CB_HD unsigned w_eval(const WCosmo& W, double z, const Vote& vote, double v[4], double dz[4]) {
@@ -189,7 +279,7 @@ CB_HD unsigned w_eval(const WCosmo& W, double z, const Vote& vote, double v[4], 
     const double q1x = fma(fma(W.f1, x, W.g1), x, W.h1), q2x = fma(fma(W.f2, x, W.g2), x, W.h2);
     const double a1 = q1x * W.q21, a2 = W.q11 * q2x;
     if (!(a1 > 0.0) || !(a2 > 0.0)) st[0] |= ST_ROOT_ON_PATH;          // E^2 <= 0 on the way (or NaN input)
-    const double ra = sqrt(a1), rb = sqrt(a2), U12 = ra + rb;
+    const double ra = cb_sqrt0(a1), rb = cb_sqrt0(a2), U12 = ra + rb;
     double xa[1] = {U12 * U12}, mp[1], s[1], p5[1] = {0.0}, p0[1] = {0.0};
     const double hd = 0.5 * z2 * W.theta, hs = z2 * W.sDr;
     mp[0] = xa[0] - hd;
@@ -199,14 +289,14 @@ CB_HD unsigned w_eval(const WCosmo& W, double z, const Vote& vote, double v[4], 
     carlson_dup<double, false, false, false, 1, Vote>(xa, mp, s, p5, p0, dl5, dl0, Qc, Q5v, Q0v, st, vote, g2, tailD, sum5, sum0);
     const double RF = carlson_rf_series<double>(xa[0], mp[0], g2, hd, s[0]);
     const double I0 = 2.0 * z * RF;                                        // eq. (3.7) / (B.1)
-    const double iE = 1.0 / (ra * rb);                                     // E(1) = 1: a1 a2 = E^2(x)
+    const double iE = cb_rcp(ra * rb);                                     // E(1) = 1: a1 a2 = E^2(x)
     double F, Fi, Fk;
     sinn<double>(W.Ok, I0, F, Fi, Fk);
     v[0] = W.dH * I0; v[1] = W.dH * F; v[2] = x * v[1];
     dz[0] = W.dH * iE; dz[1] = W.dH * Fi * iE; dz[2] = fma(x, dz[1], v[1]);
     if (v[2] > 0.0) {
-        v[3] = fma(CB_KT.five_over_ln10, log(v[2]), 25.0);
-        dz[3] = CB_KT.five_over_ln10 * dz[2] / v[2];
+        v[3] = fma(CB_KT.five_over_ln10, Num<double>::log_(v[2]), 25.0);
+        dz[3] = CB_KT.five_over_ln10 * dz[2] * cb_rcp(v[2]);
     } else {
         v[3] = dz[3] = NAN;
         if (!(st[0] & (ST_ROOT_ON_PATH | ST_UNSUPPORTED))) st[0] |= ST_DL_NONPOS;
@@ -407,8 +497,8 @@ CB_HD_NOINLINE unsigned w_grad_quad(const WCosmo& W, double z, double out[12]) {
         for (int i = 0; i < 12; ++i) {
             const double t = fma(wd, X12[i], tlo), x = 1.0 + t;
             const double e2 = fma(fma(fma(fma(W.a[4], x, W.a[3]), x, W.a[2]), x, W.a[1]), x, W.a[0]);
-            const double ie = 1.0 / sqrt(e2), f = (W12[i] * wd) * (ie * ie) * (ie * t);
-            const double x2 = x * x, xp1 = x + 1.0, ix = 1.0 / x;
+            const double ie = Num<double>::rsqrt_(e2), f = (W12[i] * wd) * (ie * ie) * (ie * t);
+            const double x2 = x * x, xp1 = x + 1.0, ix = cb_rcp(x);
             const double d[4] = {f * x2, -f * xp1, f * x2 * xp1, -f * x};
 #pragma unroll
             for (int th = 0; th < 4; ++th) { out[th] += d[th]; out[4 + th] = fma(d[th], ix, out[4 + th]); out[8 + th] = fma(d[th], x2, out[8 + th]); }
