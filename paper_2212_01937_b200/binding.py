@@ -148,8 +148,22 @@ def workspace_bytes(n_z, n_cosmo, mode, which, with_grad) -> int:
     return int(lib().cosmo_workspace_bytes(n_z, n_cosmo, mode, which_mask(which), int(with_grad)))
 
 
+def _given(t, shape, dtype, torch, name, device):
+    """a caller-supplied output buffer: contiguous CUDA tensor of the expected dtype, element count and device"""
+    if t is None:
+        return None
+    n = 1
+    for d in shape:
+        n *= d
+    if not (t.is_cuda and t.dtype == dtype and t.is_contiguous() and t.numel() == n and t.device == device):
+        raise CosmoError(f"{name}: expected a contiguous {dtype} CUDA tensor with {n} elements {tuple(shape)} on {device}")
+    return t
+
+
 def _workspace(torch, nbytes, device, workspace):
     if workspace is not None:
+        if not (workspace.is_cuda and workspace.is_contiguous() and workspace.device == device):
+            raise CosmoError(f"workspace: expected a contiguous CUDA tensor on {device}")
         if workspace.numel() * workspace.element_size() < nbytes:
             raise CosmoError("workspace tensor too small")
         return workspace
@@ -167,6 +181,8 @@ def cosmo_eval(z, Om, OL, Or, H0, mode=ELEMENTWISE, which=("DC",), out=None, sta
     n_z = z.numel()
     rows = n_cosmo if mode == OUTER else 1
     nw = bin(mask).count("1")
+    _given(out, (nw, rows, n_z), dt, torch, "out", z.device)
+    _given(status, (rows, n_z), torch.uint8, torch, "status", z.device)
     if out is None:
         out = torch.empty((nw, rows, n_z), dtype=dt, device=z.device)
     if status is None:
@@ -174,7 +190,8 @@ def cosmo_eval(z, Om, OL, Or, H0, mode=ELEMENTWISE, which=("DC",), out=None, sta
     ws_b = workspace_bytes(n_z, n_cosmo, mode, mask, False)
     ws = _workspace(torch, ws_b, z.device, workspace)
     fn = lib().cosmo_eval_f32 if f32 else lib().cosmo_eval
-    _check(fn(_ptr(z), n_z, P, n_cosmo, mode, mask, _ptr(out), _ptr(status), _ptr(ws), ws.numel(), _stream(torch)))
+    with torch.cuda.device(z.device):          # kernels and stream of the tensors' device, whatever the current one is
+        _check(fn(_ptr(z), n_z, P, n_cosmo, mode, mask, _ptr(out), _ptr(status), _ptr(ws), ws.numel() * ws.element_size(), _stream(torch)))
     return out, status
 
 
@@ -193,6 +210,10 @@ def cosmo_vjp(z, Om, OL, Or, H0, grad_out, mode=ELEMENTWISE, which=("DC",), want
     nw = bin(mask).count("1")
     if grad_out.numel() != nw * rows * n_z:
         raise CosmoError("grad_out must have shape [n_which, rows, n_z]")
+    _given(out, (nw, rows, n_z), dt, torch, "out", z.device)
+    _given(grad_z, (n_z,), dt, torch, "grad_z", z.device)
+    _given(grad_params, (4, n_cosmo), torch.float64, torch, "grad_params", z.device)
+    _given(status, (rows, n_z), torch.uint8, torch, "status", z.device)
     if want_out and out is None:
         out = torch.empty((nw, rows, n_z), dtype=dt, device=z.device)
     if grad_z is None:
@@ -204,8 +225,9 @@ def cosmo_vjp(z, Om, OL, Or, H0, grad_out, mode=ELEMENTWISE, which=("DC",), want
     ws_b = workspace_bytes(n_z, n_cosmo, mode, mask, True)
     ws = _workspace(torch, ws_b, z.device, workspace)
     fn = lib().cosmo_vjp_f32 if f32 else lib().cosmo_vjp
-    _check(fn(_ptr(z), n_z, P, n_cosmo, mode, mask, _ptr(grad_out), _ptr(out), _ptr(grad_z), _ptr(grad_params), _ptr(status),
-              _ptr(ws), ws.numel(), _stream(torch)))
+    with torch.cuda.device(z.device):
+        _check(fn(_ptr(z), n_z, P, n_cosmo, mode, mask, _ptr(grad_out), _ptr(out), _ptr(grad_z), _ptr(grad_params), _ptr(status),
+                  _ptr(ws), ws.numel() * ws.element_size(), _stream(torch)))
     return grad_z, grad_params, out, status
 
 
@@ -218,6 +240,10 @@ def cosmo_snia_loglike(z, mu_obs, sigma, Om, OL, Or, H0, want_grad=True, logL=No
         _dev(t, dt, torch, nm)
     P, S, keep = _params(Om, OL, Or, H0, torch)
     N = z.numel()
+    _given(logL, (S,), torch.float64, torch, "logL", z.device)
+    _given(grad, (4, S), torch.float64, torch, "grad", z.device)
+    if mu_obs.numel() != N or sigma.numel() != N:
+        raise CosmoError("z, mu_obs and sigma must have the same length")
     if logL is None:
         logL = torch.empty(S, dtype=torch.float64, device=z.device)
     if want_grad and grad is None:
@@ -225,7 +251,8 @@ def cosmo_snia_loglike(z, mu_obs, sigma, Om, OL, Or, H0, want_grad=True, logL=No
     ws_b = workspace_bytes(N, S, OUTER, MU, True)
     ws = _workspace(torch, ws_b, z.device, workspace)
     fn = lib().cosmo_snia_loglike_f32 if f32 else lib().cosmo_snia_loglike
-    _check(fn(_ptr(z), _ptr(mu_obs), _ptr(sigma), N, P, S, _ptr(logL), _ptr(grad), _ptr(ws), ws.numel(), _stream(torch)))
+    with torch.cuda.device(z.device):
+        _check(fn(_ptr(z), _ptr(mu_obs), _ptr(sigma), N, P, S, _ptr(logL), _ptr(grad), _ptr(ws), ws.numel() * ws.element_size(), _stream(torch)))
     return logL, grad
 
 

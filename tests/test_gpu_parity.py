@@ -330,6 +330,26 @@ def test_errors(cb):
         cb.cosmo_eval(z, *p, cb.OUTER, ("DC",), workspace=torch.empty(8, dtype=torch.uint8, device="cuda"))
 
 
+def test_binding_validates_supplied_buffers(cb):
+    """caller-supplied output buffers of the wrong size or dtype are refused by the binding, not written past"""
+    import torch
+    z = dev(np.linspace(0.1, 1.0, 64))
+    p = [dev(np.array([v])) for v in (0.3, 0.7, 9e-5, 70.0)]
+    with pytest.raises(cb.CosmoError):
+        cb.cosmo_eval(z, *p, cb.ELEMENTWISE, ("DC", "MU"), out=torch.empty((1, 1, 64), dtype=torch.float64, device="cuda"))
+    with pytest.raises(cb.CosmoError):
+        cb.cosmo_eval(z, *p, cb.ELEMENTWISE, ("DC",), status=torch.empty((1, 64), dtype=torch.int32, device="cuda"))
+    g = dev(np.ones((1, 1, 64)))
+    with pytest.raises(cb.CosmoError):
+        cb.cosmo_vjp(z, *p, g, cb.OUTER, ("DC",), grad_params=torch.empty((4, 2), dtype=torch.float64, device="cuda"))
+    with pytest.raises(cb.CosmoError):
+        cb.cosmo_vjp(z, *p, g, cb.OUTER, ("DC",), grad_z=torch.empty(64, dtype=torch.float32, device="cuda"))
+    with pytest.raises(cb.CosmoError):
+        cb.cosmo_snia_loglike(z, z[:10].contiguous(), z, *p)
+    out, st = cb.cosmo_eval(z, *p, cb.ELEMENTWISE, ("DC",), out=torch.empty((1, 1, 64), dtype=torch.float64, device="cuda"))
+    assert bool(torch.isfinite(out).all())
+
+
 def test_host_call_matches_device_call(cb):
     w = W.config3(n=4001, S=3)
     out_h, gz_h, gp_h, st_h = cb.cosmo_eval_host(w.z, w.Om, w.OL, w.Or, w.H0, cb.OUTER, w.which, grad_out=w.grad_out)
