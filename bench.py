@@ -368,7 +368,7 @@ def run_ours(args):
                 "algorithmic_bytes": alg_bytes,
                 "pipe_frac": (pipe * evals / (k_ms * 1e-3)) / (peak_tflops * 0.5e12) if (pipe and k_ms > 0 and peak_tflops) else None,
                 "kernel": kernel, "kernel_ms": k_ms, "kernel_launches_timed": k_n,
-                "flops_per_eval": fpe, "flops_source": RL.SOURCE.get(key),
+                "flops_per_eval": fpe, "flops_source": RL.SOURCE.get(key), "flops_build_matches": RL.csrc_hash() == RL.CAPTURED_CSRC_HASH,
                 "peak_source": f"measured live: cosmo_probe_fma_{args.dtype} (8 FMA chains/thread)",
                 "nominal_tflops": RL.NOMINAL_FP64_TFLOPS if not f32 else RL.NOMINAL_FP32_TFLOPS,
                 "hbm_gbs_achieved": alg_bytes / (k_ms * 1e-3) / 1e9 if k_ms > 0 else None}
