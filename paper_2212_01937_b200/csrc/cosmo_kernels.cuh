@@ -362,15 +362,6 @@ __global__ void k_reduce_vjp(const double* __restrict__ part, int64_t ntiles, in
     if (lane == 0) grad[(int64_t)j * S + s] = v;
 }
 
-template <typename T>
-__global__ void k_reduce_gz(const T* __restrict__ part, int ny, int64_t N, T* __restrict__ gz) {
-    int64_t n = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-    if (n >= N) return;
-    T v = T(0);
-    for (int y = 0; y < ny; ++y) v += part[(int64_t)y * N + n];
-    gz[n] = v;
-}
-
 // ELEMENTWISE with one cosmology per redshift: S1-S8 per thread (cosmo_obs.cuh, elem_one), no reductions.
 // Register budget: left alone the all-outputs variants take 255 registers (8 warps/SM) and wait on latency at a third of the
 // FP64 pipe; capped at 128 (VJP) / 80 (forward) registers they run 16 / 24 warps per SM (profiles/).  Blocks of 256 threads measured 7-10 %

@@ -61,7 +61,6 @@ void launch_elem_f32(bool with_grad, const ElemArgs& a, cudaStream_t st);
 void launch_reduce_params(int np, const double* part, int64_t ntiles, int64_t S, double* logL, double* grad, cudaStream_t st);
 void launch_reduce_vjp(bool f32, const double* part, int64_t ntiles, int64_t S, double* grad, const void* gzpart, int ny, int64_t N, void* gz,
                        cudaStream_t st);
-void launch_reduce_gz(bool f32, const void* part, int ny, int64_t N, void* gz, cudaStream_t st);
 void launch_two(const double* z1, const double* z2, const double* Om, const double* OL, const double* Or, const double* H0, int64_t n,
                 int64_t n_cosmo, unsigned which, const double* gout, double* out, double* gz1, double* gz2, double* gparams,
                 uint8_t* status, unsigned* ws, cudaStream_t st);

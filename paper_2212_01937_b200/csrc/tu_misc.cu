@@ -132,10 +132,6 @@ void launch_reduce_vjp(bool f32, const double* part, int64_t ntiles, int64_t S, 
     if (f32) launch_pdl(k_reduce_vjp<float>, dim3(nb_gz + nb_p), dim3(256), st, part, ntiles, S, grad, static_cast<const float*>(gzpart), ny, N, static_cast<float*>(gz), nb_gz);
     else launch_pdl(k_reduce_vjp<double>, dim3(nb_gz + nb_p), dim3(256), st, part, ntiles, S, grad, static_cast<const double*>(gzpart), ny, N, static_cast<double*>(gz), nb_gz);
 }
-void launch_reduce_gz(bool f32, const void* part, int ny, int64_t N, void* gz, cudaStream_t st) {
-    if (f32) k_reduce_gz<float><<<(unsigned)cdiv64(N, 256), 256, 0, st>>>(static_cast<const float*>(part), ny, N, static_cast<float*>(gz));
-    else k_reduce_gz<double><<<(unsigned)cdiv64(N, 256), 256, 0, st>>>(static_cast<const double*>(part), ny, N, static_cast<double*>(gz));
-}
 void launch_two(const double* z1, const double* z2, const double* Om, const double* OL, const double* Or, const double* H0, int64_t n,
                 int64_t n_cosmo, unsigned which, const double* gout, double* out, double* gz1, double* gz2, double* gparams,
                 uint8_t* status, unsigned* ws, cudaStream_t st) {

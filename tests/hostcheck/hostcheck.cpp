@@ -12,7 +12,7 @@ using namespace cb;
 
 template <typename T>
 static void run(int64_t n, const double* z, const double* Om, const double* OL, const double* Or, const double* H0,
-                unsigned which, const double* gup, double* out, double* gz, double* gp, uint8_t* status, double* cond_out = nullptr) {
+                unsigned which, const double* gup, double* out, double* gz, double* gp, uint8_t* status) {
     for (int64_t i = 0; i < n; ++i) {
         Cosmo<double> Cd;
         cosmo_prep(Om[i], OL[i], Or[i], H0[i], gup ? 2 : 0, Cd);
@@ -31,13 +31,8 @@ static void run(int64_t n, const double* z, const double* Om, const double* OL, 
         if (gup) {
             T g[N_PLANES], a = 0, p[4] = {0, 0, 0, 0};
             for (int w = 0; w < N_PLANES; ++w) g[w] = (which >> w & 1) ? (T)gup[w * n + i] : T(0);
-            if (cond_out) {   // the gradient bases alone, with their cancellation factor
-                T cond = 0;
-                backward<T, true, true, true>(C, (T)z[i], R, O, g, a, p, &cond);
-                cond_out[i] = (double)cond;
-            } else {          // what the ELEMENTWISE kernel does: bases where accurate, quadrature elsewhere
-                status[i] |= (uint8_t)backward_robust<T, true, true>(C, (T)z[i], R, O, g, a, p, which);
-            }
+            // what the OUTER kernels' checked row does: bases where accurate, quadrature elsewhere
+            status[i] |= (uint8_t)backward_robust<T, true, true>(C, (T)z[i], R, O, g, a, p, which);
             gz[i] = (double)a;
             for (int t = 0; t < 4; ++t) gp[t * n + i] = (double)p[t];
         }
@@ -73,18 +68,6 @@ extern "C" void hostcheck_elem_f64(int64_t n, const double* z, const double* Om,
 extern "C" void hostcheck_elem_f32(int64_t n, const double* z, const double* Om, const double* OL, const double* Or, const double* H0,
                                    unsigned which, const double* gup, double* out, double* gz, double* gp, uint8_t* status) {
     run_elem<float>(n, z, Om, OL, Or, H0, which, gup, out, gz, gp, status);
-}
-extern "C" void hostcheck_f64_cond(int64_t n, const double* z, const double* Om, const double* OL, const double* Or, const double* H0,
-                                   unsigned which, const double* gup, double* out, double* gz, double* gp, uint8_t* status, double* cond) {
-    run<double>(n, z, Om, OL, Or, H0, which, gup, out, gz, gp, status, cond);
-}
-// the whole per-cosmology block as doubles: out[COSMO_NFIELDS + 2] (fields in declaration order, then status, cubic)
-extern "C" void hostcheck_cosmo(double Om, double OL, double Or, double H0, int want_grad, double* out) {
-    Cosmo<double> C;
-    memset(&C, 0, sizeof(C));
-    cosmo_prep(Om, OL, Or, H0, want_grad, C);
-    memcpy(out, &C, COSMO_NFIELDS * sizeof(double));
-    out[COSMO_NFIELDS] = (double)C.status; out[COSMO_NFIELDS + 1] = (double)C.cubic;
 }
 extern "C" void hostcheck_factor(double Om, double OL, double Or, double* out5) {
     Cosmo<double> C;
