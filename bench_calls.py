@@ -90,6 +90,20 @@ def main():
         g32, out32, gz32 = g.to(torch.float32), out.to(torch.float32), gz.to(torch.float32)
         timed(lambda: cb.cosmo_vjp(*a32, g32, cb.OUTER, w.which, out=out32, grad_z=gz32, grad_params=gp, status=st, workspace=ws), S * N,
               "config3 fwd+VJP mu OUTER f32")
+    if want("outer6"):
+        # every plane in OUTER mode (the SBI use, PAPER.md:287 fn.24): 10^6 redshifts x 16 cosmologies, all six outputs
+        w = W.config3(n=1_000_000 // f, S=16, which=("DC", "DM", "DL", "MU", "TL", "DABS"))
+        a = [dev(x) for x in (w.z, w.Om, w.OL, w.Or, w.H0)]
+        g = dev(w.grad_out)
+        S, N = w.n_cosmo, w.n_z
+        out = torch.empty((6, S, N), dtype=torch.float64, device="cuda")
+        gz = torch.empty(N, dtype=torch.float64, device="cuda")
+        gp = torch.empty((4, S), dtype=torch.float64, device="cuda")
+        st = torch.empty((S, N), dtype=torch.uint8, device="cuda")
+        ws = torch.empty(cb.workspace_bytes(N, S, cb.OUTER, w.which, True), dtype=torch.uint8, device="cuda")
+        timed(lambda: cb.cosmo_vjp(*a, g, cb.OUTER, w.which, out=out, grad_z=gz, grad_params=gp, status=st, workspace=ws), S * N,
+              "OUTER all six outputs fwd+VJP, N=1e6 x S=16 f64")
+        timed(lambda: cb.cosmo_eval(*a, cb.OUTER, w.which, out=out, status=st, workspace=ws), S * N, "OUTER all six outputs fwd only, N=1e6 x S=16 f64")
     if want("config4"):
         n = 1_000_000 // f
         z = rng.uniform(0.01, 1.5, n)
