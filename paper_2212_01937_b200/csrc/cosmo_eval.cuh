@@ -489,7 +489,7 @@ CB_HD void eval_core_k(const Cosmo<T>& C0, const T (&z)[K], const Vote& vote, Co
                 // the same Carlson values are assembled without that cancellation: with
                 // u_j = int x^j dx/E, d(x^k E) gives  (k+3/2) Om u_{k+2} = [x^k E] - (k+2) Or u_{k+3} - (k+1) Ok u_{k+1}
                 // - k OL u_{k-1};  u_0 = I0 and u_1 = 2 z B0 + rn I0 are known, the Or terms are iterated (Gauss-Seidel).
-                constexpr int KS = 8;
+                constexpr int KS = REC_KS;
                 T u[KS + 4], bk[KS + 1];
                 u[0] = R[k].I0;
                 u[1] = N::fma_(T(2) * z[k], B0, C.rn * R[k].I0);

@@ -267,8 +267,8 @@ CB_HD void grad_basis(const Cosmo<T>& C, const Rows& rows, T z, const Core<T>& R
         // (the x^5, x^6 rows), which loses Om/Or digits.  Instead J'_p = int x^p dx/E^3, p = 2, 3, 4, come from the basis and
         // J'_5.. follow from d(x^k / E) = N_k / E^3:  Om (k - 3/2) J'_{k+2} = [x^k/E] - k OL J'_{k-1} - (k-1) Ok J'_{k+1}
         // - (k-2) Or J'_{k+3}, the Or terms iterated (same scheme as the forward d_abs).
-        constexpr int KJ = 12;                // levels k = 3 .. 3 + KJ - 1
-        T Jp[17], Sp[7];
+        constexpr int KJ = REC_KJ;            // levels k = 3 .. 3 + KJ - 1
+        T Jp[KJ + 5], Sp[7];
         Jp[0] = Jp[1] = T(0); Sp[0] = Sp[1] = T(0);
 #pragma unroll
         for (int p = 2; p < 5; ++p) {
@@ -278,7 +278,7 @@ CB_HD void grad_basis(const Cosmo<T>& C, const Rows& rows, T z, const Core<T>& R
             Sp[p] = kCond ? asum5(gj) : T(0);
         }
 #pragma unroll
-        for (int p = 5; p < 17; ++p) Jp[p] = T(0);
+        for (int p = 5; p < KJ + 5; ++p) Jp[p] = T(0);
         T bk[KJ];
         {
             T dk = n3;             // x^k - 1 = x (x^(k-1) - 1) + z, from x^3 - 1: no cancellation at small z

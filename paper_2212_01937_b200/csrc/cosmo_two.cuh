@@ -82,7 +82,7 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
             const double t4 = dz * C.sig * B0;
             const double A39 = (t1 + t2) + (t3 + t4);
             // radiation-perturbative assembly (see eval_core_k): u_j = int x^j dx/E between the limits
-            constexpr int KS = 8;
+            constexpr int KS = REC_KS;
             double u[KS + 4], bk[KS + 1];
             u[0] = I0;
             u[1] = fma(2.0 * dz, B0, C.rn * I0);
@@ -118,10 +118,10 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
     if (!with_grad) return;
     // ---- S8: the same bases (GI, GT, GA/GJ) on two-limit basis values; b_k = x2^k/E2 - x1^k/E1
     const double iE1 = cb_rcp(E1), iE2 = cb_rcp(E2), diE = -dE * iE1 * iE2;            // 1/E2 - 1/E1
-    double btv[16];
+    double btv[REC_KJ + 4];
     {
         double xk1 = 1.0, dk = 0.0;
-        for (int k = 0; k < 16; ++k) { btv[k] = fma(dk, iE2, xk1 * diE); dk = fma(x2, dk, xk1 * dz); xk1 *= x1; }
+        for (int k = 0; k < REC_KJ + 4; ++k) { btv[k] = fma(dk, iE2, xk1 * diE); dk = fma(x2, dk, xk1 * dz); xk1 *= x1; }
     }
     // raw gradient integrals int D_theta p_X / E^3 dx between the limits (cosmo_obs.cuh, GradInt) with their cancellation factor
     double rI[3], rT[3], rA[3];
@@ -133,17 +133,17 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
     const double aI0 = fabs(I0), aK = fabs(K), a0 = fabs(btv[0]), a1 = fabs(btv[1]), a2 = fabs(btv[2]);
     auto dot5 = [&](const double* g) { return g[0] * I0 + g[1] * K + g[2] * btv[0] + g[3] * btv[1] + g[4] * btv[2]; };
     auto abs5 = [&](const double* g) { return fabs(g[0]) * aI0 + fabs(g[1]) * aK + fabs(g[2]) * a0 + fabs(g[3]) * a1 + fabs(g[4]) * a2; };
-    double Jp[17], Sp[7];
+    double Jp[REC_KJ + 5], Sp[7];
     bool useJ = false;
     {
-        constexpr int KJ = 12;
+        constexpr int KJ = REC_KJ;
         Jp[0] = Jp[1] = 0.0; Sp[0] = Sp[1] = 0.0;
         for (int p = 2; p < 5; ++p) {
             double g[5];
             S.rowJ(p, g);
             Jp[p] = dot5(g); Sp[p] = abs5(g);
         }
-        for (int p = 5; p < 17; ++p) Jp[p] = 0.0;
+        for (int p = 5; p < REC_KJ + 5; ++p) Jp[p] = 0.0;
         double prev5 = 0.0, prev6 = 0.0;
 #pragma unroll
         for (int sw = 0; sw < KJ - 1; ++sw) {
