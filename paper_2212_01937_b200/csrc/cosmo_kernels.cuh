@@ -148,8 +148,13 @@ __device__ __noinline__ void outer_slow_row(const OuterArgs& a, const Cosmo<T>& 
 #ifndef CB_MINBLOCKS
 #define CB_MINBLOCKS 3     // chi-family kernels: 160 registers, 12 warps/SM (measured best with KZ = 4, profiles/)
 #endif
+// The VJP kernels that also carry the R_J tracks (t_L, d_abs, age) hold ~60 doubles of per-element state for two elements in lock-step
+// besides the loop state and spill 1.4 KB per thread at any register cap.  They take the one-element-at-a-time row function for every
+// cosmology instead (with 255 registers, 8 warps/SM): 3.07 -> 2.37 ms on 10^6 x 16, all six planes (profiles/, bench_calls.py outer6).
+__host__ __device__ constexpr bool outer_sequential(bool kT, bool kA, int mode) { return mode == MODE_VJP && (kT || kA); }
+
 template <typename T, bool kT, bool kA, int MODE, unsigned WCT>
-__global__ void __launch_bounds__(OUTER_THREADS, CB_MINBLOCKS) k_outer(OuterArgs a) {
+__global__ void __launch_bounds__(OUTER_THREADS, outer_sequential(kT, kA, MODE) ? 2 : CB_MINBLOCKS) k_outer(OuterArgs a) {
     constexpr int KZ = outer_kz(kT, kA), TILE = outer_tile(kT, kA);
     const unsigned which = WCT ? WCT : a.which;      // WCT != 0: output set known at compile time (drops dead planes)
     constexpr bool kG = MODE != MODE_FWD;
@@ -202,8 +207,9 @@ __global__ void __launch_bounds__(OUTER_THREADS, CB_MINBLOCKS) k_outer(OuterArgs
             const Cosmo<T>& C = sc[sl];
             const int64_t row = c0 + sl;
             if (MODE == MODE_JOINT) load2(zp + roff, n0, N, vec, zv);      // latent redshifts: one row per sample
-            // two complex root pairs, or (with gradients) bases that need the per-element conditioning check: whole row apart
-            if ((C.cubic & 2u) || (kG && (C.cubic & 12u))) {
+            // two complex root pairs, or (with gradients) bases that need the per-element conditioning check: whole row apart; so do
+            // the variants whose per-element state does not fit two elements in lock-step (outer_sequential)
+            if ((C.cubic & 2u) || (kG && (C.cubic & 12u)) || outer_sequential(kT, kA, MODE)) {
                 outer_slow_row<T, kT, kA, MODE>(a, C, row, n0, zv, mo, isig2, lnorm, zo, kLike ? (unsigned)W_MU : which,
                                                 kG ? &sacc[warp][sl][0] : nullptr, lane, gzacc);
                 continue;
