@@ -159,7 +159,8 @@ size_t cosmo_eval2_workspace_bytes(int64_t n, int with_grad);
  *   status (nullable): 1 root of E^2 on the path / E^2 <= 0; 2 unsupported input or factorisation failure -- also set, with NaN in the
  *   t_L / d_abs planes only, where E^2 has degree <= 2 with distinct roots (the method needs degree 3 or 4; monomials
  *   E^2 = a x^n are served in closed form); 4 D_L <= 0; 8 iteration cap; 16 as above.
- *   workspace: cosmo_eval_w_workspace_bytes(n_cosmo) bytes (a shared cosmology is factored once per call into it; 0 for n_cosmo = n). */
+ *   workspace: cosmo_eval_w_workspace_bytes(n_cosmo) bytes: a shared cosmology is factored once per call into it; with per-element
+ *   cosmologies it holds the work list of the second pass (elements that need the general root solve), n < 2^32. */
 int cosmo_eval_w(const double* z, int64_t n, const double* Om, const double* OL, const double* Or, const double* Ow13,
                  const double* Ow23, const double* H0, int64_t n_cosmo, uint32_t which, const double* grad_out, double* out,
                  double* dout_dz, double* grad_z, double* grad_params, uint8_t* status, void* workspace, size_t ws_bytes, void* stream);

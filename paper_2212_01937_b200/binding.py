@@ -347,7 +347,7 @@ def cosmo_eval_w(z, Om, OL, Or, Ow13, Ow23, H0, which=("DC",), want_dz=True, gra
         gz = torch.empty(n, dtype=torch.float64, device=z.device)
         gp = torch.empty((6, n), dtype=torch.float64, device=z.device)
     ws_b = int(lib().cosmo_eval_w_workspace_bytes(n_cosmo))
-    ws = _workspace(torch, ws_b, z.device, workspace) if ws_b else None
+    ws = _workspace(torch, ws_b, z.device, workspace)
     _check(lib().cosmo_eval_w(_ptr(z), n, *[_ptr(t) for t in ps], n_cosmo, mask, _ptr(grad_out), _ptr(out), _ptr(dz), _ptr(gz), _ptr(gp),
                               _ptr(status), _ptr(ws), ws_b, _stream(torch)))
     if grad_out is None:

@@ -434,7 +434,11 @@ int cosmo_eval2(const double* z1, const double* z2, int64_t n, cosmo_params p, i
     return check_launch();
 }
 
-size_t cosmo_eval_w_workspace_bytes(int64_t n_cosmo) { return n_cosmo == 1 ? align256(w_cosmo_bytes()) : 0; }
+size_t cosmo_eval_w_workspace_bytes(int64_t n_cosmo) {
+    if (n_cosmo <= 0) return 0;
+    // a shared cosmology's factored block, or (per-element cosmologies) the counter + work list of the second pass
+    return n_cosmo == 1 ? align256(w_cosmo_bytes()) : 256 + align256((size_t)n_cosmo * sizeof(unsigned));
+}
 
 int cosmo_eval_w(const double* z, int64_t n, const double* Om, const double* OL, const double* Or, const double* Ow13,
                  const double* Ow23, const double* H0, int64_t n_cosmo, uint32_t which, const double* grad_out, double* out,
@@ -444,15 +448,14 @@ int cosmo_eval_w(const double* z, int64_t n, const double* Om, const double* OL,
     if (n == 0) return COSMO_OK;
     if (!z || !Om || !OL || !Or || !Ow13 || !Ow23 || !H0) return COSMO_E_NULL;
     if (grad_out ? (!grad_z || !grad_params) : !out) return COSMO_E_NULL;
-    if (n_cosmo == 1) {
-        if (!workspace) return COSMO_E_NULL;
-        if (ws_bytes < cosmo_eval_w_workspace_bytes(1)) return COSMO_E_WORKSPACE;
-    }
+    if (n > (int64_t)0xffffffffll) return COSMO_E_SIZE;                  // 32-bit work list
+    if (!workspace) return COSMO_E_NULL;
+    if (ws_bytes < cosmo_eval_w_workspace_bytes(n_cosmo)) return COSMO_E_WORKSPACE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     prof_begin(st);
     launch_w(z, Om, OL, Or, Ow13, Ow23, H0, n, n_cosmo, which, grad_out, out, dout_dz, grad_z, grad_params, status, workspace, st);
     prof_end(st);
-    if (n_cosmo == 1) g_launches += 1;
+    g_launches += (n_cosmo == 1) ? 1 : 2;          // prep kernel, or memset-free second pass (+ its list reset)
     return check_launch();
 }
 

@@ -97,6 +97,7 @@ CB_HD_NOINLINE void w_prep_general(double Om, double OL, double Or, double Ow13,
                 else r[2] = cx_(-q0 / q1);
             }
         }
+        double prev_big = 1e300;
         for (int it = 0; it < 200 && nd > 0 && !fast; ++it) {
             double big = 0.0;
             for (int k = 0; k < nd; ++k) {
@@ -112,6 +113,10 @@ CB_HD_NOINLINE void w_prep_general(double Om, double OL, double Or, double Ow13,
                 big = fmax(big, cx_abs(d) / fmax(cx_abs(r[k]), 1e-300));
             }
             if (big < 4e-16) break;
+            // at rounding level the steps stop shrinking (a root with a close neighbour settles to ~sqrt(eps) steps): stop instead of
+            // spending the remaining sweeps on noise; the coefficient-residual check below still guards the result
+            if (big < 1e-7 && big > 0.25 * prev_big) break;
+            prev_big = big;
         }
         W.deg = n;
         for (int k = 0; k < n; ++k) W.rt[k] = r[k];
@@ -184,6 +189,9 @@ CB_HD_NOINLINE void w_prep_general(double Om, double OL, double Or, double Ow13,
 // (x = rho e^{+-i pi/3}, rho = cbrt(a0/a3)) splits E^2 into the two real quadratics directly; roots by the quadratic formula; no
 // indexed arrays, fast reciprocals.  Anything else (and any doubt: no convergence, both factors with real roots, where the pairing
 // of the four real roots matters) goes to w_prep_general.
+// kDefer (main pass of k_w): anything but the fast structure is only marked ST_INTERNAL_REDO (W then holds E^2 = 1, harmless to
+// evaluate); the kernel lists such elements and its second pass runs them through the general solve.
+template <bool kDefer = false>
 CB_HD void w_prep(double Om, double OL, double Or, double Ow13, double Ow23, double H0, WCosmo& W) {
     const double Ok = 1.0 - Om - OL - Or - Ow13 - Ow23;
     const double a0 = OL, a1 = Ow23, a2 = Ok + Ow13, a3 = Om, a4 = Or;
@@ -213,7 +221,18 @@ CB_HD void w_prep(double Om, double OL, double Or, double Ow13, double Ow23, dou
     const double d1 = q1 * q1 - 4.0 * q2 * q0;                    // disc of q2 x^2 + q1 x + q0 (quartic case)
     // the pairing is forced only if a conjugate pair exists; three or four real roots: general path (pairs real roots with neighbours)
     ok = ok && ((d2 < 0.0) || (quart && d1 < 0.0)) && (quart || q1 != 0.0);
-    if (!ok) { w_prep_general(Om, OL, Or, Ow13, Ow23, H0, W); return; }
+    if (!ok) {
+        if (!kDefer) { w_prep_general(Om, OL, Or, Ow13, Ow23, H0, W); return; }
+        W.f1 = W.g1 = 0.0; W.h1 = 1.0; W.f2 = W.g2 = 0.0; W.h2 = 1.0;
+        W.q11 = W.q21 = 1.0; W.theta = W.sD = W.sDr = 0.0;
+        W.rr[0] = W.rr[1] = W.rr[2] = W.rr[3] = 0.0; W.nreal = 0;
+        W.Ok = 0.0; W.dH = W.tH = 1.0;
+        W.a[0] = 1.0; W.a[1] = W.a[2] = W.a[3] = W.a[4] = 0.0;
+        W.rt[0] = W.rt[1] = W.rt[2] = W.rt[3] = cx_(0.0);
+        W.deg = 0; W.iA = 3;
+        W.status = ST_INTERNAL_REDO;
+        return;
+    }
     W.Ok = Ok;
     { const double iH = cb_rcp(H0); W.dH = C_KM_S * iH; W.tH = HUBBLE_GYR * iH; }
     W.a[0] = a0; W.a[1] = a1; W.a[2] = a2; W.a[3] = a3; W.a[4] = a4;
