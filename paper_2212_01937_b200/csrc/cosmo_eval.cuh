@@ -362,6 +362,46 @@ CB_HD T carlson_Qj(T xa, T mp, T hs, T p) {
     return N::QJ * N::max_(N::max_(N::abs_(A0 - xa), N::abs_(A0 - mp) + hs), N::abs_(A0 - p));
 }
 
+// Direct solve of the moment recurrences of d_abs and of its gradient.  Both are
+//     Om (j + 3/2) v_j + Or (j + SO) v_{j+1} + Ok (j + AO) v_{j-1} + OL (j + CO) v_{j-3} = b_j,     j = 0 .. NR-1,
+// with v_{-1}, v_{-2}, v_{-3} known (km1, km2, km3) and v_NR = 0 (truncation).  Upward substitution is unstable (it divides by
+// Or); the matrix is lower-banded plus ONE small superdiagonal, so one elimination pass downwards leaves the bidiagonal rows
+// v_j + sig_j v_{j+1} = gam_j and one pass back gives every v_j: O(NR) work where the Gauss-Seidel sweeps that this replaces
+// took O(NR^2).  The neglected v_NR changes v_j0 by prod_{j >= j0}(sig_j) v_NR, and |v_NR| <= x |v_{NR-1}| (the moments are
+// integrals of x^j times one positive weight over [1, x]): `trunc` returns that bound.  The pivots follow
+// sig_j ~ Or / (Om - Ok sig_{j-1}), which settles at the small root of Ok sig^2 - Om sig + Or = 0 when Om^2 > 4 Or Ok (always
+// for Ok <= 0) and wanders, with pivots of either sign, when E^2 has no real negative root; `trunc` is infinite unless
+// Om^2 >= 8 Or Ok, and the caller falls back to the closed form.
+template <typename T, int NR, int SO, int AO, int CO, int J0>
+CB_HD void band_solve(T Om, T OL, T Or, T Ok, const T (&b)[NR], T km1, T km2, T km3, T x, T (&v)[NR], T& trunc) {
+    using N = Num<T>;
+    T sig[NR], gam[NR];
+    T P = T(1);
+#pragma unroll
+    for (int j = 0; j < NR; ++j) {
+        const T dj = T(j + 1.5) * Om, sj = T(j + SO) * Or, aj = T(j + AO) * Ok;
+        T f = aj, num = b[j], den = dj;
+        if (j + CO != 0) {
+            const T cj = T(j + CO) * OL;
+            if (j >= 3) {
+                const T e1 = cj * sig[j - 3];
+                f = N::fma_(e1, sig[j - 2], aj);
+                num = N::fma_(e1, gam[j - 2], num);
+            }
+            num = N::fma_(-cj, j >= 3 ? gam[j >= 3 ? j - 3 : 0] : (j == 2 ? km1 : (j == 1 ? km2 : km3)), num);
+        }
+        num = N::fma_(-f, j >= 1 ? gam[j >= 1 ? j - 1 : 0] : km1, num);
+        if (j >= 1) den = N::fma_(-f, sig[j - 1], den);
+        const T pi = N::rcp_(den);
+        sig[j] = pi * sj; gam[j] = pi * num;
+        if (j >= J0) P = P * sig[j];
+    }
+    v[NR - 1] = gam[NR - 1];
+#pragma unroll
+    for (int j = NR - 2; j >= 0; --j) v[j] = N::fma_(-sig[j], v[j + 1], gam[j]);
+    trunc = (Om * Om >= T(8) * Or * Ok) ? N::abs_(P * x * v[NR - 1]) : T(INFINITY);
+}
+
 // S4-S6 for K elements of the SAME cosmology in lock-step (K independent dependency chains per thread: the FP64
 // pipe has ~9 cycles of latency and few warps fit, so instruction-level parallelism is what keeps it busy).
 // kT: lookback integral, kA: absorption integral, kK: the second-kind integral K (needs R_D).
@@ -488,31 +528,18 @@ CB_HD void eval_core_k(const Cosmo<T>& C0, const T (&z)[K], const Vote& vote, Co
                 // The R_D and R_J groups of (3.9) cancel by ~Om/(Or x).  Where radiation is a perturbation
                 // the same Carlson values are assembled without that cancellation: with
                 // u_j = int x^j dx/E, d(x^k E) gives  (k+3/2) Om u_{k+2} = [x^k E] - (k+2) Or u_{k+3} - (k+1) Ok u_{k+1}
-                // - k OL u_{k-1};  u_0 = I0 and u_1 = 2 z B0 + rn I0 are known, the Or terms are iterated (Gauss-Seidel).
+                // - k OL u_{k-1};  u_0 = I0 and u_1 = 2 z B0 + rn I0 are known; the rows k = 0 .. KS are solved directly (band_solve).
                 constexpr int KS = REC_KS;
-                T u[KS + 4], bk[KS + 1];
-                u[0] = R[k].I0;
-                u[1] = N::fma_(T(2) * z[k], B0, C.rn * R[k].I0);
+                T bk[KS + 1], u2[KS + 1], trunc;
+                const T u1 = N::fma_(T(2) * z[k], B0, C.rn * R[k].I0);
                 {
                     T dk = T(0);           // x^j - 1 = x (x^(j-1) - 1) + z: no cancellation at small z
 #pragma unroll
                     for (int j = 0; j <= KS; ++j) { bk[j] = N::fma_(dk, R[k].E, R[k].Em1); dk = N::fma_(x, dk, z[k]); }
-#pragma unroll
-                    for (int j = 2; j < KS + 4; ++j) u[j] = T(0);
                 }
-                T prev = T(0);
-#pragma unroll
-                for (int sw = 0; sw < KS; ++sw) {
-                    if (sw == KS - 1) prev = u[2];
-#pragma unroll
-                    for (int j = 0; j <= KS - sw; ++j) {
-                        T acc = bk[j] - T(j + 2) * C.Or * u[j + 3] - T(j + 1) * C.Ok * u[j + 1];
-                        if (j >= 1) acc -= T(j) * C.OL * u[j - 1];
-                        u[j + 2] = acc * C.iOm * T(1.0 / (j + 1.5));
-                    }
-                }
-                const bool conv = N::abs_(u[2] - prev) <= T(sizeof(T) == 8 ? 1e-14 : 1e-6) * N::abs_(u[2]);
-                R[k].AA = conv ? u[2] : A39;
+                band_solve<T, KS + 1, 2, 1, 0, 0>(C.Om, C.OL, C.Or, C.Ok, bk, u1, R[k].I0, T(0), x, u2, trunc);       // u2[j] = u_{j+2}
+                const bool conv = trunc <= T(sizeof(T) == 8 ? 1e-15 : 1e-7) * N::abs_(u2[0]);
+                R[k].AA = conv ? u2[0] : A39;
             } else {
                 // eq. (B.3) with i = rn
                 R[k].AA = T(CB_KT.two_thirds) * z[k] * (R[k].Em1 * N::rcp_(C.m * z[k]) + C.aF * RF

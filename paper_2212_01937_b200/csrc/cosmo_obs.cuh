@@ -267,8 +267,8 @@ CB_HD void grad_basis(const Cosmo<T>& C, const Rows& rows, T z, const Core<T>& R
         // (the x^5, x^6 rows), which loses Om/Or digits.  Instead J'_p = int x^p dx/E^3, p = 2, 3, 4, come from the basis and
         // J'_5.. follow from d(x^k / E) = N_k / E^3:  Om (k - 3/2) J'_{k+2} = [x^k/E] - k OL J'_{k-1} - (k-1) Ok J'_{k+1}
         // - (k-2) Or J'_{k+3}, the Or terms iterated (same scheme as the forward d_abs).
-        constexpr int KJ = REC_KJ;            // levels k = 3 .. 3 + KJ - 1
-        T Jp[KJ + 5], Sp[7];
+        constexpr int KJ = REC_KJ;            // levels k = 3 .. 3 + KJ - 2, solved directly (band_solve)
+        T Jp[7], Sp[7];
         Jp[0] = Jp[1] = T(0); Sp[0] = Sp[1] = T(0);
 #pragma unroll
         for (int p = 2; p < 5; ++p) {
@@ -277,27 +277,16 @@ CB_HD void grad_basis(const Cosmo<T>& C, const Rows& rows, T z, const Core<T>& R
             Jp[p] = gj[0] * R.I0 + gj[1] * R.K + gj[2] * bt0 + gj[3] * bt1 + gj[4] * bt2;
             Sp[p] = kCond ? asum5(gj) : T(0);
         }
-#pragma unroll
-        for (int p = 5; p < KJ + 5; ++p) Jp[p] = T(0);
-        T bk[KJ];
+        T bk[KJ - 1], vj[KJ - 1], trunc;
         {
             T dk = n3;             // x^k - 1 = x (x^(k-1) - 1) + z, from x^3 - 1: no cancellation at small z
 #pragma unroll
-            for (int j = 0; j < KJ; ++j) { bk[j] = N::fma_(dk, iE, bt0); dk = N::fma_(x, dk, z); }     // x^k/E - 1 = (x^k - 1)/E + (1/E - 1)
+            for (int j = 0; j < KJ - 1; ++j) { bk[j] = N::fma_(dk, iE, bt0); dk = N::fma_(x, dk, z); }     // x^k/E - 1 = (x^k - 1)/E + (1/E - 1)
         }
-        T prev5 = T(0), prev6 = T(0);
-#pragma unroll
-        for (int sw = 0; sw < KJ - 1; ++sw) {
-            if (sw == KJ - 2) { prev5 = Jp[5]; prev6 = Jp[6]; }
-#pragma unroll
-            for (int j = 0; j < KJ - 1 - sw; ++j) {
-                const int k = 3 + j;
-                const T a = bk[j] - T(k) * C.OL * Jp[k - 1] - T(k - 1) * C.Ok * Jp[k + 1] - T(k - 2) * C.Or * Jp[k + 3];
-                Jp[k + 2] = a * C.iOm * T(1.0 / (k - 1.5));
-            }
-        }
-        const T tol = T(sizeof(T) == 8 ? 1e-12 : 1e-5);
-        const bool useJ = N::abs_(Jp[5] - prev5) <= tol * N::abs_(Jp[5]) && N::abs_(Jp[6] - prev6) <= tol * N::abs_(Jp[6]);
+        band_solve<T, KJ - 1, 1, 2, 3, 1>(C.Om, C.OL, C.Or, C.Ok, bk, Jp[4], Jp[3], Jp[2], x, vj, trunc);               // vj[j] = J'_{j+5}
+        Jp[5] = vj[0]; Jp[6] = vj[1];
+        const T tol = T(sizeof(T) == 8 ? 1e-13 : 1e-6);
+        const bool useJ = trunc <= tol * N::abs_(Jp[5]) && trunc <= tol * N::abs_(Jp[6]);
         if (kCond) {      // error bounds of J'_5, J'_6 through the first two levels of the recursion (the Or terms are small where it is used)
             Sp[5] = (N::abs_(bk[0]) + T(3) * C.OL * Sp[2] + T(2) * N::abs_(C.Ok) * Sp[4]) * C.iOm * T(1.0 / 1.5);
             Sp[6] = (N::abs_(bk[1]) + T(4) * C.OL * Sp[3] + T(3) * N::abs_(C.Ok) * Sp[5]) * C.iOm * T(1.0 / 2.5);

@@ -83,24 +83,12 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
             const double A39 = (t1 + t2) + (t3 + t4);
             // radiation-perturbative assembly (see eval_core_k): u_j = int x^j dx/E between the limits
             constexpr int KS = REC_KS;
-            double u[KS + 4], bk[KS + 1];
-            u[0] = I0;
-            u[1] = fma(2.0 * dz, B0, C.rn * I0);
+            double bk[KS + 1], u2[KS + 1], trunc;
+            const double u1 = fma(2.0 * dz, B0, C.rn * I0);
             double xk1 = 1.0, dk = 0.0;      // dk = x2^j - x1^j = x2 (x2^(j-1) - x1^(j-1)) + x1^(j-1) dz: no cancellation as z2 -> z1
             for (int j = 0; j <= KS; ++j) { bk[j] = fma(dk, E2, xk1 * dE); dk = fma(x2, dk, xk1 * dz); xk1 *= x1; }    // x2^j E2 - x1^j E1
-            for (int j = 2; j < KS + 4; ++j) u[j] = 0.0;
-            double prev = 0.0;
-#pragma unroll
-            for (int sw = 0; sw < KS; ++sw) {
-                if (sw == KS - 1) prev = u[2];
-#pragma unroll
-                for (int j = 0; j <= KS - sw; ++j) {
-                    double acc = bk[j] - (j + 2) * C.Or * u[j + 3] - (j + 1) * C.Ok * u[j + 1];
-                    if (j >= 1) acc -= j * C.OL * u[j - 1];
-                    u[j + 2] = acc * C.iOm * (1.0 / (j + 1.5));
-                }
-            }
-            AA = (fabs(u[2] - prev) <= 1e-14 * fabs(u[2])) ? u[2] : A39;
+            band_solve<double, KS + 1, 2, 1, 0, 0>(C.Om, C.OL, C.Or, C.Ok, bk, u1, I0, 0.0, fmax(x1, x2), u2, trunc);    // u2[j] = u_{j+2}
+            AA = (trunc <= 1e-15 * fabs(u2[0])) ? u2[0] : A39;
         } else {                                                                        // eq. (B.3), i = rn
             AA = CB_KT.two_thirds * dz * (dE * cb_rcp(C.m * dz) + C.aF * RF + 2.0 * C.sig * fma(dz2 * CB_KT.third * C.Q2n * C.m, RD, bnd));
             if (dz == 0.0) AA = 0.0;
@@ -118,10 +106,10 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
     if (!with_grad) return;
     // ---- S8: the same bases (GI, GT, GA/GJ) on two-limit basis values; b_k = x2^k/E2 - x1^k/E1
     const double iE1 = cb_rcp(E1), iE2 = cb_rcp(E2), diE = -dE * iE1 * iE2;            // 1/E2 - 1/E1
-    double btv[REC_KJ + 4];
+    double btv[REC_KJ + 2];
     {
         double xk1 = 1.0, dk = 0.0;
-        for (int k = 0; k < REC_KJ + 4; ++k) { btv[k] = fma(dk, iE2, xk1 * diE); dk = fma(x2, dk, xk1 * dz); xk1 *= x1; }
+        for (int k = 0; k < REC_KJ + 2; ++k) { btv[k] = fma(dk, iE2, xk1 * diE); dk = fma(x2, dk, xk1 * dz); xk1 *= x1; }
     }
     // raw gradient integrals int D_theta p_X / E^3 dx between the limits (cosmo_obs.cuh, GradInt) with their cancellation factor
     double rI[3], rT[3], rA[3];
@@ -133,7 +121,7 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
     const double aI0 = fabs(I0), aK = fabs(K), a0 = fabs(btv[0]), a1 = fabs(btv[1]), a2 = fabs(btv[2]);
     auto dot5 = [&](const double* g) { return g[0] * I0 + g[1] * K + g[2] * btv[0] + g[3] * btv[1] + g[4] * btv[2]; };
     auto abs5 = [&](const double* g) { return fabs(g[0]) * aI0 + fabs(g[1]) * aK + fabs(g[2]) * a0 + fabs(g[3]) * a1 + fabs(g[4]) * a2; };
-    double Jp[REC_KJ + 5], Sp[7];
+    double Jp[7], Sp[7];
     bool useJ = false;
     {
         constexpr int KJ = REC_KJ;
@@ -143,19 +131,12 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
             S.rowJ(p, g);
             Jp[p] = dot5(g); Sp[p] = abs5(g);
         }
-        for (int p = 5; p < REC_KJ + 5; ++p) Jp[p] = 0.0;
-        double prev5 = 0.0, prev6 = 0.0;
+        double bj[KJ - 1], vj[KJ - 1], trunc;
 #pragma unroll
-        for (int sw = 0; sw < KJ - 1; ++sw) {
-            if (sw == KJ - 2) { prev5 = Jp[5]; prev6 = Jp[6]; }
-#pragma unroll
-            for (int j = 0; j < KJ - 1 - sw; ++j) {
-                const int k = 3 + j;
-                const double a = btv[k] - k * C.OL * Jp[k - 1] - (k - 1) * C.Ok * Jp[k + 1] - (k - 2) * C.Or * Jp[k + 3];
-                Jp[k + 2] = a * C.iOm * (1.0 / (k - 1.5));
-            }
-        }
-        useJ = fabs(Jp[5] - prev5) <= 1e-12 * fabs(Jp[5]) && fabs(Jp[6] - prev6) <= 1e-12 * fabs(Jp[6]);
+        for (int j = 0; j < KJ - 1; ++j) bj[j] = btv[3 + j];
+        band_solve<double, KJ - 1, 1, 2, 3, 1>(C.Om, C.OL, C.Or, C.Ok, bj, Jp[4], Jp[3], Jp[2], fmax(x1, x2), vj, trunc);    // vj[j] = J'_{j+5}
+        Jp[5] = vj[0]; Jp[6] = vj[1];
+        useJ = trunc <= 1e-13 * fabs(Jp[5]) && trunc <= 1e-13 * fabs(Jp[6]);
         Sp[5] = (fabs(btv[3]) + 3.0 * C.OL * Sp[2] + 2.0 * fabs(C.Ok) * Sp[4]) * C.iOm / 1.5;
         Sp[6] = (fabs(btv[4]) + 4.0 * C.OL * Sp[3] + 3.0 * fabs(C.Ok) * Sp[5]) * C.iOm / 2.5;
     }

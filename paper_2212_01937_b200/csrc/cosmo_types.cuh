@@ -104,9 +104,10 @@ enum : unsigned { ST_ROOT_ON_PATH = 1, ST_UNSUPPORTED = 2, ST_DL_NONPOS = 4, ST_
 constexpr double GRAD_COND_LIMIT = 1.0e6;
 constexpr double GRAD_COND_LIMIT_F32 = 30.0;
 
-// depth of the perturbative d_abs recursions: REC_KS Gauss-Seidel sweeps for the value, REC_KJ - 1 for the
-// gradient's J'_5, J'_6.  A sweep gains a factor ~ (Or/Om) x; where that is too slow for the depth the direct forms take over (eq. (3.9),
-// whose cancellation Om/(Or x) is then mild; the exact gradient basis, guarded by the cancellation check).
+// depth of the perturbative d_abs recursions: rows k = 0 .. REC_KS of the moment recurrence for the value,
+// k = 3 .. REC_KJ + 1 for the gradient's J'_5, J'_6, each solved directly (cosmo_eval.cuh, band_solve).  The truncation costs
+// ~ ((Or/Om) x)^depth; where that exceeds the tolerance the direct forms take over (eq. (3.9), whose cancellation Om/(Or x) is then
+// mild; the exact gradient basis, guarded by the cancellation check).
 #ifndef CB_REC_KS
 #define CB_REC_KS 8
 #endif
