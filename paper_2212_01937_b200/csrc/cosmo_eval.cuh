@@ -45,7 +45,8 @@ template <> struct Num<double> {
     static CB_HD void sincos_(double a, double* s, double* c) { *s = sin(a); *c = cos(a); }
     static CB_HD double fma_(double a, double b, double c) { return fma(a, b, c); }
     static CB_HD double abs_(double a) { return fabs(a); }
-    static CB_HD double max_(double a, double b) { return fmax(a, b); }
+    // the larger of two magnitudes; a NaN in b is ignored, one in a is returned (fmax() compiles to eight instructions here)
+    static CB_HD double max_(double a, double b) { return b > a ? b : a; }
     // Branch-free reciprocal square root / reciprocal: MUFU seed (2^-20, measured) + one cubic step (error ~ 2^-58).
     // No special-case handling: arguments on the hot path are positive, finite and far from the subnormal range.
     static CB_HD double rsqrt_(double a) {
@@ -142,7 +143,7 @@ template <> struct Num<float> {
     static CB_HD void sincos_(float a, float* s, float* c) { *s = sinf(a); *c = cosf(a); }
     static CB_HD float fma_(float a, float b, float c) { return fmaf(a, b, c); }
     static CB_HD float abs_(float a) { return fabsf(a); }
-    static CB_HD float max_(float a, float b) { return fmaxf(a, b); }
+    static CB_HD float max_(float a, float b) { return b > a ? b : a; }
     static CB_HD float rsqrt_(float a) {
 #ifdef __CUDA_ARCH__
         return rsqrtf(a);

@@ -395,24 +395,24 @@ __global__ void __launch_bounds__(CB_ELEM_BLOCK, kG ? CB_ELEM_MINB_G : CB_ELEM_M
     const T* __restrict__ gout = static_cast<const T*>(a.gout);
     T g[N_PLANES], v[N_PLANES];
     if (kG) {
-        int pl = 0;
+        const T* __restrict__ gpl = gout + ii;               // the present planes follow one another, N apart
+#pragma unroll
         for (int w = 0; w < N_PLANES; ++w) {
-            g[w] = T(0);
-            if (!(which >> w & 1)) continue;
-            g[w] = gout[(int64_t)pl * N + ii];
-            ++pl;
+            const bool on = which >> w & 1;
+            g[w] = on ? *gpl : T(0);
+            gpl += on ? N : 0;
         }
     }
     T dz = T(0), gp[4] = {T(0), T(0), T(0), T(0)};
     const unsigned st = elem_one<T, kT, kA, kG, VoteWarp, true, kAge>(static_cast<const T*>(a.z)[ii], a.Om[ii], a.OL[ii], a.Or[ii], a.H0[ii], which,
                                                                 VoteWarp(), g, v, dz, gp);
     if (live && a.out != nullptr) {
-        T* __restrict__ out = static_cast<T*>(a.out);
-        int pl = 0;
+        T* __restrict__ opl = static_cast<T*>(a.out) + i;
+#pragma unroll
         for (int w = 0; w < N_PLANES; ++w) {
-            if (!(which >> w & 1)) continue;
-            out[(int64_t)pl * N + i] = v[w];
-            ++pl;
+            const bool on = which >> w & 1;
+            if (on) *opl = v[w];
+            opl += on ? N : 0;
         }
     }
     if (live && a.status != nullptr) a.status[i] = (uint8_t)(st & ~(unsigned)ST_INTERNAL_REDO);
