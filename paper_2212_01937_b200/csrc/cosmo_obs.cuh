@@ -549,8 +549,16 @@ CB_HD void backward(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, c
 // kDefer: do not run the quadrature here; return ST_INTERNAL_REDO for an element that needs it (the ELEMENTWISE kernels collect
 // those few per cent of elements and a second, dense pass redoes them: a divergent call inside the main kernel costs it a third
 // of its time, measured).
-template <typename T, bool kT, bool kA, bool kSolve = false, bool kDefer = false>
-CB_HD unsigned backward_robust(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, const T g[N_PLANES], T& gz, T gp[4],
+// (G: the upstream gradients as an array, or an IO object whose get_grads() fetches them only now -- elem_one_io)
+template <typename T>
+CB_HD void fetch_grads(const T* g, T (&go)[N_PLANES]) {
+#pragma unroll
+    for (int w = 0; w < N_PLANES; ++w) go[w] = g[w];
+}
+template <typename T, typename IO>
+CB_HD void fetch_grads(const IO& io, T (&go)[N_PLANES]) { io.get_grads(go); }
+template <typename T, bool kT, bool kA, bool kSolve = false, bool kDefer = false, typename G = const T*>
+CB_HD unsigned backward_robust(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, const G& gsrc, T& gz, T gp[4],
                                unsigned which = W_ALL) {
     GradInt<T> D;
     T cond = T(0);
@@ -578,6 +586,8 @@ CB_HD unsigned backward_robust(const Cosmo<T>& C, T z, const Core<T>& R, const O
             st = grad_robust_fix<T>(C, z, kT && (which & (W_TL | W_AGE)), kA && (which & W_DABS), singular ? T(INFINITY) : cond, D);
         }
     }
+    T g[N_PLANES];
+    fetch_grads<T>(gsrc, g);
     backward_chain<T, kT, kA>(C, z, R, O, D, g, gz, gp, which);
     return st;
 }
@@ -589,8 +599,23 @@ CB_HD unsigned backward_robust(const Cosmo<T>& C, T z, const Core<T>& R, const O
 // kDefer: the main pass of the ELEMENTWISE kernels -- elements that need a slow path (complex root structure, ill-conditioned
 // gradient bases: backward_robust) are only marked ST_INTERNAL_REDO; the second pass runs them again without kDefer.
 // kAge: the age plane may be asked for (its T_inf costs a second pass of eq. (3.8) per element: kept out of the other instantiations)
-template <typename T, bool kT, bool kA, bool kG, typename Vote, bool kDefer = false, bool kAge = true>
-CB_HD unsigned elem_one(T zv, double Om, double OL, double Or, double H0, unsigned which, const Vote& vote, const T* g, T* v, T& dz, T gp[4]) {
+// IO: where the values go and the upstream gradients come from.  put_values() is called as soon as the observables exist and
+// get_grads() only when the backward chain needs them, so that in the kernel neither set occupies registers through the other
+// half of the element (ArrayIO: plain arrays, for the second pass and the host checks).
+template <typename T>
+struct ArrayIO {
+    const T* g; T* v;
+    CB_HD void put_values(const T (&o)[N_PLANES]) const {
+#pragma unroll
+        for (int w = 0; w < N_PLANES; ++w) v[w] = o[w];
+    }
+    CB_HD void get_grads(T (&go)[N_PLANES]) const {
+#pragma unroll
+        for (int w = 0; w < N_PLANES; ++w) go[w] = g[w];
+    }
+};
+template <typename T, bool kT, bool kA, bool kG, typename Vote, bool kDefer = false, bool kAge = true, typename IO = ArrayIO<T>>
+CB_HD unsigned elem_one_io(T zv, double Om, double OL, double Or, double H0, unsigned which, const Vote& vote, const IO& io, T& dz, T gp[4]) {
     Cosmo<T> C0{}, C{};
     {
         Cosmo<double> Cd{};
@@ -609,8 +634,7 @@ CB_HD unsigned elem_one(T zv, double Om, double OL, double Or, double H0, unsign
     else apply_c4<T, kT, kA, kG>(C, zv, R);
     Obs<T> O;
     observables<T, kT, kA>(C, zv, R, which, O);
-#pragma unroll
-    for (int w = 0; w < N_PLANES; ++w) v[w] = O.v[w];
+    io.put_values(O.v);
     unsigned st = O.status | redo;
     if (kG) {
         dz = T(0); gp[0] = gp[1] = gp[2] = gp[3] = T(0);
@@ -627,23 +651,34 @@ CB_HD unsigned elem_one(T zv, double Om, double OL, double Or, double H0, unsign
             // even hold the pair's gap): such elements are evaluated by the FP64 path, values included (second pass of the kernel when kDefer)
             if (peaked && kDefer) st |= ST_INTERNAL_REDO;
             if (peaked && !kDefer) {
+                T g[N_PLANES], v[N_PLANES];
+                io.get_grads(g);
                 double gd[N_PLANES], vd[N_PLANES], dzd = 0.0, gpd[4] = {0.0, 0.0, 0.0, 0.0};
 #pragma unroll
                 for (int w = 0; w < N_PLANES; ++w) gd[w] = (double)g[w];
-                st = elem_one<double, kT, kA, kG, VoteNone, false, kAge>((double)zv, Om, OL, Or, H0, which, VoteNone(), gd, vd, dzd, gpd);
+                const ArrayIO<double> iod{gd, vd};
+                st = elem_one_io<double, kT, kA, kG, VoteNone, false, kAge, ArrayIO<double>>((double)zv, Om, OL, Or, H0, which, VoteNone(), iod, dzd, gpd);
 #pragma unroll
                 for (int w = 0; w < N_PLANES; ++w) v[w] = (T)vd[w];
+                io.put_values(v);
                 dz = (T)dzd;
 #pragma unroll
                 for (int j = 0; j < 4; ++j) gp[j] = (T)gpd[j];
             } else {
+                T g[N_PLANES];
+                io.get_grads(g);
                 backward_chain<T, kT, kA>(C, zv, R, O, D, g, dz, gp, which);
             }
         } else {
-            st |= backward_robust<T, kT, kA, true, kDefer>(C, zv, R, O, g, dz, gp, which);
+            st |= backward_robust<T, kT, kA, true, kDefer, IO>(C, zv, R, O, io, dz, gp, which);
         }
     }
     return st;
+}
+template <typename T, bool kT, bool kA, bool kG, typename Vote, bool kDefer = false, bool kAge = true>
+CB_HD unsigned elem_one(T zv, double Om, double OL, double Or, double H0, unsigned which, const Vote& vote, const T* g, T* v, T& dz, T gp[4]) {
+    const ArrayIO<T> io{g, v};
+    return elem_one_io<T, kT, kA, kG, Vote, kDefer, kAge>(zv, Om, OL, Or, H0, which, vote, io, dz, gp);
 }
 
 }  // namespace cb
