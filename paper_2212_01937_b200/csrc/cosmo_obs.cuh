@@ -102,6 +102,13 @@ CB_HD void observables_k(const Cosmo<T>& C, const T (&z)[K], const Core<T> (&R)[
             sinn_poly<T, 7>(C.Ok * I0[k] * I0[k], sf, sg, sd);
             O[k].F = I0[k] * sf; O[k].Fi = sg; O[k].Fk = I0[k] * I0[k] * I0[k] * sd;
         }
+    } else if (wmax <= T(1)) {                 // same straight-line form at degree 10 (next term 1/23! ~ 4e-23)
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            T sf, sg, sd;
+            sinn_poly<T, 10>(C.Ok * I0[k] * I0[k], sf, sg, sd);
+            O[k].F = I0[k] * sf; O[k].Fi = sg; O[k].Fk = I0[k] * I0[k] * I0[k] * sd;
+        }
     } else {
         for (int k = 0; k < K; ++k) sinn<T>(C.Ok, I0[k], O[k].F, O[k].Fi, O[k].Fk);
     }
