@@ -335,7 +335,7 @@ def run_ours(args):
             e2e_s = float(tt.item())
         e2e = {"value": evals * world / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                "ms_per_step": e2e_s * 1e3,
-               "api": "cosmo_eval_host (pinned host buffers, chunked over two streams)" if cfg != 4 else
+               "api": "cosmo_eval_host (pinned host buffers, chunked over three streams)" if cfg != 4 else
                       "pinned torch copies around cosmo_snia_loglike (the call has no host-buffer twin)"}
 
     # ---- ALU roofline: FMA peak of the arithmetic type measured live with the library's probe, kernel time from CUDA events on its stream

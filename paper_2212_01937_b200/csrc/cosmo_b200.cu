@@ -239,13 +239,14 @@ int run_joint(const T* z, const T* z_obs, const T* mu_obs, const T* sigma_mu, do
 }
 
 // staging of the host-buffer call cosmo_eval_host: device scratch (grow-only until cosmo_host_release), a pinned block for the per-chunk
-// parameter sums, two streams and one event
+// parameter sums, HOST_SETS streams and one event
+constexpr int HOST_SETS = 3;
 std::mutex g_host_mu;
 void* g_host_buf = nullptr;
 size_t g_host_cap = 0;
 void* g_host_pin = nullptr;
 size_t g_host_pin_cap = 0;
-cudaStream_t g_host_streams[2] = {nullptr, nullptr};
+cudaStream_t g_host_streams[HOST_SETS] = {};
 cudaEvent_t g_host_ev = nullptr;
 
 }  // namespace
@@ -293,9 +294,11 @@ int cosmo_snia_loglike_f32(const float* z, const float* mu_obs, const float* sig
     return run_snia<float>(z, mu_obs, sigma, N, p, S, logL, grad, workspace, ws_bytes, stream);
 }
 
-// Host-buffer call: the redshift axis is cut into chunks that travel through two streams with two sets of device staging buffers, so
-// that the H2D copy of chunk i+1, the kernels of chunk i and the D2H copy of chunk i-1 overlap (PCIe is full duplex; the path is
-// PCIe-bound: 8 B of grad_out per eval against ~20 ps of kernel time).  Pinned host memory is needed for the overlap; pageable
+// Host-buffer call: the redshift axis is cut into chunks that travel through three streams with three sets of device staging buffers,
+// so that the H2D copy of chunk i+1, the kernels of chunk i and the D2H copy of chunk i-1 overlap (PCIe is full duplex; the path is
+// PCIe-bound: 8 B of grad_out per eval against ~20 ps of kernel time).  Three sets, not two: with two, the H2D copy of chunk i+2 waits
+// in its stream behind the D2H copy of chunk i, and where as much comes back as goes in (per-element cosmologies with the VJP:
+// 88 B each way per element) the two directions then run one after the other instead of together.  Pinned host memory is needed for the overlap; pageable
 // memory still gives the right result.  Per-chunk parameter-gradient sums are added on the host in chunk order (deterministic).
 int cosmo_eval_host(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosmo, int mode, uint32_t which,
                     const double* grad_out, double* out, double* grad_z, double* grad_params, uint8_t* status) {
@@ -309,12 +312,18 @@ int cosmo_eval_host(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosm
     const int64_t rows = outer ? n_cosmo : 1;
     const int np = __builtin_popcount(which);
     const int64_t n_par = per_elem ? 0 : n_cosmo;             // parameters copied once (shared) or chunked with z (per element)
-    // chunk length: ~32 MB of the widest per-redshift stream, at least 64 Ki redshifts, even (128-bit accesses), at most 64 chunks
+    // chunk length: ~32 MB of traffic per chunk (COSMO_HOST_CHUNK_MB), at least 64 Ki redshifts, even (128-bit accesses); a job of more
+    // than 16 such chunks is cut into 16, up to 256 MB each: every copy call costs ~10 us of set-up, which at 32 MB was a quarter of
+    // the time of a per-element VJP call (10 copies per chunk; measured 26.9 -> 22.6 ms on config 5)
     const int64_t bytes_per_z = (int64_t)sizeof(double) * ((int64_t)np * rows * ((with_grad ? 1 : 0) + (out ? 1 : 0)) + 2 + (per_elem ? 8 : 0)) + rows;
     static const int64_t chunk_mb = []() { const char* e = getenv("COSMO_HOST_CHUNK_MB"); const long v = e ? atol(e) : 0; return (int64_t)(v > 0 ? v : 32); }();
     int64_t nc = (chunk_mb << 20) / bytes_per_z;
     if (nc < 65536) nc = 65536;
-    if (nc * 64 < n_z) nc = cdiv(n_z, 64);
+    if (nc * 16 < n_z) {
+        const int64_t nmax = (int64_t(256) << 20) / bytes_per_z;
+        nc = cdiv(n_z, 16);
+        if (nc > nmax && nmax >= 65536) nc = nmax;
+    }
     nc = (nc + 1) & ~int64_t(1);
     if (nc > n_z) nc = n_z;
     const int64_t nchunks = cdiv(n_z, nc);
@@ -324,10 +333,10 @@ int cosmo_eval_host(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosm
     const size_t b_ws = align256(cosmo_workspace_bytes(nc, per_elem ? nc : n_cosmo, mode, which, with_grad));
     const size_t per_set = b_z + 4 * b_pc + (out ? b_pl : 0) + (with_grad ? b_pl + b_z + b_gp : 0) + (status ? b_st : 0) + b_ws;
     const size_t b_par = align256(sizeof(double) * (n_par > 0 ? n_par : 1));
-    const size_t total = 4 * b_par + 2 * per_set;
+    const size_t total = 4 * b_par + HOST_SETS * per_set;
     std::lock_guard<std::mutex> lk(g_host_mu);
     if (!g_host_streams[0]) {
-        for (int i = 0; i < 2; ++i)
+        for (int i = 0; i < HOST_SETS; ++i)
             if (cudaStreamCreateWithFlags(&g_host_streams[i], cudaStreamNonBlocking) != cudaSuccess) { g_last_cuda = (int)cudaGetLastError(); return COSMO_E_CUDA; }
         if (cudaEventCreateWithFlags(&g_host_ev, cudaEventDisableTiming) != cudaSuccess) { g_last_cuda = (int)cudaGetLastError(); return COSMO_E_CUDA; }
     }
@@ -350,8 +359,8 @@ int cosmo_eval_host(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosm
     auto take = [&](size_t b) { char* q = base + off; off += b; return q; };
     double* d_par[4];
     for (int i = 0; i < 4; ++i) d_par[i] = (double*)take(b_par);
-    struct Set { double *z, *pc[4], *out, *gout, *gz, *gp; uint8_t* st; void* ws; } S[2];
-    for (int k = 0; k < 2; ++k) {
+    struct Set { double *z, *pc[4], *out, *gout, *gz, *gp; uint8_t* st; void* ws; } S[HOST_SETS];
+    for (int k = 0; k < HOST_SETS; ++k) {
         S[k].z = (double*)take(b_z);
         for (int i = 0; i < 4; ++i) S[k].pc[i] = per_elem ? (double*)take(b_pc) : d_par[i];
         S[k].out = out ? (double*)take(b_pl) : nullptr;
@@ -362,17 +371,17 @@ int cosmo_eval_host(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosm
         S[k].ws = take(b_ws);
     }
     const double* hp[4] = {p.Om, p.OL, p.Or, p.H0};
-    cudaStream_t s0 = g_host_streams[0], s1 = g_host_streams[1];
+    cudaStream_t s0 = g_host_streams[0];
     if (!per_elem) {
         for (int i = 0; i < 4; ++i) cudaMemcpyAsync(d_par[i], hp[i], sizeof(double) * n_cosmo, cudaMemcpyHostToDevice, s0);
         cudaEventRecord(g_host_ev, s0);
-        cudaStreamWaitEvent(s1, g_host_ev, 0);
+        for (int k = 1; k < HOST_SETS; ++k) cudaStreamWaitEvent(g_host_streams[k], g_host_ev, 0);
     }
     const size_t hpitch = sizeof(double) * n_z;               // host planes [np][rows][n_z]: row pitch n_z
     double* hsum = static_cast<double*>(g_host_pin);
     for (int64_t c = 0; c < nchunks && rc == COSMO_OK; ++c) {
-        const int k = (int)(c & 1);
-        cudaStream_t st = k ? s1 : s0;
+        const int k = (int)(c % HOST_SETS);
+        cudaStream_t st = g_host_streams[k];
         const int64_t n0 = c * nc, n = (n0 + nc <= n_z) ? nc : (n_z - n0);
         cudaMemcpyAsync(S[k].z, z + n0, sizeof(double) * n, cudaMemcpyHostToDevice, st);
         if (per_elem)
@@ -392,9 +401,10 @@ int cosmo_eval_host(const double* z, int64_t n_z, cosmo_params p, int64_t n_cosm
             else cudaMemcpyAsync(hsum + c * 4 * n_cosmo, S[k].gp, sizeof(double) * 4 * n_cosmo, cudaMemcpyDeviceToHost, st);
         }
     }
-    cudaError_t e0 = cudaStreamSynchronize(s0), e1 = cudaStreamSynchronize(s1);
+    cudaError_t es = cudaSuccess;
+    for (int k = 0; k < HOST_SETS; ++k) { const cudaError_t e = cudaStreamSynchronize(g_host_streams[k]); if (es == cudaSuccess) es = e; }
     if (rc) return rc;
-    if (e0 != cudaSuccess || e1 != cudaSuccess) { g_last_cuda = (int)(e0 != cudaSuccess ? e0 : e1); return COSMO_E_CUDA; }
+    if (es != cudaSuccess) { g_last_cuda = (int)es; return COSMO_E_CUDA; }
     if (with_grad && !per_elem) {
         for (int64_t i = 0; i < 4 * n_cosmo; ++i) {
             double v = 0.0;
