@@ -118,3 +118,25 @@ extern "C" void hostcheck_w_full(int64_t n, const double* z, const double* Om, c
         }
     }
 }
+
+// the curvature transform on its own (cosmo_eval.cuh, sinn): F = I0 S(w), Fi = C(w), Fk = I0^3 S'(w), w = k I0^2
+extern "C" void hostcheck_sinn(int64_t n, const double* k, const double* I0, double* F, double* Fi, double* Fk) {
+    for (int64_t i = 0; i < n; ++i) sinn<double>(k[i], I0[i], F[i], Fi[i], Fk[i]);
+}
+
+// the banded solve of the d_abs moment recurrences on its own (cosmo_eval.cuh, band_solve), in the two shapes the path uses:
+// shape 0: value (rows k = 0..8: SO, AO, CO = 2, 1, 0), shape 1: gradient (rows k = 3..13: 1, 2, 3; error bound from row 1 on)
+extern "C" void hostcheck_band(int shape, double Om, double OL, double Or, double Ok, const double* b, double km1, double km2, double km3,
+                               double x, double* v, double* trunc) {
+    if (shape == 0) {
+        double bb[REC_KS + 1], vv[REC_KS + 1];
+        for (int j = 0; j <= REC_KS; ++j) bb[j] = b[j];
+        band_solve<double, REC_KS + 1, 2, 1, 0, 0>(Om, OL, Or, Ok, bb, km1, km2, km3, x, vv, *trunc);
+        for (int j = 0; j <= REC_KS; ++j) v[j] = vv[j];
+    } else {
+        double bb[REC_KJ - 1], vv[REC_KJ - 1];
+        for (int j = 0; j < REC_KJ - 1; ++j) bb[j] = b[j];
+        band_solve<double, REC_KJ - 1, 1, 2, 3, 1>(Om, OL, Or, Ok, bb, km1, km2, km3, x, vv, *trunc);
+        for (int j = 0; j < REC_KJ - 1; ++j) v[j] = vv[j];
+    }
+}

@@ -412,3 +412,78 @@ def test_binding_refuses_cpu():
     z = torch.zeros(4, dtype=torch.float64)
     with pytest.raises(binding.CosmoError):
         binding.cosmo_eval(z, z, z, z, z)
+
+
+def test_sinn_quartering_against_mpmath(hc):
+    """cosmo_eval.cuh sinn(): S = sin(sqrt(-w))/sqrt(-w) (sinh for w > 0), C = cos / cosh, S' = (C - S)/(2w), by the degree-7 series on the
+    quartered argument and the doubling steps back -- against 40-digit values over closed models up to the antipode (w = -pi^2), open
+    ones up to w = 200, the series range, zero and the switch points between m and m + 1 quarterings"""
+    import mpmath as mp
+    mp.mp.dps = 40
+    rng = np.random.default_rng(11)
+    w = np.concatenate([rng.uniform(-9.8, 0, 300), rng.uniform(0, 200, 300), rng.uniform(-0.5, 0.5, 100), -np.pi ** 2 + 10.0 ** rng.uniform(-8, 0, 50),
+                        [0.0, 0.5, -0.5, np.nextafter(0.5, 1), 2.0, np.nextafter(2.0, 3), -2.0, 8.0, np.nextafter(8.0, 9), 1e-300, -1e-12]])
+    I0 = rng.uniform(0.05, 3.0, w.size)
+    k = w / I0 ** 2
+    F, Fi, Fk = np.zeros_like(w), np.zeros_like(w), np.zeros_like(w)
+    hc.hostcheck_sinn(C.c_int64(w.size), k.ctypes.data_as(DP), I0.ctypes.data_as(DP), F.ctypes.data_as(DP), Fi.ctypes.data_as(DP), Fk.ctypes.data_as(DP))
+    for i in range(w.size):
+        ww = mp.mpf(float(k[i])) * mp.mpf(float(I0[i])) ** 2
+        if ww < 0:
+            y = mp.sqrt(-ww); S, Cc = mp.sin(y) / y, mp.cos(y)
+        elif ww > 0:
+            y = mp.sqrt(ww); S, Cc = mp.sinh(y) / y, mp.cosh(y)
+        else:
+            S, Cc = mp.mpf(1), mp.mpf(1)
+        Sd = (Cc - S) / (2 * ww) if abs(ww) > 1e-6 else mp.mpf(1) / 6 + ww / 60
+        # S -> 0 at the antipode: the error is absolute there (it is the rounding of w that decides, |dS/dw| = 1/2 pi^2)
+        assert abs(F[i] / I0[i] - S) <= 4e-15 * max(1.0, abs(S)), (w[i], float(S))
+        assert abs(Fi[i] - Cc) <= 4e-15 * max(1.0, abs(Cc)), (w[i], float(Cc))
+        assert abs(Fk[i] / I0[i] ** 3 - Sd) <= 2e-14 * max(abs(Sd), 0.05), (w[i], float(Sd))
+    # not-a-number and infinite arguments stay what they are
+    kk = np.array([np.nan, 1e300, 1.0]); ii = np.array([1.0, 1e10, np.nan]); o = [np.zeros(3) for _ in range(3)]
+    hc.hostcheck_sinn(C.c_int64(3), kk.ctypes.data_as(DP), ii.ctypes.data_as(DP), *[a.ctypes.data_as(DP) for a in o])
+    assert not np.isfinite(o[0]).any()
+
+
+def test_band_solve_against_moments(hc):
+    """cosmo_eval.cuh band_solve(): the truncated moment recurrences of d_abs against the moments themselves by quadrature --
+    value shape: u_j = int_1^x t^j dt/E from u_0, u_1 and b_k = [t^k E]; gradient shape: J'_p = int t^p dt/E^3 from J'_2..J'_4 and
+    b_k = [t^k/E].  The returned bound has to cover the truncation error wherever that is visible; outside Om^2 >= 8 Or Ok it is infinite"""
+    from scipy.integrate import quad
+    rng = np.random.default_rng(5)
+    seen_trunc = 0
+    for it in range(60):
+        if it < 30:      # radiation as a perturbation: the truncation is far below rounding
+            Om, OL, Or = rng.uniform(0.05, 1.0), rng.uniform(0, 1.2), 10.0 ** rng.uniform(-6, -3.5)
+        else:            # radiation large enough for the truncation to show, so that the bound is really tested
+            Om, OL, Or = rng.uniform(0.5, 1.0), rng.uniform(0.3, 0.9), 10.0 ** rng.uniform(-1.8, -1.0)
+        Ok = 1 - Om - OL - Or
+        x = rng.uniform(1.05, 3.5)
+        E = lambda t: np.sqrt(Or * t ** 4 + Om * t ** 3 + Ok * t ** 2 + OL)
+        for shape, NR in ((0, 9), (1, 11)):
+            if shape == 0:
+                mom = [quad(lambda t: t ** j / E(t), 1, x, epsabs=0, epsrel=1e-13)[0] for j in range(NR + 2)]
+                b = np.array([x ** k * E(x) - E(1.0) for k in range(NR)])
+                km, truth, j0 = (mom[1], mom[0], 0.0), np.array(mom[2:NR + 2]), 0
+            else:
+                mom = [quad(lambda t: t ** p / E(t) ** 3, 1, x, epsabs=0, epsrel=1e-13)[0] for p in range(NR + 5)]
+                b = np.array([x ** k / E(x) - 1.0 / E(1.0) for k in range(3, NR + 3)])
+                km, truth, j0 = (mom[4], mom[3], mom[2]), np.array(mom[5:NR + 5]), 1
+            v = np.zeros(NR); tr = C.c_double()
+            hc.hostcheck_band(shape, C.c_double(Om), C.c_double(OL), C.c_double(Or), C.c_double(Ok), b.ctypes.data_as(DP), C.c_double(km[0]),
+                              C.c_double(km[1]), C.c_double(km[2]), C.c_double(x), v.ctypes.data_as(DP), C.byref(tr))
+            err = abs(v[j0] - truth[j0])
+            if Om * Om >= 8 * Or * Ok:
+                assert err <= 1.001 * tr.value + 2e-12 * abs(truth[j0]), (shape, Om, OL, Or, x, err, tr.value)
+                seen_trunc += err > 1e-10 * abs(truth[j0])
+                if it < 30:
+                    assert err <= 2e-12 * abs(truth[j0]) and tr.value <= 1e-15 * abs(truth[j0])
+            else:
+                assert np.isinf(tr.value)
+    assert seen_trunc >= 10        # the bound was exercised where the truncation is visible
+    # no real negative root (Om^2 < 4 Or Ok): refused
+    v = np.zeros(9); tr = C.c_double(); b = np.ones(10)
+    hc.hostcheck_band(0, C.c_double(0.05), C.c_double(0.0), C.c_double(1e-3), C.c_double(0.949), b.ctypes.data_as(DP), C.c_double(1.0), C.c_double(1.0),
+                      C.c_double(0.0), C.c_double(2.0), v.ctypes.data_as(DP), C.byref(tr))
+    assert np.isinf(tr.value)
