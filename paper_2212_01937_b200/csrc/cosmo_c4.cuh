@@ -120,11 +120,11 @@ CB_HD void c4_carlson(double x, double y, double z, cx p, bool want_j, C4Carlson
 
 // I0, T, A of eqs. (3.7)-(3.9) with the roots r_1 = conj(r_2) of Q1 = Or x^2 + g1 x + h1 and r_3 = conj(r_4) of
 // Q2 = x^2 + b x + c, permutation (i, j, k, l) = (1, 2, 3, 4); everything in x = 1 + z (d_i5 = -rho_i), between the limits
-// x1 = 1 + z1 and x = 1 + z2 (the hot path calls it with x1 = 1).
+// x1 = 1 + z1 and x = 1 + z2 (the hot path calls it with x1 = 1).  dz = z2 - z1 comes in from the caller: formed as x - x1 it
+// would carry the rounding of 1 + z, eps/z of every result at small z (3.7e-11 at z = 1e-6 before this was an argument).
 // (never inlined: a rare path must not cost the hot kernels registers)
-CB_HD_NOINLINE void eval_c4(double Or, double g1, double h1, double b, double c, double x1, double x, bool want_T, bool want_A,
+CB_HD_NOINLINE void eval_c4(double Or, double g1, double h1, double b, double c, double x1, double x, double dz, bool want_T, bool want_A,
                    double& I0, double& TT, double& AA, double& KK) {
-    const double dz = x - x1;
     const double D1 = 4.0 * Or * h1 - g1 * g1, D2 = 4.0 * c - b * b;       // both > 0 here
     const cx r1 = cx_(-g1 / (2.0 * Or), sqrt(D1) / (2.0 * Or)), r2 = cx_conj(r1);
     const cx r3 = cx_(-0.5 * b, 0.5 * sqrt(D2)), r4 = cx_conj(r3);
@@ -156,7 +156,17 @@ CB_HD_NOINLINE void eval_c4(double Or, double g1, double h1, double b, double c,
         c4_carlson(ya, za, xa, p0, true, K0);
         const cx q0 = p0 / ((cx_(x1) - r1) * (cx_(x) - r1));
         const cx s0 = q0 + cx_(dz * dz);
-        const cx bnd = X1 * X3 * X4 / X2 - Y1 * Y3 * Y4 / Y2;
+        // boundary term [F] between the limits, F = X1 X3 X4 / X2, F^2 = N(x)/(x - r2), N = (x - r1) Q2.  Close limits: the difference
+        // through F^2, with the factor dz taken out of N(x)(x1 - r2) - N(x1)(x - r2) = dz ([N; x, x1] (x1 - r2) - N(x1)) analytically
+        // (subtracted directly it loses eps/dz: 2e-10 of d_abs at z = 1e-4)
+        const cx Fx = X1 * X3 * X4 / X2, F1 = Y1 * Y3 * Y4 / Y2;
+        cx bnd = Fx - F1;
+        if (fabs(dz) <= 0.05 * fmin(x, x1)) {
+            const cx br1 = cx_(b) - r1, cr1 = cx_(c) - b * r1;                              // N = x^3 + br1 x^2 + cr1 x - c r1
+            const cx dd = cx_(x * x + x * x1 + x1 * x1) + (x + x1) * br1 + cr1;             // divided difference [N; x, x1]
+            const cx N1 = (x1 * x1 + b * x1 + c) * (cx_(x1) - r1);
+            bnd = dz * ((dd * (cx_(x1) - r2) - N1) / ((cx_(x) - r2) * (cx_(x1) - r2) * (Fx + F1)));
+        }
         const cx sig = r1 + r2 + r3 + r4;
         const cx t2 = dz * ((2.0 * (r1 * r1) - d13 * d14) * cx_(K0.RF));
         const cx t3 = dz * ((d23 * d24) * (((dz * dz / 3.0) * (d13 * d14)) * cx_(K0.RDz) + (X1 * Y1) / (X2 * Y2 * u12)));

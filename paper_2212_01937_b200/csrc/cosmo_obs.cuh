@@ -25,7 +25,7 @@ template <typename T, bool kT, bool kA, bool kGrad>
 CB_HD void apply_c4(const Cosmo<T>& C, T z, Core<T>& R) {
     if (!(C.cubic & 2u)) return;
     double I0, TT, AA, KK;
-    eval_c4((double)C.Or, (double)C.m, (double)C.rn, (double)C.b, (double)C.c, 1.0, 1.0 + (double)z, kT, kA, I0, TT, AA, KK);
+    eval_c4((double)C.Or, (double)C.m, (double)C.rn, (double)C.b, (double)C.c, 1.0, 1.0 + (double)z, (double)z, kT, kA, I0, TT, AA, KK);
     R.I0 = (T)I0; R.TT = (T)TT; R.AA = (T)AA; R.K = (T)KK;
     {
         const double x = 1.0 + (double)z, xp1 = x + 1.0, c2 = fma(xp1, x, 1.0);

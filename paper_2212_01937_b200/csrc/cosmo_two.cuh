@@ -29,7 +29,7 @@ CB_HD void eval_two(const Cosmo<double>& C, double z1, double z2, bool with_grad
         st[0] |= ST_INTERNAL_REDO;
     } else if (C.cubic & 2u) {
         // two complex pairs (C.m, C.rn carry g1, h1): eqs. (3.7)-(3.9) as printed with a complex r_i, cosmo_c4.cuh
-        eval_c4(C.Or, C.m, C.rn, C.b, C.c, x1, x2, true, true, I0, TT, AA, K);
+        eval_c4(C.Or, C.m, C.rn, C.b, C.c, x1, x2, dz, true, true, I0, TT, AA, K);
         E1 = sqrt(fma(fma(C.Or, x1, C.m), x1, C.rn) * fma(x1 + C.b, x1, C.c));
         E2 = sqrt(fma(fma(C.Or, x2, C.m), x2, C.rn) * fma(x2 + C.b, x2, C.c));
         const double s12 = x1 + x2, p12 = x1 * x2, sq = fma(x2, x2, x1 * x1);

@@ -487,3 +487,29 @@ def test_band_solve_against_moments(hc):
     hc.hostcheck_band(0, C.c_double(0.05), C.c_double(0.0), C.c_double(1e-3), C.c_double(0.949), b.ctypes.data_as(DP), C.c_double(1.0), C.c_double(1.0),
                       C.c_double(0.0), C.c_double(2.0), v.ctypes.data_as(DP), C.byref(tr))
     assert np.isinf(tr.value)
+
+
+def test_two_complex_pairs_tiny_z(hc):
+    """the complex slow path (cosmo_c4.cuh) at z = 1e-8 .. 1e-3: the range has to come in as z, not as (1 + z) - 1 (which cost eps/z of
+    every integral), and the boundary term of eq. (3.9) has its factor z taken out analytically (subtracted directly it cost d_abs another
+    eps/z); found by a wide-prior comparison with the oracle"""
+    rng = np.random.default_rng(17)
+    n = 80
+    Om = rng.uniform(0.050, 0.20, n); Or = rng.uniform(0.03, 0.08, n); OL = rng.uniform(0.0, 0.3, n)
+    z = 10.0 ** rng.uniform(-8, -3, n); H0 = rng.uniform(60, 80, n)
+    assert (Om ** 2 < 4 * Or * (1 - Om - OL - Or)).all()          # no real negative root: every row takes the slow path
+    out, _, _, st = run(hc, z, Om, OL, Or, H0)
+    assert (st == 0).all()
+    val, grad, sto = oracle.observables_batch(z, Om, OL, Or, H0, with_grad=True)
+    val, grad = val.astype(np.float64), grad.astype(np.float64)
+    for i, tol in ((0, 2e-14), (1, 2e-14), (4, 2e-14), (5, 1e-12)):
+        assert (np.abs(out[i] - val[:, i]) / np.abs(val[:, i])).max() <= tol, (i, (np.abs(out[i] - val[:, i]) / np.abs(val[:, i])).max())
+    for pl in (0, 4, 5):
+        g1 = np.zeros((6, n)); g1[pl] = 1
+        _, gz, gp, st = run(hc, z, Om, OL, Or, H0, 63, g1)
+        assert (st == 0).all()
+        mine = np.vstack([gz[None], gp])
+        for p in range(5):
+            ref = grad[:, pl, p]
+            e = np.abs(mine[p] - ref) / np.maximum(np.abs(ref), 1e-3 * np.abs(val[:, pl]))
+            assert e.max() <= 1e-8, (pl, p, e.max())
