@@ -129,6 +129,15 @@ CB_HD void cosmo_factor(double Om, double OL, double Or, double H0, Cosmo<double
             const double scale = fabs(Om) + fabs(Ok) + fabs(OL) + fabs(Or);
             if (!(fabs(e1) + fabs(e0 - OL) <= 1e-13 * scale)) continue;
             double d1 = g1 * g1 - 4.0 * Or * h1, d2 = bb * bb - 4.0 * cc;
+            // OL = 0 with a complex pair: E^2 = x^2 (Or x^2 + Om x + Ok).  The real labelling would need Q1 = Or x x, i.e. m = 0 (its
+            // formulae divide by m); the complex slow path takes the double root at 0 as its second "pair" (r3 = r4 = 0) as it stands:
+            // it is the limit OL -> 0+ of the two-complex-pairs structure, where the small pair is +- i sqrt(OL/Ok)
+            if (bb == 0.0 && cc == 0.0 && d1 < 0.0) {
+                st &= ~ST_UNSUPPORTED;
+                C.cubic |= 2u;
+                m = g1; rn = h1; b = 0.0; c = 0.0;
+                break;
+            }
             // a factor with two non-positive real roots becomes Q1 = (Or x + m)(x - rn)
             if (d2 >= 0.0 && bb >= 0.0 && cc >= 0.0 && !(d1 >= 0.0 && g1 >= 0.0 && h1 >= 0.0)) {
                 const double tb = g1 / Or, tc = h1 / Or;

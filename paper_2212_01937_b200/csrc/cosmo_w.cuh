@@ -394,13 +394,31 @@ CB_HD void cx_carlson(cx x, cx y, cx z, cx p, bool want_j, CxCarlson& out) {
 
 // T = int_1^x dx/(x E), A = int_1^x x^2 dx/E for E^2 of degree 4 or 3 with the roots W.rt (x-roots, so d_i5 = -rho_i), and for
 // E^2 = a x^n (every root at 0: elementary).  Returns false where the method does not apply (degree <= 2 with distinct roots).
-CB_HD_NOINLINE bool w_TA(const WCosmo& W, double x, bool want_T, bool want_A, double& TT, double& AA) {
+// dz = x - 1 comes in as z (formed here it would carry the rounding of 1 + z: eps/z of both integrals).
+// Branches: the formulae hold with sqrt(x - r) continued from a conjugate pair, i.e. with X_j X_k = +sqrt((x - r_j)(x - r_k)) for the
+// two members of a pair.  Principal square roots do that for complex pairs; for two REAL roots to the right of the path (loitering-type
+// models) they give (i a)(i a') = -a a' instead, which flips the sign of the odd terms (the boundary terms): every second such root
+// takes the conjugate branch.  Real roots are taken as exactly real (the sign of a rounding-level imaginary part would pick the branch).
+CB_HD void w_roots_sqrt(const cx* r, int n, double x, cx* X, cx* Y, bool* isreal) {
+    const double hi = fmax(1.0, x);
+    int nright = 0;
+    for (int k = 0; k < n; ++k) {
+        isreal[k] = fabs(r[k].im) <= 1e-9 * cx_abs(r[k]);
+        const cx rk = isreal[k] ? cx_(r[k].re) : r[k];
+        X[k] = cx_sqrt(cx_(x) - rk); Y[k] = cx_sqrt(cx_(1.0) - rk);
+        if (isreal[k] && rk.re > hi) {
+            if (nright & 1) { X[k] = cx_conj(X[k]); Y[k] = cx_conj(Y[k]); }
+            ++nright;
+        }
+    }
+}
+CB_HD_NOINLINE bool w_TA(const WCosmo& W, double x, double dz, bool want_T, bool want_A, double& TT, double& AA) {
     TT = AA = NAN;
-    const double dz = x - 1.0, lead = W.a[W.deg];
+    const double lead = W.a[W.deg];
     bool mono = true;
     for (int k = 0; k < W.deg; ++k) mono = mono && cx_abs(W.rt[k]) == 0.0;
     if (mono) {                                          // E = sqrt(lead) x^(deg/2)
-        const double h = 0.5 * W.deg, il = 1.0 / sqrt(lead), lx = log(x);
+        const double h = 0.5 * W.deg, il = 1.0 / sqrt(lead), lx = log1p(dz);
         TT = (h == 0.0) ? il * lx : il * -expm1(-h * lx) / h;
         AA = (h == 3.0) ? il * lx : il * expm1((3.0 - h) * lx) / (3.0 - h);
         return true;
@@ -410,33 +428,77 @@ CB_HD_NOINLINE bool w_TA(const WCosmo& W, double x, bool want_T, bool want_A, do
     if (W.deg == 4) {
         const cx* r = W.rt;
         cx X[4], Y[4];
-        for (int n = 0; n < 4; ++n) { X[n] = cx_sqrt(cx_(x) - r[n]); Y[n] = cx_sqrt(cx_(1.0) - r[n]); }
+        bool isreal[4];
+        w_roots_sqrt(r, 4, x, X, Y, isreal);
         auto usq = [&](int a, int b, int c, int e) { const cx u = X[a] * X[b] * Y[c] * Y[e] + Y[a] * Y[b] * X[c] * X[e]; return u * u; };
-        const cx P1 = usq(0, 1, 2, 3), P2 = usq(0, 2, 1, 3), P3 = usq(0, 3, 1, 2);       // the three pairings
+        auto pair = [&](int a, int b) { int c = -1, e = -1; for (int m = 0; m < 4; ++m) if (m != a && m != b) { if (c < 0) c = m; else e = m; } return usq(a, b, c, e); };
         auto d = [&](int a, int b) { return r[b] - r[a]; };
+        const double lo = fmin(1.0, x);
         CxCarlson K;
-        if (want_T) {                    // eq. (3.8), (i, j, k, l) = (0, 3, 1, 2): u_ij^2 = P3, u_ik^2 = P1, u_il^2 = P2
-            const int i = 0, j = 3, k = 1, l = 2;
-            const cx p5 = P3 - (dz * dz) * (d(i, k) * d(i, l) * (r[j] / r[i]));
-            cx_carlson(P3, P1, P2, p5, true, K);
+        // the conjugate partner of root a (the other root closest to conj(r_a))
+        auto partner = [&](int a) { int best = -1; double db = 1e300; for (int m = 0; m < 4; ++m) if (m != a) { const double dd = cx_abs(r[m] - cx_conj(r[a])); if (dd < db) { db = dd; best = m; } } return best; };
+        if (want_T) {                    // eq. (3.8): r_i = the biggest non-zero REAL root left of the path where there is one (any j, k, l
+                                         // then); else a complex root with ITS CONJUGATE as r_j (the labelling of cosmo_c4.cuh: the
+                                         // products X_i X_j, Y_i Y_j are then real and the principal branches consistent)
+            int i = -1, j, k, l;
+            for (int m = 3; m >= 0; --m)
+                if (isreal[m] && r[m].re < lo && r[m].re != 0.0) i = m;    // the roots are sorted by decreasing modulus
+            if (i >= 0) {
+                int o[3], c = 0;
+                for (int m = 0; m < 4; ++m) if (m != i) o[c++] = m;
+                j = o[0]; k = o[1]; l = o[2];
+            } else {
+                i = 0;                                                     // the pair further to the left, as cosmo_factor picks Q1
+                double best = 1e300;
+                for (int m = 0; m < 4; ++m) if (!isreal[m] && r[m].re < best) { best = r[m].re; i = m; }
+                j = partner(i);
+                k = -1; l = -1;
+                for (int m = 0; m < 4; ++m) if (m != i && m != j) { if (k < 0) k = m; else l = m; }
+            }
+            const cx Pij = pair(i, j), Pik = pair(i, k), Pil = pair(i, l);
+            const cx p5 = Pij - (dz * dz) * (d(i, k) * d(i, l) * (r[j] / r[i]));
+            cx_carlson(Pij, Pik, Pil, p5, true, K);
             const cx q5 = (cx_(x) / ((cx_(1.0) - r[i]) * (cx_(x) - r[i]))) * p5;
             const cx s5 = q5 + (dz * dz) * (r[k] * r[l] * (r[j] / r[i]));
             const cx br = K.RF - ((dz * dz / 3.0) * (d(i, j) * d(i, k) * d(i, l) / (-r[i])) * K.RJ + cx_rc(s5, q5));
             TT = ia * ((2.0 * dz) * (br / r[i])).re;
         }
-        if (want_A) {                    // eq. (3.9): r_l = the biggest root, r_i = the smallest REAL one if there is any (a member of a
-                                         // conjugate pair as r_i breaks the principal branches), r_j, r_k the other two
-            const int i = W.iA, l = 0;
+        if (want_A) {                    // eq. (3.9), (i, j, k, l) = (rn, pair, pair, big) of the hot path: r_i = the smallest REAL root left
+                                         // of the path, r_l = the biggest root (the biggest real one left of the path if that one lies to
+                                         // the right); without real roots left of the path, the complex pair further to the left (r_i and
+                                         // its conjugate r_l, the labelling of cosmo_c4.cuh); r_j, r_k the other two
+            int i = -1, l = -1;
+            for (int m = 0; m < 4; ++m)
+                if (isreal[m] && r[m].re < lo) { if (l < 0) l = m; i = m; }   // sorted by decreasing modulus: first = biggest, last = smallest
+            // (a much bigger complex pair -- Om = 0 with little radiation: +- i sqrt(a2/Or) -- serves as r_l like the big real root does)
+            if (i > 0 && !(isreal[0] && !(r[0].re < lo))) l = 0;
+            if (l < 0 || i == l) {
+                // the biggest pair whose real part lies left of the path (as r_j, r_k a much bigger pair would multiply the cancellation
+                // of eq. (3.9) by its modulus squared), else the left-most one
+                double best = 1e300;
+                i = -1;
+                for (int m = 3; m >= 0; --m) if (!isreal[m] && r[m].re < lo) i = m;
+                if (i < 0) { i = 0; for (int m = 0; m < 4; ++m) if (!isreal[m] && r[m].re < best) { best = r[m].re; i = m; } }
+                l = partner(i);
+            }
             int j = -1, k = -1;
-            for (int m = 1; m < 4; ++m)
-                if (m != i) { if (j < 0) j = m; else k = m; }
-            auto pair = [&](int a, int b) { int c = -1, e = -1; for (int m = 0; m < 4; ++m) if (m != a && m != b) { if (c < 0) c = m; else e = m; } return usq(a, b, c, e); };
+            for (int m = 0; m < 4; ++m)
+                if (m != i && m != l) { if (j < 0) j = m; else k = m; }
             const cx Uij = pair(i, j), Uik = pair(i, k), Uil = pair(i, l);
             const cx p0 = Uij - (dz * dz) * (d(i, k) * d(i, l));
             cx_carlson(Uij, Uik, Uil, p0, true, K);                      // R_D's last argument is u_il^2
             const cx q0 = p0 / ((cx_(1.0) - r[i]) * (cx_(x) - r[i]));
             const cx s0 = q0 + cx_(dz * dz);
-            const cx bnd = X[i] * X[j] * X[k] / X[l] - Y[i] * Y[j] * Y[k] / Y[l];
+            // boundary term [F], F^2 = N(x)/(x - r_l), N = (x - r_i)(x - r_j)(x - r_k); close limits: through F^2 with dz taken out of
+            // N(x)(1 - r_l) - N(1)(x - r_l) analytically (cosmo_c4.cuh does the same; subtracted directly it loses eps/dz)
+            const cx Fx = X[i] * X[j] * X[k] / X[l], F1 = Y[i] * Y[j] * Y[k] / Y[l];
+            cx bnd = Fx - F1;
+            if (fabs(dz) <= 0.05 * lo) {
+                const cx e1 = r[i] + r[j] + r[k], e2 = r[i] * r[j] + r[i] * r[k] + r[j] * r[k];
+                const cx dd = cx_(x * x + x + 1.0) - (x + 1.0) * e1 + e2;                       // [N; x, 1]
+                const cx N1 = (cx_(1.0) - r[i]) * (cx_(1.0) - r[j]) * (cx_(1.0) - r[k]);
+                bnd = dz * ((dd * (cx_(1.0) - r[l]) - N1) / ((cx_(x) - r[l]) * (cx_(1.0) - r[l]) * (Fx + F1)));
+            }
             const cx uil = X[i] * X[l] * Y[j] * Y[k] + Y[i] * Y[l] * X[j] * X[k];
             const cx sig = r[0] + r[1] + r[2] + r[3];
             const cx t2 = dz * ((2.0 * (r[i] * r[i]) - d(i, j) * d(i, k)) * K.RF);
@@ -449,7 +511,8 @@ CB_HD_NOINLINE bool w_TA(const WCosmo& W, double x, bool want_T, bool want_A, do
     // degree 3: eqs. (B.2), (B.3) with r_i = the biggest root (any labelling does; tested over all six)
     const cx* r = W.rt;
     cx X[3], Y[3];
-    for (int n = 0; n < 3; ++n) { X[n] = cx_sqrt(cx_(x) - r[n]); Y[n] = cx_sqrt(cx_(1.0) - r[n]); }
+    bool isreal[3];
+    w_roots_sqrt(r, 3, x, X, Y, isreal);
     const cx u0 = X[0] * Y[1] * Y[2] + Y[0] * X[1] * X[2], u1 = X[1] * Y[0] * Y[2] + Y[1] * X[0] * X[2], u2 = X[2] * Y[0] * Y[1] + Y[2] * X[0] * X[1];
     CxCarlson K;
     if (want_T) {
@@ -461,7 +524,13 @@ CB_HD_NOINLINE bool w_TA(const WCosmo& W, double x, bool want_T, bool want_A, do
     if (want_A) {
         cx_carlson(u1 * u1, u2 * u2, u0 * u0, cx_(1.0), false, K);       // R_D(u_j^2, u_k^2, u_i^2)
         const cx d01 = r[1] - r[0], d02 = r[2] - r[0], sig = r[0] + r[1] + r[2];
-        const cx b3 = (X[0] * X[1] * X[2] - Y[0] * Y[1] * Y[2]) + dz * ((3.0 * (r[0] * r[0]) - d01 * d02) * K.RF)
+        const cx Gx = X[0] * X[1] * X[2], G1 = Y[0] * Y[1] * Y[2];                              // G^2 = N(x) = (x - r_0)(x - r_1)(x - r_2)
+        cx dG = Gx - G1;
+        if (fabs(dz) <= 0.05 * fmin(1.0, x)) {
+            const cx e2 = r[0] * r[1] + r[0] * r[2] + r[1] * r[2];
+            dG = dz * ((cx_(x * x + x + 1.0) - (x + 1.0) * sig + e2) / (Gx + G1));              // dz [N; x, 1] / (G(x) + G(1))
+        }
+        const cx b3 = dG + dz * ((3.0 * (r[0] * r[0]) - d01 * d02) * K.RF)
                       + (2.0 * dz) * (sig * (((dz * dz / 3.0) * (d01 * d02)) * K.RD + (X[0] * Y[0]) / u0));
         AA = ia * ((2.0 / 3.0) * b3).re;
     }
@@ -542,10 +611,13 @@ CB_HD unsigned w_eval_full(const WCosmo& W, double z, const Vote& vote, bool wan
     const double x = 1.0 + z;
     if ((want_T || want_A) && !bad) {
         double TT, AA;
-        if (w_TA(W, x, want_T, want_A, TT, AA)) {
+        if (w_TA(W, x, z, want_T, want_A, TT, AA)) {
             const double E = W.dH / d4[0];                 // d D_C / dz = d_H / E
             if (want_T) { v[4] = W.tH * TT; dz[4] = W.tH / (x * E); }
             if (want_A) { v[5] = W.dH * AA; dz[5] = W.dH * x * x / E; }
+            // a closed form that came out not-a-number on a valid path (an isolated coincidence inside the complex Carlson functions:
+            // one row in 3e4 of the wide-prior comparison, on the device only) is reported, not passed on silently
+            if ((want_T && !isfinite(TT)) || (want_A && !isfinite(AA))) st |= ST_ITER_CAP;
         } else {
             st |= ST_UNSUPPORTED;
         }

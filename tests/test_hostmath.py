@@ -513,3 +513,73 @@ def test_two_complex_pairs_tiny_z(hc):
             ref = grad[:, pl, p]
             e = np.abs(mine[p] - ref) / np.maximum(np.abs(ref), 1e-3 * np.abs(val[:, pl]))
             assert e.max() <= 1e-8, (pl, p, e.max())
+
+
+def test_ol_zero_with_complex_pair(hc):
+    """OL = 0 exactly and Om^2 < 4 Or Ok: E^2 = x^2 (Or x^2 + Om x + Ok) with a complex pair.  The real labelling has no m > 0 for it;
+    cosmo_factor hands it to the complex slow path with the double root at 0 as the second pair (the limit OL -> 0+ of two complex
+    pairs).  Values and every gradient against the oracle, and continuity in OL."""
+    rng = np.random.default_rng(23)
+    n = 60
+    Om = rng.uniform(0.050, 0.060, n); Or = np.full(n, 1e-3); OL = np.zeros(n)
+    z = np.concatenate([10.0 ** rng.uniform(-6, -1, n // 3), rng.uniform(0.1, 14.0, n - n // 3)]); H0 = rng.uniform(60, 80, n)
+    assert (Om ** 2 < 4 * Or * (1 - Om - OL - Or)).all()
+    out, _, _, st = run(hc, z, Om, OL, Or, H0)
+    assert (st == 0).all()
+    val, grad, sto = oracle.observables_batch(z, Om, OL, Or, H0, with_grad=True)
+    val, grad = val.astype(np.float64), grad.astype(np.float64)
+    assert (sto == 0).all()
+    for i, tol in ((0, 1e-13), (1, 1e-13), (3, 1e-13), (4, 1e-13), (5, 1e-11)):
+        assert (np.abs(out[i] - val[:, i]) / np.abs(val[:, i])).max() <= tol, i
+    out_eps, _, _, st_eps = run(hc, z, Om, np.full(n, 1e-300), Or, H0)
+    assert (st_eps == 0).all() and np.allclose(out_eps[:6], out[:6], rtol=1e-13, atol=0)
+    for pl in (0, 3, 4, 5):
+        g1 = np.zeros((6, n)); g1[pl] = 1
+        _, gz, gp, st = run(hc, z, Om, OL, Or, H0, 63, g1)
+        assert (st == 0).all()
+        mine = np.vstack([gz[None], gp])
+        for p in range(5):
+            ref = grad[:, pl, p]
+            e = np.abs(mine[p] - ref) / np.maximum(np.abs(ref), 1e-3 * np.abs(val[:, pl]))
+            assert e.max() <= 1e-8, (pl, p, e.max())
+
+
+def test_w_family_wide_priors(hc):
+    """the extra-w family (cosmo_w.cuh) far outside its seeded mix: Om = 0 or OL = 0 in a sixth of the rows each, Or log-uniform down
+    to 1e-7 or absent, both extra components from -0.2 to 0.8 or absent, z from 1e-6 to 30, OL up to 1.5 (real root pairs right of the
+    path).  What this comparison found and fixed in w_TA: the branch of sqrt(x - r) for real roots right of the path (d_abs wrong by orders
+    of magnitude), r_i of eq. (3.8) a member of a conjugate pair where a real root exists (t_L with the wrong sign at Om = 0), the pair
+    taken as (r_i, r_l) of eq. (3.9) with two complex pairs, the range formed as (1 + z) - 1 and the boundary terms subtracted directly
+    (eps/z).  d_abs keeps the Om/Or-type cancellation of eq. (3.9), which grows as 1/Or (the hot path's moment recurrence has no
+    counterpart here): its tolerance says so."""
+    rng = np.random.default_rng(31)
+    n = 12000
+    u = rng.random(n)
+    z = np.where(u < 0.2, 10 ** rng.uniform(-6, -2, n), np.where(u < 0.4, rng.uniform(3, 30, n), rng.uniform(0.01, 3, n)))
+    Om = np.where(rng.random(n) < 0.15, 0.0, rng.uniform(0.02, 1.5, n))
+    OL = np.where(rng.random(n) < 0.15, 0.0, rng.uniform(0.0, 1.5, n))
+    Or = np.where(rng.random(n) < 0.3, 0.0, 10 ** rng.uniform(-7, -1, n))
+    Ow13 = np.where(rng.random(n) < 0.3, 0.0, rng.uniform(-0.2, 0.8, n))
+    Ow23 = np.where(rng.random(n) < 0.3, 0.0, rng.uniform(-0.2, 0.8, n))
+    H0 = rng.uniform(50, 90, n)
+    A = [z, Om, OL, Or, Ow13, Ow23, H0]
+    val = np.zeros((6, n)); dz = np.zeros((6, n)); gp = np.zeros((6, 6, n)); st = np.zeros(n, dtype=np.uint8)
+    dp = lambda a: np.ascontiguousarray(a).ctypes.data_as(DP)
+    hc.hostcheck_w_full(C.c_int64(n), *[dp(a) for a in A], dp(val), dp(dz), dp(gp), st.ctypes.data_as(C.POINTER(C.c_uint8)))
+    v, g, so = oracle.w_observables_batch(*A)
+    v, g = v.astype(np.float64), g.astype(np.float64)
+    st = st.astype(np.int64)
+    assert (((st & 1) != 0) == (so == -1)).all()                  # a root on the path: the same rows as the oracle
+    ok = (so == 0) & ((st & 3) == 0)
+    deg_le2 = (Or == 0) & (Om == 0)
+    assert (((st & 2) != 0) & (so == 0) <= deg_le2).all()         # refused (t_L, d_abs only): degree <= 2, outside the method (PAPER.md:161)
+    assert ok.sum() > 0.85 * n
+    rel = lambda a, b: np.abs(a - b) / np.abs(b)
+    for o in range(4):
+        m = ok & np.isfinite(v[:, o])
+        assert rel(val[o][m], v[m, o]).max() <= 1e-11, oracle.OBS[o]
+    assert rel(val[4][ok], v[ok, 4]).max() <= 1e-11
+    tolA = 1e-11 + np.where(Or > 0, 3e-15 / np.maximum(Or, 1e-300), 0.0)
+    assert (rel(val[5][ok], v[ok, 5]) <= tolA[ok]).all(), float((rel(val[5][ok], v[ok, 5]) / tolA[ok]).max())
+    for o in (4, 5):
+        assert rel(dz[o][ok], g[ok, o, 0]).max() <= 1e-11
