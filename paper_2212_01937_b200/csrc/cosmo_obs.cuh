@@ -173,7 +173,7 @@ CB_HD void prep_age(Cosmo<double>& C, bool with_grad) {
     if (R.status) return;
     const double tail = (C.Or * X > C.Om) ? 0.5 / (sqrt(C.Or) * X * X) : (2.0 / 3.0) / (sqrt(C.Om) * X * sqrt(X));
     C.Tinf = R.TT + tail;
-    if (!with_grad) return;
+    if (!with_grad) { C.dTinf[0] = C.dTinf[1] = C.dTinf[2] = 0.0; return; }      // (NaN there means "basis singular" to observables_k)
     const double iE = R.iE;
     const double bt0 = -R.Em1 * iE, bt1 = (z - R.Em1) * iE, bt2 = (z * (X + 1.0) - R.Em1) * iE;
     GradSolve S;

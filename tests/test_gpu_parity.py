@@ -1006,3 +1006,30 @@ def test_extra_w_wide_priors(cb):
             eg = np.abs(gp[t] - r) / np.maximum(np.abs(r), 1e-3 * np.abs(v6[:, k]))
             tg = 1e-8 + (1e3 * tolA if nm == "DABS" else 0.0)
             assert (eg[mm] <= (tg[mm] if nm == "DABS" else tg)).all(), (nm, oracle.WRTW[1 + t], float(eg[mm].max()))
+
+
+def test_age_high_z(cb):
+    """the age plane up to z = 1100: as T_inf - T(z) it carries t(inf)/age(z) times the error of t_L (include/cosmo_b200.h); the
+    two-limit call between z and 1e10 plus the analytic remainder gives the early-universe age to full precision.  Forward-only calls
+    do not flag the age plane (the flag belongs to its gradient)."""
+    rng = np.random.default_rng(3)
+    n = 20000
+    z = 10 ** rng.uniform(-2, 3.04, n); Om = rng.uniform(0.05, 1.0, n); OL = rng.uniform(0, 1.2, n)
+    Or = rng.choice([0.0, 1e-5, 9e-5, 1e-3], n); H0 = rng.uniform(60, 80, n)
+    dv, _, so = oracle.derived_batch(z, Om, OL, Or, H0)
+    age = dv[:, 2].astype(np.float64)
+    ok = (so >= 0) & np.isfinite(age)
+    assert ok.mean() > 0.95
+    a = [dev(x) for x in (z, Om, OL, Or, H0)]
+    out, st = cb.cosmo_eval(*a, cb.ELEMENTWISE, ("TL", "AGE"))
+    out, st = out.cpu().numpy()[:, 0], st.cpu().numpy()[0]
+    assert (st[ok] == 0).all()
+    val, _, _ = oracle_batch(z, Om, OL, Or, H0, False)
+    amp = (val[:, OBS["TL"]] + age) / age                        # t(inf) / age(z)
+    assert (relerr(out[1], age)[ok] <= TOL_VAL * np.maximum(1.0, amp[ok])).all()
+    assert relerr(out[1], age)[ok & (z < 10)].max() <= TOL_VAL
+    X = 1e10
+    o2, _, _, _, st2 = cb.cosmo_eval2(a[0], dev(np.full(n, X)), *a[1:], ("TL",))
+    tail = np.where(Or * X > Om, 0.5 / (np.sqrt(np.maximum(Or, 1e-300)) * X * X), (2.0 / 3.0) / (np.sqrt(Om) * X * np.sqrt(X))) * 977.7922216807891 / H0
+    assert (st2.cpu().numpy()[ok] == 0).all()
+    assert relerr(o2.cpu().numpy()[0] + tail, age)[ok].max() <= 1e-13
