@@ -52,7 +52,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
                 sys.stderr.write(f"--- {src}\n{r.stdout}{r.stderr}")
             if r.returncode:
                 raise subprocess.CalledProcessError(r.returncode, f"nvcc {src}")
-    subprocess.run([nvcc(), "-shared", "-o", LIB] + objs, check=True, cwd=CSRC)
+    subprocess.run([nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", LIB] + objs, check=True, cwd=CSRC)
     return LIB
 
 
