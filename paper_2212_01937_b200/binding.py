@@ -399,6 +399,13 @@ def carlson_pair(x, m, s, p):
     return rf, rd, rj
 
 
+def cosmo_host_release():
+    """frees the device staging buffers cosmo_eval_host keeps between calls"""
+    f = lib().cosmo_host_release
+    f.restype = None
+    f()
+
+
 def probe_fma(dtype="f64", blocks=148 * 8, iters=4096):
     """Launch the FMA-chain roofline probe on the current stream; returns flops of the launch."""
     torch = _torch()

@@ -360,6 +360,42 @@ def test_host_call_matches_device_call(cb):
     assert np.array_equal(gp_h, gp.cpu().numpy())
 
 
+@pytest.mark.parametrize("case", ["outer-5-chunks", "elementwise-6-chunks", "elementwise-16-chunk-rule", "forward-only"])
+def test_host_call_chunking(cb, case):
+    """cosmo_eval_host cuts the redshift axis into chunks over three staging sets: results are those of the one-shot device call (to
+    rounding: chunk boundaries change the warps and the partial sums), for ragged odd lengths, per-element parameters and the rule that
+    caps a job at 16 chunks"""
+    rng = np.random.default_rng(8)
+    if case == "outer-5-chunks":
+        w = W.config3(n=300_001, S=64)
+        out_h, gz_h, gp_h, st_h = cb.cosmo_eval_host(w.z, w.Om, w.OL, w.Or, w.H0, cb.OUTER, w.which, grad_out=w.grad_out)
+        gz, gp, out, st = cb.cosmo_vjp(dev(w.z), dev(w.Om), dev(w.OL), dev(w.Or), dev(w.H0), dev(w.grad_out), cb.OUTER, w.which, want_out=True)
+        assert np.array_equal(out_h, out.cpu().numpy()) and np.array_equal(st_h, st.cpu().numpy())
+        # grad_z is a sum over the 64 cosmologies inside each tile: chunk boundaries move the tiles, not the terms
+        assert np.allclose(gz_h, gz.cpu().numpy(), rtol=1e-12, atol=0)
+        assert np.allclose(gp_h, gp.cpu().numpy(), rtol=1e-10, atol=0)
+        return
+    n = {"elementwise-6-chunks": 1_000_003, "elementwise-16-chunk-rule": 4_000_001, "forward-only": 2_000_001}[case]
+    z = rng.uniform(0.01, 3.0, n); Om = rng.uniform(0.1, 0.5, n); OL = rng.uniform(0.3, 0.9, n); Or = rng.choice([0.0, 9e-5, 1e-3], n)
+    H0 = rng.uniform(60, 80, n)
+    which = ("DC", "DM", "DL", "MU", "TL", "DABS")
+    a = [dev(x) for x in (z, Om, OL, Or, H0)]
+    if case == "forward-only":
+        out_h, _, _, st_h = cb.cosmo_eval_host(z, Om, OL, Or, H0, cb.ELEMENTWISE, ("DC", "TL"))
+        out, st = cb.cosmo_eval(*a, cb.ELEMENTWISE, ("DC", "TL"))
+        assert np.allclose(out_h, out.cpu().numpy(), rtol=1e-12, atol=0, equal_nan=True) and np.array_equal(st_h, st.cpu().numpy())
+        return
+    g = rng.standard_normal((6, 1, n))
+    out_h, gz_h, gp_h, st_h = cb.cosmo_eval_host(z, Om, OL, Or, H0, cb.ELEMENTWISE, which, grad_out=g)
+    gz, gp, out, st = cb.cosmo_vjp(*a, dev(g), cb.ELEMENTWISE, which, want_out=True)
+    # (not bit for bit: the duplication loop runs until every lane of a warp has converged, and a chunk boundary changes which
+    # elements share a warp -- a lane that iterates once more than it needs moves its result by a rounding error)
+    close = lambda u, v: np.allclose(u, v, rtol=1e-12, atol=0, equal_nan=True)
+    assert close(out_h, out.cpu().numpy()) and np.array_equal(st_h, st.cpu().numpy())
+    assert close(gz_h, gz.cpu().numpy()) and np.allclose(gp_h, gp.cpu().numpy(), rtol=1e-9, atol=1e-9 * np.abs(gp_h).max(), equal_nan=True)
+    cb.cosmo_host_release()
+
+
 # ---------------------------------------------------------------- FP32 variant
 def test_fp32_variant(cb):
     import torch
