@@ -397,8 +397,9 @@ CB_HD T carlson_Qj(T xa, T mp, T hs, T p) {
 // sig_j ~ Or / (Om - Ok sig_{j-1}), which settles at the small root of Ok sig^2 - Om sig + Or = 0 when Om^2 > 4 Or Ok (always
 // for Ok <= 0) and wanders, with pivots of either sign, when E^2 has no real negative root; `trunc` is infinite unless
 // Om^2 >= 8 Or Ok, and the caller falls back to the closed form.
-template <typename T, int NR, int SO, int AO, int CO, int J0>
-CB_HD void band_solve(T Om, T OL, T Or, T Ok, const T (&b)[NR], T km1, T km2, T km3, T x, T (&v)[NR], T& trunc) {
+// kB (extra-w family, cosmo_w.cuh): a further term B (j + 1/2) v_{j-2} in every row (the x^1 coefficient of E^2).
+template <typename T, int NR, int SO, int AO, int CO, int J0, bool kB = false>
+CB_HD void band_solve(T Om, T OL, T Or, T Ok, const T (&b)[NR], T km1, T km2, T km3, T x, T (&v)[NR], T& trunc, T Bc = T(0)) {
     using N = Num<T>;
     T sig[NR], gam[NR];
     T P = T(1);
@@ -406,14 +407,20 @@ CB_HD void band_solve(T Om, T OL, T Or, T Ok, const T (&b)[NR], T km1, T km2, T 
     for (int j = 0; j < NR; ++j) {
         const T dj = T(j + 1.5) * Om, sj = T(j + SO) * Or, aj = T(j + AO) * Ok;
         T f = aj, num = b[j], den = dj;
+        T bq = kB ? T(j + 0.5) * Bc : T(0);                  // coefficient of v_{j-2}: B's own term plus the fill of the v_{j-3} term
+        bool hasq = kB;
         if (j + CO != 0) {
             const T cj = T(j + CO) * OL;
             if (j >= 3) {
                 const T e1 = cj * sig[j - 3];
-                f = N::fma_(e1, sig[j - 2], aj);
-                num = N::fma_(e1, gam[j - 2], num);
+                bq = kB ? bq - e1 : -e1;
+                hasq = true;
             }
             num = N::fma_(-cj, j >= 3 ? gam[j >= 3 ? j - 3 : 0] : (j == 2 ? km1 : (j == 1 ? km2 : km3)), num);
+        }
+        if (hasq) {
+            if (j >= 2) { f = N::fma_(-bq, sig[j - 2], aj); num = N::fma_(-bq, gam[j - 2], num); }
+            else num = N::fma_(-bq, j == 1 ? km1 : km2, num);
         }
         num = N::fma_(-f, j >= 1 ? gam[j >= 1 ? j - 1 : 0] : km1, num);
         if (j >= 1) den = N::fma_(-f, sig[j - 1], den);

@@ -503,8 +503,29 @@ CB_HD_NOINLINE bool w_TA(const WCosmo& W, double x, double dz, bool want_T, bool
             const cx sig = r[0] + r[1] + r[2] + r[3];
             const cx t2 = dz * ((2.0 * (r[i] * r[i]) - d(i, j) * d(i, k)) * K.RF);
             const cx t3 = dz * ((d(j, l) * d(k, l)) * (((dz * dz / 3.0) * (d(i, j) * d(i, k))) * K.RD + (X[i] * Y[i]) / (X[l] * Y[l] * uil)));
-            const cx t4 = dz * (sig * (cx_rc(s0, q0) - ((dz * dz / 3.0) * (d(i, j) * d(i, k) * d(i, l))) * K.RJ));
+            const cx B0 = cx_rc(s0, q0) - ((dz * dz / 3.0) * (d(i, j) * d(i, k) * d(i, l))) * K.RJ;     // = int (x - r_i) dx / (2 dz sqrt(lead) E)
+            const cx t4 = dz * (sig * B0);
             AA = ia * (bnd + t2 + t3 + t4).re;
+            // The groups of eq. (3.9) cancel by ~ a3/(a4 x).  Where radiation is a perturbation of a model with matter the
+            // same Carlson values are assembled through the moment recurrence of the hot path (cosmo_eval.cuh, band_solve; DESIGN.md
+            // "d_abs") with the x^1 term of this family: u_0 = I0, u_1 = 2 dz B0 / sqrt(lead) + r_i I0, d_abs integral = u_2.
+            if (W.a[3] > 0.0) {
+                constexpr int KS = REC_KS;
+                double bk[KS + 1], u2[KS + 1], trunc, e2m1 = 0.0;
+                {
+                    double dk = 0.0;                               // x^j - 1 = x (x^(j-1) - 1) + dz
+                    for (int m = 0; m <= 4; ++m) { e2m1 = fma(W.a[m], dk, e2m1); dk = fma(x, dk, dz); }       // E^2 - 1 (the coefficients sum to 1)
+                }
+                const double Ex = sqrt(1.0 + e2m1), Em1 = e2m1 / (Ex + 1.0);
+                {
+                    double dk = 0.0;
+                    for (int m = 0; m <= KS; ++m) { bk[m] = fma(dk, Ex, Em1); dk = fma(x, dk, dz); }          // x^m E(x) - E(1)
+                }
+                const double I0 = ia * 2.0 * dz * K.RF.re;
+                const double u1 = (ia * (2.0 * dz) * B0 + I0 * r[i]).re;
+                band_solve<double, KS + 1, 2, 1, 0, 0, true>(W.a[3], W.a[0], W.a[4], W.a[2], bk, u1, I0, 0.0, x, u2, trunc, W.a[1]);
+                if (trunc <= 1e-15 * fabs(u2[0])) AA = u2[0];
+            }
         }
         return true;
     }
