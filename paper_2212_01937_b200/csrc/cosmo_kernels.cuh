@@ -456,7 +456,13 @@ __global__ void __launch_bounds__(CB_ELEM_BLOCK, kG ? CB_ELEM_MINB_G : CB_ELEM_M
 // second pass: the listed elements again with every slow path available (elem_one without kDefer).  Dense: consecutive threads take
 // consecutive list entries, whatever their position in the batch.
 template <typename T, bool kT, bool kA, bool kG>      // (kG = true: only the VJP has a second pass)
-__global__ void __launch_bounds__(ELEM_THREADS, 4) k_elem_redo(ElemArgs a) {
+#ifndef CB_REDO_MINB
+#define CB_REDO_MINB 2      // 254 registers, no spills (at 4 blocks: 128 registers, 800 B of spills per thread; measured 2.177 -> 2.135 ms on config 5)
+#endif
+#ifndef CB_REDO_GRID
+#define CB_REDO_GRID 8      // blocks per SM of the persistent grid (finer tail)
+#endif
+__global__ void __launch_bounds__(ELEM_THREADS, CB_REDO_MINB) k_elem_redo(ElemArgs a) {
     const int64_t N = a.N;
     const unsigned which = a.which;
     const unsigned count = *a.redo_count;
@@ -474,7 +480,7 @@ __global__ void __launch_bounds__(ELEM_THREADS, 4) k_elem_redo(ElemArgs a) {
             }
         }
         T dz = T(0), gp[4] = {T(0), T(0), T(0), T(0)};
-        const unsigned st = elem_one<T, kT, kA, kG, VoteNone, false>(static_cast<const T*>(a.z)[i], a.Om[i], a.OL[i], a.Or[i], a.H0[i], which,
+        const unsigned st = elem_one<T, kT, kA, kG, VoteNone, false, true, sizeof(T) == 8>(static_cast<const T*>(a.z)[i], a.Om[i], a.OL[i], a.Or[i], a.H0[i], which,
                                                                      VoteNone(), g, v, dz, gp);
         if (a.out != nullptr) {
             T* __restrict__ out = static_cast<T*>(a.out);

@@ -564,13 +564,26 @@ CB_HD void fetch_grads(const T* g, T (&go)[N_PLANES]) {
 }
 template <typename T, typename IO>
 CB_HD void fetch_grads(const IO& io, T (&go)[N_PLANES]) { io.get_grads(go); }
-template <typename T, bool kT, bool kA, bool kSolve = false, bool kDefer = false, typename G = const T*>
+// kQuadOnly (second pass of the FP64 ELEMENTWISE kernel): an element with the real root structure is on the work list because its bases
+// are singular or cancel beyond the limit -- the main pass has established that -- so the bases are not formed again and the
+// quadrature is taken straight away (a third of the second pass's instructions).
+template <typename T, bool kT, bool kA, bool kSolve = false, bool kDefer = false, typename G = const T*, bool kQuadOnly = false>
 CB_HD unsigned backward_robust(const Cosmo<T>& C, T z, const Core<T>& R, const Obs<T>& O, const G& gsrc, T& gz, T gp[4],
                                unsigned which = W_ALL) {
     GradInt<T> D;
     T cond = T(0);
     const T limit = T(sizeof(T) == 8 ? GRAD_COND_LIMIT : GRAD_COND_LIMIT_F32);
     bool singular = (C.cubic & 4u) != 0;
+    if (kQuadOnly && !(C.cubic & 2u)) {
+        for (int t = 0; t < 3; ++t) { D.dI[t] = D.dT[t] = D.dA[t] = T(0); }
+        unsigned st = 0u;
+        if (!(R.status & (ST_ROOT_ON_PATH | ST_UNSUPPORTED)))
+            st = grad_robust_fix<T>(C, z, kT && (which & (W_TL | W_AGE)), kA && (which & W_DABS), T(INFINITY), D);
+        T g[N_PLANES];
+        fetch_grads<T>(gsrc, g);
+        backward_chain<T, kT, kA>(C, z, R, O, D, g, gz, gp, which);
+        return st;
+    }
     if (kSolve) {
         Cosmo<double> Cd;
         Cd.Om = (double)C.Om; Cd.OL = (double)C.OL; Cd.Or = (double)C.Or; Cd.Ok = (double)C.Ok;
@@ -621,7 +634,7 @@ struct ArrayIO {
         for (int w = 0; w < N_PLANES; ++w) go[w] = g[w];
     }
 };
-template <typename T, bool kT, bool kA, bool kG, typename Vote, bool kDefer = false, bool kAge = true, typename IO = ArrayIO<T>>
+template <typename T, bool kT, bool kA, bool kG, typename Vote, bool kDefer = false, bool kAge = true, typename IO = ArrayIO<T>, bool kRedo = false>
 CB_HD unsigned elem_one_io(T zv, double Om, double OL, double Or, double H0, unsigned which, const Vote& vote, const IO& io, T& dz, T gp[4]) {
     Cosmo<T> C0{}, C{};
     {
@@ -677,15 +690,15 @@ CB_HD unsigned elem_one_io(T zv, double Om, double OL, double Or, double H0, uns
                 backward_chain<T, kT, kA>(C, zv, R, O, D, g, dz, gp, which);
             }
         } else {
-            st |= backward_robust<T, kT, kA, true, kDefer, IO>(C, zv, R, O, io, dz, gp, which);
+            st |= backward_robust<T, kT, kA, true, kDefer, IO, kRedo>(C, zv, R, O, io, dz, gp, which);
         }
     }
     return st;
 }
-template <typename T, bool kT, bool kA, bool kG, typename Vote, bool kDefer = false, bool kAge = true>
+template <typename T, bool kT, bool kA, bool kG, typename Vote, bool kDefer = false, bool kAge = true, bool kRedo = false>
 CB_HD unsigned elem_one(T zv, double Om, double OL, double Or, double H0, unsigned which, const Vote& vote, const T* g, T* v, T& dz, T gp[4]) {
     const ArrayIO<T> io{g, v};
-    return elem_one_io<T, kT, kA, kG, Vote, kDefer, kAge>(zv, Om, OL, Or, H0, which, vote, io, dz, gp);
+    return elem_one_io<T, kT, kA, kG, Vote, kDefer, kAge, ArrayIO<T>, kRedo>(zv, Om, OL, Or, H0, which, vote, io, dz, gp);
 }
 
 }  // namespace cb

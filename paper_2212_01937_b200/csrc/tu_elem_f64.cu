@@ -7,7 +7,7 @@ template <bool kG>
 static void elem_dispatch_f64(const ElemArgs& a, cudaStream_t st) {
     using T = double;
     const bool kT = a.which & (W_TL | W_AGE), kA = a.which & W_DABS;
-    const dim3 grid((unsigned)cdiv64(a.N, CB_ELEM_BLOCK)), redo(148 * 4);      // second pass: persistent over a list whose length only the device knows
+    const dim3 grid((unsigned)cdiv64(a.N, CB_ELEM_BLOCK)), redo(148 * CB_REDO_GRID);      // second pass: persistent over a list whose length only the device knows
     if (kG) cudaMemsetAsync(a.redo_count, 0, sizeof(unsigned), st);
     const bool age = (a.which & W_AGE) != 0;
     if (kT && kA && age) { k_elem<T, true, true, kG, true><<<grid, CB_ELEM_BLOCK, 0, st>>>(a); if (kG) k_elem_redo<T, true, true, true><<<redo, ELEM_THREADS, 0, st>>>(a); }
