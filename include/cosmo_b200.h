@@ -32,7 +32,8 @@
  *       2  unsupported input: Om <= 0, Or < 0, OL < 0, H0 <= 0, z <= -1, non-finite, or a root structure that could not be
  *          factorised (the method needs E^2 of degree 3 or 4)
  *       4  D_L <= 0 (closed universe at/after the antipode): mu is NaN, the other outputs are valid
- *       8  the duplication loop hit its iteration cap before Carlson's stopping rule was met
+ *       8  the duplication loop hit its iteration cap before Carlson's stopping rule was met; from cosmo_eval_w also: t_L or d_abs
+ *          came out not-a-number on a valid path (an isolated coincidence inside the complex Carlson functions: reported, not silent)
  *      16  a parameter gradient of this element is not served to the documented accuracy (set by the VJP calls; values valid).
  *          Where roots of E^2 (nearly) coincide the closed-form gradient bases cancel -- the 1/prod(r_j - r_k) of PAPER.md:320-345 --
  *          and the element's gradient integrals are taken from Gauss-Legendre quadrature of their definition instead (also at
