@@ -156,7 +156,10 @@ __host__ __device__ constexpr bool outer_sequential(bool kT, bool kA, int mode) 
 template <typename T, bool kT, bool kA, int MODE, unsigned WCT>
 // (forward-only chi-family kernels need 128 registers as they stand: the fourth block per SM is asked for so that a few registers more
 // after an unrelated change cannot silently cost a quarter of the occupancy -- 0.581 -> 0.609 ms on config 3 forward when that happened)
-__global__ void __launch_bounds__(OUTER_THREADS, outer_sequential(kT, kA, MODE) ? 2 : ((MODE == MODE_FWD && !kT && !kA) ? 4 : CB_MINBLOCKS)) k_outer(OuterArgs a) {
+#ifndef CB_SEQ_MINB
+#define CB_SEQ_MINB 2
+#endif
+__global__ void __launch_bounds__(OUTER_THREADS, outer_sequential(kT, kA, MODE) ? CB_SEQ_MINB : ((MODE == MODE_FWD && !kT && !kA) ? 4 : CB_MINBLOCKS)) k_outer(OuterArgs a) {
     constexpr int KZ = outer_kz(kT, kA), TILE = outer_tile(kT, kA);
     const unsigned which = WCT ? WCT : a.which;      // WCT != 0: output set known at compile time (drops dead planes)
     constexpr bool kG = MODE != MODE_FWD;
