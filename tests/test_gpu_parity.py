@@ -1069,3 +1069,47 @@ def test_age_high_z(cb):
     tail = np.where(Or * X > Om, 0.5 / (np.sqrt(np.maximum(Or, 1e-300)) * X * X), (2.0 / 3.0) / (np.sqrt(Om) * X * np.sqrt(X))) * 977.7922216807891 / H0
     assert (st2.cpu().numpy()[ok] == 0).all()
     assert relerr(o2.cpu().numpy()[0] + tail, age)[ok].max() <= 1e-13
+
+
+def test_two_limit_wide_priors(cb):
+    """cosmo_eval2 on the wide priors of test_wide_priors_all_planes_and_gradients: limits from 0 to 5 with ranges from 1e-7 to 16,
+    a fifth of the pairs reversed (z2 < z1), z1 = 0 in a third; all five planes and all six derivative columns of each plane"""
+    n = 30_000
+    rng = np.random.default_rng(1)
+    reg = rng.integers(0, 5, n)
+    Om = np.where(reg == 0, rng.uniform(0.02, 2.0, n), np.where(reg == 1, 10 ** rng.uniform(-1.7, 0.3, n), rng.uniform(0.05, 1.0, n)))
+    OL = np.where(reg == 2, rng.uniform(0.0, 2.0, n), np.where(reg == 3, 0.0, rng.uniform(0.0, 1.2, n)))
+    Or = np.where(reg == 4, 10 ** rng.uniform(-8, -0.5, n), np.where(reg == 3, rng.choice([0.0, 1e-5, 1e-3], n), 10 ** rng.uniform(-6, -3, n)))
+    H0 = rng.uniform(50, 90, n)
+    z1 = np.where(rng.random(n) < 0.3, 0.0, rng.uniform(0, 5, n))
+    dz = np.where(rng.random(n) < 0.3, 10 ** rng.uniform(-7, -2, n), 10 ** rng.uniform(-2, 1.2, n))
+    z2 = z1 + dz
+    sw = rng.random(n) < 0.2
+    z1, z2 = np.where(sw, z2, z1), np.where(sw, z1, z2)
+    which = ("DC", "DM", "TL", "DABS", "DA")
+    v, gr, so = oracle.observables2_batch(z1, z2, Om, OL, Or, H0)
+    v, gr = v.astype(np.float64), gr.astype(np.float64)
+    order = [oracle.OBS2.index(w) for w in which]
+    a = [dev(x) for x in (z1, z2, Om, OL, Or, H0)]
+    ok = (so == 0) & np.isfinite(v).all(axis=1)
+    assert ok.mean() > 0.95
+    for k, nm in enumerate(which):
+        g = np.zeros((5, n)); g[k] = 1.0
+        out, g1, g2, gp, st = cb.cosmo_eval2(*a, which, grad_out=dev(g))
+        out, st = out.cpu().numpy(), st.cpu().numpy()
+        mine = np.vstack([g1.cpu().numpy()[None], g2.cpu().numpy()[None], gp.cpu().numpy()])
+        if k == 0:
+            assert (st[ok] == 0).all() and (st[so != 0] != 0).all()
+            tiny_om = Om < 0.02                    # d_abs there: DESIGN.md section 6 (the moment recurrence divides by Om)
+            for kk, o in enumerate(order):
+                m = ok & ~(tiny_om & (which[kk] == "DABS"))
+                assert relerr(out[kk], v[:, o])[m].max() <= TOL_VAL, which[kk]
+        o = order[k]
+        m = ok & ~(tiny_om & (nm == "DABS"))
+        for c in range(6):
+            r = gr[:, o, c]
+            # the limits' derivatives are the integrand at the limit: for a tiny range they dwarf the value, which is then no floor
+            floor = 1e-3 * np.abs(v[:, o]) / np.maximum(np.abs(z2 - z1), 1e-300) if c < 2 else 1e-3 * np.abs(v[:, o])
+            eg = np.abs(mine[c] - r) / np.maximum(np.abs(r), floor)
+            mm = m & np.isfinite(r)
+            assert eg[mm].max() <= TOL_GRAD, (nm, c, float(eg[mm].max()))
