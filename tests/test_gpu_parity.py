@@ -1113,3 +1113,51 @@ def test_two_limit_wide_priors(cb):
             eg = np.abs(mine[c] - r) / np.maximum(np.abs(r), floor)
             mm = m & np.isfinite(r)
             assert eg[mm].max() <= TOL_GRAD, (nm, c, float(eg[mm].max()))
+
+
+def test_outer_wide_priors(cb):
+    """OUTER calls with 400 cosmologies from the wide priors (every root structure the slow rows of k_outer serve: complex pairs,
+    OL = 0, loitering-type pairs right of the path) x 120 redshifts from 1e-6 to 30: values of all six planes per element, the parameter
+    gradients per cosmology and grad_z per redshift for one-hot upstreams on D_C and d_abs"""
+    N, S = 120, 400
+    rng = np.random.default_rng(4)
+    reg = rng.integers(0, 5, S)
+    Om = np.where(reg == 0, rng.uniform(0.02, 2.0, S), np.where(reg == 1, 10 ** rng.uniform(-1.7, 0.3, S), rng.uniform(0.05, 1.0, S)))
+    OL = np.where(reg == 2, rng.uniform(0.0, 2.0, S), np.where(reg == 3, 0.0, rng.uniform(0.0, 1.2, S)))
+    Or = np.where(reg == 4, 10 ** rng.uniform(-8, -0.5, S), np.where(reg == 3, rng.choice([0.0, 1e-5, 1e-3], S), 10 ** rng.uniform(-6, -3, S)))
+    H0 = rng.uniform(50, 90, S)
+    u = rng.random(N)
+    z = np.sort(np.where(u < 0.2, 10 ** rng.uniform(-6, -1, N), np.where(u < 0.4, rng.uniform(3, 30, N), rng.uniform(0.01, 3, N))))
+    which = ("DC", "DM", "DL", "MU", "TL", "DABS")
+    rep = lambda x: np.repeat(x, N)
+    zz = np.tile(z, S)
+    val, grad, sto = oracle_batch(zz, rep(Om), rep(OL), rep(Or), rep(H0), True)
+    val = val.reshape(S, N, -1); grad = grad.reshape(S, N, val.shape[2], 5); sto = sto.reshape(S, N)
+    a = [dev(x) for x in (z, Om, OL, Or, H0)]
+    for nm in ("DC", "DABS"):
+        k = which.index(nm)
+        g = np.zeros((6, S, N)); g[k] = 1.0
+        gz, gp, out, st = cb.cosmo_vjp(*a, dev(g), cb.OUTER, which, want_out=True)
+        out, st, gz, gp = out.cpu().numpy(), st.cpu().numpy().astype(np.int64), gz.cpu().numpy(), gp.cpu().numpy()
+        valid = (sto >= 0) & np.isfinite(val[:, :, 0])
+        assert (((st & 3) != 0) == ~valid).all()
+        ok = valid & ((st & ~np.int64(4)) == 0)
+        assert ok.sum() > 0.98 * valid.sum()
+        I0 = np.where(ok, val[:, :, 0] / (299792.458 / H0[:, None]), 1.0)
+        tau, amp = TT.row_conditioning(zz, rep(Om), rep(OL), rep(Or), rep(H0), I0.ravel(), TOL_VAL)
+        if nm == "DC":
+            for kk, name in enumerate(which):
+                ref = val[:, :, OBS[name]]
+                tol = TT.value_tolerance(name, tau, amp, val[:, :, OBS["MU"]].ravel()).reshape(S, N)
+                m = ok & np.isfinite(ref)
+                assert (relerr(out[kk], ref)[m] <= tol[m]).all(), name
+        gref = grad[:, :, OBS[nm], :]
+        full = ok.all(axis=1) & np.isfinite(gref).all(axis=(1, 2))
+        assert full.sum() > 0.8 * S
+        infl = (tau / TOL_VAL).reshape(S, N).max(axis=1)            # loitering rows loosen their cosmology's sums by the same factor
+        for p in range(4):
+            rs, ra = gref[:, :, 1 + p].sum(axis=1), np.abs(gref[:, :, 1 + p]).sum(axis=1)
+            assert (np.abs(gp[p] - rs)[full] <= TOL_GRAD * infl[full] * ra[full]).all(), (nm, p)
+        col = ok.all(axis=0)
+        rs, ra = gref[:, :, 0].sum(axis=0), np.abs(gref[:, :, 0]).sum(axis=0)
+        assert (np.abs(gz - rs)[col] <= TOL_GRAD * (tau / TOL_VAL).reshape(S, N).max(axis=0)[col] * ra[col]).all(), nm
