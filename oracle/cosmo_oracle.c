@@ -175,7 +175,7 @@ static void gk21_adapt(const cosmo_t *c, ld a, ld b, ld frac, const ld scale[NV]
 }
 
 /* out[0..2] = I0,T,A ; if with_grad out[3..11] = their d/d(Om,OL,Or).  Returns panels used,
- * or -1 if E^2 <= 0 somewhere on the sampled path (unphysical, no Big Bang). */
+ * or -1 if E^2 <= 0 somewhere on the path -- found by a scan of 65 points or by the quadrature itself (unphysical, no Big Bang). */
 int oracle_integrals(ld z, ld Om, ld OL, ld Or, int with_grad, ld out[NV]) {
     cosmo_t c = { Om, OL, Or, 1.0L - Om - OL - Or, with_grad ? NV : 3 };
     for (int v = 0; v < NV; ++v) out[v] = 0.0L;
@@ -200,6 +200,9 @@ int oracle_integrals(ld z, ld Om, ld OL, ld Or, int with_grad, ld out[NV]) {
         gk21_adapt(&c, a, b, 1.0L / nseg, scale, 0, out, &npanels);
     }
     if (npanels >= GK_MAXPANELS) return -2;
+    /* a stretch with E^2 <= 0 that is narrower than the scan's step (two real roots close to each other on the path) is met by the
+     * quadrature instead: sqrt of a negative number.  Same verdict as the scan's. */
+    if (out[0] != out[0] || out[1] != out[1] || out[2] != out[2]) return -1;
     return npanels;
 }
 
